@@ -1,0 +1,277 @@
+"""Pins P3-P6, P10-P12 for the oracle's solver.
+
+Each test fixes the oracle against something other than itself: a dense linear solve, a
+textbook linear system, the MM descent property, first-order optimality evaluated directly
+from K (never through U), closed-form limits, or an independent Newton solve.
+"""
+import numpy as np
+import pytest
+
+import oracle as o
+import workloads as wl
+from oracle import LOSS_HINGE, LOSS_LOGISTIC, LOSS_QUANTILE
+
+
+def _problem(loss, n=50, p=4, seed=5):
+    rng = np.random.default_rng(seed)
+    if loss == LOSS_QUANTILE:
+        X = rng.uniform(-1, 1, (n, p))
+        y = np.sin(np.pi * X.sum(1) / np.sqrt(p)) + 0.3 * rng.standard_t(3, n)
+    else:
+        w = wl.config0(n=n, p=p, seed=seed)
+        X, y = w.X, w.y
+    sigma = wl.median_distance(X)
+    K = o.gram_rbf(X, sigma)
+    return X, y, K, o.spectral_setup(K), o.make_folds(n, 4, 3)
+
+
+# ---------------------------------------------------------------- losses
+def test_smoothed_hinge_matches_printed_formula():
+    d = 0.25
+    u = np.array([-2.0, 0.75, 0.9, 1.0, 1.2, 1.25, 3.0])
+    want = np.array([3.0, 0.25, (0.9 - 1.25) ** 2, (1.0 - 1.25) ** 2, (1.2 - 1.25) ** 2, 0.0, 0.0])
+    want[2:5] /= 4 * d
+    got = o.smooth_loss(LOSS_HINGE, np.ones_like(u), u, d)
+    assert np.allclose(got, want, atol=1e-15)
+    # delta -> 0 recovers the hinge of eq. (1); L_delta - hinge in [0, delta/4]
+    gap = got - np.maximum(1 - u, 0)
+    assert np.all(gap >= -1e-15) and np.all(gap <= d / 4 + 1e-15)
+
+
+@pytest.mark.parametrize("loss,smooth,tau", [(LOSS_HINGE, 0.3, None), (LOSS_LOGISTIC, None, None),
+                                             (LOSS_QUANTILE, 0.2, 0.1), (LOSS_QUANTILE, 0.2, 0.9)])
+def test_psi_is_derivative_and_curvature_bounds_it(loss, smooth, tau):
+    rng = np.random.default_rng(1)
+    y = np.where(rng.random(400) < 0.5, 1.0, -1.0) if loss != LOSS_QUANTILE else rng.standard_normal(400)
+    f = 2.5 * rng.standard_normal(400)
+    h = 1e-6
+    num = (o.smooth_loss(loss, y, f + h, smooth, tau) - o.smooth_loss(loss, y, f - h, smooth, tau)) / (2 * h)
+    assert np.max(np.abs(num - o.psi(loss, y, f, smooth, tau))) < 1e-5 / (smooth or 1.0)
+    # second difference of the loss never exceeds the curvature constant (majoriser validity)
+    f2 = np.linspace(-4, 4, 4001)
+    yy = np.ones_like(f2) if loss != LOSS_QUANTILE else np.zeros_like(f2)
+    p = o.psi(loss, yy, f2, smooth, tau)
+    assert np.max(np.diff(p) / np.diff(f2)) <= o.curvature(loss, smooth) * (1 + 1e-9)
+    assert np.min(np.diff(p)) >= -1e-15                                  # convex
+
+
+def test_quantile_nominal_is_check_loss():
+    t = np.array([-2.0, -0.5, 0.0, 0.5, 2.0])
+    assert np.allclose(o.nominal_loss(LOSS_QUANTILE, t, 0 * t, 0.1), [1.8, 0.45, 0.0, 0.05, 0.2])
+    # smoothed check loss is C^1 at +-gamma and within gamma/4 of the check loss
+    g, tau = 0.3, 0.7
+    tt = np.linspace(-1, 1, 2001)
+    gap = o.smooth_loss(LOSS_QUANTILE, tt, 0 * tt, g, tau) - o.nominal_loss(LOSS_QUANTILE, tt, 0 * tt, tau)
+    assert gap.min() >= -1e-15 and gap.max() <= g / 4 + 1e-15
+
+
+# ---------------------------------------------------------------- P3: spectral step == dense solve
+@pytest.mark.parametrize("loss,smooth,tau", [(LOSS_HINGE, 0.125, None), (LOSS_LOGISTIC, None, None),
+                                             (LOSS_QUANTILE, 0.125, 0.3)])
+def test_spectral_step_equals_dense_majoriser_solve(loss, smooth, tau):
+    X, y, K, spec, foldid = _problem(loss, n=40)
+    n = len(y)
+    rng = np.random.default_rng(2)
+    lam = 3e-3
+    mask = (foldid != 1).astype(float)
+    n_c = mask.sum()
+    alpha_bar = 0.1 * rng.standard_normal(n)
+    bbar = 0.2
+    a_bar = spec.U.T @ alpha_bar
+    c, S, s = o.column_constants(spec, lam, n_c, o.curvature(loss, smooth))
+    # oracle step (as in fit_column)
+    f = spec.U @ (spec.lam * a_bar) + bbar
+    z = mask * o.psi(loss, y, f, smooth, tau) / n_c
+    rho = spec.U.T @ z + 2 * lam * a_bar
+    dbeta = (z.sum() - c * np.sum(S * spec.lam * spec.u1 * rho)) / s
+    da = S * (rho - dbeta * c * spec.u1)
+    # dense: P (dbeta; dalpha) = (1^T z ; K z + 2 lam K alpha)   (G1/G2)
+    P = o.dense_majoriser(K, lam, c)
+    fd = K @ alpha_bar + bbar
+    zd = mask * o.psi(loss, y, fd, smooth, tau) / n_c
+    rhs = np.concatenate([[zd.sum()], K @ zd + 2 * lam * K @ alpha_bar])
+    got = np.concatenate([[dbeta], spec.U @ da])
+    assert np.max(np.abs(P @ got - rhs)) < 1e-11 * max(1.0, np.abs(rhs).max())
+    # and the paper's g as printed (no minus sign) does NOT satisfy it: G1
+    g_printed = 1.0 / (n * np.sum(spec.u1 ** 2 * spec.lam ** 2 / (2 * lam * spec.lam + c * spec.lam ** 2 + 1e-300)))
+    assert abs(g_printed - 1.0 / s) > 1e-3 * abs(1.0 / s)
+
+
+# ---------------------------------------------------------------- P4: one step == LS-SVM system
+def test_huge_delta_one_step_is_lssvm():
+    X, y, K, spec, _ = _problem(LOSS_HINGE, n=45)
+    n = len(y)
+    lam, delta = 2e-2, 100.0
+    a, b0, it, kkt, flag = o.fit_column(spec, y, LOSS_HINGE, [delta], lam, np.ones(n), maxit=1, momentum=False)
+    A = np.zeros((n + 1, n + 1))
+    A[0, 1:] = 1.0
+    A[1:, 0] = 1.0
+    A[1:, 1:] = K + 4 * delta * n * lam * np.eye(n)
+    sol = np.linalg.solve(A, np.concatenate([[0.0], (1 + delta) * y]))
+    assert abs(b0 - sol[0]) < 1e-9 * max(1, abs(sol[0]))
+    assert np.max(np.abs(spec.U @ a - sol[1:])) < 1e-9 * np.abs(sol[1:]).max()
+
+
+def test_huge_gamma_one_step_is_least_squares_kqr():
+    X, y, K, spec, _ = _problem(LOSS_QUANTILE, n=45)
+    n = len(y)
+    lam, gam, tau = 1e-2, 100.0, 0.3
+    a, b0, *_ = o.fit_column(spec, y, LOSS_QUANTILE, [gam], lam, np.ones(n), tau=tau, maxit=1, momentum=False)
+    A = np.zeros((n + 1, n + 1))
+    A[0, 1:] = 1.0
+    A[1:, 0] = 1.0
+    A[1:, 1:] = K + 4 * gam * n * lam * np.eye(n)
+    sol = np.linalg.solve(A, np.concatenate([[0.0], y + 2 * gam * (tau - 0.5)]))
+    assert abs(b0 - sol[0]) < 1e-9 * max(1, abs(sol[0]))
+    assert np.max(np.abs(spec.U @ a - sol[1:])) < 1e-9 * np.abs(sol[1:]).max()
+
+
+# ---------------------------------------------------------------- P5: MM descent
+@pytest.mark.parametrize("loss,smooth,tau", [(LOSS_HINGE, 0.125, None), (LOSS_LOGISTIC, None, None),
+                                             (LOSS_QUANTILE, 0.125, 0.9)])
+def test_objective_never_increases_without_momentum(loss, smooth, tau):
+    X, y, K, spec, foldid = _problem(loss, n=40)
+    mask = (foldid != 0).astype(float)
+    lam = 1e-3
+    trace = []
+    o.fit_column(spec, y, loss, [smooth], lam, mask, tau=tau, maxit=60, momentum=False, trace=trace)
+    vals = [o.objective(K, y, spec.U @ ab, bb, lam, loss, mask, smooth, tau) for (_, _, ab, bb) in trace]
+    assert len(vals) == 60
+    assert np.all(np.diff(vals) <= 1e-13 * max(1.0, abs(vals[0])))
+    assert vals[-1] < vals[0]
+
+
+# ---------------------------------------------------------------- P6: KKT at convergence
+@pytest.mark.parametrize("loss,taus", [(LOSS_HINGE, ()), (LOSS_LOGISTIC, ()), (LOSS_QUANTILE, (0.1, 0.5, 0.9))])
+def test_kkt_of_every_path_solution(loss, taus):
+    X, y, K, spec, foldid = _problem(loss, n=48)
+    lambdas = wl.lambda_grid(0, -4, 4)
+    V = 4
+    res = o.fit_path(spec, y, loss, lambdas, foldid, V, taus=taus, smooth0=1.0, eta=0.125, rounds=3,
+                     tol=1e-12, maxit=100000)
+    assert res.flags.sum() == 0
+    cols = res.cols
+    for c in range(cols["B"]):
+        lam, M, n_c = cols["lam"][c], cols["M"][:, c], cols["n_c"][c]
+        tau = cols["tau"][c] if loss == LOSS_QUANTILE else None
+        alpha = spec.U @ res.a[:, c]
+        f = K @ alpha + res.beta0[c]                                   # straight from K, not U
+        z = M * o.psi(loss, y, f, res.smooth_final, tau) / n_c
+        assert abs(z.sum()) < 1e-11                                    # d/d beta0 = 1^T z = 0
+        assert np.max(np.abs(z + 2 * lam * alpha)) * n_c < 1e-9        # alpha = -z / (2 lam)
+        assert abs(alpha.sum()) * 2 * lam * n_c < 1e-9                 # sum alpha = 0
+        w2 = 2 * lam * n_c * alpha
+        if loss == LOSS_QUANTILE:
+            assert np.all(w2 >= tau - 1 - 1e-9) and np.all(w2 <= tau + 1e-9)
+        else:
+            assert np.all(y * w2 >= -1e-9) and np.all(y * w2 <= 1 + 1e-9)
+        assert np.all(np.abs(alpha[M == 0]) * 2 * lam * n_c < 1e-9)    # P8: held-out alpha = 0
+    # column mode and batched mode reach the same point
+    levels = o.smoothing_levels(loss, 1.0, 0.125, 3)
+    for c in (0, cols["B"] // 2, cols["B"] - 1):
+        tau = cols["tau"][c] if loss == LOSS_QUANTILE else None
+        a, b0, *_ = o.fit_column(spec, y, loss, levels, cols["lam"][c], cols["M"][:, c], tau=tau,
+                                 tol=1e-12, maxit=100000)
+        al, al2 = spec.U @ a, spec.U @ res.a[:, c]
+        assert np.linalg.norm(al - al2) <= 1e-8 * np.linalg.norm(al2)
+        assert abs(b0 - res.beta0[c]) < 1e-8
+
+
+def test_logistic_against_independent_newton():
+    """Independent solve of the stationarity equations alpha + z(K alpha + b)/(2 lam) = 0,
+    1^T z = 0 by Newton's method on the dense system (no eigendecomposition, no MM)."""
+    X, y, K, spec, foldid = _problem(LOSS_LOGISTIC, n=40)
+    n = len(y)
+    lam = 5e-3
+    mask = (foldid != 2).astype(float)
+    n_c = mask.sum()
+    a, b0, *_ = o.fit_column(spec, y, LOSS_LOGISTIC, [None], lam, mask, tol=1e-13, maxit=100000)
+    alpha, beta = np.zeros(n), 0.0
+    for _ in range(50):
+        f = K @ alpha + beta
+        sg = 1.0 / (1.0 + np.exp(y * f))
+        z = mask * (-y * sg) / n_c
+        D = mask * sg * (1 - sg) / n_c                                 # d z / d f
+        G = np.concatenate([alpha + z / (2 * lam), [z.sum()]])
+        J = np.zeros((n + 1, n + 1))
+        J[:n, :n] = np.eye(n) + (D[:, None] * K) / (2 * lam)
+        J[:n, n] = D / (2 * lam)
+        J[n, :n] = D @ K
+        J[n, n] = D.sum()
+        step = np.linalg.solve(J, G)
+        alpha -= step[:n]
+        beta -= step[n]
+        if np.max(np.abs(step)) < 1e-14:
+            break
+    assert np.linalg.norm(spec.U @ a - alpha) < 1e-9 * np.linalg.norm(alpha)
+    assert abs(b0 - beta) < 1e-9
+
+
+def test_hinge_against_scipy_minimiser():
+    """Objective value of the converged smoothed-hinge fit vs a generic quasi-Newton
+    minimiser of the same objective in (beta0, a) coordinates."""
+    from scipy.optimize import minimize
+    X, y, K, spec, foldid = _problem(LOSS_HINGE, n=30)
+    n = len(y)
+    lam, delta = 1e-2, 0.125
+    mask = (foldid != 0).astype(float)
+    a, b0, *_ = o.fit_column(spec, y, LOSS_HINGE, [delta], lam, mask, tol=1e-12, maxit=100000)
+    mine = o.objective(K, y, spec.U @ a, b0, lam, LOSS_HINGE, mask, delta)
+
+    def fun(x):
+        return o.objective(K, y, x[1:], x[0], lam, LOSS_HINGE, mask, delta)
+    best = minimize(fun, np.zeros(n + 1), method="BFGS", options=dict(gtol=1e-10, maxiter=5000))
+    assert mine <= best.fun + 1e-12
+    assert best.fun - mine < 1e-7
+
+
+# ---------------------------------------------------------------- P10: large-lambda limit
+def test_large_lambda_limit_closed_forms():
+    n = 60
+    rng = np.random.default_rng(8)
+    X = rng.standard_normal((n, 3))
+    K = o.gram_rbf(X, 1.5)
+    spec = o.spectral_setup(K)
+    y = np.ones(n)
+    y[:21] = -1.0                                                      # n+ = 39, n- = 21
+    lam = 1e7
+    ones = np.ones(n)
+    delta = 0.125
+    a, b0, *_ = o.fit_column(spec, y, LOSS_HINGE, [delta], lam, ones, tol=1e-13, maxit=100000)
+    assert b0 == pytest.approx(1 + delta - 2 * delta * 21 / 39, abs=1e-5)
+    alpha = spec.U @ a
+    assert np.max(np.abs(alpha)) < 1e-6
+    assert np.allclose(2 * lam * n * alpha, -o.psi(LOSS_HINGE, y, b0 * ones, delta), atol=1e-4)
+    a, b0, *_ = o.fit_column(spec, y, LOSS_LOGISTIC, [None], lam, ones, tol=1e-13, maxit=100000)
+    assert b0 == pytest.approx(np.log(39 / 21), abs=1e-5)
+    yq = rng.standard_normal(n)
+    g, tau = 0.05, 0.3
+    a, b0, *_ = o.fit_column(spec, yq, LOSS_QUANTILE, [g], lam, ones, tau=tau, tol=1e-13, maxit=100000)
+    # root of sum_j H'(y_j - b0) = 0
+    t = yq - b0
+    hp = np.where(t < -g, tau - 1, np.where(t > g, tau, t / (2 * g) + tau - 0.5))
+    assert abs(hp.sum()) < 1e-4
+    assert abs(np.mean(t < 0) - tau) <= (np.sum(np.abs(t) <= g) + 1) / n      # P11
+
+
+# ---------------------------------------------------------------- P11, P12
+def test_kqr_residual_fraction_and_path_ordering():
+    X, y, K, spec, foldid = _problem(LOSS_QUANTILE, n=80, seed=9)
+    n = len(y)
+    lambdas = wl.lambda_grid(-1, -4, 5)
+    taus = (0.1, 0.5, 0.9)
+    res = o.fit_path(spec, y, LOSS_QUANTILE, lambdas, foldid, 4, taus=taus, rounds=4, tol=1e-11, maxit=200000)
+    cols = res.cols
+    g = res.smooth_final
+    for t, tau in enumerate(taus):
+        pen, fit = [], []
+        for l in range(5):
+            c = (t * 5 + 4) * 5 + l                                    # v = V: no fold held out
+            alpha = spec.U @ res.a[:, c]
+            f = K @ alpha + res.beta0[c]
+            r = y - f
+            assert abs(np.mean(r < 0) - tau) <= (np.sum(np.abs(r) <= g) + 1) / n   # P11
+            pen.append(alpha @ K @ alpha)
+            fit.append(np.mean(o.smooth_loss(LOSS_QUANTILE, y, f, g, tau)))
+        # lambdas descending: penalty non-decreasing, training loss non-increasing (P12)
+        assert np.all(np.diff(pen) >= -1e-9) and np.all(np.diff(fit) <= 1e-9)
