@@ -1,0 +1,187 @@
+/* tkm.h -- C ABI of libtkm: the B200 (sm_100a) spectral solution-path + exact cross-validation
+ * library for kernel machines (smoothed-hinge SVM, kernel logistic regression, kernel quantile
+ * regression).  Method: "TorchKM", arxiv/paper_2606_06742; citations below are PAPER.md:<line>
+ * of that paper's text, plus the readings G1..G19 of SURVEY.md section 8(c) / DESIGN.md.
+ *
+ * Conventions
+ *   - extern "C"; every call returns a tkm_status (0 = TKM_OK).  tkm_last_error() returns a
+ *     thread-local, NUL-terminated description of the last failure on the calling thread.
+ *     No exception crosses the boundary; there is no global mutable state besides that string.
+ *   - [dev]  = pointer to DEVICE memory owned by the caller (e.g. a torch tensor's data_ptr()).
+ *     [host] = pointer to HOST memory owned by the caller.  Nothing passed in is retained after
+ *     the call returns except where stated (tkm_path keeps a pointer to its tkm_spectral).
+ *   - Matrices are row-major with an explicit leading dimension in ELEMENTS.
+ *   - Handles (tkm_spectral*, tkm_path*) are owned by the library: free with tkm_*_free.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Calls that
+ *     write [host] outputs synchronise the stream before returning; the others are asynchronous
+ *     with respect to the host.
+ *   - There is no CPU fallback: without a CUDA device every compute call returns TKM_ECUDA.
+ *
+ * Column ordering of a path:  c = (t (V+1) + v) L + l, with t the loss variant
+ * (quantile level), v the held-out fold (v = V: nothing held out, the final model) and l the
+ * index into the lambda grid.  B = T L (V+1) columns.
+ */
+#ifndef TKM_H
+#define TKM_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TKM_VERSION_MAJOR 0
+#define TKM_VERSION_MINOR 1
+
+typedef enum {
+  TKM_OK = 0,
+  TKM_EINVAL = 1,    /* bad argument (message says which) */
+  TKM_ENOMEM = 2,    /* device or host allocation failed */
+  TKM_ECUDA = 3,     /* CUDA runtime error / no device */
+  TKM_ESOLVER = 4,   /* cuSOLVER failure or info != 0 */
+  TKM_ENOTCONV = 5,  /* warning: some column hit maxit; all outputs are still written */
+  TKM_ENOTIMPL = 6
+} tkm_status;
+
+typedef enum { TKM_F32 = 0, TKM_F64 = 1 } tkm_dtype;
+
+typedef enum {
+  TKM_LOSS_HINGE = 0,    /* delta-smoothed hinge */
+  TKM_LOSS_LOGISTIC = 1, /* log(1 + exp(-y f)); reading G9 */
+  TKM_LOSS_QUANTILE = 2  /* gamma-smoothed check loss; reading G10 */
+} tkm_loss;
+
+typedef struct tkm_spectral tkm_spectral; /* K = U Lam U^T and derived device arrays */
+typedef struct tkm_path tkm_path;         /* the fitted columns (a, beta0) of one grid */
+
+/* Options of the loss / smoothing schedule (reading G7: fixed schedule
+ * smooth_k = smooth0 * eta^k, k = 0..rounds-1, each round warm-started from the previous one). */
+typedef struct {
+  double smooth0;     /* delta_0 (hinge) / gamma_0 (quantile); ignored for logistic          */
+  double eta;         /* shrink factor, the paper's 0.125                      */
+  int32_t rounds;     /* R >= 1 smoothing rounds (forced to 1 for logistic)                   */
+  int32_t T;          /* number of quantile levels (0 or 1 => one variant)                    */
+  const double* taus; /* [host] T quantile levels in (0,1); NULL unless loss == QUANTILE      */
+  int32_t restart;    /* 1: gradient restart of the Nesterov sequence (default), 0: plain     */
+  int32_t check_every;/* iterations between host convergence polls; <= 0 => library default   */
+  double warm_tol;    /* tolerance of rounds 0..R-2 (warm starts only); <= 0 => same as tol   */
+} tkm_loss_opts;
+
+/* Nystrom inputs for tkm_spectral_setup (reading G11). */
+typedef struct {
+  const double* K_nm;        /* [dev] n x m cross kernel k(x_i, x_landmark_j), FP64            */
+  int64_t ld_nm;
+  const double* K_mm;        /* [dev] m x m landmark kernel, FP64                              */
+  int64_t ld_mm;
+  int64_t m;                 /* number of landmarks                                            */
+  const int64_t* landmark_idx; /* [host] m row indices into X (kept for tkm_predict)           */
+} tkm_nystrom;
+
+/* ---- S1  RBF Gram matrix (PAPER.md:69 kernel="rbf"; reading G12) -----------------------------
+ * K[i][j] = exp(-||X[i,:] - X2[j,:]||^2 / (2 sigma^2)), FP64 arithmetic, direct differences.
+ * X  [dev] n x p FP64 (ldx >= p).  X2 [dev] n2 x p FP64 or NULL: NULL => X2 = X, n2 = n, only
+ * the upper-triangular tiles are computed and mirrored, so K is bit-exactly symmetric with an
+ * exact unit diagonal.  K [dev] n x n2, out_dt FP64 or FP32 (rounded once from FP64), ldk >= n2.
+ * Errors: sigma <= 0, n/p/ld out of range -> TKM_EINVAL.  Asynchronous. */
+int tkm_gram(const void* X, int64_t n, int64_t p, int64_t ldx,
+             const void* X2, int64_t n2, int64_t ldx2,
+             double sigma, tkm_dtype out_dt, void* K, int64_t ldk, void* stream);
+
+/* ---- S2  one-time spectral setup (Alg.1 l.3, 226; readings G11, G16, G19) --------
+ * Full kernel (ny == NULL): K [dev] n x n FP64 symmetric (not modified); decomposes in FP64 with
+ * cuSOLVER syevd, clamps Lam >= 0, forms u1 = U^T 1, and keeps U Lam (n x r) and U^T (r x n) in
+ * `sweep_dt` precision for the two contractions of the sweep (TKM_F32: split into TF32 hi + lo
+ * parts for the 3xTF32 tensor-core path; TKM_F64: FP64 DMMA path).  r = n.
+ * Nystrom (ny != NULL): K is ignored (may be NULL); thin U (n x r, r <= m) from K_nm, K_mm.
+ * The handle is shared by every lambda, fold and quantile level.  Synchronises `stream`.
+ * Errors: TKM_ESOLVER if cuSOLVER reports info != 0; TKM_ENOMEM. */
+int tkm_spectral_setup(const void* K, int64_t n, int64_t ldk, const tkm_nystrom* ny,
+                       tkm_dtype sweep_dt, tkm_spectral** out, void* stream);
+void tkm_spectral_free(tkm_spectral* s);
+/* n, r, and [host] copies of Lam (r) and u1 (r); either output pointer may be NULL. */
+int tkm_spectral_info(const tkm_spectral* s, int64_t* n, int64_t* r, double* lam, double* u1);
+/* Copy U (n x r, FP64, row-major, ld = r) to [dev] U_out -- test / diagnostic accessor. */
+int tkm_spectral_get_u(const tkm_spectral* s, double* U_out, void* stream);
+
+/* ---- S3-S8  the batched spectral MM sweep (Alg.1 178-224, 226-232) --
+ * Fits all B = T L (V+1) columns: for column (t, l, v) the minimiser of
+ *   (1/n_c) sum_{j: foldid_j != v} loss_t(y_j, K_j^T alpha + beta0) + lambda_l alpha^T K alpha
+ * (eq.(1), 166) at the final smoothing level, by the Nesterov-accelerated
+ * majorise-minimise iteration applied through the spectral block inverse (all columns stacked,
+ * two contractions with U per iteration).  State is kept in spectral coordinates a = U^T alpha.
+ *   y       [dev]  n FP64 (+-1 for HINGE / LOGISTIC, checked; real for QUANTILE)
+ *   lambdas [host] L values > 0          foldid [host] n values in [0, V), every fold non-empty
+ *   tol     stop when max(|1^T z|, n_c ||rho||_2 / sqrt(n)) <= tol per column (reading G6)
+ *   maxit   per column per round; columns that hit it are flagged and TKM_ENOTCONV is returned
+ *   warm    optional path of the same shape on the same spectral handle to start from, or NULL
+ * The path keeps a pointer to `s`, which must outlive it.  Synchronises `stream`. */
+int tkm_fit_path(const tkm_spectral* s, const void* y, tkm_loss loss, const tkm_loss_opts* opts,
+                 const double* lambdas, int32_t L, const int32_t* foldid, int32_t V,
+                 double tol, int32_t maxit, const tkm_path* warm, tkm_path** out, void* stream);
+void tkm_path_free(tkm_path* p);
+/* Shape and per-column diagnostics, all [host], any pointer may be NULL:
+ * B, r; iters[B] (total over rounds), kkt[B] (last residual), flags[B] (1 = hit maxit),
+ * beta0[B]; total_col_iters = sum of iters (the unit of the roofline). */
+int tkm_path_info(const tkm_path* p, int32_t* B, int64_t* r, int32_t* iters, double* kkt,
+                  int32_t* flags, double* beta0, int64_t* total_col_iters);
+/* Spectral coordinates of all columns: [dev] a_out, B x r FP64 row-major (ld = r). */
+int tkm_path_get_a(const tkm_path* p, double* a_out, void* stream);
+
+/* ---- S9  exact cross-validation scores (readings G14, G15) -------------
+ * For every (t, l, v), v < V: decision values f_j = [U (Lam * a_c)]_j + beta0_c on the rows of
+ * fold v, cv_loss = mean nominal loss (hinge / deviance / check), cv_err = #{label(f_j) != y_j}
+ * (classifiers; -1 for QUANTILE), cv_mean[t][l] = (1/n) sum_v |v| cv_loss[t][l][v],
+ * best_l[t] = argmin_l cv_mean[t][l], ties -> the largest lambda.  No refitting.
+ *   cv_loss [host] T x L x V doubles, cv_err [host] T x L x V int64 or NULL,
+ *   cv_mean [host] T x L, best_l [host] T.   Synchronises `stream`. */
+int tkm_exact_cv(const tkm_path* p, const void* y, const int32_t* foldid,
+                 double* cv_loss, int64_t* cv_err, double* cv_mean, int32_t* best_l, void* stream);
+
+/* ---- S10 coefficients and prediction (readings G11, G15) --------------------
+ * tkm_path_coef: alpha = U a of column (t, l, v) into [dev] alpha (n FP64; Nystrom: the m landmark
+ * weights gamma), and beta0 into [host] *beta0.  Synchronises `stream`. */
+int tkm_path_coef(const tkm_path* p, int32_t t, int32_t l, int32_t v, double* alpha, double* beta0,
+                  void* stream);
+/* tkm_predict: f(x) = sum_i exp(-||x - x_i||^2 / (2 sigma^2)) alpha_i + beta0 with the v = V
+ * column of (t, l); the cross-kernel is fused with the contraction and never written.
+ *   X_train [dev] n x p FP64 (the training matrix; Nystrom: landmark rows are gathered from it)
+ *   X_new   [dev] n_new x p FP64;  f_out [dev] n_new FP64;  label_out [dev] n_new int8 (+1 if
+ *   f >= 0 else -1) or NULL.  Asynchronous after an internal coefficient computation. */
+int tkm_predict(const tkm_path* p, int32_t t, int32_t l,
+                const void* X_train, int64_t ldx, const void* X_new, int64_t n_new, int64_t ldxn,
+                int64_t pdim, double sigma, void* f_out, int8_t* label_out, void* stream);
+
+/* ---- whole pipeline from HOST buffers (the end-to-end call timed as `e2e` by bench.py) ---------
+ * X [host] n x p FP64, y [host] n FP64; copies them to the device, runs S1, S2, S3-S8, S9 for one
+ * sigma and returns [host] cv tables as in tkm_exact_cv plus the final-model coefficients of the
+ * selected lambda of variant 0 ([host] alpha_best n doubles or NULL, *beta0_best).
+ * Full kernel only.  stage_ms [host] 5 floats or NULL: copy-in, gram, eig, sweep, cv (ms). */
+int tkm_train_tune_host(const double* X, int64_t n, int64_t p, const double* y, double sigma,
+                        tkm_loss loss, const tkm_loss_opts* opts, const double* lambdas, int32_t L,
+                        const int32_t* foldid, int32_t V, double tol, int32_t maxit,
+                        tkm_dtype sweep_dt, double* cv_loss, int64_t* cv_err, double* cv_mean,
+                        int32_t* best_l, double* alpha_best, double* beta0_best, float* stage_ms,
+                        void* stream);
+
+/* ---- helpers ------------------------------------------------------------------------------------
+ * tkm_make_folds: integer-only fold assignment (reading G13): SplitMix64(seed) -> Fisher-Yates
+ * permutation pi (j = next() mod (i+1), i = n-1..1) -> foldid[pi[i]] = i mod V.  [host] output.
+ * Needs 2 <= V <= n. */
+int tkm_make_folds(int64_t n, int32_t V, uint64_t seed, int32_t* foldid);
+/* Number of kernels launched by this library on the calling thread since the last reset
+ * (bench.py's `gpu_launches`). */
+int64_t tkm_launch_count(void);
+void tkm_launch_count_reset(void);
+/* Dense FP64 GEMM probe on the library's own DMMA kernel (roofline calibration / tests):
+ * Dt[N][M] = P[N][K] Q[M][K]^T, all [dev] FP64 row-major with leading dims ldp, ldq, ldd that are
+ * multiples of 2 and >= K (P, Q) / >= M (Dt); the K-padding up to a multiple of 16 must be
+ * readable zeros.  Asynchronous. */
+int tkm_dgemm_nt(const double* P, int64_t ldp, const double* Q, int64_t ldq, double* Dt, int64_t ldd,
+                 int64_t N, int64_t M, int64_t K, void* stream);
+int tkm_version(void);
+const char* tkm_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TKM_H */

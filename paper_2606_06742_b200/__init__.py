@@ -1,0 +1,15 @@
+"""paper_2606_06742_b200 -- thin Python binding of libtkm, the B200 (sm_100a) C-ABI library for the
+spectral solution path + exact cross-validation of kernel machines (TorchKM, arxiv/paper_2606_06742).
+
+Argument marshalling only: every step of the path (Gram, spectral setup, sweep, exact CV, predict)
+runs in the CUDA kernels of `csrc/`, reached through the `tkm_*` entry points declared in
+`include/tkm.h`.  PyTorch is used for device memory and streams.  There is no CPU fallback: a
+missing `libtkm.so` or a missing GPU raises.
+"""
+from .api import (  # noqa: F401
+    TkmError, LOSS_HINGE, LOSS_LOGISTIC, LOSS_QUANTILE, F32, F64,
+    lib, lib_path, tkm_version, tkm_last_error, tkm_make_folds,
+    tkm_gram, tkm_spectral_setup, tkm_fit_path, tkm_exact_cv, tkm_predict, tkm_path_coef,
+    tkm_train_tune_host, tkm_dgemm_nt, tkm_launch_count, tkm_launch_count_reset,
+    Spectral, Path, EXPORTED_SYMBOLS,
+)

@@ -1,0 +1,335 @@
+"""ctypes binding of libtkm.so: same names as the C ABI (include/tkm.h), torch tensors for [dev]
+arguments, numpy arrays for [host] arguments.  No arithmetic of the method lives here."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+LOSS_HINGE, LOSS_LOGISTIC, LOSS_QUANTILE = 0, 1, 2
+F32, F64 = 0, 1
+TKM_OK, TKM_ENOTCONV = 0, 5
+
+EXPORTED_SYMBOLS = [
+    "tkm_gram", "tkm_spectral_setup", "tkm_spectral_free", "tkm_spectral_info", "tkm_spectral_get_u",
+    "tkm_fit_path", "tkm_path_free", "tkm_path_info", "tkm_path_get_a", "tkm_exact_cv", "tkm_path_coef",
+    "tkm_predict", "tkm_train_tune_host", "tkm_make_folds", "tkm_launch_count", "tkm_launch_count_reset",
+    "tkm_dgemm_nt", "tkm_version", "tkm_last_error",
+]
+
+
+class TkmError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("libtkm error %d: %s" % (code, msg))
+        self.code = code
+
+
+class _LossOpts(C.Structure):
+    _fields_ = [("smooth0", C.c_double), ("eta", C.c_double), ("rounds", C.c_int32), ("T", C.c_int32),
+                ("taus", C.POINTER(C.c_double)), ("restart", C.c_int32), ("check_every", C.c_int32),
+                ("warm_tol", C.c_double)]
+
+
+class _Nystrom(C.Structure):
+    _fields_ = [("K_nm", C.c_void_p), ("ld_nm", C.c_int64), ("K_mm", C.c_void_p), ("ld_mm", C.c_int64),
+                ("m", C.c_int64), ("landmark_idx", C.POINTER(C.c_int64))]
+
+
+def lib_path() -> str:
+    return os.path.join(os.path.dirname(os.path.abspath(__file__)), "libtkm.so")
+
+
+_lib = None
+
+
+def lib():
+    """Loads libtkm.so (built by `python -m paper_2606_06742_b200.build`); raises if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = lib_path()
+    if not os.path.exists(path):
+        raise TkmError(-1, "%s not found: build it with `python -m paper_2606_06742_b200.build` "
+                           "(there is no CPU fallback)" % path)
+    L = C.CDLL(path)
+    vp, i64, i32, dbl = C.c_void_p, C.c_int64, C.c_int32, C.c_double
+    L.tkm_gram.argtypes = [vp, i64, i64, i64, vp, i64, i64, dbl, C.c_int, vp, i64, vp]
+    L.tkm_spectral_setup.argtypes = [vp, i64, i64, C.POINTER(_Nystrom), C.c_int, C.POINTER(vp), vp]
+    L.tkm_spectral_free.argtypes = [vp]
+    L.tkm_spectral_free.restype = None
+    L.tkm_spectral_info.argtypes = [vp, C.POINTER(i64), C.POINTER(i64), vp, vp]
+    L.tkm_spectral_get_u.argtypes = [vp, vp, vp]
+    L.tkm_fit_path.argtypes = [vp, vp, C.c_int, C.POINTER(_LossOpts), vp, i32, vp, i32, dbl, i32, vp,
+                               C.POINTER(vp), vp]
+    L.tkm_path_free.argtypes = [vp]
+    L.tkm_path_free.restype = None
+    L.tkm_path_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i64), vp, vp, vp, vp, C.POINTER(i64)]
+    L.tkm_path_get_a.argtypes = [vp, vp, vp]
+    L.tkm_exact_cv.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
+    L.tkm_path_coef.argtypes = [vp, i32, i32, i32, vp, C.POINTER(dbl), vp]
+    L.tkm_predict.argtypes = [vp, i32, i32, vp, i64, vp, i64, i64, i64, dbl, vp, vp, vp]
+    L.tkm_train_tune_host.argtypes = [vp, i64, i64, vp, dbl, C.c_int, C.POINTER(_LossOpts), vp, i32, vp, i32,
+                                      dbl, i32, C.c_int, vp, vp, vp, vp, vp, C.POINTER(dbl), vp, vp]
+    L.tkm_make_folds.argtypes = [i64, i32, C.c_uint64, vp]
+    L.tkm_launch_count.restype = i64
+    L.tkm_launch_count_reset.restype = None
+    L.tkm_dgemm_nt.argtypes = [vp, i64, vp, i64, vp, i64, i64, i64, i64, vp]
+    L.tkm_last_error.restype = C.c_char_p
+    for name in EXPORTED_SYMBOLS:
+        getattr(L, name)   # AttributeError if the library does not export a declared symbol
+    _lib = L
+    return L
+
+
+def _check(rc, allow_notconv=False):
+    if rc == TKM_OK or (allow_notconv and rc == TKM_ENOTCONV):
+        return rc
+    raise TkmError(rc, lib().tkm_last_error().decode())
+
+
+def _stream(stream=None):
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return C.c_void_p(s.cuda_stream)
+
+
+def _dev_f64(t, name):
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64):
+        raise TypeError("%s must be a CUDA float64 tensor" % name)
+    return t
+
+
+def _host(a, dtype):
+    return np.ascontiguousarray(a, dtype=dtype)
+
+
+def _ptr(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def tkm_version() -> int:
+    return lib().tkm_version()
+
+
+def tkm_last_error() -> str:
+    return lib().tkm_last_error().decode()
+
+
+def tkm_launch_count() -> int:
+    return int(lib().tkm_launch_count())
+
+
+def tkm_launch_count_reset() -> None:
+    lib().tkm_launch_count_reset()
+
+
+def tkm_make_folds(n: int, V: int, seed: int) -> np.ndarray:
+    out = np.empty(n, dtype=np.int32)
+    _check(lib().tkm_make_folds(n, V, C.c_uint64(seed & (2 ** 64 - 1)), _ptr(out)))
+    return out
+
+
+def tkm_gram(X, sigma: float, X2=None, out_dtype=F64, stream=None):
+    """K = exp(-||x_i - x'_j||^2 / (2 sigma^2)); X, X2 CUDA float64 2-D tensors (row stride = ld)."""
+    import torch
+    X = _dev_f64(X, "X")
+    if X.dim() != 2 or X.stride(1) != 1:
+        raise ValueError("X must be 2-D with unit inner stride")
+    n, p = X.shape
+    if X2 is not None:
+        X2 = _dev_f64(X2, "X2")
+        if X2.dim() != 2 or X2.stride(1) != 1 or X2.shape[1] != p:
+            raise ValueError("X2 must be n2 x p with unit inner stride")
+        n2, ld2, p2 = X2.shape[0], X2.stride(0), C.c_void_p(X2.data_ptr())
+    else:
+        n2, ld2, p2 = 0, 0, None
+    K = torch.empty((n, n2 if X2 is not None else n), device=X.device,
+                    dtype=torch.float64 if out_dtype == F64 else torch.float32)
+    _check(lib().tkm_gram(X.data_ptr(), n, p, X.stride(0), p2, n2, ld2, float(sigma), out_dtype,
+                          K.data_ptr(), K.stride(0), _stream(stream)))
+    return K
+
+
+class Spectral:
+    """Owner of a tkm_spectral* (freed on garbage collection)."""
+
+    def __init__(self, handle, keepalive=()):
+        self._h = handle
+        self._keep = keepalive
+        n, r = C.c_int64(), C.c_int64()
+        _check(lib().tkm_spectral_info(self._h, C.byref(n), C.byref(r), None, None))
+        self.n, self.r = n.value, r.value
+
+    def eigenvalues(self):
+        lam, u1 = np.empty(self.r), np.empty(self.r)
+        _check(lib().tkm_spectral_info(self._h, None, None, _ptr(lam), _ptr(u1)))
+        return lam, u1
+
+    def U(self, stream=None):
+        import torch
+        out = torch.empty((self.n, self.r), device="cuda", dtype=torch.float64)
+        _check(lib().tkm_spectral_get_u(self._h, out.data_ptr(), _stream(stream)))
+        return out
+
+    def close(self):
+        if self._h:
+            lib().tkm_spectral_free(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def tkm_spectral_setup(K=None, n=None, nystrom=None, sweep_dtype=F64, stream=None) -> Spectral:
+    """Full kernel: K (n x n CUDA float64).  Nystrom: nystrom=(K_nm, K_mm, landmark_idx), n = rows."""
+    h = C.c_void_p()
+    if nystrom is None:
+        K = _dev_f64(K, "K")
+        n = K.shape[0]
+        _check(lib().tkm_spectral_setup(K.data_ptr(), n, K.stride(0), None, sweep_dtype, C.byref(h), _stream(stream)))
+        return Spectral(h)
+    K_nm, K_mm, idx = nystrom
+    K_nm, K_mm = _dev_f64(K_nm, "K_nm"), _dev_f64(K_mm, "K_mm")
+    idx = _host(idx, np.int64)
+    ny = _Nystrom(K_nm.data_ptr(), K_nm.stride(0), K_mm.data_ptr(), K_mm.stride(0), K_mm.shape[0],
+                  idx.ctypes.data_as(C.POINTER(C.c_int64)))
+    _check(lib().tkm_spectral_setup(None, K_nm.shape[0], 0, C.byref(ny), sweep_dtype, C.byref(h), _stream(stream)))
+    return Spectral(h)
+
+
+class Path:
+    """Owner of a tkm_path*; keeps its Spectral alive."""
+
+    def __init__(self, handle, spec, status):
+        self._h = handle
+        self.spec = spec
+        self.status = status            # TKM_OK or TKM_ENOTCONV
+        B, r, tot = C.c_int32(), C.c_int64(), C.c_int64()
+        _check(lib().tkm_path_info(self._h, C.byref(B), C.byref(r), None, None, None, None, C.byref(tot)))
+        self.B, self.r, self.total_col_iters = B.value, r.value, tot.value
+
+    def info(self):
+        iters = np.empty(self.B, dtype=np.int32)
+        kkt = np.empty(self.B)
+        flags = np.empty(self.B, dtype=np.int32)
+        beta0 = np.empty(self.B)
+        _check(lib().tkm_path_info(self._h, None, None, _ptr(iters), _ptr(kkt), _ptr(flags), _ptr(beta0), None))
+        return dict(iters=iters, kkt=kkt, flags=flags, beta0=beta0)
+
+    def a(self, stream=None):
+        import torch
+        out = torch.empty((self.B, self.r), device="cuda", dtype=torch.float64)
+        _check(lib().tkm_path_get_a(self._h, out.data_ptr(), _stream(stream)))
+        return out
+
+    def close(self):
+        if self._h:
+            lib().tkm_path_free(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol):
+    taus_arr = _host(taus if taus is not None else [], np.float64)
+    o = _LossOpts(float(smooth0), float(eta), int(rounds), int(len(taus_arr)),
+                  taus_arr.ctypes.data_as(C.POINTER(C.c_double)) if len(taus_arr) else None,
+                  int(bool(restart)), int(check_every), float(warm_tol))
+    return o, taus_arr
+
+
+def tkm_fit_path(spec: Spectral, y, loss: int, lambdas, foldid, V: int, tol: float, maxit: int,
+                 smooth0=1.0, eta=0.125, rounds=4, taus=None, restart=True, check_every=0, warm_tol=0.0,
+                 warm: Path | None = None, stream=None) -> Path:
+    y = _dev_f64(y, "y")
+    lam = _host(lambdas, np.float64)
+    fid = _host(foldid, np.int32)
+    o, keep = _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol)
+    h = C.c_void_p()
+    rc = lib().tkm_fit_path(spec._h, y.data_ptr(), loss, C.byref(o), _ptr(lam), len(lam), _ptr(fid), V,
+                            float(tol), int(maxit), warm._h if warm is not None else None, C.byref(h),
+                            _stream(stream))
+    _check(rc, allow_notconv=True)
+    return Path(h, spec, rc)
+
+
+def tkm_exact_cv(path: Path, y, foldid, T: int, L: int, V: int, stream=None):
+    y = _dev_f64(y, "y")
+    fid = _host(foldid, np.int32)
+    cv_loss = np.empty((T, L, V))
+    cv_err = np.empty((T, L, V), dtype=np.int64)
+    cv_mean = np.empty((T, L))
+    best = np.empty(T, dtype=np.int32)
+    _check(lib().tkm_exact_cv(path._h, y.data_ptr(), _ptr(fid), _ptr(cv_loss), _ptr(cv_err), _ptr(cv_mean),
+                              _ptr(best), _stream(stream)))
+    return cv_loss, cv_err, cv_mean, best
+
+
+def tkm_path_coef(path: Path, t: int, l: int, v: int, stream=None):
+    import torch
+    n = path.spec.n
+    out = torch.empty(n, device="cuda", dtype=torch.float64)   # Nystrom: first m entries are used
+    b0 = C.c_double()
+    _check(lib().tkm_path_coef(path._h, t, l, v, out.data_ptr(), C.byref(b0), _stream(stream)))
+    return out, b0.value
+
+
+def tkm_predict(path: Path, t: int, l: int, X_train, X_new, sigma: float, labels=True, stream=None):
+    import torch
+    X_train, X_new = _dev_f64(X_train, "X_train"), _dev_f64(X_new, "X_new")
+    n_new, p = X_new.shape
+    f = torch.empty(n_new, device="cuda", dtype=torch.float64)
+    lab = torch.empty(n_new, device="cuda", dtype=torch.int8) if labels else None
+    _check(lib().tkm_predict(path._h, t, l, X_train.data_ptr(), X_train.stride(0), X_new.data_ptr(), n_new,
+                             X_new.stride(0), p, float(sigma), f.data_ptr(),
+                             lab.data_ptr() if lab is not None else None, _stream(stream)))
+    return f, lab
+
+
+def tkm_train_tune_host(X, y, sigma, loss, lambdas, foldid, V, tol, maxit, smooth0=1.0, eta=0.125, rounds=4,
+                        taus=None, restart=True, check_every=0, warm_tol=0.0, sweep_dtype=F64,
+                        want_alpha=True, stream=None):
+    """Whole pipeline from HOST numpy buffers (the `e2e` call of bench.py)."""
+    X = _host(X, np.float64)
+    y = _host(y, np.float64)
+    lam = _host(lambdas, np.float64)
+    fid = _host(foldid, np.int32)
+    n, p = X.shape
+    o, keep = _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol)
+    T, L = max(1, len(keep)), len(lam)
+    cv_loss = np.empty((T, L, V))
+    cv_err = np.empty((T, L, V), dtype=np.int64)
+    cv_mean = np.empty((T, L))
+    best = np.empty(T, dtype=np.int32)
+    alpha = np.empty(n) if want_alpha else None
+    b0 = C.c_double()
+    stage = np.zeros(5, dtype=np.float32)
+    rc = lib().tkm_train_tune_host(_ptr(X), n, p, _ptr(y), float(sigma), loss, C.byref(o), _ptr(lam), L, _ptr(fid),
+                                   V, float(tol), int(maxit), sweep_dtype, _ptr(cv_loss), _ptr(cv_err),
+                                   _ptr(cv_mean), _ptr(best), _ptr(alpha) if want_alpha else None, C.byref(b0),
+                                   _ptr(stage), _stream(stream))
+    _check(rc, allow_notconv=True)
+    return dict(cv_loss=cv_loss, cv_err=cv_err, cv_mean=cv_mean, best_l=best, alpha=alpha, beta0=b0.value,
+                stage_ms=stage, status=rc)
+
+
+def tkm_dgemm_nt(P, Q, stream=None):
+    """Dt[N][M] = P[N][K] Q[M][K]^T on the library's DMMA kernel (probe / tests)."""
+    import torch
+    P, Q = _dev_f64(P, "P"), _dev_f64(Q, "Q")
+    N, K = P.shape
+    M = Q.shape[0]
+    ldd = (M + 1) // 2 * 2
+    D = torch.empty((N, ldd), device="cuda", dtype=torch.float64)
+    _check(lib().tkm_dgemm_nt(P.data_ptr(), P.stride(0), Q.data_ptr(), Q.stride(0), D.data_ptr(), ldd, N, M, K,
+                              _stream(stream)))
+    return D[:, :M]

@@ -1,0 +1,131 @@
+// api.cu -- library-wide plumbing of the C ABI: error string, launch counter, device check, the
+// integer-only fold generator and the whole-pipeline host entry point.
+#include <cstdarg>
+#include <new>
+
+#include "handles.cuh"
+
+namespace tkm {
+
+char* err_buf() {
+  static thread_local char buf[512] = {0};
+  return buf;
+}
+
+int set_error(int code, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(err_buf(), 512, fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+int64_t& launch_counter() {
+  static thread_local int64_t c = 0;
+  return c;
+}
+
+int device_check() {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    return set_error(TKM_ECUDA, "no CUDA device: %s (libtkm has no CPU fallback)", cudaGetErrorString(e));
+  }
+  static thread_local int checked_dev = -1;
+  if (checked_dev == dev) return TKM_OK;
+  int major = 0;
+  e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+  if (e != cudaSuccess) return set_error(TKM_ECUDA, "cudaDeviceGetAttribute: %s", cudaGetErrorString(e));
+  if (major != 10)
+    return set_error(TKM_ECUDA, "libtkm is built for sm_100a only; device %d has compute capability %d.x", dev, major);
+  checked_dev = dev;
+  return TKM_OK;
+}
+
+}  // namespace tkm
+
+using namespace tkm;
+
+extern "C" int tkm_version(void) { return TKM_VERSION_MAJOR * 100 + TKM_VERSION_MINOR; }
+extern "C" const char* tkm_last_error(void) { return err_buf(); }
+extern "C" int64_t tkm_launch_count(void) { return launch_counter(); }
+extern "C" void tkm_launch_count_reset(void) { launch_counter() = 0; }
+
+// SplitMix64 (Steele, Lea, Flood 2014) -> Fisher-Yates -> round-robin fold labels (reading G13).
+extern "C" int tkm_make_folds(int64_t n, int32_t V, uint64_t seed, int32_t* foldid) {
+  if (!foldid) return set_error(TKM_EINVAL, "tkm_make_folds: foldid is NULL");
+  if (V < 2 || (int64_t)V > n) return set_error(TKM_EINVAL, "tkm_make_folds: need 2 <= V <= n");
+  std::vector<int64_t> pi((size_t)n);
+  for (int64_t i = 0; i < n; ++i) pi[i] = i;
+  uint64_t x = seed;
+  for (int64_t i = n - 1; i >= 1; --i) {
+    x += 0x9E3779B97F4A7C15ull;
+    uint64_t z = x;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+    z ^= z >> 31;
+    const int64_t j = (int64_t)(z % (uint64_t)(i + 1));
+    std::swap(pi[i], pi[j]);
+  }
+  for (int64_t i = 0; i < n; ++i) foldid[pi[i]] = (int32_t)(i % V);
+  return TKM_OK;
+}
+
+extern "C" int tkm_train_tune_host(const double* X, int64_t n, int64_t p, const double* y, double sigma,
+                                   tkm_loss loss, const tkm_loss_opts* opts, const double* lambdas, int32_t L,
+                                   const int32_t* foldid, int32_t V, double tol, int32_t maxit,
+                                   tkm_dtype sweep_dt, double* cv_loss, int64_t* cv_err, double* cv_mean,
+                                   int32_t* best_l, double* alpha_best, double* beta0_best, float* stage_ms,
+                                   void* stream) {
+  if (!X || !y || !opts || !lambdas || !foldid || !cv_loss || !cv_mean || !best_l)
+    return set_error(TKM_EINVAL, "tkm_train_tune_host: NULL argument");
+  if (n <= 1 || p <= 0) return set_error(TKM_EINVAL, "tkm_train_tune_host: bad n / p");
+  TKM_TRY(device_check());
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaEvent_t ev[6];
+  for (auto& e : ev) TKM_CUDA(cudaEventCreate(&e));
+  struct EvGuard {
+    cudaEvent_t* e;
+    ~EvGuard() {
+      for (int i = 0; i < 6; ++i) cudaEventDestroy(e[i]);
+    }
+  } evg{ev};
+  DevBuf dX, dy, dK, dalpha;
+  TKM_CUDA(cudaEventRecord(ev[0], st));
+  TKM_TRY(dX.alloc((size_t)n * p * sizeof(double), false, st));
+  TKM_TRY(dy.alloc((size_t)n * sizeof(double), false, st));
+  TKM_TRY(dK.alloc((size_t)n * n * sizeof(double), false, st));
+  TKM_CUDA(cudaMemcpyAsync(dX.p, X, (size_t)n * p * sizeof(double), cudaMemcpyHostToDevice, st));
+  TKM_CUDA(cudaMemcpyAsync(dy.p, y, (size_t)n * sizeof(double), cudaMemcpyHostToDevice, st));
+  TKM_CUDA(cudaEventRecord(ev[1], st));
+  TKM_TRY(tkm_gram(dX.p, n, p, p, nullptr, 0, 0, sigma, TKM_F64, dK.p, n, st));
+  TKM_CUDA(cudaEventRecord(ev[2], st));
+  tkm_spectral* spec = nullptr;
+  TKM_TRY(tkm_spectral_setup(dK.p, n, n, nullptr, sweep_dt, &spec, st));
+  dK.release();
+  TKM_CUDA(cudaEventRecord(ev[3], st));
+  tkm_path* path = nullptr;
+  int rc = tkm_fit_path(spec, dy.p, loss, opts, lambdas, L, foldid, V, tol, maxit, nullptr, &path, st);
+  if (rc != TKM_OK && rc != TKM_ENOTCONV) {
+    tkm_spectral_free(spec);
+    return rc;
+  }
+  cudaEventRecord(ev[4], st);
+  int rc2 = tkm_exact_cv(path, dy.p, foldid, cv_loss, cv_err, cv_mean, best_l, st);
+  if (rc2 == TKM_OK && alpha_best) {
+    rc2 = dalpha.alloc((size_t)n * sizeof(double), false, st);
+    if (rc2 == TKM_OK) rc2 = tkm_path_coef(path, 0, best_l[0], V, dalpha.as<double>(), beta0_best, st);
+    if (rc2 == TKM_OK) {
+      cudaError_t e = cudaMemcpyAsync(alpha_best, dalpha.p, n * sizeof(double), cudaMemcpyDeviceToHost, st);
+      if (e != cudaSuccess) rc2 = set_error(TKM_ECUDA, "copy of alpha failed: %s", cudaGetErrorString(e));
+    }
+  }
+  cudaEventRecord(ev[5], st);
+  cudaStreamSynchronize(st);
+  if (stage_ms)
+    for (int i = 0; i < 5; ++i) cudaEventElapsedTime(&stage_ms[i], ev[i], ev[i + 1]);
+  tkm_path_free(path);
+  tkm_spectral_free(spec);
+  return rc2 != TKM_OK ? rc2 : rc;
+}

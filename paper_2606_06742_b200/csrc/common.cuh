@@ -1,0 +1,141 @@
+// common.cuh -- shared host/device helpers of libtkm (error handling, launch counting, PTX wrappers).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cstdarg>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <vector>
+
+#include "../../include/tkm.h"
+
+namespace tkm {
+
+// ---- thread-local error string + launch counter (tkm_last_error / tkm_launch_count) ----------
+char* err_buf();
+int set_error(int code, const char* fmt, ...);
+int64_t& launch_counter();
+inline void count_launch(int64_t k = 1) { launch_counter() += k; }
+
+#define TKM_CUDA(expr)                                                                       \
+  do {                                                                                       \
+    cudaError_t _e = (expr);                                                                 \
+    if (_e != cudaSuccess)                                                                   \
+      return ::tkm::set_error(_e == cudaErrorMemoryAllocation ? TKM_ENOMEM : TKM_ECUDA,      \
+                              "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(_e),        \
+                              __FILE__, __LINE__);                                           \
+  } while (0)
+
+#define TKM_LAUNCH_CHECK()                                                                   \
+  do {                                                                                       \
+    ::tkm::count_launch();                                                                   \
+    cudaError_t _e = cudaGetLastError();                                                     \
+    if (_e != cudaSuccess)                                                                   \
+      return ::tkm::set_error(TKM_ECUDA, "kernel launch failed: %s (%s:%d)",                 \
+                              cudaGetErrorString(_e), __FILE__, __LINE__);                   \
+  } while (0)
+
+#define TKM_TRY(expr)                 \
+  do {                                \
+    int _s = (expr);                  \
+    if (_s != TKM_OK) return _s;      \
+  } while (0)
+
+inline int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
+inline int64_t ceil_div(int64_t x, int64_t m) { return (x + m - 1) / m; }
+
+// RAII device buffer (cudaMalloc / cudaFree); zero-initialised on request.
+struct DevBuf {
+  void* p = nullptr;
+  size_t bytes = 0;
+  DevBuf() = default;
+  DevBuf(const DevBuf&) = delete;
+  DevBuf& operator=(const DevBuf&) = delete;
+  ~DevBuf() { release(); }
+  void release() {
+    if (p) cudaFree(p);
+    p = nullptr;
+    bytes = 0;
+  }
+  int alloc(size_t nbytes, bool zero, cudaStream_t st) {
+    release();
+    if (nbytes == 0) nbytes = 16;
+    cudaError_t e = cudaMalloc(&p, nbytes);
+    if (e != cudaSuccess) {
+      p = nullptr;
+      return set_error(TKM_ENOMEM, "cudaMalloc(%zu bytes) failed: %s", nbytes, cudaGetErrorString(e));
+    }
+    bytes = nbytes;
+    if (zero) {
+      e = cudaMemsetAsync(p, 0, nbytes, st);
+      if (e != cudaSuccess) return set_error(TKM_ECUDA, "cudaMemsetAsync failed: %s", cudaGetErrorString(e));
+    }
+    return TKM_OK;
+  }
+  template <class T>
+  T* as() const { return reinterpret_cast<T*>(p); }
+};
+
+// Pinned host buffer.
+struct PinBuf {
+  void* p = nullptr;
+  ~PinBuf() {
+    if (p) cudaFreeHost(p);
+  }
+  int alloc(size_t nbytes) {
+    if (p) cudaFreeHost(p);
+    p = nullptr;
+    cudaError_t e = cudaMallocHost(&p, nbytes ? nbytes : 16);
+    if (e != cudaSuccess) {
+      p = nullptr;
+      return set_error(TKM_ENOMEM, "cudaMallocHost(%zu) failed: %s", nbytes, cudaGetErrorString(e));
+    }
+    return TKM_OK;
+  }
+  template <class T>
+  T* as() const { return reinterpret_cast<T*>(p); }
+};
+
+int device_check();   // TKM_OK when a CUDA device of compute capability 10.x is current
+
+#ifdef __CUDACC__
+// ---- device-side PTX wrappers ------------------------------------------------------------------
+// 16-byte async copy; only the first `src_bytes` (0, 8 or 16) are read, the rest is zero-filled.
+__device__ __forceinline__ void cp_async_16(void* smem_dst, const void* gmem_src, int src_bytes) {
+  unsigned s = static_cast<unsigned>(__cvta_generic_to_shared(smem_dst));
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem_src), "r"(src_bytes));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() {
+  asm volatile("cp.async.wait_group %0;\n" ::"n"(N));
+}
+
+// D(8x8) += A(8x4, row) * B(4x8, col), FP64 tensor core (SASS: DMMA.8x8x4).
+__device__ __forceinline__ void dmma_884(double& c0, double& c1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+               : "+d"(c0), "+d"(c1)
+               : "d"(a), "d"(b));
+}
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+// Block-wide sum (all threads get the result); `red` holds >= 32 doubles of shared memory.
+__device__ __forceinline__ double block_sum(double v, double* red) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+  v = warp_sum(v);
+  __syncthreads();   // protect `red` from a previous use
+  if (lane == 0) red[w] = v;
+  __syncthreads();
+  double t = (lane < nw) ? red[lane] : 0.0;
+  t = warp_sum(t);
+  return t;
+}
+#endif  // __CUDACC__
+
+}  // namespace tkm

@@ -1,0 +1,51 @@
+// handles.cuh -- the two opaque handles of the C ABI (include/tkm.h) and internal entry points
+// shared between translation units.
+#pragma once
+
+#include <vector>
+
+#include "common.cuh"
+
+// K = U Lam U^T and what the sweep derives from it once (data D4/D7).
+struct tkm_spectral {
+  int64_t n = 0, r = 0;
+  int64_t ldr = 0;   // round_up(r, 16): leading dimension of every [.][r] array (zero padded)
+  int64_t ldn = 0;   // round_up(n, 16): leading dimension of every [.][n] array (zero padded)
+  tkm_dtype sweep_dt = TKM_F64;
+  tkm::DevBuf UL;    // [n][ldr] FP64   U * diag(Lam)   (Q operand of GEMM-A)
+  tkm::DevBuf Ut;    // [r][ldn] FP64   U^T             (Q operand of GEMM-B)
+  tkm::DevBuf lam;   // [ldr]    FP64   eigenvalues >= 0 (padding 0)
+  tkm::DevBuf u1;    // [ldr]    FP64   U^T 1            (padding 0)
+  double thin = 0.0; // n - ||u1||^2 for a thin U, exactly 0 for the full kernel (reading G1)
+  std::vector<double> h_lam, h_u1;
+  // FP32 sweep (3xTF32): TF32-rounded hi and lo parts of UL and Ut
+  tkm::DevBuf UL_hi, UL_lo, Ut_hi, Ut_lo;
+  // Nystrom (reading G11)
+  int64_t m = 0;
+  int64_t ldm = 0;
+  tkm::DevBuf lmap_t;             // [r][ldm]: gamma = lmap_t^T a  (landmark weights)
+  tkm::DevBuf d_landmark_idx;     // [m] int64
+  std::vector<int64_t> landmark_idx;
+};
+
+// The fitted columns of one grid (data D6).
+struct tkm_path {
+  const tkm_spectral* spec = nullptr;
+  int32_t L = 0, V = 0, T = 1, B = 0;
+  tkm_loss loss = TKM_LOSS_HINGE;
+  double smooth_final = 0.0;
+  std::vector<double> lambdas, taus;
+  tkm::DevBuf a;        // [B][ldr] FP64 spectral coordinates, one column of the batch per row
+  tkm::DevBuf beta0;    // [B]
+  tkm::DevBuf col_lam, col_tau, col_nc;   // [B] per-column lambda, tau, n_c
+  tkm::DevBuf col_v;    // [B] int32 held-out fold (V = none)
+  std::vector<double> h_beta0, h_kkt;
+  std::vector<int32_t> h_iters, h_flags;
+  int64_t total_col_iters = 0;
+};
+
+namespace tkm {
+// transpose.cu-style helpers living in spectral.cu
+int transpose_scale_f64(const double* src, int64_t lds, int64_t rows, int64_t cols, const double* row_scale,
+                        double* dst, int64_t ldd, cudaStream_t st);   // dst[c][r] = src[r][c] * row_scale[r]
+}  // namespace tkm

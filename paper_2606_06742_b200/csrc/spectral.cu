@@ -1,0 +1,282 @@
+// spectral.cu -- S2: one-time spectral setup K = U Lam U^T (Alg.1 l.3, 226; readings
+// G11 Nystrom, G16 eigenvalue clamp, G19 one decomposition shared by all folds).
+//
+// The eigendecomposition itself is cuSOLVER Dsyevd (allowed as setup by BASELINE.json north_star and
+// timed separately from the sweep).  Everything else -- transposes, scalings, u1 = U^T 1, and the
+// Nystrom products -- is this library's own kernels (the products use the DMMA GEMM of gemm_f64.cuh).
+#include <cusolverDn.h>
+
+#include <cmath>
+#include <new>
+
+#include "gemm_f64.cuh"
+#include "handles.cuh"
+
+namespace tkm {
+
+// dst[c][r] = src[r][c] * (row_scale ? row_scale[r] : 1): 32x32 shared-memory tile transpose.
+__global__ void transpose_scale_kernel(const double* __restrict__ src, int64_t lds, int rows, int cols,
+                                       const double* __restrict__ row_scale, double* __restrict__ dst,
+                                       int64_t ldd) {
+  __shared__ double tile[32][33];
+  const int r0 = blockIdx.y * 32, c0 = blockIdx.x * 32;
+  for (int i = threadIdx.y; i < 32; i += blockDim.y) {
+    const int r = r0 + i, c = c0 + threadIdx.x;
+    double v = 0.0;
+    if (r < rows && c < cols) v = src[(int64_t)r * lds + c] * (row_scale ? row_scale[r] : 1.0);
+    tile[i][threadIdx.x] = v;
+  }
+  __syncthreads();
+  for (int i = threadIdx.y; i < 32; i += blockDim.y) {
+    const int c = c0 + i, r = r0 + threadIdx.x;
+    if (r < rows && c < cols) dst[(int64_t)c * ldd + r] = tile[threadIdx.x][i];
+  }
+}
+
+int transpose_scale_f64(const double* src, int64_t lds, int64_t rows, int64_t cols, const double* row_scale,
+                        double* dst, int64_t ldd, cudaStream_t st) {
+  dim3 grid((unsigned)ceil_div(cols, 32), (unsigned)ceil_div(rows, 32));
+  transpose_scale_kernel<<<grid, dim3(32, 8), 0, st>>>(src, lds, (int)rows, (int)cols, row_scale, dst, ldd);
+  TKM_LAUNCH_CHECK();
+  return TKM_OK;
+}
+
+// rows[j][0..cols) *= scale[j]
+__global__ void row_scale_kernel(double* __restrict__ A, int64_t lda, int rows, int cols,
+                                 const double* __restrict__ scale) {
+  const int j = blockIdx.x;
+  const double s = scale[j];
+  for (int i = threadIdx.x; i < cols; i += blockDim.x) A[(int64_t)j * lda + i] *= s;
+}
+
+// out[j] = sum_i A[j][i]  (one CTA per row, fixed-order reduction => deterministic)
+__global__ void row_sum_kernel(const double* __restrict__ A, int64_t lda, int cols, double* __restrict__ out) {
+  __shared__ double red[32];
+  const int j = blockIdx.x;
+  double s = 0.0;
+  for (int i = threadIdx.x; i < cols; i += blockDim.x) s += A[(int64_t)j * lda + i];
+  s = block_sum(s, red);
+  if (threadIdx.x == 0) out[j] = s;
+}
+
+// v[i] = op(v[i]): 0 clamp to >= 0, 1 -> 1/sqrt(v), 2 -> sqrt(v)
+__global__ void vec_op_kernel(double* v, int n, int op) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const double x = v[i];
+  v[i] = op == 0 ? fmax(x, 0.0) : (op == 1 ? 1.0 / sqrt(x) : sqrt(x));
+}
+
+struct Solver {
+  cusolverDnHandle_t h = nullptr;
+  ~Solver() {
+    if (h) cusolverDnDestroy(h);
+  }
+};
+
+// In-place symmetric eigendecomposition of the n x n matrix in A (column-major, lda): on return
+// column j of A (= row j of the row-major view) is eigenvector j, W ascending.
+static int syevd_inplace(double* A, int64_t lda, int64_t n, double* W, cudaStream_t st) {
+  Solver sv;
+  if (cusolverDnCreate(&sv.h) != CUSOLVER_STATUS_SUCCESS) return set_error(TKM_ESOLVER, "cusolverDnCreate failed");
+  if (cusolverDnSetStream(sv.h, st) != CUSOLVER_STATUS_SUCCESS) return set_error(TKM_ESOLVER, "cusolverDnSetStream failed");
+  int lwork = 0;
+  cusolverStatus_t cs = cusolverDnDsyevd_bufferSize(sv.h, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER,
+                                                    (int)n, A, (int)lda, W, &lwork);
+  if (cs != CUSOLVER_STATUS_SUCCESS) return set_error(TKM_ESOLVER, "Dsyevd_bufferSize failed (%d)", (int)cs);
+  DevBuf work, info;
+  TKM_TRY(work.alloc((size_t)lwork * sizeof(double), false, st));
+  TKM_TRY(info.alloc(sizeof(int), true, st));
+  cs = cusolverDnDsyevd(sv.h, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER, (int)n, A, (int)lda, W,
+                        work.as<double>(), lwork, info.as<int>());
+  if (cs != CUSOLVER_STATUS_SUCCESS) return set_error(TKM_ESOLVER, "cusolverDnDsyevd failed (%d)", (int)cs);
+  int h_info = 0;
+  TKM_CUDA(cudaMemcpyAsync(&h_info, info.p, sizeof(int), cudaMemcpyDeviceToHost, st));
+  TKM_CUDA(cudaStreamSynchronize(st));
+  if (h_info != 0) return set_error(TKM_ESOLVER, "Dsyevd: info = %d", h_info);
+  return TKM_OK;
+}
+
+static int dgemm_nt(const double* P, int64_t ldp, const double* Q, int64_t ldq, double* Dt, int64_t ldd,
+                    int64_t N, int64_t M, int64_t K, cudaStream_t st) {
+  if ((ldp & 1) || (ldq & 1) || (ldd & 1) || ((uintptr_t)P & 15) || ((uintptr_t)Q & 15) || ((uintptr_t)Dt & 15))
+    return set_error(TKM_EINVAL, "dgemm_nt: operands must be 16-byte aligned with even leading dimensions");
+  GemmOperands g{P, ldp, Q, ldq, (int)N, (int)M, (int)K};
+  StoreEpi epi{Dt, ldd, 1.0};
+  return gemm_f64_dispatch(g, epi, st);
+}
+
+// Finish a handle whose Ut ([r][ldn], rows = orthonormal eigenvectors) and lam are in place.
+static int finish_spectral(tkm_spectral* s, cudaStream_t st) {
+  const int64_t n = s->n, r = s->r;
+  vec_op_kernel<<<(unsigned)ceil_div(r, 256), 256, 0, st>>>(s->lam.as<double>(), (int)r, 0);   // clamp (G16)
+  TKM_LAUNCH_CHECK();
+  row_sum_kernel<<<(unsigned)r, 256, 0, st>>>(s->Ut.as<double>(), s->ldn, (int)n, s->u1.as<double>());
+  TKM_LAUNCH_CHECK();
+  TKM_TRY(s->UL.alloc((size_t)n * s->ldr * sizeof(double), true, st));
+  TKM_TRY(transpose_scale_f64(s->Ut.as<double>(), s->ldn, r, n, s->lam.as<double>(), s->UL.as<double>(), s->ldr, st));
+  s->h_lam.resize(r);
+  s->h_u1.resize(r);
+  TKM_CUDA(cudaMemcpyAsync(s->h_lam.data(), s->lam.p, r * sizeof(double), cudaMemcpyDeviceToHost, st));
+  TKM_CUDA(cudaMemcpyAsync(s->h_u1.data(), s->u1.p, r * sizeof(double), cudaMemcpyDeviceToHost, st));
+  TKM_CUDA(cudaStreamSynchronize(st));
+  if (s->r == s->n) {
+    s->thin = 0.0;   // ||U^T 1||^2 = n exactly for an orthogonal U (reading G1)
+  } else {
+    long double acc = 0.0L;
+    for (int64_t i = 0; i < r; ++i) acc += (long double)s->h_u1[i] * s->h_u1[i];
+    s->thin = (double)((long double)n - acc);
+    if (s->thin < 0.0) s->thin = 0.0;
+  }
+  return TKM_OK;
+}
+
+static int setup_full(const double* K, int64_t n, int64_t ldk, tkm_spectral* s, cudaStream_t st) {
+  s->n = s->r = n;
+  s->ldn = s->ldr = round_up(n, 16);
+  TKM_TRY(s->Ut.alloc((size_t)n * s->ldn * sizeof(double), true, st));
+  TKM_TRY(s->lam.alloc((size_t)s->ldr * sizeof(double), true, st));
+  TKM_TRY(s->u1.alloc((size_t)s->ldr * sizeof(double), true, st));
+  TKM_CUDA(cudaMemcpy2DAsync(s->Ut.p, s->ldn * sizeof(double), K, ldk * sizeof(double), n * sizeof(double), n,
+                             cudaMemcpyDeviceToDevice, st));
+  TKM_TRY(syevd_inplace(s->Ut.as<double>(), s->ldn, n, s->lam.as<double>(), st));
+  return finish_spectral(s, st);
+}
+
+constexpr double NYS_RANK_TOL = 1e-12;
+
+static int setup_nystrom(int64_t n, const tkm_nystrom* ny, tkm_spectral* s, cudaStream_t st) {
+  const int64_t m = ny->m;
+  const int64_t ldm = round_up(m, 16);
+  s->n = n;
+  s->m = m;
+  s->ldm = ldm;
+  s->ldn = round_up(n, 16);
+  // 1. K_mm = W Theta W^T
+  DevBuf Wv, theta;
+  TKM_TRY(Wv.alloc((size_t)m * ldm * sizeof(double), true, st));
+  TKM_TRY(theta.alloc((size_t)ldm * sizeof(double), true, st));
+  TKM_CUDA(cudaMemcpy2DAsync(Wv.p, ldm * sizeof(double), ny->K_mm, ny->ld_mm * sizeof(double), m * sizeof(double), m,
+                             cudaMemcpyDeviceToDevice, st));
+  TKM_TRY(syevd_inplace(Wv.as<double>(), ldm, m, theta.as<double>(), st));
+  std::vector<double> h_theta(m);
+  TKM_CUDA(cudaMemcpyAsync(h_theta.data(), theta.p, m * sizeof(double), cudaMemcpyDeviceToHost, st));
+  TKM_CUDA(cudaStreamSynchronize(st));
+  int64_t k0 = 0;   // eigenvalues ascend: keep the suffix above the rank tolerance
+  while (k0 < m && !(h_theta[k0] > NYS_RANK_TOL * h_theta[m - 1])) ++k0;
+  const int64_t rp = m - k0;
+  if (rp <= 0) return set_error(TKM_ESOLVER, "nystrom: K_mm has no positive eigenvalue");
+  const int64_t ldrp = round_up(rp, 16);
+  double* Wts = Wv.as<double>() + k0 * ldm;   // [rp][ldm]; rows become w_k / sqrt(theta_k)
+  vec_op_kernel<<<(unsigned)ceil_div(rp, 256), 256, 0, st>>>(theta.as<double>() + k0, (int)rp, 1);
+  TKM_LAUNCH_CHECK();
+  row_scale_kernel<<<(unsigned)rp, 256, 0, st>>>(Wts, ldm, (int)rp, (int)m, theta.as<double>() + k0);
+  TKM_LAUNCH_CHECK();
+  // 2. Phi^T [rp][ldn] = Wts K_nm^T ; Phi [n][ldrp]
+  DevBuf PhiT, Phi;
+  TKM_TRY(PhiT.alloc((size_t)rp * s->ldn * sizeof(double), true, st));
+  TKM_TRY(Phi.alloc((size_t)n * ldrp * sizeof(double), true, st));
+  TKM_TRY(dgemm_nt(Wts, ldm, ny->K_nm, ny->ld_nm, PhiT.as<double>(), s->ldn, rp, n, m, st));
+  TKM_TRY(transpose_scale_f64(PhiT.as<double>(), s->ldn, rp, n, nullptr, Phi.as<double>(), ldrp, st));
+  // 3. G = Phi^T Phi = Q Lam Q^T
+  DevBuf G, lamv;
+  TKM_TRY(G.alloc((size_t)rp * ldrp * sizeof(double), true, st));
+  TKM_TRY(lamv.alloc((size_t)ldrp * sizeof(double), true, st));
+  TKM_TRY(dgemm_nt(PhiT.as<double>(), s->ldn, PhiT.as<double>(), s->ldn, G.as<double>(), ldrp, rp, rp, n, st));
+  TKM_TRY(syevd_inplace(G.as<double>(), ldrp, rp, lamv.as<double>(), st));
+  std::vector<double> h_l(rp);
+  TKM_CUDA(cudaMemcpyAsync(h_l.data(), lamv.p, rp * sizeof(double), cudaMemcpyDeviceToHost, st));
+  TKM_CUDA(cudaStreamSynchronize(st));
+  int64_t j0 = 0;
+  while (j0 < rp && !(h_l[j0] > NYS_RANK_TOL * h_l[rp - 1])) ++j0;
+  const int64_t r = rp - j0;
+  if (r <= 0) return set_error(TKM_ESOLVER, "nystrom: Phi^T Phi has no positive eigenvalue");
+  s->r = r;
+  s->ldr = round_up(r, 16);
+  const double* Qe = G.as<double>() + j0 * ldrp;   // [r][ldrp], rows = eigenvectors
+  // 4. U^T [r][ldn] = Lam^-1/2 Qe Phi^T
+  TKM_TRY(s->Ut.alloc((size_t)r * s->ldn * sizeof(double), true, st));
+  TKM_TRY(s->lam.alloc((size_t)s->ldr * sizeof(double), true, st));
+  TKM_TRY(s->u1.alloc((size_t)s->ldr * sizeof(double), true, st));
+  TKM_CUDA(cudaMemcpyAsync(s->lam.p, lamv.as<double>() + j0, r * sizeof(double), cudaMemcpyDeviceToDevice, st));
+  DevBuf isq;
+  TKM_TRY(isq.alloc((size_t)r * sizeof(double), false, st));
+  TKM_CUDA(cudaMemcpyAsync(isq.p, s->lam.p, r * sizeof(double), cudaMemcpyDeviceToDevice, st));
+  vec_op_kernel<<<(unsigned)ceil_div(r, 256), 256, 0, st>>>(isq.as<double>(), (int)r, 1);
+  TKM_LAUNCH_CHECK();
+  TKM_TRY(dgemm_nt(Qe, ldrp, Phi.as<double>(), ldrp, s->Ut.as<double>(), s->ldn, r, n, rp, st));
+  row_scale_kernel<<<(unsigned)r, 256, 0, st>>>(s->Ut.as<double>(), s->ldn, (int)r, (int)n, isq.as<double>());
+  TKM_LAUNCH_CHECK();
+  // 5. landmark map: lmap_t[j][l] = sqrt(Lam_j) sum_k Qe[j][k] Wts[k][l]
+  DevBuf WtsT;
+  TKM_TRY(WtsT.alloc((size_t)m * ldrp * sizeof(double), true, st));
+  TKM_TRY(transpose_scale_f64(Wts, ldm, rp, m, nullptr, WtsT.as<double>(), ldrp, st));
+  TKM_TRY(s->lmap_t.alloc((size_t)r * ldm * sizeof(double), true, st));
+  TKM_TRY(dgemm_nt(Qe, ldrp, WtsT.as<double>(), ldrp, s->lmap_t.as<double>(), ldm, r, m, rp, st));
+  TKM_CUDA(cudaMemcpyAsync(isq.p, s->lam.p, r * sizeof(double), cudaMemcpyDeviceToDevice, st));   // -> sqrt(Lam)
+  vec_op_kernel<<<(unsigned)ceil_div(r, 256), 256, 0, st>>>(isq.as<double>(), (int)r, 2);
+  TKM_LAUNCH_CHECK();
+  row_scale_kernel<<<(unsigned)r, 256, 0, st>>>(s->lmap_t.as<double>(), ldm, (int)r, (int)m, isq.as<double>());
+  TKM_LAUNCH_CHECK();
+  s->landmark_idx.assign(ny->landmark_idx, ny->landmark_idx + m);
+  TKM_TRY(s->d_landmark_idx.alloc((size_t)m * sizeof(int64_t), false, st));
+  TKM_CUDA(cudaMemcpyAsync(s->d_landmark_idx.p, s->landmark_idx.data(), m * sizeof(int64_t), cudaMemcpyHostToDevice, st));
+  TKM_TRY(finish_spectral(s, st));   // synchronises: the temporaries above may now be freed
+  return TKM_OK;
+}
+
+}  // namespace tkm
+
+extern "C" int tkm_spectral_setup(const void* K, int64_t n, int64_t ldk, const tkm_nystrom* ny,
+                                  tkm_dtype sweep_dt, tkm_spectral** out, void* stream) {
+  using namespace tkm;
+  if (!out) return set_error(TKM_EINVAL, "tkm_spectral_setup: out is NULL");
+  *out = nullptr;
+  if (n <= 1 || n > (1 << 30)) return set_error(TKM_EINVAL, "tkm_spectral_setup: n out of range");
+  if (sweep_dt != TKM_F64 && sweep_dt != TKM_F32) return set_error(TKM_EINVAL, "tkm_spectral_setup: bad sweep_dt");
+  if (!ny && (!K || ldk < n)) return set_error(TKM_EINVAL, "tkm_spectral_setup: K NULL or ldk < n");
+  if (ny && (!ny->K_nm || !ny->K_mm || ny->m < 1 || ny->m > n || ny->ld_nm < ny->m || ny->ld_mm < ny->m ||
+             !ny->landmark_idx))
+    return set_error(TKM_EINVAL, "tkm_spectral_setup: bad tkm_nystrom fields");
+  TKM_TRY(device_check());
+  cudaStream_t st = (cudaStream_t)stream;
+  tkm_spectral* s = new (std::nothrow) tkm_spectral();
+  if (!s) return set_error(TKM_ENOMEM, "out of host memory");
+  s->sweep_dt = sweep_dt;
+  int rc = ny ? setup_nystrom(n, ny, s, st) : setup_full((const double*)K, n, ldk, s, st);
+  if (rc == TKM_OK && sweep_dt == TKM_F32) rc = set_error(TKM_ENOTIMPL, "FP32 (3xTF32) sweep not built yet");
+  if (rc != TKM_OK) {
+    cudaStreamSynchronize(st);
+    delete s;
+    return rc;
+  }
+  *out = s;
+  return TKM_OK;
+}
+
+extern "C" void tkm_spectral_free(tkm_spectral* s) { delete s; }
+
+extern "C" int tkm_spectral_info(const tkm_spectral* s, int64_t* n, int64_t* r, double* lam, double* u1) {
+  using namespace tkm;
+  if (!s) return set_error(TKM_EINVAL, "tkm_spectral_info: NULL handle");
+  if (n) *n = s->n;
+  if (r) *r = s->r;
+  if (lam) memcpy(lam, s->h_lam.data(), s->r * sizeof(double));
+  if (u1) memcpy(u1, s->h_u1.data(), s->r * sizeof(double));
+  return TKM_OK;
+}
+
+extern "C" int tkm_spectral_get_u(const tkm_spectral* s, double* U_out, void* stream) {
+  using namespace tkm;
+  if (!s || !U_out) return set_error(TKM_EINVAL, "tkm_spectral_get_u: NULL argument");
+  return transpose_scale_f64(s->Ut.as<double>(), s->ldn, s->r, s->n, nullptr, U_out, s->r, (cudaStream_t)stream);
+}
+
+extern "C" int tkm_dgemm_nt(const double* P, int64_t ldp, const double* Q, int64_t ldq, double* Dt, int64_t ldd,
+                            int64_t N, int64_t M, int64_t K, void* stream) {
+  using namespace tkm;
+  if (!P || !Q || !Dt || N <= 0 || M <= 0 || K <= 0 || ldp < K || ldq < K || ldd < M)
+    return set_error(TKM_EINVAL, "tkm_dgemm_nt: bad arguments");
+  TKM_TRY(device_check());
+  return dgemm_nt(P, ldp, Q, ldq, Dt, ldd, N, M, K, (cudaStream_t)stream);
+}

@@ -1,0 +1,282 @@
+"""GPU parity tests: the CUDA path (through the C ABI of libtkm.so) against the FP64 oracle, element by
+element on the same seeded inputs.  Tolerances are BASELINE.json's: coefficients relative l2 <= 1e-10
+(FP64 path), CV loss per (lambda, fold) within 1e-5, selected lambda identical, fold assignments and
+predicted labels bit-exact.  Where several results are correct (U; beta0 of a degenerate column,
+reading G18) only what is unique is compared."""
+import numpy as np
+import pytest
+
+import oracle as o
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+COEF_TOL_F64 = 1e-10
+CV_TOL = 1e-5
+
+
+@pytest.fixture(scope="module")
+def tkm():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (no CPU fallback exists)")
+    import paper_2606_06742_b200 as t
+    t.lib()
+    return t
+
+
+def dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+# ------------------------------------------------------------------------------- S1 Gram
+@pytest.mark.parametrize("n,p", [(200, 10), (333, 7), (64, 1), (129, 50), (1, 3)])
+def test_gram_symmetric(tkm, n, p):
+    rng = np.random.default_rng(n + p)
+    X = rng.standard_normal((n, p))
+    sigma = 1.7 * np.sqrt(p)
+    K = tkm.tkm_gram(dev(X), sigma).cpu().numpy()
+    Ko = o.gram_rbf(X, sigma)
+    assert np.array_equal(K, K.T)                       # bit-exact symmetry
+    assert np.all(np.diag(K) == 1.0)
+    assert np.max(np.abs(K - Ko) / Ko) < 1e-13
+
+
+def test_gram_cross_and_strided(tkm):
+    import torch
+    rng = np.random.default_rng(5)
+    A, Bm = rng.standard_normal((150, 12)), rng.standard_normal((77, 12))
+    K = tkm.tkm_gram(dev(A), 2.0, dev(Bm)).cpu().numpy()
+    assert K.shape == (150, 77)
+    assert np.max(np.abs(K - o.gram_rbf(A, 2.0, Bm))) < 1e-14
+    wide = torch.zeros((150, 20), dtype=torch.float64, device="cuda")
+    wide[:, :12] = dev(A)
+    K2 = tkm.tkm_gram(wide[:, :12], 2.0).cpu().numpy()   # ldx = 20 > p
+    assert np.max(np.abs(K2 - o.gram_rbf(A, 2.0))) < 1e-14
+    Kf = tkm.tkm_gram(dev(A), 2.0, out_dtype=tkm.F32).cpu().numpy()
+    assert Kf.dtype == np.float32 and np.array_equal(Kf, o.gram_rbf(A, 2.0).astype(np.float32)) or \
+        np.max(np.abs(Kf - o.gram_rbf(A, 2.0))) < 1e-7
+    with pytest.raises(tkm.TkmError):
+        tkm.tkm_gram(dev(A), 0.0)
+
+
+# ------------------------------------------------------------------------------- DMMA GEMM
+@pytest.mark.parametrize("N,M,K", [(300, 2000, 2000), (37, 130, 70), (64, 64, 16), (1, 5, 3), (130, 257, 1001),
+                                   (600, 4096, 512)])
+def test_dgemm_nt(tkm, N, M, K):
+    rng = np.random.default_rng(N + M + K)
+    ldk = (K + 1) // 2 * 2
+    P = np.zeros((N, ldk))
+    Q = np.zeros((M, ldk))
+    P[:, :K] = rng.standard_normal((N, K))
+    Q[:, :K] = rng.standard_normal((M, K))
+    D = tkm.tkm_dgemm_nt(dev(P)[:, :K], dev(Q)[:, :K]).cpu().numpy()
+    ref = P[:, :K] @ Q[:, :K].T
+    assert np.max(np.abs(D - ref)) < 1e-13 * K
+
+
+# ------------------------------------------------------------------------------- S2 spectral setup
+def test_spectral_invariants(tkm):
+    w = wl.config0(n=333, p=6, seed=4)
+    Ko = o.gram_rbf(w.X, w.sigmas[0])
+    K = tkm.tkm_gram(dev(w.X), w.sigmas[0])
+    spec = tkm.tkm_spectral_setup(K)
+    assert (spec.n, spec.r) == (333, 333)
+    U = spec.U().cpu().numpy()
+    lam, u1 = spec.eigenvalues()
+    n = 333
+    assert np.max(np.abs(U.T @ U - np.eye(n))) < 1e-12 * n
+    assert np.max(np.abs((U * lam) @ U.T - Ko)) < 1e-12 * n
+    assert np.all(lam >= 0)
+    assert np.max(np.abs(np.sort(lam) - o.spectral_setup(Ko).lam)) < 1e-12 * n
+    assert np.max(np.abs(u1 - U.sum(axis=0))) < 1e-12
+
+
+# ------------------------------------------------------------------------------- S3-S10 full pipeline
+def _run_gpu(tkm, w, sigma, foldid, tol, maxit, **kw):
+    X, y = dev(w.X), dev(w.y)
+    K = tkm.tkm_gram(X, sigma)
+    spec = tkm.tkm_spectral_setup(K)
+    path = tkm.tkm_fit_path(spec, y, w.loss, w.lambdas, foldid, w.V, tol, maxit, smooth0=w.smooth0, eta=w.eta,
+                            rounds=w.rounds, taus=w.taus if len(w.taus) else None, **kw)
+    cv = tkm.tkm_exact_cv(path, y, foldid, w.T, w.L, w.V)
+    return X, y, spec, path, cv
+
+
+def _degenerate(w, spec_o, res, c):
+    """G18: hinge column whose training rows all sit on the linear piece with balanced labels."""
+    if w.loss != o.LOSS_HINGE:
+        return False
+    M = res.cols["M"][:, c] > 0
+    f = spec_o.U @ (spec_o.lam * res.a[:, c]) + res.beta0[c]
+    return bool(np.all((w.y * f)[M] <= 1 - res.smooth_final) and w.y[M].sum() == 0)
+
+
+def _compare_path(tkm, w, sigma, foldid, spec, path, cv, columns=None, coef_tol=COEF_TOL_F64):
+    Ko = o.gram_rbf(w.X, sigma)
+    spec_o = o.spectral_setup(Ko)
+    res = o.fit_path(spec_o, w.y, w.loss, w.lambdas, foldid, w.V, taus=w.taus, smooth0=w.smooth0, eta=w.eta,
+                     rounds=w.rounds, tol=1e-12, maxit=400000, columns=columns)
+    sel = np.arange(res.cols["B"]) if columns is None else np.asarray(columns)
+    assert res.flags[sel].sum() == 0
+    info = path.info()
+    assert info["flags"].sum() == 0, "GPU columns hit maxit"
+    U = spec.U().cpu().numpy()
+    a_gpu = path.a().cpu().numpy()
+    worst = 0.0
+    degenerate = set()
+    for c in sel:
+        alpha_o = spec_o.U @ res.a[:, c]
+        alpha_g = U @ a_gpu[c]
+        err = np.linalg.norm(alpha_g - alpha_o) / max(np.linalg.norm(alpha_o), 1e-300)
+        worst = max(worst, err)
+        assert err <= coef_tol, "column %d: relative l2 coefficient error %.3g" % (c, err)
+        if _degenerate(w, spec_o, res, c):
+            degenerate.add(int(c))
+            continue
+        assert abs(info["beta0"][c] - res.beta0[c]) <= coef_tol * max(1.0, abs(res.beta0[c])) * 10
+    return res, spec_o, worst, degenerate
+
+
+@pytest.mark.parametrize("name", ["cfg0", "logit_ragged", "kqr_ragged", "hinge_tiny"])
+def test_fit_path_and_exact_cv_parity(tkm, name):
+    if name == "cfg0":
+        w = wl.config0()                                       # BASELINE.json configs[0], full size
+    elif name == "logit_ragged":
+        w = wl.config2(n=333, p=9, L=7, V=3)
+    elif name == "kqr_ragged":
+        w = wl.config3(n=261, p=5, L=5, V=4, taus=(0.1, 0.5, 0.9))
+    else:
+        w = wl.config0(n=37, p=3, L=3, V=2, seed=8)
+    sigma = float(w.sigmas[0])
+    foldid = tkm.tkm_make_folds(w.n, w.V, w.fold_seed)
+    assert np.array_equal(foldid, o.make_folds(w.n, w.V, w.fold_seed))          # bit-exact folds
+    X, y, spec, path, cv = _run_gpu(tkm, w, sigma, foldid, 1e-11, 200000)
+    res, spec_o, worst, degenerate = _compare_path(tkm, w, sigma, foldid, spec, path, cv)
+    cv_o = o.exact_cv(spec_o, res, w.y, foldid, w.loss, w.taus)
+    cv_loss, cv_err, cv_mean, best = cv
+    T, L, V = w.T, w.L, w.V
+    for t in range(T):
+        for l in range(L):
+            for v in range(V):
+                if (t * (V + 1) + v) * L + l in degenerate:
+                    continue
+                assert abs(cv_loss[t, l, v] - cv_o[0][t, l, v]) <= CV_TOL
+                if w.loss != o.LOSS_QUANTILE:
+                    assert cv_err[t, l, v] == cv_o[1][t, l, v]
+                else:
+                    assert cv_err[t, l, v] == -1
+    if not degenerate:
+        assert np.max(np.abs(cv_mean - cv_o[2])) <= CV_TOL
+        assert np.array_equal(best, cv_o[3])                                     # selected lambda identical
+    # S10: coefficients and prediction with the selected lambda of variant 0
+    l_best = int(cv_o[3][0])
+    c = (0 * (V + 1) + V) * L + l_best
+    alpha_g, b0_g = tkm.tkm_path_coef(path, 0, l_best, V)
+    alpha_o = spec_o.U @ res.a[:, c]
+    assert np.linalg.norm(alpha_g.cpu().numpy() - alpha_o) <= COEF_TOL_F64 * np.linalg.norm(alpha_o)
+    Xn = wl.new_points(w, 203)
+    f_g, lab_g = tkm.tkm_predict(path, 0, l_best, X, dev(Xn), sigma)
+    f_o, lab_o = o.predict(w.X, alpha_o, res.beta0[c], sigma, Xn)
+    assert np.max(np.abs(f_g.cpu().numpy() - f_o)) <= 1e-9 * max(1.0, np.abs(f_o).max())
+    margin = np.min(np.abs(f_o))
+    if w.loss != o.LOSS_QUANTILE and margin > 1e-8:
+        assert np.array_equal(lab_g.cpu().numpy(), lab_o)                        # labels bit-exact
+
+
+def test_config1_full_size_sampled_columns(tkm):
+    """BASELINE.json configs[1] at full size (n=2000, p=50, 50 lambdas, 5 folds; one of the 5 sigmas), in
+    the launch configuration bench.py times.  The oracle fits a stated sample of columns one by one."""
+    w = wl.config1()
+    sigma = float(w.sigmas[2])
+    foldid = tkm.tkm_make_folds(w.n, w.V, w.fold_seed)
+    X, y, spec, path, cv = _run_gpu(tkm, w, sigma, foldid, 1e-11, 200000)
+    L, V = w.L, w.V
+    cols = [(0 * (V + 1) + v) * L + l for (v, l) in [(0, 0), (1, 17), (2, 30), (5, 24), (4, 40), (3, 49)]]
+    res, spec_o, worst, degenerate = _compare_path(tkm, w, sigma, foldid, spec, path, cv, columns=cols)
+    cv_loss = cv[0]
+    for c in cols:
+        v, l = (c // L) % (V + 1), c % L
+        if v == V or c in degenerate:
+            continue
+        rows = np.nonzero(foldid == v)[0]
+        f = spec_o.U[rows] @ (spec_o.lam * res.a[:, c]) + res.beta0[c]
+        want = np.mean(o.nominal_loss(w.loss, w.y[rows], f))
+        assert abs(cv_loss[0, l, v] - want) <= CV_TOL
+    # properties that hold at any size: every column converged, held-out alpha ~ 0, sum alpha = 0
+    info = path.info()
+    assert info["flags"].sum() == 0 and np.all(info["kkt"] <= 1e-11)
+    U = spec.U().cpu().numpy()
+    a_gpu = path.a().cpu().numpy()
+    for c in (3, 77, 160, 299):
+        v = (c // L) % (V + 1)
+        alpha = U @ a_gpu[c]
+        sc = np.abs(alpha).max()
+        assert abs(alpha.sum()) < 1e-8 * sc * w.n
+        if v < V:
+            assert np.abs(alpha[foldid == v]).max() < 1e-8 * sc
+
+
+def test_nystrom_parity(tkm):
+    w = wl.config4(n=700, p=8, m=96, L=5, V=3)
+    sigma = float(w.sigmas[0])
+    idx = wl.landmarks(w.n, w.m_landmarks, w.landmark_seed)
+    foldid = tkm.tkm_make_folds(w.n, w.V, w.fold_seed)
+    X, y = dev(w.X), dev(w.y)
+    Xl = X[dev(idx)]
+    K_nm = tkm.tkm_gram(X, sigma, Xl)
+    K_mm = tkm.tkm_gram(Xl, sigma)
+    spec = tkm.tkm_spectral_setup(nystrom=(K_nm, K_mm, idx))
+    spec_o = o.nystrom_setup(w.X, sigma, idx)
+    assert spec.r == spec_o.r
+    U = spec.U().cpu().numpy()
+    lam, _ = spec.eigenvalues()
+    Kt_o = (spec_o.U * spec_o.lam) @ spec_o.U.T
+    assert np.max(np.abs((U * lam) @ U.T - Kt_o)) < 1e-9
+    path = tkm.tkm_fit_path(spec, y, w.loss, w.lambdas, foldid, w.V, 1e-11, 200000, rounds=w.rounds)
+    res = o.fit_path(spec_o, w.y, w.loss, w.lambdas, foldid, w.V, rounds=w.rounds, tol=1e-12, maxit=400000)
+    a_gpu = path.a().cpu().numpy()
+    info = path.info()
+    for c in range(res.cols["B"]):
+        f_o = spec_o.U @ (spec_o.lam * res.a[:, c]) + res.beta0[c]
+        f_g = U @ (lam * a_gpu[c]) + info["beta0"][c]
+        assert np.max(np.abs(f_g - f_o)) < 1e-7 * max(1.0, np.abs(f_o).max())
+    cv = tkm.tkm_exact_cv(path, y, foldid, 1, w.L, w.V)
+    cv_o = o.exact_cv(spec_o, res, w.y, foldid, w.loss)
+    assert np.max(np.abs(cv[0] - cv_o[0])) <= CV_TOL and np.array_equal(cv[1], cv_o[1])
+    assert np.array_equal(cv[3], cv_o[3])
+    l = int(cv_o[3][0])
+    c = w.V * w.L + l
+    gam_g, b0 = tkm.tkm_path_coef(path, 0, l, w.V)
+    gam_o = o.nystrom_landmark_weights(spec_o, res.a[:, c])
+    Xn = wl.new_points(w, 64)
+    f_g, lab_g = tkm.tkm_predict(path, 0, l, X, dev(Xn), sigma)
+    f_o, lab_o = o.predict(w.X[idx], gam_o, res.beta0[c], sigma, Xn)
+    assert np.max(np.abs(f_g.cpu().numpy() - f_o)) < 1e-6
+    if np.min(np.abs(f_o)) > 1e-6:
+        assert np.array_equal(lab_g.cpu().numpy(), lab_o)
+
+
+# ------------------------------------------------------------------------------- edge cases / errors
+def test_error_paths_and_maxit_flag(tkm):
+    w = wl.config0(n=50, p=3, L=2, V=2, seed=3)
+    foldid = tkm.tkm_make_folds(w.n, w.V, 1)
+    X, y = dev(w.X), dev(w.y)
+    spec = tkm.tkm_spectral_setup(tkm.tkm_gram(X, float(w.sigmas[0])))
+    with pytest.raises(tkm.TkmError) as e:
+        tkm.tkm_fit_path(spec, y, w.loss, [1.0, -1.0], foldid, w.V, 1e-9, 100)
+    assert e.value.code == 1
+    bad = w.y.copy()
+    bad[3] = 0.5
+    with pytest.raises(tkm.TkmError):
+        tkm.tkm_fit_path(spec, dev(bad), w.loss, w.lambdas, foldid, w.V, 1e-9, 100)
+    with pytest.raises(tkm.TkmError):
+        tkm.tkm_fit_path(spec, y, w.loss, w.lambdas, np.zeros(w.n, dtype=np.int32), w.V, 1e-9, 100)
+    path = tkm.tkm_fit_path(spec, y, w.loss, w.lambdas, foldid, w.V, 1e-13, 3, rounds=2)
+    assert path.status == 5 and path.info()["flags"].sum() > 0            # TKM_ENOTCONV, results written
+    assert np.all(path.info()["iters"] <= 6)
+    # warm start from a converged path converges immediately
+    p1 = tkm.tkm_fit_path(spec, y, w.loss, w.lambdas, foldid, w.V, 1e-10, 100000, rounds=1, smooth0=0.125)
+    p2 = tkm.tkm_fit_path(spec, y, w.loss, w.lambdas, foldid, w.V, 1e-10, 100000, rounds=1, smooth0=0.125, warm=p1)
+    assert p2.info()["iters"].max() <= 2
