@@ -1,0 +1,348 @@
+#!/usr/bin/env python
+"""bench.py -- the driver's benchmark contract for libtkm.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--dtype f64]
+
+Metric (BASELINE.json): (lambda x fold) path fits per second on BASELINE.json configs[1]
+(smoothed-hinge kernel SVM, n=2000, p=50, 5 folds, 50 lambdas x 5 sigma values).  One STEP is one pass
+of the whole hot path over that workload: for each of the 5 bandwidths  S1 Gram -> S2 spectral setup
+-> S3-S8 sweep over all 50 x (5+1) columns -> S9 exact CV (and S10 coefficients in the e2e leg).
+`value` = columns fitted per second by the whole job, X and y resident in HBM before the timed
+region; `e2e` = the same through tkm_train_tune_host from pinned HOST buffers.
+
+N > 1 (torchrun): the path has no exchange step -- every rank runs the same-size workload on its own
+seeded data set (independent problems, "weak" scaling); the only communication is the barrier and the
+max-over-ranks of the device time.
+
+`--impl reference` times the FP64 CPU oracle (oracle/, test infrastructure) on a bounded sample of
+the same workload on the host cores; rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads as wl  # noqa: E402
+
+METRIC = "lambda_x_fold_path_fits_per_s"
+UNIT = "fits/s"
+STOP_TOL = {"f64": 1e-12, "f32": 1e-6}
+MAXIT = 200000
+# nominal dense tensor ratios to bf16 (B200_PROFILING.md / B300_MICROARCH.md tables): FP64 45 TF,
+# TF32 1125 TF, bf16 2250 TF.  3xTF32 does three MMAs per useful one.
+NOMINAL_RATIO = {"f64": 45.0 / 2250.0, "f32": (1125.0 / 2250.0) / 3.0}
+# dram bytes per launch of the dominant kernel from the committed ncu --set full capture
+# (profiles/): filled in by hand after each capture, None until one exists.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+# columns of the bounded CPU sample: all V+1 hold-out settings x these lambda indices, one sigma
+CPU_SAMPLE_LAMBDA_IDX = (0, 12, 24, 36, 49)
+CPU_SAMPLE_SIGMA_IDX = 2
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        d = json.load(open(path))
+        return dict(hbm=d["hbm_gbs"], bf16_burst=d["bf16_tflops"], bf16_sus=d["bf16_tflops_sustained"],
+                    src="measured")
+    return dict(hbm=6650.0, bf16_burst=1590.0, bf16_sus=1400.0, src="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.lines.append(ln.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+                pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nme, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ----------------------------------------------------------------------------------------- oracle arm
+def oracle_sample_step(w, want_all=False):
+    """One bounded sample of the workload on the CPU oracle: one sigma, 5 lambdas x (V+1) columns,
+    Gram + eigh + path + exact CV.  Returns (#columns fitted, seconds)."""
+    import oracle as o
+    t0 = time.perf_counter()
+    sigma = float(w.sigmas[CPU_SAMPLE_SIGMA_IDX])
+    foldid = o.make_folds(w.n, w.V, w.fold_seed)
+    K = o.gram_rbf(w.X, sigma)
+    spec = o.spectral_setup(K)
+    L, V = w.L, w.V
+    cols = [v * L + l for v in range(V + 1) for l in CPU_SAMPLE_LAMBDA_IDX if l < L]
+    res = o.fit_path(spec, w.y, w.loss, w.lambdas, foldid, V, taus=w.taus, smooth0=w.smooth0, eta=w.eta,
+                     rounds=w.rounds, tol=STOP_TOL["f64"], maxit=MAXIT, columns=cols)
+    o.exact_cv(spec, res, w.y, foldid, w.loss, w.taus)
+    return len(cols), time.perf_counter() - t0, int(res.iters.sum())
+
+
+def blas_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        return max([p.get("num_threads", 1) for p in threadpool_info()] or [1])
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def run_reference(args, w, rank):
+    if rank != 0:
+        return
+    for _ in range(args.warmup):
+        oracle_sample_step(w)
+    t0 = time.perf_counter()
+    fits = 0
+    for _ in range(args.steps):
+        c, _, _ = oracle_sample_step(w)
+        fits += c
+    dt = time.perf_counter() - t0
+    val = fits / dt
+    sample = ("sigma index %d, lambda indices %s x %d hold-out settings = %d of %d columns per step, "
+              "full n; Gram + eigh + path + exact CV" % (CPU_SAMPLE_SIGMA_IDX, list(CPU_SAMPLE_LAMBDA_IDX),
+                                                        w.V + 1, fits // max(args.steps, 1), w.B * len(w.sigmas)))
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": workload_config(w, "f64"),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def workload_config(w, dtype):
+    return {"workload": "BASELINE.json configs[1]: smoothed-hinge kernel SVM, n=%d, p=%d, %d folds, %d lambdas "
+                        "1e2..1e-5 x %d sigma (median x {0.25,0.5,1,2,4}), delta 1 -> 1/512 in %d rounds, %s"
+                        % (w.n, w.p, w.V, w.L, len(w.sigmas), w.rounds, dtype),
+            "n": w.n, "p": w.p, "folds": w.V, "lambdas": w.L, "sigmas": len(w.sigmas),
+            "columns_per_step": w.B * len(w.sigmas), "stop_tol": STOP_TOL[dtype], "maxit": MAXIT,
+            "l2": "flushed between steps (256 MiB memset)", "parallelism": "independent replicas, no collective"}
+
+
+# ----------------------------------------------------------------------------------------- CUDA arm
+def run_ours(args, w, rank, world):
+    import torch
+    import paper_2606_06742_b200 as tkm
+    tkm.lib()   # raises if libtkm.so is missing: there is no fallback
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (libtkm has no CPU fallback)")
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dt = args.dtype
+    sweep_dt = tkm.F64 if dt == "f64" else tkm.F32
+    tol = STOP_TOL[dt]
+    foldid = tkm.tkm_make_folds(w.n, w.V, w.fold_seed)
+    X = torch.from_numpy(w.X).cuda()
+    y = torch.from_numpy(w.y).cuda()
+    Xh = torch.from_numpy(w.X).pin_memory()
+    yh = torch.from_numpy(w.y).pin_memory()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    prof = dict(ms=np.zeros(2), flops=0.0, samples=0, col_iters=0)
+    stage = np.zeros(4)
+
+    def ev():
+        e = torch.cuda.Event(enable_timing=True)
+        e.record()
+        return e
+
+    def step_device(collect):
+        flush.zero_()
+        best = []
+        for sigma in w.sigmas:
+            e0 = ev()
+            K = tkm.tkm_gram(X, float(sigma))
+            e1 = ev()
+            spec = tkm.tkm_spectral_setup(K, sweep_dtype=sweep_dt)
+            del K
+            e2 = ev()
+            path = tkm.tkm_fit_path(spec, y, w.loss, w.lambdas, foldid, w.V, tol, MAXIT, smooth0=w.smooth0,
+                                    eta=w.eta, rounds=w.rounds, profile=True)
+            e3 = ev()
+            cv = tkm.tkm_exact_cv(path, y, foldid, w.T, w.L, w.V)
+            e4 = ev()
+            best.append(int(cv[3][0]))
+            if collect:
+                e4.synchronize()
+                for i, (a, b) in enumerate(((e0, e1), (e1, e2), (e2, e3), (e3, e4))):
+                    stage[i] += a.elapsed_time(b)
+                pr = path.profile()
+                prof["ms"] += pr["gemm_ms"]
+                prof["flops"] += pr["gemm_flops"]
+                prof["samples"] += pr["samples"]
+                prof["col_iters"] += path.total_col_iters
+                if path.status != 0:
+                    raise RuntimeError("columns hit maxit: the timed work is not the stated work")
+            path.close()
+            spec.close()
+        return best
+
+    def step_e2e():
+        flush.zero_()
+        nb_in = nb_out = 0
+        for sigma in w.sigmas:
+            r = tkm.tkm_train_tune_host(Xh.numpy(), yh.numpy(), float(sigma), w.loss, w.lambdas, foldid, w.V, tol,
+                                        MAXIT, smooth0=w.smooth0, eta=w.eta, rounds=w.rounds, sweep_dtype=sweep_dt)
+            nb_in += Xh.numel() * 8 + yh.numel() * 8
+            nb_out += r["cv_loss"].nbytes + r["cv_err"].nbytes + r["cv_mean"].nbytes + r["best_l"].nbytes + \
+                r["alpha"].nbytes + 8
+        return nb_in, nb_out
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(ms):
+        if dist is None:
+            return ms
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    for _ in range(args.warmup):
+        step_device(False)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    barrier()
+    tkm.tkm_launch_count_reset()
+    s_ev = ev()
+    for _ in range(args.steps):
+        step_device(True)
+    e_ev = ev()
+    barrier()
+    launches = tkm.tkm_launch_count()
+    ms_total = max_over_ranks(s_ev.elapsed_time(e_ev))
+    clocks = sampler.stop() if rank == 0 else None
+
+    # e2e leg: host buffers -> tkm_train_tune_host -> host results
+    step_e2e()
+    barrier()
+    s_ev = ev()
+    for _ in range(args.steps):
+        nb_in, nb_out = step_e2e()
+    e_ev = ev()
+    barrier()
+    ms_e2e = max_over_ranks(s_ev.elapsed_time(e_ev))
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+    fits_per_step = w.B * len(w.sigmas)
+    ms_per_step = ms_total / args.steps
+    value = world * fits_per_step / (ms_per_step / 1e3)
+    pk = peaks()
+    peak_tf = pk["bf16_sus"] * NOMINAL_RATIO[dt]
+    gemm_ms = float(prof["ms"].sum())
+    achieved = (2.0 * prof["flops"] / 1e12) / (gemm_ms / 1e3) if gemm_ms > 0 else 0.0
+    roofline = {"bound": "tensor", "kernel": "gemm_%s_nt_kernel (GEMM-A loss epilogue + GEMM-B spectral epilogue)" % dt,
+                "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved / peak_tf,
+                "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
+                "peak_source": "%s bf16 sustained %.1f TF/s x nominal %s/bf16 ratio %.4f" %
+                               (pk["src"], pk["bf16_sus"], dt, NOMINAL_RATIO[dt]),
+                "sampled_launches": int(2 * prof["samples"]),
+                "avg_launch_ms": gemm_ms / max(1, 2 * prof["samples"]),
+                "avg_flops_per_launch": prof["flops"] / max(1, prof["samples"]),
+                "gemm_a_ms": float(prof["ms"][0]), "gemm_b_ms": float(prof["ms"][1])}
+    sweep_s = stage[2] / 1e3
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": dt, "data": "synthetic", "config": workload_config(w, dt),
+            "stages_ms_per_step": {"gram": stage[0] / args.steps, "eig_setup": stage[1] / args.steps,
+                                   "sweep": stage[2] / args.steps, "exact_cv": stage[3] / args.steps},
+            "exact_cv_ms_per_grid": stage[3] / args.steps / len(w.sigmas),
+            "fits_per_s_sweep_only": args.steps * fits_per_step / sweep_s,
+            "col_iters_per_step": prof["col_iters"] / args.steps,
+            "sweep_useful_tflops": 4.0 * w.n * w.n * prof["col_iters"] / sweep_s / 1e12,
+            "gram_gbs": len(w.sigmas) * w.n * w.n * 8 / (stage[0] / args.steps / 1e3) / 1e9,
+            "roofline": roofline, "clocks": clocks, "gpu_launches": int(launches),
+            "e2e": {"value": world * fits_per_step / (ms_e2e / args.steps / 1e3), "unit": UNIT,
+                    "h2d_bytes_per_step": int(nb_in), "d2h_bytes_per_step": int(nb_out),
+                    "ms_per_step": ms_e2e / args.steps}}
+    if world == 1:
+        ncol, secs, its = oracle_sample_step(w)
+        line["cpu_baseline"] = {"value": ncol / secs, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
+                                "sample": "sigma index %d, lambda indices %s x %d hold-out settings = %d of %d columns, "
+                                          "full n, Gram + eigh + path + exact CV, %.1f s, %d column-iterations"
+                                          % (CPU_SAMPLE_SIGMA_IDX, list(CPU_SAMPLE_LAMBDA_IDX), w.V + 1, ncol,
+                                             fits_per_step, secs, its)}
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    w = wl.config1(seed=1001 + (rank if args.impl == "ours" else 0))
+    if args.impl == "reference":
+        run_reference(args, w, rank)
+    else:
+        run_ours(args, w, rank, world)
+
+
+if __name__ == "__main__":
+    main()

@@ -65,6 +65,8 @@ typedef struct {
   int32_t restart;    /* 1: gradient restart of the Nesterov sequence (default), 0: plain     */
   int32_t check_every;/* iterations between host convergence polls; <= 0 => library default   */
   double warm_tol;    /* tolerance of rounds 0..R-2 (warm starts only); <= 0 => same as tol   */
+  int32_t profile;    /* 1: time the two contractions of the first iteration after every poll */
+                      /* with CUDA events (read with tkm_path_profile); 0: no events          */
 } tkm_loss_opts;
 
 /* Nystrom inputs for tkm_spectral_setup (reading G11). */
@@ -124,6 +126,11 @@ void tkm_path_free(tkm_path* p);
  * beta0[B]; total_col_iters = sum of iters (the unit of the roofline). */
 int tkm_path_info(const tkm_path* p, int32_t* B, int64_t* r, int32_t* iters, double* kkt,
                   int32_t* flags, double* beta0, int64_t* total_col_iters);
+/* Sampled kernel timings of the sweep (only when tkm_loss_opts.profile was 1), all [host]:
+ * gemm_ms[2] = summed CUDA-event durations of the sampled GEMM-A and GEMM-B launches,
+ * gemm_flops = sum over the samples of 2 n r (live columns) -- the algorithmic flops of ONE of the
+ * two contractions (4 n r flops per column-iteration), samples = their number. */
+int tkm_path_profile(const tkm_path* p, double* gemm_ms, double* gemm_flops, int64_t* samples);
 /* Spectral coordinates of all columns: [dev] a_out, B x r FP64 row-major (ld = r). */
 int tkm_path_get_a(const tkm_path* p, double* a_out, void* stream);
 

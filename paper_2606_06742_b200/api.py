@@ -13,7 +13,7 @@ TKM_OK, TKM_ENOTCONV = 0, 5
 
 EXPORTED_SYMBOLS = [
     "tkm_gram", "tkm_spectral_setup", "tkm_spectral_free", "tkm_spectral_info", "tkm_spectral_get_u",
-    "tkm_fit_path", "tkm_path_free", "tkm_path_info", "tkm_path_get_a", "tkm_exact_cv", "tkm_path_coef",
+    "tkm_fit_path", "tkm_path_free", "tkm_path_info", "tkm_path_profile", "tkm_path_get_a", "tkm_exact_cv", "tkm_path_coef",
     "tkm_predict", "tkm_train_tune_host", "tkm_make_folds", "tkm_launch_count", "tkm_launch_count_reset",
     "tkm_dgemm_nt", "tkm_version", "tkm_last_error",
 ]
@@ -28,7 +28,7 @@ class TkmError(RuntimeError):
 class _LossOpts(C.Structure):
     _fields_ = [("smooth0", C.c_double), ("eta", C.c_double), ("rounds", C.c_int32), ("T", C.c_int32),
                 ("taus", C.POINTER(C.c_double)), ("restart", C.c_int32), ("check_every", C.c_int32),
-                ("warm_tol", C.c_double)]
+                ("warm_tol", C.c_double), ("profile", C.c_int32)]
 
 
 class _Nystrom(C.Structure):
@@ -65,6 +65,7 @@ def lib():
     L.tkm_path_free.argtypes = [vp]
     L.tkm_path_free.restype = None
     L.tkm_path_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i64), vp, vp, vp, vp, C.POINTER(i64)]
+    L.tkm_path_profile.argtypes = [vp, vp, C.POINTER(dbl), C.POINTER(i64)]
     L.tkm_path_get_a.argtypes = [vp, vp, vp]
     L.tkm_exact_cv.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
     L.tkm_path_coef.argtypes = [vp, i32, i32, i32, vp, C.POINTER(dbl), vp]
@@ -221,6 +222,12 @@ class Path:
         _check(lib().tkm_path_info(self._h, None, None, _ptr(iters), _ptr(kkt), _ptr(flags), _ptr(beta0), None))
         return dict(iters=iters, kkt=kkt, flags=flags, beta0=beta0)
 
+    def profile(self):
+        ms = np.zeros(2)
+        fl, ns = C.c_double(), C.c_int64()
+        _check(lib().tkm_path_profile(self._h, _ptr(ms), C.byref(fl), C.byref(ns)))
+        return dict(gemm_ms=ms, gemm_flops=fl.value, samples=ns.value)
+
     def a(self, stream=None):
         import torch
         out = torch.empty((self.B, self.r), device="cuda", dtype=torch.float64)
@@ -239,21 +246,21 @@ class Path:
             pass
 
 
-def _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol):
+def _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, profile=False):
     taus_arr = _host(taus if taus is not None else [], np.float64)
     o = _LossOpts(float(smooth0), float(eta), int(rounds), int(len(taus_arr)),
                   taus_arr.ctypes.data_as(C.POINTER(C.c_double)) if len(taus_arr) else None,
-                  int(bool(restart)), int(check_every), float(warm_tol))
+                  int(bool(restart)), int(check_every), float(warm_tol), int(bool(profile)))
     return o, taus_arr
 
 
 def tkm_fit_path(spec: Spectral, y, loss: int, lambdas, foldid, V: int, tol: float, maxit: int,
                  smooth0=1.0, eta=0.125, rounds=4, taus=None, restart=True, check_every=0, warm_tol=0.0,
-                 warm: Path | None = None, stream=None) -> Path:
+                 warm: Path | None = None, profile=False, stream=None) -> Path:
     y = _dev_f64(y, "y")
     lam = _host(lambdas, np.float64)
     fid = _host(foldid, np.int32)
-    o, keep = _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol)
+    o, keep = _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, profile)
     h = C.c_void_p()
     rc = lib().tkm_fit_path(spec._h, y.data_ptr(), loss, C.byref(o), _ptr(lam), len(lam), _ptr(fid), V,
                             float(tol), int(maxit), warm._h if warm is not None else None, C.byref(h),

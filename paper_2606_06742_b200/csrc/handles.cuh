@@ -42,6 +42,10 @@ struct tkm_path {
   std::vector<double> h_beta0, h_kkt;
   std::vector<int32_t> h_iters, h_flags;
   int64_t total_col_iters = 0;
+  // sampled CUDA-event timings of the two contractions (tkm_loss_opts.profile)
+  double prof_gemm_ms[2] = {0.0, 0.0};   // GEMM-A, GEMM-B: sum over the sampled launches
+  double prof_gemm_flops = 0.0;          // sum over the samples of 2 n r (live columns), per GEMM
+  int64_t prof_gemm_samples = 0;
 };
 
 namespace tkm {

@@ -438,6 +438,18 @@ extern "C" int tkm_fit_path(const tkm_spectral* s, const void* y, tkm_loss loss,
 
   const int check_every = opts->check_every > 0 ? opts->check_every : 16;
   const int restart = opts->restart ? 1 : 0;
+  // optional sampling of the two contractions with CUDA events: the first iteration after every
+  // poll (all `nslots` columns are live there), read back at the next poll (bench.py `roofline`)
+  cudaEvent_t pev[3] = {nullptr, nullptr, nullptr};
+  struct PevGuard {
+    cudaEvent_t* e;
+    ~PevGuard() {
+      for (int i = 0; i < 3; ++i)
+        if (e[i]) cudaEventDestroy(e[i]);
+    }
+  } pev_guard{pev};
+  if (opts->profile)
+    for (auto& e : pev) TKM_CUDA(cudaEventCreate(&e));
   double smooth = opts->smooth0;
   for (int rnd = 0; rnd < rounds; ++rnd) {
     if (loss != TKM_LOSS_LOGISTIC && rnd > 0) smooth *= opts->eta;   // PAPER.md:220 (Alg.1 l.22)
@@ -456,16 +468,20 @@ extern "C" int tkm_fit_path(const tkm_spectral* s, const void* y, tkm_loss loss,
     while (nslots > 0) {
       const int steps = std::max(1, std::min(check_every, maxit - it));
       for (int k = 0; k < steps; ++k) {
+        const bool sample = opts->profile && k == 0;
+        if (sample) TKM_CUDA(cudaEventRecord(pev[0], st));
         GemmOperands ga{Abar.as<double>(), ldr, s->UL.as<double>(), ldr, nslots, (int)n, (int)r};
         LossEpi le{(const double*)y, d_fold.as<int32_t>(), col_of_slot.as<int32_t>(), bbar.as<double>(),
                    p->col_nc.as<double>(), p->col_tau.as<double>(), p->col_v.as<int32_t>(), (int)loss, smooth,
                    Zt.as<double>(), ldn, gpart.as<double>(), ldpart};
         TKM_TRY(gemm_f64_dispatch(ga, le, st));
+        if (sample) TKM_CUDA(cudaEventRecord(pev[1], st));
         GemmOperands gb{Zt.as<double>(), ldn, s->Ut.as<double>(), ldn, nslots, (int)r, (int)n};
         SpecEpi se{s->lam.as<double>(), s->u1.as<double>(), col_of_slot.as<int32_t>(), p->col_lam.as<double>(),
                    col_c.as<double>(), Abar.as<double>(), ldr, Rho.as<double>(), qpart.as<double>(),
                    r2part.as<double>(), ldpart};
         TKM_TRY(gemm_f64_dispatch(gb, se, st));
+        if (sample) TKM_CUDA(cudaEventRecord(pev[2], st));
         UpdateArgs ua{(int)r, (int)n, (int)ceil_div(n, gemm_f64_tile_bm(nslots, n)),
                       (int)ceil_div(r, gemm_f64_tile_bm(nslots, r)), restart, maxit, ldr, ldpart, rtol,
                       s->lam.as<double>(), s->u1.as<double>(), col_of_slot.as<int32_t>(), p->col_lam.as<double>(),
@@ -480,6 +496,15 @@ extern "C" int tkm_fit_path(const tkm_spectral* s, const void* y, tkm_loss loss,
       it += steps;
       TKM_CUDA(cudaMemcpyAsync(h_done.p, done.p, (size_t)B * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
       TKM_CUDA(cudaStreamSynchronize(st));
+      if (opts->profile) {
+        float ma = 0.f, mb = 0.f;
+        TKM_CUDA(cudaEventElapsedTime(&ma, pev[0], pev[1]));
+        TKM_CUDA(cudaEventElapsedTime(&mb, pev[1], pev[2]));
+        p->prof_gemm_ms[0] += ma;
+        p->prof_gemm_ms[1] += mb;
+        p->prof_gemm_flops += 2.0 * (double)nslots * (double)n * (double)r;   // per GEMM
+        p->prof_gemm_samples += 1;
+      }
       const int32_t* hd = h_done.as<int32_t>();
       // finished slots are copied to the result rows, then holes are filled from the tail
       int32_t* src = h_idx.as<int32_t>();
@@ -563,6 +588,17 @@ extern "C" int tkm_path_info(const tkm_path* p, int32_t* B, int64_t* r, int32_t*
   if (flags) memcpy(flags, p->h_flags.data(), p->B * sizeof(int32_t));
   if (beta0) memcpy(beta0, p->h_beta0.data(), p->B * sizeof(double));
   if (total_col_iters) *total_col_iters = p->total_col_iters;
+  return TKM_OK;
+}
+
+extern "C" int tkm_path_profile(const tkm_path* p, double* gemm_ms, double* gemm_flops, int64_t* samples) {
+  if (!p) return set_error(TKM_EINVAL, "tkm_path_profile: NULL handle");
+  if (gemm_ms) {
+    gemm_ms[0] = p->prof_gemm_ms[0];
+    gemm_ms[1] = p->prof_gemm_ms[1];
+  }
+  if (gemm_flops) *gemm_flops = p->prof_gemm_flops;
+  if (samples) *samples = p->prof_gemm_samples;
   return TKM_OK;
 }
 

@@ -12,6 +12,8 @@ import workloads as wl
 pytestmark = pytest.mark.gpu
 
 COEF_TOL_F64 = 1e-10
+STOP_TOL = 1e-12   # stop tolerance on BOTH sides: coefficient error ~ 30 x tol; 1e-13 is below the FP64
+                   # rounding floor of the residual for small lambda
 CV_TOL = 1e-5
 
 
@@ -117,7 +119,7 @@ def _compare_path(tkm, w, sigma, foldid, spec, path, cv, columns=None, coef_tol=
     Ko = o.gram_rbf(w.X, sigma)
     spec_o = o.spectral_setup(Ko)
     res = o.fit_path(spec_o, w.y, w.loss, w.lambdas, foldid, w.V, taus=w.taus, smooth0=w.smooth0, eta=w.eta,
-                     rounds=w.rounds, tol=1e-12, maxit=400000, columns=columns)
+                     rounds=w.rounds, tol=STOP_TOL, maxit=400000, columns=columns)
     sel = np.arange(res.cols["B"]) if columns is None else np.asarray(columns)
     assert res.flags[sel].sum() == 0
     info = path.info()
@@ -152,7 +154,7 @@ def test_fit_path_and_exact_cv_parity(tkm, name):
     sigma = float(w.sigmas[0])
     foldid = tkm.tkm_make_folds(w.n, w.V, w.fold_seed)
     assert np.array_equal(foldid, o.make_folds(w.n, w.V, w.fold_seed))          # bit-exact folds
-    X, y, spec, path, cv = _run_gpu(tkm, w, sigma, foldid, 1e-11, 200000)
+    X, y, spec, path, cv = _run_gpu(tkm, w, sigma, foldid, STOP_TOL, 200000)
     res, spec_o, worst, degenerate = _compare_path(tkm, w, sigma, foldid, spec, path, cv)
     cv_o = o.exact_cv(spec_o, res, w.y, foldid, w.loss, w.taus)
     cv_loss, cv_err, cv_mean, best = cv
@@ -191,7 +193,7 @@ def test_config1_full_size_sampled_columns(tkm):
     w = wl.config1()
     sigma = float(w.sigmas[2])
     foldid = tkm.tkm_make_folds(w.n, w.V, w.fold_seed)
-    X, y, spec, path, cv = _run_gpu(tkm, w, sigma, foldid, 1e-11, 200000)
+    X, y, spec, path, cv = _run_gpu(tkm, w, sigma, foldid, STOP_TOL, 200000)
     L, V = w.L, w.V
     cols = [(0 * (V + 1) + v) * L + l for (v, l) in [(0, 0), (1, 17), (2, 30), (5, 24), (4, 40), (3, 49)]]
     res, spec_o, worst, degenerate = _compare_path(tkm, w, sigma, foldid, spec, path, cv, columns=cols)
@@ -206,7 +208,7 @@ def test_config1_full_size_sampled_columns(tkm):
         assert abs(cv_loss[0, l, v] - want) <= CV_TOL
     # properties that hold at any size: every column converged, held-out alpha ~ 0, sum alpha = 0
     info = path.info()
-    assert info["flags"].sum() == 0 and np.all(info["kkt"] <= 1e-11)
+    assert info["flags"].sum() == 0 and np.all(info["kkt"] <= STOP_TOL)
     U = spec.U().cpu().numpy()
     a_gpu = path.a().cpu().numpy()
     for c in (3, 77, 160, 299):
@@ -234,8 +236,8 @@ def test_nystrom_parity(tkm):
     lam, _ = spec.eigenvalues()
     Kt_o = (spec_o.U * spec_o.lam) @ spec_o.U.T
     assert np.max(np.abs((U * lam) @ U.T - Kt_o)) < 1e-9
-    path = tkm.tkm_fit_path(spec, y, w.loss, w.lambdas, foldid, w.V, 1e-11, 200000, rounds=w.rounds)
-    res = o.fit_path(spec_o, w.y, w.loss, w.lambdas, foldid, w.V, rounds=w.rounds, tol=1e-12, maxit=400000)
+    path = tkm.tkm_fit_path(spec, y, w.loss, w.lambdas, foldid, w.V, STOP_TOL, 200000, rounds=w.rounds)
+    res = o.fit_path(spec_o, w.y, w.loss, w.lambdas, foldid, w.V, rounds=w.rounds, tol=STOP_TOL, maxit=400000)
     a_gpu = path.a().cpu().numpy()
     info = path.info()
     for c in range(res.cols["B"]):
