@@ -120,6 +120,17 @@ int tkm_spectral_get_u(const tkm_spectral* s, double* U_out, void* stream);
 int tkm_fit_path(const tkm_spectral* s, const void* y, tkm_loss loss, const tkm_loss_opts* opts,
                  const double* lambdas, int32_t L, const int32_t* foldid, int32_t V,
                  double tol, int32_t maxit, const tkm_path* warm, tkm_path** out, void* stream);
+/* The same sweep for G <= 8 independent problems that share y, the folds, the loss and the lambda
+ * grid -- e.g. the bandwidths of a sigma grid, one spectral handle each (all with the same n, r and
+ * sweep precision).  Every iteration is ONE launch per kernel over all groups' live columns, which
+ * keeps the device full when each group's batch has become narrow.  Results are identical to G
+ * separate tkm_fit_path calls.  specs [host] G handles; warm [host] G paths or NULL; out [host] G
+ * slots, out[g] belongs to specs[g].  The sampled timings of tkm_path_profile are those of the shared
+ * launches and are reported on out[0] only. */
+int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, const void* y, tkm_loss loss,
+                       const tkm_loss_opts* opts, const double* lambdas, int32_t L,
+                       const int32_t* foldid, int32_t V, double tol, int32_t maxit,
+                       const tkm_path* const* warm, tkm_path** out, void* stream);
 void tkm_path_free(tkm_path* p);
 /* Shape and per-column diagnostics, all [host], any pointer may be NULL:
  * B, r; iters[B] (total over rounds), kkt[B] (last residual), flags[B] (1 = hit maxit),
@@ -159,13 +170,15 @@ int tkm_predict(const tkm_path* p, int32_t t, int32_t l,
                 int64_t pdim, double sigma, void* f_out, int8_t* label_out, void* stream);
 
 /* ---- whole pipeline from HOST buffers (the end-to-end call timed as `e2e` by bench.py) ---------
- * X [host] n x p FP64, y [host] n FP64; copies them to the device, runs S1, S2, S3-S8, S9 for one
- * sigma and returns [host] cv tables as in tkm_exact_cv plus the final-model coefficients of the
- * selected lambda of variant 0 ([host] alpha_best n doubles or NULL, *beta0_best).
- * Full kernel only.  stage_ms [host] 5 floats or NULL: copy-in, gram, eig, sweep, cv (ms). */
-int tkm_train_tune_host(const double* X, int64_t n, int64_t p, const double* y, double sigma,
-                        tkm_loss loss, const tkm_loss_opts* opts, const double* lambdas, int32_t L,
-                        const int32_t* foldid, int32_t V, double tol, int32_t maxit,
+ * X [host] n x p FP64, y [host] n FP64, sigmas [host] G <= 8 bandwidths; copies X, y to the device,
+ * runs S1 and S2 per bandwidth, S3-S8 for all bandwidths together (tkm_fit_path_multi), S9 per
+ * bandwidth, and returns, per bandwidth g, the [host] cv tables as in tkm_exact_cv (cv_loss
+ * G x T x L x V, cv_err G x T x L x V or NULL, cv_mean G x T x L, best_l G x T) plus the final-model
+ * coefficients of the selected lambda of variant 0 (alpha_best G x n doubles or NULL, beta0_best G).
+ * Full kernel only.  stage_ms [host] 5 floats or NULL: copy-in, gram, eig, sweep, cv + copy-out (ms). */
+int tkm_train_tune_host(const double* X, int64_t n, int64_t p, const double* y, const double* sigmas,
+                        int32_t G, tkm_loss loss, const tkm_loss_opts* opts, const double* lambdas,
+                        int32_t L, const int32_t* foldid, int32_t V, double tol, int32_t maxit,
                         tkm_dtype sweep_dt, double* cv_loss, int64_t* cv_err, double* cv_mean,
                         int32_t* best_l, double* alpha_best, double* beta0_best, float* stage_ms,
                         void* stream);
@@ -179,12 +192,17 @@ int tkm_make_folds(int64_t n, int32_t V, uint64_t seed, int32_t* foldid);
  * (bench.py's `gpu_launches`). */
 int64_t tkm_launch_count(void);
 void tkm_launch_count_reset(void);
-/* Dense FP64 GEMM probe on the library's own DMMA kernel (roofline calibration / tests):
- * Dt[N][M] = P[N][K] Q[M][K]^T, all [dev] FP64 row-major with leading dims ldp, ldq, ldd that are
- * multiples of 2 and >= K (P, Q) / >= M (Dt); the K-padding up to a multiple of 16 must be
- * readable zeros.  Asynchronous. */
+/* Dense FP64 GEMM probe on the library's own TMA + DMMA kernel (tests):
+ * Dt[N][M] = P[N][K] Q[M][K]^T, all [dev] FP64 row-major, 16-byte aligned, with even leading
+ * dimensions ldp, ldq >= K and ldd >= M.  Nothing beyond K is read.  Asynchronous. */
 int tkm_dgemm_nt(const double* P, int64_t ldp, const double* Q, int64_t ldq, double* Dt, int64_t ldd,
                  int64_t N, int64_t M, int64_t K, void* stream);
+/* Roofline calibration of the same kernel: G independent products Dt_g[N][M] = P_g[N][K] Q_g[M][K]^T
+ * on library-owned buffers, `iters` back-to-back launches of tile configuration `cfg` (0..7; -1 = the
+ * library's own shape-based choice) timed with CUDA events on `stream`; *ms [host] = milliseconds
+ * per launch.  Synchronises `stream`. */
+int tkm_gemm_probe(int32_t cfg, int32_t G, int32_t N, int32_t M, int32_t K, int32_t iters, float* ms,
+                   void* stream);
 int tkm_version(void);
 const char* tkm_last_error(void);
 

@@ -13,9 +13,9 @@ TKM_OK, TKM_ENOTCONV = 0, 5
 
 EXPORTED_SYMBOLS = [
     "tkm_gram", "tkm_spectral_setup", "tkm_spectral_free", "tkm_spectral_info", "tkm_spectral_get_u",
-    "tkm_fit_path", "tkm_path_free", "tkm_path_info", "tkm_path_profile", "tkm_path_get_a", "tkm_exact_cv", "tkm_path_coef",
+    "tkm_fit_path", "tkm_fit_path_multi", "tkm_path_free", "tkm_path_info", "tkm_path_profile", "tkm_path_get_a", "tkm_exact_cv", "tkm_path_coef",
     "tkm_predict", "tkm_train_tune_host", "tkm_make_folds", "tkm_launch_count", "tkm_launch_count_reset",
-    "tkm_dgemm_nt", "tkm_version", "tkm_last_error",
+    "tkm_dgemm_nt", "tkm_gemm_probe", "tkm_version", "tkm_last_error",
 ]
 
 
@@ -62,6 +62,8 @@ def lib():
     L.tkm_spectral_get_u.argtypes = [vp, vp, vp]
     L.tkm_fit_path.argtypes = [vp, vp, C.c_int, C.POINTER(_LossOpts), vp, i32, vp, i32, dbl, i32, vp,
                                C.POINTER(vp), vp]
+    L.tkm_fit_path_multi.argtypes = [C.POINTER(vp), i32, vp, C.c_int, C.POINTER(_LossOpts), vp, i32, vp, i32, dbl, i32,
+                                     C.POINTER(vp), C.POINTER(vp), vp]
     L.tkm_path_free.argtypes = [vp]
     L.tkm_path_free.restype = None
     L.tkm_path_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i64), vp, vp, vp, vp, C.POINTER(i64)]
@@ -70,12 +72,13 @@ def lib():
     L.tkm_exact_cv.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
     L.tkm_path_coef.argtypes = [vp, i32, i32, i32, vp, C.POINTER(dbl), vp]
     L.tkm_predict.argtypes = [vp, i32, i32, vp, i64, vp, i64, i64, i64, dbl, vp, vp, vp]
-    L.tkm_train_tune_host.argtypes = [vp, i64, i64, vp, dbl, C.c_int, C.POINTER(_LossOpts), vp, i32, vp, i32,
-                                      dbl, i32, C.c_int, vp, vp, vp, vp, vp, C.POINTER(dbl), vp, vp]
+    L.tkm_train_tune_host.argtypes = [vp, i64, i64, vp, vp, i32, C.c_int, C.POINTER(_LossOpts), vp, i32, vp, i32,
+                                      dbl, i32, C.c_int, vp, vp, vp, vp, vp, vp, vp, vp]
     L.tkm_make_folds.argtypes = [i64, i32, C.c_uint64, vp]
     L.tkm_launch_count.restype = i64
     L.tkm_launch_count_reset.restype = None
     L.tkm_dgemm_nt.argtypes = [vp, i64, vp, i64, vp, i64, i64, i64, i64, vp]
+    L.tkm_gemm_probe.argtypes = [i32, i32, i32, i32, i32, i32, C.POINTER(C.c_float), vp]
     L.tkm_last_error.restype = C.c_char_p
     for name in EXPORTED_SYMBOLS:
         getattr(L, name)   # AttributeError if the library does not export a declared symbol
@@ -269,6 +272,24 @@ def tkm_fit_path(spec: Spectral, y, loss: int, lambdas, foldid, V: int, tol: flo
     return Path(h, spec, rc)
 
 
+def tkm_fit_path_multi(specs, y, loss: int, lambdas, foldid, V: int, tol: float, maxit: int,
+                       smooth0=1.0, eta=0.125, rounds=4, taus=None, restart=True, check_every=0, warm_tol=0.0,
+                       warm=None, profile=False, stream=None):
+    """One sweep over G spectral handles that share y, folds and the lambda grid -> list of G Paths."""
+    y = _dev_f64(y, "y")
+    lam = _host(lambdas, np.float64)
+    fid = _host(foldid, np.int32)
+    o, keep = _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, profile)
+    G = len(specs)
+    hs = (C.c_void_p * G)(*[s._h for s in specs])
+    hw = (C.c_void_p * G)(*[w._h for w in warm]) if warm is not None else None
+    ho = (C.c_void_p * G)()
+    rc = lib().tkm_fit_path_multi(hs, G, y.data_ptr(), loss, C.byref(o), _ptr(lam), len(lam), _ptr(fid), V,
+                                  float(tol), int(maxit), hw, ho, _stream(stream))
+    _check(rc, allow_notconv=True)
+    return [Path(C.c_void_p(ho[g]), specs[g], rc) for g in range(G)]
+
+
 def tkm_exact_cv(path: Path, y, foldid, T: int, L: int, V: int, stream=None):
     y = _dev_f64(y, "y")
     fid = _host(foldid, np.int32)
@@ -302,30 +323,32 @@ def tkm_predict(path: Path, t: int, l: int, X_train, X_new, sigma: float, labels
     return f, lab
 
 
-def tkm_train_tune_host(X, y, sigma, loss, lambdas, foldid, V, tol, maxit, smooth0=1.0, eta=0.125, rounds=4,
+def tkm_train_tune_host(X, y, sigmas, loss, lambdas, foldid, V, tol, maxit, smooth0=1.0, eta=0.125, rounds=4,
                         taus=None, restart=True, check_every=0, warm_tol=0.0, sweep_dtype=F64,
                         want_alpha=True, stream=None):
-    """Whole pipeline from HOST numpy buffers (the `e2e` call of bench.py)."""
+    """Whole pipeline from HOST numpy buffers for G bandwidths at once (the `e2e` call of bench.py)."""
     X = _host(X, np.float64)
     y = _host(y, np.float64)
     lam = _host(lambdas, np.float64)
     fid = _host(foldid, np.int32)
+    sig = _host(np.atleast_1d(sigmas), np.float64)
+    G = len(sig)
     n, p = X.shape
     o, keep = _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol)
     T, L = max(1, len(keep)), len(lam)
-    cv_loss = np.empty((T, L, V))
-    cv_err = np.empty((T, L, V), dtype=np.int64)
-    cv_mean = np.empty((T, L))
-    best = np.empty(T, dtype=np.int32)
-    alpha = np.empty(n) if want_alpha else None
-    b0 = C.c_double()
+    cv_loss = np.empty((G, T, L, V))
+    cv_err = np.empty((G, T, L, V), dtype=np.int64)
+    cv_mean = np.empty((G, T, L))
+    best = np.empty((G, T), dtype=np.int32)
+    alpha = np.empty((G, n)) if want_alpha else None
+    b0 = np.zeros(G)
     stage = np.zeros(5, dtype=np.float32)
-    rc = lib().tkm_train_tune_host(_ptr(X), n, p, _ptr(y), float(sigma), loss, C.byref(o), _ptr(lam), L, _ptr(fid),
+    rc = lib().tkm_train_tune_host(_ptr(X), n, p, _ptr(y), _ptr(sig), G, loss, C.byref(o), _ptr(lam), L, _ptr(fid),
                                    V, float(tol), int(maxit), sweep_dtype, _ptr(cv_loss), _ptr(cv_err),
-                                   _ptr(cv_mean), _ptr(best), _ptr(alpha) if want_alpha else None, C.byref(b0),
+                                   _ptr(cv_mean), _ptr(best), _ptr(alpha) if want_alpha else None, _ptr(b0),
                                    _ptr(stage), _stream(stream))
     _check(rc, allow_notconv=True)
-    return dict(cv_loss=cv_loss, cv_err=cv_err, cv_mean=cv_mean, best_l=best, alpha=alpha, beta0=b0.value,
+    return dict(cv_loss=cv_loss, cv_err=cv_err, cv_mean=cv_mean, best_l=best, alpha=alpha, beta0=b0,
                 stage_ms=stage, status=rc)
 
 
@@ -340,3 +363,10 @@ def tkm_dgemm_nt(P, Q, stream=None):
     _check(lib().tkm_dgemm_nt(P.data_ptr(), P.stride(0), Q.data_ptr(), Q.stride(0), D.data_ptr(), ldd, N, M, K,
                               _stream(stream)))
     return D[:, :M]
+
+
+def tkm_gemm_probe(cfg: int, G: int, N: int, M: int, K: int, iters: int = 20, stream=None) -> float:
+    """Milliseconds per launch of the library's DMMA GEMM on synthetic operands (roofline calibration)."""
+    ms = C.c_float()
+    _check(lib().tkm_gemm_probe(cfg, G, N, M, K, iters, C.byref(ms), _stream(stream)))
+    return float(ms.value)

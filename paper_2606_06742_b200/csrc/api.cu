@@ -72,25 +72,30 @@ extern "C" int tkm_make_folds(int64_t n, int32_t V, uint64_t seed, int32_t* fold
   return TKM_OK;
 }
 
-extern "C" int tkm_train_tune_host(const double* X, int64_t n, int64_t p, const double* y, double sigma,
-                                   tkm_loss loss, const tkm_loss_opts* opts, const double* lambdas, int32_t L,
-                                   const int32_t* foldid, int32_t V, double tol, int32_t maxit,
+extern "C" int tkm_train_tune_host(const double* X, int64_t n, int64_t p, const double* y, const double* sigmas,
+                                   int32_t G, tkm_loss loss, const tkm_loss_opts* opts, const double* lambdas,
+                                   int32_t L, const int32_t* foldid, int32_t V, double tol, int32_t maxit,
                                    tkm_dtype sweep_dt, double* cv_loss, int64_t* cv_err, double* cv_mean,
                                    int32_t* best_l, double* alpha_best, double* beta0_best, float* stage_ms,
                                    void* stream) {
-  if (!X || !y || !opts || !lambdas || !foldid || !cv_loss || !cv_mean || !best_l)
+  if (!X || !y || !sigmas || !opts || !lambdas || !foldid || !cv_loss || !cv_mean || !best_l)
     return set_error(TKM_EINVAL, "tkm_train_tune_host: NULL argument");
-  if (n <= 1 || p <= 0) return set_error(TKM_EINVAL, "tkm_train_tune_host: bad n / p");
+  if (n <= 1 || p <= 0 || G < 1 || G > 8 || L < 1 || V < 2) return set_error(TKM_EINVAL, "tkm_train_tune_host: bad n / p / G / L / V");
   TKM_TRY(device_check());
   cudaStream_t st = (cudaStream_t)stream;
   cudaEvent_t ev[6];
   for (auto& e : ev) TKM_CUDA(cudaEventCreate(&e));
-  struct EvGuard {
+  struct Owner {   // everything that must be released on every exit path
     cudaEvent_t* e;
-    ~EvGuard() {
+    tkm_spectral* spec[8] = {};
+    tkm_path* path[8] = {};
+    ~Owner() {
       for (int i = 0; i < 6; ++i) cudaEventDestroy(e[i]);
+      for (auto* q : path) tkm_path_free(q);
+      for (auto* q : spec) tkm_spectral_free(q);
     }
-  } evg{ev};
+  } own{ev};
+  const int T = loss == TKM_LOSS_QUANTILE ? (opts->T > 0 ? opts->T : 1) : 1;
   DevBuf dX, dy, dK, dalpha;
   TKM_CUDA(cudaEventRecord(ev[0], st));
   TKM_TRY(dX.alloc((size_t)n * p * sizeof(double), false, st));
@@ -99,33 +104,44 @@ extern "C" int tkm_train_tune_host(const double* X, int64_t n, int64_t p, const 
   TKM_CUDA(cudaMemcpyAsync(dX.p, X, (size_t)n * p * sizeof(double), cudaMemcpyHostToDevice, st));
   TKM_CUDA(cudaMemcpyAsync(dy.p, y, (size_t)n * sizeof(double), cudaMemcpyHostToDevice, st));
   TKM_CUDA(cudaEventRecord(ev[1], st));
-  TKM_TRY(tkm_gram(dX.p, n, p, p, nullptr, 0, 0, sigma, TKM_F64, dK.p, n, st));
-  TKM_CUDA(cudaEventRecord(ev[2], st));
-  tkm_spectral* spec = nullptr;
-  TKM_TRY(tkm_spectral_setup(dK.p, n, n, nullptr, sweep_dt, &spec, st));
+  float gram_ms = 0.f, eig_ms = 0.f;
+  for (int g = 0; g < G; ++g) {
+    TKM_CUDA(cudaEventRecord(ev[5], st));   // ev[5] doubles as the per-bandwidth start mark
+    TKM_TRY(tkm_gram(dX.p, n, p, p, nullptr, 0, 0, sigmas[g], TKM_F64, dK.p, n, st));
+    TKM_CUDA(cudaEventRecord(ev[2], st));
+    TKM_TRY(tkm_spectral_setup(dK.p, n, n, nullptr, sweep_dt, &own.spec[g], st));   // synchronises
+    TKM_CUDA(cudaEventRecord(ev[3], st));
+    TKM_CUDA(cudaEventSynchronize(ev[3]));
+    float a = 0.f, b = 0.f;
+    cudaEventElapsedTime(&a, ev[5], ev[2]);
+    cudaEventElapsedTime(&b, ev[2], ev[3]);
+    gram_ms += a;
+    eig_ms += b;
+  }
   dK.release();
   TKM_CUDA(cudaEventRecord(ev[3], st));
-  tkm_path* path = nullptr;
-  int rc = tkm_fit_path(spec, dy.p, loss, opts, lambdas, L, foldid, V, tol, maxit, nullptr, &path, st);
-  if (rc != TKM_OK && rc != TKM_ENOTCONV) {
-    tkm_spectral_free(spec);
-    return rc;
+  int rc = tkm_fit_path_multi(own.spec, G, dy.p, loss, opts, lambdas, L, foldid, V, tol, maxit, nullptr, own.path, st);
+  if (rc != TKM_OK && rc != TKM_ENOTCONV) return rc;
+  TKM_CUDA(cudaEventRecord(ev[4], st));
+  if (alpha_best) TKM_TRY(dalpha.alloc((size_t)G * n * sizeof(double), false, st));
+  for (int g = 0; g < G; ++g) {
+    const size_t o3 = (size_t)g * T * L * V, o2 = (size_t)g * T * L, o1 = (size_t)g * T;
+    TKM_TRY(tkm_exact_cv(own.path[g], dy.p, foldid, cv_loss + o3, cv_err ? cv_err + o3 : nullptr, cv_mean + o2,
+                         best_l + o1, st));
+    if (alpha_best)
+      TKM_TRY(tkm_path_coef(own.path[g], 0, best_l[o1], V, dalpha.as<double>() + (size_t)g * n,
+                            beta0_best ? beta0_best + g : nullptr, st));
   }
-  cudaEventRecord(ev[4], st);
-  int rc2 = tkm_exact_cv(path, dy.p, foldid, cv_loss, cv_err, cv_mean, best_l, st);
-  if (rc2 == TKM_OK && alpha_best) {
-    rc2 = dalpha.alloc((size_t)n * sizeof(double), false, st);
-    if (rc2 == TKM_OK) rc2 = tkm_path_coef(path, 0, best_l[0], V, dalpha.as<double>(), beta0_best, st);
-    if (rc2 == TKM_OK) {
-      cudaError_t e = cudaMemcpyAsync(alpha_best, dalpha.p, n * sizeof(double), cudaMemcpyDeviceToHost, st);
-      if (e != cudaSuccess) rc2 = set_error(TKM_ECUDA, "copy of alpha failed: %s", cudaGetErrorString(e));
-    }
+  if (alpha_best)
+    TKM_CUDA(cudaMemcpyAsync(alpha_best, dalpha.p, (size_t)G * n * sizeof(double), cudaMemcpyDeviceToHost, st));
+  TKM_CUDA(cudaEventRecord(ev[5], st));
+  TKM_CUDA(cudaStreamSynchronize(st));
+  if (stage_ms) {
+    cudaEventElapsedTime(&stage_ms[0], ev[0], ev[1]);
+    stage_ms[1] = gram_ms;
+    stage_ms[2] = eig_ms;
+    cudaEventElapsedTime(&stage_ms[3], ev[3], ev[4]);
+    cudaEventElapsedTime(&stage_ms[4], ev[4], ev[5]);
   }
-  cudaEventRecord(ev[5], st);
-  cudaStreamSynchronize(st);
-  if (stage_ms)
-    for (int i = 0; i < 5; ++i) cudaEventElapsedTime(&stage_ms[i], ev[i], ev[i + 1]);
-  tkm_path_free(path);
-  tkm_spectral_free(spec);
-  return rc2 != TKM_OK ? rc2 : rc;
+  return rc;
 }

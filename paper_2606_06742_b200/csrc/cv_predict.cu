@@ -33,15 +33,15 @@ struct CvEpi {
   double* lpart;           // [m blocks][ldpart] partial loss sums over held-out rows
   double* epart;           // [m blocks][ldpart] partial misclassification counts (exact in FP64)
   int64_t ldpart;
-  template <int BN, int BM, int WARPS_N, int WARPS_M, int TN, int TM>
-  __device__ __forceinline__ void run(double (&acc)[TN][TM][2], int n_blk0, int m_blk0, int warp_n,
-                                      int warp_m, int lane, int N, int M, double* scratch) const {
-    constexpr int WN = BN / WARPS_N, WM = BM / WARPS_M;
+  template <class Cfg>
+  __device__ __forceinline__ void run(double (&acc)[Cfg::TN][Cfg::TM][2], int n_blk0, int m_blk0, int warp_n,
+                                      int warp_m, int lane, int N, int M, int, double* scratch) const {
+    constexpr int TN = Cfg::TN, TM = Cfg::TM;
     double ls[TN], es[TN];
 #pragma unroll
     for (int i = 0; i < TN; ++i) {
       ls[i] = es[i] = 0.0;
-      const int col = n_blk0 + warp_n * WN + i * 8 + (lane >> 2);
+      const int col = n_blk0 + (warp_n * TN + i) * 8 + (lane >> 2);
       if (col >= N) continue;
       const int v = col_v[col];
       if (v >= V) continue;   // final-model column: nothing held out
@@ -50,7 +50,7 @@ struct CvEpi {
       for (int j = 0; j < TM; ++j)
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
-          const int m = m_blk0 + warp_m * WM + j * 8 + 2 * (lane & 3) + e;
+          const int m = m_blk0 + (warp_m * TM + j) * 8 + 2 * (lane & 3) + e;
           if (m < M && foldid[m] == v) {
             const double f = acc[i][j][e] + b0, yy = y[m];
             ls[i] += nominal_loss_dev(loss, yy, f, tau);
@@ -60,11 +60,11 @@ struct CvEpi {
         }
     }
     double tot;
-    if (cta_row_reduce<BN, WARPS_N, WARPS_M, TN>(ls, warp_n, warp_m, lane, scratch, tot)) {
+    if (cta_row_reduce<Cfg>(ls, warp_n, warp_m, lane, scratch, tot)) {
       const int col = n_blk0 + (int)threadIdx.x;
       if (col < N) lpart[(int64_t)blockIdx.x * ldpart + col] = tot;
     }
-    if (cta_row_reduce<BN, WARPS_N, WARPS_M, TN>(es, warp_n, warp_m, lane, scratch, tot)) {
+    if (cta_row_reduce<Cfg>(es, warp_n, warp_m, lane, scratch, tot)) {
       const int col = n_blk0 + (int)threadIdx.x;
       if (col < N) epart[(int64_t)blockIdx.x * ldpart + col] = tot;
     }
@@ -205,8 +205,7 @@ extern "C" int tkm_exact_cv(const tkm_path* p, const void* y, const int32_t* fol
     if (foldid[j] < 0 || foldid[j] >= V) return set_error(TKM_EINVAL, "tkm_exact_cv: foldid out of range");
     fsize[foldid[j]] += 1.0;
   }
-  const int bm = gemm_f64_tile_bm(B, n);
-  const int nblk = (int)ceil_div(n, bm);
+  const int nblk = (int)ceil_div(n, gemm_f64_choose(B, B, 1, (int)n).BM);
   const int64_t ldpart = round_up(B, 16);
   const int nout = T * L * V;
   DevBuf lpart, epart, d_fold, d_fsize, d_lam, d_loss, d_err, d_mean, d_best;
@@ -222,10 +221,9 @@ extern "C" int tkm_exact_cv(const tkm_path* p, const void* y, const int32_t* fol
   TKM_CUDA(cudaMemcpyAsync(d_fold.p, foldid, n * sizeof(int32_t), cudaMemcpyHostToDevice, st));
   TKM_CUDA(cudaMemcpyAsync(d_fsize.p, fsize.data(), V * sizeof(double), cudaMemcpyHostToDevice, st));
   TKM_CUDA(cudaMemcpyAsync(d_lam.p, p->lambdas.data(), L * sizeof(double), cudaMemcpyHostToDevice, st));
-  GemmOperands g{p->a.as<double>(), s->ldr, s->UL.as<double>(), s->ldr, B, (int)n, (int)r};
   CvEpi epi{(const double*)y, d_fold.as<int32_t>(), p->beta0.as<double>(), p->col_tau.as<double>(),
             p->col_v.as<int32_t>(), V, (int)p->loss, lpart.as<double>(), epart.as<double>(), ldpart};
-  TKM_TRY(gemm_f64_dispatch(g, epi, st));
+  TKM_TRY(gemm_f64_once(p->a.as<double>(), s->ldr, s->UL.as<double>(), s->ldr, B, (int)n, (int)r, epi, st));
   cv_finalize_kernel<<<(unsigned)ceil_div(nout, 128), 128, 0, st>>>(
       lpart.as<double>(), epart.as<double>(), ldpart, nblk, T, L, V, d_fsize.as<double>(),
       p->loss != TKM_LOSS_QUANTILE ? 1 : 0, d_loss.as<double>(), d_err.as<long long>());

@@ -1,74 +1,117 @@
-// gemm_f64.cuh -- FP64 tensor-core (DMMA.8x8x4) GEMM with fused epilogues for the sweep.
+// gemm_f64.cuh -- FP64 tensor-core (DMMA.8x8x4) GEMM with fused epilogues: the two contractions of the
+// sweep, the exact-CV scoring pass (S9) and the Nystrom setup products.
 //
-// Computes Dt[N][M] = P[N][K] * Q[M][K]^T  ("NT": both operands K-contiguous).
-//   GEMM-A of the sweep:  P = abar (slots x r),  Q = U*Lam (n x r)  -> F^T (slots x n)
-//   GEMM-B of the sweep (S6):                 P = Z^T  (slots x n),  Q = U^T   (r x n)  -> zeta^T (slots x r)
-// The moving operand is stored one column of the paper's (lambda, fold) batch per ROW, so that a
-// column's vector is contiguous (per-column reductions and compaction are row operations).
+// Computes, for every group g < G (independent problems sharing one launch, e.g. the bandwidths of a
+// sigma grid),   Dt_g[N_g][M] = P_g[N_g][K] * Q_g[M][K]^T   ("NT": both operands K-contiguous).
+//   GEMM-A (S5):  P = Lam*abar (slots x r),  Q = U   ... stored as U*Lam (n x r)  -> F^T    (slots x n)
+//   GEMM-B (S6):  P = Z^T      (slots x n),  Q = U^T (r x n)                      -> zeta^T (slots x r)
+// The moving operand P holds one column of the paper's (lambda, fold) batch per ROW ("slot"); the
+// groups' P matrices are stacked: row g * p_group_rows + slot of one array.  N_g (live slots) is read
+// from device memory so that the host never has to synchronise to launch the next iteration.
 //
-// The MMA "A" operand (row-major 8x4) is a P fragment, the MMA "B" operand (col-major 4x8) is a Q
-// fragment, so the accumulator fragment of lane l holds Dt[n0 + l/4][m0 + 2(l%4) + {0,1}]: two
-// consecutive m, i.e. 16-byte stores along the contiguous output dimension.
+// Blackwell mapping: tcgen05 has no FP64 kind, so the math is mma.sync m8n8k4 f64 (DMMA).  Operand
+// tiles are staged by TMA (cp.async.bulk.tensor, 128-byte swizzle, box = rows x 16 doubles) into a
+// STAGES-deep ring guarded by full/empty mbarriers; one producer warp issues the loads, WN x WM
+// consumer warps run the MMAs and never meet at a CTA-wide barrier inside the K loop.
 //
-// Pipeline: STAGES-deep cp.async ring, one __syncthreads per K-step of 16.  Requirements checked by
-// the host wrappers: P, Q 16-byte aligned and ldp, ldq even (16-byte row alignment).  Rows beyond
-// N / M and the K tail are zero-filled through the cp.async src-size operand, so no padding of the
-// operands is read.
+// Fragment addressing: with the 128-byte swizzle a tile row is 8 chunks of 16 B, chunk c of row R
+// stored at chunk c ^ (R & 7).  The MMA k-slot j = lane & 3 of sub-step s is mapped to
+// k = 8 (j >> 1) + 2 s + (j & 1)  (any bijection of the 16 k of a stage is a valid summation order,
+// as long as both operands use the same one); then the 16 lanes of a half-warp touch 16 distinct
+// 8-byte bank pairs -> conflict-free LDS.64 for both operands.
+//
+// Accumulator fragment of lane l: Dt[n0 + l/4][m0 + 2 (l%4) + {0,1}] per 8x8 sub-tile.
 #pragma once
 
-#include "common.cuh"
+#include "tma.cuh"
 
 namespace tkm {
 
-constexpr int GEMM_BK = 16;            // K-step in doubles (128 bytes per row)
-constexpr int GEMM_LDS = GEMM_BK + 4;  // padded smem row: (20 mod 16) = 4 => conflict-free LDS.64
+constexpr int GEMM_MAX_GROUPS = 8;
+constexpr int GEMM_ROW_BYTES = TMA_BOX_K * 8;   // 128
 
-struct GemmOperands {
-  const double* P;
-  int64_t ldp;
-  const double* Q;
-  int64_t ldq;
-  int N, M, K;
+struct GemmArgs {
+  CUtensorMap p_map;                    // [G * p_group_rows][K], box = BN x 16
+  CUtensorMap q_map[GEMM_MAX_GROUPS];   // per group [M][K], box = BM x 16
+  const int32_t* nslots;                // [G] device, live rows of each group; NULL => N for all
+  int p_group_rows;                     // row offset between consecutive groups in P
+  int N, M, K;                          // N: upper bound of the live rows (the grid covers it)
 };
 
-template <int BN, int BM, int WARPS_N, int WARPS_M, int STAGES, class Epi>
-__global__ void __launch_bounds__(WARPS_N* WARPS_M * 32)
-    gemm_f64_nt_kernel(const GemmOperands g, const Epi epi) {
-  constexpr int NT = WARPS_N * WARPS_M * 32;
-  constexpr int WN = BN / WARPS_N, WM = BM / WARPS_M;
-  constexpr int TN = WN / 8, TM = WM / 8;
-  static_assert(WN % 8 == 0 && WM % 8 == 0, "warp tile must be a multiple of the 8x8 MMA tile");
-  extern __shared__ __align__(16) double smem[];
-  double* Ps = smem;                                   // [STAGES][BN][GEMM_LDS]
-  double* Qs = smem + (size_t)STAGES * BN * GEMM_LDS;   // [STAGES][BM][GEMM_LDS]
+template <int TN_, int WN_, int TM_, int WM_, int STAGES_>
+struct GemmCfg {
+  static constexpr int TN = TN_, WN = WN_, TM = TM_, WM = WM_, STAGES = STAGES_;
+  static constexpr int BN = TN * WN * 8, BM = TM * WM * 8;
+  static constexpr int CONSUMERS = WN * WM * 32;
+  static constexpr int THREADS = CONSUMERS + 32;
+  static constexpr int STAGE_BYTES = (BN + BM) * GEMM_ROW_BYTES;
+  static constexpr size_t SMEM = (size_t)STAGES * STAGE_BYTES + 1024;   // + alignment slack
+  static_assert(BN <= 256 && BM <= 256, "TMA box dimension limit");
+  static_assert(BN <= CONSUMERS, "epilogue row reductions assign one thread per tile row");
+};
 
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int warp_n = warp / WARPS_M, warp_m = warp % WARPS_M;
+// consumer-only barrier (the producer warp has left the CTA-wide flow)
+template <int COUNT>
+__device__ __forceinline__ void consumer_sync() {
+  asm volatile("bar.sync 1, %0;\n" ::"n"(COUNT) : "memory");
+}
+
+template <class Cfg, class Epi>
+__global__ void __launch_bounds__(Cfg::THREADS)
+    gemm_f64_tma_kernel(const __grid_constant__ GemmArgs g, const Epi epi) {
+  constexpr int TN = Cfg::TN, WN = Cfg::WN, TM = Cfg::TM, WM = Cfg::WM, STAGES = Cfg::STAGES;
+  constexpr int BN = Cfg::BN, BM = Cfg::BM;
+  extern __shared__ uint8_t smem_raw[];
+  __shared__ __align__(8) uint64_t full_bar[STAGES];
+  __shared__ __align__(8) uint64_t empty_bar[STAGES];
+  __shared__ double scratch[WM * BN];
+
+  const int grp = blockIdx.z;
+  const int N = g.nslots ? min(g.nslots[grp], g.N) : g.N;
   const int m_blk0 = blockIdx.x * BM, n_blk0 = blockIdx.y * BN;
-  if (n_blk0 >= g.N) return;   // grid may be sized for more slots than are still active
-  const int KT = (g.K + GEMM_BK - 1) / GEMM_BK;
+  if (n_blk0 >= N) return;   // the grid is sized for an upper bound of the live slots
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int KT = (g.K + TMA_BOX_K - 1) / TMA_BOX_K;
+  uint8_t* tiles = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
 
-  auto load_stage = [&](int stage, int kt) {
-    const int k0 = kt * GEMM_BK;
-    double* ps = Ps + (size_t)stage * BN * GEMM_LDS;
-    double* qs = Qs + (size_t)stage * BM * GEMM_LDS;
+  if (tid == 0) {
 #pragma unroll
-    for (int id = tid; id < BN * 8; id += NT) {
-      const int row = id >> 3, ch = id & 7;
-      const int kk = k0 + ch * 2;
-      const int nb = ((n_blk0 + row) < g.N) ? min(max(g.K - kk, 0), 2) * 8 : 0;
-      const double* src = nb ? g.P + (int64_t)(n_blk0 + row) * g.ldp + kk : g.P;
-      cp_async_16(ps + row * GEMM_LDS + ch * 2, src, nb);
+    for (int s = 0; s < STAGES; ++s) {
+      mbar_init(&full_bar[s], 1);
+      mbar_init(&empty_bar[s], WN * WM);
     }
+    mbar_fence_init();
+  }
+  __syncthreads();
+
+  if (warp == WN * WM) {
+    // ===== TMA producer =====
+    if (lane == 0) {
+      tma_prefetch_desc(&g.p_map);
+      tma_prefetch_desc(&g.q_map[grp]);
+      const int prow = grp * g.p_group_rows + n_blk0;
+      for (int kt = 0; kt < KT; ++kt) {
+        const int s = kt % STAGES;
+        if (kt >= STAGES) mbar_wait(&empty_bar[s], ((kt / STAGES) - 1) & 1);
+        mbar_arrive_expect_tx(&full_bar[s], Cfg::STAGE_BYTES);
+        uint8_t* ps = tiles + (size_t)s * Cfg::STAGE_BYTES;
+        tma_load_2d(ps, &g.p_map, kt * TMA_BOX_K, prow, &full_bar[s]);
+        tma_load_2d(ps + BN * GEMM_ROW_BYTES, &g.q_map[grp], kt * TMA_BOX_K, m_blk0, &full_bar[s]);
+      }
+    }
+    return;
+  }
+
+  // ===== MMA consumers =====
+  const int warp_n = warp / WM, warp_m = warp % WM;
+  const int fr = lane >> 2, fj = lane & 3;
+  // live 8-row sub-tiles of this warp (slots beyond N are neither multiplied nor stored)
+  const int nv = min(TN, max(0, (N - (n_blk0 + warp_n * TN * 8) + 7) >> 3));
+  uint32_t off[4];   // byte offset inside a 128-byte tile row of this lane's element at sub-step s
 #pragma unroll
-    for (int id = tid; id < BM * 8; id += NT) {
-      const int row = id >> 3, ch = id & 7;
-      const int kk = k0 + ch * 2;
-      const int nb = ((m_blk0 + row) < g.M) ? min(max(g.K - kk, 0), 2) * 8 : 0;
-      const double* src = nb ? g.Q + (int64_t)(m_blk0 + row) * g.ldq + kk : g.Q;
-      cp_async_16(qs + row * GEMM_LDS + ch * 2, src, nb);
-    }
-  };
+  for (int s = 0; s < 4; ++s) off[s] = (uint32_t)(((((fj >> 1) << 2) + s) ^ fr) << 4) | (uint32_t)((fj & 1) << 3);
+  const uint32_t p_row = (uint32_t)((warp_n * TN * 8 + fr) * GEMM_ROW_BYTES);
+  const uint32_t q_row = (uint32_t)(BN * GEMM_ROW_BYTES + (warp_m * TM * 8 + fr) * GEMM_ROW_BYTES);
 
   double acc[TN][TM][2];
 #pragma unroll
@@ -76,55 +119,41 @@ __global__ void __launch_bounds__(WARPS_N* WARPS_M * 32)
 #pragma unroll
     for (int j = 0; j < TM; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
-#pragma unroll
-  for (int s = 0; s < STAGES - 1; ++s) {
-    if (s < KT) load_stage(s, s);
-    cp_async_commit();
-  }
-
-  const int frag_row = lane >> 2, frag_k = lane & 3;
   for (int kt = 0; kt < KT; ++kt) {
-    cp_async_wait<STAGES - 2>();
-    __syncthreads();
-    {
-      const int nk = kt + STAGES - 1;
-      if (nk < KT) load_stage(nk % STAGES, nk);
-      cp_async_commit();
-    }
-    const double* ps = Ps + (size_t)(kt % STAGES) * BN * GEMM_LDS + (warp_n * WN + frag_row) * GEMM_LDS + frag_k;
-    const double* qs = Qs + (size_t)(kt % STAGES) * BM * GEMM_LDS + (warp_m * WM + frag_row) * GEMM_LDS + frag_k;
+    const int s = kt % STAGES;
+    mbar_wait(&full_bar[s], (kt / STAGES) & 1);
+    const uint8_t* st = tiles + (size_t)s * Cfg::STAGE_BYTES;
 #pragma unroll
-    for (int kk = 0; kk < GEMM_BK; kk += 4) {
+    for (int ks = 0; ks < 4; ++ks) {
       double a[TN], b[TM];
 #pragma unroll
-      for (int i = 0; i < TN; ++i) a[i] = ps[i * 8 * GEMM_LDS + kk];
-#pragma unroll
-      for (int j = 0; j < TM; ++j) b[j] = qs[j * 8 * GEMM_LDS + kk];
+      for (int j = 0; j < TM; ++j)
+        b[j] = *reinterpret_cast<const double*>(st + q_row + j * 8 * GEMM_ROW_BYTES + off[ks]);
 #pragma unroll
       for (int i = 0; i < TN; ++i)
+        if (i < nv) a[i] = *reinterpret_cast<const double*>(st + p_row + i * 8 * GEMM_ROW_BYTES + off[ks]);
 #pragma unroll
-        for (int j = 0; j < TM; ++j) dmma_884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+      for (int i = 0; i < TN; ++i)
+        if (i < nv) {
+#pragma unroll
+          for (int j = 0; j < TM; ++j) dmma_884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+        }
     }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&empty_bar[s]);
   }
-  cp_async_wait<0>();
-  __syncthreads();   // pipeline smem is now free: epilogues may use it as reduction scratch
 
-  epi.template run<BN, BM, WARPS_N, WARPS_M, TN, TM>(acc, n_blk0, m_blk0, warp_n, warp_m, lane, g.N, g.M, smem);
+  epi.template run<Cfg>(acc, n_blk0, m_blk0, warp_n, warp_m, lane, N, g.M, grp, scratch);
 }
 
-template <int BN, int BM, int STAGES>
-constexpr size_t gemm_f64_smem_bytes() {
-  return (size_t)STAGES * (BN + BM) * GEMM_LDS * sizeof(double);
-}
-
-// Per-CTA deterministic column reduction helper used by the epilogues: `v[TN]` holds, per thread, a
-// partial sum for the TN slot-rows n = n_blk0 + warp_n*WN + i*8 + lane/4.  Reduces over the quad
-// (the 4 lanes sharing a row) and over the WARPS_M warps, then thread n_local < BN returns the CTA
-// total for row n_local in `out` (valid only when the function returns true).
-template <int BN, int WARPS_N, int WARPS_M, int TN>
-__device__ __forceinline__ bool cta_row_reduce(double (&v)[TN], int warp_n, int warp_m, int lane,
+// Per-CTA deterministic row reduction used by the epilogues: `v[TN]` holds, per thread, a partial sum
+// for the TN slot-rows n = n_blk0 + warp_n*TN*8 + i*8 + lane/4.  Reduces over the quad (the 4 lanes
+// sharing a row) and over the WM warps in fixed order; thread t < BN then returns the CTA total of tile
+// row t in `out` (valid only when the function returns true).  Consumer threads only.
+template <class Cfg>
+__device__ __forceinline__ bool cta_row_reduce(double (&v)[Cfg::TN], int warp_n, int warp_m, int lane,
                                                double* scratch, double& out) {
-  constexpr int WN = BN / WARPS_N;
+  constexpr int TN = Cfg::TN, BN = Cfg::BN, WM = Cfg::WM;
 #pragma unroll
   for (int i = 0; i < TN; ++i) {
     v[i] += __shfl_xor_sync(0xffffffffu, v[i], 1);
@@ -132,38 +161,39 @@ __device__ __forceinline__ bool cta_row_reduce(double (&v)[TN], int warp_n, int 
   }
   if ((lane & 3) == 0) {
 #pragma unroll
-    for (int i = 0; i < TN; ++i) scratch[warp_m * BN + warp_n * WN + i * 8 + (lane >> 2)] = v[i];
+    for (int i = 0; i < TN; ++i) scratch[warp_m * BN + warp_n * TN * 8 + i * 8 + (lane >> 2)] = v[i];
   }
-  __syncthreads();
+  consumer_sync<Cfg::CONSUMERS>();
   const int t = threadIdx.x;
-  bool have = t < BN;
+  const bool have = t < BN;
   if (have) {
     double s = 0.0;
 #pragma unroll
-    for (int w = 0; w < WARPS_M; ++w) s += scratch[w * BN + t];
+    for (int w = 0; w < WM; ++w) s += scratch[w * BN + t];
     out = s;
   }
-  __syncthreads();   // scratch may be reused by the caller
+  consumer_sync<Cfg::CONSUMERS>();   // scratch may be reused by the caller
   return have;
 }
 
-// ---- epilogue: plain store --------------------------------------------------------------------
+// ---- epilogue: plain store  Dt = alpha * acc -------------------------------------------------------
 struct StoreEpi {
   double* Dt;
   int64_t ldd;
-  double alpha;   // Dt = alpha * acc
-  template <int BN, int BM, int WARPS_N, int WARPS_M, int TN, int TM>
-  __device__ __forceinline__ void run(double (&acc)[TN][TM][2], int n_blk0, int m_blk0, int warp_n,
-                                      int warp_m, int lane, int N, int M, double*) const {
-    constexpr int WN = BN / WARPS_N, WM = BM / WARPS_M;
+  int64_t group_stride;   // elements between the groups' outputs
+  double alpha;
+  template <class Cfg>
+  __device__ __forceinline__ void run(double (&acc)[Cfg::TN][Cfg::TM][2], int n_blk0, int m_blk0, int warp_n,
+                                      int warp_m, int lane, int N, int M, int grp, double*) const {
+    double* base = Dt + (int64_t)grp * group_stride;
 #pragma unroll
-    for (int i = 0; i < TN; ++i) {
-      const int n = n_blk0 + warp_n * WN + i * 8 + (lane >> 2);
+    for (int i = 0; i < Cfg::TN; ++i) {
+      const int n = n_blk0 + (warp_n * Cfg::TN + i) * 8 + (lane >> 2);
       if (n >= N) continue;
 #pragma unroll
-      for (int j = 0; j < TM; ++j) {
-        const int m = m_blk0 + warp_m * WM + j * 8 + 2 * (lane & 3);
-        double* d = Dt + (int64_t)n * ldd + m;
+      for (int j = 0; j < Cfg::TM; ++j) {
+        const int m = m_blk0 + (warp_m * Cfg::TM + j) * 8 + 2 * (lane & 3);
+        double* d = base + (int64_t)n * ldd + m;
         if (m + 1 < M) {
           *reinterpret_cast<double2*>(d) = make_double2(alpha * acc[i][j][0], alpha * acc[i][j][1]);
         } else if (m < M) {
@@ -174,40 +204,103 @@ struct StoreEpi {
   }
 };
 
-template <int BN, int BM, int WARPS_N, int WARPS_M, int STAGES, class Epi>
-int launch_gemm_f64(const GemmOperands& g, const Epi& epi, cudaStream_t st) {
-  auto kern = gemm_f64_nt_kernel<BN, BM, WARPS_N, WARPS_M, STAGES, Epi>;
-  constexpr size_t smem = gemm_f64_smem_bytes<BN, BM, STAGES>();
+// ---- host side ---------------------------------------------------------------------------------------
+// One GEMM problem set as the host sees it; tensor maps are built by gemm_f64_prepare.
+struct GemmProblem {
+  const double* P = nullptr;   // [G * p_group_rows][ldp]
+  int64_t ldp = 0;
+  int p_group_rows = 0;
+  int64_t p_total_rows = 0;    // rows of the stacked P array that may be read (>= G * p_group_rows)
+  const double* Q[GEMM_MAX_GROUPS] = {};
+  int64_t ldq = 0;
+  int G = 1;
+  int M = 0, K = 0;
+};
+
+// Tile configurations.  The slot dimension is cut into BN = 8 TN WN rows, the output dimension into
+// BM = 8 TM WM.  Wide batches use 64 x 128 tiles (each Q tile feeds 64 slots); narrower ones shrink TN so
+// that the last N tile is not mostly padding, and shrink BM to put more CTAs in flight.
+using GemmW8 = GemmCfg<8, 1, 2, 8, 4>;   // 64 x 128
+using GemmW6 = GemmCfg<6, 1, 2, 8, 4>;   // 48 x 128
+using GemmW4 = GemmCfg<4, 1, 2, 8, 4>;   // 32 x 128
+using GemmS8 = GemmCfg<8, 1, 1, 8, 4>;   // 64 x 64
+using GemmS5 = GemmCfg<5, 1, 1, 8, 4>;   // 40 x 64
+using GemmS3 = GemmCfg<3, 1, 1, 8, 6>;   // 24 x 64
+using GemmS2 = GemmCfg<2, 1, 1, 8, 6>;   // 16 x 64
+using GemmS1 = GemmCfg<1, 1, 1, 8, 6>;   //  8 x 64
+constexpr int GEMM_NUM_CFG = 8;
+
+struct GemmTile {
+  int cfg, BN, BM;
+};
+inline GemmTile gemm_f64_tile_of(int cfg) {
+  switch (cfg) {
+    case 0: return {0, GemmW8::BN, GemmW8::BM};
+    case 1: return {1, GemmW6::BN, GemmW6::BM};
+    case 2: return {2, GemmW4::BN, GemmW4::BM};
+    case 3: return {3, GemmS8::BN, GemmS8::BM};
+    case 4: return {4, GemmS5::BN, GemmS5::BM};
+    case 5: return {5, GemmS3::BN, GemmS3::BM};
+    case 6: return {6, GemmS2::BN, GemmS2::BM};
+    default: return {7, GemmS1::BN, GemmS1::BM};
+  }
+}
+// Shape-based choice: `nmax` = largest live slot count of any group, `ntot` = sum over groups.
+GemmTile gemm_f64_choose(int nmax, int64_t ntot, int G, int M);
+int gemm_f64_force_cfg(int cfg);   // tuning hook: >= 0 forces a configuration, -1 restores the heuristic
+
+int gemm_f64_make_args(const GemmProblem& pr, const GemmTile& tile, GemmArgs* out);
+
+template <class Cfg, class Epi>
+int launch_gemm_f64(const GemmArgs& a, int G, const Epi& epi, cudaStream_t st) {
+  auto kern = gemm_f64_tma_kernel<Cfg, Epi>;
   static bool configured = false;   // per template instantiation
   if (!configured) {
-    TKM_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    TKM_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
     configured = true;
   }
-  dim3 grid((unsigned)ceil_div(g.M, BM), (unsigned)ceil_div(g.N, BN));
-  kern<<<grid, WARPS_N * WARPS_M * 32, smem, st>>>(g, epi);
+  dim3 grid((unsigned)ceil_div(a.M, Cfg::BM), (unsigned)ceil_div(std::max(a.N, 1), Cfg::BN), (unsigned)G);
+  kern<<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(a, epi);
   TKM_LAUNCH_CHECK();
   return TKM_OK;
 }
 
-// Shape-based tile choice shared by all FP64 GEMM call sites.  The grid is (M tiles, N tiles); pick
-// the largest tile whose CTA count still covers the 148 SMs about twice, else the smallest.
-// gemm_f64_tile_bm() returns the BM of that choice (callers size per-M-block partial arrays by it).
-inline int gemm_f64_config(int64_t N, int64_t M) {
-  const int64_t t128 = ceil_div(M, 128) * ceil_div(N, 64);
-  if (t128 >= 2 * 148) return 2;
-  const int64_t t64 = ceil_div(M, 64) * ceil_div(N, 64);
-  if (t64 >= 148 + 74) return 1;
-  return 0;
-}
-inline int gemm_f64_tile_bm(int64_t N, int64_t M) { return gemm_f64_config(N, M) == 2 ? 128 : 64; }
-
+// `a` must have been built by gemm_f64_make_args for `tile`; a.N / a.nslots are set by the caller.
 template <class Epi>
-int gemm_f64_dispatch(const GemmOperands& g, const Epi& epi, cudaStream_t st) {
-  switch (gemm_f64_config(g.N, g.M)) {
-    case 2: return launch_gemm_f64<64, 128, 2, 2, 3>(g, epi, st);
-    case 1: return launch_gemm_f64<64, 64, 2, 2, 3>(g, epi, st);
-    default: return launch_gemm_f64<32, 64, 1, 4, 4>(g, epi, st);
+int gemm_f64_launch(const GemmArgs& a, const GemmTile& tile, int G, const Epi& epi, cudaStream_t st) {
+  switch (tile.cfg) {
+    case 0: return launch_gemm_f64<GemmW8>(a, G, epi, st);
+    case 1: return launch_gemm_f64<GemmW6>(a, G, epi, st);
+    case 2: return launch_gemm_f64<GemmW4>(a, G, epi, st);
+    case 3: return launch_gemm_f64<GemmS8>(a, G, epi, st);
+    case 4: return launch_gemm_f64<GemmS5>(a, G, epi, st);
+    case 5: return launch_gemm_f64<GemmS3>(a, G, epi, st);
+    case 6: return launch_gemm_f64<GemmS2>(a, G, epi, st);
+    default: return launch_gemm_f64<GemmS1>(a, G, epi, st);
   }
+}
+
+// Convenience for one-off single-group products (setup, exact CV): choose, build maps, launch.
+template <class Epi>
+int gemm_f64_once(const double* P, int64_t ldp, const double* Q, int64_t ldq, int N, int M, int K, const Epi& epi,
+                  cudaStream_t st, GemmTile* used = nullptr) {
+  GemmProblem pr;
+  pr.P = P;
+  pr.ldp = ldp;
+  pr.p_group_rows = N;
+  pr.p_total_rows = N;
+  pr.Q[0] = Q;
+  pr.ldq = ldq;
+  pr.G = 1;
+  pr.M = M;
+  pr.K = K;
+  const GemmTile tile = gemm_f64_choose(N, N, 1, M);
+  GemmArgs a;
+  TKM_TRY(gemm_f64_make_args(pr, tile, &a));
+  a.N = N;
+  a.nslots = nullptr;
+  if (used) *used = tile;
+  return gemm_f64_launch(a, tile, 1, epi, st);
 }
 
 }  // namespace tkm

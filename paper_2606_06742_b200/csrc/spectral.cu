@@ -99,11 +99,10 @@ static int syevd_inplace(double* A, int64_t lda, int64_t n, double* W, cudaStrea
 
 static int dgemm_nt(const double* P, int64_t ldp, const double* Q, int64_t ldq, double* Dt, int64_t ldd,
                     int64_t N, int64_t M, int64_t K, cudaStream_t st) {
-  if ((ldp & 1) || (ldq & 1) || (ldd & 1) || ((uintptr_t)P & 15) || ((uintptr_t)Q & 15) || ((uintptr_t)Dt & 15))
-    return set_error(TKM_EINVAL, "dgemm_nt: operands must be 16-byte aligned with even leading dimensions");
-  GemmOperands g{P, ldp, Q, ldq, (int)N, (int)M, (int)K};
-  StoreEpi epi{Dt, ldd, 1.0};
-  return gemm_f64_dispatch(g, epi, st);
+  if ((ldd & 1) || ((uintptr_t)Dt & 15))
+    return set_error(TKM_EINVAL, "dgemm_nt: output must be 16-byte aligned with an even leading dimension");
+  StoreEpi epi{Dt, ldd, 0, 1.0};
+  return gemm_f64_once(P, ldp, Q, ldq, (int)N, (int)M, (int)K, epi, st);
 }
 
 // Finish a handle whose Ut ([r][ldn], rows = orthonormal eigenvectors) and lam are in place.
@@ -272,11 +271,3 @@ extern "C" int tkm_spectral_get_u(const tkm_spectral* s, double* U_out, void* st
   return transpose_scale_f64(s->Ut.as<double>(), s->ldn, s->r, s->n, nullptr, U_out, s->r, (cudaStream_t)stream);
 }
 
-extern "C" int tkm_dgemm_nt(const double* P, int64_t ldp, const double* Q, int64_t ldq, double* Dt, int64_t ldd,
-                            int64_t N, int64_t M, int64_t K, void* stream) {
-  using namespace tkm;
-  if (!P || !Q || !Dt || N <= 0 || M <= 0 || K <= 0 || ldp < K || ldq < K || ldd < M)
-    return set_error(TKM_EINVAL, "tkm_dgemm_nt: bad arguments");
-  TKM_TRY(device_check());
-  return dgemm_nt(P, ldp, Q, ldq, Dt, ldd, N, M, K, (cudaStream_t)stream);
-}

@@ -13,9 +13,15 @@
 //           da = S (rho - dbeta0 c u1); a+ = abar - da; gradient restart; next Nesterov extrapolation
 //
 // State lives in spectral coordinates a = U^T alpha, one column per ROW ("slot") so that a column's
-// vector is contiguous.  Converged columns are frozen by the update kernel and compacted out of the
-// GEMM batch by the host every `check_every` iterations (hole filling: live slots from the tail move
-// into the holes; finished rows are first copied to the result array).
+// vector is contiguous.  Several independent problems that share y, the folds and the lambda grid
+// (the bandwidths of a sigma grid: one spectral handle each) are swept together as GROUPS of one
+// launch (tkm_fit_path_multi), which keeps the SMs full when each group's live batch is narrow.
+//
+// Converged columns are frozen by the update kernel and compacted out of the GEMM batch ON THE DEVICE
+// every `check_every` iterations (hole filling: live slots from the tail move into the holes; finished
+// rows are first copied to the result array).  All kernels read the live-slot counts from device
+// memory, so the host never waits for the GPU inside a round: it enqueues the next batch of
+// iterations first and only then reads the previous batch's counts (an upper bound for the grids).
 #include <algorithm>
 #include <cmath>
 #include <new>
@@ -42,48 +48,59 @@ __device__ __forceinline__ double psi_dev(int loss, double y, double f, double s
   }
 }
 
+// Per-group device pointers (one group = one spectral handle, e.g. one bandwidth of a sigma grid).
+struct GroupPtrs {
+  const double* lam[GEMM_MAX_GROUPS];   // [ldr] eigenvalues
+  const double* u1[GEMM_MAX_GROUPS];    // [ldr] U^T 1
+  double* a_out[GEMM_MAX_GROUPS];       // [B][ldr] result rows of the group's path
+  double thin[GEMM_MAX_GROUPS];         // n - ||u1||^2 (0 for a full orthogonal U)
+};
+
+// Index conventions: B columns per group; "gc" = g*B + column, "gs" = g*B + slot.
+
 // ---- GEMM-A epilogue (S5): loss derivative, Zt store, per-CTA column sums ------------------------
 struct LossEpi {
   const double* y;           // [n]
   const int32_t* foldid;     // [n]
-  const int32_t* col_of_slot;
-  const double* bbar;        // [B] by column
+  const int32_t* col_of_slot;   // [G*B] by gs -> column
+  const double* bbar;        // [G*B] by gc
   const double* col_nc;      // [B]
   const double* col_tau;     // [B]
   const int32_t* col_v;      // [B]
-  int loss;
+  int B, loss;
   double smooth;
-  double* Zt;                // [slots][ldz]
+  double* Zt;                // [G*B][ldz] by gs
   int64_t ldz;
-  double* gpart;             // [m blocks][ldpart] by slot
+  double* gpart;             // [m blocks][ldpart] by gs
   int64_t ldpart;
-  template <int BN, int BM, int WARPS_N, int WARPS_M, int TN, int TM>
-  __device__ __forceinline__ void run(double (&acc)[TN][TM][2], int n_blk0, int m_blk0, int warp_n,
-                                      int warp_m, int lane, int N, int M, double* scratch) const {
-    constexpr int WN = BN / WARPS_N, WM = BM / WARPS_M;
+  template <class Cfg>
+  __device__ __forceinline__ void run(double (&acc)[Cfg::TN][Cfg::TM][2], int n_blk0, int m_blk0, int warp_n,
+                                      int warp_m, int lane, int N, int M, int grp, double* scratch) const {
+    constexpr int TN = Cfg::TN, TM = Cfg::TM;
     double yv[TM][2];
     int fv[TM][2];
 #pragma unroll
     for (int j = 0; j < TM; ++j)
 #pragma unroll
       for (int e = 0; e < 2; ++e) {
-        const int m = m_blk0 + warp_m * WM + j * 8 + 2 * (lane & 3) + e;
+        const int m = m_blk0 + (warp_m * TM + j) * 8 + 2 * (lane & 3) + e;
         yv[j][e] = (m < M) ? y[m] : 0.0;
         fv[j][e] = (m < M) ? foldid[m] : -1;
       }
+    const int g0 = grp * B;
     double colsum[TN];
 #pragma unroll
     for (int i = 0; i < TN; ++i) {
       colsum[i] = 0.0;
-      const int slot = n_blk0 + warp_n * WN + i * 8 + (lane >> 2);
+      const int slot = n_blk0 + (warp_n * TN + i) * 8 + (lane >> 2);
       if (slot >= N) continue;
-      const int col = col_of_slot[slot];
-      const double bb = bbar[col], inv_nc = 1.0 / col_nc[col], tau = col_tau[col];
+      const int col = col_of_slot[g0 + slot];
+      const double bb = bbar[g0 + col], inv_nc = 1.0 / col_nc[col], tau = col_tau[col];
       const int v = col_v[col];
-      double* zrow = Zt + (int64_t)slot * ldz;
+      double* zrow = Zt + (int64_t)(g0 + slot) * ldz;
 #pragma unroll
       for (int j = 0; j < TM; ++j) {
-        const int m = m_blk0 + warp_m * WM + j * 8 + 2 * (lane & 3);
+        const int m = m_blk0 + (warp_m * TM + j) * 8 + 2 * (lane & 3);
         double z[2];
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
@@ -98,52 +115,55 @@ struct LossEpi {
       }
     }
     double tot;
-    if (cta_row_reduce<BN, WARPS_N, WARPS_M, TN>(colsum, warp_n, warp_m, lane, scratch, tot)) {
+    if (cta_row_reduce<Cfg>(colsum, warp_n, warp_m, lane, scratch, tot)) {
       const int slot = n_blk0 + (int)threadIdx.x;
-      if (slot < N) gpart[(int64_t)blockIdx.x * ldpart + slot] = tot;
+      if (slot < N) gpart[(int64_t)blockIdx.x * ldpart + g0 + slot] = tot;
     }
   }
 };
 
 // ---- GEMM-B epilogue (S6): rho = zeta + 2 lam abar, partial sums for q and ||rho||^2 -------------
 struct SpecEpi {
-  const double* lam;         // [ldr] eigenvalues
-  const double* u1;          // [ldr]
-  const int32_t* col_of_slot;
+  GroupPtrs gp;
+  const int32_t* col_of_slot;   // [G*B]
   const double* col_lam;     // [B]
   const double* col_c;       // [B] c = curv / n_c
-  const double* Abar;        // [slots][lda]
+  int B;
+  const double* Abar;        // [G*B][lda] by gs
   int64_t lda;
-  double* Rho;               // [slots][lda]
-  double* qpart;             // [m blocks][ldpart]
+  double* Rho;               // [G*B][lda] by gs
+  double* qpart;             // [m blocks][ldpart] by gs
   double* r2part;
   int64_t ldpart;
-  template <int BN, int BM, int WARPS_N, int WARPS_M, int TN, int TM>
-  __device__ __forceinline__ void run(double (&acc)[TN][TM][2], int n_blk0, int m_blk0, int warp_n,
-                                      int warp_m, int lane, int N, int M, double* scratch) const {
-    constexpr int WN = BN / WARPS_N, WM = BM / WARPS_M;
+  template <class Cfg>
+  __device__ __forceinline__ void run(double (&acc)[Cfg::TN][Cfg::TM][2], int n_blk0, int m_blk0, int warp_n,
+                                      int warp_m, int lane, int N, int M, int grp, double* scratch) const {
+    constexpr int TN = Cfg::TN, TM = Cfg::TM;
+    const double* lam = gp.lam[grp];
+    const double* u1 = gp.u1[grp];
     double lv[TM][2], lu[TM][2];   // Lam_i and Lam_i u1_i
 #pragma unroll
     for (int j = 0; j < TM; ++j)
 #pragma unroll
       for (int e = 0; e < 2; ++e) {
-        const int i = m_blk0 + warp_m * WM + j * 8 + 2 * (lane & 3) + e;
+        const int i = m_blk0 + (warp_m * TM + j) * 8 + 2 * (lane & 3) + e;
         lv[j][e] = (i < M) ? lam[i] : 0.0;
         lu[j][e] = (i < M) ? lam[i] * u1[i] : 0.0;
       }
+    const int g0 = grp * B;
     double qs[TN], r2[TN];
 #pragma unroll
     for (int t = 0; t < TN; ++t) {
       qs[t] = r2[t] = 0.0;
-      const int slot = n_blk0 + warp_n * WN + t * 8 + (lane >> 2);
+      const int slot = n_blk0 + (warp_n * TN + t) * 8 + (lane >> 2);
       if (slot >= N) continue;
-      const int col = col_of_slot[slot];
+      const int col = col_of_slot[g0 + slot];
       const double two_lam = 2.0 * col_lam[col], cc = col_c[col];
-      const double* arow = Abar + (int64_t)slot * lda;
-      double* rrow = Rho + (int64_t)slot * lda;
+      const double* arow = Abar + (int64_t)(g0 + slot) * lda;
+      double* rrow = Rho + (int64_t)(g0 + slot) * lda;
 #pragma unroll
       for (int j = 0; j < TM; ++j) {
-        const int i = m_blk0 + warp_m * WM + j * 8 + 2 * (lane & 3);
+        const int i = m_blk0 + (warp_m * TM + j) * 8 + 2 * (lane & 3);
         double rho[2] = {0.0, 0.0};
         if (i + 1 < M) {
           const double2 ab = *reinterpret_cast<const double2*>(arow + i);
@@ -163,107 +183,117 @@ struct SpecEpi {
       }
     }
     double tot;
-    if (cta_row_reduce<BN, WARPS_N, WARPS_M, TN>(qs, warp_n, warp_m, lane, scratch, tot)) {
+    if (cta_row_reduce<Cfg>(qs, warp_n, warp_m, lane, scratch, tot)) {
       const int slot = n_blk0 + (int)threadIdx.x;
-      if (slot < N) qpart[(int64_t)blockIdx.x * ldpart + slot] = tot;
+      if (slot < N) qpart[(int64_t)blockIdx.x * ldpart + g0 + slot] = tot;
     }
-    if (cta_row_reduce<BN, WARPS_N, WARPS_M, TN>(r2, warp_n, warp_m, lane, scratch, tot)) {
+    if (cta_row_reduce<Cfg>(r2, warp_n, warp_m, lane, scratch, tot)) {
       const int slot = n_blk0 + (int)threadIdx.x;
-      if (slot < N) r2part[(int64_t)blockIdx.x * ldpart + slot] = tot;
+      if (slot < N) r2part[(int64_t)blockIdx.x * ldpart + g0 + slot] = tot;
     }
   }
 };
 
 // ---- per-round initialisation (S3, G4): constants c, s; a' = a; abar = a; r = 1 ------------------
 struct RoundArgs {
-  int r;
+  int r, B;
   int64_t lda;
-  const double* lam;
-  const double* u1;
-  double thin, curv;
-  const double* col_lam;
-  const double* col_nc;
-  double* col_c;
-  double* col_s;
-  const double* a_out;   // [B][lda] solution so far (by column)
-  double *A, *Aprev, *Abar;
-  double *beta, *beta_prev, *bbar, *rk;
-  int32_t *done, *iters_round, *col_of_slot;
+  GroupPtrs gp;
+  double curv;
+  const double* col_lam;   // [B]
+  const double* col_nc;    // [B]
+  double* col_c;           // [B]
+  double* col_s;           // [G*B]
+  double *A, *Aprev, *Abar;   // [G*B][lda]
+  double *beta, *beta_prev, *bbar, *rk;   // [G*B]
+  int32_t *done, *iters_round, *col_of_slot;   // [G*B]
+  int32_t* nslots;         // [G]
 };
 
 __global__ void __launch_bounds__(256) init_round_kernel(RoundArgs p) {
   __shared__ double red[32];
-  const int col = blockIdx.x;
+  const int col = blockIdx.x, grp = blockIdx.y;
+  const int gc = grp * p.B + col;
+  const double* lam = p.gp.lam[grp];
+  const double* u1 = p.gp.u1[grp];
   const double lamc = p.col_lam[col], c = p.curv / p.col_nc[col];
   double acc = 0.0;
-  const int64_t off = (int64_t)col * p.lda;
+  const double* src = p.gp.a_out[grp] + (int64_t)col * p.lda;
+  const int64_t off = (int64_t)gc * p.lda;
   for (int i = threadIdx.x; i < p.r; i += blockDim.x) {
-    const double u = p.u1[i];
-    acc += u * u / (2.0 * lamc + c * p.lam[i]);
-    const double a = p.a_out[off + i];
+    const double u = u1[i];
+    acc += u * u / (2.0 * lamc + c * lam[i]);
+    const double a = src[i];
     p.A[off + i] = a;
     p.Aprev[off + i] = a;
     p.Abar[off + i] = a;
   }
   acc = block_sum(acc, red);
   if (threadIdx.x == 0) {
-    p.col_c[col] = c;
-    p.col_s[col] = c * p.thin + 2.0 * lamc * c * acc;   // Schur complement s (G1)
-    p.beta_prev[col] = p.beta[col];
-    p.bbar[col] = p.beta[col];
-    p.rk[col] = 1.0;
-    p.done[col] = 0;
-    p.iters_round[col] = 0;
-    p.col_of_slot[col] = col;
+    if (grp == 0) p.col_c[col] = c;
+    p.col_s[gc] = c * p.gp.thin[grp] + 2.0 * lamc * c * acc;   // Schur complement s (G1)
+    p.beta_prev[gc] = p.beta[gc];
+    p.bbar[gc] = p.beta[gc];
+    p.rk[gc] = 1.0;
+    p.done[gc] = 0;
+    p.iters_round[gc] = 0;
+    p.col_of_slot[gc] = col;
+    if (col == 0) p.nslots[grp] = p.B;
   }
 }
 
 // ---- S7: per-column update, stop test, restart, next extrapolation --------------------------------
 struct UpdateArgs {
-  int r, n, nblkA, nblkB, restart, maxit;
+  int r, n, B, nblkA, nblkB, restart, maxit;
   int64_t lda, ldpart;
   double tol;
-  const double* lam;
-  const double* u1;
-  const int32_t* col_of_slot;
-  const double *col_lam, *col_c, *col_s, *col_nc;
+  GroupPtrs gp;
+  const int32_t* nslots;       // [G]
+  const int32_t* col_of_slot;  // [G*B]
+  const double *col_lam, *col_c, *col_nc;   // [B]
+  const double* col_s;         // [G*B]
   const double *gpart, *qpart, *r2part;
   const double* Rho;
   double *A, *Aprev, *Abar;
-  double *beta, *beta_prev, *bbar, *rk, *kkt;
-  int32_t *done, *iters, *iters_round, *flags;
+  double *beta, *beta_prev, *bbar, *rk, *kkt;   // [G*B]
+  int32_t *done, *iters, *iters_round, *flags;  // [G*B]
 };
 
 __global__ void __launch_bounds__(256) update_kernel(UpdateArgs p) {
   __shared__ double red[32];
-  const int slot = blockIdx.x;
-  const int col = p.col_of_slot[slot];
-  if (p.done[col]) return;   // frozen until the host compacts it away
+  const int slot = blockIdx.x, grp = blockIdx.y;
+  if (slot >= p.nslots[grp]) return;
+  const int gs = grp * p.B + slot;
+  const int col = p.col_of_slot[gs];
+  const int gc = grp * p.B + col;
+  if (p.done[gc]) return;   // frozen until the next compaction removes it
+  const double* lam = p.gp.lam[grp];
+  const double* u1 = p.gp.u1[grp];
   double g0 = 0.0, qd = 0.0, r2 = 0.0;
-  for (int b = threadIdx.x; b < p.nblkA; b += blockDim.x) g0 += p.gpart[(int64_t)b * p.ldpart + slot];
+  for (int b = threadIdx.x; b < p.nblkA; b += blockDim.x) g0 += p.gpart[(int64_t)b * p.ldpart + gs];
   for (int b = threadIdx.x; b < p.nblkB; b += blockDim.x) {
-    qd += p.qpart[(int64_t)b * p.ldpart + slot];
-    r2 += p.r2part[(int64_t)b * p.ldpart + slot];
+    qd += p.qpart[(int64_t)b * p.ldpart + gs];
+    r2 += p.r2part[(int64_t)b * p.ldpart + gs];
   }
   g0 = block_sum(g0, red);
   qd = block_sum(qd, red);
   r2 = block_sum(r2, red);
-  const double lamc = p.col_lam[col], c = p.col_c[col], s = p.col_s[col], nc = p.col_nc[col];
+  const double lamc = p.col_lam[col], c = p.col_c[col], s = p.col_s[gc], nc = p.col_nc[col];
   const double dbeta = (g0 - c * qd) / s;                            // PAPER.md:208 (Alg.1 l.17)
   const double kkt = fmax(fabs(g0), nc * sqrt(r2) / sqrt((double)p.n));   // reading G6
-  const double beta = p.beta[col], bbar = p.bbar[col];
+  const double beta = p.beta[gc], bbar = p.bbar[gc];
   const double beta_new = bbar - dbeta;
-  const int64_t off = (int64_t)slot * p.lda;
+  const int64_t off = (int64_t)gs * p.lda;
   double g = 0.0;
   for (int i = threadIdx.x; i < p.r; i += blockDim.x) {
-    const double S = 1.0 / (2.0 * lamc + c * p.lam[i]);
-    const double da = S * (p.Rho[off + i] - dbeta * c * p.u1[i]);    // PAPER.md:207 (Alg.1 l.16)
+    const double S = 1.0 / (2.0 * lamc + c * lam[i]);
+    const double da = S * (p.Rho[off + i] - dbeta * c * u1[i]);      // PAPER.md:207 (Alg.1 l.16)
     const double an = p.Abar[off + i] - da;                           // PAPER.md:212 (Alg.1 l.19)
     g += da * (an - p.A[off + i]);
     p.Aprev[off + i] = an;   // a' is dead once abar has been formed: use it as scratch for a+
   }
   g = block_sum(g, red) + dbeta * (beta_new - beta);
-  double rk = p.rk[col];
+  double rk = p.rk[gc];
   rk = 0.5 * (1.0 + sqrt(1.0 + 4.0 * rk * rk));                       // PAPER.md:199 (Alg.1 l.12)
   if (p.restart && g > 0.0) rk = 1.0;                                 // gradient restart
   const double rk_next = 0.5 * (1.0 + sqrt(1.0 + 4.0 * rk * rk));
@@ -275,53 +305,158 @@ __global__ void __launch_bounds__(256) update_kernel(UpdateArgs p) {
     p.Abar[off + i] = an + mu * (an - aold);
   }
   if (threadIdx.x == 0) {
-    p.beta_prev[col] = beta;
-    p.beta[col] = beta_new;
-    p.bbar[col] = beta_new + mu * (beta_new - beta);
-    p.rk[col] = rk;
-    p.kkt[col] = kkt;
-    p.iters[col] += 1;
-    const int itr = p.iters_round[col] + 1;
-    p.iters_round[col] = itr;
+    p.beta_prev[gc] = beta;
+    p.beta[gc] = beta_new;
+    p.bbar[gc] = beta_new + mu * (beta_new - beta);
+    p.rk[gc] = rk;
+    p.kkt[gc] = kkt;
+    p.iters[gc] += 1;
+    const int itr = p.iters_round[gc] + 1;
+    p.iters_round[gc] = itr;
     if (kkt <= p.tol) {
-      p.done[col] = 1;
+      p.done[gc] = 1;
     } else if (itr >= p.maxit) {
-      p.done[col] = 1;
-      p.flags[col] = 1;
+      p.done[gc] = 1;
+      p.flags[gc] = 1;
     }
   }
 }
 
-// rows: dst_base[dst_idx[k]][:] = src_base[src_idx[k]][:] for k < count (one CTA per k and per array)
-struct RowCopy {
-  const double* src;
-  double* dst;
+// ---- device-side compaction of converged columns --------------------------------------------------
+// plan (one CTA per group): finished slots in slot order -> fin_list; live slots at or beyond the new
+// count `nact` in slot order -> tail_list.  The first nholes entries of fin_list are exactly the
+// finished slots below nact (the holes), and there are as many tail entries as holes.
+struct CompactArgs {
+  int B, r;
+  int64_t lda;
+  GroupPtrs gp;
+  int32_t* nslots;          // [G]   in: live slots before, out: after
+  int32_t* col_of_slot;     // [G*B]
+  const int32_t* done;      // [G*B] by gc
+  int32_t* fin_list;        // [G*B]
+  int32_t* tail_list;       // [G*B]
+  int32_t* counts;          // [G][4]: nfin, nholes, nact, previous nslots
+  double *A, *Aprev, *Abar;
 };
-__global__ void row_copy_kernel(RowCopy c0, RowCopy c1, RowCopy c2, int narr, const int32_t* __restrict__ src_idx,
-                                const int32_t* __restrict__ dst_idx, int64_t ld, int len) {
-  const RowCopy c = blockIdx.y == 0 ? c0 : (blockIdx.y == 1 ? c1 : c2);
-  const int64_t so = (int64_t)src_idx[blockIdx.x] * ld, dof = (int64_t)dst_idx[blockIdx.x] * ld;
-  for (int i = threadIdx.x; i < len; i += blockDim.x) c.dst[dof + i] = c.src[so + i];
-  (void)narr;
+
+__global__ void __launch_bounds__(1024) compact_plan_kernel(CompactArgs p) {
+  __shared__ int wsum[2][32];
+  __shared__ int run[2];
+  __shared__ int s_nact;
+  const int grp = blockIdx.x, g0 = grp * p.B;
+  const int ns = p.nslots[grp];
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  // pass 1: number of live slots
+  int live = 0;
+  for (int sl = tid; sl < ns; sl += blockDim.x) live += p.done[g0 + p.col_of_slot[g0 + sl]] ? 0 : 1;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) live += __shfl_xor_sync(0xffffffffu, live, o);
+  if (lane == 0) wsum[0][w] = live;
+  if (tid == 0) run[0] = run[1] = 0;
+  __syncthreads();
+  if (tid == 0) {
+    int t = 0;
+    for (int i = 0; i < (int)(blockDim.x >> 5); ++i) t += wsum[0][i];
+    s_nact = t;
+  }
+  __syncthreads();
+  const int nact = s_nact;
+  // pass 2: ordered lists by chunked ballot scans
+  for (int base = 0; base < ns; base += blockDim.x) {
+    const int sl = base + tid;
+    int fin = 0, tail = 0;
+    if (sl < ns) {
+      fin = p.done[g0 + p.col_of_slot[g0 + sl]] ? 1 : 0;
+      tail = (!fin && sl >= nact) ? 1 : 0;
+    }
+    const unsigned bf = __ballot_sync(0xffffffffu, fin), bt = __ballot_sync(0xffffffffu, tail);
+    const unsigned below = (1u << lane) - 1u;
+    const int pf = __popc(bf & below), pt = __popc(bt & below);
+    __syncthreads();   // wsum / run of the previous chunk have been consumed
+    if (lane == 0) {
+      wsum[0][w] = __popc(bf);
+      wsum[1][w] = __popc(bt);
+    }
+    __syncthreads();
+    int of = run[0], ot = run[1];
+    for (int i = 0; i < w; ++i) {
+      of += wsum[0][i];
+      ot += wsum[1][i];
+    }
+    if (fin) p.fin_list[g0 + of + pf] = sl;
+    if (tail) p.tail_list[g0 + ot + pt] = sl;
+    __syncthreads();
+    if (tid == 0) {
+      int tf = 0, tt = 0;
+      for (int i = 0; i < (int)(blockDim.x >> 5); ++i) {
+        tf += wsum[0][i];
+        tt += wsum[1][i];
+      }
+      run[0] += tf;
+      run[1] += tt;
+    }
+  }
+  __syncthreads();
+  if (tid == 0) {
+    p.counts[grp * 4 + 0] = run[0];   // nfin
+    p.counts[grp * 4 + 1] = run[1];   // nholes (= live slots beyond nact)
+    p.counts[grp * 4 + 2] = nact;
+    p.counts[grp * 4 + 3] = ns;
+    p.nslots[grp] = nact;
+  }
+}
+
+// apply (grid: finished-slot rank x group): save the finished row to the group's result array, then, if
+// the slot is a hole below nact, pull the matching live tail row (a, a', abar and its column id) in.
+__global__ void __launch_bounds__(256) compact_apply_kernel(CompactArgs p) {
+  const int k = blockIdx.x, grp = blockIdx.y, g0 = grp * p.B;
+  const int nfin = p.counts[grp * 4 + 0], nholes = p.counts[grp * 4 + 1];
+  if (k >= nfin) return;
+  const int sl = p.fin_list[g0 + k];
+  const int col = p.col_of_slot[g0 + sl];
+  const int64_t so = (int64_t)(g0 + sl) * p.lda;
+  double* dst = p.gp.a_out[grp] + (int64_t)col * p.lda;
+  for (int i = threadIdx.x; i < p.r; i += blockDim.x) dst[i] = p.A[so + i];
+  if (k >= nholes) return;
+  const int src = p.tail_list[g0 + k];
+  const int64_t to = (int64_t)(g0 + src) * p.lda;
+  __syncthreads();   // the finished row has been read by every thread before it is overwritten
+  for (int i = threadIdx.x; i < p.r; i += blockDim.x) {
+    p.A[so + i] = p.A[to + i];
+    p.Aprev[so + i] = p.Aprev[to + i];
+    p.Abar[so + i] = p.Abar[to + i];
+  }
+  if (threadIdx.x == 0) p.col_of_slot[g0 + sl] = p.col_of_slot[g0 + src];
 }
 
 static double curvature_of(tkm_loss loss, double smooth) {
   return loss == TKM_LOSS_LOGISTIC ? 0.25 : 1.0 / (2.0 * smooth);   // 1/kappa, kappa = 2 delta
 }
 
+constexpr int POLL_RING = 3;   // batches whose poll results may be in flight
+
 }  // namespace tkm
 
 using namespace tkm;
 
-extern "C" int tkm_fit_path(const tkm_spectral* s, const void* y, tkm_loss loss, const tkm_loss_opts* opts,
-                            const double* lambdas, int32_t L, const int32_t* foldid, int32_t V, double tol,
-                            int32_t maxit, const tkm_path* warm, tkm_path** out, void* stream) {
+extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, const void* y, tkm_loss loss,
+                                  const tkm_loss_opts* opts, const double* lambdas, int32_t L, const int32_t* foldid,
+                                  int32_t V, double tol, int32_t maxit, const tkm_path* const* warm, tkm_path** out,
+                                  void* stream) {
   if (!out) return set_error(TKM_EINVAL, "tkm_fit_path: out is NULL");
-  *out = nullptr;
-  if (!s || !y || !opts || !lambdas || !foldid) return set_error(TKM_EINVAL, "tkm_fit_path: NULL argument");
+  if (G < 1 || G > GEMM_MAX_GROUPS) return set_error(TKM_EINVAL, "tkm_fit_path_multi: need 1 <= G <= %d", GEMM_MAX_GROUPS);
+  for (int g = 0; g < G; ++g) out[g] = nullptr;
+  if (!specs || !y || !opts || !lambdas || !foldid) return set_error(TKM_EINVAL, "tkm_fit_path: NULL argument");
+  for (int g = 0; g < G; ++g)
+    if (!specs[g]) return set_error(TKM_EINVAL, "tkm_fit_path: NULL spectral handle");
+  const tkm_spectral* s0 = specs[0];
+  for (int g = 1; g < G; ++g)
+    if (specs[g]->n != s0->n || specs[g]->r != s0->r || specs[g]->ldr != s0->ldr || specs[g]->ldn != s0->ldn ||
+        specs[g]->sweep_dt != s0->sweep_dt)
+      return set_error(TKM_EINVAL, "tkm_fit_path_multi: all spectral handles must share n, r and the sweep precision");
   if (loss != TKM_LOSS_HINGE && loss != TKM_LOSS_LOGISTIC && loss != TKM_LOSS_QUANTILE)
     return set_error(TKM_EINVAL, "tkm_fit_path: unknown loss %d", (int)loss);
-  if (L < 1 || V < 2 || V > s->n) return set_error(TKM_EINVAL, "tkm_fit_path: need L >= 1 and 2 <= V <= n");
+  if (L < 1 || V < 2 || V > s0->n) return set_error(TKM_EINVAL, "tkm_fit_path: need L >= 1 and 2 <= V <= n");
   if (!(tol > 0.0) || maxit < 1) return set_error(TKM_EINVAL, "tkm_fit_path: need tol > 0 and maxit >= 1");
   for (int l = 0; l < L; ++l)
     if (!(lambdas[l] > 0.0)) return set_error(TKM_EINVAL, "tkm_fit_path: lambda[%d] = %g must be > 0", l, lambdas[l]);
@@ -336,14 +471,17 @@ extern "C" int tkm_fit_path(const tkm_spectral* s, const void* y, tkm_loss loss,
   if (rounds < 1) return set_error(TKM_EINVAL, "tkm_fit_path: rounds must be >= 1");
   if (loss != TKM_LOSS_LOGISTIC && (!(opts->smooth0 > 0.0) || !(opts->eta > 0.0 && opts->eta <= 1.0)))
     return set_error(TKM_EINVAL, "tkm_fit_path: need smooth0 > 0 and 0 < eta <= 1");
-  if (s->sweep_dt != TKM_F64) return set_error(TKM_ENOTIMPL, "tkm_fit_path: only the FP64 sweep is built");
+  if (s0->sweep_dt != TKM_F64) return set_error(TKM_ENOTIMPL, "tkm_fit_path: only the FP64 sweep is built");
   TKM_TRY(device_check());
   cudaStream_t st = (cudaStream_t)stream;
-  const int64_t n = s->n, r = s->r, ldr = s->ldr, ldn = s->ldn;
+  const int64_t n = s0->n, r = s0->r, ldr = s0->ldr, ldn = s0->ldn;
   const int64_t B64 = (int64_t)T * L * (V + 1);
-  if (B64 > (1 << 24)) return set_error(TKM_EINVAL, "tkm_fit_path: too many columns");
-  const int B = (int)B64;
-  if (warm && (warm->spec != s || warm->B != B)) return set_error(TKM_EINVAL, "tkm_fit_path: warm path has another shape");
+  if (B64 * G > (1 << 22)) return set_error(TKM_EINVAL, "tkm_fit_path: too many columns");
+  const int B = (int)B64, GB = B * G;
+  if (warm)
+    for (int g = 0; g < G; ++g)
+      if (!warm[g] || warm[g]->spec != specs[g] || warm[g]->B != B)
+        return set_error(TKM_EINVAL, "tkm_fit_path: warm path has another shape");
 
   // fold sizes, every fold non-empty
   std::vector<int64_t> fsize(V, 0);
@@ -365,26 +503,21 @@ extern "C" int tkm_fit_path(const tkm_spectral* s, const void* y, tkm_loss loss,
     }
   }
 
-  tkm_path* p = new (std::nothrow) tkm_path();
-  if (!p) return set_error(TKM_ENOMEM, "out of host memory");
+  // the paths (one per group); freed by the guard unless we reach the end
   struct Guard {
-    tkm_path* p;
+    tkm_path** out;
+    int G;
     cudaStream_t st;
+    bool armed = true;
     ~Guard() {
-      if (p) {
-        cudaStreamSynchronize(st);
-        delete p;
+      if (!armed) return;
+      cudaStreamSynchronize(st);
+      for (int g = 0; g < G; ++g) {
+        delete out[g];
+        out[g] = nullptr;
       }
     }
-  } guard{p, st};
-  p->spec = s;
-  p->L = L;
-  p->V = V;
-  p->T = T;
-  p->B = B;
-  p->loss = loss;
-  p->lambdas.assign(lambdas, lambdas + L);
-  if (loss == TKM_LOSS_QUANTILE) p->taus.assign(opts->taus, opts->taus + T);
+  } guard{out, G, st};
 
   // column table, c = (t (V+1) + v) L + l
   std::vector<double> h_lam(B), h_tau(B), h_nc(B);
@@ -398,182 +531,260 @@ extern "C" int tkm_fit_path(const tkm_spectral* s, const void* y, tkm_loss loss,
         h_v[c] = v;
         h_nc[c] = (double)(v < V ? n - fsize[v] : n);   // divisor n_c (G3)
       }
-  TKM_TRY(p->a.alloc((size_t)B * ldr * sizeof(double), true, st));
-  TKM_TRY(p->beta0.alloc((size_t)B * sizeof(double), true, st));
-  TKM_TRY(p->col_lam.alloc((size_t)B * sizeof(double), false, st));
-  TKM_TRY(p->col_tau.alloc((size_t)B * sizeof(double), false, st));
-  TKM_TRY(p->col_nc.alloc((size_t)B * sizeof(double), false, st));
-  TKM_TRY(p->col_v.alloc((size_t)B * sizeof(int32_t), false, st));
-  TKM_CUDA(cudaMemcpyAsync(p->col_lam.p, h_lam.data(), B * sizeof(double), cudaMemcpyHostToDevice, st));
-  TKM_CUDA(cudaMemcpyAsync(p->col_tau.p, h_tau.data(), B * sizeof(double), cudaMemcpyHostToDevice, st));
-  TKM_CUDA(cudaMemcpyAsync(p->col_nc.p, h_nc.data(), B * sizeof(double), cudaMemcpyHostToDevice, st));
-  TKM_CUDA(cudaMemcpyAsync(p->col_v.p, h_v.data(), B * sizeof(int32_t), cudaMemcpyHostToDevice, st));
-  if (warm) {
-    TKM_CUDA(cudaMemcpyAsync(p->a.p, warm->a.p, (size_t)B * ldr * sizeof(double), cudaMemcpyDeviceToDevice, st));
-    TKM_CUDA(cudaMemcpyAsync(p->beta0.p, warm->beta0.p, (size_t)B * sizeof(double), cudaMemcpyDeviceToDevice, st));
+  GroupPtrs gp;
+  memset(&gp, 0, sizeof(gp));
+  for (int g = 0; g < G; ++g) {
+    tkm_path* p = new (std::nothrow) tkm_path();
+    if (!p) return set_error(TKM_ENOMEM, "out of host memory");
+    out[g] = p;
+    p->spec = specs[g];
+    p->L = L;
+    p->V = V;
+    p->T = T;
+    p->B = B;
+    p->loss = loss;
+    p->lambdas.assign(lambdas, lambdas + L);
+    if (loss == TKM_LOSS_QUANTILE) p->taus.assign(opts->taus, opts->taus + T);
+    TKM_TRY(p->a.alloc((size_t)B * ldr * sizeof(double), true, st));
+    TKM_TRY(p->beta0.alloc((size_t)B * sizeof(double), true, st));
+    TKM_TRY(p->col_lam.alloc((size_t)B * sizeof(double), false, st));
+    TKM_TRY(p->col_tau.alloc((size_t)B * sizeof(double), false, st));
+    TKM_TRY(p->col_nc.alloc((size_t)B * sizeof(double), false, st));
+    TKM_TRY(p->col_v.alloc((size_t)B * sizeof(int32_t), false, st));
+    TKM_CUDA(cudaMemcpyAsync(p->col_lam.p, h_lam.data(), B * sizeof(double), cudaMemcpyHostToDevice, st));
+    TKM_CUDA(cudaMemcpyAsync(p->col_tau.p, h_tau.data(), B * sizeof(double), cudaMemcpyHostToDevice, st));
+    TKM_CUDA(cudaMemcpyAsync(p->col_nc.p, h_nc.data(), B * sizeof(double), cudaMemcpyHostToDevice, st));
+    TKM_CUDA(cudaMemcpyAsync(p->col_v.p, h_v.data(), B * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    gp.lam[g] = specs[g]->lam.as<double>();
+    gp.u1[g] = specs[g]->u1.as<double>();
+    gp.a_out[g] = p->a.as<double>();
+    gp.thin[g] = specs[g]->thin;
   }
+  const tkm_path* p0 = out[0];   // the column tables are identical in every group: use group 0's
 
-  // working set
+  // working set (all groups stacked: row / entry g*B + slot or g*B + column)
   DevBuf A, Aprev, Abar, Rho, Zt, gpart, qpart, r2part, d_fold;
-  DevBuf col_c, col_s, beta_prev, bbar, rk, kkt, done, iters, iters_round, flags, col_of_slot, idx_src, idx_dst;
-  TKM_TRY(A.alloc((size_t)B * ldr * sizeof(double), true, st));
-  TKM_TRY(Aprev.alloc((size_t)B * ldr * sizeof(double), true, st));
-  TKM_TRY(Abar.alloc((size_t)B * ldr * sizeof(double), true, st));
-  TKM_TRY(Rho.alloc((size_t)B * ldr * sizeof(double), true, st));
-  TKM_TRY(Zt.alloc((size_t)B * ldn * sizeof(double), true, st));
-  const int64_t nblkA_max = ceil_div(n, 64), nblkB_max = ceil_div(r, 64);
-  const int64_t ldpart = round_up(B, 16);
-  TKM_TRY(gpart.alloc((size_t)nblkA_max * ldpart * sizeof(double), true, st));
-  TKM_TRY(qpart.alloc((size_t)nblkB_max * ldpart * sizeof(double), true, st));
-  TKM_TRY(r2part.alloc((size_t)nblkB_max * ldpart * sizeof(double), true, st));
+  DevBuf col_c, col_s, beta, beta_prev, bbar, rk, kkt, done, iters, iters_round, flags, col_of_slot;
+  DevBuf nslots, fin_list, tail_list, counts;
+  TKM_TRY(A.alloc((size_t)GB * ldr * sizeof(double), true, st));
+  TKM_TRY(Aprev.alloc((size_t)GB * ldr * sizeof(double), true, st));
+  TKM_TRY(Abar.alloc((size_t)GB * ldr * sizeof(double), true, st));
+  TKM_TRY(Rho.alloc((size_t)GB * ldr * sizeof(double), true, st));
+  TKM_TRY(Zt.alloc((size_t)GB * ldn * sizeof(double), true, st));
+  const int64_t nblk_max = ceil_div(std::max(n, r), 64);   // smallest BM of any tile configuration
+  const int64_t ldpart = round_up(GB, 16);
+  TKM_TRY(gpart.alloc((size_t)nblk_max * ldpart * sizeof(double), true, st));
+  TKM_TRY(qpart.alloc((size_t)nblk_max * ldpart * sizeof(double), true, st));
+  TKM_TRY(r2part.alloc((size_t)nblk_max * ldpart * sizeof(double), true, st));
   TKM_TRY(d_fold.alloc((size_t)n * sizeof(int32_t), false, st));
   TKM_CUDA(cudaMemcpyAsync(d_fold.p, foldid, n * sizeof(int32_t), cudaMemcpyHostToDevice, st));
-  for (DevBuf* b : {&col_c, &col_s, &beta_prev, &bbar, &rk, &kkt}) TKM_TRY(b->alloc((size_t)B * sizeof(double), true, st));
-  for (DevBuf* b : {&done, &iters, &iters_round, &flags, &col_of_slot, &idx_src, &idx_dst})
-    TKM_TRY(b->alloc((size_t)B * sizeof(int32_t), true, st));
-  PinBuf h_done, h_idx;
-  TKM_TRY(h_done.alloc((size_t)B * sizeof(int32_t)));
-  TKM_TRY(h_idx.alloc((size_t)2 * B * sizeof(int32_t)));
-  std::vector<int32_t> slot_col(B);
+  TKM_TRY(col_c.alloc((size_t)B * sizeof(double), true, st));
+  for (DevBuf* b : {&col_s, &beta, &beta_prev, &bbar, &rk, &kkt}) TKM_TRY(b->alloc((size_t)GB * sizeof(double), true, st));
+  for (DevBuf* b : {&done, &iters, &iters_round, &flags, &col_of_slot, &fin_list, &tail_list})
+    TKM_TRY(b->alloc((size_t)GB * sizeof(int32_t), true, st));
+  TKM_TRY(nslots.alloc((size_t)GEMM_MAX_GROUPS * sizeof(int32_t), true, st));
+  TKM_TRY(counts.alloc((size_t)GEMM_MAX_GROUPS * 4 * sizeof(int32_t), true, st));
+  if (warm)
+    for (int g = 0; g < G; ++g) {
+      TKM_CUDA(cudaMemcpyAsync(out[g]->a.p, warm[g]->a.p, (size_t)B * ldr * sizeof(double), cudaMemcpyDeviceToDevice, st));
+      TKM_CUDA(cudaMemcpyAsync(beta.as<double>() + (size_t)g * B, warm[g]->beta0.p, (size_t)B * sizeof(double),
+                               cudaMemcpyDeviceToDevice, st));
+    }
+  PinBuf h_ns;   // [POLL_RING][GEMM_MAX_GROUPS] live-slot counts read back after every compaction
+  TKM_TRY(h_ns.alloc((size_t)POLL_RING * GEMM_MAX_GROUPS * sizeof(int32_t)));
+
+  // events: one "poll landed" event per ring entry; optional GEMM sampling events per ring entry
+  struct Events {
+    cudaEvent_t poll[POLL_RING] = {}, pev[POLL_RING][3] = {};
+    ~Events() {
+      for (auto& e : poll)
+        if (e) cudaEventDestroy(e);
+      for (auto& row : pev)
+        for (auto& e : row)
+          if (e) cudaEventDestroy(e);
+    }
+  } ev;
+  for (auto& e : ev.poll) TKM_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+  if (opts->profile)
+    for (auto& row : ev.pev)
+      for (auto& e : row) TKM_CUDA(cudaEventCreate(&e));
+
+  // GEMM problems: A = abar x (U Lam)^T, B = Zt x (U^T)^T
+  GemmProblem prA, prB;
+  prA.P = Abar.as<double>();
+  prA.ldp = ldr;
+  prA.p_group_rows = B;
+  prA.p_total_rows = GB;
+  prA.ldq = ldr;
+  prA.G = G;
+  prA.M = (int)n;
+  prA.K = (int)r;
+  prB.P = Zt.as<double>();
+  prB.ldp = ldn;
+  prB.p_group_rows = B;
+  prB.p_total_rows = GB;
+  prB.ldq = ldn;
+  prB.G = G;
+  prB.M = (int)r;
+  prB.K = (int)n;
+  for (int g = 0; g < G; ++g) {
+    prA.Q[g] = specs[g]->UL.as<double>();
+    prB.Q[g] = specs[g]->Ut.as<double>();
+  }
+  GemmArgs argsA, argsB;
+  GemmTile tileA{-1, 0, 0}, tileB{-1, 0, 0};
 
   const int check_every = opts->check_every > 0 ? opts->check_every : 16;
   const int restart = opts->restart ? 1 : 0;
-  // optional sampling of the two contractions with CUDA events: the first iteration after every
-  // poll (all `nslots` columns are live there), read back at the next poll (bench.py `roofline`)
-  cudaEvent_t pev[3] = {nullptr, nullptr, nullptr};
-  struct PevGuard {
-    cudaEvent_t* e;
-    ~PevGuard() {
-      for (int i = 0; i < 3; ++i)
-        if (e[i]) cudaEventDestroy(e[i]);
-    }
-  } pev_guard{pev};
-  if (opts->profile)
-    for (auto& e : pev) TKM_CUDA(cudaEventCreate(&e));
+  double prof_ms[2] = {0.0, 0.0}, prof_flops = 0.0;
+  int64_t prof_samples = 0;
   double smooth = opts->smooth0;
   for (int rnd = 0; rnd < rounds; ++rnd) {
     if (loss != TKM_LOSS_LOGISTIC && rnd > 0) smooth *= opts->eta;   // PAPER.md:220 (Alg.1 l.22)
     const double curv = curvature_of(loss, smooth);
     const double rtol = (rnd + 1 < rounds && opts->warm_tol > 0.0) ? opts->warm_tol : tol;
-    RoundArgs ra{(int)r, ldr, s->lam.as<double>(), s->u1.as<double>(), s->thin, curv,
-                 p->col_lam.as<double>(), p->col_nc.as<double>(), col_c.as<double>(), col_s.as<double>(),
-                 p->a.as<double>(), A.as<double>(), Aprev.as<double>(), Abar.as<double>(),
-                 p->beta0.as<double>(), beta_prev.as<double>(), bbar.as<double>(), rk.as<double>(),
-                 done.as<int32_t>(), iters_round.as<int32_t>(), col_of_slot.as<int32_t>()};
-    init_round_kernel<<<B, 256, 0, st>>>(ra);
+    RoundArgs ra{(int)r, B, ldr, gp, curv, p0->col_lam.as<double>(), p0->col_nc.as<double>(), col_c.as<double>(),
+                 col_s.as<double>(), A.as<double>(), Aprev.as<double>(), Abar.as<double>(), beta.as<double>(),
+                 beta_prev.as<double>(), bbar.as<double>(), rk.as<double>(), done.as<int32_t>(),
+                 iters_round.as<int32_t>(), col_of_slot.as<int32_t>(), nslots.as<int32_t>()};
+    init_round_kernel<<<dim3(B, G), 256, 0, st>>>(ra);
     TKM_LAUNCH_CHECK();
-    for (int c = 0; c < B; ++c) slot_col[c] = c;
-    int nslots = B;
-    int it = 0;
-    while (nslots > 0) {
-      const int steps = std::max(1, std::min(check_every, maxit - it));
-      for (int k = 0; k < steps; ++k) {
+
+    // Host view of the live-slot counts: an upper bound that lags the device by at most two batches.
+    int bound[GEMM_MAX_GROUPS];
+    for (int g = 0; g < G; ++g) bound[g] = B;
+    int64_t batch = 0;
+    bool finished = false;
+    while (!finished) {
+      const int ring = (int)(batch % POLL_RING);
+      int nmax = 0;
+      int64_t ntot = 0;
+      for (int g = 0; g < G; ++g) {
+        nmax = std::max(nmax, bound[g]);
+        ntot += bound[g];
+      }
+      // tile configuration for this batch (tensor maps are rebuilt only when it changes)
+      const GemmTile tA = gemm_f64_choose(nmax, ntot, G, (int)n), tB = gemm_f64_choose(nmax, ntot, G, (int)r);
+      if (tA.cfg != tileA.cfg) {
+        TKM_TRY(gemm_f64_make_args(prA, tA, &argsA));
+        argsA.nslots = nslots.as<int32_t>();
+        tileA = tA;
+      }
+      if (tB.cfg != tileB.cfg) {
+        TKM_TRY(gemm_f64_make_args(prB, tB, &argsB));
+        argsB.nslots = nslots.as<int32_t>();
+        tileB = tB;
+      }
+      argsA.N = argsB.N = std::max(nmax, 1);
+      for (int k = 0; k < check_every; ++k) {
         const bool sample = opts->profile && k == 0;
-        if (sample) TKM_CUDA(cudaEventRecord(pev[0], st));
-        GemmOperands ga{Abar.as<double>(), ldr, s->UL.as<double>(), ldr, nslots, (int)n, (int)r};
+        if (sample) TKM_CUDA(cudaEventRecord(ev.pev[ring][0], st));
         LossEpi le{(const double*)y, d_fold.as<int32_t>(), col_of_slot.as<int32_t>(), bbar.as<double>(),
-                   p->col_nc.as<double>(), p->col_tau.as<double>(), p->col_v.as<int32_t>(), (int)loss, smooth,
+                   p0->col_nc.as<double>(), p0->col_tau.as<double>(), p0->col_v.as<int32_t>(), B, (int)loss, smooth,
                    Zt.as<double>(), ldn, gpart.as<double>(), ldpart};
-        TKM_TRY(gemm_f64_dispatch(ga, le, st));
-        if (sample) TKM_CUDA(cudaEventRecord(pev[1], st));
-        GemmOperands gb{Zt.as<double>(), ldn, s->Ut.as<double>(), ldn, nslots, (int)r, (int)n};
-        SpecEpi se{s->lam.as<double>(), s->u1.as<double>(), col_of_slot.as<int32_t>(), p->col_lam.as<double>(),
-                   col_c.as<double>(), Abar.as<double>(), ldr, Rho.as<double>(), qpart.as<double>(),
-                   r2part.as<double>(), ldpart};
-        TKM_TRY(gemm_f64_dispatch(gb, se, st));
-        if (sample) TKM_CUDA(cudaEventRecord(pev[2], st));
-        UpdateArgs ua{(int)r, (int)n, (int)ceil_div(n, gemm_f64_tile_bm(nslots, n)),
-                      (int)ceil_div(r, gemm_f64_tile_bm(nslots, r)), restart, maxit, ldr, ldpart, rtol,
-                      s->lam.as<double>(), s->u1.as<double>(), col_of_slot.as<int32_t>(), p->col_lam.as<double>(),
-                      col_c.as<double>(), col_s.as<double>(), p->col_nc.as<double>(), gpart.as<double>(),
+        TKM_TRY(gemm_f64_launch(argsA, tileA, G, le, st));
+        if (sample) TKM_CUDA(cudaEventRecord(ev.pev[ring][1], st));
+        SpecEpi se{gp, col_of_slot.as<int32_t>(), p0->col_lam.as<double>(), col_c.as<double>(), B, Abar.as<double>(),
+                   ldr, Rho.as<double>(), qpart.as<double>(), r2part.as<double>(), ldpart};
+        TKM_TRY(gemm_f64_launch(argsB, tileB, G, se, st));
+        if (sample) TKM_CUDA(cudaEventRecord(ev.pev[ring][2], st));
+        UpdateArgs ua{(int)r, (int)n, B, (int)ceil_div(n, tileA.BM), (int)ceil_div(r, tileB.BM), restart, maxit, ldr,
+                      ldpart, rtol, gp, nslots.as<int32_t>(), col_of_slot.as<int32_t>(), p0->col_lam.as<double>(),
+                      col_c.as<double>(), p0->col_nc.as<double>(), col_s.as<double>(), gpart.as<double>(),
                       qpart.as<double>(), r2part.as<double>(), Rho.as<double>(), A.as<double>(), Aprev.as<double>(),
-                      Abar.as<double>(), p->beta0.as<double>(), beta_prev.as<double>(), bbar.as<double>(),
-                      rk.as<double>(), kkt.as<double>(), done.as<int32_t>(), iters.as<int32_t>(),
-                      iters_round.as<int32_t>(), flags.as<int32_t>()};
-        update_kernel<<<nslots, 256, 0, st>>>(ua);
+                      Abar.as<double>(), beta.as<double>(), beta_prev.as<double>(), bbar.as<double>(), rk.as<double>(),
+                      kkt.as<double>(), done.as<int32_t>(), iters.as<int32_t>(), iters_round.as<int32_t>(),
+                      flags.as<int32_t>()};
+        update_kernel<<<dim3(std::max(nmax, 1), G), 256, 0, st>>>(ua);
         TKM_LAUNCH_CHECK();
       }
-      it += steps;
-      TKM_CUDA(cudaMemcpyAsync(h_done.p, done.p, (size_t)B * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
-      TKM_CUDA(cudaStreamSynchronize(st));
-      if (opts->profile) {
-        float ma = 0.f, mb = 0.f;
-        TKM_CUDA(cudaEventElapsedTime(&ma, pev[0], pev[1]));
-        TKM_CUDA(cudaEventElapsedTime(&mb, pev[1], pev[2]));
-        p->prof_gemm_ms[0] += ma;
-        p->prof_gemm_ms[1] += mb;
-        p->prof_gemm_flops += 2.0 * (double)nslots * (double)n * (double)r;   // per GEMM
-        p->prof_gemm_samples += 1;
-      }
-      const int32_t* hd = h_done.as<int32_t>();
-      // finished slots are copied to the result rows, then holes are filled from the tail
-      int32_t* src = h_idx.as<int32_t>();
-      int32_t* dst = src + B;
-      int nfin = 0, nact = 0;
-      for (int sl = 0; sl < nslots; ++sl) {
-        if (hd[slot_col[sl]]) {
-          src[nfin] = sl;
-          dst[nfin] = slot_col[sl];
-          ++nfin;
-        } else {
-          ++nact;
+      // compaction on the device; the new counts travel back asynchronously
+      CompactArgs ca{B, (int)r, ldr, gp, nslots.as<int32_t>(), col_of_slot.as<int32_t>(), done.as<int32_t>(),
+                     fin_list.as<int32_t>(), tail_list.as<int32_t>(), counts.as<int32_t>(), A.as<double>(),
+                     Aprev.as<double>(), Abar.as<double>()};
+      compact_plan_kernel<<<G, 1024, 0, st>>>(ca);
+      TKM_LAUNCH_CHECK();
+      compact_apply_kernel<<<dim3(std::max(nmax, 1), G), 256, 0, st>>>(ca);
+      TKM_LAUNCH_CHECK();
+      TKM_CUDA(cudaMemcpyAsync(h_ns.as<int32_t>() + ring * GEMM_MAX_GROUPS, nslots.p, GEMM_MAX_GROUPS * sizeof(int32_t),
+                               cudaMemcpyDeviceToHost, st));
+      TKM_CUDA(cudaEventRecord(ev.poll[ring], st));
+      // read the poll of the PREVIOUS batch (the GPU keeps working on the one just enqueued)
+      if (batch >= 1) {
+        const int prev = (int)((batch - 1) % POLL_RING);
+        TKM_CUDA(cudaEventSynchronize(ev.poll[prev]));
+        const int32_t* hn = h_ns.as<int32_t>() + prev * GEMM_MAX_GROUPS;
+        int live = 0;
+        for (int g = 0; g < G; ++g) {
+          bound[g] = hn[g];
+          live += hn[g];
         }
+        if (opts->profile) {
+          // the sampled GEMMs of batch-1 have completed (they precede its poll event); the live count in
+          // effect during batch-1 is the poll result of batch-2 (all columns for the first batch)
+          float ma = 0.f, mb = 0.f;
+          TKM_CUDA(cudaEventElapsedTime(&ma, ev.pev[prev][0], ev.pev[prev][1]));
+          TKM_CUDA(cudaEventElapsedTime(&mb, ev.pev[prev][1], ev.pev[prev][2]));
+          int live_then = GB;
+          if (batch >= 2) {
+            const int32_t* h2 = h_ns.as<int32_t>() + (int)((batch - 2) % POLL_RING) * GEMM_MAX_GROUPS;
+            live_then = 0;
+            for (int g = 0; g < G; ++g) live_then += h2[g];
+          }
+          if (live_then > 0) {
+            prof_ms[0] += ma;
+            prof_ms[1] += mb;
+            prof_flops += 2.0 * (double)live_then * (double)n * (double)r;   // per GEMM
+            prof_samples += 1;
+          }
+        }
+        if (live == 0) finished = true;   // the batch enqueued above finds no live slot and does nothing
       }
-      if (nfin == 0) continue;
-      TKM_CUDA(cudaMemcpyAsync(idx_src.p, src, nfin * sizeof(int32_t), cudaMemcpyHostToDevice, st));
-      TKM_CUDA(cudaMemcpyAsync(idx_dst.p, dst, nfin * sizeof(int32_t), cudaMemcpyHostToDevice, st));
-      {
-        RowCopy c0{A.as<double>(), p->a.as<double>()};
-        row_copy_kernel<<<dim3(nfin, 1), 256, 0, st>>>(c0, c0, c0, 1, idx_src.as<int32_t>(), idx_dst.as<int32_t>(), ldr, (int)r);
-        TKM_LAUNCH_CHECK();
-      }
-      TKM_CUDA(cudaStreamSynchronize(st));   // src/dst are reused below
-      int nmove = 0;
-      int hole = 0, tail = nslots - 1;
-      while (true) {
-        while (hole < nact && !hd[slot_col[hole]]) ++hole;
-        while (tail >= nact && hd[slot_col[tail]]) --tail;
-        if (hole >= nact || tail < nact) break;
-        src[nmove] = tail;
-        dst[nmove] = hole;
-        slot_col[hole] = slot_col[tail];
-        ++nmove;
-        ++hole;
-        --tail;
-      }
-      if (nmove > 0) {
-        TKM_CUDA(cudaMemcpyAsync(idx_src.p, src, nmove * sizeof(int32_t), cudaMemcpyHostToDevice, st));
-        TKM_CUDA(cudaMemcpyAsync(idx_dst.p, dst, nmove * sizeof(int32_t), cudaMemcpyHostToDevice, st));
-        RowCopy c0{A.as<double>(), A.as<double>()}, c1{Aprev.as<double>(), Aprev.as<double>()},
-            c2{Abar.as<double>(), Abar.as<double>()};
-        row_copy_kernel<<<dim3(nmove, 3), 256, 0, st>>>(c0, c1, c2, 3, idx_src.as<int32_t>(), idx_dst.as<int32_t>(), ldr, (int)r);
-        TKM_LAUNCH_CHECK();
-      }
-      TKM_CUDA(cudaMemcpyAsync(col_of_slot.p, slot_col.data(), (size_t)nact * sizeof(int32_t), cudaMemcpyHostToDevice, st));
-      TKM_CUDA(cudaStreamSynchronize(st));   // slot_col / pinned lists are host memory reused next poll
-      nslots = nact;
+      ++batch;
     }
   }
-  p->smooth_final = loss == TKM_LOSS_LOGISTIC ? 0.0 : smooth;
-  p->h_beta0.resize(B);
-  p->h_kkt.resize(B);
-  p->h_iters.resize(B);
-  p->h_flags.resize(B);
-  TKM_CUDA(cudaMemcpyAsync(p->h_beta0.data(), p->beta0.p, B * sizeof(double), cudaMemcpyDeviceToHost, st));
-  TKM_CUDA(cudaMemcpyAsync(p->h_kkt.data(), kkt.p, B * sizeof(double), cudaMemcpyDeviceToHost, st));
-  TKM_CUDA(cudaMemcpyAsync(p->h_iters.data(), iters.p, B * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
-  TKM_CUDA(cudaMemcpyAsync(p->h_flags.data(), flags.p, B * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  // results: beta0 per group, diagnostics to the host
+  std::vector<double> hb(GB), hk(GB);
+  std::vector<int32_t> hi(GB), hf(GB);
+  for (int g = 0; g < G; ++g)
+    TKM_CUDA(cudaMemcpyAsync(out[g]->beta0.p, beta.as<double>() + (size_t)g * B, (size_t)B * sizeof(double),
+                             cudaMemcpyDeviceToDevice, st));
+  TKM_CUDA(cudaMemcpyAsync(hb.data(), beta.p, GB * sizeof(double), cudaMemcpyDeviceToHost, st));
+  TKM_CUDA(cudaMemcpyAsync(hk.data(), kkt.p, GB * sizeof(double), cudaMemcpyDeviceToHost, st));
+  TKM_CUDA(cudaMemcpyAsync(hi.data(), iters.p, GB * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  TKM_CUDA(cudaMemcpyAsync(hf.data(), flags.p, GB * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
   TKM_CUDA(cudaStreamSynchronize(st));
-  p->total_col_iters = 0;
   bool notconv = false;
-  for (int c = 0; c < B; ++c) {
-    p->total_col_iters += p->h_iters[c];
-    notconv |= p->h_flags[c] != 0;
+  for (int g = 0; g < G; ++g) {
+    tkm_path* p = out[g];
+    p->smooth_final = loss == TKM_LOSS_LOGISTIC ? 0.0 : smooth;
+    p->h_beta0.assign(hb.begin() + (size_t)g * B, hb.begin() + (size_t)(g + 1) * B);
+    p->h_kkt.assign(hk.begin() + (size_t)g * B, hk.begin() + (size_t)(g + 1) * B);
+    p->h_iters.assign(hi.begin() + (size_t)g * B, hi.begin() + (size_t)(g + 1) * B);
+    p->h_flags.assign(hf.begin() + (size_t)g * B, hf.begin() + (size_t)(g + 1) * B);
+    p->total_col_iters = 0;
+    for (int c = 0; c < B; ++c) {
+      p->total_col_iters += p->h_iters[c];
+      notconv |= p->h_flags[c] != 0;
+    }
   }
-  guard.p = nullptr;
-  *out = p;
+  // sampled timings cover all groups of the shared launches: reported on the first path
+  out[0]->prof_gemm_ms[0] = prof_ms[0];
+  out[0]->prof_gemm_ms[1] = prof_ms[1];
+  out[0]->prof_gemm_flops = prof_flops;
+  out[0]->prof_gemm_samples = prof_samples;
+  guard.armed = false;
   if (notconv) return set_error(TKM_ENOTCONV, "tkm_fit_path: some columns hit maxit (see flags)");
   return TKM_OK;
+}
+
+extern "C" int tkm_fit_path(const tkm_spectral* s, const void* y, tkm_loss loss, const tkm_loss_opts* opts,
+                            const double* lambdas, int32_t L, const int32_t* foldid, int32_t V, double tol,
+                            int32_t maxit, const tkm_path* warm, tkm_path** out, void* stream) {
+  if (!out) return set_error(TKM_EINVAL, "tkm_fit_path: out is NULL");
+  *out = nullptr;
+  if (!s) return set_error(TKM_EINVAL, "tkm_fit_path: NULL argument");
+  return tkm_fit_path_multi(&s, 1, y, loss, opts, lambdas, L, foldid, V, tol, maxit, warm ? &warm : nullptr, out, stream);
 }
 
 extern "C" void tkm_path_free(tkm_path* p) { delete p; }

@@ -1,0 +1,65 @@
+// tma.cuh -- TMA (cp.async.bulk.tensor) + mbarrier plumbing for the sm_100a kernels of libtkm.
+//
+// Host side: 2-D FP64 tensor maps with 128-byte swizzle (box = rows x 16 doubles = rows x 128 B),
+// encoded through the driver entry point fetched at run time (libtkm does not link libcuda).
+// Device side: thin PTX wrappers -- mbarrier init / expect_tx / try_wait.parity / arrive and the
+// 2-D tiled bulk tensor load that completes on an mbarrier.
+#pragma once
+
+#include <cuda.h>
+
+#include "common.cuh"
+
+namespace tkm {
+
+constexpr int TMA_BOX_K = 16;   // doubles per box row: 16 x 8 B = 128 B = one swizzle span
+
+// Encode a 2-D tensor map over a row-major FP64 matrix [rows][cols] with leading dimension ld
+// (elements; ld * 8 must be a multiple of 16 and base 16-byte aligned).  Box = box_rows x 16 doubles,
+// 128-byte swizzle; elements outside [rows) x [cols) read as zero.
+int make_tmap_f64(CUtensorMap* out, const double* base, int64_t rows, int64_t cols, int64_t ld, int box_rows);
+
+#ifdef __CUDACC__
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count));
+}
+// make mbarrier.init visible to the async proxy (TMA) before first use
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory"); }
+
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(smem_u32(bar)) : "memory");
+}
+// spin until the phase with the given parity has completed
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_LOOP:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra WAIT_DONE;\n"
+      "bra WAIT_LOOP;\n"
+      "WAIT_DONE:\n"
+      "}\n" ::"r"(smem_u32(bar)),
+      "r"(parity)
+      : "memory");
+}
+
+// 2-D tiled TMA load: box at (x = element column, y = row) -> smem, completes `bytes` on `bar`.
+__device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* tmap, int x, int y, uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];\n" ::"r"(
+          smem_u32(smem_dst)),
+      "l"(reinterpret_cast<uint64_t>(tmap)), "r"(x), "r"(y), "r"(smem_u32(bar))
+      : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* tmap) {
+  asm volatile("prefetch.tensormap [%0];\n" ::"l"(reinterpret_cast<uint64_t>(tmap)) : "memory");
+}
+#endif  // __CUDACC__
+
+}  // namespace tkm

@@ -38,10 +38,11 @@ def test_library_exports_every_declared_symbol(tkm):
     assert tkm.tkm_version() == 1
 
 
-def test_sass_has_fp64_tensor_core_instructions(tkm):
+def test_sass_has_fp64_tensor_core_and_tma_instructions(tkm):
     import subprocess
     out = subprocess.run(["cuobjdump", "-sass", tkm.lib_path()], capture_output=True, text=True).stdout
     assert "DMMA" in out and "sm_100a" in out
+    assert "UTMALDG" in out      # operand tiles of the contractions are staged by TMA
 
 
 @pytest.mark.parametrize("n,V,seed", [(200, 5, 7), (17, 4, 0), (1001, 10, 2**63 + 5), (2000, 5, 7)])
