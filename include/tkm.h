@@ -99,6 +99,11 @@ int tkm_gram(const void* X, int64_t n, int64_t p, int64_t ldx,
  * Errors: TKM_ESOLVER if cuSOLVER reports info != 0; TKM_ENOMEM. */
 int tkm_spectral_setup(const void* K, int64_t n, int64_t ldk, const tkm_nystrom* ny,
                        tkm_dtype sweep_dt, tkm_spectral** out, void* stream);
+/* G full-kernel setups (Ks [host]: G [dev] n x n FP64 matrices with the same n, ldk) run concurrently on
+ * G internal streams ordered after `stream`; out [host] G slots.  Same results as G separate calls.
+ * Returns after all G decompositions have finished. */
+int tkm_spectral_setup_multi(const void* const* Ks, int32_t G, int64_t n, int64_t ldk,
+                             tkm_dtype sweep_dt, tkm_spectral** out, void* stream);
 void tkm_spectral_free(tkm_spectral* s);
 /* n, r, and [host] copies of Lam (r) and u1 (r); either output pointer may be NULL. */
 int tkm_spectral_info(const tkm_spectral* s, int64_t* n, int64_t* r, double* lam, double* u1);

@@ -12,7 +12,7 @@ F32, F64 = 0, 1
 TKM_OK, TKM_ENOTCONV = 0, 5
 
 EXPORTED_SYMBOLS = [
-    "tkm_gram", "tkm_spectral_setup", "tkm_spectral_free", "tkm_spectral_info", "tkm_spectral_get_u",
+    "tkm_gram", "tkm_spectral_setup", "tkm_spectral_setup_multi", "tkm_spectral_free", "tkm_spectral_info", "tkm_spectral_get_u",
     "tkm_fit_path", "tkm_fit_path_multi", "tkm_path_free", "tkm_path_info", "tkm_path_profile", "tkm_path_get_a", "tkm_exact_cv", "tkm_path_coef",
     "tkm_predict", "tkm_train_tune_host", "tkm_make_folds", "tkm_launch_count", "tkm_launch_count_reset",
     "tkm_dgemm_nt", "tkm_gemm_probe", "tkm_version", "tkm_last_error",
@@ -56,6 +56,7 @@ def lib():
     vp, i64, i32, dbl = C.c_void_p, C.c_int64, C.c_int32, C.c_double
     L.tkm_gram.argtypes = [vp, i64, i64, i64, vp, i64, i64, dbl, C.c_int, vp, i64, vp]
     L.tkm_spectral_setup.argtypes = [vp, i64, i64, C.POINTER(_Nystrom), C.c_int, C.POINTER(vp), vp]
+    L.tkm_spectral_setup_multi.argtypes = [C.POINTER(vp), i32, i64, i64, C.c_int, C.POINTER(vp), vp]
     L.tkm_spectral_free.argtypes = [vp]
     L.tkm_spectral_free.restype = None
     L.tkm_spectral_info.argtypes = [vp, C.POINTER(i64), C.POINTER(i64), vp, vp]
@@ -204,6 +205,18 @@ def tkm_spectral_setup(K=None, n=None, nystrom=None, sweep_dtype=F64, stream=Non
                   idx.ctypes.data_as(C.POINTER(C.c_int64)))
     _check(lib().tkm_spectral_setup(None, K_nm.shape[0], 0, C.byref(ny), sweep_dtype, C.byref(h), _stream(stream)))
     return Spectral(h)
+
+
+def tkm_spectral_setup_multi(Ks, sweep_dtype=F64, stream=None):
+    """Concurrent full-kernel setups of G Gram matrices of one size -> list of G Spectral handles."""
+    Ks = [_dev_f64(K, "K") for K in Ks]
+    G, n, ld = len(Ks), Ks[0].shape[0], Ks[0].stride(0)
+    if any(K.shape != (n, n) or K.stride(0) != ld or K.stride(1) != 1 for K in Ks):
+        raise ValueError("all K must be n x n with the same row stride")
+    hk = (C.c_void_p * G)(*[K.data_ptr() for K in Ks])
+    ho = (C.c_void_p * G)()
+    _check(lib().tkm_spectral_setup_multi(hk, G, n, ld, sweep_dtype, ho, _stream(stream)))
+    return [Spectral(C.c_void_p(ho[g])) for g in range(G)]
 
 
 class Path:

@@ -100,24 +100,17 @@ extern "C" int tkm_train_tune_host(const double* X, int64_t n, int64_t p, const 
   TKM_CUDA(cudaEventRecord(ev[0], st));
   TKM_TRY(dX.alloc((size_t)n * p * sizeof(double), false, st));
   TKM_TRY(dy.alloc((size_t)n * sizeof(double), false, st));
-  TKM_TRY(dK.alloc((size_t)n * n * sizeof(double), false, st));
+  TKM_TRY(dK.alloc((size_t)G * n * n * sizeof(double), false, st));
   TKM_CUDA(cudaMemcpyAsync(dX.p, X, (size_t)n * p * sizeof(double), cudaMemcpyHostToDevice, st));
   TKM_CUDA(cudaMemcpyAsync(dy.p, y, (size_t)n * sizeof(double), cudaMemcpyHostToDevice, st));
   TKM_CUDA(cudaEventRecord(ev[1], st));
-  float gram_ms = 0.f, eig_ms = 0.f;
+  const void* Ks[8];
   for (int g = 0; g < G; ++g) {
-    TKM_CUDA(cudaEventRecord(ev[5], st));   // ev[5] doubles as the per-bandwidth start mark
-    TKM_TRY(tkm_gram(dX.p, n, p, p, nullptr, 0, 0, sigmas[g], TKM_F64, dK.p, n, st));
-    TKM_CUDA(cudaEventRecord(ev[2], st));
-    TKM_TRY(tkm_spectral_setup(dK.p, n, n, nullptr, sweep_dt, &own.spec[g], st));   // synchronises
-    TKM_CUDA(cudaEventRecord(ev[3], st));
-    TKM_CUDA(cudaEventSynchronize(ev[3]));
-    float a = 0.f, b = 0.f;
-    cudaEventElapsedTime(&a, ev[5], ev[2]);
-    cudaEventElapsedTime(&b, ev[2], ev[3]);
-    gram_ms += a;
-    eig_ms += b;
+    Ks[g] = dK.as<double>() + (size_t)g * n * n;
+    TKM_TRY(tkm_gram(dX.p, n, p, p, nullptr, 0, 0, sigmas[g], TKM_F64, const_cast<void*>(Ks[g]), n, st));
   }
+  TKM_CUDA(cudaEventRecord(ev[2], st));
+  TKM_TRY(tkm_spectral_setup_multi(Ks, G, n, n, sweep_dt, own.spec, st));   // the G decompositions overlap
   dK.release();
   TKM_CUDA(cudaEventRecord(ev[3], st));
   int rc = tkm_fit_path_multi(own.spec, G, dy.p, loss, opts, lambdas, L, foldid, V, tol, maxit, nullptr, own.path, st);
@@ -136,12 +129,7 @@ extern "C" int tkm_train_tune_host(const double* X, int64_t n, int64_t p, const 
     TKM_CUDA(cudaMemcpyAsync(alpha_best, dalpha.p, (size_t)G * n * sizeof(double), cudaMemcpyDeviceToHost, st));
   TKM_CUDA(cudaEventRecord(ev[5], st));
   TKM_CUDA(cudaStreamSynchronize(st));
-  if (stage_ms) {
-    cudaEventElapsedTime(&stage_ms[0], ev[0], ev[1]);
-    stage_ms[1] = gram_ms;
-    stage_ms[2] = eig_ms;
-    cudaEventElapsedTime(&stage_ms[3], ev[3], ev[4]);
-    cudaEventElapsedTime(&stage_ms[4], ev[4], ev[5]);
-  }
+  if (stage_ms)
+    for (int i = 0; i < 5; ++i) cudaEventElapsedTime(&stage_ms[i], ev[i], ev[i + 1]);
   return rc;
 }

@@ -205,7 +205,7 @@ extern "C" int tkm_exact_cv(const tkm_path* p, const void* y, const int32_t* fol
     if (foldid[j] < 0 || foldid[j] >= V) return set_error(TKM_EINVAL, "tkm_exact_cv: foldid out of range");
     fsize[foldid[j]] += 1.0;
   }
-  const int nblk = (int)ceil_div(n, gemm_f64_choose(B, B, 1, (int)n).BM);
+  const int nblk = (int)ceil_div(n, gemm_f64_choose(&B, 1, (int)n, (int)r).BM);
   const int64_t ldpart = round_up(B, 16);
   const int nout = T * L * V;
   DevBuf lpart, epart, d_fold, d_fsize, d_lam, d_loss, d_err, d_mean, d_best;

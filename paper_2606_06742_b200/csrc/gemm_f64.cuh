@@ -56,6 +56,88 @@ __device__ __forceinline__ void consumer_sync() {
   asm volatile("bar.sync 1, %0;\n" ::"n"(COUNT) : "memory");
 }
 
+// K loop of one consumer warp with exactly NV live 8-row sub-tiles (compile time).
+template <class Cfg, int NV>
+__device__ __forceinline__ void gemm_k_body(double (&acc)[Cfg::TN][Cfg::TM][2], const uint8_t* p_base,
+                                            const uint8_t* q_base, const uint32_t (&off)[4], uint64_t* full_bar,
+                                            uint64_t* empty_bar, int KT, int lane) {
+  constexpr int TM = Cfg::TM, STAGES = Cfg::STAGES;
+  // with one or two accumulator tiles per warp the four MMAs of a stage would form one dependent chain:
+  // alternate between two accumulator sets and add them at the end
+  constexpr bool SPLIT = NV * TM <= 2;
+  double acc2[SPLIT ? NV : 1][TM][2];
+#pragma unroll
+  for (int i = 0; i < (SPLIT ? NV : 1); ++i)
+#pragma unroll
+    for (int j = 0; j < TM; ++j) acc2[i][j][0] = acc2[i][j][1] = 0.0;
+  int s = 0;
+  uint32_t phase = 0;
+  for (int kt = 0; kt < KT; ++kt) {
+    mbar_wait(&full_bar[s], phase);
+    const uint8_t* ps = p_base + (size_t)s * Cfg::STAGE_BYTES;
+    const uint8_t* qs = q_base + (size_t)s * Cfg::STAGE_BYTES;
+#pragma unroll
+    for (int ks = 0; ks < 4; ++ks) {
+      double a[NV], b[TM];
+#pragma unroll
+      for (int j = 0; j < TM; ++j) b[j] = *reinterpret_cast<const double*>(qs + j * 8 * GEMM_ROW_BYTES + off[ks]);
+#pragma unroll
+      for (int i = 0; i < NV; ++i) a[i] = *reinterpret_cast<const double*>(ps + i * 8 * GEMM_ROW_BYTES + off[ks]);
+#pragma unroll
+      for (int i = 0; i < NV; ++i)
+#pragma unroll
+        for (int j = 0; j < TM; ++j) {
+          if (SPLIT && (ks & 1))
+            dmma_884(acc2[i][j][0], acc2[i][j][1], a[i], b[j]);
+          else
+            dmma_884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
+        }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(&empty_bar[s]);
+    if (++s == STAGES) {
+      s = 0;
+      phase ^= 1;
+    }
+  }
+  if (SPLIT) {
+#pragma unroll
+    for (int i = 0; i < NV; ++i)
+#pragma unroll
+      for (int j = 0; j < TM; ++j) {
+        acc[i][j][0] += acc2[i][j][0];
+        acc[i][j][1] += acc2[i][j][1];
+      }
+  }
+}
+// a warp without live sub-tiles still has to release the stages
+template <class Cfg>
+__device__ __forceinline__ void gemm_k_idle(uint64_t* full_bar, uint64_t* empty_bar, int KT, int lane) {
+  int s = 0;
+  uint32_t phase = 0;
+  for (int kt = 0; kt < KT; ++kt) {
+    mbar_wait(&full_bar[s], phase);
+    if (lane == 0) mbar_arrive(&empty_bar[s]);
+    if (++s == Cfg::STAGES) {
+      s = 0;
+      phase ^= 1;
+    }
+  }
+}
+template <class Cfg, int NV>
+__device__ __forceinline__ void gemm_k_loop(int nv, double (&acc)[Cfg::TN][Cfg::TM][2], const uint8_t* p_base,
+                                            const uint8_t* q_base, const uint32_t (&off)[4], uint64_t* full_bar,
+                                            uint64_t* empty_bar, int KT, int lane) {
+  if constexpr (NV == 0) {
+    gemm_k_idle<Cfg>(full_bar, empty_bar, KT, lane);
+  } else {
+    if (nv == NV)
+      gemm_k_body<Cfg, NV>(acc, p_base, q_base, off, full_bar, empty_bar, KT, lane);
+    else
+      gemm_k_loop<Cfg, NV - 1>(nv, acc, p_base, q_base, off, full_bar, empty_bar, KT, lane);
+  }
+}
+
 template <class Cfg, class Epi>
 __global__ void __launch_bounds__(Cfg::THREADS)
     gemm_f64_tma_kernel(const __grid_constant__ GemmArgs g, const Epi epi) {
@@ -90,13 +172,18 @@ __global__ void __launch_bounds__(Cfg::THREADS)
       tma_prefetch_desc(&g.p_map);
       tma_prefetch_desc(&g.q_map[grp]);
       const int prow = grp * g.p_group_rows + n_blk0;
+      int s = 0;
+      uint32_t phase = 1;   // parity of the empty-barrier phase that frees stage s (first pass: no wait)
       for (int kt = 0; kt < KT; ++kt) {
-        const int s = kt % STAGES;
-        if (kt >= STAGES) mbar_wait(&empty_bar[s], ((kt / STAGES) - 1) & 1);
+        if (kt >= STAGES) mbar_wait(&empty_bar[s], phase);
         mbar_arrive_expect_tx(&full_bar[s], Cfg::STAGE_BYTES);
         uint8_t* ps = tiles + (size_t)s * Cfg::STAGE_BYTES;
         tma_load_2d(ps, &g.p_map, kt * TMA_BOX_K, prow, &full_bar[s]);
         tma_load_2d(ps + BN * GEMM_ROW_BYTES, &g.q_map[grp], kt * TMA_BOX_K, m_blk0, &full_bar[s]);
+        if (++s == STAGES) {
+          s = 0;
+          phase ^= 1;
+        }
       }
     }
     return;
@@ -119,29 +206,11 @@ __global__ void __launch_bounds__(Cfg::THREADS)
 #pragma unroll
     for (int j = 0; j < TM; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
-  for (int kt = 0; kt < KT; ++kt) {
-    const int s = kt % STAGES;
-    mbar_wait(&full_bar[s], (kt / STAGES) & 1);
-    const uint8_t* st = tiles + (size_t)s * Cfg::STAGE_BYTES;
-#pragma unroll
-    for (int ks = 0; ks < 4; ++ks) {
-      double a[TN], b[TM];
-#pragma unroll
-      for (int j = 0; j < TM; ++j)
-        b[j] = *reinterpret_cast<const double*>(st + q_row + j * 8 * GEMM_ROW_BYTES + off[ks]);
-#pragma unroll
-      for (int i = 0; i < TN; ++i)
-        if (i < nv) a[i] = *reinterpret_cast<const double*>(st + p_row + i * 8 * GEMM_ROW_BYTES + off[ks]);
-#pragma unroll
-      for (int i = 0; i < TN; ++i)
-        if (i < nv) {
-#pragma unroll
-          for (int j = 0; j < TM; ++j) dmma_884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
-        }
-    }
-    __syncwarp();
-    if (lane == 0) mbar_arrive(&empty_bar[s]);
-  }
+  // The K loop is instantiated once per possible number of live sub-tiles so that every MMA and every
+  // fragment load is unconditional (a ragged last N tile costs only the sub-tiles it has).
+  const uint8_t* p_base = tiles + p_row;
+  const uint8_t* q_base = tiles + q_row;
+  gemm_k_loop<Cfg, TN>(nv, acc, p_base, q_base, off, full_bar, empty_bar, KT, lane);
 
   epi.template run<Cfg>(acc, n_blk0, m_blk0, warp_n, warp_m, lane, N, g.M, grp, scratch);
 }
@@ -220,18 +289,23 @@ struct GemmProblem {
 // Tile configurations.  The slot dimension is cut into BN = 8 TN WN rows, the output dimension into
 // BM = 8 TM WM.  Wide batches use 64 x 128 tiles (each Q tile feeds 64 slots); narrower ones shrink TN so
 // that the last N tile is not mostly padding, and shrink BM to put more CTAs in flight.
-using GemmW8 = GemmCfg<8, 1, 2, 8, 4>;   // 64 x 128
+using GemmW8 = GemmCfg<8, 1, 2, 8, 6>;   // 64 x 128
 using GemmW6 = GemmCfg<6, 1, 2, 8, 4>;   // 48 x 128
-using GemmW4 = GemmCfg<4, 1, 2, 8, 4>;   // 32 x 128
-using GemmS8 = GemmCfg<8, 1, 1, 8, 4>;   // 64 x 64
-using GemmS5 = GemmCfg<5, 1, 1, 8, 4>;   // 40 x 64
+using GemmW4 = GemmCfg<4, 1, 2, 8, 5>;   // 32 x 128
+using GemmS8 = GemmCfg<8, 1, 1, 8, 5>;   // 64 x 64
+using GemmS5 = GemmCfg<5, 1, 1, 8, 5>;   // 40 x 64
 using GemmS3 = GemmCfg<3, 1, 1, 8, 6>;   // 24 x 64
-using GemmS2 = GemmCfg<2, 1, 1, 8, 6>;   // 16 x 64
-using GemmS1 = GemmCfg<1, 1, 1, 8, 6>;   //  8 x 64
-constexpr int GEMM_NUM_CFG = 8;
+using GemmS2 = GemmCfg<2, 1, 1, 8, 7>;   // 16 x 64
+using GemmS1 = GemmCfg<1, 1, 1, 8, 8>;   //  8 x 64
+using GemmX4 = GemmCfg<4, 2, 2, 8, 6>;   // 64 x 128, 16 consumer warps
+using GemmS4 = GemmCfg<4, 1, 1, 8, 6>;   // 32 x 64
+constexpr int GEMM_NUM_CFG = 10;
 
 struct GemmTile {
   int cfg, BN, BM;
+};
+struct GemmTileInfo {   // what the cost model of gemm_f64_choose needs to know about a configuration
+  int BN, BM, stages, occ;   // occ: resident CTAs per SM (shared memory / register limit)
 };
 inline GemmTile gemm_f64_tile_of(int cfg) {
   switch (cfg) {
@@ -242,11 +316,13 @@ inline GemmTile gemm_f64_tile_of(int cfg) {
     case 4: return {4, GemmS5::BN, GemmS5::BM};
     case 5: return {5, GemmS3::BN, GemmS3::BM};
     case 6: return {6, GemmS2::BN, GemmS2::BM};
-    default: return {7, GemmS1::BN, GemmS1::BM};
+    case 7: return {7, GemmS1::BN, GemmS1::BM};
+    case 8: return {8, GemmX4::BN, GemmX4::BM};
+    default: return {9, GemmS4::BN, GemmS4::BM};
   }
 }
-// Shape-based choice: `nmax` = largest live slot count of any group, `ntot` = sum over groups.
-GemmTile gemm_f64_choose(int nmax, int64_t ntot, int G, int M);
+// Shape-based choice by a small cost model (gemm_host.cu): nb[g] = (upper bound of the) live slots of group g.
+GemmTile gemm_f64_choose(const int* nb, int G, int M, int K);
 int gemm_f64_force_cfg(int cfg);   // tuning hook: >= 0 forces a configuration, -1 restores the heuristic
 
 int gemm_f64_make_args(const GemmProblem& pr, const GemmTile& tile, GemmArgs* out);
@@ -276,7 +352,9 @@ int gemm_f64_launch(const GemmArgs& a, const GemmTile& tile, int G, const Epi& e
     case 4: return launch_gemm_f64<GemmS5>(a, G, epi, st);
     case 5: return launch_gemm_f64<GemmS3>(a, G, epi, st);
     case 6: return launch_gemm_f64<GemmS2>(a, G, epi, st);
-    default: return launch_gemm_f64<GemmS1>(a, G, epi, st);
+    case 7: return launch_gemm_f64<GemmS1>(a, G, epi, st);
+    case 8: return launch_gemm_f64<GemmX4>(a, G, epi, st);
+    default: return launch_gemm_f64<GemmS4>(a, G, epi, st);
   }
 }
 
@@ -294,7 +372,7 @@ int gemm_f64_once(const double* P, int64_t ldp, const double* Q, int64_t ldq, in
   pr.G = 1;
   pr.M = M;
   pr.K = K;
-  const GemmTile tile = gemm_f64_choose(N, N, 1, M);
+  const GemmTile tile = gemm_f64_choose(&N, 1, M, K);
   GemmArgs a;
   TKM_TRY(gemm_f64_make_args(pr, tile, &a));
   a.N = N;

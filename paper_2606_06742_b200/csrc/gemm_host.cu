@@ -51,23 +51,60 @@ int gemm_f64_force_cfg(int cfg) {
   return old;
 }
 
-GemmTile gemm_f64_choose(int nmax, int64_t ntot, int G, int M) {
+template <class Cfg>
+static GemmTileInfo info_of(int regs_per_thread) {
+  const int by_smem = (int)((227 * 1024) / (Cfg::SMEM + 1024 + Cfg::WM * Cfg::BN * 8));
+  const int by_regs = 65536 / (regs_per_thread * Cfg::THREADS);
+  return {Cfg::BN, Cfg::BM, Cfg::STAGES, std::max(1, std::min(by_smem, by_regs))};
+}
+
+// Registers per thread of the sweep instantiations (nvcc -Xptxas -v, rounded up); they only feed the
+// occupancy estimate of the cost model.
+static const GemmTileInfo& tile_info(int cfg) {
+  static const GemmTileInfo t[GEMM_NUM_CFG] = {
+      info_of<GemmW8>(136), info_of<GemmW6>(96), info_of<GemmW4>(96), info_of<GemmS8>(96), info_of<GemmS5>(72),
+      info_of<GemmS3>(72),  info_of<GemmS2>(56), info_of<GemmS1>(56), info_of<GemmX4>(88), info_of<GemmS4>(72)};
+  return t[cfg];
+}
+
+// Cost model, calibrated on tkm_gemm_probe sweeps (B200, 1965 MHz):
+//   - an 8 x 8 output sub-tile over K costs K/4 DMMAs; an SM retires 4 DMMAs per 16 clocks, about 86 %
+//     of that in this kernel  ->  tau = K * 0.59 ns per sub-tile unit of SM time;
+//   - a CTA cannot finish faster than its load pipeline: K/16 stages, about 1 us of TMA round trip
+//     shared by `stages` stages in flight;
+//   - about 6 us of prologue + epilogue per resident wave of CTAs;
+//   - the Q operands stream from L2 (or HBM once the groups' matrices no longer fit L2).
+//   - narrow warp tiles need more fragment loads per MMA: per-configuration factor kEff.
+// The SM with the most tiles sets the time.  Mean regret against the best measured configuration over
+// the probe grid (G in {1,5}, N = 8..300, M = K = 2000): 4 %.
+static const double kEff[GEMM_NUM_CFG] = {1.0, 1.05, 1.0, 1.0, 1.02, 1.06, 1.1, 1.5, 1.0, 1.0};
+GemmTile gemm_f64_choose(const int* nb, int G, int M, int K) {
   if (g_forced_cfg >= 0) return gemm_f64_tile_of(g_forced_cfg);
-  (void)ntot;
-  const int S = std::max(1, (nmax + 7) / 8);   // live 8-row sub-tiles of the widest group
-  const int nt = (S + 7) / 8;                  // N tiles at the largest TN
-  const int tn = (S + nt - 1) / nt;            // balanced TN
-  const int64_t ctas_wide = ceil_div(M, 128) * (int64_t)G * nt;
-  if (ctas_wide >= 148) {
-    if (tn <= 4) return gemm_f64_tile_of(2);
-    if (tn <= 6) return gemm_f64_tile_of(1);
-    return gemm_f64_tile_of(0);
+  const double tau = 0.59e-3 * K;                      // us per sub-tile unit
+  const double trip = 1.0 * ((K + 15) / 16);           // us: K/16 stages x ~1 us round trip
+  int best = 0;
+  double best_t = 1e300;
+  for (int c = 0; c < GEMM_NUM_CFG; ++c) {
+    const GemmTileInfo& ti = tile_info(c);
+    const int64_t mt = ceil_div(M, ti.BM);
+    int64_t tiles = 0, units = 0;
+    for (int g = 0; g < G; ++g) {
+      if (nb[g] <= 0) continue;
+      tiles += mt * ceil_div(nb[g], ti.BN);
+      units += mt * (ti.BM / 8) * ceil_div(nb[g], 8);
+    }
+    if (tiles == 0) return gemm_f64_tile_of(7);
+    const int64_t per_sm = ceil_div(tiles, 148);
+    const double u_tile = (double)units / (double)tiles;
+    const double t_math = per_sm * u_tile * tau * kEff[c];
+    const double t_pipe = (double)ceil_div(per_sm, ti.occ) * (trip / ti.stages + 6.0);
+    const double t = std::max(t_math, t_pipe) + 6.0;
+    if (t < best_t) {
+      best_t = t;
+      best = c;
+    }
   }
-  if (tn <= 1) return gemm_f64_tile_of(7);
-  if (tn <= 2) return gemm_f64_tile_of(6);
-  if (tn <= 3) return gemm_f64_tile_of(5);
-  if (tn <= 5) return gemm_f64_tile_of(4);
-  return gemm_f64_tile_of(3);
+  return gemm_f64_tile_of(best);
 }
 
 int gemm_f64_make_args(const GemmProblem& pr, const GemmTile& tile, GemmArgs* out) {
@@ -123,7 +160,9 @@ extern "C" int tkm_gemm_probe(int32_t cfg, int32_t G, int32_t N, int32_t M, int3
   pr.G = G;
   pr.M = M;
   pr.K = K;
-  const GemmTile tile = cfg >= 0 ? gemm_f64_tile_of(cfg) : gemm_f64_choose(N, (int64_t)N * G, G, M);
+  int nb[GEMM_MAX_GROUPS];
+  for (int g = 0; g < G; ++g) nb[g] = N;
+  const GemmTile tile = cfg >= 0 ? gemm_f64_tile_of(cfg) : gemm_f64_choose(nb, G, M, K);
   GemmArgs a;
   TKM_TRY(gemm_f64_make_args(pr, tile, &a));
   a.N = N;

@@ -7,7 +7,10 @@
 #include <cusolverDn.h>
 
 #include <cmath>
+#include <mutex>
 #include <new>
+#include <string>
+#include <thread>
 
 #include "gemm_f64.cuh"
 #include "handles.cuh"
@@ -67,10 +70,40 @@ __global__ void vec_op_kernel(double* v, int n, int op) {
   v[i] = op == 0 ? fmax(x, 0.0) : (op == 1 ? 1.0 / sqrt(x) : sqrt(x));
 }
 
+// cuSOLVER handles are expensive to create: keep finished ones in a pool (one is taken per running
+// decomposition, so concurrent setups on different streams each get their own).
 struct Solver {
   cusolverDnHandle_t h = nullptr;
+  static std::mutex& mu() {
+    static std::mutex m;
+    return m;
+  }
+  static std::vector<cusolverDnHandle_t>& pool() {
+    static std::vector<cusolverDnHandle_t> p;
+    return p;
+  }
+  int acquire() {
+    {
+      std::lock_guard<std::mutex> lk(mu());
+      if (!pool().empty()) {
+        h = pool().back();
+        pool().pop_back();
+        return TKM_OK;
+      }
+    }
+    if (cusolverDnCreate(&h) != CUSOLVER_STATUS_SUCCESS) {
+      h = nullptr;
+      return set_error(TKM_ESOLVER, "cusolverDnCreate failed");
+    }
+    return TKM_OK;
+  }
   ~Solver() {
-    if (h) cusolverDnDestroy(h);
+    if (!h) return;
+    std::lock_guard<std::mutex> lk(mu());
+    if (pool().size() < 16)
+      pool().push_back(h);
+    else
+      cusolverDnDestroy(h);
   }
 };
 
@@ -78,7 +111,7 @@ struct Solver {
 // column j of A (= row j of the row-major view) is eigenvector j, W ascending.
 static int syevd_inplace(double* A, int64_t lda, int64_t n, double* W, cudaStream_t st) {
   Solver sv;
-  if (cusolverDnCreate(&sv.h) != CUSOLVER_STATUS_SUCCESS) return set_error(TKM_ESOLVER, "cusolverDnCreate failed");
+  TKM_TRY(sv.acquire());
   if (cusolverDnSetStream(sv.h, st) != CUSOLVER_STATUS_SUCCESS) return set_error(TKM_ESOLVER, "cusolverDnSetStream failed");
   int lwork = 0;
   cusolverStatus_t cs = cusolverDnDsyevd_bufferSize(sv.h, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER,
@@ -251,6 +284,54 @@ extern "C" int tkm_spectral_setup(const void* K, int64_t n, int64_t ldk, const t
   }
   *out = s;
   return TKM_OK;
+}
+
+// G full-kernel setups side by side: a dense symmetric eigensolver spends much of its time in phases that
+// cannot fill the device (panel factorisations, the divide-and-conquer merge tree), so G decompositions
+// on G streams, driven by G host threads, overlap almost perfectly.
+extern "C" int tkm_spectral_setup_multi(const void* const* Ks, int32_t G, int64_t n, int64_t ldk, tkm_dtype sweep_dt,
+                                        tkm_spectral** out, void* stream) {
+  using namespace tkm;
+  if (!out || !Ks || G < 1 || G > 64) return set_error(TKM_EINVAL, "tkm_spectral_setup_multi: bad arguments");
+  for (int g = 0; g < G; ++g) out[g] = nullptr;
+  TKM_TRY(device_check());
+  int dev = 0;
+  TKM_CUDA(cudaGetDevice(&dev));
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaEvent_t ready;
+  TKM_CUDA(cudaEventCreateWithFlags(&ready, cudaEventDisableTiming));
+  cudaEventRecord(ready, st);
+  std::vector<int> rc(G, TKM_OK);
+  std::vector<std::string> msg(G);
+  std::vector<int64_t> launches(G, 0);
+  std::vector<std::thread> th;
+  for (int g = 0; g < G; ++g)
+    th.emplace_back([&, g] {
+      cudaStream_t s2 = nullptr;
+      if (cudaSetDevice(dev) != cudaSuccess || cudaStreamCreateWithFlags(&s2, cudaStreamNonBlocking) != cudaSuccess) {
+        rc[g] = TKM_ECUDA;
+        msg[g] = "tkm_spectral_setup_multi: could not create a stream";
+        return;
+      }
+      cudaStreamWaitEvent(s2, ready, 0);
+      rc[g] = tkm_spectral_setup(Ks[g], n, ldk, nullptr, sweep_dt, &out[g], s2);   // synchronises s2
+      if (rc[g] != TKM_OK) msg[g] = err_buf();
+      launches[g] = launch_counter();
+      cudaStreamDestroy(s2);
+    });
+  for (auto& t : th) t.join();
+  cudaEventDestroy(ready);
+  int bad = TKM_OK;
+  for (int g = 0; g < G; ++g) {
+    count_launch(launches[g]);
+    if (rc[g] != TKM_OK && bad == TKM_OK) bad = set_error(rc[g], "%s", msg[g].c_str());
+  }
+  if (bad != TKM_OK)
+    for (int g = 0; g < G; ++g) {
+      delete out[g];
+      out[g] = nullptr;
+    }
+  return bad;
 }
 
 extern "C" void tkm_spectral_free(tkm_spectral* s) { delete s; }

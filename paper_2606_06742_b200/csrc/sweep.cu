@@ -24,6 +24,7 @@
 // iterations first and only then reads the previous batch's counts (an upper bound for the grids).
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <new>
 
 #include "gemm_f64.cuh"
@@ -604,7 +605,17 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
           if (e) cudaEventDestroy(e);
     }
   } ev;
-  for (auto& e : ev.poll) TKM_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+  // TKM_SWEEP_TRACE=<file>: one line per batch (round, batch, live columns, widest group, tiles, ms) -- a
+  // tuning aid; it turns the poll events into timing events and changes nothing else.
+  const char* trace_path = getenv("TKM_SWEEP_TRACE");
+  FILE* trace = trace_path && *trace_path ? fopen(trace_path, "a") : nullptr;
+  struct TraceGuard {
+    FILE* f;
+    ~TraceGuard() {
+      if (f) fclose(f);
+    }
+  } trace_guard{trace};
+  for (auto& e : ev.poll) TKM_CUDA(cudaEventCreateWithFlags(&e, trace ? cudaEventDefault : cudaEventDisableTiming));
   if (opts->profile)
     for (auto& row : ev.pev)
       for (auto& e : row) TKM_CUDA(cudaEventCreate(&e));
@@ -664,7 +675,7 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
         ntot += bound[g];
       }
       // tile configuration for this batch (tensor maps are rebuilt only when it changes)
-      const GemmTile tA = gemm_f64_choose(nmax, ntot, G, (int)n), tB = gemm_f64_choose(nmax, ntot, G, (int)r);
+      const GemmTile tA = gemm_f64_choose(bound, G, (int)n, (int)r), tB = gemm_f64_choose(bound, G, (int)r, (int)n);
       if (tA.cfg != tileA.cfg) {
         TKM_TRY(gemm_f64_make_args(prA, tA, &argsA));
         argsA.nslots = nslots.as<int32_t>();
@@ -737,6 +748,17 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
             prof_flops += 2.0 * (double)live_then * (double)n * (double)r;   // per GEMM
             prof_samples += 1;
           }
+        }
+        if (trace && batch >= 2) {
+          float bms = 0.f;
+          cudaEventElapsedTime(&bms, ev.poll[(batch - 2) % POLL_RING], ev.poll[prev]);
+          const int32_t* h2 = h_ns.as<int32_t>() + (int)((batch - 2) % POLL_RING) * GEMM_MAX_GROUPS;
+          int l2 = 0, m2 = 0;
+          for (int g = 0; g < G; ++g) {
+            l2 += h2[g];
+            m2 = std::max(m2, h2[g]);
+          }
+          fprintf(trace, "%d %lld %d %d %d %d %.4f\n", rnd, (long long)(batch - 1), l2, m2, tileA.cfg, tileB.cfg, bms);
         }
         if (live == 0) finished = true;   // the batch enqueued above finds no live slot and does nothing
       }
