@@ -178,6 +178,7 @@ def workload_config(w, dtype):
 def run_ours(args, w, rank, world):
     import torch
     import paper_2606_06742_b200 as tkm
+    from paper_2606_06742_b200 import ranks
     tkm.lib()   # raises if libtkm.so is missing: there is no fallback
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device (libtkm has no CPU fallback)")
@@ -256,11 +257,7 @@ def run_ours(args, w, rank, world):
         torch.cuda.synchronize()
 
     def max_over_ranks(ms):
-        if dist is None:
-            return ms
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return ranks.max_over_ranks(ms, dist, device="cuda")
 
     for _ in range(args.warmup):
         step_device(False)
@@ -345,7 +342,8 @@ def main():
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
-    w = wl.config1(seed=1001 + (rank if args.impl == "ours" else 0))
+    from paper_2606_06742_b200.ranks import replica_seed
+    w = wl.config1(seed=replica_seed(1001, rank if args.impl == "ours" else 0))
     if args.impl == "reference":
         run_reference(args, w, rank)
     else:

@@ -260,52 +260,132 @@ struct UpdateArgs {
   int32_t *done, *iters, *iters_round, *flags;  // [G*B]
 };
 
-__global__ void __launch_bounds__(256) update_kernel(UpdateArgs p) {
-  __shared__ double red[32];
+// One CTA per live slot.  The vectors are walked in chunks of 256 x UPD_EPT pairs with all loads of a chunk
+// issued before its arithmetic (the dependent chain is then two block reductions plus two memory round
+// trips, not one round trip per element); when the whole vector fits one chunk (r <= 2048) the second
+// pass works from registers.  Padded entries (i >= r) hold zeros in every array and stay zero.
+constexpr int UPD_EPT = 4;   // double2 elements per thread and chunk
+__global__ void __launch_bounds__(256, 2) update_kernel(UpdateArgs p) {
+  __shared__ double red[3][32];
   const int slot = blockIdx.x, grp = blockIdx.y;
   if (slot >= p.nslots[grp]) return;
   const int gs = grp * p.B + slot;
   const int col = p.col_of_slot[gs];
   const int gc = grp * p.B + col;
   if (p.done[gc]) return;   // frozen until the next compaction removes it
-  const double* lam = p.gp.lam[grp];
-  const double* u1 = p.gp.u1[grp];
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+  const double2* __restrict__ lam2 = reinterpret_cast<const double2*>(p.gp.lam[grp]);
+  const double2* __restrict__ u12 = reinterpret_cast<const double2*>(p.gp.u1[grp]);
+  // per-column sums from the per-tile partials of the two epilogues (fixed order => deterministic)
   double g0 = 0.0, qd = 0.0, r2 = 0.0;
-  for (int b = threadIdx.x; b < p.nblkA; b += blockDim.x) g0 += p.gpart[(int64_t)b * p.ldpart + gs];
-  for (int b = threadIdx.x; b < p.nblkB; b += blockDim.x) {
+  for (int b = tid; b < p.nblkA; b += 256) g0 += p.gpart[(int64_t)b * p.ldpart + gs];
+  for (int b = tid; b < p.nblkB; b += 256) {
     qd += p.qpart[(int64_t)b * p.ldpart + gs];
     r2 += p.r2part[(int64_t)b * p.ldpart + gs];
   }
-  g0 = block_sum(g0, red);
-  qd = block_sum(qd, red);
-  r2 = block_sum(r2, red);
+  g0 = warp_sum(g0);
+  qd = warp_sum(qd);
+  r2 = warp_sum(r2);
+  if (lane == 0) {
+    red[0][w] = g0;
+    red[1][w] = qd;
+    red[2][w] = r2;
+  }
+  __syncthreads();
+  g0 = qd = r2 = 0.0;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) {
+    g0 += red[0][k];
+    qd += red[1][k];
+    r2 += red[2][k];
+  }
   const double lamc = p.col_lam[col], c = p.col_c[col], s = p.col_s[gc], nc = p.col_nc[col];
   const double dbeta = (g0 - c * qd) / s;                            // PAPER.md:208 (Alg.1 l.17)
   const double kkt = fmax(fabs(g0), nc * sqrt(r2) / sqrt((double)p.n));   // reading G6
   const double beta = p.beta[gc], bbar = p.bbar[gc];
   const double beta_new = bbar - dbeta;
-  const int64_t off = (int64_t)gs * p.lda;
+  const int64_t off2 = ((int64_t)gs * p.lda) >> 1;   // lda is a multiple of 16
+  const double2* __restrict__ Rho2 = reinterpret_cast<const double2*>(p.Rho) + off2;
+  double2* __restrict__ A2 = reinterpret_cast<double2*>(p.A) + off2;
+  double2* __restrict__ Ap2 = reinterpret_cast<double2*>(p.Aprev) + off2;
+  double2* __restrict__ Ab2 = reinterpret_cast<double2*>(p.Abar) + off2;
+  const int npair = (int)(p.lda >> 1);
+  const bool single = npair <= 256 * UPD_EPT;
+  const double two_lam = 2.0 * lamc, dbc = dbeta * c;
+  double2 a_old[UPD_EPT], a_new[UPD_EPT];
   double g = 0.0;
-  for (int i = threadIdx.x; i < p.r; i += blockDim.x) {
-    const double S = 1.0 / (2.0 * lamc + c * lam[i]);
-    const double da = S * (p.Rho[off + i] - dbeta * c * u1[i]);      // PAPER.md:207 (Alg.1 l.16)
-    const double an = p.Abar[off + i] - da;                           // PAPER.md:212 (Alg.1 l.19)
-    g += da * (an - p.A[off + i]);
-    p.Aprev[off + i] = an;   // a' is dead once abar has been formed: use it as scratch for a+
+  for (int base = 0; base < npair; base += 256 * UPD_EPT) {
+    double2 rho[UPD_EPT], ab[UPD_EPT], lm[UPD_EPT], uu[UPD_EPT];
+#pragma unroll
+    for (int e = 0; e < UPD_EPT; ++e) {
+      const int i = base + e * 256 + tid;
+      if (i < npair) {
+        rho[e] = Rho2[i];
+        ab[e] = Ab2[i];
+        a_old[e] = A2[i];
+        lm[e] = lam2[i];
+        uu[e] = u12[i];
+      }
+    }
+#pragma unroll
+    for (int e = 0; e < UPD_EPT; ++e) {
+      const int i = base + e * 256 + tid;
+      if (i < npair) {
+        // S_i = 1/(2 lam + c Lam_i); da = S (rho - dbeta c u1)  PAPER.md:207 (Alg.1 l.16); a+ = abar - da (l.19)
+        const double dax = (rho[e].x - dbc * uu[e].x) / (two_lam + c * lm[e].x);
+        const double day = (rho[e].y - dbc * uu[e].y) / (two_lam + c * lm[e].y);
+        a_new[e] = make_double2(ab[e].x - dax, ab[e].y - day);
+        g += dax * (a_new[e].x - a_old[e].x) + day * (a_new[e].y - a_old[e].y);
+        if (!single) Ap2[i] = a_new[e];   // a' is dead once abar has been formed: scratch for a+
+      }
+    }
   }
-  g = block_sum(g, red) + dbeta * (beta_new - beta);
+  g = warp_sum(g);
+  __syncthreads();   // red[] of the first reduction has been consumed
+  if (lane == 0) red[0][w] = g;
+  __syncthreads();
+  g = 0.0;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) g += red[0][k];
+  g += dbeta * (beta_new - beta);
   double rk = p.rk[gc];
   rk = 0.5 * (1.0 + sqrt(1.0 + 4.0 * rk * rk));                       // PAPER.md:199 (Alg.1 l.12)
   if (p.restart && g > 0.0) rk = 1.0;                                 // gradient restart
   const double rk_next = 0.5 * (1.0 + sqrt(1.0 + 4.0 * rk * rk));
   const double mu = (rk - 1.0) / rk_next;                             // PAPER.md:203 (Alg.1 l.14)
-  for (int i = threadIdx.x; i < p.r; i += blockDim.x) {
-    const double aold = p.A[off + i], an = p.Aprev[off + i];
-    p.Aprev[off + i] = aold;
-    p.A[off + i] = an;
-    p.Abar[off + i] = an + mu * (an - aold);
+  if (single) {
+#pragma unroll
+    for (int e = 0; e < UPD_EPT; ++e) {
+      const int i = e * 256 + tid;
+      if (i < npair) {
+        Ap2[i] = a_old[e];
+        A2[i] = a_new[e];
+        Ab2[i] = make_double2(a_new[e].x + mu * (a_new[e].x - a_old[e].x), a_new[e].y + mu * (a_new[e].y - a_old[e].y));
+      }
+    }
+  } else {
+    for (int base = 0; base < npair; base += 256 * UPD_EPT) {
+#pragma unroll
+      for (int e = 0; e < UPD_EPT; ++e) {
+        const int i = base + e * 256 + tid;
+        if (i < npair) {
+          a_old[e] = A2[i];
+          a_new[e] = Ap2[i];
+        }
+      }
+#pragma unroll
+      for (int e = 0; e < UPD_EPT; ++e) {
+        const int i = base + e * 256 + tid;
+        if (i < npair) {
+          Ap2[i] = a_old[e];
+          A2[i] = a_new[e];
+          Ab2[i] =
+              make_double2(a_new[e].x + mu * (a_new[e].x - a_old[e].x), a_new[e].y + mu * (a_new[e].y - a_old[e].y));
+        }
+      }
+    }
   }
-  if (threadIdx.x == 0) {
+  if (tid == 0) {
     p.beta_prev[gc] = beta;
     p.beta[gc] = beta_new;
     p.bbar[gc] = beta_new + mu * (beta_new - beta);
