@@ -48,7 +48,7 @@ WARM_TOL = 1e-3
 NOMINAL_RATIO = {"f64": 45.0 / 2250.0, "f32": (1125.0 / 2250.0) / 3.0}
 # dram bytes per launch of the dominant kernel from the committed ncu --set full capture
 # (profiles/): filled in by hand after each capture, None until one exists.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 218.0e6   # profiles/r01c: full-width launch, dram read + write
 # columns of the bounded CPU sample: all V+1 hold-out settings x these lambda indices, one sigma
 CPU_SAMPLE_LAMBDA_IDX = (0, 12, 24, 36, 49)
 CPU_SAMPLE_SIGMA_IDX = 2

@@ -298,7 +298,7 @@ using GemmS3 = GemmCfg<3, 1, 1, 8, 6>;   // 24 x 64
 using GemmS2 = GemmCfg<2, 1, 1, 8, 7>;   // 16 x 64
 using GemmS1 = GemmCfg<1, 1, 1, 8, 8>;   //  8 x 64
 using GemmX4 = GemmCfg<4, 2, 2, 8, 6>;   // 64 x 128, 16 consumer warps
-using GemmS4 = GemmCfg<4, 1, 1, 8, 6>;   // 32 x 64
+using GemmS4 = GemmCfg<4, 1, 1, 8, 5>;   // 32 x 64 (5 stages: 3 CTAs per SM)
 constexpr int GEMM_NUM_CFG = 10;
 
 struct GemmTile {

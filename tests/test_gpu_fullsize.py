@@ -1,0 +1,160 @@
+"""Full-size GPU checks for BASELINE.json configs[2..4] (n = 10000 / 20000 / 100000): the oracle cannot fit
+these sizes in test time, so every sampled column is checked against what the DEFINITION fixes at any size
+(SURVEY.md 8(c) "Definition of the result", pin P6): with f = K alpha + beta0 computed independently of the
+sweep (torch FP64 mat-vec on the Gram matrix), z = M psi(y, f)/n_c from the oracle's loss table must satisfy
+the first-order conditions  sum z = 0  and  z + 2 lambda alpha = 0  to the stop tolerance, held-out alpha = 0,
+and the exact-CV table must equal the nominal loss of those f on the held-out rows.  Sampled Gram entries are
+compared with the oracle's Gram."""
+import numpy as np
+import pytest
+
+import oracle as o
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10        # stop tolerance of these runs (an input); the checks below allow 20 x for rounding of K alpha
+WARM_TOL = 1e-3
+MAXIT = 50000
+
+
+@pytest.fixture(scope="module")
+def tkm():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (no CPU fallback exists)")
+    import paper_2606_06742_b200 as t
+    t.lib()
+    return t
+
+
+def _dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _check_gram_entries(K, X, sigma, rng, count=300):
+    n = X.shape[0]
+    ii, jj = rng.integers(0, n, count), rng.integers(0, K.shape[1], count)
+    got = K[_dev(ii), _dev(jj)].cpu().numpy()
+    return ii, jj, got
+
+
+def _first_order(w, tkm, path, K, y_np, foldid, cols, smooth_final):
+    """Returns max over the sampled columns of (|sum z|, n_c ||z + 2 lam alpha|| / sqrt(n), held-out |alpha|)."""
+    import torch
+    L, V, n = w.L, w.V, w.n
+    worst = [0.0, 0.0, 0.0]
+    fs = {}
+    for c in cols:
+        t, v, l = c // ((V + 1) * L), (c // L) % (V + 1), c % L
+        alpha, b0 = tkm.tkm_path_coef(path, t, l, v)
+        f = (torch.mv(K, alpha) + b0).cpu().numpy()
+        a = alpha.cpu().numpy()
+        M = (foldid != v).astype(np.float64)
+        nc = M.sum()
+        tau = w.taus[t] if len(w.taus) else None
+        z = M * o.psi(w.loss, y_np, f, smooth_final, tau) / nc
+        lam = w.lambdas[l]
+        worst[0] = max(worst[0], abs(z.sum()))
+        worst[1] = max(worst[1], nc * np.linalg.norm(z + 2.0 * lam * a) / np.sqrt(n))
+        if v < V:
+            worst[2] = max(worst[2], np.abs(a[foldid == v]).max() / max(np.abs(a).max(), 1e-300))
+        fs[c] = f
+    return worst, fs
+
+
+@pytest.mark.parametrize("cfg", [2, 3])
+def test_full_kernel_configs_first_order_optimality(tkm, cfg):
+    import torch
+    w = wl.CONFIGS[cfg]()
+    sigma = float(w.sigmas[0])
+    foldid = tkm.tkm_make_folds(w.n, w.V, w.fold_seed)
+    X, y = _dev(w.X), _dev(w.y)
+    K = tkm.tkm_gram(X, sigma)
+    rng = np.random.default_rng(cfg)
+    ii, jj, got = _check_gram_entries(K, w.X, sigma, rng)
+    d2 = ((w.X[ii] - w.X[jj]) ** 2).sum(axis=1)
+    assert np.max(np.abs(got - np.exp(-d2 / (2 * sigma * sigma)))) < 1e-13
+    rows = np.sort(rng.integers(0, w.n, 40))
+    assert np.max(np.abs(K[_dev(rows)][:, _dev(rows)].cpu().numpy() - o.gram_rbf(w.X[rows], sigma))) < 1e-13
+    spec = tkm.tkm_spectral_setup(K)
+    path = tkm.tkm_fit_path(spec, y, w.loss, w.lambdas, foldid, w.V, TOL, MAXIT, smooth0=w.smooth0, eta=w.eta,
+                            rounds=w.rounds, taus=w.taus if len(w.taus) else None, warm_tol=WARM_TOL)
+    info = path.info()
+    assert info["flags"].sum() == 0 and np.all(info["kkt"] <= TOL)
+    cv_loss, cv_err, cv_mean, best = tkm.tkm_exact_cv(path, y, foldid, w.T, w.L, w.V)
+    L, V = w.L, w.V
+    smooth_final = w.smooth0 * w.eta ** (w.rounds - 1)
+    cols = [(t * (V + 1) + v) * L + l for (t, v, l) in
+            [(0, 0, 0), (0, 1, L // 3), (0, V, L // 2), (w.T - 1, V - 1, (3 * L) // 4), (w.T - 1, 2, L - 1)]]
+    worst, fs = _first_order(w, tkm, path, K, w.y, foldid, cols, smooth_final)
+    print("cfg %d: |sum z| %.2e, n_c||z + 2 lam alpha||/sqrt(n) %.2e, held-out alpha %.2e" % (cfg, *worst))
+    assert worst[0] <= 20 * TOL and worst[1] <= 20 * TOL and worst[2] <= 1e-7
+    for c in cols:
+        t, v, l = c // ((V + 1) * L), (c // L) % (V + 1), c % L
+        if v == V:
+            continue
+        r = np.nonzero(foldid == v)[0]
+        tau = w.taus[t] if len(w.taus) else None
+        want = np.mean(o.nominal_loss(w.loss, w.y[r], fs[c][r], tau))
+        assert abs(cv_loss[t, l, v] - want) <= 1e-5
+        if w.loss != o.LOSS_QUANTILE:
+            assert cv_err[t, l, v] == int(np.sum(np.where(fs[c][r] >= 0, 1.0, -1.0) != w.y[r]))
+    # selected lambda = argmin of the pooled mean, ties -> largest lambda (G14), recomputed on the host
+    fsize = np.bincount(foldid, minlength=V).astype(np.float64)
+    pooled = (cv_loss * fsize).sum(axis=2) / w.n
+    assert np.max(np.abs(pooled - cv_mean)) <= 1e-12
+    assert np.array_equal(best, np.array([int(np.flatnonzero(p == p.min())[0]) for p in pooled]))
+    del K
+    torch.cuda.empty_cache()
+
+
+def test_nystrom_config4_first_order_optimality(tkm):
+    """configs[4]: n = 100000, m = 4096 landmarks.  The model is the minimiser of the problem with
+    K~ = K_nm K_mm^+ K_nm^T (reading G11); with alpha~ = -z/(2 lambda) its decision values must satisfy
+    f = K~ alpha~ + beta0 and sum z = 0, where f is evaluated from the landmark weights the library returns."""
+    import torch
+    w = wl.config4()
+    sigma = float(w.sigmas[0])
+    idx = wl.landmarks(w.n, w.m_landmarks, w.landmark_seed)
+    foldid = tkm.tkm_make_folds(w.n, w.V, w.fold_seed)
+    X, y = _dev(w.X), _dev(w.y)
+    Xl = X[_dev(idx)]
+    K_nm = tkm.tkm_gram(X, sigma, Xl)
+    K_mm = tkm.tkm_gram(Xl, sigma)
+    rng = np.random.default_rng(4)
+    ii, jj, got = _check_gram_entries(K_nm, w.X, sigma, rng)
+    d2 = ((w.X[ii] - w.X[idx[jj]]) ** 2).sum(axis=1)
+    assert np.max(np.abs(got - np.exp(-d2 / (2 * sigma * sigma)))) < 1e-13
+    spec = tkm.tkm_spectral_setup(nystrom=(K_nm, K_mm, idx))
+    assert spec.n == w.n and 0 < spec.r <= w.m_landmarks
+    path = tkm.tkm_fit_path(spec, y, w.loss, w.lambdas, foldid, w.V, TOL, MAXIT, smooth0=w.smooth0, eta=w.eta,
+                            rounds=w.rounds, warm_tol=WARM_TOL)
+    info = path.info()
+    assert info["flags"].sum() == 0 and np.all(info["kkt"] <= TOL)
+    cv_loss, cv_err, cv_mean, best = tkm.tkm_exact_cv(path, y, foldid, 1, w.L, w.V)
+    # K_mm^+ with the truncation of reading G11
+    th, W = torch.linalg.eigh(K_mm)
+    keep = th > 1e-12 * th.max()
+    Wk, thk = W[:, keep], th[keep]
+    L, V = w.L, w.V
+    smooth_final = w.smooth0 * w.eta ** (w.rounds - 1)
+    for (v, l) in [(0, 0), (1, L // 3), (V, L // 2), (V - 1, (3 * L) // 4), (2, L - 1)]:
+        gam, b0 = tkm.tkm_path_coef(path, 0, l, v)
+        f = torch.mv(K_nm, gam[:w.m_landmarks]) + b0
+        f_np = f.cpu().numpy()
+        M = (foldid != v).astype(np.float64)
+        nc = M.sum()
+        z = M * o.psi(w.loss, w.y, f_np, smooth_final) / nc
+        assert abs(z.sum()) <= 20 * TOL
+        at = _dev(-z / (2.0 * w.lambdas[l]))
+        t1 = torch.mv(K_nm.T, at)
+        f_def = torch.mv(K_nm, torch.mv(Wk, torch.mv(Wk.T, t1) / thk)) + b0
+        err = float((f_def - f).abs().max() / max(1.0, float(f.abs().max())))
+        print("cfg 4 (v=%d, l=%d): |sum z| %.2e, max |f - (K~ alpha~ + b0)| %.2e" % (v, l, abs(z.sum()), err))
+        assert err <= 1e-6
+        if v < V:
+            r = np.nonzero(foldid == v)[0]
+            assert abs(cv_loss[0, l, v] - np.mean(o.nominal_loss(w.loss, w.y[r], f_np[r]))) <= 1e-5
+            assert cv_err[0, l, v] == int(np.sum(np.where(f_np[r] >= 0, 1.0, -1.0) != w.y[r]))
