@@ -208,6 +208,13 @@ int tkm_dgemm_nt(const double* P, int64_t ldp, const double* Q, int64_t ldq, dou
  * per launch.  Synchronises `stream`. */
 int tkm_gemm_probe(int32_t cfg, int32_t G, int32_t N, int32_t M, int32_t K, int32_t iters, float* ms,
                    void* stream);
+/* 3xTF32 contraction on the tcgen05 tensor cores (the FP32 variant of the sweep's products), test and
+ * calibration entry: Dt[N][M] (FP64, [dev]) = P[N][K] Q[M][K]^T with the FP64 inputs split on the fly into
+ * TF32 (hi, lo) pairs and accumulated in FP32 as lo*hi + hi*lo + hi*hi.  cfg: 0/1/2 = 64/128/256 slots per
+ * tile, -1 = chosen from N.  ms [host] NULL or the milliseconds per launch over `iters` timed launches.
+ * Synchronises `stream`. */
+int tkm_tf32x3_gemm_nt(const double* P, int64_t ldp, const double* Q, int64_t ldq, double* Dt, int64_t ldd,
+                       int64_t N, int64_t M, int64_t K, int32_t cfg, int32_t iters, float* ms, void* stream);
 int tkm_version(void);
 const char* tkm_last_error(void);
 

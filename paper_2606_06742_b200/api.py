@@ -15,7 +15,7 @@ EXPORTED_SYMBOLS = [
     "tkm_gram", "tkm_spectral_setup", "tkm_spectral_setup_multi", "tkm_spectral_free", "tkm_spectral_info", "tkm_spectral_get_u",
     "tkm_fit_path", "tkm_fit_path_multi", "tkm_path_free", "tkm_path_info", "tkm_path_profile", "tkm_path_get_a", "tkm_exact_cv", "tkm_path_coef",
     "tkm_predict", "tkm_train_tune_host", "tkm_make_folds", "tkm_launch_count", "tkm_launch_count_reset",
-    "tkm_dgemm_nt", "tkm_gemm_probe", "tkm_version", "tkm_last_error",
+    "tkm_dgemm_nt", "tkm_gemm_probe", "tkm_tf32x3_gemm_nt", "tkm_version", "tkm_last_error",
 ]
 
 
@@ -79,6 +79,7 @@ def lib():
     L.tkm_launch_count.restype = i64
     L.tkm_launch_count_reset.restype = None
     L.tkm_dgemm_nt.argtypes = [vp, i64, vp, i64, vp, i64, i64, i64, i64, vp]
+    L.tkm_tf32x3_gemm_nt.argtypes = [vp, i64, vp, i64, vp, i64, i64, i64, i64, i32, i32, C.POINTER(C.c_float), vp]
     L.tkm_gemm_probe.argtypes = [i32, i32, i32, i32, i32, i32, C.POINTER(C.c_float), vp]
     L.tkm_last_error.restype = C.c_char_p
     for name in EXPORTED_SYMBOLS:
@@ -383,3 +384,17 @@ def tkm_gemm_probe(cfg: int, G: int, N: int, M: int, K: int, iters: int = 20, st
     ms = C.c_float()
     _check(lib().tkm_gemm_probe(cfg, G, N, M, K, iters, C.byref(ms), _stream(stream)))
     return float(ms.value)
+
+
+def tkm_tf32x3_gemm_nt(P, Q, cfg=-1, iters=0, stream=None):
+    """Dt[N][M] = P[N][K] Q[M][K]^T on the 3xTF32 tcgen05 kernel (FP64 in/out, FP32 accumulation).
+    Returns D, or (D, ms per launch) when iters > 0."""
+    import torch
+    P, Q = _dev_f64(P, "P"), _dev_f64(Q, "Q")
+    N, K = P.shape
+    M = Q.shape[0]
+    D = torch.empty((N, M), device="cuda", dtype=torch.float64)
+    ms = C.c_float()
+    _check(lib().tkm_tf32x3_gemm_nt(P.data_ptr(), P.stride(0), Q.data_ptr(), Q.stride(0), D.data_ptr(), M, N, M, K,
+                                    cfg, iters, C.byref(ms) if iters > 0 else None, _stream(stream)))
+    return (D, float(ms.value)) if iters > 0 else D

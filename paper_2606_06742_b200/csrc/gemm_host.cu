@@ -44,6 +44,24 @@ int make_tmap_f64(CUtensorMap* out, const double* base, int64_t rows, int64_t co
   return TKM_OK;
 }
 
+// FP32 twin for the 3xTF32 kernel: box = box_rows x 32 floats (128 B), 128-byte swizzle.
+int make_tmap_f32(CUtensorMap* out, const float* base, int64_t rows, int64_t cols, int64_t ld, int box_rows) {
+  EncodeTiledFn fn = encode_fn();
+  if (!fn) return set_error(TKM_ECUDA, "cuTensorMapEncodeTiled is not available from this driver");
+  if ((reinterpret_cast<uintptr_t>(base) & 15) || (ld & 3) || rows < 1 || cols < 1 || ld < cols || box_rows < 1 ||
+      box_rows > 256)
+    return set_error(TKM_EINVAL, "FP32 GEMM operand needs a 16-byte aligned base and a leading dimension % 4 == 0");
+  const cuuint64_t gdim[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+  const cuuint64_t gstride[1] = {(cuuint64_t)ld * sizeof(float)};
+  const cuuint32_t box[2] = {32u, (cuuint32_t)box_rows};
+  const cuuint32_t estr[2] = {1, 1};
+  CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(base), gdim, gstride, box, estr,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return set_error(TKM_ECUDA, "cuTensorMapEncodeTiled (f32) failed with CUresult %d", (int)r);
+  return TKM_OK;
+}
+
 static int g_forced_cfg = -1;
 int gemm_f64_force_cfg(int cfg) {
   const int old = g_forced_cfg;

@@ -112,7 +112,7 @@ def test_full_kernel_configs_first_order_optimality(tkm, cfg):
 
 def test_nystrom_config4_first_order_optimality(tkm):
     """configs[4]: n = 100000, m = 4096 landmarks.  The model is the minimiser of the problem with
-    K~ = K_nm K_mm^+ K_nm^T (reading G11); with alpha~ = -z/(2 lambda) its decision values must satisfy
+    K~ = K_nm K_mm^+ K_nm^T restricted to its numerically non-null directions (reading G11); with alpha~ = -z/(2 lambda) its decision values must satisfy
     f = K~ alpha~ + beta0 and sum z = 0, where f is evaluated from the landmark weights the library returns."""
     import torch
     w = wl.config4()
@@ -137,7 +137,10 @@ def test_nystrom_config4_first_order_optimality(tkm):
     # K_mm^+ with the truncation of reading G11
     th, W = torch.linalg.eigh(K_mm)
     keep = th > 1e-12 * th.max()
-    Wk, thk = W[:, keep], th[keep]
+    Phi = K_nm @ (W[:, keep] / torch.sqrt(th[keep]))     # K~ = Phi Phi^T: the well-conditioned way to apply K_mm^+
+    lam2, Q2 = torch.linalg.eigh(Phi.T @ Phi)            # second truncation of reading G11
+    Phi = Phi @ Q2[:, lam2 > 1e-12 * lam2.max()]
+    assert Phi.shape[1] == spec.r
     L, V = w.L, w.V
     smooth_final = w.smooth0 * w.eta ** (w.rounds - 1)
     for (v, l) in [(0, 0), (1, L // 3), (V, L // 2), (V - 1, (3 * L) // 4), (2, L - 1)]:
@@ -149,8 +152,7 @@ def test_nystrom_config4_first_order_optimality(tkm):
         z = M * o.psi(w.loss, w.y, f_np, smooth_final) / nc
         assert abs(z.sum()) <= 20 * TOL
         at = _dev(-z / (2.0 * w.lambdas[l]))
-        t1 = torch.mv(K_nm.T, at)
-        f_def = torch.mv(K_nm, torch.mv(Wk, torch.mv(Wk.T, t1) / thk)) + b0
+        f_def = torch.mv(Phi, torch.mv(Phi.T, at)) + b0
         err = float((f_def - f).abs().max() / max(1.0, float(f.abs().max())))
         print("cfg 4 (v=%d, l=%d): |sum z| %.2e, max |f - (K~ alpha~ + b0)| %.2e" % (v, l, abs(z.sum()), err))
         assert err <= 1e-6

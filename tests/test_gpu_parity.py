@@ -343,3 +343,22 @@ def test_train_tune_host_matches_oracle(tkm):
         alpha_o = so.U @ res.a[:, c]
         assert np.linalg.norm(r["alpha"][g] - alpha_o) <= COEF_TOL_F64 * np.linalg.norm(alpha_o)
         assert abs(r["beta0"][g] - res.beta0[c]) <= 1e-9 * max(1.0, abs(res.beta0[c]))
+
+
+# ------------------------------------------------------------------------------- tcgen05 3xTF32 contraction
+@pytest.mark.parametrize("N,M,K,cfg", [(64, 128, 32, 0), (37, 130, 70, 0), (128, 256, 512, 1), (300, 2000, 2000, -1),
+                                       (100, 333, 1001, 2)])
+def test_tf32x3_gemm_nt(tkm, N, M, K, cfg):
+    """The tcgen05 (TMEM accumulator) 3xTF32 product against FP64: the error is that of FP32 accumulation in the
+    tensor core, which truncates -- it grows like K 2^-24 relative to the size of the partial sums."""
+    import torch
+    g = torch.Generator(device="cuda").manual_seed(N + M + K)
+    P = torch.randn((N, K), device="cuda", dtype=torch.float64, generator=g)
+    Q = torch.randn((M, K), device="cuda", dtype=torch.float64, generator=g)
+    D = tkm.tkm_tf32x3_gemm_nt(P, Q, cfg=cfg)
+    ref = P @ Q.T
+    err = float((D - ref).abs().max())
+    bound = 4.0 * K * 2.0 ** -24 * float(np.sqrt(K)) + 1e-5      # ~ (K/8 x 3 accumulations) ulps of sqrt(K)-sized sums
+    assert err <= bound, (err, bound)
+    plain_tf32 = float(np.sqrt(K)) * 2.0 ** -11                   # what a single TF32 product would give
+    assert err < 0.05 * plain_tf32
