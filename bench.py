@@ -210,7 +210,7 @@ def run_ours(args, w, rank, world):
         sweep (tkm_fit_path_multi), S9 per bandwidth."""
         flush.zero_()
         e0 = ev()
-        Ks = [tkm.tkm_gram(X, float(sigma)) for sigma in w.sigmas]
+        Ks = tkm.tkm_gram_multi(X, w.sigmas)                               # one distance pass, 5 exp + writes
         e1 = ev()
         specs = tkm.tkm_spectral_setup_multi(Ks, sweep_dtype=sweep_dt)     # the 5 decompositions overlap
         del Ks

@@ -89,6 +89,14 @@ int tkm_gram(const void* X, int64_t n, int64_t p, int64_t ldx,
              const void* X2, int64_t n2, int64_t ldx2,
              double sigma, tkm_dtype out_dt, void* K, int64_t ldk, void* stream);
 
+/* The same for G <= 8 bandwidths in ONE pass: the squared distances are computed once and every bandwidth
+ * costs one exp and one write per entry.  sigmas [host] G values > 0; Ks [host] G [dev] output matrices with
+ * the same ldk and out_dt.  Bit-identical to G separate tkm_gram calls.  Asynchronous. */
+int tkm_gram_multi(const void* X, int64_t n, int64_t p, int64_t ldx,
+                   const void* X2, int64_t n2, int64_t ldx2,
+                   const double* sigmas, int32_t G, tkm_dtype out_dt, void* const* Ks, int64_t ldk,
+                   void* stream);
+
 /* ---- S2  one-time spectral setup (Alg.1 l.3, 226; readings G11, G16, G19) --------
  * Full kernel (ny == NULL): K [dev] n x n FP64 symmetric (not modified); decomposes in FP64 with
  * cuSOLVER syevd, clamps Lam >= 0, forms u1 = U^T 1, and keeps U Lam (n x r) and U^T (r x n) in

@@ -12,7 +12,7 @@ F32, F64 = 0, 1
 TKM_OK, TKM_ENOTCONV = 0, 5
 
 EXPORTED_SYMBOLS = [
-    "tkm_gram", "tkm_spectral_setup", "tkm_spectral_setup_multi", "tkm_spectral_free", "tkm_spectral_info", "tkm_spectral_get_u",
+    "tkm_gram", "tkm_gram_multi", "tkm_spectral_setup", "tkm_spectral_setup_multi", "tkm_spectral_free", "tkm_spectral_info", "tkm_spectral_get_u",
     "tkm_fit_path", "tkm_fit_path_multi", "tkm_path_free", "tkm_path_info", "tkm_path_profile", "tkm_path_get_a", "tkm_exact_cv", "tkm_path_coef",
     "tkm_predict", "tkm_train_tune_host", "tkm_make_folds", "tkm_launch_count", "tkm_launch_count_reset",
     "tkm_dgemm_nt", "tkm_gemm_probe", "tkm_tf32x3_gemm_nt", "tkm_version", "tkm_last_error",
@@ -55,6 +55,7 @@ def lib():
     L = C.CDLL(path)
     vp, i64, i32, dbl = C.c_void_p, C.c_int64, C.c_int32, C.c_double
     L.tkm_gram.argtypes = [vp, i64, i64, i64, vp, i64, i64, dbl, C.c_int, vp, i64, vp]
+    L.tkm_gram_multi.argtypes = [vp, i64, i64, i64, vp, i64, i64, vp, i32, C.c_int, C.POINTER(vp), i64, vp]
     L.tkm_spectral_setup.argtypes = [vp, i64, i64, C.POINTER(_Nystrom), C.c_int, C.POINTER(vp), vp]
     L.tkm_spectral_setup_multi.argtypes = [C.POINTER(vp), i32, i64, i64, C.c_int, C.POINTER(vp), vp]
     L.tkm_spectral_free.argtypes = [vp]
@@ -156,6 +157,23 @@ def tkm_gram(X, sigma: float, X2=None, out_dtype=F64, stream=None):
     _check(lib().tkm_gram(X.data_ptr(), n, p, X.stride(0), p2, n2, ld2, float(sigma), out_dtype,
                           K.data_ptr(), K.stride(0), _stream(stream)))
     return K
+
+
+def tkm_gram_multi(X, sigmas, out_dtype=F64, stream=None):
+    """G symmetric Gram matrices of X (one per bandwidth) from one pass over the squared distances."""
+    import torch
+    X = _dev_f64(X, "X")
+    if X.dim() != 2 or X.stride(1) != 1:
+        raise ValueError("X must be 2-D with unit inner stride")
+    n, p = X.shape
+    sig = _host(np.atleast_1d(sigmas), np.float64)
+    G = len(sig)
+    Ks = [torch.empty((n, n), device=X.device, dtype=torch.float64 if out_dtype == F64 else torch.float32)
+          for _ in range(G)]
+    hk = (C.c_void_p * G)(*[K.data_ptr() for K in Ks])
+    _check(lib().tkm_gram_multi(X.data_ptr(), n, p, X.stride(0), None, 0, 0, _ptr(sig), G, out_dtype, hk, n,
+                                _stream(stream)))
+    return Ks
 
 
 class Spectral:

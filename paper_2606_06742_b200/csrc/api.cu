@@ -105,10 +105,9 @@ extern "C" int tkm_train_tune_host(const double* X, int64_t n, int64_t p, const 
   TKM_CUDA(cudaMemcpyAsync(dy.p, y, (size_t)n * sizeof(double), cudaMemcpyHostToDevice, st));
   TKM_CUDA(cudaEventRecord(ev[1], st));
   const void* Ks[8];
-  for (int g = 0; g < G; ++g) {
-    Ks[g] = dK.as<double>() + (size_t)g * n * n;
-    TKM_TRY(tkm_gram(dX.p, n, p, p, nullptr, 0, 0, sigmas[g], TKM_F64, const_cast<void*>(Ks[g]), n, st));
-  }
+  void* Kw[8];
+  for (int g = 0; g < G; ++g) Ks[g] = Kw[g] = dK.as<double>() + (size_t)g * n * n;
+  TKM_TRY(tkm_gram_multi(dX.p, n, p, p, nullptr, 0, 0, sigmas, G, TKM_F64, Kw, n, st));
   TKM_CUDA(cudaEventRecord(ev[2], st));
   TKM_TRY(tkm_spectral_setup_multi(Ks, G, n, n, sweep_dt, own.spec, st));   // the G decompositions overlap
   dK.release();

@@ -155,7 +155,10 @@ def test_nystrom_config4_first_order_optimality(tkm):
         f_def = torch.mv(Phi, torch.mv(Phi.T, at)) + b0
         err = float((f_def - f).abs().max() / max(1.0, float(f.abs().max())))
         print("cfg 4 (v=%d, l=%d): |sum z| %.2e, max |f - (K~ alpha~ + b0)| %.2e" % (v, l, abs(z.sum()), err))
-        assert err <= 1e-6
+        # f - f_def = U Lam rho / (2 lambda) with rho the stationarity residual the stop test bounds (G6):
+        # n_c ||rho|| / sqrt(n) <= TOL, so the admissible gap grows like 1/lambda
+        bound = 1e-8 + float(lam2.max()) * TOL * np.sqrt(w.n) / (nc * 2.0 * w.lambdas[l])
+        assert err <= bound, (err, bound)
         if v < V:
             r = np.nonzero(foldid == v)[0]
             assert abs(cv_loss[0, l, v] - np.mean(o.nominal_loss(w.loss, w.y[r], f_np[r]))) <= 1e-5

@@ -360,5 +360,41 @@ def test_tf32x3_gemm_nt(tkm, N, M, K, cfg):
     err = float((D - ref).abs().max())
     bound = 4.0 * K * 2.0 ** -24 * float(np.sqrt(K)) + 1e-5      # ~ (K/8 x 3 accumulations) ulps of sqrt(K)-sized sums
     assert err <= bound, (err, bound)
-    plain_tf32 = float(np.sqrt(K)) * 2.0 ** -11                   # what a single TF32 product would give
-    assert err < 0.05 * plain_tf32
+    plain_tf32 = float(np.sqrt(K)) * 2.0 ** -11                   # rms error of a single-TF32 product sum
+    assert err < 0.25 * plain_tf32                                # max over all outputs vs that rms
+
+
+def test_gram_multi_bit_identical_to_single(tkm):
+    rng = np.random.default_rng(3)
+    X = rng.standard_normal((333, 17))
+    sig = [1.1, 2.9, 7.0]
+    Ks = tkm.tkm_gram_multi(dev(X), sig)
+    for s, K in zip(sig, Ks):
+        K1 = tkm.tkm_gram(dev(X), s)
+        assert bool((K == K1).all())
+        Kn = K.cpu().numpy()
+        assert np.array_equal(Kn, Kn.T) and np.all(np.diag(Kn) == 1.0)
+        assert np.max(np.abs(Kn - o.gram_rbf(X, s)) / o.gram_rbf(X, s)) < 1e-13
+    with pytest.raises(tkm.TkmError):
+        tkm.tkm_gram_multi(dev(X), [1.0, 0.0])
+
+
+def test_leave_one_out_form(tkm):
+    """Algorithm 1 in its printed leave-one-out form: V = n folds of one sample each,
+    B = L (n + 1) columns.  Every held-out decision value must equal the oracle's."""
+    w = wl.config0(n=48, p=4, L=3, V=48, seed=13)
+    sigma = float(w.sigmas[0])
+    foldid = tkm.tkm_make_folds(w.n, w.V, w.fold_seed)
+    assert sorted(foldid.tolist()) == list(range(w.n))                       # a permutation: one row per fold
+    X, y, spec, path, cv = _run_gpu(tkm, w, sigma, foldid, STOP_TOL, 400000)
+    assert path.B == w.L * (w.n + 1)
+    res, spec_o, worst, degenerate = _compare_path(tkm, w, sigma, foldid, spec, path, cv)
+    cv_o = o.exact_cv(spec_o, res, w.y, foldid, w.loss, w.taus)
+    keep = np.ones((1, w.L, w.V), dtype=bool)
+    for c in degenerate:
+        if (c // w.L) % (w.V + 1) < w.V:
+            keep[0, c % w.L, (c // w.L) % (w.V + 1)] = False
+    assert np.max(np.abs(cv[0] - cv_o[0])[keep]) <= CV_TOL
+    assert np.array_equal(cv[1][keep], cv_o[1][keep])
+    if not degenerate:
+        assert np.array_equal(cv[3], cv_o[3])
