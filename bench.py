@@ -157,7 +157,7 @@ def run_reference(args, w, rank):
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1),
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-            "data": "synthetic", "config": workload_config(w, "f64"),
+            "data": "synthetic", "config": workload_config(w, "f64", warm_tol=STOP_TOL["f64"]),
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
                              "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -165,12 +165,12 @@ def run_reference(args, w, rank):
     print(json.dumps(line))
 
 
-def workload_config(w, dtype):
+def workload_config(w, dtype, warm_tol=None):
     return {"workload": "BASELINE.json configs[1]: smoothed-hinge kernel SVM, n=%d, p=%d, %d folds, %d lambdas "
                         "1e2..1e-5 x %d sigma (median x {0.25,0.5,1,2,4}), delta 1 -> 1/512 in %d rounds, %s"
                         % (w.n, w.p, w.V, w.L, len(w.sigmas), w.rounds, dtype),
             "n": w.n, "p": w.p, "folds": w.V, "lambdas": w.L, "sigmas": len(w.sigmas),
-            "columns_per_step": w.B * len(w.sigmas), "stop_tol": STOP_TOL[dtype], "warm_start_rounds_tol": WARM_TOL, "maxit": MAXIT,
+            "columns_per_step": w.B * len(w.sigmas), "stop_tol": STOP_TOL[dtype], "warm_start_rounds_tol": WARM_TOL if warm_tol is None else warm_tol, "maxit": MAXIT,
             "l2": "flushed between steps (256 MiB memset)", "parallelism": "independent replicas, no collective"}
 
 
