@@ -28,7 +28,7 @@ results): delta_0, R, tol, maxit, the t3 noise scale, the landmark seed.
 """
 from .gram import gram_rbf
 from .spectral import spectral_setup, Spectral
-from .losses import psi, curvature, nominal_loss, smooth_loss, LOSS_HINGE, LOSS_LOGISTIC, LOSS_QUANTILE
+from .losses import psi, curvature, nominal_loss, smooth_loss, LOSS_HINGE, LOSS_LOGISTIC, LOSS_QUANTILE, LOSS_DWD
 from .folds import make_folds, splitmix64_stream
 from .path import (column_table, column_constants, fit_column, fit_path, PathResult,
                    smoothing_levels, path_coef)

@@ -5,6 +5,9 @@ nominal loss = the non-smoothed loss used to score cross-validation.
 
   smoothed hinge   PAPER.md:138 (L_delta), kappa = 2 delta
   logistic         not printed: reading G9, log(1 + exp(-y f)), curv 1/4
+  DWD              not printed (PAPER.md:47, 81, 85 name the estimator; it cites Wang and Zou 2018): reading
+                   G20, the generalised DWD loss with q = 1,  V(u) = 1 - u (u <= 1/2), 1/(4u) (u > 1/2),
+                   which is C^1 with sup V'' = V''(1/2+) = 4; no smoothing round
   smoothed check   not printed: reading G10, the C^1 quadratic blend of the
                    check loss rho_tau on [-gamma, gamma], curvature 1/(2 gamma)
 """
@@ -13,6 +16,7 @@ import numpy as np
 LOSS_HINGE = 0
 LOSS_LOGISTIC = 1
 LOSS_QUANTILE = 2
+LOSS_DWD = 3
 
 
 def curvature(loss, smooth):
@@ -23,6 +27,8 @@ def curvature(loss, smooth):
         return 0.25
     if loss == LOSS_QUANTILE:
         return 1.0 / (2.0 * smooth)
+    if loss == LOSS_DWD:
+        return 4.0                           # V''(u) = 1/(2 u^3) on u > 1/2, largest at u = 1/2
     raise ValueError(loss)
 
 
@@ -47,6 +53,10 @@ def psi(loss, y, f, smooth=None, tau=None):
         t = y - f
         hp = np.where(t < -g, tau - 1.0, np.where(t > g, tau, t / (2.0 * g) + tau - 0.5))
         return -hp
+    if loss == LOSS_DWD:
+        u = y * f
+        us = np.maximum(u, 0.5)               # keeps the unused branch finite
+        return y * np.where(u <= 0.5, -1.0, -1.0 / (4.0 * us * us))
     raise ValueError(loss)
 
 
@@ -67,6 +77,9 @@ def smooth_loss(loss, y, f, smooth=None, tau=None):
         t = y - f
         return np.where(t < -g, (tau - 1.0) * t,
                         np.where(t > g, tau * t, t * t / (4.0 * g) + t * (tau - 0.5) + g / 4.0))
+    if loss == LOSS_DWD:
+        u = y * f
+        return np.where(u <= 0.5, 1.0 - u, 1.0 / (4.0 * np.maximum(u, 0.5)))
     raise ValueError(loss)
 
 
@@ -82,4 +95,7 @@ def nominal_loss(loss, y, f, tau=None):
     if loss == LOSS_QUANTILE:
         t = y - f
         return t * (tau - (t < 0))
+    if loss == LOSS_DWD:
+        u = y * f
+        return np.where(u <= 0.5, 1.0 - u, 1.0 / (4.0 * np.maximum(u, 0.5)))
     raise ValueError(loss)

@@ -25,7 +25,7 @@ out" (the final model for (t, l)).
 import dataclasses
 import numpy as np
 
-from .losses import psi, curvature, LOSS_HINGE, LOSS_LOGISTIC, LOSS_QUANTILE
+from .losses import psi, curvature, LOSS_HINGE, LOSS_LOGISTIC, LOSS_QUANTILE, LOSS_DWD
 
 
 @dataclasses.dataclass
@@ -42,7 +42,7 @@ class PathResult:
 def smoothing_levels(loss, smooth0, eta, rounds):
     """delta_k (hinge) / gamma_k (quantile) = smooth0 eta^k, k = 0..R-1; logistic: [None].
     PAPER.md:182, 220 (eta = 0.125); reading G7 (fixed R)."""
-    if loss == LOSS_LOGISTIC:
+    if loss in (LOSS_LOGISTIC, LOSS_DWD):
         return [None]
     return [smooth0 * eta ** k for k in range(rounds)]
 

@@ -5,7 +5,7 @@ import pytest
 
 import oracle as o
 import workloads as wl
-from oracle import LOSS_HINGE, LOSS_LOGISTIC, LOSS_QUANTILE
+from oracle import LOSS_HINGE, LOSS_LOGISTIC, LOSS_QUANTILE, LOSS_DWD
 
 
 def _data(loss, n, p=4, seed=21):
@@ -21,7 +21,7 @@ def _data(loss, n, p=4, seed=21):
 
 # ------------------------------------------------------------ P7 / P8
 @pytest.mark.parametrize("loss,taus,rounds", [(LOSS_HINGE, (), 3), (LOSS_LOGISTIC, (), 1),
-                                              (LOSS_QUANTILE, (0.1, 0.9), 3)])
+                                              (LOSS_QUANTILE, (0.1, 0.9), 3), (LOSS_DWD, (), 1)])
 def test_exact_cv_equals_brute_force_refit(loss, taus, rounds):
     n, V = 64, 4
     X, y, sigma = _data(loss, n)

@@ -9,7 +9,7 @@ import pytest
 
 import oracle as o
 import workloads as wl
-from oracle import LOSS_HINGE, LOSS_LOGISTIC, LOSS_QUANTILE
+from oracle import LOSS_HINGE, LOSS_LOGISTIC, LOSS_QUANTILE, LOSS_DWD
 
 
 def _problem(loss, n=50, p=4, seed=5):
@@ -39,7 +39,8 @@ def test_smoothed_hinge_matches_printed_formula():
 
 
 @pytest.mark.parametrize("loss,smooth,tau", [(LOSS_HINGE, 0.3, None), (LOSS_LOGISTIC, None, None),
-                                             (LOSS_QUANTILE, 0.2, 0.1), (LOSS_QUANTILE, 0.2, 0.9)])
+                                             (LOSS_QUANTILE, 0.2, 0.1), (LOSS_QUANTILE, 0.2, 0.9),
+                                             (LOSS_DWD, None, None)])
 def test_psi_is_derivative_and_curvature_bounds_it(loss, smooth, tau):
     rng = np.random.default_rng(1)
     y = np.where(rng.random(400) < 0.5, 1.0, -1.0) if loss != LOSS_QUANTILE else rng.standard_normal(400)
@@ -67,7 +68,7 @@ def test_quantile_nominal_is_check_loss():
 
 # ---------------------------------------------------------------- P3: spectral step == dense solve
 @pytest.mark.parametrize("loss,smooth,tau", [(LOSS_HINGE, 0.125, None), (LOSS_LOGISTIC, None, None),
-                                             (LOSS_QUANTILE, 0.125, 0.3)])
+                                             (LOSS_QUANTILE, 0.125, 0.3), (LOSS_DWD, None, None)])
 def test_spectral_step_equals_dense_majoriser_solve(loss, smooth, tau):
     X, y, K, spec, foldid = _problem(loss, n=40)
     n = len(y)
@@ -128,7 +129,7 @@ def test_huge_gamma_one_step_is_least_squares_kqr():
 
 # ---------------------------------------------------------------- P5: MM descent
 @pytest.mark.parametrize("loss,smooth,tau", [(LOSS_HINGE, 0.125, None), (LOSS_LOGISTIC, None, None),
-                                             (LOSS_QUANTILE, 0.125, 0.9)])
+                                             (LOSS_QUANTILE, 0.125, 0.9), (LOSS_DWD, None, None)])
 def test_objective_never_increases_without_momentum(loss, smooth, tau):
     X, y, K, spec, foldid = _problem(loss, n=40)
     mask = (foldid != 0).astype(float)
@@ -142,7 +143,8 @@ def test_objective_never_increases_without_momentum(loss, smooth, tau):
 
 
 # ---------------------------------------------------------------- P6: KKT at convergence
-@pytest.mark.parametrize("loss,taus", [(LOSS_HINGE, ()), (LOSS_LOGISTIC, ()), (LOSS_QUANTILE, (0.1, 0.5, 0.9))])
+@pytest.mark.parametrize("loss,taus", [(LOSS_HINGE, ()), (LOSS_LOGISTIC, ()), (LOSS_QUANTILE, (0.1, 0.5, 0.9)),
+                                       (LOSS_DWD, ())])
 def test_kkt_of_every_path_solution(loss, taus):
     X, y, K, spec, foldid = _problem(loss, n=48)
     lambdas = wl.lambda_grid(0, -4, 4)
@@ -275,3 +277,39 @@ def test_kqr_residual_fraction_and_path_ordering():
             fit.append(np.mean(o.smooth_loss(LOSS_QUANTILE, y, f, g, tau)))
         # lambdas descending: penalty non-decreasing, training loss non-increasing (P12)
         assert np.all(np.diff(pen) >= -1e-9) and np.all(np.diff(fit) <= 1e-9)
+
+
+# ---------------------------------------------------------------- DWD (reading G20)
+def test_dwd_loss_matches_its_definition_and_limits():
+    """Generalised DWD loss with q = 1 (Wang and Zou 2018, cited at PAPER.md:81): linear for u <= 1/2, 1/(4u)
+    beyond; C^1 at the joint, convex, and the large-lambda intercept has a closed form."""
+    u = np.array([-2.0, 0.0, 0.5, 0.5 + 1e-9, 1.0, 4.0])
+    got = o.smooth_loss(LOSS_DWD, np.ones_like(u), u)
+    assert np.allclose(got, [3.0, 1.0, 0.5, 0.5, 0.25, 0.0625], atol=1e-8)
+    assert np.allclose(o.psi(LOSS_DWD, np.ones(3), np.array([0.5 - 1e-12, 0.5 + 1e-12, 1.0])), [-1.0, -1.0, -0.25])
+    grid = np.linspace(0.5, 6.0, 4001)
+    curv = np.diff(o.psi(LOSS_DWD, np.ones_like(grid), grid)) / np.diff(grid)
+    assert curv.max() <= o.curvature(LOSS_DWD, None) + 1e-6 and curv.max() > 3.9 and curv.min() >= 0
+    # large lambda: alpha -> 0 and beta0 solves n+ V'(b) = n- V'(-b); for n+ > n-: b = sqrt(n+/n-)/2 > 1/2
+    n = 60
+    rng = np.random.default_rng(8)
+    K = o.gram_rbf(rng.standard_normal((n, 3)), 1.5)
+    spec = o.spectral_setup(K)
+    y = np.ones(n)
+    y[:21] = -1.0
+    a, b0, *_ = o.fit_column(spec, y, LOSS_DWD, [None], 1e7, np.ones(n), tol=1e-13, maxit=100000)
+    assert abs(b0 - 0.5 * np.sqrt(39.0 / 21.0)) < 1e-6
+    assert np.abs(spec.U @ a).max() < 1e-6
+
+
+def test_dwd_against_scipy_minimiser():
+    from scipy.optimize import minimize
+    X, y, K, spec, foldid = _problem(LOSS_DWD, n=30)
+    n = len(y)
+    lam = 1e-2
+    mask = (foldid != 0).astype(float)
+    a, b0, *_ = o.fit_column(spec, y, LOSS_DWD, [None], lam, mask, tol=1e-12, maxit=100000)
+    mine = o.objective(K, y, spec.U @ a, b0, lam, LOSS_DWD, mask, None)
+    best = minimize(lambda x: o.objective(K, y, x[1:], x[0], lam, LOSS_DWD, mask, None), np.zeros(n + 1),
+                    method="BFGS", options=dict(gtol=1e-10, maxiter=5000))
+    assert mine <= best.fun + 1e-12 and best.fun - mine < 1e-7
