@@ -48,7 +48,9 @@ typedef enum { TKM_F32 = 0, TKM_F64 = 1 } tkm_dtype;
 typedef enum {
   TKM_LOSS_HINGE = 0,    /* delta-smoothed hinge */
   TKM_LOSS_LOGISTIC = 1, /* log(1 + exp(-y f)); reading G9 */
-  TKM_LOSS_QUANTILE = 2  /* gamma-smoothed check loss; reading G10 */
+  TKM_LOSS_QUANTILE = 2, /* gamma-smoothed check loss; reading G10 */
+  TKM_LOSS_DWD = 3       /* distance-weighted discrimination; reading G20:   */
+                         /* V(u) = 1 - u (u <= 1/2), 1/(4u) (u > 1/2); smooth, one round           */
 } tkm_loss;
 
 typedef struct tkm_spectral tkm_spectral; /* K = U Lam U^T and derived device arrays */
@@ -124,7 +126,7 @@ int tkm_spectral_get_u(const tkm_spectral* s, double* U_out, void* stream);
  * (eq.(1), 166) at the final smoothing level, by the Nesterov-accelerated
  * majorise-minimise iteration applied through the spectral block inverse (all columns stacked,
  * two contractions with U per iteration).  State is kept in spectral coordinates a = U^T alpha.
- *   y       [dev]  n FP64 (+-1 for HINGE / LOGISTIC, checked; real for QUANTILE)
+ *   y       [dev]  n FP64 (+-1 for HINGE / LOGISTIC / DWD, checked; real for QUANTILE)
  *   lambdas [host] L values > 0          foldid [host] n values in [0, V), every fold non-empty
  *   tol     stop when max(|1^T z|, n_c ||rho||_2 / sqrt(n)) <= tol per column (reading G6)
  *   maxit   per column per round; columns that hit it are flagged and TKM_ENOTCONV is returned

@@ -7,7 +7,7 @@ import os
 
 import numpy as np
 
-LOSS_HINGE, LOSS_LOGISTIC, LOSS_QUANTILE = 0, 1, 2
+LOSS_HINGE, LOSS_LOGISTIC, LOSS_QUANTILE, LOSS_DWD = 0, 1, 2, 3
 F32, F64 = 0, 1
 TKM_OK, TKM_ENOTCONV = 0, 5
 

@@ -19,6 +19,10 @@ __device__ __forceinline__ double nominal_loss_dev(int loss, double y, double f,
     const double u = y * f;
     return fmax(-u, 0.0) + log1p(exp(-fabs(u)));
   }
+  if (loss == TKM_LOSS_DWD) {
+    const double u = y * f;
+    return (u <= 0.5) ? 1.0 - u : 1.0 / (4.0 * u);
+  }
   const double t = y - f;
   return t * (tau - (t < 0.0 ? 1.0 : 0.0));
 }

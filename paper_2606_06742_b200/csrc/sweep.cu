@@ -42,6 +42,9 @@ __device__ __forceinline__ double psi_dev(int loss, double y, double f, double s
     const double e = exp(-fabs(u));
     const double sg = (u >= 0.0) ? e / (1.0 + e) : 1.0 / (1.0 + e);
     return -y * sg;
+  } else if (loss == TKM_LOSS_DWD) {
+    const double u = y * f;   // V'(u) = -1 (u <= 1/2), -1/(4 u^2) (u > 1/2)   (reading G20)
+    return y * ((u <= 0.5) ? -1.0 : -1.0 / (4.0 * u * u));
   } else {
     const double t = y - f;   // -H'_gamma(t)  (reading G10)
     const double hp = (t < -smooth) ? tau - 1.0 : ((t > smooth) ? tau : t / (2.0 * smooth) + tau - 0.5);
@@ -511,7 +514,9 @@ __global__ void __launch_bounds__(256) compact_apply_kernel(CompactArgs p) {
 }
 
 static double curvature_of(tkm_loss loss, double smooth) {
-  return loss == TKM_LOSS_LOGISTIC ? 0.25 : 1.0 / (2.0 * smooth);   // 1/kappa, kappa = 2 delta
+  if (loss == TKM_LOSS_LOGISTIC) return 0.25;
+  if (loss == TKM_LOSS_DWD) return 4.0;   // sup V'' = V''(1/2+)
+  return 1.0 / (2.0 * smooth);   // 1/kappa, kappa = 2 delta
 }
 
 constexpr int POLL_RING = 3;   // batches whose poll results may be in flight
@@ -535,7 +540,7 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
     if (specs[g]->n != s0->n || specs[g]->r != s0->r || specs[g]->ldr != s0->ldr || specs[g]->ldn != s0->ldn ||
         specs[g]->sweep_dt != s0->sweep_dt)
       return set_error(TKM_EINVAL, "tkm_fit_path_multi: all spectral handles must share n, r and the sweep precision");
-  if (loss != TKM_LOSS_HINGE && loss != TKM_LOSS_LOGISTIC && loss != TKM_LOSS_QUANTILE)
+  if (loss != TKM_LOSS_HINGE && loss != TKM_LOSS_LOGISTIC && loss != TKM_LOSS_QUANTILE && loss != TKM_LOSS_DWD)
     return set_error(TKM_EINVAL, "tkm_fit_path: unknown loss %d", (int)loss);
   if (L < 1 || V < 2 || V > s0->n) return set_error(TKM_EINVAL, "tkm_fit_path: need L >= 1 and 2 <= V <= n");
   if (!(tol > 0.0) || maxit < 1) return set_error(TKM_EINVAL, "tkm_fit_path: need tol > 0 and maxit >= 1");
@@ -548,9 +553,10 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
     for (int t = 0; t < T; ++t)
       if (!(opts->taus[t] > 0.0 && opts->taus[t] < 1.0)) return set_error(TKM_EINVAL, "tkm_fit_path: tau must be in (0,1)");
   }
-  const int rounds = loss == TKM_LOSS_LOGISTIC ? 1 : opts->rounds;
+  const bool smoothed = loss == TKM_LOSS_HINGE || loss == TKM_LOSS_QUANTILE;   // logistic and DWD are smooth
+  const int rounds = smoothed ? opts->rounds : 1;
   if (rounds < 1) return set_error(TKM_EINVAL, "tkm_fit_path: rounds must be >= 1");
-  if (loss != TKM_LOSS_LOGISTIC && (!(opts->smooth0 > 0.0) || !(opts->eta > 0.0 && opts->eta <= 1.0)))
+  if (smoothed && (!(opts->smooth0 > 0.0) || !(opts->eta > 0.0 && opts->eta <= 1.0)))
     return set_error(TKM_EINVAL, "tkm_fit_path: need smooth0 > 0 and 0 < eta <= 1");
   if (s0->sweep_dt != TKM_F64) return set_error(TKM_ENOTIMPL, "tkm_fit_path: only the FP64 sweep is built");
   TKM_TRY(device_check());
@@ -731,7 +737,7 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
   int64_t prof_samples = 0;
   double smooth = opts->smooth0;
   for (int rnd = 0; rnd < rounds; ++rnd) {
-    if (loss != TKM_LOSS_LOGISTIC && rnd > 0) smooth *= opts->eta;   // PAPER.md:220 (Alg.1 l.22)
+    if (smoothed && rnd > 0) smooth *= opts->eta;   // PAPER.md:220 (Alg.1 l.22)
     const double curv = curvature_of(loss, smooth);
     const double rtol = (rnd + 1 < rounds && opts->warm_tol > 0.0) ? opts->warm_tol : tol;
     RoundArgs ra{(int)r, B, ldr, gp, curv, p0->col_lam.as<double>(), p0->col_nc.as<double>(), col_c.as<double>(),
@@ -859,7 +865,7 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
   bool notconv = false;
   for (int g = 0; g < G; ++g) {
     tkm_path* p = out[g];
-    p->smooth_final = loss == TKM_LOSS_LOGISTIC ? 0.0 : smooth;
+    p->smooth_final = smoothed ? smooth : 0.0;
     p->h_beta0.assign(hb.begin() + (size_t)g * B, hb.begin() + (size_t)(g + 1) * B);
     p->h_kkt.assign(hk.begin() + (size_t)g * B, hk.begin() + (size_t)(g + 1) * B);
     p->h_iters.assign(hi.begin() + (size_t)g * B, hi.begin() + (size_t)(g + 1) * B);

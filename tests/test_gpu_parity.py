@@ -141,7 +141,7 @@ def _compare_path(tkm, w, sigma, foldid, spec, path, cv, columns=None, coef_tol=
     return res, spec_o, worst, degenerate
 
 
-@pytest.mark.parametrize("name", ["cfg0", "logit_ragged", "kqr_ragged", "hinge_tiny"])
+@pytest.mark.parametrize("name", ["cfg0", "logit_ragged", "kqr_ragged", "hinge_tiny", "dwd_ragged"])
 def test_fit_path_and_exact_cv_parity(tkm, name):
     if name == "cfg0":
         w = wl.config0()                                       # BASELINE.json configs[0], full size
@@ -149,6 +149,9 @@ def test_fit_path_and_exact_cv_parity(tkm, name):
         w = wl.config2(n=333, p=9, L=7, V=3)
     elif name == "kqr_ragged":
         w = wl.config3(n=261, p=5, L=5, V=4, taus=(0.1, 0.5, 0.9))
+    elif name == "dwd_ragged":                                 # DWD (reading G20) on the config-0 generator
+        import dataclasses
+        w = dataclasses.replace(wl.config0(n=205, p=6, L=6, V=3, seed=17), loss=wl.LOSS_DWD, rounds=1)
     else:
         w = wl.config0(n=37, p=3, L=3, V=2, seed=8)
     # The stop tolerance is an input of both sides (reading G6).  At n = 37, lambda = 1e-4 the oracle's own

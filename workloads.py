@@ -20,6 +20,7 @@ import numpy as np
 LOSS_HINGE = 0      # delta-smoothed hinge SVM
 LOSS_LOGISTIC = 1   # kernel logistic regression
 LOSS_QUANTILE = 2   # kernel quantile regression
+LOSS_DWD = 3        # distance-weighted discrimination
 
 
 @dataclasses.dataclass
