@@ -184,6 +184,20 @@ int tkm_predict(const tkm_path* p, int32_t t, int32_t l,
                 const void* X_train, int64_t ldx, const void* X_new, int64_t n_new, int64_t ldxn,
                 int64_t pdim, double sigma, void* f_out, int8_t* label_out, void* stream);
 
+/* ---- probability calibration on the exact-CV path (G21) ----
+ * tkm_cv_decision_values: f_out [dev] n FP64, f_out[j] = held-out decision value of training row j at
+ * (t, lambda_l), i.e. from the column that held out fold foldid[j] (no refitting).  foldid [host] n.
+ * Synchronises `stream`. */
+int tkm_cv_decision_values(const tkm_path* p, int32_t t, int32_t l, const int32_t* foldid, double* f_out,
+                           void* stream);
+/* tkm_platt_fit: Platt's sigmoid P(y = +1 | f) = 1 / (1 + exp(A f + B)) fitted to scores f [dev] n and labels
+ * y [dev] n (+-1) with the targets and the Newton iteration of Lin, Lin & Weng (2007); A, B [host], iters
+ * [host] or NULL.  TKM_ENOTCONV if the line search fails (A, B still written).  Synchronises `stream`. */
+int tkm_platt_fit(const double* f, const double* y, int64_t n, double* A, double* B, int32_t* iters,
+                  void* stream);
+/* p_out[i] = 1 / (1 + exp(A f[i] + B)); f, p_out [dev] n.  Asynchronous. */
+int tkm_platt_proba(const double* f, int64_t n, double A, double B, double* p_out, void* stream);
+
 /* ---- whole pipeline from HOST buffers (the end-to-end call timed as `e2e` by bench.py) ---------
  * X [host] n x p FP64, y [host] n FP64, sigmas [host] G <= 8 bandwidths; copies X, y to the device,
  * runs S1 and S2 per bandwidth, S3-S8 for all bandwidths together (tkm_fit_path_multi), S9 per

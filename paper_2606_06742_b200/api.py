@@ -14,7 +14,7 @@ TKM_OK, TKM_ENOTCONV = 0, 5
 EXPORTED_SYMBOLS = [
     "tkm_gram", "tkm_gram_multi", "tkm_spectral_setup", "tkm_spectral_setup_multi", "tkm_spectral_free", "tkm_spectral_info", "tkm_spectral_get_u",
     "tkm_fit_path", "tkm_fit_path_multi", "tkm_path_free", "tkm_path_info", "tkm_path_profile", "tkm_path_get_a", "tkm_exact_cv", "tkm_path_coef",
-    "tkm_predict", "tkm_train_tune_host", "tkm_make_folds", "tkm_launch_count", "tkm_launch_count_reset",
+    "tkm_predict", "tkm_cv_decision_values", "tkm_platt_fit", "tkm_platt_proba", "tkm_train_tune_host", "tkm_make_folds", "tkm_launch_count", "tkm_launch_count_reset",
     "tkm_dgemm_nt", "tkm_gemm_probe", "tkm_tf32x3_gemm_nt", "tkm_version", "tkm_last_error",
 ]
 
@@ -74,6 +74,9 @@ def lib():
     L.tkm_exact_cv.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
     L.tkm_path_coef.argtypes = [vp, i32, i32, i32, vp, C.POINTER(dbl), vp]
     L.tkm_predict.argtypes = [vp, i32, i32, vp, i64, vp, i64, i64, i64, dbl, vp, vp, vp]
+    L.tkm_cv_decision_values.argtypes = [vp, i32, i32, vp, vp, vp]
+    L.tkm_platt_fit.argtypes = [vp, vp, i64, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(i32), vp]
+    L.tkm_platt_proba.argtypes = [vp, i64, dbl, dbl, vp, vp]
     L.tkm_train_tune_host.argtypes = [vp, i64, i64, vp, vp, i32, C.c_int, C.POINTER(_LossOpts), vp, i32, vp, i32,
                                       dbl, i32, C.c_int, vp, vp, vp, vp, vp, vp, vp, vp]
     L.tkm_make_folds.argtypes = [i64, i32, C.c_uint64, vp]
@@ -416,3 +419,29 @@ def tkm_tf32x3_gemm_nt(P, Q, cfg=-1, iters=0, stream=None):
     _check(lib().tkm_tf32x3_gemm_nt(P.data_ptr(), P.stride(0), Q.data_ptr(), Q.stride(0), D.data_ptr(), M, N, M, K,
                                     cfg, iters, C.byref(ms) if iters > 0 else None, _stream(stream)))
     return (D, float(ms.value)) if iters > 0 else D
+
+
+def tkm_cv_decision_values(path: Path, t: int, l: int, foldid, stream=None):
+    """Held-out decision value of every training row at (t, lambda_l) from the exact-CV columns."""
+    import torch
+    fid = _host(foldid, np.int32)
+    f = torch.empty(path.spec.n, device="cuda", dtype=torch.float64)
+    _check(lib().tkm_cv_decision_values(path._h, t, l, _ptr(fid), f.data_ptr(), _stream(stream)))
+    return f
+
+
+def tkm_platt_fit(f, y, stream=None):
+    """(A, B, iterations) of Platt's sigmoid 1 / (1 + exp(A f + B))."""
+    f, y = _dev_f64(f, "f"), _dev_f64(y, "y")
+    A, B, it = C.c_double(), C.c_double(), C.c_int32()
+    _check(lib().tkm_platt_fit(f.data_ptr(), y.data_ptr(), f.numel(), C.byref(A), C.byref(B), C.byref(it),
+                               _stream(stream)))
+    return A.value, B.value, it.value
+
+
+def tkm_platt_proba(f, A: float, B: float, stream=None):
+    import torch
+    f = _dev_f64(f, "f")
+    p = torch.empty_like(f)
+    _check(lib().tkm_platt_proba(f.data_ptr(), f.numel(), float(A), float(B), p.data_ptr(), _stream(stream)))
+    return p

@@ -401,3 +401,28 @@ def test_leave_one_out_form(tkm):
     assert np.array_equal(cv[1][keep], cv_o[1][keep])
     if not degenerate:
         assert np.array_equal(cv[3], cv_o[3])
+
+
+# ------------------------------------------------------------------------------- Platt scaling (reading G21)
+def test_platt_on_held_out_decision_values(tkm):
+    w = wl.config0(n=260, p=6, L=5, V=4, seed=23)
+    sigma = float(w.sigmas[0])
+    foldid = tkm.tkm_make_folds(w.n, w.V, w.fold_seed)
+    X, y, spec, path, cv = _run_gpu(tkm, w, sigma, foldid, STOP_TOL, 400000)
+    res, spec_o, worst, degenerate = _compare_path(tkm, w, sigma, foldid, spec, path, cv)
+    l = int(cv[3][0])
+    f_g = tkm.tkm_cv_decision_values(path, 0, l, foldid)
+    f_o = o.cv_decision_values(spec_o, res, foldid, 0, l, w.L, w.V)
+    assert np.max(np.abs(f_g.cpu().numpy() - f_o)) <= 1e-8 * max(1.0, np.abs(f_o).max())
+    A, B, it = tkm.tkm_platt_fit(f_g, y)
+    Ao, Bo = o.platt_fit(f_o, w.y)
+    p_g = tkm.tkm_platt_proba(f_g, A, B).cpu().numpy()
+    assert np.max(np.abs(p_g - o.platt_proba(f_o, Ao, Bo))) <= 1e-6      # same stopping rule on both sides
+    assert abs(A - Ao) <= 1e-5 * max(1.0, abs(Ao)) and abs(B - Bo) <= 1e-5 * max(1.0, abs(Bo)) and it >= 1
+    # a second, larger and unbalanced score set straight into the fit kernel
+    rng = np.random.default_rng(6)
+    yy = np.where(rng.random(5003) < 0.3, 1.0, -1.0)
+    ff = 0.8 * yy + rng.standard_normal(5003) - 0.4
+    A2, B2, _ = tkm.tkm_platt_fit(dev(ff), dev(yy))
+    A2o, B2o = o.platt_fit(ff, yy)
+    assert np.max(np.abs(o.platt_proba(ff, A2, B2) - o.platt_proba(ff, A2o, B2o))) <= 1e-6
