@@ -199,6 +199,7 @@ def run_ours(args, w, rank, world):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     prof = dict(ms=np.zeros(2), flops=0.0, samples=0, col_iters=0)
     stage = np.zeros(4)
+    e2e_stage = np.zeros(5)     # last e2e step: copy-in, gram, eig, sweep, cv + coefficients + copy-out (ms)
 
     def ev():
         e = torch.cuda.Event(enable_timing=True)
@@ -246,6 +247,7 @@ def run_ours(args, w, rank, world):
                                     warm_tol=WARM_TOL, sweep_dtype=sweep_dt)
         if r["status"] != 0:
             raise RuntimeError("columns hit maxit in the e2e leg")
+        e2e_stage[:] = r["stage_ms"]
         nb_in = Xh.numel() * 8 + yh.numel() * 8
         nb_out = r["cv_loss"].nbytes + r["cv_err"].nbytes + r["cv_mean"].nbytes + r["best_l"].nbytes + \
             r["alpha"].nbytes + r["beta0"].nbytes
@@ -319,7 +321,9 @@ def run_ours(args, w, rank, world):
             "sweep_iters_sampled": int(prof["samples"]), "roofline": roofline, "clocks": clocks, "gpu_launches": int(launches),
             "e2e": {"value": world * fits_per_step / (ms_e2e / args.steps / 1e3), "unit": UNIT,
                     "h2d_bytes_per_step": int(nb_in), "d2h_bytes_per_step": int(nb_out),
-                    "ms_per_step": ms_e2e / args.steps}}
+                    "ms_per_step": ms_e2e / args.steps,
+                    "last_step_stages_ms": {k: float(v) for k, v in zip(("h2d", "gram", "eig_setup", "sweep",
+                                                                          "cv_coef_d2h"), e2e_stage)}}}
     if world == 1:
         ncol, secs, its = oracle_sample_step(w)
         line["cpu_baseline"] = {"value": ncol / secs, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
