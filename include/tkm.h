@@ -69,6 +69,12 @@ typedef struct {
   double warm_tol;    /* tolerance of rounds 0..R-2 (warm starts only); <= 0 => same as tol   */
   int32_t profile;    /* 1: time the two contractions of the first iteration after every poll */
                       /* with CUDA events (read with tkm_path_profile); 0: no events          */
+  int32_t tf32_delta; /* 1: delta-form GEMM-B.  zeta = U^T z is kept in FP64 and advanced by        */
+                      /* zeta += U^T (z - z_old) with the increment contracted in 3xTF32 on the     */
+                      /* tcgen05 tensor cores (its error is relative to the increment, which        */
+                      /* vanishes at convergence); zeta is recomputed in FP64 after every           */
+                      /* compaction (every check_every iterations).  Same fixed point and           */
+                      /* tolerances as 0 (all FP64 DMMA); DESIGN.md section 12.                     */
 } tkm_loss_opts;
 
 /* Nystrom inputs for tkm_spectral_setup (reading G11). */

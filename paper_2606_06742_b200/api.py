@@ -28,7 +28,7 @@ class TkmError(RuntimeError):
 class _LossOpts(C.Structure):
     _fields_ = [("smooth0", C.c_double), ("eta", C.c_double), ("rounds", C.c_int32), ("T", C.c_int32),
                 ("taus", C.POINTER(C.c_double)), ("restart", C.c_int32), ("check_every", C.c_int32),
-                ("warm_tol", C.c_double), ("profile", C.c_int32)]
+                ("warm_tol", C.c_double), ("profile", C.c_int32), ("tf32_delta", C.c_int32)]
 
 
 class _Nystrom(C.Structure):
@@ -284,21 +284,21 @@ class Path:
             pass
 
 
-def _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, profile=False):
+def _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, profile=False, tf32_delta=False):
     taus_arr = _host(taus if taus is not None else [], np.float64)
     o = _LossOpts(float(smooth0), float(eta), int(rounds), int(len(taus_arr)),
                   taus_arr.ctypes.data_as(C.POINTER(C.c_double)) if len(taus_arr) else None,
-                  int(bool(restart)), int(check_every), float(warm_tol), int(bool(profile)))
+                  int(bool(restart)), int(check_every), float(warm_tol), int(bool(profile)), int(bool(tf32_delta)))
     return o, taus_arr
 
 
 def tkm_fit_path(spec: Spectral, y, loss: int, lambdas, foldid, V: int, tol: float, maxit: int,
                  smooth0=1.0, eta=0.125, rounds=4, taus=None, restart=True, check_every=0, warm_tol=0.0,
-                 warm: Path | None = None, profile=False, stream=None) -> Path:
+                 warm: Path | None = None, profile=False, tf32_delta=False, stream=None) -> Path:
     y = _dev_f64(y, "y")
     lam = _host(lambdas, np.float64)
     fid = _host(foldid, np.int32)
-    o, keep = _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, profile)
+    o, keep = _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, profile, tf32_delta)
     h = C.c_void_p()
     rc = lib().tkm_fit_path(spec._h, y.data_ptr(), loss, C.byref(o), _ptr(lam), len(lam), _ptr(fid), V,
                             float(tol), int(maxit), warm._h if warm is not None else None, C.byref(h),
@@ -309,12 +309,12 @@ def tkm_fit_path(spec: Spectral, y, loss: int, lambdas, foldid, V: int, tol: flo
 
 def tkm_fit_path_multi(specs, y, loss: int, lambdas, foldid, V: int, tol: float, maxit: int,
                        smooth0=1.0, eta=0.125, rounds=4, taus=None, restart=True, check_every=0, warm_tol=0.0,
-                       warm=None, profile=False, stream=None):
+                       warm=None, profile=False, tf32_delta=False, stream=None):
     """One sweep over G spectral handles that share y, folds and the lambda grid -> list of G Paths."""
     y = _dev_f64(y, "y")
     lam = _host(lambdas, np.float64)
     fid = _host(foldid, np.int32)
-    o, keep = _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, profile)
+    o, keep = _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, profile, tf32_delta)
     G = len(specs)
     hs = (C.c_void_p * G)(*[s._h for s in specs])
     hw = (C.c_void_p * G)(*[w._h for w in warm]) if warm is not None else None
@@ -360,7 +360,7 @@ def tkm_predict(path: Path, t: int, l: int, X_train, X_new, sigma: float, labels
 
 def tkm_train_tune_host(X, y, sigmas, loss, lambdas, foldid, V, tol, maxit, smooth0=1.0, eta=0.125, rounds=4,
                         taus=None, restart=True, check_every=0, warm_tol=0.0, sweep_dtype=F64,
-                        want_alpha=True, stream=None):
+                        want_alpha=True, tf32_delta=False, stream=None):
     """Whole pipeline from HOST numpy buffers for G bandwidths at once (the `e2e` call of bench.py)."""
     X = _host(X, np.float64)
     y = _host(y, np.float64)
@@ -369,7 +369,7 @@ def tkm_train_tune_host(X, y, sigmas, loss, lambdas, foldid, V, tol, maxit, smoo
     sig = _host(np.atleast_1d(sigmas), np.float64)
     G = len(sig)
     n, p = X.shape
-    o, keep = _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol)
+    o, keep = _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, False, tf32_delta)
     T, L = max(1, len(keep)), len(lam)
     cv_loss = np.empty((G, T, L, V))
     cv_err = np.empty((G, T, L, V), dtype=np.int64)

@@ -6,8 +6,6 @@
 
 namespace tkm {
 
-int make_tmap_f32(CUtensorMap* out, const float* base, int64_t rows, int64_t cols, int64_t ld, int box_rows);
-
 // x -> hi = tf32(x), lo = tf32(x - hi); both stored as FP32 bit patterns with the low 13 mantissa bits zero
 __global__ void split_tf32_kernel(const double* __restrict__ src, int64_t lds, int rows, int cols, float* __restrict__ hi,
                                   float* __restrict__ lo, int64_t ldo) {
@@ -22,41 +20,14 @@ __global__ void split_tf32_kernel(const double* __restrict__ src, int64_t lds, i
   (void)rows;
 }
 
+int tf32_bn_of(int cfg) { return cfg == 0 ? 64 : (cfg == 1 ? 128 : 256); }
+
 int split_tf32(const double* src, int64_t lds, int64_t rows, int64_t cols, float* hi, float* lo, int64_t ldo,
                cudaStream_t st) {
   dim3 grid((unsigned)std::min<int64_t>(ceil_div(cols, 256), 64), (unsigned)rows);
   split_tf32_kernel<<<grid, 256, 0, st>>>(src, lds, (int)rows, (int)cols, hi, lo, ldo);
   TKM_LAUNCH_CHECK();
   return TKM_OK;
-}
-
-template <class Cfg, class Epi>
-int launch_gemm_tf32(const Tf32Args& a, int G, const Epi& epi, cudaStream_t st) {
-  auto kern = gemm_tf32x3_kernel<Cfg, Epi>;
-  static bool configured = false;
-  if (!configured) {
-    TKM_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
-    configured = true;
-  }
-  dim3 grid((unsigned)ceil_div(a.M, TF32_BM), (unsigned)ceil_div(std::max(a.N, 1), Cfg::BN), (unsigned)G);
-  kern<<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(a, epi);
-  TKM_LAUNCH_CHECK();
-  return TKM_OK;
-}
-
-using Tf32N64 = Tf32Cfg<64, 4>;     // 48 KB per stage
-using Tf32N128 = Tf32Cfg<128, 3>;   // 64 KB per stage
-using Tf32N256 = Tf32Cfg<256, 2>;   // 96 KB per stage
-
-int tf32_bn_of(int cfg) { return cfg == 0 ? 64 : (cfg == 1 ? 128 : 256); }
-
-template <class Epi>
-int gemm_tf32_launch(const Tf32Args& a, int cfg, int G, const Epi& epi, cudaStream_t st) {
-  switch (cfg) {
-    case 0: return launch_gemm_tf32<Tf32N64>(a, G, epi, st);
-    case 1: return launch_gemm_tf32<Tf32N128>(a, G, epi, st);
-    default: return launch_gemm_tf32<Tf32N256>(a, G, epi, st);
-  }
 }
 
 }  // namespace tkm

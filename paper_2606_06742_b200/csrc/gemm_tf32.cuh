@@ -12,6 +12,8 @@
 // epilogue (warp w owns TMEM lanes 32 (w % 4) .. +31, i.e. 32 rows of the tile); warp 2 allocates TMEM.
 #pragma once
 
+#include <algorithm>
+
 #include "tcgen05.cuh"
 
 namespace tkm {
@@ -95,7 +97,8 @@ __global__ void __launch_bounds__(Cfg::THREADS, 1) gemm_tf32x3_kernel(const __gr
   } else if (warp == 1) {
     if (lane == 0) {
       // ===== MMA issuer =====
-      constexpr uint32_t idesc = umma_idesc_tf32(TF32_BM, BN);
+      // a ragged last tile multiplies only the live slots (UMMA N is any multiple of 16)
+      const uint32_t idesc = umma_idesc_tf32(TF32_BM, min(BN, ((N - n_blk0 + 15) >> 4) << 4));
       int s = 0;
       uint32_t phase = 0, acc = 0;
       for (int kt = 0; kt < KT; ++kt) {
@@ -153,5 +156,38 @@ struct Tf32StoreEpi {
       if (n0 + i < N) base[(int64_t)(n0 + i) * ldd] = (double)v[i];
   }
 };
+
+// ---- host side (gemm_tf32.cu, gemm_host.cu) -------------------------------------------------------------
+int make_tmap_f32(CUtensorMap* out, const float* base, int64_t rows, int64_t cols, int64_t ld, int box_rows);
+int split_tf32(const double* src, int64_t lds, int64_t rows, int64_t cols, float* hi, float* lo, int64_t ldo,
+               cudaStream_t st);   // x -> (tf32(x), tf32(x - hi))
+int tf32_bn_of(int cfg);           // slots per tile of configuration 0 / 1 / 2 = 64 / 128 / 256
+
+template <class Cfg, class Epi>
+int launch_gemm_tf32(const Tf32Args& a, int G, const Epi& epi, cudaStream_t st) {
+  auto kern = gemm_tf32x3_kernel<Cfg, Epi>;
+  static bool configured = false;
+  if (!configured) {
+    TKM_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
+    configured = true;
+  }
+  dim3 grid((unsigned)ceil_div(a.M, TF32_BM), (unsigned)ceil_div(std::max(a.N, 1), Cfg::BN), (unsigned)G);
+  kern<<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(a, epi);
+  TKM_LAUNCH_CHECK();
+  return TKM_OK;
+}
+
+using Tf32N64 = Tf32Cfg<64, 4>;     // 48 KB per stage
+using Tf32N128 = Tf32Cfg<128, 3>;   // 64 KB per stage
+using Tf32N256 = Tf32Cfg<256, 2>;   // 96 KB per stage
+
+template <class Epi>
+int gemm_tf32_launch(const Tf32Args& a, int cfg, int G, const Epi& epi, cudaStream_t st) {
+  switch (cfg) {
+    case 0: return launch_gemm_tf32<Tf32N64>(a, G, epi, st);
+    case 1: return launch_gemm_tf32<Tf32N128>(a, G, epi, st);
+    default: return launch_gemm_tf32<Tf32N256>(a, G, epi, st);
+  }
+}
 
 }  // namespace tkm

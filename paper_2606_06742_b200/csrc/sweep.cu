@@ -28,6 +28,7 @@
 #include <new>
 
 #include "gemm_f64.cuh"
+#include "gemm_tf32.cuh"
 #include "handles.cuh"
 
 namespace tkm {
@@ -77,6 +78,9 @@ struct LossEpi {
   int64_t ldz;
   double* gpart;             // [m blocks][ldpart] by gs
   int64_t ldpart;
+  float* dz_hi;              // [G*B][lddz] by gs or NULL: TF32 (hi, lo) split of z - z_old, the operand of the
+  float* dz_lo;              //   delta-form GEMM-B (zeta += U^T dz on the tcgen05 tensor cores)
+  int64_t lddz;
   template <class Cfg>
   __device__ __forceinline__ void run(double (&acc)[Cfg::TN][Cfg::TM][2], int n_blk0, int m_blk0, int warp_n,
                                       int warp_m, int lane, int N, int M, int grp, double* scratch) const {
@@ -111,6 +115,14 @@ struct LossEpi {
           z[e] = (m + e < M && fv[j][e] != v) ? psi_dev(loss, yv[j][e], acc[i][j][e] + bb, smooth, tau) * inv_nc : 0.0;
           colsum[i] += z[e];
         }
+        if (dz_hi && m < M) {   // m is even and lddz a multiple of 32: the pair is in bounds (padding is never read)
+          const double2 zo = *reinterpret_cast<const double2*>(zrow + m);
+          const double d0 = z[0] - zo.x, d1 = (m + 1 < M) ? z[1] - zo.y : 0.0;
+          const float h0 = to_tf32((float)d0), h1 = to_tf32((float)d1);
+          const int64_t o = (int64_t)(g0 + slot) * lddz + m;
+          *reinterpret_cast<float2*>(dz_hi + o) = make_float2(h0, h1);
+          *reinterpret_cast<float2*>(dz_lo + o) = make_float2(to_tf32((float)(d0 - (double)h0)), to_tf32((float)(d1 - (double)h1)));
+        }
         if (m + 1 < M) {
           *reinterpret_cast<double2*>(zrow + m) = make_double2(z[0], z[1]);
         } else if (m < M) {
@@ -126,74 +138,66 @@ struct LossEpi {
   }
 };
 
-// ---- GEMM-B epilogue (S6): rho = zeta + 2 lam abar, partial sums for q and ||rho||^2 -------------
+// ---- GEMM-B epilogue (S6): rho = zeta + 2 lam abar (the column sums of rho are taken by update_kernel) ----
 struct SpecEpi {
-  GroupPtrs gp;
   const int32_t* col_of_slot;   // [G*B]
   const double* col_lam;     // [B]
-  const double* col_c;       // [B] c = curv / n_c
   int B;
   const double* Abar;        // [G*B][lda] by gs
   int64_t lda;
   double* Rho;               // [G*B][lda] by gs
-  double* qpart;             // [m blocks][ldpart] by gs
-  double* r2part;
-  int64_t ldpart;
+  double* Zeta;              // [G*B][lda] by gs or NULL: keeps zeta = U^T z for the delta-form iterations
   template <class Cfg>
   __device__ __forceinline__ void run(double (&acc)[Cfg::TN][Cfg::TM][2], int n_blk0, int m_blk0, int warp_n,
-                                      int warp_m, int lane, int N, int M, int grp, double* scratch) const {
+                                      int warp_m, int lane, int N, int M, int grp, double*) const {
     constexpr int TN = Cfg::TN, TM = Cfg::TM;
-    const double* lam = gp.lam[grp];
-    const double* u1 = gp.u1[grp];
-    double lv[TM][2], lu[TM][2];   // Lam_i and Lam_i u1_i
-#pragma unroll
-    for (int j = 0; j < TM; ++j)
-#pragma unroll
-      for (int e = 0; e < 2; ++e) {
-        const int i = m_blk0 + (warp_m * TM + j) * 8 + 2 * (lane & 3) + e;
-        lv[j][e] = (i < M) ? lam[i] : 0.0;
-        lu[j][e] = (i < M) ? lam[i] * u1[i] : 0.0;
-      }
     const int g0 = grp * B;
-    double qs[TN], r2[TN];
 #pragma unroll
     for (int t = 0; t < TN; ++t) {
-      qs[t] = r2[t] = 0.0;
       const int slot = n_blk0 + (warp_n * TN + t) * 8 + (lane >> 2);
       if (slot >= N) continue;
-      const int col = col_of_slot[g0 + slot];
-      const double two_lam = 2.0 * col_lam[col], cc = col_c[col];
-      const double* arow = Abar + (int64_t)(g0 + slot) * lda;
-      double* rrow = Rho + (int64_t)(g0 + slot) * lda;
+      const double two_lam = 2.0 * col_lam[col_of_slot[g0 + slot]];
+      const int64_t row = (int64_t)(g0 + slot) * lda;
 #pragma unroll
       for (int j = 0; j < TM; ++j) {
         const int i = m_blk0 + (warp_m * TM + j) * 8 + 2 * (lane & 3);
-        double rho[2] = {0.0, 0.0};
         if (i + 1 < M) {
-          const double2 ab = *reinterpret_cast<const double2*>(arow + i);
-          rho[0] = acc[t][j][0] + two_lam * ab.x;
-          rho[1] = acc[t][j][1] + two_lam * ab.y;
-          *reinterpret_cast<double2*>(rrow + i) = make_double2(rho[0], rho[1]);
+          const double2 ab = *reinterpret_cast<const double2*>(Abar + row + i);
+          *reinterpret_cast<double2*>(Rho + row + i) =
+              make_double2(acc[t][j][0] + two_lam * ab.x, acc[t][j][1] + two_lam * ab.y);
+          if (Zeta) *reinterpret_cast<double2*>(Zeta + row + i) = make_double2(acc[t][j][0], acc[t][j][1]);
         } else if (i < M) {
-          rho[0] = acc[t][j][0] + two_lam * arow[i];
-          rrow[i] = rho[0];
-        }
-#pragma unroll
-        for (int e = 0; e < 2; ++e) {
-          // S_i Lam_i u1_i rho_i with S_i = 1/(2 lam + c Lam_i)  (G1)
-          qs[t] += lu[j][e] * rho[e] / (two_lam + cc * lv[j][e]);
-          r2[t] += rho[e] * rho[e];
+          Rho[row + i] = acc[t][j][0] + two_lam * Abar[row + i];
+          if (Zeta) Zeta[row + i] = acc[t][j][0];
         }
       }
     }
-    double tot;
-    if (cta_row_reduce<Cfg>(qs, warp_n, warp_m, lane, scratch, tot)) {
-      const int slot = n_blk0 + (int)threadIdx.x;
-      if (slot < N) qpart[(int64_t)blockIdx.x * ldpart + g0 + slot] = tot;
-    }
-    if (cta_row_reduce<Cfg>(r2, warp_n, warp_m, lane, scratch, tot)) {
-      const int slot = n_blk0 + (int)threadIdx.x;
-      if (slot < N) r2part[(int64_t)blockIdx.x * ldpart + g0 + slot] = tot;
+  }
+};
+
+// ---- delta-form GEMM-B epilogue (tcgen05 kernel): zeta += U^T dz, rho = zeta + 2 lam abar --------------------
+// Thread = one spectral index i (a TMEM lane), 16 consecutive slots per call; for a fixed slot the 32 lanes
+// of a warp touch 32 consecutive doubles.
+struct ZetaEpi {
+  const int32_t* col_of_slot;   // [G*B]
+  const double* col_lam;        // [B]
+  int B;
+  const double* Abar;           // [G*B][lda]
+  int64_t lda;
+  double* Zeta;                 // [G*B][lda]
+  double* Rho;                  // [G*B][lda]
+  __device__ __forceinline__ void chunk(const float (&v)[16], int i, int n0, int N, int M, int grp) const {
+    if (i >= M) return;
+    const int g0 = grp * B;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+      const int slot = n0 + k;
+      if (slot >= N) break;
+      const double two_lam = 2.0 * col_lam[col_of_slot[g0 + slot]];
+      const int64_t o = (int64_t)(g0 + slot) * lda + i;
+      const double z = Zeta[o] + (double)v[k];
+      Zeta[o] = z;
+      Rho[o] = z + two_lam * Abar[o];
     }
   }
 };
@@ -248,7 +252,8 @@ __global__ void __launch_bounds__(256) init_round_kernel(RoundArgs p) {
 
 // ---- S7: per-column update, stop test, restart, next extrapolation --------------------------------
 struct UpdateArgs {
-  int r, n, B, nblkA, nblkB, restart, maxit;
+  int r, n, B, nblkA, restart, maxit;
+  int exact;   // 0: rho came from the delta-form recurrence -- a column may not be declared converged on it
   int64_t lda, ldpart;
   double tol;
   GroupPtrs gp;
@@ -256,7 +261,7 @@ struct UpdateArgs {
   const int32_t* col_of_slot;  // [G*B]
   const double *col_lam, *col_c, *col_nc;   // [B]
   const double* col_s;         // [G*B]
-  const double *gpart, *qpart, *r2part;
+  const double* gpart;
   const double* Rho;
   double *A, *Aprev, *Abar;
   double *beta, *beta_prev, *bbar, *rk, *kkt;   // [G*B]
@@ -279,12 +284,43 @@ __global__ void __launch_bounds__(256, 2) update_kernel(UpdateArgs p) {
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
   const double2* __restrict__ lam2 = reinterpret_cast<const double2*>(p.gp.lam[grp]);
   const double2* __restrict__ u12 = reinterpret_cast<const double2*>(p.gp.u1[grp]);
-  // per-column sums from the per-tile partials of the two epilogues (fixed order => deterministic)
+  const double lamc = p.col_lam[col], c = p.col_c[col], s = p.col_s[gc], nc = p.col_nc[col];
+  const double two_lam = 2.0 * lamc;
+  const int64_t off2 = ((int64_t)gs * p.lda) >> 1;   // lda is a multiple of 16
+  const double2* __restrict__ Rho2 = reinterpret_cast<const double2*>(p.Rho) + off2;
+  double2* __restrict__ A2 = reinterpret_cast<double2*>(p.A) + off2;
+  double2* __restrict__ Ap2 = reinterpret_cast<double2*>(p.Aprev) + off2;
+  double2* __restrict__ Ab2 = reinterpret_cast<double2*>(p.Abar) + off2;
+  const int npair = (int)(p.lda >> 1);
+  const bool single = npair <= 256 * UPD_EPT;
+  // Column sums (fixed order => deterministic): gamma0 = 1^T z from the per-tile partials of GEMM-A's epilogue;
+  // sum_i S_i Lam_i u1_i rho_i (G1) and ||rho||^2 from rho itself.  When the whole vector fits
+  // one chunk the operands loaded here stay in registers for the update below.
+  double2 rho[UPD_EPT], ab[UPD_EPT], lm[UPD_EPT], uu[UPD_EPT], a_old[UPD_EPT], a_new[UPD_EPT];
   double g0 = 0.0, qd = 0.0, r2 = 0.0;
   for (int b = tid; b < p.nblkA; b += 256) g0 += p.gpart[(int64_t)b * p.ldpart + gs];
-  for (int b = tid; b < p.nblkB; b += 256) {
-    qd += p.qpart[(int64_t)b * p.ldpart + gs];
-    r2 += p.r2part[(int64_t)b * p.ldpart + gs];
+  for (int base = 0; base < npair; base += 256 * UPD_EPT) {
+#pragma unroll
+    for (int e = 0; e < UPD_EPT; ++e) {
+      const int i = base + e * 256 + tid;
+      if (i < npair) {
+        rho[e] = Rho2[i];
+        lm[e] = lam2[i];
+        uu[e] = u12[i];
+        if (single) {
+          ab[e] = Ab2[i];
+          a_old[e] = A2[i];
+        }
+      }
+    }
+#pragma unroll
+    for (int e = 0; e < UPD_EPT; ++e) {
+      const int i = base + e * 256 + tid;
+      if (i < npair) {
+        qd += lm[e].x * uu[e].x * rho[e].x / (two_lam + c * lm[e].x) + lm[e].y * uu[e].y * rho[e].y / (two_lam + c * lm[e].y);
+        r2 += rho[e].x * rho[e].x + rho[e].y * rho[e].y;
+      }
+    }
   }
   g0 = warp_sum(g0);
   qd = warp_sum(qd);
@@ -302,32 +338,24 @@ __global__ void __launch_bounds__(256, 2) update_kernel(UpdateArgs p) {
     qd += red[1][k];
     r2 += red[2][k];
   }
-  const double lamc = p.col_lam[col], c = p.col_c[col], s = p.col_s[gc], nc = p.col_nc[col];
   const double dbeta = (g0 - c * qd) / s;                            // PAPER.md:208 (Alg.1 l.17)
   const double kkt = fmax(fabs(g0), nc * sqrt(r2) / sqrt((double)p.n));   // reading G6
   const double beta = p.beta[gc], bbar = p.bbar[gc];
   const double beta_new = bbar - dbeta;
-  const int64_t off2 = ((int64_t)gs * p.lda) >> 1;   // lda is a multiple of 16
-  const double2* __restrict__ Rho2 = reinterpret_cast<const double2*>(p.Rho) + off2;
-  double2* __restrict__ A2 = reinterpret_cast<double2*>(p.A) + off2;
-  double2* __restrict__ Ap2 = reinterpret_cast<double2*>(p.Aprev) + off2;
-  double2* __restrict__ Ab2 = reinterpret_cast<double2*>(p.Abar) + off2;
-  const int npair = (int)(p.lda >> 1);
-  const bool single = npair <= 256 * UPD_EPT;
-  const double two_lam = 2.0 * lamc, dbc = dbeta * c;
-  double2 a_old[UPD_EPT], a_new[UPD_EPT];
+  const double dbc = dbeta * c;
   double g = 0.0;
   for (int base = 0; base < npair; base += 256 * UPD_EPT) {
-    double2 rho[UPD_EPT], ab[UPD_EPT], lm[UPD_EPT], uu[UPD_EPT];
+    if (!single) {
 #pragma unroll
-    for (int e = 0; e < UPD_EPT; ++e) {
-      const int i = base + e * 256 + tid;
-      if (i < npair) {
-        rho[e] = Rho2[i];
-        ab[e] = Ab2[i];
-        a_old[e] = A2[i];
-        lm[e] = lam2[i];
-        uu[e] = u12[i];
+      for (int e = 0; e < UPD_EPT; ++e) {
+        const int i = base + e * 256 + tid;
+        if (i < npair) {
+          rho[e] = Rho2[i];
+          ab[e] = Ab2[i];
+          a_old[e] = A2[i];
+          lm[e] = lam2[i];
+          uu[e] = u12[i];
+        }
       }
     }
 #pragma unroll
@@ -397,7 +425,7 @@ __global__ void __launch_bounds__(256, 2) update_kernel(UpdateArgs p) {
     p.iters[gc] += 1;
     const int itr = p.iters_round[gc] + 1;
     p.iters_round[gc] = itr;
-    if (kkt <= p.tol) {
+    if (kkt <= p.tol && p.exact) {
       p.done[gc] = 1;
     } else if (itr >= p.maxit) {
       p.done[gc] = 1;
@@ -421,6 +449,10 @@ struct CompactArgs {
   int32_t* tail_list;       // [G*B]
   int32_t* counts;          // [G][4]: nfin, nholes, nact, previous nslots
   double *A, *Aprev, *Abar;
+  double* Zeta;             // [G*B][lda] or NULL (delta form): moves with its slot
+  double* Zt;               // [G*B][ldz] or NULL (delta form)
+  int64_t ldz;
+  int n;
 };
 
 __global__ void __launch_bounds__(1024) compact_plan_kernel(CompactArgs p) {
@@ -509,6 +541,11 @@ __global__ void __launch_bounds__(256) compact_apply_kernel(CompactArgs p) {
     p.A[so + i] = p.A[to + i];
     p.Aprev[so + i] = p.Aprev[to + i];
     p.Abar[so + i] = p.Abar[to + i];
+    if (p.Zeta) p.Zeta[so + i] = p.Zeta[to + i];
+  }
+  if (p.Zt) {
+    const int64_t zs = (int64_t)(g0 + sl) * p.ldz, zt = (int64_t)(g0 + src) * p.ldz;
+    for (int i = threadIdx.x; i < p.n; i += blockDim.x) p.Zt[zs + i] = p.Zt[zt + i];
   }
   if (threadIdx.x == 0) p.col_of_slot[g0 + sl] = p.col_of_slot[g0 + src];
 }
@@ -650,7 +687,7 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
   const tkm_path* p0 = out[0];   // the column tables are identical in every group: use group 0's
 
   // working set (all groups stacked: row / entry g*B + slot or g*B + column)
-  DevBuf A, Aprev, Abar, Rho, Zt, gpart, qpart, r2part, d_fold;
+  DevBuf A, Aprev, Abar, Rho, Zt, gpart, d_fold;
   DevBuf col_c, col_s, beta, beta_prev, bbar, rk, kkt, done, iters, iters_round, flags, col_of_slot;
   DevBuf nslots, fin_list, tail_list, counts;
   TKM_TRY(A.alloc((size_t)GB * ldr * sizeof(double), true, st));
@@ -661,8 +698,6 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
   const int64_t nblk_max = ceil_div(std::max(n, r), 64);   // smallest BM of any tile configuration
   const int64_t ldpart = round_up(GB, 16);
   TKM_TRY(gpart.alloc((size_t)nblk_max * ldpart * sizeof(double), true, st));
-  TKM_TRY(qpart.alloc((size_t)nblk_max * ldpart * sizeof(double), true, st));
-  TKM_TRY(r2part.alloc((size_t)nblk_max * ldpart * sizeof(double), true, st));
   TKM_TRY(d_fold.alloc((size_t)n * sizeof(int32_t), false, st));
   TKM_CUDA(cudaMemcpyAsync(d_fold.p, foldid, n * sizeof(int32_t), cudaMemcpyHostToDevice, st));
   TKM_TRY(col_c.alloc((size_t)B * sizeof(double), true, st));
@@ -677,6 +712,23 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
       TKM_CUDA(cudaMemcpyAsync(beta.as<double>() + (size_t)g * B, warm[g]->beta0.p, (size_t)B * sizeof(double),
                                cudaMemcpyDeviceToDevice, st));
     }
+  // delta-form GEMM-B (tkm_loss_opts.tf32_delta): zeta state, the (hi, lo) increment operand, U^T as (hi, lo)
+  const bool delta = opts->tf32_delta != 0;
+  const int64_t ldn32 = round_up(n, 32);
+  DevBuf Zeta, dz_hi, dz_lo, ut_hi[GEMM_MAX_GROUPS], ut_lo[GEMM_MAX_GROUPS];
+  if (delta) {
+    TKM_TRY(Zeta.alloc((size_t)GB * ldr * sizeof(double), true, st));
+    TKM_TRY(dz_hi.alloc((size_t)GB * ldn32 * sizeof(float), true, st));
+    TKM_TRY(dz_lo.alloc((size_t)GB * ldn32 * sizeof(float), true, st));
+    for (int g = 0; g < G; ++g) {
+      TKM_TRY(ut_hi[g].alloc((size_t)r * ldn32 * sizeof(float), true, st));
+      TKM_TRY(ut_lo[g].alloc((size_t)r * ldn32 * sizeof(float), true, st));
+      TKM_TRY(split_tf32(specs[g]->Ut.as<double>(), ldn, r, n, ut_hi[g].as<float>(), ut_lo[g].as<float>(), ldn32, st));
+    }
+  }
+  Tf32Args targs;
+  memset(&targs, 0, sizeof(targs));
+  int tcfg = -1;
   PinBuf h_ns;   // [POLL_RING][GEMM_MAX_GROUPS] live-slot counts read back after every compaction
   TKM_TRY(h_ns.alloc((size_t)POLL_RING * GEMM_MAX_GROUPS * sizeof(int32_t)));
 
@@ -773,22 +825,51 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
         tileB = tB;
       }
       argsA.N = argsB.N = std::max(nmax, 1);
+      if (delta) {
+        const int want = nmax <= 64 ? 0 : (nmax <= 128 ? 1 : 2);
+        if (want != tcfg) {
+          const int bn = tf32_bn_of(want);
+          TKM_TRY(make_tmap_f32(&targs.p_hi, dz_hi.as<float>(), GB, n, ldn32, bn));
+          TKM_TRY(make_tmap_f32(&targs.p_lo, dz_lo.as<float>(), GB, n, ldn32, bn));
+          for (int g = 0; g < G; ++g) {
+            TKM_TRY(make_tmap_f32(&targs.q_hi[g], ut_hi[g].as<float>(), r, n, ldn32, TF32_BM));
+            TKM_TRY(make_tmap_f32(&targs.q_lo[g], ut_lo[g].as<float>(), r, n, ldn32, TF32_BM));
+          }
+          targs.nslots = nslots.as<int32_t>();
+          targs.p_group_rows = B;
+          targs.M = (int)r;
+          targs.K = (int)n;
+          tcfg = want;
+        }
+        targs.N = std::max(nmax, 1);
+      }
       for (int k = 0; k < check_every; ++k) {
-        const bool sample = opts->profile && k == 0;
+        // FP64 GEMM-B: always without the delta form; with it, on the first iteration of a round (no zeta yet)
+        // and on the last iteration of every batch, whose exact rho carries the stop test before the compaction
+        const bool exact_it = !delta || (batch == 0 && k == 0) || k == check_every - 1;
+        const bool sample = opts->profile && k == check_every - 1;
         if (sample) TKM_CUDA(cudaEventRecord(ev.pev[ring][0], st));
         LossEpi le{(const double*)y, d_fold.as<int32_t>(), col_of_slot.as<int32_t>(), bbar.as<double>(),
                    p0->col_nc.as<double>(), p0->col_tau.as<double>(), p0->col_v.as<int32_t>(), B, (int)loss, smooth,
-                   Zt.as<double>(), ldn, gpart.as<double>(), ldpart};
+                   Zt.as<double>(), ldn, gpart.as<double>(), ldpart, delta ? dz_hi.as<float>() : nullptr,
+                   delta ? dz_lo.as<float>() : nullptr, ldn32};
         TKM_TRY(gemm_f64_launch(argsA, tileA, G, le, st));
         if (sample) TKM_CUDA(cudaEventRecord(ev.pev[ring][1], st));
-        SpecEpi se{gp, col_of_slot.as<int32_t>(), p0->col_lam.as<double>(), col_c.as<double>(), B, Abar.as<double>(),
-                   ldr, Rho.as<double>(), qpart.as<double>(), r2part.as<double>(), ldpart};
-        TKM_TRY(gemm_f64_launch(argsB, tileB, G, se, st));
+        if (exact_it) {
+          // FP64 contraction; in delta form it also re-establishes zeta = U^T z exactly
+          SpecEpi se{col_of_slot.as<int32_t>(), p0->col_lam.as<double>(), B, Abar.as<double>(), ldr, Rho.as<double>(),
+                     delta ? Zeta.as<double>() : nullptr};
+          TKM_TRY(gemm_f64_launch(argsB, tileB, G, se, st));
+        } else {
+          ZetaEpi ze{col_of_slot.as<int32_t>(), p0->col_lam.as<double>(), B, Abar.as<double>(), ldr, Zeta.as<double>(),
+                     Rho.as<double>()};
+          TKM_TRY(gemm_tf32_launch(targs, tcfg, G, ze, st));
+        }
         if (sample) TKM_CUDA(cudaEventRecord(ev.pev[ring][2], st));
-        UpdateArgs ua{(int)r, (int)n, B, (int)ceil_div(n, tileA.BM), (int)ceil_div(r, tileB.BM), restart, maxit, ldr,
+        UpdateArgs ua{(int)r, (int)n, B, (int)ceil_div(n, tileA.BM), restart, maxit, exact_it ? 1 : 0, ldr,
                       ldpart, rtol, gp, nslots.as<int32_t>(), col_of_slot.as<int32_t>(), p0->col_lam.as<double>(),
                       col_c.as<double>(), p0->col_nc.as<double>(), col_s.as<double>(), gpart.as<double>(),
-                      qpart.as<double>(), r2part.as<double>(), Rho.as<double>(), A.as<double>(), Aprev.as<double>(),
+                      Rho.as<double>(), A.as<double>(), Aprev.as<double>(),
                       Abar.as<double>(), beta.as<double>(), beta_prev.as<double>(), bbar.as<double>(), rk.as<double>(),
                       kkt.as<double>(), done.as<int32_t>(), iters.as<int32_t>(), iters_round.as<int32_t>(),
                       flags.as<int32_t>()};
@@ -798,7 +879,8 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
       // compaction on the device; the new counts travel back asynchronously
       CompactArgs ca{B, (int)r, ldr, gp, nslots.as<int32_t>(), col_of_slot.as<int32_t>(), done.as<int32_t>(),
                      fin_list.as<int32_t>(), tail_list.as<int32_t>(), counts.as<int32_t>(), A.as<double>(),
-                     Aprev.as<double>(), Abar.as<double>()};
+                     Aprev.as<double>(), Abar.as<double>(), delta ? Zeta.as<double>() : nullptr,
+                     delta ? Zt.as<double>() : nullptr, ldn, (int)n};
       compact_plan_kernel<<<G, 1024, 0, st>>>(ca);
       TKM_LAUNCH_CHECK();
       compact_apply_kernel<<<dim3(std::max(nmax, 1), G), 256, 0, st>>>(ca);
