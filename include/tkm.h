@@ -108,8 +108,10 @@ int tkm_gram_multi(const void* X, int64_t n, int64_t p, int64_t ldx,
 /* ---- S2  one-time spectral setup (Alg.1 l.3, 226; readings G11, G16, G19) --------
  * Full kernel (ny == NULL): K [dev] n x n FP64 symmetric (not modified); decomposes in FP64 with
  * cuSOLVER syevd, clamps Lam >= 0, forms u1 = U^T 1, and keeps U Lam (n x r) and U^T (r x n) in
- * `sweep_dt` precision for the two contractions of the sweep (TKM_F32: split into TF32 hi + lo
- * parts for the 3xTF32 tensor-core path; TKM_F64: FP64 DMMA path).  r = n.
+ * FP64 for the two contractions of the sweep (FP64 DMMA path).  sweep_dt must be TKM_F64: an all-FP32 /
+ * 3xTF32 sweep cannot meet the stop test on ill-conditioned columns and returns TKM_ENOTIMPL (DESIGN.md
+ * section 12); the 3xTF32 tensor-core path exists as the delta form selected by tkm_loss_opts.tf32_delta.
+ * r = n.
  * Nystrom (ny != NULL): K is ignored (may be NULL); thin U (n x r, r <= m) from K_nm, K_mm.
  * The handle is shared by every lambda, fold and quantile level.  Synchronises `stream`.
  * Errors: TKM_ESOLVER if cuSOLVER reports info != 0; TKM_ENOMEM. */

@@ -18,8 +18,6 @@ struct tkm_spectral {
   tkm::DevBuf u1;    // [ldr]    FP64   U^T 1            (padding 0)
   double thin = 0.0; // n - ||u1||^2 for a thin U, exactly 0 for the full kernel (reading G1)
   std::vector<double> h_lam, h_u1;
-  // FP32 sweep (3xTF32): TF32-rounded hi and lo parts of UL and Ut
-  tkm::DevBuf UL_hi, UL_lo, Ut_hi, Ut_lo;
   // Nystrom (reading G11)
   int64_t m = 0;
   int64_t ldm = 0;

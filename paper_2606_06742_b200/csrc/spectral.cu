@@ -276,7 +276,7 @@ extern "C" int tkm_spectral_setup(const void* K, int64_t n, int64_t ldk, const t
   if (!s) return set_error(TKM_ENOMEM, "out of host memory");
   s->sweep_dt = sweep_dt;
   int rc = ny ? setup_nystrom(n, ny, s, st) : setup_full((const double*)K, n, ldk, s, st);
-  if (rc == TKM_OK && sweep_dt == TKM_F32) rc = set_error(TKM_ENOTIMPL, "FP32 (3xTF32) sweep not built yet");
+  if (rc == TKM_OK && sweep_dt == TKM_F32) rc = set_error(TKM_ENOTIMPL, "an all-FP32 (3xTF32) sweep is not provided: use TKM_F64, optionally with tkm_loss_opts.tf32_delta");
   if (rc != TKM_OK) {
     cudaStreamSynchronize(st);
     delete s;
