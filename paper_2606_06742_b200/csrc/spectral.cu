@@ -6,6 +6,7 @@
 // Nystrom products -- is this library's own kernels (the products use the DMMA GEMM of gemm_f64.cuh).
 #include <cusolverDn.h>
 
+#include <algorithm>
 #include <cmath>
 #include <mutex>
 #include <new>
@@ -117,11 +118,20 @@ static int syevd_inplace(double* A, int64_t lda, int64_t n, double* W, cudaStrea
   cusolverStatus_t cs = cusolverDnDsyevd_bufferSize(sv.h, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER,
                                                     (int)n, A, (int)lda, W, &lwork);
   if (cs != CUSOLVER_STATUS_SUCCESS) return set_error(TKM_ESOLVER, "Dsyevd_bufferSize failed (%d)", (int)cs);
-  DevBuf work, info;
-  TKM_TRY(work.alloc((size_t)lwork * sizeof(double), false, st));
-  TKM_TRY(info.alloc(sizeof(int), true, st));
+  // stream-ordered temporaries: cudaFree would synchronise the whole device and stall the other setups of a
+  // tkm_spectral_setup_multi call that run concurrently on their own streams
+  struct AsyncBuf {
+    void* p = nullptr;
+    cudaStream_t st;
+    ~AsyncBuf() {
+      if (p) cudaFreeAsync(p, st);
+    }
+  } work{nullptr, st}, info{nullptr, st};
+  TKM_CUDA(cudaMallocAsync(&work.p, (size_t)std::max(lwork, 1) * sizeof(double), st));
+  TKM_CUDA(cudaMallocAsync(&info.p, sizeof(int), st));
+  TKM_CUDA(cudaMemsetAsync(info.p, 0, sizeof(int), st));
   cs = cusolverDnDsyevd(sv.h, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER, (int)n, A, (int)lda, W,
-                        work.as<double>(), lwork, info.as<int>());
+                        (double*)work.p, lwork, (int*)info.p);
   if (cs != CUSOLVER_STATUS_SUCCESS) return set_error(TKM_ESOLVER, "cusolverDnDsyevd failed (%d)", (int)cs);
   int h_info = 0;
   TKM_CUDA(cudaMemcpyAsync(&h_info, info.p, sizeof(int), cudaMemcpyDeviceToHost, st));
@@ -145,7 +155,7 @@ static int finish_spectral(tkm_spectral* s, cudaStream_t st) {
   TKM_LAUNCH_CHECK();
   row_sum_kernel<<<(unsigned)r, 256, 0, st>>>(s->Ut.as<double>(), s->ldn, (int)n, s->u1.as<double>());
   TKM_LAUNCH_CHECK();
-  TKM_TRY(s->UL.alloc((size_t)n * s->ldr * sizeof(double), true, st));
+  if (!s->UL.p) TKM_TRY(s->UL.alloc((size_t)n * s->ldr * sizeof(double), true, st));
   TKM_TRY(transpose_scale_f64(s->Ut.as<double>(), s->ldn, r, n, s->lam.as<double>(), s->UL.as<double>(), s->ldr, st));
   s->h_lam.resize(r);
   s->h_u1.resize(r);
@@ -163,16 +173,26 @@ static int finish_spectral(tkm_spectral* s, cudaStream_t st) {
   return TKM_OK;
 }
 
-static int setup_full(const double* K, int64_t n, int64_t ldk, tkm_spectral* s, cudaStream_t st) {
+// Allocations of a full-kernel handle, separated from the arithmetic so that tkm_spectral_setup_multi can make
+// them before its worker threads start (cudaMalloc serialises with work of the other streams).
+static int alloc_full(int64_t n, tkm_spectral* s, cudaStream_t st) {
   s->n = s->r = n;
   s->ldn = s->ldr = round_up(n, 16);
   TKM_TRY(s->Ut.alloc((size_t)n * s->ldn * sizeof(double), true, st));
   TKM_TRY(s->lam.alloc((size_t)s->ldr * sizeof(double), true, st));
   TKM_TRY(s->u1.alloc((size_t)s->ldr * sizeof(double), true, st));
+  TKM_TRY(s->UL.alloc((size_t)n * s->ldr * sizeof(double), true, st));
+  return TKM_OK;
+}
+static int compute_full(const double* K, int64_t n, int64_t ldk, tkm_spectral* s, cudaStream_t st) {
   TKM_CUDA(cudaMemcpy2DAsync(s->Ut.p, s->ldn * sizeof(double), K, ldk * sizeof(double), n * sizeof(double), n,
                              cudaMemcpyDeviceToDevice, st));
   TKM_TRY(syevd_inplace(s->Ut.as<double>(), s->ldn, n, s->lam.as<double>(), st));
   return finish_spectral(s, st);
+}
+static int setup_full(const double* K, int64_t n, int64_t ldk, tkm_spectral* s, cudaStream_t st) {
+  TKM_TRY(alloc_full(n, s, st));
+  return compute_full(K, n, ldk, s, st);
 }
 
 constexpr double NYS_RANK_TOL = 1e-12;
@@ -300,10 +320,27 @@ extern "C" int tkm_spectral_setup_multi(const void* const* Ks, int32_t G, int64_
   cudaStream_t st = (cudaStream_t)stream;
   cudaEvent_t ready;
   TKM_CUDA(cudaEventCreateWithFlags(&ready, cudaEventDisableTiming));
-  cudaEventRecord(ready, st);
   std::vector<int> rc(G, TKM_OK);
   std::vector<std::string> msg(G);
   std::vector<int64_t> launches(G, 0);
+  if (n <= 1 || n > (1 << 30) || ldk < n || sweep_dt != TKM_F64) {
+    cudaEventDestroy(ready);
+    return set_error(sweep_dt != TKM_F64 ? TKM_ENOTIMPL : TKM_EINVAL, "tkm_spectral_setup_multi: bad n / ldk / sweep_dt");
+  }
+  for (int g = 0; g < G; ++g) {   // every allocation happens here, before the concurrent part
+    out[g] = new (std::nothrow) tkm_spectral();
+    int a = out[g] && Ks[g] ? alloc_full(n, out[g], st) : set_error(TKM_EINVAL, "tkm_spectral_setup_multi: NULL matrix");
+    if (a != TKM_OK) {
+      for (int h = 0; h <= g; ++h) {
+        delete out[h];
+        out[h] = nullptr;
+      }
+      cudaEventDestroy(ready);
+      return a;
+    }
+    out[g]->sweep_dt = sweep_dt;
+  }
+  cudaEventRecord(ready, st);   // K ready and the zero fills of the new buffers done
   std::vector<std::thread> th;
   for (int g = 0; g < G; ++g)
     th.emplace_back([&, g] {
@@ -314,7 +351,7 @@ extern "C" int tkm_spectral_setup_multi(const void* const* Ks, int32_t G, int64_
         return;
       }
       cudaStreamWaitEvent(s2, ready, 0);
-      rc[g] = tkm_spectral_setup(Ks[g], n, ldk, nullptr, sweep_dt, &out[g], s2);   // synchronises s2
+      rc[g] = compute_full((const double*)Ks[g], n, ldk, out[g], s2);   // synchronises s2
       if (rc[g] != TKM_OK) msg[g] = err_buf();
       launches[g] = launch_counter();
       cudaStreamDestroy(s2);
