@@ -556,7 +556,7 @@ static double curvature_of(tkm_loss loss, double smooth) {
   return 1.0 / (2.0 * smooth);   // 1/kappa, kappa = 2 delta
 }
 
-constexpr int POLL_RING = 3;   // batches whose poll results may be in flight
+constexpr int POLL_RING = 5;   // ring of poll results: up to POLL_RING - 2 batches may be in flight
 
 }  // namespace tkm
 
@@ -802,7 +802,7 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
     // Host view of the live-slot counts: an upper bound that lags the device by at most two batches.
     int bound[GEMM_MAX_GROUPS];
     for (int g = 0; g < G; ++g) bound[g] = B;
-    int64_t batch = 0;
+    int64_t batch = 0, done_polls = 0;
     bool finished = false;
     while (!finished) {
       const int ring = (int)(batch % POLL_RING);
@@ -888,47 +888,46 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
       TKM_CUDA(cudaMemcpyAsync(h_ns.as<int32_t>() + ring * GEMM_MAX_GROUPS, nslots.p, GEMM_MAX_GROUPS * sizeof(int32_t),
                                cudaMemcpyDeviceToHost, st));
       TKM_CUDA(cudaEventRecord(ev.poll[ring], st));
-      // read the poll of the PREVIOUS batch (the GPU keeps working on the one just enqueued)
-      if (batch >= 1) {
-        const int prev = (int)((batch - 1) % POLL_RING);
-        TKM_CUDA(cudaEventSynchronize(ev.poll[prev]));
-        const int32_t* hn = h_ns.as<int32_t>() + prev * GEMM_MAX_GROUPS;
+      // Read back the polls of EARLIER batches while the GPU works on the ones just enqueued.  The host runs
+      // one batch ahead while the live set is wide (fresh counts matter for the tile choice) and up to three
+      // once it is narrow (batches of ~1 ms: slack against a descheduled host thread matters more).
+      const int lag = ntot > 256 ? 1 : POLL_RING - 2;
+      while (!finished && done_polls + lag <= batch) {
+        const int64_t b = done_polls;
+        const int cur = (int)(b % POLL_RING);
+        TKM_CUDA(cudaEventSynchronize(ev.poll[cur]));
+        const int32_t* hn = h_ns.as<int32_t>() + cur * GEMM_MAX_GROUPS;
         int live = 0;
         for (int g = 0; g < G; ++g) {
           bound[g] = hn[g];
           live += hn[g];
         }
-        if (opts->profile) {
-          // the sampled GEMMs of batch-1 have completed (they precede its poll event); the live count in
-          // effect during batch-1 is the poll result of batch-2 (all columns for the first batch)
-          float ma = 0.f, mb = 0.f;
-          TKM_CUDA(cudaEventElapsedTime(&ma, ev.pev[prev][0], ev.pev[prev][1]));
-          TKM_CUDA(cudaEventElapsedTime(&mb, ev.pev[prev][1], ev.pev[prev][2]));
-          int live_then = GB;
-          if (batch >= 2) {
-            const int32_t* h2 = h_ns.as<int32_t>() + (int)((batch - 2) % POLL_RING) * GEMM_MAX_GROUPS;
-            live_then = 0;
-            for (int g = 0; g < G; ++g) live_then += h2[g];
-          }
-          if (live_then > 0) {
-            prof_ms[0] += ma;
-            prof_ms[1] += mb;
-            prof_flops += 2.0 * (double)live_then * (double)n * (double)r;   // per GEMM
-            prof_samples += 1;
-          }
-        }
-        if (trace && batch >= 2) {
-          float bms = 0.f;
-          cudaEventElapsedTime(&bms, ev.poll[(batch - 2) % POLL_RING], ev.poll[prev]);
-          const int32_t* h2 = h_ns.as<int32_t>() + (int)((batch - 2) % POLL_RING) * GEMM_MAX_GROUPS;
-          int l2 = 0, m2 = 0;
+        // live columns during batch b = the counts after the compaction of batch b-1 (all columns for b = 0)
+        int live_then = GB, max_then = B;
+        if (b >= 1) {
+          const int32_t* h1 = h_ns.as<int32_t>() + (int)((b - 1) % POLL_RING) * GEMM_MAX_GROUPS;
+          live_then = max_then = 0;
           for (int g = 0; g < G; ++g) {
-            l2 += h2[g];
-            m2 = std::max(m2, h2[g]);
+            live_then += h1[g];
+            max_then = std::max(max_then, h1[g]);
           }
-          fprintf(trace, "%d %lld %d %d %d %d %.4f\n", rnd, (long long)(batch - 1), l2, m2, tileA.cfg, tileB.cfg, bms);
         }
-        if (live == 0) finished = true;   // the batch enqueued above finds no live slot and does nothing
+        if (opts->profile && live_then > 0) {
+          float ma = 0.f, mb = 0.f;   // the sampled GEMMs of batch b precede its poll event
+          TKM_CUDA(cudaEventElapsedTime(&ma, ev.pev[cur][0], ev.pev[cur][1]));
+          TKM_CUDA(cudaEventElapsedTime(&mb, ev.pev[cur][1], ev.pev[cur][2]));
+          prof_ms[0] += ma;
+          prof_ms[1] += mb;
+          prof_flops += 2.0 * (double)live_then * (double)n * (double)r;   // per GEMM
+          prof_samples += 1;
+        }
+        if (trace && b >= 1) {
+          float bms = 0.f;
+          cudaEventElapsedTime(&bms, ev.poll[(b - 1) % POLL_RING], ev.poll[cur]);
+          fprintf(trace, "%d %lld %d %d %d %d %.4f\n", rnd, (long long)b, live_then, max_then, tileA.cfg, tileB.cfg, bms);
+        }
+        ++done_polls;
+        if (live == 0) finished = true;   // batches already enqueued beyond b find no live slot and do nothing
       }
       ++batch;
     }
