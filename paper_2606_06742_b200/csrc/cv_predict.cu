@@ -113,14 +113,25 @@ __global__ void cv_select_kernel(const double* __restrict__ cv_loss, int T, int 
   best_l[t] = bl;
 }
 
-// out[i] = sum_j Mt[j][i] a[j], i < cols (alpha = U a from U^T; gamma = lmap a from lmap^T)
-__global__ void tmatvec_kernel(const double* __restrict__ Mt, int64_t ld, int rows, int cols,
-                               const double* __restrict__ a, double* __restrict__ out) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= cols) return;
+// out[i] = sum_j Mt[j][i] a[j], i < cols (alpha = U a from U^T; gamma = lmap a from lmap^T).  One CTA per 32
+// outputs: 8 row lanes x 32 columns walk the rows with coalesced 256-byte reads and are summed in a fixed
+// order (deterministic); rows / 8 dependent loads per thread instead of rows.
+__global__ void __launch_bounds__(256) tmatvec_kernel(const double* __restrict__ Mt, int64_t ld, int rows, int cols,
+                                                      const double* __restrict__ a, double* __restrict__ out) {
+  __shared__ double part[8][33];
+  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+  const int i = blockIdx.x * 32 + tx;
   double s = 0.0;
-  for (int j = 0; j < rows; ++j) s = fma(Mt[(int64_t)j * ld + i], a[j], s);
-  out[i] = s;
+  if (i < cols)
+    for (int j = ty; j < rows; j += 8) s = fma(Mt[(int64_t)j * ld + i], a[j], s);
+  part[ty][tx] = s;
+  __syncthreads();
+  if (ty == 0 && i < cols) {
+    double t = 0.0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) t += part[k][tx];
+    out[i] = t;
+  }
 }
 
 // f(x_q) = sum_i exp(-||x_q - x_i||^2 / (2 sigma^2)) alpha_i + beta0, PQ new points per CTA
@@ -184,9 +195,9 @@ static int coef_device(const tkm_path* p, int col, double* out, cudaStream_t st)
   const tkm_spectral* s = p->spec;
   const double* a = p->a.as<double>() + (int64_t)col * s->ldr;
   if (s->m > 0) {
-    tmatvec_kernel<<<(unsigned)ceil_div(s->m, 128), 128, 0, st>>>(s->lmap_t.as<double>(), s->ldm, (int)s->r, (int)s->m, a, out);
+    tmatvec_kernel<<<(unsigned)ceil_div(s->m, 32), 256, 0, st>>>(s->lmap_t.as<double>(), s->ldm, (int)s->r, (int)s->m, a, out);
   } else {
-    tmatvec_kernel<<<(unsigned)ceil_div(s->n, 128), 128, 0, st>>>(s->Ut.as<double>(), s->ldn, (int)s->r, (int)s->n, a, out);
+    tmatvec_kernel<<<(unsigned)ceil_div(s->n, 32), 256, 0, st>>>(s->Ut.as<double>(), s->ldn, (int)s->r, (int)s->n, a, out);
   }
   TKM_LAUNCH_CHECK();
   return TKM_OK;
