@@ -847,7 +847,9 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
         // FP64 GEMM-B: always without the delta form; with it, on the first iteration of a round (no zeta yet)
         // and on the last iteration of every batch, whose exact rho carries the stop test before the compaction
         const bool exact_it = !delta || (batch == 0 && k == 0) || k == check_every - 1;
-        const bool sample = opts->profile && k == check_every - 1;
+        // sampled launches: right after a compaction every slot is live, so the counted flops are all useful; the
+        // delta form has its FP64 GEMM-B on the last iteration of the batch instead
+        const bool sample = opts->profile && k == (delta ? check_every - 1 : 0);
         if (sample) TKM_CUDA(cudaEventRecord(ev.pev[ring][0], st));
         LossEpi le{(const double*)y, d_fold.as<int32_t>(), col_of_slot.as<int32_t>(), bbar.as<double>(),
                    p0->col_nc.as<double>(), p0->col_tau.as<double>(), p0->col_v.as<int32_t>(), B, (int)loss, smooth,
