@@ -69,7 +69,8 @@ typedef struct {
   double warm_tol;    /* tolerance of rounds 0..R-2 (warm starts only); <= 0 => same as tol   */
   int32_t profile;    /* 1: time the two contractions of the first iteration after every poll */
                       /* with CUDA events (read with tkm_path_profile); 0: no events          */
-  int32_t tf32_delta; /* 1: delta-form GEMM-B.  zeta = U^T z is kept in FP64 and advanced by        */
+  int32_t tf32_delta; /* 2: both contractions in delta form (also F = U Lam a: F+ = Fbar - U Lam da, two  */
+                      /* FP64 GEMM-A per exact iteration).  1: delta-form GEMM-B only.  zeta = U^T z is kept in FP64 and advanced by        */
                       /* zeta += U^T (z - z_old) with the increment contracted in 3xTF32 on the     */
                       /* tcgen05 tensor cores (its error is relative to the increment, which        */
                       /* vanishes at convergence); zeta is recomputed in FP64 after every           */

@@ -288,7 +288,7 @@ def _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, prof
     taus_arr = _host(taus if taus is not None else [], np.float64)
     o = _LossOpts(float(smooth0), float(eta), int(rounds), int(len(taus_arr)),
                   taus_arr.ctypes.data_as(C.POINTER(C.c_double)) if len(taus_arr) else None,
-                  int(bool(restart)), int(check_every), float(warm_tol), int(bool(profile)), int(bool(tf32_delta)))
+                  int(bool(restart)), int(check_every), float(warm_tol), int(bool(profile)), int(tf32_delta))
     return o, taus_arr
 
 

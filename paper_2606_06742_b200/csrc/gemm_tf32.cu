@@ -9,8 +9,8 @@ namespace tkm {
 // x -> hi = tf32(x), lo = tf32(x - hi); both stored as FP32 bit patterns with the low 13 mantissa bits zero
 __global__ void split_tf32_kernel(const double* __restrict__ src, int64_t lds, int rows, int cols, float* __restrict__ hi,
                                   float* __restrict__ lo, int64_t ldo) {
-  const int r = blockIdx.y;
-  for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < cols; c += gridDim.x * blockDim.x) {
+  const int r = blockIdx.x;   // rows on grid.x: no 65535 limit
+  for (int c = blockIdx.y * blockDim.x + threadIdx.x; c < cols; c += gridDim.y * blockDim.x) {
     const double v = src[(int64_t)r * lds + c];
     const float h = to_tf32((float)v);
     const float l = to_tf32((float)(v - (double)h));
@@ -24,7 +24,7 @@ int tf32_bn_of(int cfg) { return cfg == 0 ? 64 : (cfg == 1 ? 128 : 256); }
 
 int split_tf32(const double* src, int64_t lds, int64_t rows, int64_t cols, float* hi, float* lo, int64_t ldo,
                cudaStream_t st) {
-  dim3 grid((unsigned)std::min<int64_t>(ceil_div(cols, 256), 64), (unsigned)rows);
+  dim3 grid((unsigned)rows, (unsigned)std::min<int64_t>(ceil_div(cols, 256), 64));
   split_tf32_kernel<<<grid, 256, 0, st>>>(src, lds, (int)rows, (int)cols, hi, lo, ldo);
   TKM_LAUNCH_CHECK();
   return TKM_OK;

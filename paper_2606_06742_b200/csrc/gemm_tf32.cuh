@@ -49,6 +49,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, 1) gemm_tf32x3_kernel(const __gr
   __shared__ __align__(8) uint64_t empty_bar[STAGES];
   __shared__ __align__(8) uint64_t accum_bar;
   __shared__ uint32_t tmem_slot;
+  __shared__ double epi_red[Epi::kReduce ? 4 : 1][Epi::kReduce ? BN : 1];   // per-warp slot sums of a reducing epilogue
 
   const int grp = blockIdx.z;
   const int N = g.nslots ? min(g.nslots[grp], g.N) : g.N;
@@ -135,7 +136,14 @@ __global__ void __launch_bounds__(Cfg::THREADS, 1) gemm_tf32x3_kernel(const __gr
       if (n_blk0 + c0 >= N) break;   // warp-uniform
       float v[16];
       tmem_ld_32x16(tmem_base + ((uint32_t)(32 * q) << 16) + (uint32_t)c0, v);
-      epi.chunk(v, m, n_blk0 + c0, N, g.M, grp);
+      epi.chunk(v, m, n_blk0 + c0, N, g.M, grp, Epi::kReduce ? &epi_red[q][c0] : nullptr, lane);
+    }
+    if constexpr (Epi::kReduce) {
+      // sum the four warps' per-slot sums in a fixed order: one thread per slot of the tile
+      asm volatile("bar.sync 2, 128;\n" ::: "memory");
+      for (int c = tid - 64; c < BN; c += 128)
+        if (n_blk0 + c < N)
+          epi.finish(n_blk0 + c, epi_red[0][c] + epi_red[1][c] + epi_red[2][c] + epi_red[3][c], (int)blockIdx.x, grp);
     }
   }
   tc_fence_before();
@@ -145,10 +153,11 @@ __global__ void __launch_bounds__(Cfg::THREADS, 1) gemm_tf32x3_kernel(const __gr
 
 // plain store epilogue: Dt[n][m] = acc  (FP64 output array, one slot per row)
 struct Tf32StoreEpi {
+  static constexpr bool kReduce = false;
   double* Dt;
   int64_t ldd;
   int64_t group_stride;
-  __device__ __forceinline__ void chunk(const float (&v)[16], int m, int n0, int N, int M, int grp) const {
+  __device__ __forceinline__ void chunk(const float (&v)[16], int m, int n0, int N, int M, int grp, double*, int) const {
     if (m >= M) return;
     double* base = Dt + (int64_t)grp * group_stride + m;
 #pragma unroll

@@ -81,6 +81,7 @@ struct LossEpi {
   float* dz_hi;              // [G*B][lddz] by gs or NULL: TF32 (hi, lo) split of z - z_old, the operand of the
   float* dz_lo;              //   delta-form GEMM-B (zeta += U^T dz on the tcgen05 tensor cores)
   int64_t lddz;
+  double* Fb;                // [G*B][ldz] by gs or NULL: keeps Fbar = U Lam abar for the delta-form GEMM-A
   template <class Cfg>
   __device__ __forceinline__ void run(double (&acc)[Cfg::TN][Cfg::TM][2], int n_blk0, int m_blk0, int warp_n,
                                       int warp_m, int lane, int N, int M, int grp, double* scratch) const {
@@ -125,8 +126,10 @@ struct LossEpi {
         }
         if (m + 1 < M) {
           *reinterpret_cast<double2*>(zrow + m) = make_double2(z[0], z[1]);
+          if (Fb) *reinterpret_cast<double2*>(Fb + (int64_t)(g0 + slot) * ldz + m) = make_double2(acc[i][j][0], acc[i][j][1]);
         } else if (m < M) {
           zrow[m] = z[0];
+          if (Fb) Fb[(int64_t)(g0 + slot) * ldz + m] = acc[i][j][0];
         }
       }
     }
@@ -179,6 +182,7 @@ struct SpecEpi {
 // Thread = one spectral index i (a TMEM lane), 16 consecutive slots per call; for a fixed slot the 32 lanes
 // of a warp touch 32 consecutive doubles.
 struct ZetaEpi {
+  static constexpr bool kReduce = false;
   const int32_t* col_of_slot;   // [G*B]
   const double* col_lam;        // [B]
   int B;
@@ -186,7 +190,7 @@ struct ZetaEpi {
   int64_t lda;
   double* Zeta;                 // [G*B][lda]
   double* Rho;                  // [G*B][lda]
-  __device__ __forceinline__ void chunk(const float (&v)[16], int i, int n0, int N, int M, int grp) const {
+  __device__ __forceinline__ void chunk(const float (&v)[16], int i, int n0, int N, int M, int grp, double*, int) const {
     if (i >= M) return;
     const int g0 = grp * B;
 #pragma unroll
@@ -199,6 +203,65 @@ struct ZetaEpi {
       Zeta[o] = z;
       Rho[o] = z + two_lam * Abar[o];
     }
+  }
+};
+
+// ---- delta-form GEMM-A epilogue (tcgen05 kernel): F+ = Fbar - U Lam da, next extrapolation, loss derivative ----
+// Thread = one sample row m (a TMEM lane), 16 consecutive slots per call.  State per slot: Fb = Fbar_k (what the
+// loss saw), Fp = F_k.  With G = U Lam da_k from the accumulator:  F_{k+1} = Fbar_k - G,
+// Fbar_{k+1} = F_{k+1} + mu_{k+1} (F_{k+1} - F_k), then z, dz and the column sum of z exactly as in LossEpi.
+struct FLossEpi {
+  static constexpr bool kReduce = true;
+  const double* y;
+  const int32_t* foldid;
+  const int32_t* col_of_slot;   // [G*B]
+  const double* bbar;           // [G*B] by gc
+  const double* mu;             // [G*B] by gc: momentum that formed the current abar
+  const double* col_nc;
+  const double* col_tau;
+  const int32_t* col_v;
+  int B, loss;
+  double smooth;
+  double* Fb;                   // [G*B][ldz]
+  double* Fp;                   // [G*B][ldz]
+  double* Zt;                   // [G*B][ldz]
+  int64_t ldz;
+  float* dz_hi;
+  float* dz_lo;
+  int64_t lddz;
+  double* gpart;
+  int64_t ldpart;
+  __device__ __forceinline__ void chunk(const float (&v)[16], int m, int n0, int N, int M, int grp, double* red,
+                                        int lane) const {
+    const bool live = m < M;
+    const double yv = live ? y[m] : 0.0;
+    const int fv = live ? foldid[m] : -1;
+    const int g0 = grp * B;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+      const int slot = n0 + k;
+      if (slot >= N) break;   // warp-uniform
+      const int gs = g0 + slot, col = col_of_slot[gs], gc = g0 + col;
+      double z = 0.0;
+      if (live) {
+        const int64_t o = (int64_t)gs * ldz + m;
+        const double fn = Fb[o] - (double)v[k];
+        const double fb = fn + mu[gc] * (fn - Fp[o]);
+        Fp[o] = fn;
+        Fb[o] = fb;
+        if (fv != col_v[col]) z = psi_dev(loss, yv, fb + bbar[gc], smooth, col_tau[col]) / col_nc[col];
+        const double d = z - Zt[o];
+        Zt[o] = z;
+        const float h = to_tf32((float)d);
+        dz_hi[(int64_t)gs * lddz + m] = h;
+        dz_lo[(int64_t)gs * lddz + m] = to_tf32((float)(d - (double)h));
+      }
+      const double t = warp_sum(z);
+      if (lane == 0) red[k] = t;
+    }
+  }
+  __device__ __forceinline__ void finish(int slot, double total, int mtile, int grp) const {
+    gpart[(int64_t)mtile * ldpart + grp * B + slot] = total;
   }
 };
 
@@ -266,6 +329,10 @@ struct UpdateArgs {
   double *A, *Aprev, *Abar;
   double *beta, *beta_prev, *bbar, *rk, *kkt;   // [G*B]
   int32_t *done, *iters, *iters_round, *flags;  // [G*B]
+  float* da_hi;    // [G*B][ldda] by gs or NULL: TF32 (hi, lo) split of the step da, operand of the delta-form GEMM-A
+  float* da_lo;
+  int64_t ldda;
+  double* mu;      // [G*B] by gc or NULL: momentum used for the new abar
 };
 
 // One CTA per live slot.  The vectors are walked in chunks of 256 x UPD_EPT pairs with all loads of a chunk
@@ -368,6 +435,13 @@ __global__ void __launch_bounds__(256, 2) update_kernel(UpdateArgs p) {
         a_new[e] = make_double2(ab[e].x - dax, ab[e].y - day);
         g += dax * (a_new[e].x - a_old[e].x) + day * (a_new[e].y - a_old[e].y);
         if (!single) Ap2[i] = a_new[e];   // a' is dead once abar has been formed: scratch for a+
+        if (p.da_hi) {
+          const float hx = to_tf32((float)dax), hy = to_tf32((float)day);
+          const int64_t o = (int64_t)gs * p.ldda + 2 * i;
+          *reinterpret_cast<float2*>(p.da_hi + o) = make_float2(hx, hy);
+          *reinterpret_cast<float2*>(p.da_lo + o) =
+              make_float2(to_tf32((float)(dax - (double)hx)), to_tf32((float)(day - (double)hy)));
+        }
       }
     }
   }
@@ -421,6 +495,7 @@ __global__ void __launch_bounds__(256, 2) update_kernel(UpdateArgs p) {
     p.beta[gc] = beta_new;
     p.bbar[gc] = beta_new + mu * (beta_new - beta);
     p.rk[gc] = rk;
+    if (p.mu) p.mu[gc] = mu;
     p.kkt[gc] = kkt;
     p.iters[gc] += 1;
     const int itr = p.iters_round[gc] + 1;
@@ -453,6 +528,9 @@ struct CompactArgs {
   double* Zt;               // [G*B][ldz] or NULL (delta form)
   int64_t ldz;
   int n;
+  double *Fb, *Fp;          // [G*B][ldz] or NULL (delta form of GEMM-A)
+  float *da_hi, *da_lo;     // [G*B][ldda] or NULL
+  int64_t ldda;
 };
 
 __global__ void __launch_bounds__(1024) compact_plan_kernel(CompactArgs p) {
@@ -546,6 +624,17 @@ __global__ void __launch_bounds__(256) compact_apply_kernel(CompactArgs p) {
   if (p.Zt) {
     const int64_t zs = (int64_t)(g0 + sl) * p.ldz, zt = (int64_t)(g0 + src) * p.ldz;
     for (int i = threadIdx.x; i < p.n; i += blockDim.x) p.Zt[zs + i] = p.Zt[zt + i];
+    if (p.Fb) {
+      for (int i = threadIdx.x; i < p.n; i += blockDim.x) {
+        p.Fb[zs + i] = p.Fb[zt + i];
+        p.Fp[zs + i] = p.Fp[zt + i];
+      }
+      const int64_t ds = (int64_t)(g0 + sl) * p.ldda, dt = (int64_t)(g0 + src) * p.ldda;
+      for (int i = threadIdx.x; i < p.r; i += blockDim.x) {
+        p.da_hi[ds + i] = p.da_hi[dt + i];
+        p.da_lo[ds + i] = p.da_lo[dt + i];
+      }
+    }
   }
   if (threadIdx.x == 0) p.col_of_slot[g0 + sl] = p.col_of_slot[g0 + src];
 }
@@ -726,9 +815,28 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
       TKM_TRY(split_tf32(specs[g]->Ut.as<double>(), ldn, r, n, ut_hi[g].as<float>(), ut_lo[g].as<float>(), ldn32, st));
     }
   }
-  Tf32Args targs;
+  // F half (tf32_delta == 2): Fbar / F state, the (hi, lo) step operand, U Lam as (hi, lo), momentum per column
+  const bool delta_f = opts->tf32_delta == 2;
+  const int64_t ldr32 = round_up(r, 32);
+  DevBuf Fb, Fp, da_hi, da_lo, mu, ul_hi[GEMM_MAX_GROUPS], ul_lo[GEMM_MAX_GROUPS];
+  if (delta_f) {
+    TKM_TRY(Fb.alloc((size_t)GB * ldn * sizeof(double), true, st));
+    TKM_TRY(Fp.alloc((size_t)GB * ldn * sizeof(double), true, st));
+    TKM_TRY(da_hi.alloc((size_t)GB * ldr32 * sizeof(float), true, st));
+    TKM_TRY(da_lo.alloc((size_t)GB * ldr32 * sizeof(float), true, st));
+    TKM_TRY(mu.alloc((size_t)GB * sizeof(double), true, st));
+    for (int g = 0; g < G; ++g) {
+      TKM_TRY(ul_hi[g].alloc((size_t)n * ldr32 * sizeof(float), true, st));
+      TKM_TRY(ul_lo[g].alloc((size_t)n * ldr32 * sizeof(float), true, st));
+      TKM_TRY(split_tf32(specs[g]->UL.as<double>(), ldr, n, r, ul_hi[g].as<float>(), ul_lo[g].as<float>(), ldr32, st));
+    }
+  }
+  Tf32Args targs, targsF;
   memset(&targs, 0, sizeof(targs));
+  memset(&targsF, 0, sizeof(targsF));
   int tcfg = -1;
+  GemmProblem prA2 = {};   // F = U Lam a on the exact iterations of the F half (same tiles as GEMM-A, P = a)
+  GemmArgs argsA2;
   PinBuf h_ns;   // [POLL_RING][GEMM_MAX_GROUPS] live-slot counts read back after every compaction
   TKM_TRY(h_ns.alloc((size_t)POLL_RING * GEMM_MAX_GROUPS * sizeof(int32_t)));
 
@@ -817,6 +925,12 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
       if (tA.cfg != tileA.cfg) {
         TKM_TRY(gemm_f64_make_args(prA, tA, &argsA));
         argsA.nslots = nslots.as<int32_t>();
+        if (delta_f) {
+          prA2 = prA;
+          prA2.P = A.as<double>();
+          TKM_TRY(gemm_f64_make_args(prA2, tA, &argsA2));
+          argsA2.nslots = nslots.as<int32_t>();
+        }
         tileA = tA;
       }
       if (tB.cfg != tileB.cfg) {
@@ -839,10 +953,23 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
           targs.p_group_rows = B;
           targs.M = (int)r;
           targs.K = (int)n;
+          if (delta_f) {
+            TKM_TRY(make_tmap_f32(&targsF.p_hi, da_hi.as<float>(), GB, r, ldr32, bn));
+            TKM_TRY(make_tmap_f32(&targsF.p_lo, da_lo.as<float>(), GB, r, ldr32, bn));
+            for (int g = 0; g < G; ++g) {
+              TKM_TRY(make_tmap_f32(&targsF.q_hi[g], ul_hi[g].as<float>(), n, r, ldr32, TF32_BM));
+              TKM_TRY(make_tmap_f32(&targsF.q_lo[g], ul_lo[g].as<float>(), n, r, ldr32, TF32_BM));
+            }
+            targsF.nslots = nslots.as<int32_t>();
+            targsF.p_group_rows = B;
+            targsF.M = (int)n;
+            targsF.K = (int)r;
+          }
           tcfg = want;
         }
-        targs.N = std::max(nmax, 1);
+        targs.N = targsF.N = std::max(nmax, 1);
       }
+      argsA2.N = argsA.N;
       for (int k = 0; k < check_every; ++k) {
         // FP64 GEMM-B: always without the delta form; with it, on the first iteration of a round (no zeta yet)
         // and on the last iteration of every batch, whose exact rho carries the stop test before the compaction
@@ -851,11 +978,26 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
         // delta form has its FP64 GEMM-B on the last iteration of the batch instead
         const bool sample = opts->profile && k == (delta ? check_every - 1 : 0);
         if (sample) TKM_CUDA(cudaEventRecord(ev.pev[ring][0], st));
-        LossEpi le{(const double*)y, d_fold.as<int32_t>(), col_of_slot.as<int32_t>(), bbar.as<double>(),
-                   p0->col_nc.as<double>(), p0->col_tau.as<double>(), p0->col_v.as<int32_t>(), B, (int)loss, smooth,
-                   Zt.as<double>(), ldn, gpart.as<double>(), ldpart, delta ? dz_hi.as<float>() : nullptr,
-                   delta ? dz_lo.as<float>() : nullptr, ldn32};
-        TKM_TRY(gemm_f64_launch(argsA, tileA, G, le, st));
+        int nblkA = (int)ceil_div(n, tileA.BM);
+        if (delta_f && !exact_it) {
+          // F half: F+ = Fbar - U Lam da on the tcgen05 tensor cores, loss derivative in its epilogue
+          FLossEpi fe{(const double*)y, d_fold.as<int32_t>(), col_of_slot.as<int32_t>(), bbar.as<double>(),
+                      mu.as<double>(), p0->col_nc.as<double>(), p0->col_tau.as<double>(), p0->col_v.as<int32_t>(), B,
+                      (int)loss, smooth, Fb.as<double>(), Fp.as<double>(), Zt.as<double>(), ldn, dz_hi.as<float>(),
+                      dz_lo.as<float>(), ldn32, gpart.as<double>(), ldpart};
+          TKM_TRY(gemm_tf32_launch(targsF, tcfg, G, fe, st));
+          nblkA = (int)ceil_div(n, TF32_BM);
+        } else {
+          LossEpi le{(const double*)y, d_fold.as<int32_t>(), col_of_slot.as<int32_t>(), bbar.as<double>(),
+                     p0->col_nc.as<double>(), p0->col_tau.as<double>(), p0->col_v.as<int32_t>(), B, (int)loss, smooth,
+                     Zt.as<double>(), ldn, gpart.as<double>(), ldpart, delta ? dz_hi.as<float>() : nullptr,
+                     delta ? dz_lo.as<float>() : nullptr, ldn32, delta_f ? Fb.as<double>() : nullptr};
+          TKM_TRY(gemm_f64_launch(argsA, tileA, G, le, st));
+          if (delta_f) {   // exact iteration of the F half: also F = U Lam a, so that both recurrence states are exact
+            StoreEpi fs{Fp.as<double>(), ldn, (int64_t)B * ldn, 1.0};
+            TKM_TRY(gemm_f64_launch(argsA2, tileA, G, fs, st));
+          }
+        }
         if (sample) TKM_CUDA(cudaEventRecord(ev.pev[ring][1], st));
         if (exact_it) {
           // FP64 contraction; in delta form it also re-establishes zeta = U^T z exactly
@@ -868,13 +1010,14 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
           TKM_TRY(gemm_tf32_launch(targs, tcfg, G, ze, st));
         }
         if (sample) TKM_CUDA(cudaEventRecord(ev.pev[ring][2], st));
-        UpdateArgs ua{(int)r, (int)n, B, (int)ceil_div(n, tileA.BM), restart, maxit, exact_it ? 1 : 0, ldr,
+        UpdateArgs ua{(int)r, (int)n, B, nblkA, restart, maxit, exact_it ? 1 : 0, ldr,
                       ldpart, rtol, gp, nslots.as<int32_t>(), col_of_slot.as<int32_t>(), p0->col_lam.as<double>(),
                       col_c.as<double>(), p0->col_nc.as<double>(), col_s.as<double>(), gpart.as<double>(),
                       Rho.as<double>(), A.as<double>(), Aprev.as<double>(),
                       Abar.as<double>(), beta.as<double>(), beta_prev.as<double>(), bbar.as<double>(), rk.as<double>(),
                       kkt.as<double>(), done.as<int32_t>(), iters.as<int32_t>(), iters_round.as<int32_t>(),
-                      flags.as<int32_t>()};
+                      flags.as<int32_t>(), delta_f ? da_hi.as<float>() : nullptr, delta_f ? da_lo.as<float>() : nullptr,
+                      ldr32, delta_f ? mu.as<double>() : nullptr};
         update_kernel<<<dim3(std::max(nmax, 1), G), 256, 0, st>>>(ua);
         TKM_LAUNCH_CHECK();
       }
@@ -882,7 +1025,9 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
       CompactArgs ca{B, (int)r, ldr, gp, nslots.as<int32_t>(), col_of_slot.as<int32_t>(), done.as<int32_t>(),
                      fin_list.as<int32_t>(), tail_list.as<int32_t>(), counts.as<int32_t>(), A.as<double>(),
                      Aprev.as<double>(), Abar.as<double>(), delta ? Zeta.as<double>() : nullptr,
-                     delta ? Zt.as<double>() : nullptr, ldn, (int)n};
+                     delta ? Zt.as<double>() : nullptr, ldn, (int)n, delta_f ? Fb.as<double>() : nullptr,
+                     delta_f ? Fp.as<double>() : nullptr, delta_f ? da_hi.as<float>() : nullptr,
+                     delta_f ? da_lo.as<float>() : nullptr, ldr32};
       compact_plan_kernel<<<G, 1024, 0, st>>>(ca);
       TKM_LAUNCH_CHECK();
       compact_apply_kernel<<<dim3(std::max(nmax, 1), G), 256, 0, st>>>(ca);

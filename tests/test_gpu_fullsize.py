@@ -64,8 +64,8 @@ def _first_order(w, tkm, path, K, y_np, foldid, cols, smooth_final):
     return worst, fs
 
 
-@pytest.mark.parametrize("cfg", [2, 3])
-def test_full_kernel_configs_first_order_optimality(tkm, cfg):
+@pytest.mark.parametrize("cfg,delta", [(2, 0), (3, 0), (3, 2)])
+def test_full_kernel_configs_first_order_optimality(tkm, cfg, delta):
     import torch
     w = wl.CONFIGS[cfg]()
     sigma = float(w.sigmas[0])
@@ -80,7 +80,7 @@ def test_full_kernel_configs_first_order_optimality(tkm, cfg):
     assert np.max(np.abs(K[_dev(rows)][:, _dev(rows)].cpu().numpy() - o.gram_rbf(w.X[rows], sigma))) < 1e-13
     spec = tkm.tkm_spectral_setup(K)
     path = tkm.tkm_fit_path(spec, y, w.loss, w.lambdas, foldid, w.V, TOL, MAXIT, smooth0=w.smooth0, eta=w.eta,
-                            rounds=w.rounds, taus=w.taus if len(w.taus) else None, warm_tol=WARM_TOL)
+                            rounds=w.rounds, taus=w.taus if len(w.taus) else None, warm_tol=WARM_TOL, tf32_delta=delta)
     info = path.info()
     assert info["flags"].sum() == 0 and np.all(info["kkt"] <= TOL)
     cv_loss, cv_err, cv_mean, best = tkm.tkm_exact_cv(path, y, foldid, w.T, w.L, w.V)
@@ -89,7 +89,8 @@ def test_full_kernel_configs_first_order_optimality(tkm, cfg):
     cols = [(t * (V + 1) + v) * L + l for (t, v, l) in
             [(0, 0, 0), (0, 1, L // 3), (0, V, L // 2), (w.T - 1, V - 1, (3 * L) // 4), (w.T - 1, 2, L - 1)]]
     worst, fs = _first_order(w, tkm, path, K, w.y, foldid, cols, smooth_final)
-    print("cfg %d: |sum z| %.2e, n_c||z + 2 lam alpha||/sqrt(n) %.2e, held-out alpha %.2e" % (cfg, *worst))
+    print("cfg %d (tf32_delta %d): |sum z| %.2e, n_c||z + 2 lam alpha||/sqrt(n) %.2e, held-out alpha %.2e"
+          % (cfg, delta, *worst))
     assert worst[0] <= 20 * TOL and worst[1] <= 20 * TOL and worst[2] <= 1e-7
     for c in cols:
         t, v, l = c // ((V + 1) * L), (c // L) % (V + 1), c % L
@@ -130,7 +131,7 @@ def test_nystrom_config4_first_order_optimality(tkm):
     spec = tkm.tkm_spectral_setup(nystrom=(K_nm, K_mm, idx))
     assert spec.n == w.n and 0 < spec.r <= w.m_landmarks
     path = tkm.tkm_fit_path(spec, y, w.loss, w.lambdas, foldid, w.V, TOL, MAXIT, smooth0=w.smooth0, eta=w.eta,
-                            rounds=w.rounds, warm_tol=WARM_TOL)
+                            rounds=w.rounds, warm_tol=WARM_TOL, tf32_delta=2)    # both contractions in delta form
     info = path.info()
     assert info["flags"].sum() == 0 and np.all(info["kkt"] <= TOL)
     cv_loss, cv_err, cv_mean, best = tkm.tkm_exact_cv(path, y, foldid, 1, w.L, w.V)

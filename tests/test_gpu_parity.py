@@ -429,17 +429,19 @@ def test_platt_on_held_out_decision_values(tkm):
 
 
 # ------------------------------------------------------------------------------- delta-form GEMM-B (tcgen05)
+@pytest.mark.parametrize("mode", [1, 2])
 @pytest.mark.parametrize("name", ["cfg0", "kqr_ragged", "logit_ragged"])
-def test_delta_form_sweep_keeps_fp64_parity(tkm, name):
-    """tkm_loss_opts.tf32_delta: zeta = U^T z advanced by 3xTF32 increments on the tcgen05 tensor cores, exact FP64
-    contraction and stop test on the last iteration of every batch.  Same 1e-10 coefficient bar."""
+def test_delta_form_sweep_keeps_fp64_parity(tkm, name, mode):
+    """tkm_loss_opts.tf32_delta: zeta = U^T z (mode 1) and also F = U Lam a (mode 2) advanced by 3xTF32 increments
+    on the tcgen05 tensor cores, exact FP64 contractions and stop test on the last iteration of every batch
+    (DESIGN.md 12).  Same 1e-10 coefficient bar."""
     w = {"cfg0": lambda: wl.config0(), "kqr_ragged": lambda: wl.config3(n=261, p=5, L=5, V=4, taus=(0.1, 0.5, 0.9)),
          "logit_ragged": lambda: wl.config2(n=333, p=9, L=7, V=3)}[name]()
     sigma = float(w.sigmas[0])
     foldid = tkm.tkm_make_folds(w.n, w.V, w.fold_seed)
-    X, y, spec, path, cv = _run_gpu(tkm, w, sigma, foldid, STOP_TOL, 400000, tf32_delta=True)
+    X, y, spec, path, cv = _run_gpu(tkm, w, sigma, foldid, STOP_TOL, 400000, tf32_delta=mode)
     res, spec_o, worst, degenerate = _compare_path(tkm, w, sigma, foldid, spec, path, cv)
-    print("%s (delta form): worst relative l2 coefficient error %.3g" % (name, worst))
+    print("%s (delta form %d): worst relative l2 coefficient error %.3g" % (name, mode, worst))
     cv_o = o.exact_cv(spec_o, res, w.y, foldid, w.loss, w.taus)
     if not degenerate:
         assert np.max(np.abs(cv[0] - cv_o[0])) <= CV_TOL and np.array_equal(cv[3], cv_o[3])
