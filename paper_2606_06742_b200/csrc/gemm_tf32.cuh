@@ -8,8 +8,10 @@
 // Mapping: the fixed operand Q (rows of U) is the UMMA "A" operand, M = 128 rows = the 128 TMEM lanes; the
 // moving operand P (slots) is the UMMA "B" operand, N = BN slots = BN FP32 TMEM columns.  K advances 32
 // floats (one 128-byte swizzle span) per pipeline stage = 4 UMMA K-steps of 8, 3 MMAs each.
-// Warp roles (192 threads): warp 0 = TMA producer, warp 1 = MMA issuer (one elected thread), warps 2..5 =
-// epilogue (warp w owns TMEM lanes 32 (w % 4) .. +31, i.e. 32 rows of the tile); warp 2 allocates TMEM.
+// Warp roles (320 threads): warp 0 = TMA producer, warp 1 = MMA issuer (one elected thread), warps 2..9 =
+// epilogue (warp w owns TMEM lanes 32 (w % 4) .. +31, i.e. 32 rows of the tile; the two warps of a lane quarter
+// take alternate 16-column chunks -- FP64 epilogue arithmetic is latency-bound with one warp per scheduler);
+// warp 2 allocates TMEM.
 #pragma once
 
 #include <algorithm>
@@ -37,7 +39,7 @@ struct Tf32Cfg {
   static constexpr int B_BYTES = BN * 128;
   static constexpr int STAGE_BYTES = 2 * TF32_A_BYTES + 2 * B_BYTES;
   static constexpr size_t SMEM = (size_t)STAGES * STAGE_BYTES + 1024;
-  static constexpr int THREADS = 192;
+  static constexpr int THREADS = 320;
   static_assert(BN == 32 || BN == 64 || BN == 128 || BN == 256, "TMEM allocations are powers of two >= 32 columns");
 };
 
@@ -127,12 +129,12 @@ __global__ void __launch_bounds__(Cfg::THREADS, 1) gemm_tf32x3_kernel(const __gr
     }
   } else {
     // ===== epilogue: TMEM -> registers -> Epi =====
-    const int q = warp & 3;
+    const int q = warp & 3, half = (warp - 2) >> 2;   // warps 2..5: even chunks, warps 6..9: odd chunks
     mbar_wait(&accum_bar, 0);
     tc_fence_after();
     const int m = m_blk0 + 32 * q + lane;
 #pragma unroll 1
-    for (int c0 = 0; c0 < BN; c0 += 16) {
+    for (int c0 = 16 * half; c0 < BN; c0 += 32) {
       if (n_blk0 + c0 >= N) break;   // warp-uniform
       float v[16];
       tmem_ld_32x16(tmem_base + ((uint32_t)(32 * q) << 16) + (uint32_t)c0, v);
@@ -140,8 +142,8 @@ __global__ void __launch_bounds__(Cfg::THREADS, 1) gemm_tf32x3_kernel(const __gr
     }
     if constexpr (Epi::kReduce) {
       // sum the four warps' per-slot sums in a fixed order: one thread per slot of the tile
-      asm volatile("bar.sync 2, 128;\n" ::: "memory");
-      for (int c = tid - 64; c < BN; c += 128)
+      asm volatile("bar.sync 2, 256;\n" ::: "memory");
+      for (int c = tid - 64; c < BN; c += 256)
         if (n_blk0 + c < N)
           epi.finish(n_blk0 + c, epi_red[0][c] + epi_red[1][c] + epi_red[2][c] + epi_red[3][c], (int)blockIdx.x, grp);
     }

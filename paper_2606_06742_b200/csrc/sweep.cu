@@ -53,6 +53,19 @@ __device__ __forceinline__ double psi_dev(int loss, double y, double f, double s
   }
 }
 
+// Same function with the divisions hoisted: inv_2s = 1 / (2 smooth) (unused by the smooth losses).
+__device__ __forceinline__ double psi_fast(int loss, double y, double f, double smooth, double inv_2s, double tau) {
+  if (loss == TKM_LOSS_HINGE) {
+    const double u = y * f;
+    const double lp = (u <= 1.0 - smooth) ? -1.0 : ((u >= 1.0 + smooth) ? 0.0 : (u - 1.0 - smooth) * inv_2s);
+    return y * lp;
+  } else if (loss == TKM_LOSS_QUANTILE) {
+    const double t = y - f;
+    return -((t < -smooth) ? tau - 1.0 : ((t > smooth) ? tau : t * inv_2s + tau - 0.5));
+  }
+  return psi_dev(loss, y, f, smooth, tau);
+}
+
 // Per-group device pointers (one group = one spectral handle, e.g. one bandwidth of a sigma grid).
 struct GroupPtrs {
   const double* lam[GEMM_MAX_GROUPS];   // [ldr] eigenvalues
@@ -193,16 +206,25 @@ struct ZetaEpi {
   __device__ __forceinline__ void chunk(const float (&v)[16], int i, int n0, int N, int M, int grp, double*, int) const {
     if (i >= M) return;
     const int g0 = grp * B;
+    const int cnt = min(16, N - n0);
+    // all loads of the chunk first (16 independent round trips in flight), then the arithmetic and the stores
+    double zo[16], ab[16], tl[16];
 #pragma unroll
-    for (int k = 0; k < 16; ++k) {
-      const int slot = n0 + k;
-      if (slot >= N) break;
-      const double two_lam = 2.0 * col_lam[col_of_slot[g0 + slot]];
-      const int64_t o = (int64_t)(g0 + slot) * lda + i;
-      const double z = Zeta[o] + (double)v[k];
-      Zeta[o] = z;
-      Rho[o] = z + two_lam * Abar[o];
-    }
+    for (int k = 0; k < 16; ++k)
+      if (k < cnt) {
+        const int64_t o = (int64_t)(g0 + n0 + k) * lda + i;
+        zo[k] = Zeta[o];
+        ab[k] = Abar[o];
+        tl[k] = 2.0 * col_lam[col_of_slot[g0 + n0 + k]];
+      }
+#pragma unroll
+    for (int k = 0; k < 16; ++k)
+      if (k < cnt) {
+        const int64_t o = (int64_t)(g0 + n0 + k) * lda + i;
+        const double z = zo[k] + (double)v[k];
+        Zeta[o] = z;
+        Rho[o] = z + tl[k] * ab[k];
+      }
   }
 };
 
@@ -221,7 +243,7 @@ struct FLossEpi {
   const double* col_tau;
   const int32_t* col_v;
   int B, loss;
-  double smooth;
+  double smooth, inv_2s;
   double* Fb;                   // [G*B][ldz]
   double* Fp;                   // [G*B][ldz]
   double* Zt;                   // [G*B][ldz]
@@ -237,27 +259,49 @@ struct FLossEpi {
     const double yv = live ? y[m] : 0.0;
     const int fv = live ? foldid[m] : -1;
     const int g0 = grp * B;
+    const int cnt = min(16, N - n0);
+    // per half chunk: all loads first (independent round trips in flight), then the arithmetic and the stores
 #pragma unroll
-    for (int k = 0; k < 16; ++k) {
-      const int slot = n0 + k;
-      if (slot >= N) break;   // warp-uniform
-      const int gs = g0 + slot, col = col_of_slot[gs], gc = g0 + col;
-      double z = 0.0;
-      if (live) {
-        const int64_t o = (int64_t)gs * ldz + m;
-        const double fn = Fb[o] - (double)v[k];
-        const double fb = fn + mu[gc] * (fn - Fp[o]);
-        Fp[o] = fn;
-        Fb[o] = fb;
-        if (fv != col_v[col]) z = psi_dev(loss, yv, fb + bbar[gc], smooth, col_tau[col]) / col_nc[col];
-        const double d = z - Zt[o];
-        Zt[o] = z;
-        const float h = to_tf32((float)d);
-        dz_hi[(int64_t)gs * lddz + m] = h;
-        dz_lo[(int64_t)gs * lddz + m] = to_tf32((float)(d - (double)h));
-      }
-      const double t = warp_sum(z);
-      if (lane == 0) red[k] = t;
+    for (int h0 = 0; h0 < 16; h0 += 8) {
+      double fbv[8], fpv[8], zov[8], muv[8], bbv[8], ncv[8], tav[8];
+      int hv[8];
+#pragma unroll
+      for (int k = 0; k < 8; ++k)
+        if (h0 + k < cnt) {
+          const int gs = g0 + n0 + h0 + k, col = col_of_slot[gs], gc = g0 + col;
+          muv[k] = mu[gc];
+          bbv[k] = bbar[gc];
+          ncv[k] = 1.0 / col_nc[col];
+          tav[k] = col_tau[col];
+          hv[k] = col_v[col];
+          if (live) {
+            const int64_t o = (int64_t)gs * ldz + m;
+            fbv[k] = Fb[o];
+            fpv[k] = Fp[o];
+            zov[k] = Zt[o];
+          }
+        }
+#pragma unroll
+      for (int k = 0; k < 8; ++k)
+        if (h0 + k < cnt) {
+          double z = 0.0;
+          if (live) {
+            const int gs = g0 + n0 + h0 + k;
+            const int64_t o = (int64_t)gs * ldz + m;
+            const double fn = fbv[k] - (double)v[h0 + k];
+            const double fb = fn + muv[k] * (fn - fpv[k]);
+            Fp[o] = fn;
+            Fb[o] = fb;
+            if (fv != hv[k]) z = psi_fast(loss, yv, fb + bbv[k], smooth, inv_2s, tav[k]) * ncv[k];
+            const double d = z - zov[k];
+            Zt[o] = z;
+            const float h = to_tf32((float)d);
+            dz_hi[(int64_t)gs * lddz + m] = h;
+            dz_lo[(int64_t)gs * lddz + m] = to_tf32((float)(d - (double)h));
+          }
+          const double t = warp_sum(z);
+          if (lane == 0) red[h0 + k] = t;
+        }
     }
   }
   __device__ __forceinline__ void finish(int slot, double total, int mtile, int grp) const {
@@ -983,7 +1027,8 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
           // F half: F+ = Fbar - U Lam da on the tcgen05 tensor cores, loss derivative in its epilogue
           FLossEpi fe{(const double*)y, d_fold.as<int32_t>(), col_of_slot.as<int32_t>(), bbar.as<double>(),
                       mu.as<double>(), p0->col_nc.as<double>(), p0->col_tau.as<double>(), p0->col_v.as<int32_t>(), B,
-                      (int)loss, smooth, Fb.as<double>(), Fp.as<double>(), Zt.as<double>(), ldn, dz_hi.as<float>(),
+                      (int)loss, smooth, smooth > 0.0 ? 1.0 / (2.0 * smooth) : 0.0, Fb.as<double>(), Fp.as<double>(),
+                      Zt.as<double>(), ldn, dz_hi.as<float>(),
                       dz_lo.as<float>(), ldn32, gpart.as<double>(), ldpart};
           TKM_TRY(gemm_tf32_launch(targsF, tcfg, G, fe, st));
           nblkA = (int)ceil_div(n, TF32_BM);
