@@ -689,6 +689,7 @@ static double curvature_of(tkm_loss loss, double smooth) {
   return 1.0 / (2.0 * smooth);   // 1/kappa, kappa = 2 delta
 }
 
+constexpr int DELTA_MIN_LIVE = 48;   // live columns (all groups) below which the delta forms are switched off
 constexpr int POLL_RING = 5;   // ring of poll results: up to POLL_RING - 2 batches may be in flight
 
 }  // namespace tkm
@@ -854,8 +855,8 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
     TKM_TRY(dz_hi.alloc((size_t)GB * ldn32 * sizeof(float), true, st));
     TKM_TRY(dz_lo.alloc((size_t)GB * ldn32 * sizeof(float), true, st));
     for (int g = 0; g < G; ++g) {
-      TKM_TRY(ut_hi[g].alloc((size_t)r * ldn32 * sizeof(float), true, st));
-      TKM_TRY(ut_lo[g].alloc((size_t)r * ldn32 * sizeof(float), true, st));
+      TKM_TRY(ut_hi[g].alloc((size_t)r * ldn32 * sizeof(float), false, st));   // padding beyond n is outside the
+      TKM_TRY(ut_lo[g].alloc((size_t)r * ldn32 * sizeof(float), false, st));   // tensor maps: never read
       TKM_TRY(split_tf32(specs[g]->Ut.as<double>(), ldn, r, n, ut_hi[g].as<float>(), ut_lo[g].as<float>(), ldn32, st));
     }
   }
@@ -870,8 +871,8 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
     TKM_TRY(da_lo.alloc((size_t)GB * ldr32 * sizeof(float), true, st));
     TKM_TRY(mu.alloc((size_t)GB * sizeof(double), true, st));
     for (int g = 0; g < G; ++g) {
-      TKM_TRY(ul_hi[g].alloc((size_t)n * ldr32 * sizeof(float), true, st));
-      TKM_TRY(ul_lo[g].alloc((size_t)n * ldr32 * sizeof(float), true, st));
+      TKM_TRY(ul_hi[g].alloc((size_t)n * ldr32 * sizeof(float), false, st));
+      TKM_TRY(ul_lo[g].alloc((size_t)n * ldr32 * sizeof(float), false, st));
       TKM_TRY(split_tf32(specs[g]->UL.as<double>(), ldr, n, r, ul_hi[g].as<float>(), ul_lo[g].as<float>(), ldr32, st));
     }
   }
@@ -1014,16 +1015,20 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
         targs.N = targsF.N = std::max(nmax, 1);
       }
       argsA2.N = argsA.N;
+      // The delta forms pay while the batch is wide; the narrow tail is latency-bound either way and its slow
+      // columns converge in fewer iterations on exact contractions, so it runs all-FP64 (the live set only
+      // shrinks within a round, and every round starts with an exact iteration).
+      const bool dz_on = delta && ntot > DELTA_MIN_LIVE, df_on = delta_f && ntot > DELTA_MIN_LIVE;
       for (int k = 0; k < check_every; ++k) {
         // FP64 GEMM-B: always without the delta form; with it, on the first iteration of a round (no zeta yet)
         // and on the last iteration of every batch, whose exact rho carries the stop test before the compaction
-        const bool exact_it = !delta || (batch == 0 && k == 0) || k == check_every - 1;
+        const bool exact_it = !dz_on || (batch == 0 && k == 0) || k == check_every - 1;
         // sampled launches: right after a compaction every slot is live, so the counted flops are all useful; the
         // delta form has its FP64 GEMM-B on the last iteration of the batch instead
         const bool sample = opts->profile && k == (delta ? check_every - 1 : 0);
         if (sample) TKM_CUDA(cudaEventRecord(ev.pev[ring][0], st));
         int nblkA = (int)ceil_div(n, tileA.BM);
-        if (delta_f && !exact_it) {
+        if (df_on && !exact_it) {
           // F half: F+ = Fbar - U Lam da on the tcgen05 tensor cores, loss derivative in its epilogue
           FLossEpi fe{(const double*)y, d_fold.as<int32_t>(), col_of_slot.as<int32_t>(), bbar.as<double>(),
                       mu.as<double>(), p0->col_nc.as<double>(), p0->col_tau.as<double>(), p0->col_v.as<int32_t>(), B,
@@ -1035,10 +1040,10 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
         } else {
           LossEpi le{(const double*)y, d_fold.as<int32_t>(), col_of_slot.as<int32_t>(), bbar.as<double>(),
                      p0->col_nc.as<double>(), p0->col_tau.as<double>(), p0->col_v.as<int32_t>(), B, (int)loss, smooth,
-                     Zt.as<double>(), ldn, gpart.as<double>(), ldpart, delta ? dz_hi.as<float>() : nullptr,
-                     delta ? dz_lo.as<float>() : nullptr, ldn32, delta_f ? Fb.as<double>() : nullptr};
+                     Zt.as<double>(), ldn, gpart.as<double>(), ldpart, dz_on ? dz_hi.as<float>() : nullptr,
+                     dz_on ? dz_lo.as<float>() : nullptr, ldn32, df_on ? Fb.as<double>() : nullptr};
           TKM_TRY(gemm_f64_launch(argsA, tileA, G, le, st));
-          if (delta_f) {   // exact iteration of the F half: also F = U Lam a, so that both recurrence states are exact
+          if (df_on) {   // exact iteration of the F half: also F = U Lam a, so that both recurrence states are exact
             StoreEpi fs{Fp.as<double>(), ldn, (int64_t)B * ldn, 1.0};
             TKM_TRY(gemm_f64_launch(argsA2, tileA, G, fs, st));
           }
@@ -1047,7 +1052,7 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
         if (exact_it) {
           // FP64 contraction; in delta form it also re-establishes zeta = U^T z exactly
           SpecEpi se{col_of_slot.as<int32_t>(), p0->col_lam.as<double>(), B, Abar.as<double>(), ldr, Rho.as<double>(),
-                     delta ? Zeta.as<double>() : nullptr};
+                     dz_on ? Zeta.as<double>() : nullptr};
           TKM_TRY(gemm_f64_launch(argsB, tileB, G, se, st));
         } else {
           ZetaEpi ze{col_of_slot.as<int32_t>(), p0->col_lam.as<double>(), B, Abar.as<double>(), ldr, Zeta.as<double>(),
@@ -1061,18 +1066,18 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
                       Rho.as<double>(), A.as<double>(), Aprev.as<double>(),
                       Abar.as<double>(), beta.as<double>(), beta_prev.as<double>(), bbar.as<double>(), rk.as<double>(),
                       kkt.as<double>(), done.as<int32_t>(), iters.as<int32_t>(), iters_round.as<int32_t>(),
-                      flags.as<int32_t>(), delta_f ? da_hi.as<float>() : nullptr, delta_f ? da_lo.as<float>() : nullptr,
-                      ldr32, delta_f ? mu.as<double>() : nullptr};
+                      flags.as<int32_t>(), df_on ? da_hi.as<float>() : nullptr, df_on ? da_lo.as<float>() : nullptr,
+                      ldr32, df_on ? mu.as<double>() : nullptr};
         update_kernel<<<dim3(std::max(nmax, 1), G), 256, 0, st>>>(ua);
         TKM_LAUNCH_CHECK();
       }
       // compaction on the device; the new counts travel back asynchronously
       CompactArgs ca{B, (int)r, ldr, gp, nslots.as<int32_t>(), col_of_slot.as<int32_t>(), done.as<int32_t>(),
                      fin_list.as<int32_t>(), tail_list.as<int32_t>(), counts.as<int32_t>(), A.as<double>(),
-                     Aprev.as<double>(), Abar.as<double>(), delta ? Zeta.as<double>() : nullptr,
-                     delta ? Zt.as<double>() : nullptr, ldn, (int)n, delta_f ? Fb.as<double>() : nullptr,
-                     delta_f ? Fp.as<double>() : nullptr, delta_f ? da_hi.as<float>() : nullptr,
-                     delta_f ? da_lo.as<float>() : nullptr, ldr32};
+                     Aprev.as<double>(), Abar.as<double>(), dz_on ? Zeta.as<double>() : nullptr,
+                     dz_on ? Zt.as<double>() : nullptr, ldn, (int)n, df_on ? Fb.as<double>() : nullptr,
+                     df_on ? Fp.as<double>() : nullptr, df_on ? da_hi.as<float>() : nullptr,
+                     df_on ? da_lo.as<float>() : nullptr, ldr32};
       compact_plan_kernel<<<G, 1024, 0, st>>>(ca);
       TKM_LAUNCH_CHECK();
       compact_apply_kernel<<<dim3(std::max(nmax, 1), G), 256, 0, st>>>(ca);
