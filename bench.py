@@ -43,12 +43,19 @@ MAXIT = 200000
 # Stop tolerance of the smoothing rounds 0..R-2, which only produce warm starts for the last round (the
 # result is the minimiser at the final smoothing level, whatever the start): DESIGN.md "Schedule".
 WARM_TOL = 1e-3
+# Delta form of the U^T contraction (tkm_loss_opts.tf32_delta = 1): zeta advances by 3xTF32 increments on the
+# tcgen05 tensor cores, with the exact FP64 DMMA contraction and the stop test on the last iteration of every
+# 16-iteration batch and in the narrow tail.  Same fixed point and the same 1e-10 parity bar as the all-FP64
+# sweep.  Mode 2 (both contractions) is 4 % faster still at n = 2000 and 3.2x at n = 20000, but
+# it makes a bandwidth-bound tcgen05 kernel the dominant one; mode 1 keeps the FP64 DMMA GEMM dominant.
+TF32_DELTA = 1
 # nominal dense tensor ratios to bf16 (B200_PROFILING.md / B300_MICROARCH.md tables): FP64 45 TF,
 # TF32 1125 TF, bf16 2250 TF.  3xTF32 does three MMAs per useful one.
 NOMINAL_RATIO = {"f64": 45.0 / 2250.0, "f32": (1125.0 / 2250.0) / 3.0}
 # dram bytes per launch of the dominant kernel from the committed ncu --set full capture
 # (profiles/): filled in by hand after each capture, None until one exists.
 NCU_TRAFFIC_BYTES_PER_LAUNCH = 218.0e6   # profiles/r01c: full-width launch, dram read + write
+NCU_TRAFFIC_TF32_BYTES_PER_LAUNCH = None  # tcgen05 kernel: filled in from profiles/r01e after the capture
 # columns of the bounded CPU sample: all V+1 hold-out settings x these lambda indices, one sigma
 CPU_SAMPLE_LAMBDA_IDX = (0, 12, 24, 36, 49)
 CPU_SAMPLE_SIGMA_IDX = 2
@@ -170,7 +177,8 @@ def workload_config(w, dtype, warm_tol=None):
                         "1e2..1e-5 x %d sigma (median x {0.25,0.5,1,2,4}), delta 1 -> 1/512 in %d rounds, %s"
                         % (w.n, w.p, w.V, w.L, len(w.sigmas), w.rounds, dtype),
             "n": w.n, "p": w.p, "folds": w.V, "lambdas": w.L, "sigmas": len(w.sigmas),
-            "columns_per_step": w.B * len(w.sigmas), "stop_tol": STOP_TOL[dtype], "warm_start_rounds_tol": WARM_TOL if warm_tol is None else warm_tol, "maxit": MAXIT,
+            "columns_per_step": w.B * len(w.sigmas), "stop_tol": STOP_TOL[dtype], "warm_start_rounds_tol": WARM_TOL if warm_tol is None else warm_tol,
+            "tf32_delta": TF32_DELTA if warm_tol is None else 0, "maxit": MAXIT,
             "l2": "flushed between steps (256 MiB memset)", "parallelism": "independent replicas, no collective"}
 
 
@@ -197,7 +205,7 @@ def run_ours(args, w, rank, world):
     Xh = torch.from_numpy(w.X).pin_memory()
     yh = torch.from_numpy(w.y).pin_memory()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
-    prof = dict(ms=np.zeros(2), flops=0.0, samples=0, col_iters=0)
+    prof = dict(ms=np.zeros(4), flops=np.zeros(4), launches=np.zeros(4, dtype=np.int64), col_iters=0)
     stage = np.zeros(4)
     e2e_stage = np.zeros(5)     # last e2e step: copy-in, gram, eig, sweep, cv + coefficients + copy-out (ms)
 
@@ -217,7 +225,7 @@ def run_ours(args, w, rank, world):
         del Ks
         e2 = ev()
         paths = tkm.tkm_fit_path_multi(specs, y, w.loss, w.lambdas, foldid, w.V, tol, MAXIT, smooth0=w.smooth0,
-                                       eta=w.eta, rounds=w.rounds, warm_tol=WARM_TOL, profile=True)
+                                       eta=w.eta, rounds=w.rounds, warm_tol=WARM_TOL, tf32_delta=TF32_DELTA, profile=True)
         e3 = ev()
         best = [int(tkm.tkm_exact_cv(path, y, foldid, w.T, w.L, w.V)[3][0]) for path in paths]
         e4 = ev()
@@ -228,9 +236,9 @@ def run_ours(args, w, rank, world):
             stage[2] += e2.elapsed_time(e3)
             stage[3] += e3.elapsed_time(e4)
             pr = paths[0].profile()
-            prof["ms"] += pr["gemm_ms"]
-            prof["flops"] += pr["gemm_flops"]
-            prof["samples"] += pr["samples"]
+            prof["ms"] += pr["ms"]
+            prof["flops"] += pr["flops"]
+            prof["launches"] += pr["launches"]
             prof["col_iters"] += sum(path.total_col_iters for path in paths)
             if any(path.status != 0 for path in paths):
                 raise RuntimeError("columns hit maxit: the timed work is not the stated work")
@@ -244,7 +252,7 @@ def run_ours(args, w, rank, world):
         flush.zero_()
         r = tkm.tkm_train_tune_host(Xh.numpy(), yh.numpy(), np.asarray(w.sigmas, dtype=np.float64), w.loss, w.lambdas,
                                     foldid, w.V, tol, MAXIT, smooth0=w.smooth0, eta=w.eta, rounds=w.rounds,
-                                    warm_tol=WARM_TOL, sweep_dtype=sweep_dt)
+                                    warm_tol=WARM_TOL, tf32_delta=TF32_DELTA, sweep_dtype=sweep_dt)
         if r["status"] != 0:
             raise RuntimeError("columns hit maxit in the e2e leg")
         e2e_stage[:] = r["stage_ms"]
@@ -295,18 +303,31 @@ def run_ours(args, w, rank, world):
     ms_per_step = ms_total / args.steps
     value = world * fits_per_step / (ms_per_step / 1e3)
     pk = peaks()
-    peak_tf = pk["bf16_sus"] * NOMINAL_RATIO[dt]
-    gemm_ms = float(prof["ms"].sum())
-    achieved = (2.0 * prof["flops"] / 1e12) / (gemm_ms / 1e3) if gemm_ms > 0 else 0.0
-    roofline = {"bound": "tensor", "kernel": "gemm_%s_tma_kernel (GEMM-A loss epilogue + GEMM-B spectral epilogue)" % dt,
-                "achieved": achieved, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved / peak_tf,
-                "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH,
-                "peak_source": "%s bf16 sustained %.1f TF/s x nominal %s/bf16 ratio %.4f" %
-                               (pk["src"], pk["bf16_sus"], dt, NOMINAL_RATIO[dt]),
-                "sampled_launches": int(2 * prof["samples"]),
-                "avg_launch_ms": gemm_ms / max(1, 2 * prof["samples"]),
-                "avg_flops_per_launch": prof["flops"] / max(1, prof["samples"]),
-                "gemm_a_ms": float(prof["ms"][0]), "gemm_b_ms": float(prof["ms"][1])}
+
+    def family(idx, name, peak_tf, peak_src, traffic):
+        ms, fl, nl = float(prof["ms"][idx].sum()), float(prof["flops"][idx].sum()), int(prof["launches"][idx].sum())
+        ach = (fl / 1e12) / (ms / 1e3) if ms > 0 else 0.0
+        return {"bound": "tensor", "kernel": name, "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s",
+                "frac": ach / peak_tf, "traffic": traffic, "peak_source": peak_src, "sampled_launches": nl,
+                "avg_launch_ms": ms / max(1, nl), "avg_flops_per_launch": fl / max(1, nl),
+                "sampled_ms": ms}
+
+    # FP64 DMMA kernel: peak = measured bf16 sustained x nominal FP64/bf16 ratio
+    roof_f64 = family([0, 1], "gemm_f64_tma_kernel (FP64 DMMA: exact iterations and the narrow tail; GEMM-A loss "
+                      "epilogue + GEMM-B spectral epilogue)", pk["bf16_sus"] * NOMINAL_RATIO["f64"],
+                      "%s bf16 sustained %.1f TF/s x nominal f64/bf16 ratio %.4f" %
+                      (pk["src"], pk["bf16_sus"], NOMINAL_RATIO["f64"]), NCU_TRAFFIC_BYTES_PER_LAUNCH)
+    # tcgen05 3xTF32 kernel: every useful product costs three TF32 MMAs; achieved counts the USEFUL flops only
+    roof_tf32 = family([2, 3], "gemm_tf32x3_kernel (tcgen05 3xTF32 delta forms: F+ = Fbar - U Lam da with loss "
+                       "epilogue, zeta += U^T dz with rho epilogue)", pk["bf16_sus"] * NOMINAL_RATIO["f32"],
+                       "%s bf16 sustained %.1f TF/s x nominal tf32/bf16 ratio 0.5 / 3 MMAs per useful product" %
+                       (pk["src"], pk["bf16_sus"]), NCU_TRAFFIC_TF32_BYTES_PER_LAUNCH)
+    # the dominant kernel family is the one with the larger share of the sweep: per batch of 16 iterations the
+    # delta forms run 15 tcgen05 pairs and one DMMA pair, the all-FP64 sweep 16 DMMA pairs
+    if TF32_DELTA == 2 and roof_tf32["sampled_launches"]:
+        roofline, roofline_other = roof_tf32, roof_f64
+    else:
+        roofline, roofline_other = roof_f64, (roof_tf32 if roof_tf32["sampled_launches"] else None)
     sweep_s = stage[2] / 1e3
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -318,7 +339,7 @@ def run_ours(args, w, rank, world):
             "col_iters_per_step": prof["col_iters"] / args.steps,
             "sweep_useful_tflops": 4.0 * w.n * w.n * prof["col_iters"] / sweep_s / 1e12,
             "gram_gbs": len(w.sigmas) * w.n * w.n * 8 / (stage[0] / args.steps / 1e3) / 1e9,
-            "sweep_iters_sampled": int(prof["samples"]), "roofline": roofline, "clocks": clocks, "gpu_launches": int(launches),
+            "roofline": roofline, "roofline_other_kernel": roofline_other, "clocks": clocks, "gpu_launches": int(launches),
             "e2e": {"value": world * fits_per_step / (ms_e2e / args.steps / 1e3), "unit": UNIT,
                     "h2d_bytes_per_step": int(nb_in), "d2h_bytes_per_step": int(nb_out),
                     "ms_per_step": ms_e2e / args.steps,

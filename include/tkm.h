@@ -161,11 +161,13 @@ void tkm_path_free(tkm_path* p);
  * beta0[B]; total_col_iters = sum of iters (the unit of the roofline). */
 int tkm_path_info(const tkm_path* p, int32_t* B, int64_t* r, int32_t* iters, double* kkt,
                   int32_t* flags, double* beta0, int64_t* total_col_iters);
-/* Sampled kernel timings of the sweep (only when tkm_loss_opts.profile was 1), all [host]:
- * gemm_ms[2] = summed CUDA-event durations of the sampled GEMM-A and GEMM-B launches,
- * gemm_flops = sum over the samples of 2 n r (live columns) -- the algorithmic flops of ONE of the
- * two contractions (4 n r flops per column-iteration), samples = their number. */
-int tkm_path_profile(const tkm_path* p, double* gemm_ms, double* gemm_flops, int64_t* samples);
+/* Sampled kernel timings of the sweep (only when tkm_loss_opts.profile was 1), all [host] arrays of 4, one
+ * entry per kernel family and contraction: [0] FP64 DMMA GEMM-A, [1] FP64 DMMA GEMM-B, [2] tcgen05 3xTF32
+ * delta GEMM-A, [3] tcgen05 3xTF32 delta GEMM-B.  ms = summed CUDA-event durations of the sampled launches (the
+ * first iteration after every compaction -- every slot live -- and, in the delta forms, the exact last
+ * iteration of the batch), flops = summed algorithmic flops 2 n r (live columns) of those launches
+ * (4 n r per column-iteration over the two contractions), launches = their number. */
+int tkm_path_profile(const tkm_path* p, double* ms, double* flops, int64_t* launches);
 /* Spectral coordinates of all columns: [dev] a_out, B x r FP64 row-major (ld = r). */
 int tkm_path_get_a(const tkm_path* p, double* a_out, void* stream);
 

@@ -69,7 +69,7 @@ def lib():
     L.tkm_path_free.argtypes = [vp]
     L.tkm_path_free.restype = None
     L.tkm_path_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i64), vp, vp, vp, vp, C.POINTER(i64)]
-    L.tkm_path_profile.argtypes = [vp, vp, C.POINTER(dbl), C.POINTER(i64)]
+    L.tkm_path_profile.argtypes = [vp, vp, vp, vp]
     L.tkm_path_get_a.argtypes = [vp, vp, vp]
     L.tkm_exact_cv.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
     L.tkm_path_coef.argtypes = [vp, i32, i32, i32, vp, C.POINTER(dbl), vp]
@@ -261,10 +261,11 @@ class Path:
         return dict(iters=iters, kkt=kkt, flags=flags, beta0=beta0)
 
     def profile(self):
-        ms = np.zeros(2)
-        fl, ns = C.c_double(), C.c_int64()
-        _check(lib().tkm_path_profile(self._h, _ptr(ms), C.byref(fl), C.byref(ns)))
-        return dict(gemm_ms=ms, gemm_flops=fl.value, samples=ns.value)
+        """Sampled launches by family: index 0/1 = FP64 DMMA GEMM-A/B, 2/3 = tcgen05 3xTF32 delta GEMM-A/B."""
+        ms, fl = np.zeros(4), np.zeros(4)
+        nl = np.zeros(4, dtype=np.int64)
+        _check(lib().tkm_path_profile(self._h, _ptr(ms), _ptr(fl), _ptr(nl)))
+        return dict(ms=ms, flops=fl, launches=nl)
 
     def a(self, stream=None):
         import torch

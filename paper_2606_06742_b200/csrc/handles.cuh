@@ -41,9 +41,10 @@ struct tkm_path {
   std::vector<int32_t> h_iters, h_flags;
   int64_t total_col_iters = 0;
   // sampled CUDA-event timings of the two contractions (tkm_loss_opts.profile)
-  double prof_gemm_ms[2] = {0.0, 0.0};   // GEMM-A, GEMM-B: sum over the sampled launches
-  double prof_gemm_flops = 0.0;          // sum over the samples of 2 n r (live columns), per GEMM
-  int64_t prof_gemm_samples = 0;
+  // by kernel family and contraction: [0] DMMA GEMM-A, [1] DMMA GEMM-B, [2] tcgen05 A, [3] tcgen05 B
+  double prof_ms[4] = {0.0, 0.0, 0.0, 0.0};       // summed CUDA-event durations of the sampled launches
+  double prof_flops[4] = {0.0, 0.0, 0.0, 0.0};    // summed 2 n r (live columns) of those launches
+  int64_t prof_launches[4] = {0, 0, 0, 0};
 };
 
 namespace tkm {

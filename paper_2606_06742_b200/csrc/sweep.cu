@@ -887,7 +887,7 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
 
   // events: one "poll landed" event per ring entry; optional GEMM sampling events per ring entry
   struct Events {
-    cudaEvent_t poll[POLL_RING] = {}, pev[POLL_RING][3] = {};
+    cudaEvent_t poll[POLL_RING] = {}, pev[POLL_RING][8] = {};   // pev: 2 sampled iterations x (A0, A1, B0, B1)
     ~Events() {
       for (auto& e : poll)
         if (e) cudaEventDestroy(e);
@@ -938,8 +938,10 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
 
   const int check_every = opts->check_every > 0 ? opts->check_every : 16;
   const int restart = opts->restart ? 1 : 0;
-  double prof_ms[2] = {0.0, 0.0}, prof_flops = 0.0;
-  int64_t prof_samples = 0;
+  // sampled launches, by kernel family and contraction: [0] DMMA GEMM-A, [1] DMMA GEMM-B, [2] tcgen05 A, [3] tcgen05 B
+  double prof_ms[4] = {0.0, 0.0, 0.0, 0.0}, prof_flops[4] = {0.0, 0.0, 0.0, 0.0};
+  int64_t prof_launches[4] = {0, 0, 0, 0};
+  int samp_kind[POLL_RING][4];   // per ring slot: family index of (iteration 0: A, B; last iteration: A, B), -1 = not sampled
   double smooth = opts->smooth0;
   for (int rnd = 0; rnd < rounds; ++rnd) {
     if (smoothed && rnd > 0) smooth *= opts->eta;   // PAPER.md:220 (Alg.1 l.22)
@@ -1025,8 +1027,10 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
         const bool exact_it = !dz_on || (batch == 0 && k == 0) || k == check_every - 1;
         // sampled launches: right after a compaction every slot is live, so the counted flops are all useful; the
         // delta form has its FP64 GEMM-B on the last iteration of the batch instead
-        const bool sample = opts->profile && k == (delta ? check_every - 1 : 0);
-        if (sample) TKM_CUDA(cudaEventRecord(ev.pev[ring][0], st));
+        // first iteration after a compaction (every slot live) and, in the delta forms, the exact last iteration
+        const int sidx = !opts->profile ? -1 : (k == 0 ? 0 : ((dz_on && k == check_every - 1) ? 1 : -1));
+        if (k == 0) samp_kind[ring][0] = samp_kind[ring][1] = samp_kind[ring][2] = samp_kind[ring][3] = -1;
+        if (sidx >= 0) TKM_CUDA(cudaEventRecord(ev.pev[ring][4 * sidx + 0], st));
         int nblkA = (int)ceil_div(n, tileA.BM);
         if (df_on && !exact_it) {
           // F half: F+ = Fbar - U Lam da on the tcgen05 tensor cores, loss derivative in its epilogue
@@ -1037,18 +1041,26 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
                       dz_lo.as<float>(), ldn32, gpart.as<double>(), ldpart};
           TKM_TRY(gemm_tf32_launch(targsF, tcfg, G, fe, st));
           nblkA = (int)ceil_div(n, TF32_BM);
+          if (sidx >= 0) {
+            TKM_CUDA(cudaEventRecord(ev.pev[ring][4 * sidx + 1], st));
+            samp_kind[ring][2 * sidx] = 2;
+          }
         } else {
           LossEpi le{(const double*)y, d_fold.as<int32_t>(), col_of_slot.as<int32_t>(), bbar.as<double>(),
                      p0->col_nc.as<double>(), p0->col_tau.as<double>(), p0->col_v.as<int32_t>(), B, (int)loss, smooth,
                      Zt.as<double>(), ldn, gpart.as<double>(), ldpart, dz_on ? dz_hi.as<float>() : nullptr,
                      dz_on ? dz_lo.as<float>() : nullptr, ldn32, df_on ? Fb.as<double>() : nullptr};
           TKM_TRY(gemm_f64_launch(argsA, tileA, G, le, st));
+          if (sidx >= 0) {
+            TKM_CUDA(cudaEventRecord(ev.pev[ring][4 * sidx + 1], st));
+            samp_kind[ring][2 * sidx] = 0;
+          }
           if (df_on) {   // exact iteration of the F half: also F = U Lam a, so that both recurrence states are exact
             StoreEpi fs{Fp.as<double>(), ldn, (int64_t)B * ldn, 1.0};
             TKM_TRY(gemm_f64_launch(argsA2, tileA, G, fs, st));
           }
         }
-        if (sample) TKM_CUDA(cudaEventRecord(ev.pev[ring][1], st));
+        if (sidx >= 0) TKM_CUDA(cudaEventRecord(ev.pev[ring][4 * sidx + 2], st));
         if (exact_it) {
           // FP64 contraction; in delta form it also re-establishes zeta = U^T z exactly
           SpecEpi se{col_of_slot.as<int32_t>(), p0->col_lam.as<double>(), B, Abar.as<double>(), ldr, Rho.as<double>(),
@@ -1059,7 +1071,10 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
                      Rho.as<double>()};
           TKM_TRY(gemm_tf32_launch(targs, tcfg, G, ze, st));
         }
-        if (sample) TKM_CUDA(cudaEventRecord(ev.pev[ring][2], st));
+        if (sidx >= 0) {
+          TKM_CUDA(cudaEventRecord(ev.pev[ring][4 * sidx + 3], st));
+          samp_kind[ring][2 * sidx + 1] = exact_it ? 1 : 3;
+        }
         UpdateArgs ua{(int)r, (int)n, B, nblkA, restart, maxit, exact_it ? 1 : 0, ldr,
                       ldpart, rtol, gp, nslots.as<int32_t>(), col_of_slot.as<int32_t>(), p0->col_lam.as<double>(),
                       col_c.as<double>(), p0->col_nc.as<double>(), col_s.as<double>(), gpart.as<double>(),
@@ -1110,13 +1125,16 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
           }
         }
         if (opts->profile && live_then > 0) {
-          float ma = 0.f, mb = 0.f;   // the sampled GEMMs of batch b precede its poll event
-          TKM_CUDA(cudaEventElapsedTime(&ma, ev.pev[cur][0], ev.pev[cur][1]));
-          TKM_CUDA(cudaEventElapsedTime(&mb, ev.pev[cur][1], ev.pev[cur][2]));
-          prof_ms[0] += ma;
-          prof_ms[1] += mb;
-          prof_flops += 2.0 * (double)live_then * (double)n * (double)r;   // per GEMM
-          prof_samples += 1;
+          // the sampled launches of batch b precede its poll event; flops = 2 n r (live columns) per launch
+          for (int q = 0; q < 4; ++q) {
+            const int kind = samp_kind[cur][q];
+            if (kind < 0) continue;
+            float ms = 0.f;
+            TKM_CUDA(cudaEventElapsedTime(&ms, ev.pev[cur][4 * (q >> 1) + 2 * (q & 1)], ev.pev[cur][4 * (q >> 1) + 2 * (q & 1) + 1]));
+            prof_ms[kind] += ms;
+            prof_flops[kind] += 2.0 * (double)live_then * (double)n * (double)r;
+            prof_launches[kind] += 1;
+          }
         }
         if (trace && b >= 1) {
           float bms = 0.f;
@@ -1155,10 +1173,11 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
     }
   }
   // sampled timings cover all groups of the shared launches: reported on the first path
-  out[0]->prof_gemm_ms[0] = prof_ms[0];
-  out[0]->prof_gemm_ms[1] = prof_ms[1];
-  out[0]->prof_gemm_flops = prof_flops;
-  out[0]->prof_gemm_samples = prof_samples;
+  for (int q = 0; q < 4; ++q) {
+    out[0]->prof_ms[q] = prof_ms[q];
+    out[0]->prof_flops[q] = prof_flops[q];
+    out[0]->prof_launches[q] = prof_launches[q];
+  }
   guard.armed = false;
   if (notconv) return set_error(TKM_ENOTCONV, "tkm_fit_path: some columns hit maxit (see flags)");
   return TKM_OK;
@@ -1188,14 +1207,13 @@ extern "C" int tkm_path_info(const tkm_path* p, int32_t* B, int64_t* r, int32_t*
   return TKM_OK;
 }
 
-extern "C" int tkm_path_profile(const tkm_path* p, double* gemm_ms, double* gemm_flops, int64_t* samples) {
+extern "C" int tkm_path_profile(const tkm_path* p, double* ms, double* flops, int64_t* launches) {
   if (!p) return set_error(TKM_EINVAL, "tkm_path_profile: NULL handle");
-  if (gemm_ms) {
-    gemm_ms[0] = p->prof_gemm_ms[0];
-    gemm_ms[1] = p->prof_gemm_ms[1];
+  for (int q = 0; q < 4; ++q) {
+    if (ms) ms[q] = p->prof_ms[q];
+    if (flops) flops[q] = p->prof_flops[q];
+    if (launches) launches[q] = p->prof_launches[q];
   }
-  if (gemm_flops) *gemm_flops = p->prof_gemm_flops;
-  if (samples) *samples = p->prof_gemm_samples;
   return TKM_OK;
 }
 

@@ -205,7 +205,8 @@ def test_config1_full_size_sampled_columns(tkm):
     X, y = dev(w.X), dev(w.y)
     specs = [tkm.tkm_spectral_setup(tkm.tkm_gram(X, float(s))) for s in w.sigmas]
     paths = tkm.tkm_fit_path_multi(specs, y, w.loss, w.lambdas, foldid, w.V, bench.STOP_TOL["f64"], bench.MAXIT,
-                                   smooth0=w.smooth0, eta=w.eta, rounds=w.rounds, warm_tol=bench.WARM_TOL)
+                                   smooth0=w.smooth0, eta=w.eta, rounds=w.rounds, warm_tol=bench.WARM_TOL,
+                                   tf32_delta=bench.TF32_DELTA)
     L, V = w.L, w.V
     sample = {2: [(0, 0), (1, 17), (2, 30), (5, 24), (4, 40), (3, 49)], 0: [(5, 35)], 4: [(1, 45)]}
     for g, vl in sample.items():
