@@ -55,7 +55,7 @@ NOMINAL_RATIO = {"f64": 45.0 / 2250.0, "f32": (1125.0 / 2250.0) / 3.0}
 # dram bytes per launch of the dominant kernel from the committed ncu --set full capture
 # (profiles/): filled in by hand after each capture, None until one exists.
 NCU_TRAFFIC_BYTES_PER_LAUNCH = 218.0e6   # profiles/r01c: full-width launch, dram read + write
-NCU_TRAFFIC_TF32_BYTES_PER_LAUNCH = None  # tcgen05 kernel: filled in from profiles/r01e after the capture
+NCU_TRAFFIC_TF32_BYTES_PER_LAUNCH = 271.0e6  # profiles/r01e: tcgen05 ZetaEpi kernel, full-width launch
 # columns of the bounded CPU sample: all V+1 hold-out settings x these lambda indices, one sigma
 CPU_SAMPLE_LAMBDA_IDX = (0, 12, 24, 36, 49)
 CPU_SAMPLE_SIGMA_IDX = 2
