@@ -181,6 +181,13 @@ int tkm_path_get_a(const tkm_path* p, double* a_out, void* stream);
 int tkm_exact_cv(const tkm_path* p, const void* y, const int32_t* foldid,
                  double* cv_loss, int64_t* cv_err, double* cv_mean, int32_t* best_l, void* stream);
 
+/* tkm_cv_select: the selection step of tkm_exact_cv on its own (lambda columns sharded
+ * over GPUs, the T x L x V loss table gathered before the argmin).  cv_loss [host] T x L x V fold means,
+ * fold_sizes [host] V (> 0), lambdas [host] L; writes [host] cv_mean T x L (pooled over folds, weights
+ * fold_sizes / n) and best_l T (argmin, ties -> largest lambda, reading G14).  Synchronises `stream`. */
+int tkm_cv_select(const double* cv_loss, const double* fold_sizes, const double* lambdas, int32_t T,
+                  int32_t L, int32_t V, double* cv_mean, int32_t* best_l, void* stream);
+
 /* ---- S10 coefficients and prediction (readings G11, G15) --------------------
  * tkm_path_coef: alpha = U a of column (t, l, v) into [dev] alpha (n FP64; Nystrom: the m landmark
  * weights gamma), and beta0 into [host] *beta0.  Synchronises `stream`. */

@@ -13,7 +13,7 @@ TKM_OK, TKM_ENOTCONV = 0, 5
 
 EXPORTED_SYMBOLS = [
     "tkm_gram", "tkm_gram_multi", "tkm_spectral_setup", "tkm_spectral_setup_multi", "tkm_spectral_free", "tkm_spectral_info", "tkm_spectral_get_u",
-    "tkm_fit_path", "tkm_fit_path_multi", "tkm_path_free", "tkm_path_info", "tkm_path_profile", "tkm_path_get_a", "tkm_exact_cv", "tkm_path_coef",
+    "tkm_fit_path", "tkm_fit_path_multi", "tkm_path_free", "tkm_path_info", "tkm_path_profile", "tkm_path_get_a", "tkm_exact_cv", "tkm_cv_select", "tkm_path_coef",
     "tkm_predict", "tkm_cv_decision_values", "tkm_platt_fit", "tkm_platt_proba", "tkm_train_tune_host", "tkm_make_folds", "tkm_launch_count", "tkm_launch_count_reset",
     "tkm_dgemm_nt", "tkm_gemm_probe", "tkm_tf32x3_gemm_nt", "tkm_version", "tkm_last_error",
 ]
@@ -72,6 +72,7 @@ def lib():
     L.tkm_path_profile.argtypes = [vp, vp, vp, vp]
     L.tkm_path_get_a.argtypes = [vp, vp, vp]
     L.tkm_exact_cv.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
+    L.tkm_cv_select.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp, vp]
     L.tkm_path_coef.argtypes = [vp, i32, i32, i32, vp, C.POINTER(dbl), vp]
     L.tkm_predict.argtypes = [vp, i32, i32, vp, i64, vp, i64, i64, i64, dbl, vp, vp, vp]
     L.tkm_cv_decision_values.argtypes = [vp, i32, i32, vp, vp, vp]
@@ -336,6 +337,44 @@ def tkm_exact_cv(path: Path, y, foldid, T: int, L: int, V: int, stream=None):
     _check(lib().tkm_exact_cv(path._h, y.data_ptr(), _ptr(fid), _ptr(cv_loss), _ptr(cv_err), _ptr(cv_mean),
                               _ptr(best), _stream(stream)))
     return cv_loss, cv_err, cv_mean, best
+
+
+def tkm_cv_select(cv_loss, fold_sizes, lambdas, stream=None):
+    """Pooled CV mean and selected lambda from a T x L x V fold-loss table (host arrays)."""
+    cv_loss = _host(cv_loss, np.float64)
+    T, L, V = cv_loss.shape
+    fs = _host(fold_sizes, np.float64)
+    lam = _host(lambdas, np.float64)
+    assert fs.shape == (V,) and lam.shape == (L,)
+    cv_mean = np.empty((T, L))
+    best = np.empty(T, dtype=np.int32)
+    _check(lib().tkm_cv_select(_ptr(cv_loss), _ptr(fs), _ptr(lam), T, L, V, _ptr(cv_mean), _ptr(best),
+                               _stream(stream)))
+    return cv_mean, best
+
+
+def tkm_fit_cv_sharded(spec: Spectral, y, loss: int, lambdas, foldid, V: int, tol: float, maxit: int, dist=None,
+                       rank=None, world=None, taus=None, stream=None, **fit_kw):
+    """Column sharding over GPUs: this rank fits the lambdas `ranks.lambda_slice` gives it
+    (interleaved: the iteration count grows as lambda falls) for every fold and variant, runs exact CV on
+    its own columns, the ranks exchange the fold-loss tables (kilobytes; the only communication), and every
+    rank selects lambda from the full table.  Returns (path of this rank's lambdas, their indices in
+    `lambdas`, cv_loss, cv_err, cv_mean, best) with the tables in the full grid's order."""
+    from . import ranks
+    if rank is None:
+        rank = dist.get_rank() if dist is not None and dist.is_initialized() else 0
+    if world is None:
+        world = dist.get_world_size() if dist is not None and dist.is_initialized() else 1
+    lam = _host(lambdas, np.float64)
+    mine = ranks.lambda_slice(len(lam), rank, world)
+    T = len(taus) if taus is not None and len(taus) else 1
+    path = tkm_fit_path(spec, y, loss, lam[mine], foldid, V, tol, maxit, taus=taus, stream=stream, **fit_kw)
+    loc_loss, loc_err, _, _ = tkm_exact_cv(path, y, foldid, T, len(mine), V, stream=stream)
+    cv_loss = ranks.gather_lambda_tables(loc_loss, len(lam), rank, world, dist)
+    cv_err = ranks.gather_lambda_tables(loc_err, len(lam), rank, world, dist)
+    fsize = np.bincount(_host(foldid, np.int32), minlength=V).astype(np.float64)
+    cv_mean, best = tkm_cv_select(cv_loss, fsize, lam, stream=stream)
+    return path, mine, cv_loss, cv_err, cv_mean, best
 
 
 def tkm_path_coef(path: Path, t: int, l: int, v: int, stream=None):

@@ -255,6 +255,38 @@ extern "C" int tkm_exact_cv(const tkm_path* p, const void* y, const int32_t* fol
   return TKM_OK;
 }
 
+// Pooled mean and selected lambda from a (gathered) fold-loss table: the last step of S9 on its own, for a
+// lambda grid whose columns were fitted on several GPUs.  All arguments [host].
+extern "C" int tkm_cv_select(const double* cv_loss, const double* fold_sizes, const double* lambdas, int32_t T,
+                             int32_t L, int32_t V, double* cv_mean, int32_t* best_l, void* stream) {
+  if (!cv_loss || !fold_sizes || !lambdas || !cv_mean || !best_l || T < 1 || L < 1 || V < 1)
+    return set_error(TKM_EINVAL, "tkm_cv_select: bad arguments");
+  TKM_TRY(device_check());
+  cudaStream_t st = (cudaStream_t)stream;
+  double n = 0.0;
+  for (int v = 0; v < V; ++v) {
+    if (!(fold_sizes[v] > 0.0)) return set_error(TKM_EINVAL, "tkm_cv_select: empty fold");
+    n += fold_sizes[v];
+  }
+  const size_t nout = (size_t)T * L * V;
+  DevBuf d_loss, d_fsize, d_lam, d_mean, d_best;
+  TKM_TRY(d_loss.alloc(nout * sizeof(double), false, st));
+  TKM_TRY(d_fsize.alloc((size_t)V * sizeof(double), false, st));
+  TKM_TRY(d_lam.alloc((size_t)L * sizeof(double), false, st));
+  TKM_TRY(d_mean.alloc((size_t)T * L * sizeof(double), false, st));
+  TKM_TRY(d_best.alloc((size_t)T * sizeof(int), false, st));
+  TKM_CUDA(cudaMemcpyAsync(d_loss.p, cv_loss, nout * sizeof(double), cudaMemcpyHostToDevice, st));
+  TKM_CUDA(cudaMemcpyAsync(d_fsize.p, fold_sizes, V * sizeof(double), cudaMemcpyHostToDevice, st));
+  TKM_CUDA(cudaMemcpyAsync(d_lam.p, lambdas, L * sizeof(double), cudaMemcpyHostToDevice, st));
+  cv_select_kernel<<<(unsigned)ceil_div(T, 32), 32, 0, st>>>(d_loss.as<double>(), T, L, V, d_fsize.as<double>(), n,
+                                                            d_lam.as<double>(), d_mean.as<double>(), d_best.as<int>());
+  TKM_LAUNCH_CHECK();
+  TKM_CUDA(cudaMemcpyAsync(cv_mean, d_mean.p, (size_t)T * L * sizeof(double), cudaMemcpyDeviceToHost, st));
+  TKM_CUDA(cudaMemcpyAsync(best_l, d_best.p, (size_t)T * sizeof(int), cudaMemcpyDeviceToHost, st));
+  TKM_CUDA(cudaStreamSynchronize(st));
+  return TKM_OK;
+}
+
 extern "C" int tkm_path_coef(const tkm_path* p, int32_t t, int32_t l, int32_t v, double* alpha, double* beta0,
                              void* stream) {
   if (!p || !alpha) return set_error(TKM_EINVAL, "tkm_path_coef: NULL argument");

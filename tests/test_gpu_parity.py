@@ -446,3 +446,48 @@ def test_delta_form_sweep_keeps_fp64_parity(tkm, name, mode):
     cv_o = o.exact_cv(spec_o, res, w.y, foldid, w.loss, w.taus)
     if not degenerate:
         assert np.max(np.abs(cv[0] - cv_o[0])) <= CV_TOL and np.array_equal(cv[3], cv_o[3])
+
+
+# ----------------------------------------------------------------- column sharding over GPUs
+def test_column_sharded_lambda_grid_matches_single_gpu_and_oracle(tkm):
+    """The lambda grid interleaved over `world` ranks (here the ranks' shares run one after another on the one
+    GPU: they never wait on each other), tables reassembled, lambda selected by tkm_cv_select: identical
+    selection, tables equal to the unsharded run's and the oracle's."""
+    from paper_2606_06742_b200 import ranks
+    w = wl.config0(n=300, p=6, L=7, V=4, seed=31)
+    sigma = float(w.sigmas[0])
+    foldid = tkm.tkm_make_folds(w.n, w.V, w.fold_seed)
+    X, y, spec, path, cv = _run_gpu(tkm, w, sigma, foldid, STOP_TOL, 400000)
+    res, spec_o, worst, degenerate = _compare_path(tkm, w, sigma, foldid, spec, path, cv)
+    cv_o = o.exact_cv(spec_o, res, w.y, foldid, w.loss, w.taus)
+    fsize = np.bincount(foldid, minlength=w.V).astype(np.float64)
+    for world in (2, 3):
+        loss_full = np.full((1, w.L, w.V), np.nan)
+        err_full = np.full((1, w.L, w.V), -7, dtype=np.int64)
+        for rank in range(world):
+            mine = ranks.lambda_slice(w.L, rank, world)
+            part = tkm.tkm_fit_path(spec, y, w.loss, w.lambdas[mine], foldid, w.V, STOP_TOL, 400000, smooth0=w.smooth0,
+                                    eta=w.eta, rounds=w.rounds)
+            assert part.info()["flags"].sum() == 0
+            l_loss, l_err, _, _ = tkm.tkm_exact_cv(part, y, foldid, 1, len(mine), w.V)
+            loss_full[:, mine], err_full[:, mine] = l_loss, l_err
+            for j, l in enumerate(mine):      # a sharded column is the same fit as the unsharded one
+                a_p, b_p = tkm.tkm_path_coef(part, 0, j, w.V)
+                a_f, b_f = tkm.tkm_path_coef(path, 0, int(l), w.V)
+                assert float((a_p - a_f).norm() / a_f.norm()) <= 2 * COEF_TOL_F64 and abs(b_p - b_f) <= 1e-9
+        cv_mean, best = tkm.tkm_cv_select(loss_full, fsize, w.lambdas)
+        assert np.max(np.abs(loss_full - cv[0])) <= 1e-9 and np.array_equal(err_full, cv[1])
+        assert np.max(np.abs(loss_full - cv_o[0])) <= CV_TOL and np.array_equal(err_full, cv_o[1])
+        assert np.array_equal(best, cv[3]) and np.array_equal(best, cv_o[3])
+        assert np.max(np.abs(cv_mean - (loss_full * fsize).sum(axis=2) / w.n)) <= 1e-14
+    # world = 1 through the driver itself
+    p1, mine, cl, ce, cm, b = tkm.tkm_fit_cv_sharded(spec, y, w.loss, w.lambdas, foldid, w.V, STOP_TOL, 400000,
+                                                     smooth0=w.smooth0, eta=w.eta, rounds=w.rounds)
+    assert mine.tolist() == list(range(w.L)) and np.array_equal(b, cv[3]) and np.array_equal(ce, cv[1])
+    assert np.max(np.abs(cl - cv[0])) <= 1e-9
+    # ties -> largest lambda (reading G14): a flat table selects index of max(lambda)
+    flat = np.ones((2, w.L, w.V))
+    _, bt = tkm.tkm_cv_select(flat, fsize, w.lambdas)
+    assert np.all(bt == int(np.argmax(w.lambdas)))
+    with pytest.raises(tkm.TkmError):
+        tkm.tkm_cv_select(flat, np.zeros(w.V), w.lambdas)
