@@ -118,6 +118,15 @@ int tkm_gram_multi(const void* X, int64_t n, int64_t p, int64_t ldx,
  * Errors: TKM_ESOLVER if cuSOLVER reports info != 0; TKM_ENOMEM. */
 int tkm_spectral_setup(const void* K, int64_t n, int64_t ldk, const tkm_nystrom* ny,
                        tkm_dtype sweep_dt, tkm_spectral** out, void* stream);
+/* Nystrom setup straight from the training matrix (n ~ 10^6 rows):
+ * X [dev] n x p FP64 (ldx >= p), RBF bandwidth sigma, landmark_idx [host] m row indices into X.  The
+ * landmark rows are gathered, K_mm is formed, and K_nm is produced by the Gram kernel and consumed
+ * block_rows rows at a time (0 = 32768), so it is never resident: beyond X the peak is one r x n array
+ * (Phi^T, overwritten block by block by U^T), the n x r array U Lam and three blocks.  Same handle, same
+ * truncations (reading G11) as tkm_spectral_setup with a tkm_nystrom.  Synchronises `stream`. */
+int tkm_spectral_setup_nystrom_x(const void* X, int64_t n, int64_t p, int64_t ldx, double sigma,
+                                 const int64_t* landmark_idx, int64_t m, int64_t block_rows,
+                                 tkm_spectral** out, void* stream);
 /* G full-kernel setups (Ks [host]: G [dev] n x n FP64 matrices with the same n, ldk) run concurrently on
  * G internal streams ordered after `stream`; out [host] G slots.  Same results as G separate calls.
  * Returns after all G decompositions have finished. */

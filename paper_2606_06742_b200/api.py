@@ -12,7 +12,7 @@ F32, F64 = 0, 1
 TKM_OK, TKM_ENOTCONV = 0, 5
 
 EXPORTED_SYMBOLS = [
-    "tkm_gram", "tkm_gram_multi", "tkm_spectral_setup", "tkm_spectral_setup_multi", "tkm_spectral_free", "tkm_spectral_info", "tkm_spectral_get_u",
+    "tkm_gram", "tkm_gram_multi", "tkm_spectral_setup", "tkm_spectral_setup_multi", "tkm_spectral_setup_nystrom_x", "tkm_spectral_free", "tkm_spectral_info", "tkm_spectral_get_u",
     "tkm_fit_path", "tkm_fit_path_multi", "tkm_path_free", "tkm_path_info", "tkm_path_profile", "tkm_path_get_a", "tkm_exact_cv", "tkm_cv_select", "tkm_path_coef",
     "tkm_predict", "tkm_cv_decision_values", "tkm_platt_fit", "tkm_platt_proba", "tkm_train_tune_host", "tkm_make_folds", "tkm_launch_count", "tkm_launch_count_reset",
     "tkm_dgemm_nt", "tkm_gemm_probe", "tkm_tf32x3_gemm_nt", "tkm_version", "tkm_last_error",
@@ -58,6 +58,7 @@ def lib():
     L.tkm_gram_multi.argtypes = [vp, i64, i64, i64, vp, i64, i64, vp, i32, C.c_int, C.POINTER(vp), i64, vp]
     L.tkm_spectral_setup.argtypes = [vp, i64, i64, C.POINTER(_Nystrom), C.c_int, C.POINTER(vp), vp]
     L.tkm_spectral_setup_multi.argtypes = [C.POINTER(vp), i32, i64, i64, C.c_int, C.POINTER(vp), vp]
+    L.tkm_spectral_setup_nystrom_x.argtypes = [vp, i64, i64, i64, dbl, vp, i64, i64, C.POINTER(vp), vp]
     L.tkm_spectral_free.argtypes = [vp]
     L.tkm_spectral_free.restype = None
     L.tkm_spectral_info.argtypes = [vp, C.POINTER(i64), C.POINTER(i64), vp, vp]
@@ -230,6 +231,16 @@ def tkm_spectral_setup(K=None, n=None, nystrom=None, sweep_dtype=F64, stream=Non
     return Spectral(h)
 
 
+def tkm_spectral_setup_nystrom_x(X, sigma: float, landmark_idx, block_rows: int = 0, stream=None) -> Spectral:
+    """Nystrom setup from the training matrix itself: K_nm is produced and consumed block_rows rows at a time."""
+    X = _dev_f64(X, "X")
+    idx = _host(landmark_idx, np.int64)
+    h = C.c_void_p()
+    _check(lib().tkm_spectral_setup_nystrom_x(X.data_ptr(), X.shape[0], X.shape[1], X.stride(0), float(sigma), _ptr(idx),
+                                              len(idx), int(block_rows), C.byref(h), _stream(stream)))
+    return Spectral(h, keepalive=(idx,))
+
+
 def tkm_spectral_setup_multi(Ks, sweep_dtype=F64, stream=None):
     """Concurrent full-kernel setups of G Gram matrices of one size -> list of G Spectral handles."""
     Ks = [_dev_f64(K, "K") for K in Ks]
@@ -286,7 +297,7 @@ class Path:
             pass
 
 
-def _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, profile=False, tf32_delta=False):
+def _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, profile=False, tf32_delta=0):
     taus_arr = _host(taus if taus is not None else [], np.float64)
     o = _LossOpts(float(smooth0), float(eta), int(rounds), int(len(taus_arr)),
                   taus_arr.ctypes.data_as(C.POINTER(C.c_double)) if len(taus_arr) else None,
@@ -296,7 +307,7 @@ def _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, prof
 
 def tkm_fit_path(spec: Spectral, y, loss: int, lambdas, foldid, V: int, tol: float, maxit: int,
                  smooth0=1.0, eta=0.125, rounds=4, taus=None, restart=True, check_every=0, warm_tol=0.0,
-                 warm: Path | None = None, profile=False, tf32_delta=False, stream=None) -> Path:
+                 warm: Path | None = None, profile=False, tf32_delta=0, stream=None) -> Path:
     y = _dev_f64(y, "y")
     lam = _host(lambdas, np.float64)
     fid = _host(foldid, np.int32)
@@ -311,7 +322,7 @@ def tkm_fit_path(spec: Spectral, y, loss: int, lambdas, foldid, V: int, tol: flo
 
 def tkm_fit_path_multi(specs, y, loss: int, lambdas, foldid, V: int, tol: float, maxit: int,
                        smooth0=1.0, eta=0.125, rounds=4, taus=None, restart=True, check_every=0, warm_tol=0.0,
-                       warm=None, profile=False, tf32_delta=False, stream=None):
+                       warm=None, profile=False, tf32_delta=0, stream=None):
     """One sweep over G spectral handles that share y, folds and the lambda grid -> list of G Paths."""
     y = _dev_f64(y, "y")
     lam = _host(lambdas, np.float64)

@@ -73,6 +73,13 @@ struct DevBuf {
     }
     return TKM_OK;
   }
+  void take(DevBuf& o) {   // move o's allocation here
+    release();
+    p = o.p;
+    bytes = o.bytes;
+    o.p = nullptr;
+    o.bytes = 0;
+  }
   template <class T>
   T* as() const { return reinterpret_cast<T*>(p); }
 };

@@ -36,7 +36,12 @@ struct GemmArgs {
   const int32_t* nslots;                // [G] device, live rows of each group; NULL => N for all
   int p_group_rows;                     // row offset between consecutive groups in P
   int N, M, K;                          // N: upper bound of the live rows (the grid covers it)
+  int ksplit;                           // <= 1: one CTA contracts all of K; S > 1: blockIdx.y = split * n_tiles + n_tile,
+                                        // split s contracts K-tiles [s KT/S, (s+1) KT/S) and the epilogue sees a partial sum
 };
+
+// K-split index of this CTA, for epilogues that store partial sums (ksplit as in GemmArgs / Tf32Args)
+__device__ __forceinline__ int gemm_split_index(int ksplit) { return ksplit > 1 ? (int)(blockIdx.y / (gridDim.y / ksplit)) : 0; }
 
 template <int TN_, int WN_, int TM_, int WM_, int STAGES_>
 struct GemmCfg {
@@ -150,10 +155,12 @@ __global__ void __launch_bounds__(Cfg::THREADS)
 
   const int grp = blockIdx.z;
   const int N = g.nslots ? min(g.nslots[grp], g.N) : g.N;
-  const int m_blk0 = blockIdx.x * BM, n_blk0 = blockIdx.y * BN;
+  const int S = max(g.ksplit, 1), ny = (int)gridDim.y / S, split = (int)blockIdx.y / ny;
+  const int m_blk0 = blockIdx.x * BM, n_blk0 = ((int)blockIdx.y - split * ny) * BN;
   if (n_blk0 >= N) return;   // the grid is sized for an upper bound of the live slots
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int KT = (g.K + TMA_BOX_K - 1) / TMA_BOX_K;
+  const int KT_all = (g.K + TMA_BOX_K - 1) / TMA_BOX_K;
+  const int kt0 = (int)((int64_t)split * KT_all / S), KT = (int)((int64_t)(split + 1) * KT_all / S) - kt0;
   uint8_t* tiles = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
 
   if (tid == 0) {
@@ -178,8 +185,8 @@ __global__ void __launch_bounds__(Cfg::THREADS)
         if (kt >= STAGES) mbar_wait(&empty_bar[s], phase);
         mbar_arrive_expect_tx(&full_bar[s], Cfg::STAGE_BYTES);
         uint8_t* ps = tiles + (size_t)s * Cfg::STAGE_BYTES;
-        tma_load_2d(ps, &g.p_map, kt * TMA_BOX_K, prow, &full_bar[s]);
-        tma_load_2d(ps + BN * GEMM_ROW_BYTES, &g.q_map[grp], kt * TMA_BOX_K, m_blk0, &full_bar[s]);
+        tma_load_2d(ps, &g.p_map, (kt0 + kt) * TMA_BOX_K, prow, &full_bar[s]);
+        tma_load_2d(ps + BN * GEMM_ROW_BYTES, &g.q_map[grp], (kt0 + kt) * TMA_BOX_K, m_blk0, &full_bar[s]);
         if (++s == STAGES) {
           s = 0;
           phase ^= 1;
@@ -335,7 +342,8 @@ int launch_gemm_f64(const GemmArgs& a, int G, const Epi& epi, cudaStream_t st) {
     TKM_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
     configured = true;
   }
-  dim3 grid((unsigned)ceil_div(a.M, Cfg::BM), (unsigned)ceil_div(std::max(a.N, 1), Cfg::BN), (unsigned)G);
+  dim3 grid((unsigned)ceil_div(a.M, Cfg::BM), (unsigned)(ceil_div(std::max(a.N, 1), Cfg::BN) * std::max(a.ksplit, 1)),
+            (unsigned)G);
   kern<<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(a, epi);
   TKM_LAUNCH_CHECK();
   return TKM_OK;

@@ -31,6 +31,7 @@ struct Tf32Args {
   const int32_t* nslots;                                   // [G] device or NULL
   int p_group_rows;
   int N, M, K;
+  int ksplit;   // as in GemmArgs: S > 1 => blockIdx.y = split * n_tiles + n_tile, K-tiles [s KT/S, (s+1) KT/S)
 };
 
 template <int BN_, int STAGES_>
@@ -55,10 +56,12 @@ __global__ void __launch_bounds__(Cfg::THREADS, 1) gemm_tf32x3_kernel(const __gr
 
   const int grp = blockIdx.z;
   const int N = g.nslots ? min(g.nslots[grp], g.N) : g.N;
-  const int m_blk0 = blockIdx.x * TF32_BM, n_blk0 = blockIdx.y * BN;
+  const int S = max(g.ksplit, 1), ny = (int)gridDim.y / S, split = (int)blockIdx.y / ny;
+  const int m_blk0 = blockIdx.x * TF32_BM, n_blk0 = ((int)blockIdx.y - split * ny) * BN;
   if (n_blk0 >= N) return;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int KT = (g.K + TF32_BK - 1) / TF32_BK;
+  const int KT_all = (g.K + TF32_BK - 1) / TF32_BK;
+  const int kt0 = (int)((int64_t)split * KT_all / S), KT = (int)((int64_t)(split + 1) * KT_all / S) - kt0;   // host: S <= KT_all
   uint8_t* tiles = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
 
   if (tid == 0) {
@@ -86,7 +89,7 @@ __global__ void __launch_bounds__(Cfg::THREADS, 1) gemm_tf32x3_kernel(const __gr
         if (kt >= STAGES) mbar_wait(&empty_bar[s], phase);
         mbar_arrive_expect_tx(&full_bar[s], Cfg::STAGE_BYTES);
         uint8_t* st = tiles + (size_t)s * Cfg::STAGE_BYTES;
-        const int x = kt * TF32_BK;
+        const int x = (kt0 + kt) * TF32_BK;
         tma_load_2d(st, &g.q_hi[grp], x, m_blk0, &full_bar[s]);
         tma_load_2d(st + TF32_A_BYTES, &g.q_lo[grp], x, m_blk0, &full_bar[s]);
         tma_load_2d(st + 2 * TF32_A_BYTES, &g.p_hi, x, prow, &full_bar[s]);
@@ -182,7 +185,8 @@ int launch_gemm_tf32(const Tf32Args& a, int G, const Epi& epi, cudaStream_t st) 
     TKM_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
     configured = true;
   }
-  dim3 grid((unsigned)ceil_div(a.M, TF32_BM), (unsigned)ceil_div(std::max(a.N, 1), Cfg::BN), (unsigned)G);
+  dim3 grid((unsigned)ceil_div(a.M, TF32_BM), (unsigned)(ceil_div(std::max(a.N, 1), Cfg::BN) * std::max(a.ksplit, 1)),
+            (unsigned)G);
   kern<<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(a, epi);
   TKM_LAUNCH_CHECK();
   return TKM_OK;

@@ -197,18 +197,42 @@ static int setup_full(const double* K, int64_t n, int64_t ldk, tkm_spectral* s, 
 
 constexpr double NYS_RANK_TOL = 1e-12;
 
-static int setup_nystrom(int64_t n, const tkm_nystrom* ny, tkm_spectral* s, cudaStream_t st) {
-  const int64_t m = ny->m;
+// Where the rows of K_nm come from: a resident matrix, or X itself -- then K_nm is produced `block_rows` rows
+// at a time by the Gram kernel and never exists as a whole (n ~ 10^6 rows).
+struct NysSource {
+  const double* K_nm = nullptr;   // resident [n][ld_nm]
+  int64_t ld_nm = 0;
+  const double* X = nullptr;      // streamed: [n][ldx] training matrix, Xl [m][ldxl] its landmark rows
+  int64_t p = 0, ldx = 0;
+  const double* Xl = nullptr;
+  int64_t ldxl = 0;
+  double sigma = 0.0;
+  int64_t block_rows = 0;         // 0 = default
+};
+
+constexpr int64_t NYS_BLOCK_ROWS = 32768;
+
+__global__ void gather_rows_kernel(const double* __restrict__ X, int64_t ldx, const int64_t* __restrict__ idx, int p,
+                                   double* __restrict__ out, int64_t ldo) {
+  const double* src = X + idx[blockIdx.x] * ldx;
+  for (int c = threadIdx.x; c < p; c += blockDim.x) out[(int64_t)blockIdx.x * ldo + c] = src[c];
+}
+
+// Peak device memory beyond the inputs: one [rp][ldn] array (Phi^T, overwritten block by block with U^T), the
+// [n][ldr] array U Lam, and three blocks of block_rows rows.
+static int setup_nystrom(int64_t n, int64_t m, const double* K_mm, int64_t ld_mm, const int64_t* landmark_idx,
+                         const NysSource& src, tkm_spectral* s, cudaStream_t st) {
   const int64_t ldm = round_up(m, 16);
   s->n = n;
   s->m = m;
   s->ldm = ldm;
   s->ldn = round_up(n, 16);
+  const int64_t nb_max = std::min<int64_t>(round_up(src.block_rows > 0 ? src.block_rows : NYS_BLOCK_ROWS, 16), s->ldn);
   // 1. K_mm = W Theta W^T
   DevBuf Wv, theta;
   TKM_TRY(Wv.alloc((size_t)m * ldm * sizeof(double), true, st));
   TKM_TRY(theta.alloc((size_t)ldm * sizeof(double), true, st));
-  TKM_CUDA(cudaMemcpy2DAsync(Wv.p, ldm * sizeof(double), ny->K_mm, ny->ld_mm * sizeof(double), m * sizeof(double), m,
+  TKM_CUDA(cudaMemcpy2DAsync(Wv.p, ldm * sizeof(double), K_mm, ld_mm * sizeof(double), m * sizeof(double), m,
                              cudaMemcpyDeviceToDevice, st));
   TKM_TRY(syevd_inplace(Wv.as<double>(), ldm, m, theta.as<double>(), st));
   std::vector<double> h_theta(m);
@@ -224,12 +248,17 @@ static int setup_nystrom(int64_t n, const tkm_nystrom* ny, tkm_spectral* s, cuda
   TKM_LAUNCH_CHECK();
   row_scale_kernel<<<(unsigned)rp, 256, 0, st>>>(Wts, ldm, (int)rp, (int)m, theta.as<double>() + k0);
   TKM_LAUNCH_CHECK();
-  // 2. Phi^T [rp][ldn] = Wts K_nm^T ; Phi [n][ldrp]
-  DevBuf PhiT, Phi;
+  // 2. Phi^T [rp][ldn] = Wts K_nm^T, one block of rows of K_nm at a time
+  DevBuf PhiT, Kblk;
   TKM_TRY(PhiT.alloc((size_t)rp * s->ldn * sizeof(double), true, st));
-  TKM_TRY(Phi.alloc((size_t)n * ldrp * sizeof(double), true, st));
-  TKM_TRY(dgemm_nt(Wts, ldm, ny->K_nm, ny->ld_nm, PhiT.as<double>(), s->ldn, rp, n, m, st));
-  TKM_TRY(transpose_scale_f64(PhiT.as<double>(), s->ldn, rp, n, nullptr, Phi.as<double>(), ldrp, st));
+  if (!src.K_nm) TKM_TRY(Kblk.alloc((size_t)nb_max * ldm * sizeof(double), true, st));
+  for (int64_t b0 = 0; b0 < n; b0 += nb_max) {
+    const int64_t nb = std::min(nb_max, n - b0);
+    const double* Kb = src.K_nm ? src.K_nm + b0 * src.ld_nm : Kblk.as<double>();
+    if (!src.K_nm)
+      TKM_TRY(tkm_gram(src.X + b0 * src.ldx, nb, src.p, src.ldx, src.Xl, m, src.ldxl, src.sigma, TKM_F64, Kblk.p, ldm, st));
+    TKM_TRY(dgemm_nt(Wts, ldm, Kb, src.K_nm ? src.ld_nm : ldm, PhiT.as<double>() + b0, s->ldn, rp, nb, m, st));
+  }
   // 3. G = Phi^T Phi = Q Lam Q^T
   DevBuf G, lamv;
   TKM_TRY(G.alloc((size_t)rp * ldrp * sizeof(double), true, st));
@@ -246,17 +275,22 @@ static int setup_nystrom(int64_t n, const tkm_nystrom* ny, tkm_spectral* s, cuda
   s->r = r;
   s->ldr = round_up(r, 16);
   const double* Qe = G.as<double>() + j0 * ldrp;   // [r][ldrp], rows = eigenvectors
-  // 4. U^T [r][ldn] = Lam^-1/2 Qe Phi^T
-  TKM_TRY(s->Ut.alloc((size_t)r * s->ldn * sizeof(double), true, st));
+  // 4. U^T [r][ldn] = Lam^-1/2 Qe Phi^T, block by block over Phi^T's own storage (r <= rp rows of it)
   TKM_TRY(s->lam.alloc((size_t)s->ldr * sizeof(double), true, st));
   TKM_TRY(s->u1.alloc((size_t)s->ldr * sizeof(double), true, st));
   TKM_CUDA(cudaMemcpyAsync(s->lam.p, lamv.as<double>() + j0, r * sizeof(double), cudaMemcpyDeviceToDevice, st));
-  DevBuf isq;
+  DevBuf isq, Phib;
   TKM_TRY(isq.alloc((size_t)r * sizeof(double), false, st));
   TKM_CUDA(cudaMemcpyAsync(isq.p, s->lam.p, r * sizeof(double), cudaMemcpyDeviceToDevice, st));
   vec_op_kernel<<<(unsigned)ceil_div(r, 256), 256, 0, st>>>(isq.as<double>(), (int)r, 1);
   TKM_LAUNCH_CHECK();
-  TKM_TRY(dgemm_nt(Qe, ldrp, Phi.as<double>(), ldrp, s->Ut.as<double>(), s->ldn, r, n, rp, st));
+  TKM_TRY(Phib.alloc((size_t)nb_max * ldrp * sizeof(double), true, st));   // [nb][ldrp]: a block of Phi
+  for (int64_t b0 = 0; b0 < n; b0 += nb_max) {
+    const int64_t nb = std::min(nb_max, n - b0);
+    TKM_TRY(transpose_scale_f64(PhiT.as<double>() + b0, s->ldn, rp, nb, nullptr, Phib.as<double>(), ldrp, st));
+    TKM_TRY(dgemm_nt(Qe, ldrp, Phib.as<double>(), ldrp, PhiT.as<double>() + b0, s->ldn, r, nb, rp, st));
+  }
+  s->Ut.take(PhiT);
   row_scale_kernel<<<(unsigned)r, 256, 0, st>>>(s->Ut.as<double>(), s->ldn, (int)r, (int)n, isq.as<double>());
   TKM_LAUNCH_CHECK();
   // 5. landmark map: lmap_t[j][l] = sqrt(Lam_j) sum_k Qe[j][k] Wts[k][l]
@@ -270,11 +304,33 @@ static int setup_nystrom(int64_t n, const tkm_nystrom* ny, tkm_spectral* s, cuda
   TKM_LAUNCH_CHECK();
   row_scale_kernel<<<(unsigned)r, 256, 0, st>>>(s->lmap_t.as<double>(), ldm, (int)r, (int)m, isq.as<double>());
   TKM_LAUNCH_CHECK();
-  s->landmark_idx.assign(ny->landmark_idx, ny->landmark_idx + m);
+  s->landmark_idx.assign(landmark_idx, landmark_idx + m);
   TKM_TRY(s->d_landmark_idx.alloc((size_t)m * sizeof(int64_t), false, st));
   TKM_CUDA(cudaMemcpyAsync(s->d_landmark_idx.p, s->landmark_idx.data(), m * sizeof(int64_t), cudaMemcpyHostToDevice, st));
   TKM_TRY(finish_spectral(s, st));   // synchronises: the temporaries above may now be freed
   return TKM_OK;
+}
+
+static int nystrom_x_impl(const double* X, int64_t n, int64_t p, int64_t ldx, double sigma, const int64_t* landmark_idx,
+                          int64_t m, int64_t block_rows, tkm_spectral* s, cudaStream_t st) {
+  const int64_t ldm = round_up(m, 16), ldxl = round_up(p, 2);
+  DevBuf d_idx, Xl, Kmm;
+  TKM_TRY(d_idx.alloc((size_t)m * sizeof(int64_t), false, st));
+  TKM_TRY(Xl.alloc((size_t)m * ldxl * sizeof(double), true, st));
+  TKM_TRY(Kmm.alloc((size_t)m * ldm * sizeof(double), true, st));
+  TKM_CUDA(cudaMemcpyAsync(d_idx.p, landmark_idx, m * sizeof(int64_t), cudaMemcpyHostToDevice, st));
+  gather_rows_kernel<<<(unsigned)m, 128, 0, st>>>(X, ldx, d_idx.as<int64_t>(), (int)p, Xl.as<double>(), ldxl);
+  TKM_LAUNCH_CHECK();
+  TKM_TRY(tkm_gram(Xl.p, m, p, ldxl, nullptr, 0, 0, sigma, TKM_F64, Kmm.p, ldm, st));
+  NysSource src;
+  src.X = X;
+  src.p = p;
+  src.ldx = ldx;
+  src.Xl = Xl.as<double>();
+  src.ldxl = ldxl;
+  src.sigma = sigma;
+  src.block_rows = block_rows;
+  return setup_nystrom(n, m, Kmm.as<double>(), ldm, landmark_idx, src, s, st);   // synchronises before returning
 }
 
 }  // namespace tkm
@@ -295,8 +351,45 @@ extern "C" int tkm_spectral_setup(const void* K, int64_t n, int64_t ldk, const t
   tkm_spectral* s = new (std::nothrow) tkm_spectral();
   if (!s) return set_error(TKM_ENOMEM, "out of host memory");
   s->sweep_dt = sweep_dt;
-  int rc = ny ? setup_nystrom(n, ny, s, st) : setup_full((const double*)K, n, ldk, s, st);
+  int rc;
+  if (ny) {
+    NysSource src;
+    src.K_nm = ny->K_nm;
+    src.ld_nm = ny->ld_nm;
+    rc = setup_nystrom(n, ny->m, ny->K_mm, ny->ld_mm, ny->landmark_idx, src, s, st);
+  } else {
+    rc = setup_full((const double*)K, n, ldk, s, st);
+  }
   if (rc == TKM_OK && sweep_dt == TKM_F32) rc = set_error(TKM_ENOTIMPL, "an all-FP32 (3xTF32) sweep is not provided: use TKM_F64, optionally with tkm_loss_opts.tf32_delta");
+  if (rc != TKM_OK) {
+    cudaStreamSynchronize(st);
+    delete s;
+    return rc;
+  }
+  *out = s;
+  return TKM_OK;
+}
+
+// Nystrom setup straight from the training matrix: the landmark rows are gathered, K_mm is formed, and K_nm is
+// produced and consumed block_rows rows at a time (never resident).
+extern "C" int tkm_spectral_setup_nystrom_x(const void* X, int64_t n, int64_t p, int64_t ldx, double sigma,
+                                            const int64_t* landmark_idx, int64_t m, int64_t block_rows,
+                                            tkm_spectral** out, void* stream) {
+  using namespace tkm;
+  if (!out) return set_error(TKM_EINVAL, "tkm_spectral_setup_nystrom_x: out is NULL");
+  *out = nullptr;
+  if (!X || !landmark_idx || n <= 1 || n > (1 << 30) || p < 1 || p > (1 << 24) || ldx < p || m < 1 || m > n ||
+      !(sigma > 0.0) || block_rows < 0)
+    return set_error(TKM_EINVAL, "tkm_spectral_setup_nystrom_x: bad arguments");
+  for (int64_t i = 0; i < m; ++i)
+    if (landmark_idx[i] < 0 || landmark_idx[i] >= n)
+      return set_error(TKM_EINVAL, "tkm_spectral_setup_nystrom_x: landmark index out of range");
+  TKM_TRY(device_check());
+  cudaStream_t st = (cudaStream_t)stream;
+  tkm_spectral* s = new (std::nothrow) tkm_spectral();
+  if (!s) return set_error(TKM_ENOMEM, "out of host memory");
+  s->sweep_dt = TKM_F64;
+  int rc = nystrom_x_impl((const double*)X, n, p, ldx, sigma, landmark_idx, m, block_rows, s, st);
   if (rc != TKM_OK) {
     cudaStreamSynchronize(st);
     delete s;

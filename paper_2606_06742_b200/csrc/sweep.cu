@@ -228,6 +228,71 @@ struct ZetaEpi {
   }
 };
 
+// ---- K-split GEMM-B (thin U: r x B outputs, n ~ 10^5..10^6 deep) ------------------------------------------------
+// With few output tiles and a very long contraction the launch cannot fill the SMs, so K is cut into S ranges
+// (GemmArgs / Tf32Args::ksplit): every CTA stores its partial U^T z (or U^T dz) into part[split], and
+// spec_finalize_kernel sums the S partials in a fixed order and applies the SpecEpi / ZetaEpi arithmetic.
+struct PartEpi {   // FP64 DMMA kernel
+  int B, ksplit;
+  int64_t lda, split_stride;
+  double* part;   // [S][G*B][lda]
+  template <class Cfg>
+  __device__ __forceinline__ void run(double (&acc)[Cfg::TN][Cfg::TM][2], int n_blk0, int m_blk0, int warp_n,
+                                      int warp_m, int lane, int N, int M, int grp, double*) const {
+    constexpr int TN = Cfg::TN, TM = Cfg::TM;
+    double* base = part + (int64_t)gemm_split_index(ksplit) * split_stride;
+#pragma unroll
+    for (int t = 0; t < TN; ++t) {
+      const int slot = n_blk0 + (warp_n * TN + t) * 8 + (lane >> 2);
+      if (slot >= N) continue;
+      const int64_t row = (int64_t)(grp * B + slot) * lda;
+#pragma unroll
+      for (int j = 0; j < TM; ++j) {
+        const int i = m_blk0 + (warp_m * TM + j) * 8 + 2 * (lane & 3);
+        if (i + 1 < M)
+          *reinterpret_cast<double2*>(base + row + i) = make_double2(acc[t][j][0], acc[t][j][1]);
+        else if (i < M)
+          base[row + i] = acc[t][j][0];
+      }
+    }
+  }
+};
+
+struct ZetaPartEpi {   // tcgen05 kernel
+  static constexpr bool kReduce = false;
+  int B, ksplit;
+  int64_t lda, split_stride;
+  double* part;
+  __device__ __forceinline__ void chunk(const float (&v)[16], int i, int n0, int N, int M, int grp, double*, int) const {
+    if (i >= M) return;
+    double* base = part + (int64_t)gemm_split_index(ksplit) * split_stride + (int64_t)(grp * B + n0) * lda + i;
+    const int cnt = min(16, N - n0);
+#pragma unroll
+    for (int k = 0; k < 16; ++k)
+      if (k < cnt) base[(int64_t)k * lda] = (double)v[k];
+  }
+};
+
+// zeta = (accumulate ? Zeta : 0) + sum_s part[s];  Zeta <- zeta (if kept);  rho = zeta + 2 lam abar
+__global__ void __launch_bounds__(256) spec_finalize_kernel(const double* __restrict__ part, int S, int64_t split_stride,
+                                                            const int32_t* __restrict__ nslots,
+                                                            const int32_t* __restrict__ col_of_slot,
+                                                            const double* __restrict__ col_lam, int B, int r, int64_t lda,
+                                                            const double* __restrict__ Abar, double* __restrict__ Zeta,
+                                                            int accumulate, double* __restrict__ Rho) {
+  const int grp = blockIdx.z, slot = blockIdx.y;
+  if (slot >= nslots[grp]) return;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= r) return;
+  const int64_t o = (int64_t)(grp * B + slot) * lda + i;
+  double z = accumulate ? Zeta[o] : 0.0;
+  double acc = 0.0;
+  for (int s = 0; s < S; ++s) acc += part[(int64_t)s * split_stride + o];
+  z += acc;
+  if (Zeta) Zeta[o] = z;
+  Rho[o] = z + 2.0 * col_lam[col_of_slot[grp * B + slot]] * Abar[o];
+}
+
 // ---- delta-form GEMM-A epilogue (tcgen05 kernel): F+ = Fbar - U Lam da, next extrapolation, loss derivative ----
 // Thread = one sample row m (a TMEM lane), 16 consecutive slots per call.  State per slot: Fb = Fbar_k (what the
 // loss saw), Fp = F_k.  With G = U Lam da_k from the accumulator:  F_{k+1} = Fbar_k - G,
@@ -689,6 +754,8 @@ static double curvature_of(tkm_loss loss, double smooth) {
   return 1.0 / (2.0 * smooth);   // 1/kappa, kappa = 2 delta
 }
 
+constexpr int KSPLIT_MIN_K = 16384;   // contraction depth from which GEMM-B may be K-split (thin U, large n)
+constexpr int KSPLIT_MAX = 16;
 constexpr int DELTA_MIN_LIVE = 48;   // live columns (all groups) below which the delta forms are switched off
 constexpr int POLL_RING = 5;   // ring of poll results: up to POLL_RING - 2 batches may be in flight
 
@@ -860,6 +927,11 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
       TKM_TRY(split_tf32(specs[g]->Ut.as<double>(), ldn, r, n, ut_hi[g].as<float>(), ut_lo[g].as<float>(), ldn32, st));
     }
   }
+  // K-split GEMM-B (thin U with a long contraction): partial sums [KSPLIT_MAX][G*B][ldr]
+  const bool ksplit_ok = n >= KSPLIT_MIN_K;
+  const int64_t split_stride = (int64_t)GB * ldr;
+  DevBuf zpart;
+  if (ksplit_ok) TKM_TRY(zpart.alloc((size_t)KSPLIT_MAX * split_stride * sizeof(double), false, st));
   // F half (tf32_delta == 2): Fbar / F state, the (hi, lo) step operand, U Lam as (hi, lo), momentum per column
   const bool delta_f = opts->tf32_delta == 2;
   const int64_t ldr32 = round_up(r, 32);
@@ -1017,6 +1089,24 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
         targs.N = targsF.N = std::max(nmax, 1);
       }
       argsA2.N = argsA.N;
+      // K-split of GEMM-B: only when its output tiles cannot fill the SMs and the contraction is long
+      int ksB = 1, ksT = 1;
+      if (ksplit_ok) {
+        const int64_t mt = ceil_div((int64_t)r, (int64_t)tileB.BM), mtT = ceil_div((int64_t)r, (int64_t)TF32_BM);
+        int64_t ctas = 0, ctasT = 0;
+        for (int g = 0; g < G; ++g) {
+          ctas += mt * ceil_div((int64_t)bound[g], (int64_t)tileB.BN);
+          if (delta) ctasT += mtT * ceil_div((int64_t)bound[g], (int64_t)tf32_bn_of(tcfg));
+        }
+        const int64_t sm = 148;   // B200
+        // FP64 kernel: two resident CTAs per SM at least; tcgen05 kernel: one CTA per SM, so whole waves only
+        if (ctas > 0 && 4 * ctas < 3 * sm) ksB = (int)std::min<int64_t>({(int64_t)KSPLIT_MAX, 2 * sm / ctas, (int64_t)n / 2048});
+        if (ctasT > 0 && 4 * ctasT < 3 * sm) ksT = (int)std::min<int64_t>({(int64_t)KSPLIT_MAX, sm / ctasT, (int64_t)n / 4096});
+        ksB = std::max(ksB, 1);
+        ksT = std::max(ksT, 1);
+      }
+      argsB.ksplit = ksB;
+      targs.ksplit = ksT;
       // The delta forms pay while the batch is wide; the narrow tail is latency-bound either way and its slow
       // columns converge in fewer iterations on exact contractions, so it runs all-FP64 (the live set only
       // shrinks within a round, and every round starts with an exact iteration).
@@ -1065,7 +1155,24 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
           // FP64 contraction; in delta form it also re-establishes zeta = U^T z exactly
           SpecEpi se{col_of_slot.as<int32_t>(), p0->col_lam.as<double>(), B, Abar.as<double>(), ldr, Rho.as<double>(),
                      dz_on ? Zeta.as<double>() : nullptr};
-          TKM_TRY(gemm_f64_launch(argsB, tileB, G, se, st));
+          if (ksB > 1) {
+            PartEpi pe{B, ksB, ldr, split_stride, zpart.as<double>()};
+            TKM_TRY(gemm_f64_launch(argsB, tileB, G, pe, st));
+            spec_finalize_kernel<<<dim3((unsigned)ceil_div(r, 256), (unsigned)std::max(nmax, 1), (unsigned)G), 256, 0, st>>>(
+                zpart.as<double>(), ksB, split_stride, nslots.as<int32_t>(), col_of_slot.as<int32_t>(),
+                p0->col_lam.as<double>(), B, (int)r, ldr, Abar.as<double>(), dz_on ? Zeta.as<double>() : nullptr, 0,
+                Rho.as<double>());
+            TKM_LAUNCH_CHECK();
+          } else {
+            TKM_TRY(gemm_f64_launch(argsB, tileB, G, se, st));
+          }
+        } else if (ksT > 1) {
+          ZetaPartEpi pe{B, ksT, ldr, split_stride, zpart.as<double>()};
+          TKM_TRY(gemm_tf32_launch(targs, tcfg, G, pe, st));
+          spec_finalize_kernel<<<dim3((unsigned)ceil_div(r, 256), (unsigned)std::max(nmax, 1), (unsigned)G), 256, 0, st>>>(
+              zpart.as<double>(), ksT, split_stride, nslots.as<int32_t>(), col_of_slot.as<int32_t>(),
+              p0->col_lam.as<double>(), B, (int)r, ldr, Abar.as<double>(), Zeta.as<double>(), 1, Rho.as<double>());
+          TKM_LAUNCH_CHECK();
         } else {
           ZetaEpi ze{col_of_slot.as<int32_t>(), p0->col_lam.as<double>(), B, Abar.as<double>(), ldr, Zeta.as<double>(),
                      Rho.as<double>()};

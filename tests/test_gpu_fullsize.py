@@ -112,11 +112,24 @@ def test_full_kernel_configs_first_order_optimality(tkm, cfg, delta):
 
 
 def test_nystrom_config4_first_order_optimality(tkm):
-    """configs[4]: n = 100000, m = 4096 landmarks.  The model is the minimiser of the problem with
-    K~ = K_nm K_mm^+ K_nm^T restricted to its numerically non-null directions (reading G11); with alpha~ = -z/(2 lambda) its decision values must satisfy
+    """configs[4]: n = 100000, m = 4096 landmarks, K_nm resident."""
+    _nystrom_first_order(tkm, wl.config4(), streamed=False)
+
+
+def test_nystrom_streamed_at_paper_scale_first_order_optimality(tkm):
+    """the row count of the paper's covtype run (581,012 samples; p = 54 as in
+    that data set, synthetic rows), m = 2048 landmarks, K_nm never resident in the library (produced and
+    consumed 32768 rows at a time).  A short lambda grid keeps the test short; the checker builds its own K_nm."""
+    w = wl.config4(n=581012, p=54, m=2048, L=3, V=2, seed=1044)
+    w.lambdas[:] = np.array([1.0, 1e-2, 1e-3])
+    _nystrom_first_order(tkm, w, streamed=True)
+
+
+def _nystrom_first_order(tkm, w, streamed):
+    """The model is the minimiser of the problem with K~ = K_nm K_mm^+ K_nm^T restricted to its numerically
+    non-null directions (reading G11); with alpha~ = -z/(2 lambda) its decision values must satisfy
     f = K~ alpha~ + beta0 and sum z = 0, where f is evaluated from the landmark weights the library returns."""
     import torch
-    w = wl.config4()
     sigma = float(w.sigmas[0])
     idx = wl.landmarks(w.n, w.m_landmarks, w.landmark_seed)
     foldid = tkm.tkm_make_folds(w.n, w.V, w.fold_seed)
@@ -125,10 +138,17 @@ def test_nystrom_config4_first_order_optimality(tkm):
     K_nm = tkm.tkm_gram(X, sigma, Xl)
     K_mm = tkm.tkm_gram(Xl, sigma)
     rng = np.random.default_rng(4)
+    L, V = w.L, w.V
     ii, jj, got = _check_gram_entries(K_nm, w.X, sigma, rng)
     d2 = ((w.X[ii] - w.X[idx[jj]]) ** 2).sum(axis=1)
     assert np.max(np.abs(got - np.exp(-d2 / (2 * sigma * sigma)))) < 1e-13
-    spec = tkm.tkm_spectral_setup(nystrom=(K_nm, K_mm, idx))
+    if streamed:
+        del K_nm
+        torch.cuda.empty_cache()
+        spec = tkm.tkm_spectral_setup_nystrom_x(X, sigma, idx)
+        K_nm = tkm.tkm_gram(X, sigma, Xl)          # for the checker below only
+    else:
+        spec = tkm.tkm_spectral_setup(nystrom=(K_nm, K_mm, idx))
     assert spec.n == w.n and 0 < spec.r <= w.m_landmarks
     path = tkm.tkm_fit_path(spec, y, w.loss, w.lambdas, foldid, w.V, TOL, MAXIT, smooth0=w.smooth0, eta=w.eta,
                             rounds=w.rounds, warm_tol=WARM_TOL, tf32_delta=2)    # both contractions in delta form
@@ -142,7 +162,6 @@ def test_nystrom_config4_first_order_optimality(tkm):
     lam2, Q2 = torch.linalg.eigh(Phi.T @ Phi)            # second truncation of reading G11
     Phi = Phi @ Q2[:, lam2 > 1e-12 * lam2.max()]
     assert Phi.shape[1] == spec.r
-    L, V = w.L, w.V
     smooth_final = w.smooth0 * w.eta ** (w.rounds - 1)
     for (v, l) in [(0, 0), (1, L // 3), (V, L // 2), (V - 1, (3 * L) // 4), (2, L - 1)]:
         gam, b0 = tkm.tkm_path_coef(path, 0, l, v)
@@ -155,7 +174,7 @@ def test_nystrom_config4_first_order_optimality(tkm):
         at = _dev(-z / (2.0 * w.lambdas[l]))
         f_def = torch.mv(Phi, torch.mv(Phi.T, at)) + b0
         err = float((f_def - f).abs().max() / max(1.0, float(f.abs().max())))
-        print("cfg 4 (v=%d, l=%d): |sum z| %.2e, max |f - (K~ alpha~ + b0)| %.2e" % (v, l, abs(z.sum()), err))
+        print("nystrom n=%d (v=%d, l=%d): |sum z| %.2e, max |f - (K~ alpha~ + b0)| %.2e" % (w.n, v, l, abs(z.sum()), err))
         # f - f_def = U Lam rho / (2 lambda) with rho the stationarity residual the stop test bounds (G6):
         # n_c ||rho|| / sqrt(n) <= TOL, so the admissible gap grows like 1/lambda
         bound = 1e-8 + float(lam2.max()) * TOL * np.sqrt(w.n) / (nc * 2.0 * w.lambdas[l])

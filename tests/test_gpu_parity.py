@@ -238,7 +238,9 @@ def test_config1_full_size_sampled_columns(tkm):
                 assert np.abs(alpha[foldid == v]).max() < 1e-8 * sc
 
 
-def test_nystrom_parity(tkm):
+@pytest.mark.parametrize("streamed", [False, True])
+def test_nystrom_parity(tkm, streamed):
+    """streamed: the setup forms K_mm itself and produces K_nm 64 rows at a time (11 blocks, ragged last one)."""
     w = wl.config4(n=700, p=8, m=96, L=5, V=3)
     sigma = float(w.sigmas[0])
     idx = wl.landmarks(w.n, w.m_landmarks, w.landmark_seed)
@@ -247,7 +249,8 @@ def test_nystrom_parity(tkm):
     Xl = X[dev(idx)]
     K_nm = tkm.tkm_gram(X, sigma, Xl)
     K_mm = tkm.tkm_gram(Xl, sigma)
-    spec = tkm.tkm_spectral_setup(nystrom=(K_nm, K_mm, idx))
+    spec = (tkm.tkm_spectral_setup_nystrom_x(X, sigma, idx, block_rows=64) if streamed
+            else tkm.tkm_spectral_setup(nystrom=(K_nm, K_mm, idx)))
     spec_o = o.nystrom_setup(w.X, sigma, idx)
     assert spec.r == spec_o.r
     U = spec.U().cpu().numpy()
@@ -276,6 +279,24 @@ def test_nystrom_parity(tkm):
     assert np.max(np.abs(f_g.cpu().numpy() - f_o)) < 1e-6
     if np.min(np.abs(f_o)) > 1e-6:
         assert np.array_equal(lab_g.cpu().numpy(), lab_o)
+
+
+def test_nystrom_streamed_error_paths(tkm):
+    w = wl.config4(n=120, p=4, m=16, L=2, V=2)
+    X = dev(w.X)
+    idx = wl.landmarks(w.n, 16, 3)
+    for bad in (dict(sigma=0.0), dict(landmark_idx=np.array([0, 120])), dict(landmark_idx=np.array([-1, 3])),
+                dict(block_rows=-5)):
+        kw = dict(sigma=1.0, landmark_idx=idx, block_rows=0)
+        kw.update(bad)
+        with pytest.raises(tkm.TkmError):
+            tkm.tkm_spectral_setup_nystrom_x(X, kw["sigma"], kw["landmark_idx"], kw["block_rows"])
+    one_block = tkm.tkm_spectral_setup_nystrom_x(X, 2.0, idx)                 # block larger than n
+    many = tkm.tkm_spectral_setup_nystrom_x(X, 2.0, idx, block_rows=16)      # 8 blocks, ragged tail of 8
+    assert one_block.r == many.r
+    l1, _ = one_block.eigenvalues()
+    l2, _ = many.eigenvalues()
+    assert np.max(np.abs(l1 - l2)) <= 1e-12 * l1.max()
 
 
 # ------------------------------------------------------------------------------- edge cases / errors
@@ -491,3 +512,44 @@ def test_column_sharded_lambda_grid_matches_single_gpu_and_oracle(tkm):
     assert np.all(bt == int(np.argmax(w.lambdas)))
     with pytest.raises(tkm.TkmError):
         tkm.tkm_cv_select(flat, np.zeros(w.V), w.lambdas)
+
+
+# --------------------------------------------------- K-split GEMM-B (thin U, long contraction)
+_KSPLIT_ORACLE = {}
+
+
+@pytest.mark.parametrize("mode", [0, 2])
+def test_thin_u_long_contraction_ksplit_parity(tkm, mode):
+    """n = 17000 rows, r <= 48: GEMM-B has one output tile per 54 columns and a 17000-deep contraction, so the
+    library cuts K into ranges (FP64 DMMA kernel: mode 0 and the exact iterations; tcgen05 kernel: the delta
+    iterations of mode 2) and sums the partials in a fixed order.  Decision values and CV tables against the oracle."""
+    w = wl.config4(n=17000, p=6, m=48, L=9, V=5, seed=77)
+    w.lambdas[:] = np.logspace(0, -2, 9)
+    sigma = float(w.sigmas[0])
+    idx = wl.landmarks(w.n, w.m_landmarks, w.landmark_seed)
+    foldid = tkm.tkm_make_folds(w.n, w.V, w.fold_seed)
+    X, y = dev(w.X), dev(w.y)
+    spec = tkm.tkm_spectral_setup_nystrom_x(X, sigma, idx, block_rows=4096)
+    spec_o = o.nystrom_setup(w.X, sigma, idx)
+    assert spec.r == spec_o.r
+    tol = 1e-11
+    path = tkm.tkm_fit_path(spec, y, w.loss, w.lambdas, foldid, w.V, tol, 200000, rounds=w.rounds, tf32_delta=mode)
+    info = path.info()
+    assert info["flags"].sum() == 0 and np.all(info["kkt"] <= tol)
+    if "res" not in _KSPLIT_ORACLE:      # the oracle's fit takes most of a minute: once for both modes
+        _KSPLIT_ORACLE["res"] = o.fit_path(spec_o, w.y, w.loss, w.lambdas, foldid, w.V, rounds=w.rounds, tol=tol,
+                                           maxit=400000)
+    res = _KSPLIT_ORACLE["res"]
+    U = spec.U().cpu().numpy()
+    lam, _ = spec.eigenvalues()
+    a_gpu = path.a().cpu().numpy()
+    worst = 0.0
+    for c in range(res.cols["B"]):
+        f_o = spec_o.U @ (spec_o.lam * res.a[:, c]) + res.beta0[c]
+        f_g = U @ (lam * a_gpu[c]) + info["beta0"][c]
+        worst = max(worst, np.max(np.abs(f_g - f_o)) / max(1.0, np.abs(f_o).max()))
+    print("ksplit mode %d: max |f_gpu - f_oracle| %.2e" % (mode, worst))
+    assert worst < 1e-7
+    cv = tkm.tkm_exact_cv(path, y, foldid, 1, w.L, w.V)
+    cv_o = o.exact_cv(spec_o, res, w.y, foldid, w.loss)
+    assert np.max(np.abs(cv[0] - cv_o[0])) <= CV_TOL and np.array_equal(cv[1], cv_o[1]) and np.array_equal(cv[3], cv_o[3])
