@@ -357,6 +357,82 @@ def run_ours(args, w, rank, world):
         dist.destroy_process_group()
 
 
+# ------------------------------------------------------------- secondary workload: Nystrom at the paper's row counts
+def run_nystrom_scale(args):
+    """`--workload nystrom_covtype | nystrom_mnist8m46` (not the headline line): streamed Nystrom
+    setup + sweep + exact CV at the row counts of the paper's Table 4, one GPU, X and y resident.  One JSON line with
+    the same metric; `roofline` holds the four contraction-kernel families as sampled inside the sweep."""
+    import torch
+    import paper_2606_06742_b200 as tkm
+    tkm.lib()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (libtkm has no CPU fallback)")
+    torch.cuda.set_device(0)
+    w = wl.nystrom_paper_shape(args.workload[len("nystrom_"):])
+    sigma = float(w.sigmas[0])
+    idx = wl.landmarks(w.n, w.m_landmarks, w.landmark_seed)
+    foldid = tkm.tkm_make_folds(w.n, w.V, w.fold_seed)
+    X, y = torch.from_numpy(w.X).cuda(), torch.from_numpy(w.y).cuda()
+    pk = peaks()
+
+    def ev():
+        e = torch.cuda.Event(enable_timing=True)
+        e.record()
+        return e
+
+    tot = np.zeros(3)
+    prof = dict(ms=np.zeros(4), flops=np.zeros(4), launches=np.zeros(4, dtype=np.int64))
+    col_iters = 0
+    mon = ClockSampler(0)
+    for it in range(args.warmup + args.steps):
+        if it == args.warmup:
+            mon.start()
+        e0 = ev()
+        spec = tkm.tkm_spectral_setup_nystrom_x(X, sigma, idx)
+        e1 = ev()
+        path = tkm.tkm_fit_path(spec, y, w.loss, w.lambdas, foldid, w.V, args.tol, MAXIT, smooth0=w.smooth0, eta=w.eta,
+                                rounds=w.rounds, warm_tol=WARM_TOL, tf32_delta=2, profile=True)
+        e2 = ev()
+        tkm.tkm_exact_cv(path, y, foldid, 1, w.L, w.V)
+        e3 = ev()
+        e3.synchronize()
+        if path.status != 0:
+            raise RuntimeError("columns hit maxit: the timed work is not the stated work")
+        if it >= args.warmup:
+            tot += [e0.elapsed_time(e1), e1.elapsed_time(e2), e2.elapsed_time(e3)]
+            pr = path.profile()
+            for k in prof:
+                prof[k] += pr[k]
+            col_iters += path.total_col_iters
+        r = spec.r
+        path.close()
+        spec.close()
+    clocks = mon.stop()
+    tot /= args.steps
+    names = ["gemm_f64_tma_kernel GEMM-A (FP64 DMMA)", "gemm_f64_tma_kernel GEMM-B (FP64 DMMA, K-split)",
+             "gemm_tf32x3_kernel GEMM-A (tcgen05 3xTF32)", "gemm_tf32x3_kernel GEMM-B (tcgen05 3xTF32, K-split)"]
+    f64_tf, tf32x3_tf = pk["bf16_sus"] * NOMINAL_RATIO["f64"], pk["bf16_sus"] * NOMINAL_RATIO["f32"]   # as in run_ours
+    peak = [f64_tf, f64_tf, tf32x3_tf, tf32x3_tf]
+    fam = [{"kernel": names[i], "bound": "tensor", "achieved": float(prof["flops"][i] / prof["ms"][i] / 1e9), "peak": peak[i],
+            "unit": "TFLOP/s", "frac": float(prof["flops"][i] / prof["ms"][i] / 1e9 / peak[i]),
+            "sampled_launches": int(prof["launches"][i]), "avg_launch_ms": float(prof["ms"][i] / prof["launches"][i]),
+            "traffic": None} for i in range(4) if prof["launches"][i]]
+    print(json.dumps({
+        "metric": "lambda_x_fold_path_fits_per_s", "value": w.B / (tot.sum() / 1e3), "unit": "fits/s", "n_gpus": 1,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": float(tot.sum()), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "%s: Nystrom smoothed-hinge SVM with the shape of the paper's Table-4 data set (synthetic "
+                               "rows), n=%d, p=%d, m=%d landmarks (r=%d), %d folds, %d lambdas 1e2..1e-5; secondary "
+                               "workload, not BASELINE.json's metric configuration" % (args.workload, w.n, w.p,
+                                                                                        w.m_landmarks, r, w.V, w.L),
+                   "columns_per_step": w.B, "stop_tol": args.tol, "warm_start_rounds_tol": WARM_TOL, "tf32_delta": 2,
+                   "l2": "inputs larger than L2 (U alone is %.1f GB)" % (w.n * r * 8 / 1e9)},
+        "stages_ms_per_step": {"nystrom_setup_streamed": float(tot[0]), "sweep": float(tot[1]), "exact_cv": float(tot[2])},
+        "col_iters_per_step": col_iters / args.steps,
+        "sweep_useful_tflops": 4.0 * w.n * r * col_iters / args.steps / (tot[1] / 1e3) / 1e12,
+        "roofline": fam, "clocks": clocks}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -364,9 +440,17 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--workload", default="config1", choices=["config1", "nystrom_covtype", "nystrom_mnist8m46"],
+                    help="config1 = BASELINE.json's metric configuration (the bench line); the nystrom_* workloads are "
+                         "secondary single-GPU measurements (use --steps 1 --warmup 1: a step takes 20-100 s)")
+    ap.add_argument("--tol", type=float, default=1e-10, help="stop tolerance of the nystrom_* workloads")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.workload != "config1":
+        if args.impl != "ours" or world != 1 or args.gpus != 1:
+            raise SystemExit("--workload %s: one GPU, --impl ours only" % args.workload)
+        return run_nystrom_scale(args)
     from paper_2606_06742_b200.ranks import replica_seed
     w = wl.config1(seed=replica_seed(1001, rank if args.impl == "ours" else 0))
     if args.impl == "reference":

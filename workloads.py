@@ -162,6 +162,16 @@ def config4(n: int = 100000, p: int = 50, m: int = 4096, L: int = 100, V: int = 
                     m_landmarks=m, landmark_seed=seed + 17)
 
 
+def nystrom_paper_shape(name: str) -> Workload:
+    """Nystrom workloads with the row and feature counts of the paper's two largest Table-4 data sets
+    (covtype 581,012 x 54; MNIST8m 4-vs-6 1,270,178 x 784).  Synthetic rows (the LIBSVM
+    files are not in this container), m = 2048 landmarks, 50 lambdas 1e2..1e-5, 5 folds."""
+    n, p, seed = {"covtype": (581012, 54, 1044), "mnist8m46": (1270178, 784, 1046)}[name]
+    w = config4(n=n, p=p, m=2048, L=50, V=5, seed=seed)
+    w.lambdas[:] = lambda_grid(2, -5, 50)
+    return w
+
+
 def landmarks(n: int, m: int, seed: int) -> np.ndarray:
     """m distinct row indices: first m entries of a seeded permutation."""
     return np.sort(np.random.default_rng(seed).permutation(n)[:m]).astype(np.int64)
