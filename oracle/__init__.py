@@ -24,6 +24,7 @@ Parity pins (tests/test_oracle_*.py, `-m "not gpu"`):
   folds       sizes, permutation property, golden bytes from SplitMix64     (P14)
   C <-> lam   objective scaling                                             (P15)
   platt       zero gradient; scikit-learn's _sigmoid_calibration           (P16)
+  gap         0 <= gap = O(delta); weak duality; D <= P*(SVC) <= P          (P17)
 Parity unpinned by the paper (inputs, fixed by SURVEY.md 8(c)/DESIGN.md, not
 results): delta_0, R, tol, maxit, the t3 noise scale, the landmark seed.
 """
@@ -37,3 +38,4 @@ from .cv import exact_cv, predict, label_of
 from .nystrom import nystrom_setup, nystrom_landmark_weights
 from .platt import platt_fit, platt_proba, platt_targets, platt_objective, cv_decision_values
 from .refit import brute_force_refit, dense_majoriser, objective
+from .diagnostics import duality_gap
