@@ -190,6 +190,15 @@ int tkm_path_get_a(const tkm_path* p, double* a_out, void* stream);
 int tkm_exact_cv(const tkm_path* p, const void* y, const int32_t* foldid,
                  double* cv_loss, int64_t* cv_err, double* cv_mean, int32_t* best_l, void* stream);
 
+/* tkm_path_duality_gap: diagnostic of the fixed delta-schedule ("until the KKT conditions of
+ * all SVM models are satisfied"; readings G7, G22).  For every column c = (t (V+1) + v) L + l of a hinge or
+ * quantile path: primal[c] = (1/n_c) sum over training rows of the NON-smoothed loss + lambda alpha^T K alpha, and
+ * gap[c] = primal[c] - dual[c] >= primal[c] - optimum, with the dual point the smoothed solution supplies
+ * (theta_j = -L'_delta(y_j f_j)).  One GEMM-A pass over all columns.  y [dev] n, foldid [host] n, primal and
+ * gap [host] B.  TKM_EINVAL for the smooth losses (no smoothing, nothing to certify).  Synchronises `stream`. */
+int tkm_path_duality_gap(const tkm_path* p, const void* y, const int32_t* foldid, double* primal,
+                         double* gap, void* stream);
+
 /* tkm_cv_select: the selection step of tkm_exact_cv on its own (lambda columns sharded
  * over GPUs, the T x L x V loss table gathered before the argmin).  cv_loss [host] T x L x V fold means,
  * fold_sizes [host] V (> 0), lambdas [host] L; writes [host] cv_mean T x L (pooled over folds, weights

@@ -13,7 +13,7 @@ TKM_OK, TKM_ENOTCONV = 0, 5
 
 EXPORTED_SYMBOLS = [
     "tkm_gram", "tkm_gram_multi", "tkm_spectral_setup", "tkm_spectral_setup_multi", "tkm_spectral_setup_nystrom_x", "tkm_spectral_free", "tkm_spectral_info", "tkm_spectral_get_u",
-    "tkm_fit_path", "tkm_fit_path_multi", "tkm_path_free", "tkm_path_info", "tkm_path_profile", "tkm_path_get_a", "tkm_exact_cv", "tkm_cv_select", "tkm_path_coef",
+    "tkm_fit_path", "tkm_fit_path_multi", "tkm_path_free", "tkm_path_info", "tkm_path_profile", "tkm_path_get_a", "tkm_exact_cv", "tkm_cv_select", "tkm_path_duality_gap", "tkm_path_coef",
     "tkm_predict", "tkm_cv_decision_values", "tkm_platt_fit", "tkm_platt_proba", "tkm_train_tune_host", "tkm_make_folds", "tkm_launch_count", "tkm_launch_count_reset",
     "tkm_dgemm_nt", "tkm_gemm_probe", "tkm_tf32x3_gemm_nt", "tkm_version", "tkm_last_error",
 ]
@@ -73,6 +73,7 @@ def lib():
     L.tkm_path_profile.argtypes = [vp, vp, vp, vp]
     L.tkm_path_get_a.argtypes = [vp, vp, vp]
     L.tkm_exact_cv.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
+    L.tkm_path_duality_gap.argtypes = [vp, vp, vp, vp, vp, vp]
     L.tkm_cv_select.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp, vp]
     L.tkm_path_coef.argtypes = [vp, i32, i32, i32, vp, C.POINTER(dbl), vp]
     L.tkm_predict.argtypes = [vp, i32, i32, vp, i64, vp, i64, i64, i64, dbl, vp, vp, vp]
@@ -348,6 +349,16 @@ def tkm_exact_cv(path: Path, y, foldid, T: int, L: int, V: int, stream=None):
     _check(lib().tkm_exact_cv(path._h, y.data_ptr(), _ptr(fid), _ptr(cv_loss), _ptr(cv_err), _ptr(cv_mean),
                               _ptr(best), _stream(stream)))
     return cv_loss, cv_err, cv_mean, best
+
+
+def tkm_path_duality_gap(path: Path, y, foldid, stream=None):
+    """(primal, gap) per column of a hinge / quantile path: objective of the non-smoothed problem and its
+    duality-gap certificate (reading G22)."""
+    y = _dev_f64(y, "y")
+    fid = _host(foldid, np.int32)
+    primal, gap = np.empty(path.B), np.empty(path.B)
+    _check(lib().tkm_path_duality_gap(path._h, y.data_ptr(), _ptr(fid), _ptr(primal), _ptr(gap), _stream(stream)))
+    return primal, gap
 
 
 def tkm_cv_select(cv_loss, fold_sizes, lambdas, stream=None):

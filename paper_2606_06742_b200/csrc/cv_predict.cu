@@ -10,22 +10,9 @@
 
 #include "gemm_f64.cuh"
 #include "handles.cuh"
+#include "losses.cuh"
 
 namespace tkm {
-
-__device__ __forceinline__ double nominal_loss_dev(int loss, double y, double f, double tau) {
-  if (loss == TKM_LOSS_HINGE) return fmax(1.0 - y * f, 0.0);
-  if (loss == TKM_LOSS_LOGISTIC) {
-    const double u = y * f;
-    return fmax(-u, 0.0) + log1p(exp(-fabs(u)));
-  }
-  if (loss == TKM_LOSS_DWD) {
-    const double u = y * f;
-    return (u <= 0.5) ? 1.0 - u : 1.0 / (4.0 * u);
-  }
-  const double t = y - f;
-  return t * (tau - (t < 0.0 ? 1.0 : 0.0));
-}
 
 struct CvEpi {
   const double* y;
@@ -74,6 +61,85 @@ struct CvEpi {
     }
   }
 };
+
+// Duality-gap diagnostic (reading G22): same GEMM-A pass, but over the TRAINING rows of every
+// column: partial sums of the nominal loss and of the dual variable times y, d_j = -y_j psi_delta(y_j, f_j)
+// (hinge: theta_j in [0, 1]; check loss: s_j y_j with s_j in [tau - 1, tau]).
+struct GapEpi {
+  const double* y;
+  const int32_t* foldid;
+  const double* beta0;
+  const double* col_tau;
+  const int32_t* col_v;
+  int loss;
+  double smooth;
+  double* lpart;   // [m blocks][ldpart] sum of the nominal loss over training rows
+  double* dpart;   // [m blocks][ldpart] sum of d_j over training rows
+  int64_t ldpart;
+  template <class Cfg>
+  __device__ __forceinline__ void run(double (&acc)[Cfg::TN][Cfg::TM][2], int n_blk0, int m_blk0, int warp_n,
+                                      int warp_m, int lane, int N, int M, int, double* scratch) const {
+    constexpr int TN = Cfg::TN, TM = Cfg::TM;
+    double ls[TN], ds[TN];
+#pragma unroll
+    for (int i = 0; i < TN; ++i) {
+      ls[i] = ds[i] = 0.0;
+      const int col = n_blk0 + (warp_n * TN + i) * 8 + (lane >> 2);
+      if (col >= N) continue;
+      const int v = col_v[col];
+      const double b0 = beta0[col], tau = col_tau[col];
+#pragma unroll
+      for (int j = 0; j < TM; ++j)
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          const int m = m_blk0 + (warp_m * TM + j) * 8 + 2 * (lane & 3) + e;
+          if (m < M && foldid[m] != v) {
+            const double f = acc[i][j][e] + b0, yy = y[m];
+            ls[i] += nominal_loss_dev(loss, yy, f, tau);
+            ds[i] -= yy * psi_dev(loss, yy, f, smooth, tau);
+          }
+        }
+    }
+    double tot;
+    if (cta_row_reduce<Cfg>(ls, warp_n, warp_m, lane, scratch, tot)) {
+      const int col = n_blk0 + (int)threadIdx.x;
+      if (col < N) lpart[(int64_t)blockIdx.x * ldpart + col] = tot;
+    }
+    if (cta_row_reduce<Cfg>(ds, warp_n, warp_m, lane, scratch, tot)) {
+      const int col = n_blk0 + (int)threadIdx.x;
+      if (col < N) dpart[(int64_t)blockIdx.x * ldpart + col] = tot;
+    }
+  }
+};
+
+// one CTA per column: P = sum loss / n_c + lam a^T Lam a,  D = sum d / n_c - lam a^T Lam a  (fixed summation order)
+__global__ void __launch_bounds__(256) gap_finalize_kernel(const double* __restrict__ lpart, const double* __restrict__ dpart,
+                                                           int64_t ldpart, int nblk, const double* __restrict__ a, int64_t lda,
+                                                           const double* __restrict__ lam_spec, int r,
+                                                           const double* __restrict__ col_lam, const double* __restrict__ col_nc,
+                                                           double* __restrict__ primal, double* __restrict__ gap) {
+  __shared__ double red[8];
+  const int c = blockIdx.x;
+  double q = 0.0;
+  for (int i = threadIdx.x; i < r; i += 256) {
+    const double ai = a[(int64_t)c * lda + i];
+    q += lam_spec[i] * ai * ai;
+  }
+  q = warp_sum(q);
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = q;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double quad = 0.0, ls = 0.0, ds = 0.0;
+    for (int w = 0; w < 8; ++w) quad += red[w];
+    for (int b = 0; b < nblk; ++b) {
+      ls += lpart[(int64_t)b * ldpart + c];
+      ds += dpart[(int64_t)b * ldpart + c];
+    }
+    const double P = ls / col_nc[c] + col_lam[c] * quad, D = ds / col_nc[c] - col_lam[c] * quad;
+    primal[c] = P;
+    gap[c] = P - D;
+  }
+}
 
 // one thread per (t, l, v): sum the per-block partials in fixed order, normalise by the fold size
 __global__ void cv_finalize_kernel(const double* __restrict__ lpart, const double* __restrict__ epart,
@@ -251,6 +317,40 @@ extern "C" int tkm_exact_cv(const tkm_path* p, const void* y, const int32_t* fol
   if (cv_err) TKM_CUDA(cudaMemcpyAsync(cv_err, d_err.p, nout * sizeof(long long), cudaMemcpyDeviceToHost, st));
   TKM_CUDA(cudaMemcpyAsync(cv_mean, d_mean.p, T * L * sizeof(double), cudaMemcpyDeviceToHost, st));
   TKM_CUDA(cudaMemcpyAsync(best_l, d_best.p, T * sizeof(int), cudaMemcpyDeviceToHost, st));
+  TKM_CUDA(cudaStreamSynchronize(st));
+  return TKM_OK;
+}
+
+extern "C" int tkm_path_duality_gap(const tkm_path* p, const void* y, const int32_t* foldid, double* primal,
+                                    double* gap, void* stream) {
+  if (!p || !y || !foldid || !primal || !gap) return set_error(TKM_EINVAL, "tkm_path_duality_gap: NULL argument");
+  if (p->loss != TKM_LOSS_HINGE && p->loss != TKM_LOSS_QUANTILE)
+    return set_error(TKM_EINVAL, "tkm_path_duality_gap: defined for the smoothed losses (hinge, quantile) only");
+  TKM_TRY(device_check());
+  cudaStream_t st = (cudaStream_t)stream;
+  const tkm_spectral* s = p->spec;
+  const int64_t n = s->n, r = s->r;
+  const int B = p->B;
+  for (int64_t j = 0; j < n; ++j)
+    if (foldid[j] < 0 || foldid[j] >= p->V) return set_error(TKM_EINVAL, "tkm_path_duality_gap: foldid out of range");
+  const int nblk = (int)ceil_div(n, gemm_f64_choose(&B, 1, (int)n, (int)r).BM);
+  const int64_t ldpart = round_up(B, 16);
+  DevBuf lpart, dpart, d_fold, d_P, d_gap;
+  TKM_TRY(lpart.alloc((size_t)nblk * ldpart * sizeof(double), true, st));
+  TKM_TRY(dpart.alloc((size_t)nblk * ldpart * sizeof(double), true, st));
+  TKM_TRY(d_fold.alloc((size_t)n * sizeof(int32_t), false, st));
+  TKM_TRY(d_P.alloc((size_t)B * sizeof(double), false, st));
+  TKM_TRY(d_gap.alloc((size_t)B * sizeof(double), false, st));
+  TKM_CUDA(cudaMemcpyAsync(d_fold.p, foldid, n * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+  GapEpi epi{(const double*)y, d_fold.as<int32_t>(), p->beta0.as<double>(), p->col_tau.as<double>(),
+             p->col_v.as<int32_t>(), (int)p->loss, p->smooth_final, lpart.as<double>(), dpart.as<double>(), ldpart};
+  TKM_TRY(gemm_f64_once(p->a.as<double>(), s->ldr, s->UL.as<double>(), s->ldr, B, (int)n, (int)r, epi, st));
+  gap_finalize_kernel<<<(unsigned)B, 256, 0, st>>>(lpart.as<double>(), dpart.as<double>(), ldpart, nblk, p->a.as<double>(),
+                                                   s->ldr, s->lam.as<double>(), (int)r, p->col_lam.as<double>(),
+                                                   p->col_nc.as<double>(), d_P.as<double>(), d_gap.as<double>());
+  TKM_LAUNCH_CHECK();
+  TKM_CUDA(cudaMemcpyAsync(primal, d_P.p, (size_t)B * sizeof(double), cudaMemcpyDeviceToHost, st));
+  TKM_CUDA(cudaMemcpyAsync(gap, d_gap.p, (size_t)B * sizeof(double), cudaMemcpyDeviceToHost, st));
   TKM_CUDA(cudaStreamSynchronize(st));
   return TKM_OK;
 }

@@ -180,6 +180,17 @@ def test_fit_path_and_exact_cv_parity(tkm, name):
     if not degenerate:
         assert np.max(np.abs(cv_mean - cv_o[2])) <= CV_TOL
         assert np.array_equal(best, cv_o[3])                                     # selected lambda identical
+    # reading G22: objective of the non-smoothed problem and its duality-gap certificate, per column
+    if w.loss in (o.LOSS_HINGE, o.LOSS_QUANTILE):
+        P_o, D_o, gap_o = o.duality_gap(spec_o, res, w.y, w.loss)
+        P_g, gap_g = tkm.tkm_path_duality_gap(path, y, foldid)
+        keep = np.array([c not in degenerate for c in range(res.cols["B"])])
+        assert np.max(np.abs(P_g - P_o)[keep] / np.maximum(1.0, np.abs(P_o[keep]))) <= 1e-9
+        assert np.max(np.abs(gap_g - gap_o)[keep]) <= 1e-9 and np.all(gap_g[keep] >= -1e-10)
+        assert np.all(gap_g[keep] <= 2 * res.smooth_final)
+    else:
+        with pytest.raises(tkm.TkmError):
+            tkm.tkm_path_duality_gap(path, y, foldid)
     # S10: coefficients and prediction with the selected lambda of variant 0
     l_best = int(cv_o[3][0])
     c = (0 * (V + 1) + V) * L + l_best
