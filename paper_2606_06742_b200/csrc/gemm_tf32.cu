@@ -20,12 +20,36 @@ __global__ void split_tf32_kernel(const double* __restrict__ src, int64_t lds, i
   (void)rows;
 }
 
+__global__ void split_tf32_kblocked_kernel(const double* __restrict__ src, int64_t lds, int rows, int cols,
+                                           float* __restrict__ hi, float* __restrict__ lo) {
+  const int r = blockIdx.x;
+  const int cpad = ((cols + 31) >> 5) << 5;
+  for (int c = blockIdx.y * blockDim.x + threadIdx.x; c < cpad; c += gridDim.y * blockDim.x) {
+    float h = 0.0f, l = 0.0f;
+    if (c < cols) {
+      const double v = src[(int64_t)r * lds + c];
+      h = to_tf32((float)v);
+      l = to_tf32((float)(v - (double)h));
+    }
+    const int64_t o = ((int64_t)(c >> 5) * rows + r) * 32 + (c & 31);
+    hi[o] = h;
+    lo[o] = l;
+  }
+}
+
 int tf32_bn_of(int cfg) { return cfg == 0 ? 64 : (cfg == 1 ? 128 : 256); }
 
 int split_tf32(const double* src, int64_t lds, int64_t rows, int64_t cols, float* hi, float* lo, int64_t ldo,
                cudaStream_t st) {
   dim3 grid((unsigned)rows, (unsigned)std::min<int64_t>(ceil_div(cols, 256), 64));
   split_tf32_kernel<<<grid, 256, 0, st>>>(src, lds, (int)rows, (int)cols, hi, lo, ldo);
+  TKM_LAUNCH_CHECK();
+  return TKM_OK;
+}
+
+int split_tf32_kblocked(const double* src, int64_t lds, int64_t rows, int64_t cols, float* hi, float* lo, cudaStream_t st) {
+  dim3 grid((unsigned)rows, (unsigned)std::min<int64_t>(ceil_div(cols, 256), 64));
+  split_tf32_kblocked_kernel<<<grid, 256, 0, st>>>(src, lds, (int)rows, (int)cols, hi, lo);
   TKM_LAUNCH_CHECK();
   return TKM_OK;
 }

@@ -32,6 +32,10 @@ struct Tf32Args {
   int p_group_rows;
   int N, M, K;
   int ksplit;   // as in GemmArgs: S > 1 => blockIdx.y = split * n_tiles + n_tile, K-tiles [s KT/S, (s+1) KT/S)
+  // K-blocked operands (thin U, K = n ~ 10^5..10^6): P is stored [K/32][p_blk_rows][32] and every Q_g
+  // [K/32][q_blk_rows][32], so a stage is two contiguous reads instead of one 128-byte piece from each of
+  // several hundred rows that lie megabytes apart.  The maps are then 2-D over [(K/32) blk_rows][32].
+  int kblocked, p_blk_rows, q_blk_rows;
 };
 
 template <int BN_, int STAGES_>
@@ -89,11 +93,13 @@ __global__ void __launch_bounds__(Cfg::THREADS, 1) gemm_tf32x3_kernel(const __gr
         if (kt >= STAGES) mbar_wait(&empty_bar[s], phase);
         mbar_arrive_expect_tx(&full_bar[s], Cfg::STAGE_BYTES);
         uint8_t* st = tiles + (size_t)s * Cfg::STAGE_BYTES;
-        const int x = (kt0 + kt) * TF32_BK;
-        tma_load_2d(st, &g.q_hi[grp], x, m_blk0, &full_bar[s]);
-        tma_load_2d(st + TF32_A_BYTES, &g.q_lo[grp], x, m_blk0, &full_bar[s]);
-        tma_load_2d(st + 2 * TF32_A_BYTES, &g.p_hi, x, prow, &full_bar[s]);
-        tma_load_2d(st + 2 * TF32_A_BYTES + Cfg::B_BYTES, &g.p_lo, x, prow, &full_bar[s]);
+        const int x = g.kblocked ? 0 : (kt0 + kt) * TF32_BK;
+        const int yq = g.kblocked ? (kt0 + kt) * g.q_blk_rows + m_blk0 : m_blk0;
+        const int yp = g.kblocked ? (kt0 + kt) * g.p_blk_rows + prow : prow;
+        tma_load_2d(st, &g.q_hi[grp], x, yq, &full_bar[s]);
+        tma_load_2d(st + TF32_A_BYTES, &g.q_lo[grp], x, yq, &full_bar[s]);
+        tma_load_2d(st + 2 * TF32_A_BYTES, &g.p_hi, x, yp, &full_bar[s]);
+        tma_load_2d(st + 2 * TF32_A_BYTES + Cfg::B_BYTES, &g.p_lo, x, yp, &full_bar[s]);
         if (++s == STAGES) {
           s = 0;
           phase ^= 1;
@@ -175,6 +181,8 @@ struct Tf32StoreEpi {
 int make_tmap_f32(CUtensorMap* out, const float* base, int64_t rows, int64_t cols, int64_t ld, int box_rows);
 int split_tf32(const double* src, int64_t lds, int64_t rows, int64_t cols, float* hi, float* lo, int64_t ldo,
                cudaStream_t st);   // x -> (tf32(x), tf32(x - hi))
+// the same into the K-blocked layout [ceil(cols / 32)][rows][32] (columns beyond `cols` are written as zeros)
+int split_tf32_kblocked(const double* src, int64_t lds, int64_t rows, int64_t cols, float* hi, float* lo, cudaStream_t st);
 int tf32_bn_of(int cfg);           // slots per tile of configuration 0 / 1 / 2 = 64 / 128 / 256
 
 template <class Cfg, class Epi>

@@ -34,6 +34,12 @@
 
 namespace tkm {
 
+// Element (slot row gs, sample m) of the dz operand: row-major [G*B][lddz], or K-blocked [n/32][blk_rows][32]
+// (blk_rows = G*B) when the tcgen05 GEMM-B reads it that way (thin U, large n).
+__device__ __forceinline__ int64_t dz_index(int64_t gs, int m, int64_t lddz, int blk_rows) {
+  return blk_rows ? ((int64_t)(m >> 5) * blk_rows + gs) * 32 + (m & 31) : gs * lddz + m;
+}
+
 // Same function with the divisions hoisted: inv_2s = 1 / (2 smooth) (unused by the smooth losses).
 __device__ __forceinline__ double psi_fast(int loss, double y, double f, double smooth, double inv_2s, double tau) {
   if (loss == TKM_LOSS_HINGE) {
@@ -76,6 +82,7 @@ struct LossEpi {
   float* dz_lo;              //   delta-form GEMM-B (zeta += U^T dz on the tcgen05 tensor cores)
   int64_t lddz;
   double* Fb;                // [G*B][ldz] by gs or NULL: keeps Fbar = U Lam abar for the delta-form GEMM-A
+  int dz_blk_rows;           // 0: dz row-major; G*B: dz K-blocked (dz_index)
   template <class Cfg>
   __device__ __forceinline__ void run(double (&acc)[Cfg::TN][Cfg::TM][2], int n_blk0, int m_blk0, int warp_n,
                                       int warp_m, int lane, int N, int M, int grp, double* scratch) const {
@@ -114,7 +121,7 @@ struct LossEpi {
           const double2 zo = *reinterpret_cast<const double2*>(zrow + m);
           const double d0 = z[0] - zo.x, d1 = (m + 1 < M) ? z[1] - zo.y : 0.0;
           const float h0 = to_tf32((float)d0), h1 = to_tf32((float)d1);
-          const int64_t o = (int64_t)(g0 + slot) * lddz + m;
+          const int64_t o = dz_index(g0 + slot, m, lddz, dz_blk_rows);
           *reinterpret_cast<float2*>(dz_hi + o) = make_float2(h0, h1);
           *reinterpret_cast<float2*>(dz_lo + o) = make_float2(to_tf32((float)(d0 - (double)h0)), to_tf32((float)(d1 - (double)h1)));
         }
@@ -299,6 +306,7 @@ struct FLossEpi {
   int64_t lddz;
   double* gpart;
   int64_t ldpart;
+  int dz_blk_rows;
   __device__ __forceinline__ void chunk(const float (&v)[16], int m, int n0, int N, int M, int grp, double* red,
                                         int lane) const {
     const bool live = m < M;
@@ -342,8 +350,9 @@ struct FLossEpi {
             const double d = z - zov[k];
             Zt[o] = z;
             const float h = to_tf32((float)d);
-            dz_hi[(int64_t)gs * lddz + m] = h;
-            dz_lo[(int64_t)gs * lddz + m] = to_tf32((float)(d - (double)h));
+            const int64_t od = dz_index(gs, m, lddz, dz_blk_rows);
+            dz_hi[od] = h;
+            dz_lo[od] = to_tf32((float)(d - (double)h));
           }
           const double t = warp_sum(z);
           if (lane == 0) red[h0 + k] = t;
@@ -737,6 +746,8 @@ static double curvature_of(tkm_loss loss, double smooth) {
 
 constexpr int KSPLIT_MIN_K = 16384;   // contraction depth from which GEMM-B may be K-split (thin U, large n)
 constexpr int KSPLIT_MAX = 16;
+constexpr int KBLOCK_MIN_K = 8192;   // contraction depth from which the tcgen05 GEMM-B operands are kept K-blocked (no effect
+                                    // at n = 2000, where U^T stays in L2; 2.4x at n = 581012)
 constexpr int DELTA_MIN_LIVE = 48;   // live columns (all groups) below which the delta forms are switched off
 constexpr int POLL_RING = 5;   // ring of poll results: up to POLL_RING - 2 batches may be in flight
 
@@ -897,6 +908,10 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
   // delta-form GEMM-B (tkm_loss_opts.tf32_delta): zeta state, the (hi, lo) increment operand, U^T as (hi, lo)
   const bool delta = opts->tf32_delta != 0;
   const int64_t ldn32 = round_up(n, 32);
+  // the operands of the tcgen05 GEMM-B (U^T and dz, both (hi, lo)) are kept K-blocked, [n/32][rows][32], so that
+  // a pipeline stage is a contiguous read instead of one 128-byte piece per row (profiles/r01f: 2.4x at n = 581012)
+  const bool kblk = delta && n >= KBLOCK_MIN_K;
+  const int dz_blk_rows = kblk ? GB : 0;
   DevBuf Zeta, dz_hi, dz_lo, ut_hi[GEMM_MAX_GROUPS], ut_lo[GEMM_MAX_GROUPS];
   if (delta) {
     TKM_TRY(Zeta.alloc((size_t)GB * ldr * sizeof(double), true, st));
@@ -905,7 +920,10 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
     for (int g = 0; g < G; ++g) {
       TKM_TRY(ut_hi[g].alloc((size_t)r * ldn32 * sizeof(float), false, st));   // padding beyond n is outside the
       TKM_TRY(ut_lo[g].alloc((size_t)r * ldn32 * sizeof(float), false, st));   // tensor maps: never read
-      TKM_TRY(split_tf32(specs[g]->Ut.as<double>(), ldn, r, n, ut_hi[g].as<float>(), ut_lo[g].as<float>(), ldn32, st));
+      if (kblk)
+        TKM_TRY(split_tf32_kblocked(specs[g]->Ut.as<double>(), ldn, r, n, ut_hi[g].as<float>(), ut_lo[g].as<float>(), st));
+      else
+        TKM_TRY(split_tf32(specs[g]->Ut.as<double>(), ldn, r, n, ut_hi[g].as<float>(), ut_lo[g].as<float>(), ldn32, st));
     }
   }
   // K-split GEMM-B (thin U with a long contraction): partial sums [KSPLIT_MAX][G*B][ldr]
@@ -1043,11 +1061,24 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
         const int want = nmax <= 64 ? 0 : (nmax <= 128 ? 1 : 2);
         if (want != tcfg) {
           const int bn = tf32_bn_of(want);
-          TKM_TRY(make_tmap_f32(&targs.p_hi, dz_hi.as<float>(), GB, n, ldn32, bn));
-          TKM_TRY(make_tmap_f32(&targs.p_lo, dz_lo.as<float>(), GB, n, ldn32, bn));
-          for (int g = 0; g < G; ++g) {
-            TKM_TRY(make_tmap_f32(&targs.q_hi[g], ut_hi[g].as<float>(), r, n, ldn32, TF32_BM));
-            TKM_TRY(make_tmap_f32(&targs.q_lo[g], ut_lo[g].as<float>(), r, n, ldn32, TF32_BM));
+          if (kblk) {
+            const int64_t kb = ldn32 / 32;
+            TKM_TRY(make_tmap_f32(&targs.p_hi, dz_hi.as<float>(), kb * GB, 32, 32, bn));
+            TKM_TRY(make_tmap_f32(&targs.p_lo, dz_lo.as<float>(), kb * GB, 32, 32, bn));
+            for (int g = 0; g < G; ++g) {
+              TKM_TRY(make_tmap_f32(&targs.q_hi[g], ut_hi[g].as<float>(), kb * r, 32, 32, TF32_BM));
+              TKM_TRY(make_tmap_f32(&targs.q_lo[g], ut_lo[g].as<float>(), kb * r, 32, 32, TF32_BM));
+            }
+            targs.kblocked = 1;
+            targs.p_blk_rows = GB;
+            targs.q_blk_rows = (int)r;
+          } else {
+            TKM_TRY(make_tmap_f32(&targs.p_hi, dz_hi.as<float>(), GB, n, ldn32, bn));
+            TKM_TRY(make_tmap_f32(&targs.p_lo, dz_lo.as<float>(), GB, n, ldn32, bn));
+            for (int g = 0; g < G; ++g) {
+              TKM_TRY(make_tmap_f32(&targs.q_hi[g], ut_hi[g].as<float>(), r, n, ldn32, TF32_BM));
+              TKM_TRY(make_tmap_f32(&targs.q_lo[g], ut_lo[g].as<float>(), r, n, ldn32, TF32_BM));
+            }
           }
           targs.nslots = nslots.as<int32_t>();
           targs.p_group_rows = B;
@@ -1109,7 +1140,7 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
                       mu.as<double>(), p0->col_nc.as<double>(), p0->col_tau.as<double>(), p0->col_v.as<int32_t>(), B,
                       (int)loss, smooth, smooth > 0.0 ? 1.0 / (2.0 * smooth) : 0.0, Fb.as<double>(), Fp.as<double>(),
                       Zt.as<double>(), ldn, dz_hi.as<float>(),
-                      dz_lo.as<float>(), ldn32, gpart.as<double>(), ldpart};
+                      dz_lo.as<float>(), ldn32, gpart.as<double>(), ldpart, dz_blk_rows};
           TKM_TRY(gemm_tf32_launch(targsF, tcfg, G, fe, st));
           nblkA = (int)ceil_div(n, TF32_BM);
           if (sidx >= 0) {
@@ -1120,7 +1151,7 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
           LossEpi le{(const double*)y, d_fold.as<int32_t>(), col_of_slot.as<int32_t>(), bbar.as<double>(),
                      p0->col_nc.as<double>(), p0->col_tau.as<double>(), p0->col_v.as<int32_t>(), B, (int)loss, smooth,
                      Zt.as<double>(), ldn, gpart.as<double>(), ldpart, dz_on ? dz_hi.as<float>() : nullptr,
-                     dz_on ? dz_lo.as<float>() : nullptr, ldn32, df_on ? Fb.as<double>() : nullptr};
+                     dz_on ? dz_lo.as<float>() : nullptr, ldn32, df_on ? Fb.as<double>() : nullptr, dz_blk_rows};
           TKM_TRY(gemm_f64_launch(argsA, tileA, G, le, st));
           if (sidx >= 0) {
             TKM_CUDA(cudaEventRecord(ev.pev[ring][4 * sidx + 1], st));
