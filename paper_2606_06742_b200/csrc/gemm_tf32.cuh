@@ -34,7 +34,8 @@ struct Tf32Args {
   int ksplit;   // as in GemmArgs: S > 1 => blockIdx.y = split * n_tiles + n_tile, K-tiles [s KT/S, (s+1) KT/S)
   // K-blocked operands (thin U, K = n ~ 10^5..10^6): P is stored [K/32][p_blk_rows][32] and every Q_g
   // [K/32][q_blk_rows][32], so a stage is two contiguous reads instead of one 128-byte piece from each of
-  // several hundred rows that lie megabytes apart.  The maps are then 2-D over [(K/32) blk_rows][32].
+  // several hundred rows that lie kilo- to megabytes apart.  The maps are then 2-D over [(K/32) blk_rows][32].
+  // kblocked: bit 0 = Q blocked, bit 1 = P blocked.
   int kblocked, p_blk_rows, q_blk_rows;
 };
 
@@ -93,13 +94,14 @@ __global__ void __launch_bounds__(Cfg::THREADS, 1) gemm_tf32x3_kernel(const __gr
         if (kt >= STAGES) mbar_wait(&empty_bar[s], phase);
         mbar_arrive_expect_tx(&full_bar[s], Cfg::STAGE_BYTES);
         uint8_t* st = tiles + (size_t)s * Cfg::STAGE_BYTES;
-        const int x = g.kblocked ? 0 : (kt0 + kt) * TF32_BK;
-        const int yq = g.kblocked ? (kt0 + kt) * g.q_blk_rows + m_blk0 : m_blk0;
-        const int yp = g.kblocked ? (kt0 + kt) * g.p_blk_rows + prow : prow;
-        tma_load_2d(st, &g.q_hi[grp], x, yq, &full_bar[s]);
-        tma_load_2d(st + TF32_A_BYTES, &g.q_lo[grp], x, yq, &full_bar[s]);
-        tma_load_2d(st + 2 * TF32_A_BYTES, &g.p_hi, x, yp, &full_bar[s]);
-        tma_load_2d(st + 2 * TF32_A_BYTES + Cfg::B_BYTES, &g.p_lo, x, yp, &full_bar[s]);
+        const int x = (kt0 + kt) * TF32_BK;
+        const bool qb = g.kblocked & 1, pb = g.kblocked & 2;
+        const int xq = qb ? 0 : x, yq = qb ? (kt0 + kt) * g.q_blk_rows + m_blk0 : m_blk0;
+        const int xp = pb ? 0 : x, yp = pb ? (kt0 + kt) * g.p_blk_rows + prow : prow;
+        tma_load_2d(st, &g.q_hi[grp], xq, yq, &full_bar[s]);
+        tma_load_2d(st + TF32_A_BYTES, &g.q_lo[grp], xq, yq, &full_bar[s]);
+        tma_load_2d(st + 2 * TF32_A_BYTES, &g.p_hi, xp, yp, &full_bar[s]);
+        tma_load_2d(st + 2 * TF32_A_BYTES + Cfg::B_BYTES, &g.p_lo, xp, yp, &full_bar[s]);
         if (++s == STAGES) {
           s = 0;
           phase ^= 1;

@@ -934,6 +934,7 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
   // F half (tf32_delta == 2): Fbar / F state, the (hi, lo) step operand, U Lam as (hi, lo), momentum per column
   const bool delta_f = opts->tf32_delta == 2;
   const int64_t ldr32 = round_up(r, 32);
+  const bool kblk_f = delta_f && n >= KBLOCK_MIN_K;   // U Lam (hi, lo) K-blocked: [r/32][n][32]
   DevBuf Fb, Fp, da_hi, da_lo, mu, ul_hi[GEMM_MAX_GROUPS], ul_lo[GEMM_MAX_GROUPS];
   if (delta_f) {
     TKM_TRY(Fb.alloc((size_t)GB * ldn * sizeof(double), true, st));
@@ -944,7 +945,10 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
     for (int g = 0; g < G; ++g) {
       TKM_TRY(ul_hi[g].alloc((size_t)n * ldr32 * sizeof(float), false, st));
       TKM_TRY(ul_lo[g].alloc((size_t)n * ldr32 * sizeof(float), false, st));
-      TKM_TRY(split_tf32(specs[g]->UL.as<double>(), ldr, n, r, ul_hi[g].as<float>(), ul_lo[g].as<float>(), ldr32, st));
+      if (kblk_f)
+        TKM_TRY(split_tf32_kblocked(specs[g]->UL.as<double>(), ldr, n, r, ul_hi[g].as<float>(), ul_lo[g].as<float>(), st));
+      else
+        TKM_TRY(split_tf32(specs[g]->UL.as<double>(), ldr, n, r, ul_hi[g].as<float>(), ul_lo[g].as<float>(), ldr32, st));
     }
   }
   Tf32Args targs, targsF;
@@ -1069,7 +1073,7 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
               TKM_TRY(make_tmap_f32(&targs.q_hi[g], ut_hi[g].as<float>(), kb * r, 32, 32, TF32_BM));
               TKM_TRY(make_tmap_f32(&targs.q_lo[g], ut_lo[g].as<float>(), kb * r, 32, 32, TF32_BM));
             }
-            targs.kblocked = 1;
+            targs.kblocked = 3;
             targs.p_blk_rows = GB;
             targs.q_blk_rows = (int)r;
           } else {
@@ -1088,9 +1092,16 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
             TKM_TRY(make_tmap_f32(&targsF.p_hi, da_hi.as<float>(), GB, r, ldr32, bn));
             TKM_TRY(make_tmap_f32(&targsF.p_lo, da_lo.as<float>(), GB, r, ldr32, bn));
             for (int g = 0; g < G; ++g) {
-              TKM_TRY(make_tmap_f32(&targsF.q_hi[g], ul_hi[g].as<float>(), n, r, ldr32, TF32_BM));
-              TKM_TRY(make_tmap_f32(&targsF.q_lo[g], ul_lo[g].as<float>(), n, r, ldr32, TF32_BM));
+              if (kblk_f) {
+                TKM_TRY(make_tmap_f32(&targsF.q_hi[g], ul_hi[g].as<float>(), (ldr32 / 32) * n, 32, 32, TF32_BM));
+                TKM_TRY(make_tmap_f32(&targsF.q_lo[g], ul_lo[g].as<float>(), (ldr32 / 32) * n, 32, 32, TF32_BM));
+              } else {
+                TKM_TRY(make_tmap_f32(&targsF.q_hi[g], ul_hi[g].as<float>(), n, r, ldr32, TF32_BM));
+                TKM_TRY(make_tmap_f32(&targsF.q_lo[g], ul_lo[g].as<float>(), n, r, ldr32, TF32_BM));
+              }
             }
+            targsF.kblocked = kblk_f ? 1 : 0;
+            targsF.q_blk_rows = (int)n;
             targsF.nslots = nslots.as<int32_t>();
             targsF.p_group_rows = B;
             targsF.M = (int)n;
