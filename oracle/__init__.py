@@ -5,7 +5,7 @@ TEST INFRASTRUCTURE ONLY.  Only `tests/`, `__graft_entry__.smoke()` and
 The product (`paper_2606_06742_b200`, `libtkm.so`) never imports, links or
 executes anything in here, and this package never imports the product: the two
 share no code.  Plain numpy FP64; written from /root/reference/PAPER.md (cited
-as PAPER.md:<line>) with the readings G1..G19 listed in SURVEY.md section 8(c)
+as PAPER.md:<line>) with the readings G1..G19 listed in SURVEY.md section 8(c) (G20..G22: DESIGN.md section 3)
 and DESIGN.md.
 
 Parity pins (tests/test_oracle_*.py, `-m "not gpu"`):
