@@ -38,6 +38,8 @@ struct GemmArgs {
   int N, M, K;                          // N: upper bound of the live rows (the grid covers it)
   int ksplit;                           // <= 1: one CTA contracts all of K; S > 1: blockIdx.y = split * n_tiles + n_tile,
                                         // split s contracts K-tiles [s KT/S, (s+1) KT/S) and the epilogue sees a partial sum
+  int q_blk_rows;                       // 0: Q_g row-major [M][K]; > 0: Q_g K-blocked [K/16][q_blk_rows][16] (map over
+                                        // [(K/16) q_blk_rows][16]): a stage's Q tile is one contiguous read (thin U, K = n large)
 };
 
 // K-split index of this CTA, for epilogues that store partial sums (ksplit as in GemmArgs / Tf32Args)
@@ -186,7 +188,10 @@ __global__ void __launch_bounds__(Cfg::THREADS)
         mbar_arrive_expect_tx(&full_bar[s], Cfg::STAGE_BYTES);
         uint8_t* ps = tiles + (size_t)s * Cfg::STAGE_BYTES;
         tma_load_2d(ps, &g.p_map, (kt0 + kt) * TMA_BOX_K, prow, &full_bar[s]);
-        tma_load_2d(ps + BN * GEMM_ROW_BYTES, &g.q_map[grp], (kt0 + kt) * TMA_BOX_K, m_blk0, &full_bar[s]);
+        if (g.q_blk_rows)
+          tma_load_2d(ps + BN * GEMM_ROW_BYTES, &g.q_map[grp], 0, (kt0 + kt) * g.q_blk_rows + m_blk0, &full_bar[s]);
+        else
+          tma_load_2d(ps + BN * GEMM_ROW_BYTES, &g.q_map[grp], (kt0 + kt) * TMA_BOX_K, m_blk0, &full_bar[s]);
         if (++s == STAGES) {
           s = 0;
           phase ^= 1;
@@ -289,9 +294,13 @@ struct GemmProblem {
   int64_t p_total_rows = 0;    // rows of the stacked P array that may be read (>= G * p_group_rows)
   const double* Q[GEMM_MAX_GROUPS] = {};
   int64_t ldq = 0;
+  bool q_blocked = false;      // Q[g] is K-blocked: [ceil(K / 16)][M][16]
   int G = 1;
   int M = 0, K = 0;
 };
+
+// src [rows][lds] -> dst [ceil(cols / 16)][rows][16] (columns beyond `cols` zero): the K-blocked Q layout
+int kblock_f64(const double* src, int64_t lds, int64_t rows, int64_t cols, double* dst, cudaStream_t st);
 
 // Tile configurations.  The slot dimension is cut into BN = 8 TN WN rows, the output dimension into
 // BM = 8 TM WM.  Wide batches use 64 x 128 tiles (each Q tile feeds 64 slots); narrower ones shrink TN so

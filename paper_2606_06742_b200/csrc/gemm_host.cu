@@ -62,6 +62,20 @@ int make_tmap_f32(CUtensorMap* out, const float* base, int64_t rows, int64_t col
   return TKM_OK;
 }
 
+__global__ void kblock_f64_kernel(const double* __restrict__ src, int64_t lds, int rows, int cols, double* __restrict__ dst) {
+  const int r = blockIdx.x;
+  const int cpad = ((cols + TMA_BOX_K - 1) / TMA_BOX_K) * TMA_BOX_K;
+  for (int c = blockIdx.y * blockDim.x + threadIdx.x; c < cpad; c += gridDim.y * blockDim.x)
+    dst[((int64_t)(c / TMA_BOX_K) * rows + r) * TMA_BOX_K + (c % TMA_BOX_K)] = c < cols ? src[(int64_t)r * lds + c] : 0.0;
+}
+
+int kblock_f64(const double* src, int64_t lds, int64_t rows, int64_t cols, double* dst, cudaStream_t st) {
+  dim3 grid((unsigned)rows, (unsigned)std::min<int64_t>(ceil_div(cols, 256), 64));
+  kblock_f64_kernel<<<grid, 256, 0, st>>>(src, lds, (int)rows, (int)cols, dst);
+  TKM_LAUNCH_CHECK();
+  return TKM_OK;
+}
+
 static int g_forced_cfg = -1;
 int gemm_f64_force_cfg(int cfg) {
   const int old = g_forced_cfg;
@@ -129,7 +143,13 @@ int gemm_f64_make_args(const GemmProblem& pr, const GemmTile& tile, GemmArgs* ou
   if (pr.G < 1 || pr.G > GEMM_MAX_GROUPS) return set_error(TKM_EINVAL, "GEMM: 1..%d groups", GEMM_MAX_GROUPS);
   memset(out, 0, sizeof(*out));
   TKM_TRY(make_tmap_f64(&out->p_map, pr.P, std::max<int64_t>(pr.p_total_rows, 1), pr.K, pr.ldp, tile.BN));
-  for (int g = 0; g < pr.G; ++g) TKM_TRY(make_tmap_f64(&out->q_map[g], pr.Q[g], pr.M, pr.K, pr.ldq, tile.BM));
+  for (int g = 0; g < pr.G; ++g) {
+    if (pr.q_blocked)
+      TKM_TRY(make_tmap_f64(&out->q_map[g], pr.Q[g], ceil_div((int64_t)pr.K, (int64_t)TMA_BOX_K) * pr.M, TMA_BOX_K, TMA_BOX_K, tile.BM));
+    else
+      TKM_TRY(make_tmap_f64(&out->q_map[g], pr.Q[g], pr.M, pr.K, pr.ldq, tile.BM));
+  }
+  out->q_blk_rows = pr.q_blocked ? pr.M : 0;
   out->p_group_rows = pr.p_group_rows;
   out->M = pr.M;
   out->K = pr.K;

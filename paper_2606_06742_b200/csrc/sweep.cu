@@ -746,6 +746,7 @@ static double curvature_of(tkm_loss loss, double smooth) {
 
 constexpr int KSPLIT_MIN_K = 16384;   // contraction depth from which GEMM-B may be K-split (thin U, large n)
 constexpr int KSPLIT_MAX = 16;
+constexpr int KBLOCK_F64_MIN_K = 16384;   // thin U: from this n on, the FP64 GEMM-B reads a K-blocked copy of U^T
 constexpr int KBLOCK_MIN_K = 8192;   // contraction depth from which the tcgen05 GEMM-B operands are kept K-blocked (no effect
                                     // at n = 2000, where U^T stays in L2; 2.4x at n = 581012)
 constexpr int DELTA_MIN_LIVE = 48;   // live columns (all groups) below which the delta forms are switched off
@@ -1004,10 +1005,20 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
   prB.G = G;
   prB.M = (int)r;
   prB.K = (int)n;
+  // thin U with n >= KBLOCK_F64_MIN_K: the FP64 GEMM-B reads a K-blocked copy of U^T (its rows are n * 8 bytes
+  // apart: every 128-byte piece of a stage would come from another page; profiles/r01f)
+  const bool kblk64 = n >= KBLOCK_F64_MIN_K && r < n;
+  DevBuf utb[GEMM_MAX_GROUPS];
   for (int g = 0; g < G; ++g) {
     prA.Q[g] = specs[g]->UL.as<double>();
     prB.Q[g] = specs[g]->Ut.as<double>();
+    if (kblk64) {
+      TKM_TRY(utb[g].alloc((size_t)ceil_div(n, (int64_t)TMA_BOX_K) * r * TMA_BOX_K * sizeof(double), false, st));
+      TKM_TRY(kblock_f64(specs[g]->Ut.as<double>(), ldn, r, n, utb[g].as<double>(), st));
+      prB.Q[g] = utb[g].as<double>();
+    }
   }
+  prB.q_blocked = kblk64;
   GemmArgs argsA, argsB;
   GemmTile tileA{-1, 0, 0}, tileB{-1, 0, 0};
 
