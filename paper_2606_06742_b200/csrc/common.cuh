@@ -6,6 +6,7 @@
 #include <cstdint>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <vector>
 
 #include "../../include/tkm.h"
@@ -45,28 +46,56 @@ inline void count_launch(int64_t k = 1) { launch_counter() += k; }
 inline int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
 inline int64_t ceil_div(int64_t x, int64_t m) { return (x + m - 1) / m; }
 
-// RAII device buffer (cudaMalloc / cudaFree); zero-initialised on request.
+// Keep up to 8 GiB of freed stream-ordered allocations in the device's default pool, so that the temporaries of
+// one sweep are handed to the next without a trip through the driver's page tables.
+inline void pool_keep_once() {
+  static std::once_flag once;
+  std::call_once(once, [] {
+    int dev = 0;
+    cudaMemPool_t pool;
+    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+      uint64_t keep = 8ull << 30;
+      cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    }
+    cudaGetLastError();
+  });
+}
+
+// RAII device buffer (cudaMalloc / cudaFree); zero-initialised on request.  `pooled` buffers are stream-ordered
+// (cudaMallocAsync / cudaFreeAsync on the allocating stream): for temporaries that only that stream touches.
 struct DevBuf {
   void* p = nullptr;
   size_t bytes = 0;
+  bool pooled = false;
+  cudaStream_t pool_st = nullptr;
   DevBuf() = default;
   DevBuf(const DevBuf&) = delete;
   DevBuf& operator=(const DevBuf&) = delete;
   ~DevBuf() { release(); }
   void release() {
-    if (p) cudaFree(p);
+    if (p) {
+      if (pooled)
+        cudaFreeAsync(p, pool_st);
+      else
+        cudaFree(p);
+    }
     p = nullptr;
     bytes = 0;
+    pooled = false;
   }
-  int alloc(size_t nbytes, bool zero, cudaStream_t st) {
+  int alloc(size_t nbytes, bool zero, cudaStream_t st, bool pool = false) {
     release();
     if (nbytes == 0) nbytes = 16;
-    cudaError_t e = cudaMalloc(&p, nbytes);
+    if (pool) pool_keep_once();
+    cudaError_t e = pool ? cudaMallocAsync(&p, nbytes, st) : cudaMalloc(&p, nbytes);
     if (e != cudaSuccess) {
       p = nullptr;
-      return set_error(TKM_ENOMEM, "cudaMalloc(%zu bytes) failed: %s", nbytes, cudaGetErrorString(e));
+      return set_error(TKM_ENOMEM, "%s(%zu bytes) failed: %s", pool ? "cudaMallocAsync" : "cudaMalloc", nbytes,
+                       cudaGetErrorString(e));
     }
     bytes = nbytes;
+    pooled = pool;
+    pool_st = st;
     if (zero) {
       e = cudaMemsetAsync(p, 0, nbytes, st);
       if (e != cudaSuccess) return set_error(TKM_ECUDA, "cudaMemsetAsync failed: %s", cudaGetErrorString(e));
@@ -77,8 +106,11 @@ struct DevBuf {
     release();
     p = o.p;
     bytes = o.bytes;
+    pooled = o.pooled;
+    pool_st = o.pool_st;
     o.p = nullptr;
     o.bytes = 0;
+    o.pooled = false;
   }
   template <class T>
   T* as() const { return reinterpret_cast<T*>(p); }

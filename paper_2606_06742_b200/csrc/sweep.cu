@@ -884,22 +884,22 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
   DevBuf A, Aprev, Abar, Rho, Zt, gpart, d_fold;
   DevBuf col_c, col_s, beta, beta_prev, bbar, rk, kkt, done, iters, iters_round, flags, col_of_slot;
   DevBuf nslots, fin_list, tail_list, counts;
-  TKM_TRY(A.alloc((size_t)GB * ldr * sizeof(double), true, st));
-  TKM_TRY(Aprev.alloc((size_t)GB * ldr * sizeof(double), true, st));
-  TKM_TRY(Abar.alloc((size_t)GB * ldr * sizeof(double), true, st));
-  TKM_TRY(Rho.alloc((size_t)GB * ldr * sizeof(double), true, st));
-  TKM_TRY(Zt.alloc((size_t)GB * ldn * sizeof(double), true, st));
+  TKM_TRY(A.alloc((size_t)GB * ldr * sizeof(double), true, st, true));
+  TKM_TRY(Aprev.alloc((size_t)GB * ldr * sizeof(double), true, st, true));
+  TKM_TRY(Abar.alloc((size_t)GB * ldr * sizeof(double), true, st, true));
+  TKM_TRY(Rho.alloc((size_t)GB * ldr * sizeof(double), true, st, true));
+  TKM_TRY(Zt.alloc((size_t)GB * ldn * sizeof(double), true, st, true));
   const int64_t nblk_max = ceil_div(std::max(n, r), 64);   // smallest BM of any tile configuration
   const int64_t ldpart = round_up(GB, 16);
-  TKM_TRY(gpart.alloc((size_t)nblk_max * ldpart * sizeof(double), true, st));
-  TKM_TRY(d_fold.alloc((size_t)n * sizeof(int32_t), false, st));
+  TKM_TRY(gpart.alloc((size_t)nblk_max * ldpart * sizeof(double), true, st, true));
+  TKM_TRY(d_fold.alloc((size_t)n * sizeof(int32_t), false, st, true));
   TKM_CUDA(cudaMemcpyAsync(d_fold.p, foldid, n * sizeof(int32_t), cudaMemcpyHostToDevice, st));
-  TKM_TRY(col_c.alloc((size_t)B * sizeof(double), true, st));
-  for (DevBuf* b : {&col_s, &beta, &beta_prev, &bbar, &rk, &kkt}) TKM_TRY(b->alloc((size_t)GB * sizeof(double), true, st));
+  TKM_TRY(col_c.alloc((size_t)B * sizeof(double), true, st, true));
+  for (DevBuf* b : {&col_s, &beta, &beta_prev, &bbar, &rk, &kkt}) TKM_TRY(b->alloc((size_t)GB * sizeof(double), true, st, true));
   for (DevBuf* b : {&done, &iters, &iters_round, &flags, &col_of_slot, &fin_list, &tail_list})
-    TKM_TRY(b->alloc((size_t)GB * sizeof(int32_t), true, st));
-  TKM_TRY(nslots.alloc((size_t)GEMM_MAX_GROUPS * sizeof(int32_t), true, st));
-  TKM_TRY(counts.alloc((size_t)GEMM_MAX_GROUPS * 4 * sizeof(int32_t), true, st));
+    TKM_TRY(b->alloc((size_t)GB * sizeof(int32_t), true, st, true));
+  TKM_TRY(nslots.alloc((size_t)GEMM_MAX_GROUPS * sizeof(int32_t), true, st, true));
+  TKM_TRY(counts.alloc((size_t)GEMM_MAX_GROUPS * 4 * sizeof(int32_t), true, st, true));
   if (warm)
     for (int g = 0; g < G; ++g) {
       TKM_CUDA(cudaMemcpyAsync(out[g]->a.p, warm[g]->a.p, (size_t)B * ldr * sizeof(double), cudaMemcpyDeviceToDevice, st));
@@ -915,12 +915,12 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
   const int dz_blk_rows = kblk ? GB : 0;
   DevBuf Zeta, dz_hi, dz_lo, ut_hi[GEMM_MAX_GROUPS], ut_lo[GEMM_MAX_GROUPS];
   if (delta) {
-    TKM_TRY(Zeta.alloc((size_t)GB * ldr * sizeof(double), true, st));
-    TKM_TRY(dz_hi.alloc((size_t)GB * ldn32 * sizeof(float), true, st));
-    TKM_TRY(dz_lo.alloc((size_t)GB * ldn32 * sizeof(float), true, st));
+    TKM_TRY(Zeta.alloc((size_t)GB * ldr * sizeof(double), true, st, true));
+    TKM_TRY(dz_hi.alloc((size_t)GB * ldn32 * sizeof(float), true, st, true));
+    TKM_TRY(dz_lo.alloc((size_t)GB * ldn32 * sizeof(float), true, st, true));
     for (int g = 0; g < G; ++g) {
-      TKM_TRY(ut_hi[g].alloc((size_t)r * ldn32 * sizeof(float), false, st));   // padding beyond n is outside the
-      TKM_TRY(ut_lo[g].alloc((size_t)r * ldn32 * sizeof(float), false, st));   // tensor maps: never read
+      TKM_TRY(ut_hi[g].alloc((size_t)r * ldn32 * sizeof(float), false, st, true));   // padding beyond n is outside the
+      TKM_TRY(ut_lo[g].alloc((size_t)r * ldn32 * sizeof(float), false, st, true));   // tensor maps: never read
       if (kblk)
         TKM_TRY(split_tf32_kblocked(specs[g]->Ut.as<double>(), ldn, r, n, ut_hi[g].as<float>(), ut_lo[g].as<float>(), st));
       else
@@ -931,21 +931,21 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
   const bool ksplit_ok = n >= KSPLIT_MIN_K;
   const int64_t split_stride = (int64_t)GB * ldr;
   DevBuf zpart;
-  if (ksplit_ok) TKM_TRY(zpart.alloc((size_t)KSPLIT_MAX * split_stride * sizeof(double), false, st));
+  if (ksplit_ok) TKM_TRY(zpart.alloc((size_t)KSPLIT_MAX * split_stride * sizeof(double), false, st, true));
   // F half (tf32_delta == 2): Fbar / F state, the (hi, lo) step operand, U Lam as (hi, lo), momentum per column
   const bool delta_f = opts->tf32_delta == 2;
   const int64_t ldr32 = round_up(r, 32);
   const bool kblk_f = delta_f && n >= KBLOCK_MIN_K;   // U Lam (hi, lo) K-blocked: [r/32][n][32]
   DevBuf Fb, Fp, da_hi, da_lo, mu, ul_hi[GEMM_MAX_GROUPS], ul_lo[GEMM_MAX_GROUPS];
   if (delta_f) {
-    TKM_TRY(Fb.alloc((size_t)GB * ldn * sizeof(double), true, st));
-    TKM_TRY(Fp.alloc((size_t)GB * ldn * sizeof(double), true, st));
-    TKM_TRY(da_hi.alloc((size_t)GB * ldr32 * sizeof(float), true, st));
-    TKM_TRY(da_lo.alloc((size_t)GB * ldr32 * sizeof(float), true, st));
-    TKM_TRY(mu.alloc((size_t)GB * sizeof(double), true, st));
+    TKM_TRY(Fb.alloc((size_t)GB * ldn * sizeof(double), true, st, true));
+    TKM_TRY(Fp.alloc((size_t)GB * ldn * sizeof(double), true, st, true));
+    TKM_TRY(da_hi.alloc((size_t)GB * ldr32 * sizeof(float), true, st, true));
+    TKM_TRY(da_lo.alloc((size_t)GB * ldr32 * sizeof(float), true, st, true));
+    TKM_TRY(mu.alloc((size_t)GB * sizeof(double), true, st, true));
     for (int g = 0; g < G; ++g) {
-      TKM_TRY(ul_hi[g].alloc((size_t)n * ldr32 * sizeof(float), false, st));
-      TKM_TRY(ul_lo[g].alloc((size_t)n * ldr32 * sizeof(float), false, st));
+      TKM_TRY(ul_hi[g].alloc((size_t)n * ldr32 * sizeof(float), false, st, true));
+      TKM_TRY(ul_lo[g].alloc((size_t)n * ldr32 * sizeof(float), false, st, true));
       if (kblk_f)
         TKM_TRY(split_tf32_kblocked(specs[g]->UL.as<double>(), ldr, n, r, ul_hi[g].as<float>(), ul_lo[g].as<float>(), st));
       else
@@ -1013,7 +1013,7 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
     prA.Q[g] = specs[g]->UL.as<double>();
     prB.Q[g] = specs[g]->Ut.as<double>();
     if (kblk64) {
-      TKM_TRY(utb[g].alloc((size_t)ceil_div(n, (int64_t)TMA_BOX_K) * r * TMA_BOX_K * sizeof(double), false, st));
+      TKM_TRY(utb[g].alloc((size_t)ceil_div(n, (int64_t)TMA_BOX_K) * r * TMA_BOX_K * sizeof(double), false, st, true));
       TKM_TRY(kblock_f64(specs[g]->Ut.as<double>(), ldn, r, n, utb[g].as<double>(), st));
       prB.Q[g] = utb[g].as<double>();
     }
