@@ -25,6 +25,8 @@ Parity pins (tests/test_oracle_*.py, `-m "not gpu"`):
   C <-> lam   objective scaling                                             (P15)
   platt       zero gradient; scikit-learn's _sigmoid_calibration           (P16)
   gap         0 <= gap = O(delta); weak duality; D <= P*(SVC) <= P          (P17)
+  outer ctl   gap_tol = 0 == fixed schedule; exit level == first level with gap <= gap_tol; exited column ==
+              fixed-schedule fit of that many rounds; P - P*(SVC) <= gap_tol  (P18, reading G23)
 Parity unpinned by the paper (inputs, fixed by SURVEY.md 8(c)/DESIGN.md, not
 results): delta_0, R, tol, maxit, the t3 noise scale, the landmark seed.
 """
@@ -32,7 +34,7 @@ from .gram import gram_rbf
 from .spectral import spectral_setup, Spectral
 from .losses import psi, curvature, nominal_loss, smooth_loss, LOSS_HINGE, LOSS_LOGISTIC, LOSS_QUANTILE, LOSS_DWD
 from .folds import make_folds, splitmix64_stream
-from .path import (column_table, column_constants, fit_column, fit_path, PathResult,
+from .path import (column_table, column_constants, column_gap, fit_column, fit_path, PathResult,
                    smoothing_levels, path_coef)
 from .cv import exact_cv, predict, label_of
 from .nystrom import nystrom_setup, nystrom_landmark_weights

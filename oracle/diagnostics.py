@@ -39,6 +39,7 @@ def duality_gap(spec, res, y, loss):
         M, nc, lam = cols["M"][:, c], cols["n_c"][c], cols["lam"][c]
         tau = None if np.isnan(cols["tau"][c]) else float(cols["tau"][c])
         P[c] = float(np.sum(M * nominal_loss(loss, y, f, tau))) / nc + lam * quad
-        dual_var = -psi(loss, y, f, res.smooth_final, tau)   # hinge: y_j theta_j ; check loss: s_j
+        smooth = res.smooth_final if res.smooth_col is None else float(res.smooth_col[c])   # the column's own level (G23)
+        dual_var = -psi(loss, y, f, smooth, tau)             # hinge: y_j theta_j ; check loss: s_j
         D[c] = float(np.sum(M * dual_var * y)) / nc - lam * quad
     return P, D, P - D

@@ -168,15 +168,29 @@ def test_kkt_of_every_path_solution(loss, taus):
         else:
             assert np.all(y * w2 >= -1e-9) and np.all(y * w2 <= 1 + 1e-9)
         assert np.all(np.abs(alpha[M == 0]) * 2 * lam * n_c < 1e-9)    # P8: held-out alpha = 0
-    # column mode and batched mode reach the same point
+
+
+@pytest.mark.parametrize("loss,taus", [(LOSS_HINGE, ()), (LOSS_LOGISTIC, ()), (LOSS_QUANTILE, (0.3, 0.8))])
+def test_column_mode_and_batched_mode_agree_on_every_column(loss, taus):
+    """fit_path (the mode the GPU parity tests call) against fit_column (Algorithm 1 column by column, mat-vecs):
+    every column of a small grid, both at tol = 1e-13, to the 1e-10 coefficient bar the parity tests use."""
+    X, y, K, spec, foldid = _problem(loss, n=48)
+    lambdas = wl.lambda_grid(0, -3, 4)
+    V = 4
+    res = o.fit_path(spec, y, loss, lambdas, foldid, V, taus=taus, smooth0=1.0, eta=0.125, rounds=3,
+                     tol=1e-13, maxit=400000)
+    assert res.flags.sum() == 0
+    cols = res.cols
     levels = o.smoothing_levels(loss, 1.0, 0.125, 3)
-    for c in (0, cols["B"] // 2, cols["B"] - 1):
+    for c in range(cols["B"]):
         tau = cols["tau"][c] if loss == LOSS_QUANTILE else None
-        a, b0, *_ = o.fit_column(spec, y, loss, levels, cols["lam"][c], cols["M"][:, c], tau=tau,
-                                 tol=1e-12, maxit=100000)
+        a, b0, it, kkt, flag = o.fit_column(spec, y, loss, levels, cols["lam"][c], cols["M"][:, c], tau=tau,
+                                            tol=1e-13, maxit=400000)
+        assert flag == 0
         al, al2 = spec.U @ a, spec.U @ res.a[:, c]
-        assert np.linalg.norm(al - al2) <= 1e-8 * np.linalg.norm(al2)
-        assert abs(b0 - res.beta0[c]) < 1e-8
+        assert np.linalg.norm(al - al2) <= 1e-10 * np.linalg.norm(al2), c
+        assert abs(b0 - res.beta0[c]) <= 1e-10 * max(1.0, abs(b0)), c
+        assert abs(it - res.iters[c]) <= max(3, 0.05 * it)     # same arithmetic up to the summation order of BLAS
 
 
 def test_logistic_against_independent_newton():
@@ -313,3 +327,130 @@ def test_dwd_against_scipy_minimiser():
     best = minimize(lambda x: o.objective(K, y, x[1:], x[0], lam, LOSS_DWD, mask, None), np.zeros(n + 1),
                     method="BFGS", options=dict(gtol=1e-10, maxiter=5000))
     assert mine <= best.fun + 1e-12 and best.fun - mine < 1e-7
+
+
+# ---------------------------------------------------------------- warm-start rounds (an input, not a result)
+def test_warm_tol_does_not_move_the_result():
+    """Rounds 0..R-2 only produce starting points: a loose warm_tol changes the iteration counts, not the
+    minimiser at the final level (both stopped at the same tol)."""
+    X, y, K, spec, foldid = _problem(LOSS_HINGE, n=60)
+    lambdas = wl.lambda_grid(0, -3, 4)
+    r0 = o.fit_path(spec, y, LOSS_HINGE, lambdas, foldid, 4, rounds=4, tol=1e-13, maxit=400000)
+    r1 = o.fit_path(spec, y, LOSS_HINGE, lambdas, foldid, 4, rounds=4, tol=1e-13, maxit=400000, warm_tol=1e-3)
+    assert r0.flags.sum() == 0 and r1.flags.sum() == 0
+    assert r1.iters.sum() < r0.iters.sum()
+    for c in range(r0.cols["B"]):
+        a0, a1 = spec.U @ r0.a[:, c], spec.U @ r1.a[:, c]
+        assert np.linalg.norm(a0 - a1) <= 1e-10 * np.linalg.norm(a0)
+
+
+# ---------------------------------------------------------------- P18: outer control (reading G23, PAPER.md:220-222)
+def test_outer_control_gap_tol_zero_is_the_fixed_schedule():
+    X, y, K, spec, foldid = _problem(LOSS_HINGE, n=48)
+    lambdas = wl.lambda_grid(0, -3, 3)
+    r0 = o.fit_path(spec, y, LOSS_HINGE, lambdas, foldid, 4, rounds=3, tol=1e-12, maxit=200000)
+    r1 = o.fit_path(spec, y, LOSS_HINGE, lambdas, foldid, 4, rounds=3, tol=1e-12, maxit=200000, gap_tol=0.0)
+    assert np.array_equal(r0.a, r1.a) and np.array_equal(r0.beta0, r1.beta0) and np.all(r1.level == 2)
+
+
+@pytest.mark.parametrize("loss,taus,warm_tol", [(LOSS_HINGE, (), None), (LOSS_HINGE, (), 1e-3),
+                                                (LOSS_QUANTILE, (0.2, 0.7), 1e-3)])
+def test_outer_control_exits_at_the_first_level_that_certifies_the_gap(loss, taus, warm_tol):
+    """Every column ends on the FIRST level k whose warm-started iterate certifies gap <= gap_tol (or on the
+    cap R-1), its coefficients are the minimiser at that level (== the fixed schedule with k+1 rounds), and the
+    certificate holds for the returned solution."""
+    X, y, K, spec, foldid = _problem(loss, n=56)
+    lambdas = wl.lambda_grid(0, -3, 4)
+    V, R, gap_tol = 4, 4, 3e-3
+    res = o.fit_path(spec, y, loss, lambdas, foldid, V, taus=taus, rounds=R, tol=1e-12, maxit=400000,
+                     warm_tol=warm_tol, gap_tol=gap_tol)
+    assert res.flags.sum() == 0
+    assert len(set(res.level.tolist())) >= 2, "choose gap_tol so that the test sees several exit levels"
+    fixed = {k: o.fit_path(spec, y, loss, lambdas, foldid, V, taus=taus, rounds=k + 1, tol=1e-12, maxit=400000)
+             for k in range(R)}
+    gaps = {k: o.duality_gap(spec, fixed[k], y, loss)[2] for k in range(R)}
+    P, D, gap = o.duality_gap(spec, res, y, loss)
+    for c in range(res.cols["B"]):
+        k = int(res.level[c])
+        ref = fixed[k]
+        a0, a1 = spec.U @ ref.a[:, c], spec.U @ res.a[:, c]
+        assert np.linalg.norm(a0 - a1) <= 1e-9 * max(np.linalg.norm(a0), 1e-300), (c, k)
+        assert abs(gap[c] - gaps[k][c]) <= 1e-9
+        if k < R - 1:
+            assert gap[c] <= gap_tol + 1e-9
+        # no earlier level's minimiser carries the certificate; with warm_tol the screen runs on an iterate that is
+        # only within warm_tol of that minimiser, so a near miss may stay on the schedule (conservative, still valid)
+        for j in range(k):
+            assert gaps[j][c] > gap_tol * (1.0 if warm_tol is None else 0.7), (c, j)
+    # column mode takes the same decisions
+    levels = o.smoothing_levels(loss, 1.0, 0.125, R)
+    for c in (0, res.cols["B"] // 3, res.cols["B"] - 1):
+        tau = res.cols["tau"][c] if loss == LOSS_QUANTILE else None
+        a, b0, it, kkt, flag, lev = o.fit_column(spec, y, loss, levels, res.cols["lam"][c], res.cols["M"][:, c],
+                                                 tau=tau, tol=1e-12, maxit=400000, warm_tol=warm_tol,
+                                                 gap_tol=gap_tol, want_level=True)
+        assert lev == res.level[c] and abs(it - res.iters[c]) <= max(3, 0.05 * it)
+        assert np.linalg.norm(a - res.a[:, c]) <= 1e-10 * max(np.linalg.norm(a), 1e-300)
+
+
+def test_outer_control_certificate_against_svc():
+    """The exit test certifies the ORIGINAL problem: P(returned alpha) - P*(scikit-learn SVC dual solver) <= gap_tol
+    for every column that left the schedule early (C = 1/(2 n lambda))."""
+    from sklearn.svm import SVC
+    n = 72
+    X, y, K, spec, _ = _problem(LOSS_HINGE, n=n)
+    foldid = np.zeros(n, dtype=np.int64)
+    foldid[::2] = 1
+    lambdas = np.array([3e-2, 3e-3])
+    gap_tol = 5e-3
+    res = o.fit_path(spec, y, LOSS_HINGE, lambdas, foldid, 2, rounds=5, tol=1e-12, maxit=400000, warm_tol=1e-3,
+                     gap_tol=gap_tol)
+    early = 0
+    for l, lam in enumerate(lambdas):
+        c = 2 * len(lambdas) + l                          # v = V: the full-data column
+        svc = SVC(C=1.0 / (2 * n * lam), kernel="precomputed", tol=1e-10).fit(K, y)
+        alpha_qp = np.zeros(n)
+        alpha_qp[svc.support_] = svc.dual_coef_[0]
+        p_star = o.objective(K, y, alpha_qp, float(svc.intercept_[0]), lam, LOSS_HINGE, nominal=True)
+        alpha, b0 = o.path_coef(spec, res, c)
+        p = o.objective(K, y, alpha, b0, lam, LOSS_HINGE, nominal=True)
+        assert p >= p_star - 1e-8
+        if res.level[c] < 4:
+            early += 1
+            assert p - p_star <= gap_tol + 1e-8
+    assert early >= 1
+
+
+def test_outer_control_huge_gap_tol_stops_after_the_first_round():
+    X, y, K, spec, foldid = _problem(LOSS_HINGE, n=40)
+    lambdas = wl.lambda_grid(0, -2, 3)
+    res = o.fit_path(spec, y, LOSS_HINGE, lambdas, foldid, 4, rounds=4, tol=1e-12, maxit=200000, gap_tol=10.0)
+    one = o.fit_path(spec, y, LOSS_HINGE, lambdas, foldid, 4, rounds=1, tol=1e-12, maxit=200000)
+    assert np.all(res.level == 0) and np.array_equal(res.a, one.a)
+
+
+# ---------------------------------------------------------------- warm starts along lambda (PAPER.md:236), measured
+def test_lambda_warm_start_against_delta_warm_start():
+    """DESIGN.md section 8 keeps warm starts along delta and batches all lambda at once.  Measured here on the
+    oracle: the last smoothing round started from the converged NEIGHBOUR-lambda solution (the paper's
+    lambda-sequential order) needs at least as many iterations, summed over the small-lambda half of
+    the grid, as started from the same column's previous smoothing round."""
+    w = wl.config0(n=300, p=10, L=12, seed=1000)
+    K = o.gram_rbf(w.X, float(w.sigmas[0]))
+    spec = o.spectral_setup(K)
+    mask = np.ones(w.n)
+    levels = o.smoothing_levels(LOSS_HINGE, 1.0, 0.125, 4)
+    it_delta, it_lambda = [], []
+    prev = None
+    for l, lam in enumerate(w.lambdas):
+        aw, bw, *_ = o.fit_column(spec, w.y, LOSS_HINGE, levels[:-1], lam, mask, tol=1e-3, maxit=100000)
+        a, b, it, *_ = o.fit_column(spec, w.y, LOSS_HINGE, levels[-1:], lam, mask, tol=1e-10, maxit=200000, a0=aw, b0=bw)
+        it_delta.append(it)
+        if prev is not None:
+            _, _, it2, *_ = o.fit_column(spec, w.y, LOSS_HINGE, levels[-1:], lam, mask, tol=1e-10, maxit=200000,
+                                         a0=prev[0], b0=prev[1])
+            it_lambda.append(it2)
+        prev = (a, b)
+    half = len(w.lambdas) // 2
+    print("iterations of the last round, delta warm start: %s; lambda warm start: %s" % (it_delta[1:], it_lambda))
+    assert sum(it_lambda[half - 1:]) >= 0.9 * sum(it_delta[half:])
