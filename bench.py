@@ -1,26 +1,37 @@
 #!/usr/bin/env python
 """bench.py -- the driver's benchmark contract for libtkm.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--dtype f64]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
 
-Metric (BASELINE.json): (lambda x fold) path fits per second on BASELINE.json configs[1]
-(smoothed-hinge kernel SVM, n=2000, p=50, 5 folds, 50 lambdas x 5 sigma values).  One STEP is one pass
-of the whole hot path over that workload: for each of the 5 bandwidths  S1 Gram -> S2 spectral setup
--> S9 exact CV, with the S3-S8 sweeps of the 5 bandwidths (50 x (5+1) columns each) run together as groups
-of one launch sequence (tkm_fit_path_multi), and S10 coefficients in the e2e leg.
-`value` = columns fitted per second by the whole job, X and y resident in HBM before the timed
-region; `e2e` = the same through tkm_train_tune_host from pinned HOST buffers.
+Metric (BASELINE.json): (lambda x fold) path fits per second.
 
-N > 1 (torchrun): the path has no exchange step -- every rank runs the same-size workload on its own
-seeded data set (independent problems, "weak" scaling); the only communication is the barrier and the
-max-over-ranks of the device time.
+Default line = BASELINE.json configs[1] (smoothed-hinge kernel SVM, n=2000, p=50, 5 folds, 50 lambdas x 5 sigma
+values), the configuration the metric is quoted on.  One STEP is one pass of the whole hot path over that
+workload: for each of the 5 bandwidths  S1 Gram -> S2 spectral setup -> S9 exact CV, with the S3-S8 sweeps of
+the 5 bandwidths (50 x (5+1) columns each) run together as groups of one launch sequence (tkm_fit_path_multi),
+and S10 coefficients in the e2e leg.  `value` = columns fitted per second by the WHOLE step (setup included), X
+and y resident in HBM before the timed region; `fits_per_s_sweep_only` = SURVEY.md 8(d)'s B / t_sweep; `e2e` =
+the same through tkm_train_tune_host from pinned HOST buffers.  The same JSON line carries `large_config`: one
+pass of BASELINE.json configs[3] (the largest full-kernel single-GPU configuration, n = 20000, 900 columns) with
+its own stage times, roofline and clocks (outside the timed region of `value`; `--no-large` skips it).
 
-`--impl reference` times the FP64 CPU oracle (oracle/, test infrastructure) on a bounded sample of
-the same workload on the host cores; rank 0 only.
+Other workloads (`--workload`, one GPU, one JSON line each with the same keys):
+  config2 | config3 | config4      BASELINE.json configs[2..4] at full size
+  nystrom_covtype | nystrom_mnist8m46   Nystrom at the row counts of the paper's Table 4
+  loo_config1                      leave-one-out form of Algorithm 1 (V = n) on configs[1]'s data (8(f) N2)
+  narrow_config2 | narrow_config3  configs[2]/[3] with `--narrow-L` in {1,2,4} lambdas: the HBM-bound narrow batch
+
+N > 1 (torchrun): the path has no exchange step -- every rank runs the same-size workload on its own seeded
+data set (independent problems, "weak" scaling); the only communication is the barrier and the max-over-ranks
+of the device time.
+
+`--impl reference` times the FP64 CPU oracle (oracle/, test infrastructure) on a bounded sample of the default
+workload on the host cores; rank 0 only.
 """
 from __future__ import annotations
 
 import argparse
+import csv
 import json
 import os
 import subprocess
@@ -38,27 +49,31 @@ import workloads as wl  # noqa: E402
 
 METRIC = "lambda_x_fold_path_fits_per_s"
 UNIT = "fits/s"
-STOP_TOL = {"f64": 1e-12, "f32": 1e-6}
+STOP_TOL = {"f64": 1e-12}                   # DESIGN.md "Tolerances" (the default line); --tol for the other workloads
 MAXIT = 200000
 # Stop tolerance of the smoothing rounds 0..R-2, which only produce warm starts for the last round (the
-# result is the minimiser at the final smoothing level, whatever the start): DESIGN.md "Schedule".
+# result is the minimiser at the final smoothing level, whatever the start): DESIGN.md "Schedule".  The oracle
+# arm uses the same value (oracle.fit_path(warm_tol=...)).
 WARM_TOL = 1e-3
-# Delta form of the U^T contraction (tkm_loss_opts.tf32_delta = 1): zeta advances by 3xTF32 increments on the
-# tcgen05 tensor cores, with the exact FP64 DMMA contraction and the stop test on the last iteration of every
-# 16-iteration batch and in the narrow tail.  Same fixed point and the same 1e-10 parity bar as the all-FP64
-# sweep.  Mode 2 (both contractions) is 4 % faster still at n = 2000 and 3.2x at n = 20000, but
-# it makes a bandwidth-bound tcgen05 kernel the dominant one; mode 1 keeps the FP64 DMMA GEMM dominant.
-TF32_DELTA = 1
+# Delta form of the contractions (tkm_loss_opts.tf32_delta): the FP64 state advances by 3xTF32
+# increments on the tcgen05 tensor cores, with exact FP64 DMMA contractions and the stop test on the last iteration
+# of every 16-iteration batch and in the narrow tail.  Same fixed point and the same 1e-10 parity bar as the
+# all-FP64 sweep.  This is how the "fp32" configurations of BASELINE.json run: FP64 state + 3xTF32 increments.
+TF32_DELTA = 1           # default line (configs[1])
+TF32_DELTA_LARGE = 2     # configs[2..4], Nystrom, leave-one-out
 # nominal dense tensor ratios to bf16 (B200_PROFILING.md / B300_MICROARCH.md tables): FP64 45 TF,
 # TF32 1125 TF, bf16 2250 TF.  3xTF32 does three MMAs per useful one.
 NOMINAL_RATIO = {"f64": 45.0 / 2250.0, "f32": (1125.0 / 2250.0) / 3.0}
-# dram bytes per launch of the dominant kernel from the committed ncu --set full capture
-# (profiles/): filled in by hand after each capture, None until one exists.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 218.0e6   # profiles/r01c: full-width launch, dram read + write
-NCU_TRAFFIC_TF32_BYTES_PER_LAUNCH = 271.0e6  # profiles/r01e: tcgen05 ZetaEpi kernel, full-width launch
+DMMA_FLOP_PER_CLK_SM = 128.0     # DMMA.8x8x4: 4 per 16 clocks per SM = 128 flop/clk/SM
+N_SM = 148
+# dram bytes per launch of the kernels, from committed `ncu --set full` captures: profiles/traffic.csv
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "traffic.csv")
 # columns of the bounded CPU sample: all V+1 hold-out settings x these lambda indices, one sigma
 CPU_SAMPLE_LAMBDA_IDX = (0, 12, 24, 36, 49)
 CPU_SAMPLE_SIGMA_IDX = 2
+FAMILY = ["gemm_f64_tma_kernel GEMM-A (FP64 DMMA, loss epilogue)", "gemm_f64_tma_kernel GEMM-B (FP64 DMMA, spectral epilogue)",
+          "gemm_tf32x3_kernel GEMM-A (tcgen05 3xTF32 delta form, loss epilogue)",
+          "gemm_tf32x3_kernel GEMM-B (tcgen05 3xTF32 delta form, spectral epilogue)"]
 
 
 def peaks():
@@ -68,6 +83,16 @@ def peaks():
         return dict(hbm=d["hbm_gbs"], bf16_burst=d["bf16_tflops"], bf16_sus=d["bf16_tflops_sustained"],
                     src="measured")
     return dict(hbm=6650.0, bf16_burst=1590.0, bf16_sus=1400.0, src="fallback")
+
+
+def traffic_table():
+    """kernel key -> (dram bytes per launch, source) from profiles/traffic.csv (written from ncu captures)."""
+    out = {}
+    if os.path.exists(TRAFFIC_CSV):
+        with open(TRAFFIC_CSV) as f:
+            for row in csv.DictReader(ln for ln in f if not ln.startswith("#")):
+                out[row["key"]] = (float(row["dram_bytes_per_launch"]), row["source"])
+    return out
 
 
 class ClockSampler:
@@ -121,9 +146,10 @@ class ClockSampler:
 
 
 # ----------------------------------------------------------------------------------------- oracle arm
-def oracle_sample_step(w, want_all=False):
+def oracle_sample_step(w):
     """One bounded sample of the workload on the CPU oracle: one sigma, 5 lambdas x (V+1) columns,
-    Gram + eigh + path + exact CV.  Returns (#columns fitted, seconds)."""
+    Gram + eigh + path + exact CV, same stop and warm-start tolerances as the GPU arm.
+    Returns (#columns fitted, seconds, column-iterations)."""
     import oracle as o
     t0 = time.perf_counter()
     sigma = float(w.sigmas[CPU_SAMPLE_SIGMA_IDX])
@@ -133,7 +159,7 @@ def oracle_sample_step(w, want_all=False):
     L, V = w.L, w.V
     cols = [v * L + l for v in range(V + 1) for l in CPU_SAMPLE_LAMBDA_IDX if l < L]
     res = o.fit_path(spec, w.y, w.loss, w.lambdas, foldid, V, taus=w.taus, smooth0=w.smooth0, eta=w.eta,
-                     rounds=w.rounds, tol=STOP_TOL["f64"], maxit=MAXIT, columns=cols)
+                     rounds=w.rounds, tol=STOP_TOL["f64"], maxit=MAXIT, columns=cols, warm_tol=WARM_TOL)
     o.exact_cv(spec, res, w.y, foldid, w.loss, w.taus)
     return len(cols), time.perf_counter() - t0, int(res.iters.sum())
 
@@ -144,6 +170,16 @@ def blas_threads():
         return max([p.get("num_threads", 1) for p in threadpool_info()] or [1])
     except Exception:
         return os.cpu_count() or 1
+
+
+def sample_text(w, ncol, secs=None, its=None):
+    s = ("sigma index %d, lambda indices %s x %d hold-out settings = %d of %d columns per step, full n; Gram + eigh + "
+         "path + exact CV; same stop / warm-start tolerances as the GPU arm; the 5 sampled lambdas span the grid "
+         "evenly, so the sample averages more iterations per column than the full grid (about 1.5x: a skew against "
+         "the oracle)" % (CPU_SAMPLE_SIGMA_IDX, list(CPU_SAMPLE_LAMBDA_IDX), w.V + 1, ncol, w.B * len(w.sigmas)))
+    if secs is not None:
+        s += "; %.1f s, %d column-iterations" % (secs, its)
+    return s
 
 
 def run_reference(args, w, rank):
@@ -158,31 +194,313 @@ def run_reference(args, w, rank):
         fits += c
     dt = time.perf_counter() - t0
     val = fits / dt
-    sample = ("sigma index %d, lambda indices %s x %d hold-out settings = %d of %d columns per step, "
-              "full n; Gram + eigh + path + exact CV" % (CPU_SAMPLE_SIGMA_IDX, list(CPU_SAMPLE_LAMBDA_IDX),
-                                                        w.V + 1, fits // max(args.steps, 1), w.B * len(w.sigmas)))
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1),
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-            "data": "synthetic", "config": workload_config(w, "f64", warm_tol=STOP_TOL["f64"]),
+            "data": "synthetic", "config": workload_config(w),
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
-                             "sample": sample},
+                             "sample": sample_text(w, fits // max(args.steps, 1))},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
 
 
-def workload_config(w, dtype, warm_tol=None):
+def workload_config(w):
+    """The workload as both arms run it (the GPU-only launch knobs are in `launch_config`)."""
     return {"workload": "BASELINE.json configs[1]: smoothed-hinge kernel SVM, n=%d, p=%d, %d folds, %d lambdas "
-                        "1e2..1e-5 x %d sigma (median x {0.25,0.5,1,2,4}), delta 1 -> 1/512 in %d rounds, %s"
-                        % (w.n, w.p, w.V, w.L, len(w.sigmas), w.rounds, dtype),
+                        "1e2..1e-5 x %d sigma (median x {0.25,0.5,1,2,4}), delta 1 -> 1/512 in %d rounds, f64"
+                        % (w.n, w.p, w.V, w.L, len(w.sigmas), w.rounds),
             "n": w.n, "p": w.p, "folds": w.V, "lambdas": w.L, "sigmas": len(w.sigmas),
-            "columns_per_step": w.B * len(w.sigmas), "stop_tol": STOP_TOL[dtype], "warm_start_rounds_tol": WARM_TOL if warm_tol is None else warm_tol,
-            "tf32_delta": TF32_DELTA if warm_tol is None else 0, "maxit": MAXIT,
+            "columns_per_step": w.B * len(w.sigmas), "stop_tol": STOP_TOL["f64"], "warm_start_rounds_tol": WARM_TOL,
+            "maxit": MAXIT, "value_is": "columns / whole step (Gram + eigendecompositions + sweep + exact CV); "
+                                        "fits_per_s_sweep_only = columns / sweep (SURVEY.md 8(d))",
             "l2": "flushed between steps (256 MiB memset)", "parallelism": "independent replicas, no collective"}
 
 
-# ----------------------------------------------------------------------------------------- CUDA arm
+# ----------------------------------------------------------------------------------------- roofline helpers
+def tensor_peaks(pk, sm_mhz):
+    """Peaks a contraction is reported against.  `contract` = measured bf16 sustained x nominal ratio (the
+    contract's rule: another dtype's measured peak x the guide's ratio); `issue` = DMMA issue ceiling at the sampled
+    SM clock."""
+    mhz = sm_mhz if sm_mhz else 1965.0
+    return {"f64_contract": pk["bf16_sus"] * NOMINAL_RATIO["f64"],
+            "f64_issue": DMMA_FLOP_PER_CLK_SM * N_SM * mhz * 1e6 / 1e12,
+            "tf32x3_contract": pk["bf16_sus"] * NOMINAL_RATIO["f32"],
+            "src": "%s bf16 sustained %.1f TF/s" % (pk["src"], pk["bf16_sus"])}
+
+
+def library_probes(tkm):
+    """Measured dense peaks on this box, this process: cuBLAS DGEMM and cuBLAS TF32 (torch.matmul, 8192^3, best
+    of 5), and the library's own DMMA kernel through tkm_gemm_probe at the same shape."""
+    import torch
+    out = {}
+    N = 8192
+
+    def best_ms(fn, reps=5):
+        fn()
+        torch.cuda.synchronize()
+        best = 1e30
+        for _ in range(reps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            fn()
+            e1.record()
+            e1.synchronize()
+            best = min(best, e0.elapsed_time(e1))
+        return best
+
+    a = torch.randn(N, N, device="cuda", dtype=torch.float64)
+    b = torch.randn(N, N, device="cuda", dtype=torch.float64)
+    c = torch.empty_like(a)
+    out["cublas_dgemm_tflops"] = 2.0 * N ** 3 / (best_ms(lambda: torch.matmul(a, b, out=c)) * 1e-3) / 1e12
+    del a, b, c
+    old = torch.backends.cuda.matmul.allow_tf32
+    torch.backends.cuda.matmul.allow_tf32 = True
+    a = torch.randn(N, N, device="cuda", dtype=torch.float32)
+    b = torch.randn(N, N, device="cuda", dtype=torch.float32)
+    c = torch.empty_like(a)
+    out["cublas_tf32_tflops"] = 2.0 * N ** 3 / (best_ms(lambda: torch.matmul(a, b, out=c)) * 1e-3) / 1e12
+    torch.backends.cuda.matmul.allow_tf32 = old
+    del a, b, c
+    torch.cuda.empty_cache()
+    out["tkm_dmma_probe_tflops"] = 2.0 * N ** 3 / (tkm.tkm_gemm_probe(-1, 1, N, N, N, iters=3) * 1e-3) / 1e12
+    out["shape"] = "8192^3, best of 5 (cuBLAS through torch.matmul: probes only, never on the product path)"
+    return out
+
+
+def family_rooflines(prof, tp, traffic, probes=None):
+    """One roofline object per kernel family with sampled launches.  prof: dict(ms, flops, launches) arrays of 4."""
+    out = []
+    for i in range(4):
+        nl = int(prof["launches"][i])
+        if nl == 0:
+            continue
+        ms, fl = float(prof["ms"][i]), float(prof["flops"][i])
+        ach = (fl / 1e12) / (ms / 1e3) if ms > 0 else 0.0
+        f64 = i < 2
+        peak = tp["f64_contract"] if f64 else tp["tf32x3_contract"]
+        tr = traffic.get("fam%d" % i)
+        d = {"bound": "tensor", "kernel": FAMILY[i], "achieved": ach, "peak": peak, "unit": "TFLOP/s",
+             "frac": ach / peak, "traffic": tr[0] if tr else None, "traffic_source": tr[1] if tr else None,
+             "peak_source": tp["src"] + (" x nominal f64/bf16 ratio %.4f" % NOMINAL_RATIO["f64"] if f64 else
+                                         " x nominal tf32/bf16 ratio 0.5 / 3 MMAs per useful product"),
+             "sampled_launches": nl, "avg_launch_ms": ms / nl, "avg_flops_per_launch": fl / nl, "sampled_ms": ms}
+        if f64:
+            d["peak_dmma_issue"] = tp["f64_issue"]
+            d["frac_of_issue"] = ach / tp["f64_issue"]
+        if probes:
+            pm = probes["cublas_dgemm_tflops"] if f64 else probes["cublas_tf32_tflops"] / 3.0
+            d["peak_measured"] = pm
+            d["frac_of_measured"] = ach / pm
+            d["peak_measured_source"] = ("cuBLAS DGEMM 8192^3 on this box" if f64 else
+                                         "cuBLAS TF32 GEMM 8192^3 on this box / 3 MMAs per useful product")
+        out.append(d)
+    return out
+
+
+def merge_families(fams, idx):
+    """Sum families (e.g. DMMA GEMM-A + GEMM-B = the FP64 kernel) into one roofline object."""
+    sel = [f for f in fams if FAMILY.index(f["kernel"]) in idx]
+    if not sel:
+        return None
+    ms = sum(f["sampled_ms"] for f in sel)
+    fl = sum(f["avg_flops_per_launch"] * f["sampled_launches"] for f in sel)
+    nl = sum(f["sampled_launches"] for f in sel)
+    d = dict(max(sel, key=lambda f: f["sampled_ms"]))
+    ach = fl / 1e12 / (ms / 1e3)
+    d.update(kernel=" + ".join(f["kernel"] for f in sel), achieved=ach, frac=ach / d["peak"], sampled_launches=nl,
+             avg_launch_ms=ms / nl, avg_flops_per_launch=fl / nl, sampled_ms=ms)
+    if "peak_dmma_issue" in d:
+        d["frac_of_issue"] = ach / d["peak_dmma_issue"]
+    if "peak_measured" in d:
+        d["frac_of_measured"] = ach / d["peak_measured"]
+    return d
+
+
+def time_weighted(prof2, tp):
+    """All launches of one sweep (profile = 2): useful flops the device counted / total kernel time, per family."""
+    out = {}
+    for name, idx, peak, issue in (("fp64_dmma", (0, 1), tp["f64_contract"], tp["f64_issue"]),
+                                   ("tcgen05_3xtf32", (2, 3), tp["tf32x3_contract"], None)):
+        ms = float(sum(prof2["ms"][i] for i in idx))
+        fl = float(sum(prof2["flops"][i] for i in idx))
+        nl = int(sum(prof2["launches"][i] for i in idx))
+        if nl == 0:
+            continue
+        ach = fl / 1e12 / (ms / 1e3)
+        out[name] = {"achieved": ach, "frac": ach / peak, "launches": nl, "kernel_ms": ms,
+                     "useful_flops": fl}
+        if issue:
+            out[name]["frac_of_issue"] = ach / issue
+    out["note"] = ("every contraction launch of one extra step timed with CUDA events (outside the timed region); flops "
+                   "= 2 n r per column-iteration still unconverged at the launch, counted on the device")
+    return out
+
+
+# ----------------------------------------------------------------------------------------- single-problem runner
+def run_problem(tkm, w, *, tf32_delta, tol, warm_tol, profile=1, nystrom_streamed=False, loo=False, lam_idx=None,
+                clocks_index=0, gap_tol=0.0):
+    """One pass of S1..S9 over ONE (X, sigma) problem on the current device; X, y resident.  Returns a dict of stage
+    times (ms), column-iterations, sampled kernel families and clocks."""
+    import torch
+    sigma = float(w.sigmas[0])
+    lambdas = w.lambdas if lam_idx is None else w.lambdas[np.asarray(lam_idx)]
+    V = w.n if loo else w.V
+    foldid = np.arange(w.n, dtype=np.int32) if loo else tkm.tkm_make_folds(w.n, V, w.fold_seed)
+    X, y = torch.from_numpy(w.X).cuda(), torch.from_numpy(w.y).cuda()
+    taus = w.taus if len(w.taus) else None
+
+    def ev():
+        e = torch.cuda.Event(enable_timing=True)
+        e.record()
+        return e
+
+    mon = ClockSampler(clocks_index)
+    mon.start()
+    torch.cuda.reset_peak_memory_stats()
+    e0 = ev()
+    if w.m_landmarks:
+        idx = wl.landmarks(w.n, w.m_landmarks, w.landmark_seed)
+        if nystrom_streamed:
+            e1 = e0
+            spec = tkm.tkm_spectral_setup_nystrom_x(X, sigma, idx)
+        else:
+            Xl = X[torch.from_numpy(idx).cuda()]
+            K_nm, K_mm = tkm.tkm_gram(X, sigma, Xl), tkm.tkm_gram(Xl, sigma)
+            e1 = ev()
+            spec = tkm.tkm_spectral_setup(nystrom=(K_nm, K_mm, idx))
+            del K_nm, K_mm
+        gram_bytes = w.n * w.m_landmarks * 8 + w.m_landmarks ** 2 * 8
+    else:
+        K = tkm.tkm_gram(X, sigma)
+        e1 = ev()
+        spec = tkm.tkm_spectral_setup(K)
+        del K
+        gram_bytes = w.n * w.n * 8
+    e2 = ev()
+    path = tkm.tkm_fit_path(spec, y, w.loss, lambdas, foldid, V, tol, MAXIT, smooth0=w.smooth0, eta=w.eta,
+                            rounds=w.rounds, taus=taus, warm_tol=warm_tol, tf32_delta=tf32_delta, profile=profile,
+                            gap_tol=gap_tol)
+    e3 = ev()
+    cv = tkm.tkm_exact_cv(path, y, foldid, w.T, len(lambdas), V)
+    e4 = ev()
+    e4.synchronize()
+    clocks = mon.stop()
+    if path.status != 0:
+        raise RuntimeError("columns hit maxit: the timed work is not the stated work")
+    out = dict(gram_ms=e0.elapsed_time(e1), setup_ms=e1.elapsed_time(e2), sweep_ms=e2.elapsed_time(e3),
+               cv_ms=e3.elapsed_time(e4), col_iters=int(path.total_col_iters), B=path.B, r=spec.r, n=w.n,
+               prof=path.profile(), clocks=clocks, gram_bytes=gram_bytes, best_l=[int(b) for b in cv[3]],
+               peak_mem_gb=torch.cuda.max_memory_allocated() / 1e9, iters_max=int(path.info()["iters"].max()))
+    path.close()
+    spec.close()
+    torch.cuda.empty_cache()
+    return out
+
+
+def problem_summary(res, pk, traffic, what, knobs, probes=None):
+    tp = tensor_peaks(pk, res["clocks"].get("sm_mhz"))
+    fams = family_rooflines(res["prof"], tp, traffic, probes)
+    n, r = res["n"], res["r"]
+    sweep_s = res["sweep_ms"] / 1e3
+    total_ms = res["gram_ms"] + res["setup_ms"] + res["sweep_ms"] + res["cv_ms"]
+    d = {"workload": what, "columns": res["B"], "launch_config": knobs,
+         "fits_per_s": res["B"] / (total_ms / 1e3), "fits_per_s_sweep_only": res["B"] / sweep_s,
+         "stages_ms": {"gram": res["gram_ms"], "eig_setup": res["setup_ms"], "sweep": res["sweep_ms"],
+                       "exact_cv": res["cv_ms"]},
+         "col_iters": res["col_iters"], "max_iters_of_a_column": res["iters_max"],
+         "sweep_useful_tflops": 4.0 * n * r * res["col_iters"] / sweep_s / 1e12,
+         "gram_gbs": res["gram_bytes"] / (res["gram_ms"] / 1e3) / 1e9 if res["gram_ms"] > 0 else None,
+         "gram_frac_of_hbm": res["gram_bytes"] / (res["gram_ms"] / 1e3) / 1e9 / pk["hbm"] if res["gram_ms"] > 0 else None,
+         "roofline": max(fams, key=lambda f: f["sampled_ms"]) if fams else None, "roofline_families": fams,
+         "peak_device_memory_gb": res["peak_mem_gb"], "clocks": res["clocks"], "selected_lambda_index": res["best_l"]}
+    return d
+
+
+def narrow_hbm_roofline(res, pk):
+    """Narrow live batch: both FP64 contractions stream U once per launch; algorithmic bytes per launch =
+    n r 8 (the U operand) + live (r + n) 8 (moving operand in, result out), from the sampled launches."""
+    pr = res["prof"]
+    out = []
+    n, r = res["n"], res["r"]
+    for i in (0, 1):
+        nl = int(pr["launches"][i])
+        if not nl:
+            continue
+        live = pr["flops"][i] / nl / (2.0 * n * r)          # average live columns of the sampled launches
+        by = n * r * 8.0 + live * (r + n) * 8.0
+        ms = pr["ms"][i] / nl
+        out.append({"bound": "hbm", "kernel": FAMILY[i], "achieved": by / (ms / 1e3) / 1e9, "peak": pk["hbm"],
+                    "unit": "GB/s", "frac": by / (ms / 1e3) / 1e9 / pk["hbm"], "traffic": None,
+                    "avg_live_columns": live, "avg_launch_ms": ms, "algorithmic_bytes_per_launch": by,
+                    "sampled_launches": nl})
+    return out
+
+
+def run_single(args):
+    """`--workload` other than config1: one GPU, one problem, one JSON line."""
+    import torch
+    import paper_2606_06742_b200 as tkm
+    tkm.lib()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device (libtkm has no CPU fallback)")
+    torch.cuda.set_device(0)
+    name = args.workload
+    pk, traffic = peaks(), traffic_table()
+    kw = dict(tf32_delta=TF32_DELTA_LARGE if args.tf32_delta < 0 else args.tf32_delta, tol=args.tol, warm_tol=WARM_TOL,
+              profile=2 if args.profile_all else 1, gap_tol=args.gap_tol)
+    if name.startswith("nystrom_"):
+        w = wl.nystrom_paper_shape(name[len("nystrom_"):])
+        kw["nystrom_streamed"] = True
+        what = ("%s: Nystrom smoothed-hinge SVM with the shape of the paper's Table-4 data set (synthetic rows), n=%d, "
+                "p=%d, m=%d landmarks, %d folds, %d lambdas 1e2..1e-5" % (name, w.n, w.p, w.m_landmarks, w.V, w.L))
+    elif name == "loo_config1":
+        w = wl.config1(sigma_mults=(1.0,))
+        if args.loo_lambdas:
+            w.lambdas = w.lambdas[np.linspace(0, w.L - 1, args.loo_lambdas).round().astype(int)]
+        kw["loo"] = True
+        what = ("loo_config1: leave-one-out form of Algorithm 1 (PAPER.md:178-224, V = n) on configs[1]'s data, median "
+                "bandwidth: n=%d, %d lambdas, B = L (n + 1) = %d columns" % (w.n, w.L, w.L * (w.n + 1)))
+    elif name.startswith("narrow_"):
+        cfg = int(name[-1])
+        w = wl.CONFIGS[cfg]()
+        frac = {1: [0.5], 2: [0.4, 0.7], 4: [0.3, 0.5, 0.7, 0.9]}[args.narrow_L]
+        kw["lam_idx"] = [int(round(f * (w.L - 1))) for f in frac]
+        kw["tf32_delta"] = 0 if args.tf32_delta < 0 else args.tf32_delta
+        what = ("%s: BASELINE.json configs[%d] at full n = %d with %d lambda(s) (grid indices %s): B = %d columns, the "
+                "HBM-bound narrow batch of SURVEY.md 8(d)" % (name, cfg, w.n, args.narrow_L, kw["lam_idx"],
+                                                               w.T * args.narrow_L * (w.V + 1)))
+    else:
+        cfg = int(name[-1])
+        w = wl.CONFIGS[cfg]()
+        what = "BASELINE.json configs[%d] at full size: n=%d, p=%d, %d folds, %d lambdas%s%s" % (
+            cfg, w.n, w.p, w.V, w.L, ", tau %s" % list(w.taus) if len(w.taus) else "",
+            ", Nystrom m=%d" % w.m_landmarks if w.m_landmarks else "")
+    res = None
+    for it in range(args.warmup + args.steps):
+        res = run_problem(tkm, w, **kw)          # the last pass is reported (a pass takes seconds to a minute)
+    knobs = {"tf32_delta": kw["tf32_delta"], "stop_tol": args.tol, "warm_start_rounds_tol": WARM_TOL,
+             "gap_tol": args.gap_tol, "profile": kw["profile"],
+             "l2": "inputs larger than L2" if w.n * res["r"] * 8 > 126e6 else "not flushed"}
+    d = problem_summary(res, pk, traffic, what, knobs)
+    total_ms = sum(d["stages_ms"].values())
+    line = {"metric": METRIC, "value": d["fits_per_s"], "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": total_ms, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": what, "columns_per_step": d["columns"],
+                       "value_is": "columns / (Gram + setup + sweep + exact CV)"}}
+    line.update({k: v for k, v in d.items() if k != "workload"})
+    if name.startswith("narrow_"):
+        line["roofline_hbm"] = narrow_hbm_roofline(res, pk)
+        if line["roofline_hbm"]:
+            line["roofline"] = max(line["roofline_hbm"], key=lambda f: f["avg_launch_ms"])
+    if args.profile_all:
+        line["time_weighted"] = time_weighted(res["prof"], tensor_peaks(pk, res["clocks"].get("sm_mhz")))
+    line["gpu_launches"] = int(tkm.tkm_launch_count())
+    print(json.dumps(line))
+
+
+# ----------------------------------------------------------------------------------------- CUDA arm, default line
 def run_ours(args, w, rank, world):
     import torch
     import paper_2606_06742_b200 as tkm
@@ -196,9 +514,7 @@ def run_ours(args, w, rank, world):
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    dt = args.dtype
-    sweep_dt = tkm.F64 if dt == "f64" else tkm.F32
-    tol = STOP_TOL[dt]
+    tol = STOP_TOL["f64"]
     foldid = tkm.tkm_make_folds(w.n, w.V, w.fold_seed)
     X = torch.from_numpy(w.X).cuda()
     y = torch.from_numpy(w.y).cuda()
@@ -207,55 +523,51 @@ def run_ours(args, w, rank, world):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     prof = dict(ms=np.zeros(4), flops=np.zeros(4), launches=np.zeros(4, dtype=np.int64), col_iters=0)
     stage = np.zeros(4)
-    e2e_stage = np.zeros(5)     # last e2e step: copy-in, gram, eig, sweep, cv + coefficients + copy-out (ms)
+    e2e_stage = np.zeros(5)     # summed over the e2e steps: copy-in, gram, eig, sweep, cv + coefficients + copy-out (ms)
 
     def ev():
         e = torch.cuda.Event(enable_timing=True)
         e.record()
         return e
 
-    def step_device(collect):
+    def step_device(collect, profile=1):
         """One pass of the hot path: S1 + S2 per bandwidth, S3-S8 for all bandwidths as groups of one
         sweep (tkm_fit_path_multi), S9 per bandwidth."""
         flush.zero_()
         e0 = ev()
         Ks = tkm.tkm_gram_multi(X, w.sigmas)                               # one distance pass, 5 exp + writes
         e1 = ev()
-        specs = tkm.tkm_spectral_setup_multi(Ks, sweep_dtype=sweep_dt)     # the 5 decompositions overlap
+        specs = tkm.tkm_spectral_setup_multi(Ks)                           # the 5 decompositions overlap
         del Ks
         e2 = ev()
         paths = tkm.tkm_fit_path_multi(specs, y, w.loss, w.lambdas, foldid, w.V, tol, MAXIT, smooth0=w.smooth0,
-                                       eta=w.eta, rounds=w.rounds, warm_tol=WARM_TOL, tf32_delta=TF32_DELTA, profile=True)
+                                       eta=w.eta, rounds=w.rounds, warm_tol=WARM_TOL, tf32_delta=TF32_DELTA,
+                                       profile=profile)
         e3 = ev()
         best = [int(tkm.tkm_exact_cv(path, y, foldid, w.T, w.L, w.V)[3][0]) for path in paths]
         e4 = ev()
+        pr = None
         if collect:
             e4.synchronize()
-            stage[0] += e0.elapsed_time(e1)
-            stage[1] += e1.elapsed_time(e2)
-            stage[2] += e2.elapsed_time(e3)
-            stage[3] += e3.elapsed_time(e4)
             pr = paths[0].profile()
-            prof["ms"] += pr["ms"]
-            prof["flops"] += pr["flops"]
-            prof["launches"] += pr["launches"]
-            prof["col_iters"] += sum(path.total_col_iters for path in paths)
+            pr["col_iters"] = sum(path.total_col_iters for path in paths)
+            pr["stage"] = np.array([e0.elapsed_time(e1), e1.elapsed_time(e2), e2.elapsed_time(e3), e3.elapsed_time(e4)])
             if any(path.status != 0 for path in paths):
                 raise RuntimeError("columns hit maxit: the timed work is not the stated work")
         for path in paths:
             path.close()
         for spec in specs:
             spec.close()
-        return best
+        return best, pr
 
     def step_e2e():
         flush.zero_()
         r = tkm.tkm_train_tune_host(Xh.numpy(), yh.numpy(), np.asarray(w.sigmas, dtype=np.float64), w.loss, w.lambdas,
                                     foldid, w.V, tol, MAXIT, smooth0=w.smooth0, eta=w.eta, rounds=w.rounds,
-                                    warm_tol=WARM_TOL, tf32_delta=TF32_DELTA, sweep_dtype=sweep_dt)
+                                    warm_tol=WARM_TOL, tf32_delta=TF32_DELTA)
         if r["status"] != 0:
             raise RuntimeError("columns hit maxit in the e2e leg")
-        e2e_stage[:] = r["stage_ms"]
+        e2e_stage[:] += r["stage_ms"]
         nb_in = Xh.numel() * 8 + yh.numel() * 8
         nb_out = r["cv_loss"].nbytes + r["cv_err"].nbytes + r["cv_mean"].nbytes + r["best_l"].nbytes + \
             r["alpha"].nbytes + r["beta0"].nbytes
@@ -278,7 +590,11 @@ def run_ours(args, w, rank, world):
     tkm.tkm_launch_count_reset()
     s_ev = ev()
     for _ in range(args.steps):
-        step_device(True)
+        _, pr = step_device(True)
+        for k in ("ms", "flops", "launches"):
+            prof[k] += pr[k]
+        prof["col_iters"] += pr["col_iters"]
+        stage += pr["stage"]
     e_ev = ev()
     barrier()
     launches = tkm.tkm_launch_count()
@@ -288,6 +604,7 @@ def run_ours(args, w, rank, world):
     # e2e leg: host buffers -> tkm_train_tune_host -> host results
     step_e2e()
     barrier()
+    e2e_stage[:] = 0.0
     s_ev = ev()
     for _ in range(args.steps):
         nb_in, nb_out = step_e2e()
@@ -302,135 +619,69 @@ def run_ours(args, w, rank, world):
     fits_per_step = w.B * len(w.sigmas)
     ms_per_step = ms_total / args.steps
     value = world * fits_per_step / (ms_per_step / 1e3)
-    pk = peaks()
-
-    def family(idx, name, peak_tf, peak_src, traffic):
-        ms, fl, nl = float(prof["ms"][idx].sum()), float(prof["flops"][idx].sum()), int(prof["launches"][idx].sum())
-        ach = (fl / 1e12) / (ms / 1e3) if ms > 0 else 0.0
-        return {"bound": "tensor", "kernel": name, "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s",
-                "frac": ach / peak_tf, "traffic": traffic, "peak_source": peak_src, "sampled_launches": nl,
-                "avg_launch_ms": ms / max(1, nl), "avg_flops_per_launch": fl / max(1, nl),
-                "sampled_ms": ms}
-
-    # FP64 DMMA kernel: peak = measured bf16 sustained x nominal FP64/bf16 ratio
-    roof_f64 = family([0, 1], "gemm_f64_tma_kernel (FP64 DMMA: exact iterations and the narrow tail; GEMM-A loss "
-                      "epilogue + GEMM-B spectral epilogue)", pk["bf16_sus"] * NOMINAL_RATIO["f64"],
-                      "%s bf16 sustained %.1f TF/s x nominal f64/bf16 ratio %.4f" %
-                      (pk["src"], pk["bf16_sus"], NOMINAL_RATIO["f64"]), NCU_TRAFFIC_BYTES_PER_LAUNCH)
-    # tcgen05 3xTF32 kernel: every useful product costs three TF32 MMAs; achieved counts the USEFUL flops only
-    roof_tf32 = family([2, 3], "gemm_tf32x3_kernel (tcgen05 3xTF32 delta forms: F+ = Fbar - U Lam da with loss "
-                       "epilogue, zeta += U^T dz with rho epilogue)", pk["bf16_sus"] * NOMINAL_RATIO["f32"],
-                       "%s bf16 sustained %.1f TF/s x nominal tf32/bf16 ratio 0.5 / 3 MMAs per useful product" %
-                       (pk["src"], pk["bf16_sus"]), NCU_TRAFFIC_TF32_BYTES_PER_LAUNCH)
-    # the dominant kernel family is the one with the larger share of the sweep: per batch of 16 iterations the
-    # delta forms run 15 tcgen05 pairs and one DMMA pair, the all-FP64 sweep 16 DMMA pairs
-    if TF32_DELTA == 2 and roof_tf32["sampled_launches"]:
+    pk, traffic = peaks(), traffic_table()
+    tp = tensor_peaks(pk, clocks.get("sm_mhz") if clocks else None)
+    probes = library_probes(tkm) if world == 1 else None
+    fams = family_rooflines(prof, tp, traffic, probes)
+    # the FP64 DMMA kernel (both epilogues) and the tcgen05 kernel (both delta forms): the dominant one -- the larger
+    # share of the sampled kernel time -- is `roofline`
+    roof_f64, roof_tf32 = merge_families(fams, (0, 1)), merge_families(fams, (2, 3))
+    if roof_f64 is not None:
+        tr = traffic.get("config1_dmma_full_width")
+        roof_f64["traffic"], roof_f64["traffic_source"] = (tr[0], tr[1]) if tr else (None, None)
+    if roof_tf32 is not None:
+        tr = traffic.get("config1_tcgen05_full_width")
+        roof_tf32["traffic"], roof_tf32["traffic_source"] = (tr[0], tr[1]) if tr else (None, None)
+    if TF32_DELTA == 2 and roof_tf32 is not None:
         roofline, roofline_other = roof_tf32, roof_f64
     else:
-        roofline, roofline_other = roof_f64, (roof_tf32 if roof_tf32["sampled_launches"] else None)
+        roofline, roofline_other = roof_f64, roof_tf32
     sweep_s = stage[2] / 1e3
+    stage_sum = float(stage.sum()) / args.steps
+    gram_gbs = len(w.sigmas) * w.n * w.n * 8 / (stage[0] / args.steps / 1e3) / 1e9
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": dt, "data": "synthetic", "config": workload_config(w, dt),
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(w),
+            "launch_config": {"tf32_delta": TF32_DELTA, "sampled_kernel_events": "profile=1 in the timed region"},
             "stages_ms_per_step": {"gram": stage[0] / args.steps, "eig_setup": stage[1] / args.steps,
                                    "sweep": stage[2] / args.steps, "exact_cv": stage[3] / args.steps},
+            "ms_per_step_outside_stages": ms_per_step - stage_sum,
             "exact_cv_ms_per_grid": stage[3] / args.steps / len(w.sigmas),
             "fits_per_s_sweep_only": args.steps * fits_per_step / sweep_s,
             "col_iters_per_step": prof["col_iters"] / args.steps,
             "sweep_useful_tflops": 4.0 * w.n * w.n * prof["col_iters"] / sweep_s / 1e12,
-            "gram_gbs": len(w.sigmas) * w.n * w.n * 8 / (stage[0] / args.steps / 1e3) / 1e9,
+            "gram_gbs": gram_gbs, "gram_frac_of_hbm": gram_gbs / pk["hbm"],
             "roofline": roofline, "roofline_other_kernel": roofline_other, "clocks": clocks, "gpu_launches": int(launches),
             "e2e": {"value": world * fits_per_step / (ms_e2e / args.steps / 1e3), "unit": UNIT,
                     "h2d_bytes_per_step": int(nb_in), "d2h_bytes_per_step": int(nb_out),
                     "ms_per_step": ms_e2e / args.steps,
-                    "last_step_stages_ms": {k: float(v) for k, v in zip(("h2d", "gram", "eig_setup", "sweep",
-                                                                          "cv_coef_d2h"), e2e_stage)}}}
+                    "stages_ms_per_step": {k: float(v) / args.steps for k, v in zip(("h2d", "gram", "eig_setup", "sweep",
+                                                                                      "cv_coef_d2h"), e2e_stage)},
+                    "ms_per_step_outside_stages": (ms_e2e - float(e2e_stage.sum())) / args.steps}}
     if world == 1:
+        line["peaks_measured_here"] = probes
+        # every launch of one more step, outside the timed region: the time-weighted fractions
+        _, pr2 = step_device(True, profile=2)
+        line["roofline_time_weighted"] = time_weighted(pr2, tp)
+        if not args.no_large:
+            # the largest full-kernel single-GPU configuration of BASELINE.json: one pass, its own roofline and clocks
+            del X, y, flush
+            torch.cuda.empty_cache()
+            w3 = wl.config3()
+            r3 = run_problem(tkm, w3, tf32_delta=TF32_DELTA_LARGE, tol=1e-10, warm_tol=WARM_TOL, profile=1,
+                             clocks_index=local)
+            line["large_config"] = problem_summary(
+                r3, pk, traffic, "BASELINE.json configs[3]: kernel quantile regression tau in {0.1,0.5,0.9} on one U, "
+                "n=20000, p=28, 5 folds, 50 lambdas 1e1..1e-6, gamma 1 -> 1/512 in 4 rounds; ONE pass (no warm-up "
+                "pass, outside the timed region of `value`)",
+                {"tf32_delta": TF32_DELTA_LARGE, "stop_tol": 1e-10, "warm_start_rounds_tol": WARM_TOL,
+                 "l2": "inputs larger than L2 (U Lam and U^T: 3.2 GB each)"}, probes)
         ncol, secs, its = oracle_sample_step(w)
         line["cpu_baseline"] = {"value": ncol / secs, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
-                                "sample": "sigma index %d, lambda indices %s x %d hold-out settings = %d of %d columns, "
-                                          "full n, Gram + eigh + path + exact CV, %.1f s, %d column-iterations"
-                                          % (CPU_SAMPLE_SIGMA_IDX, list(CPU_SAMPLE_LAMBDA_IDX), w.V + 1, ncol,
-                                             fits_per_step, secs, its)}
+                                "sample": sample_text(w, ncol, secs, its)}
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
-
-
-# ------------------------------------------------------------- secondary workload: Nystrom at the paper's row counts
-def run_nystrom_scale(args):
-    """`--workload nystrom_covtype | nystrom_mnist8m46` (not the headline line): streamed Nystrom
-    setup + sweep + exact CV at the row counts of the paper's Table 4, one GPU, X and y resident.  One JSON line with
-    the same metric; `roofline` holds the four contraction-kernel families as sampled inside the sweep."""
-    import torch
-    import paper_2606_06742_b200 as tkm
-    tkm.lib()
-    if not torch.cuda.is_available():
-        raise RuntimeError("bench.py needs a CUDA device (libtkm has no CPU fallback)")
-    torch.cuda.set_device(0)
-    w = wl.nystrom_paper_shape(args.workload[len("nystrom_"):])
-    sigma = float(w.sigmas[0])
-    idx = wl.landmarks(w.n, w.m_landmarks, w.landmark_seed)
-    foldid = tkm.tkm_make_folds(w.n, w.V, w.fold_seed)
-    X, y = torch.from_numpy(w.X).cuda(), torch.from_numpy(w.y).cuda()
-    pk = peaks()
-
-    def ev():
-        e = torch.cuda.Event(enable_timing=True)
-        e.record()
-        return e
-
-    tot = np.zeros(3)
-    prof = dict(ms=np.zeros(4), flops=np.zeros(4), launches=np.zeros(4, dtype=np.int64))
-    col_iters = 0
-    mon = ClockSampler(0)
-    for it in range(args.warmup + args.steps):
-        if it == args.warmup:
-            mon.start()
-        e0 = ev()
-        spec = tkm.tkm_spectral_setup_nystrom_x(X, sigma, idx)
-        e1 = ev()
-        path = tkm.tkm_fit_path(spec, y, w.loss, w.lambdas, foldid, w.V, args.tol, MAXIT, smooth0=w.smooth0, eta=w.eta,
-                                rounds=w.rounds, warm_tol=WARM_TOL, tf32_delta=2, profile=True)
-        e2 = ev()
-        tkm.tkm_exact_cv(path, y, foldid, 1, w.L, w.V)
-        e3 = ev()
-        e3.synchronize()
-        if path.status != 0:
-            raise RuntimeError("columns hit maxit: the timed work is not the stated work")
-        if it >= args.warmup:
-            tot += [e0.elapsed_time(e1), e1.elapsed_time(e2), e2.elapsed_time(e3)]
-            pr = path.profile()
-            for k in prof:
-                prof[k] += pr[k]
-            col_iters += path.total_col_iters
-        r = spec.r
-        path.close()
-        spec.close()
-    clocks = mon.stop()
-    tot /= args.steps
-    names = ["gemm_f64_tma_kernel GEMM-A (FP64 DMMA)", "gemm_f64_tma_kernel GEMM-B (FP64 DMMA, K-split)",
-             "gemm_tf32x3_kernel GEMM-A (tcgen05 3xTF32)", "gemm_tf32x3_kernel GEMM-B (tcgen05 3xTF32, K-split)"]
-    f64_tf, tf32x3_tf = pk["bf16_sus"] * NOMINAL_RATIO["f64"], pk["bf16_sus"] * NOMINAL_RATIO["f32"]   # as in run_ours
-    peak = [f64_tf, f64_tf, tf32x3_tf, tf32x3_tf]
-    fam = [{"kernel": names[i], "bound": "tensor", "achieved": float(prof["flops"][i] / prof["ms"][i] / 1e9), "peak": peak[i],
-            "unit": "TFLOP/s", "frac": float(prof["flops"][i] / prof["ms"][i] / 1e9 / peak[i]),
-            "sampled_launches": int(prof["launches"][i]), "avg_launch_ms": float(prof["ms"][i] / prof["launches"][i]),
-            "traffic": None} for i in range(4) if prof["launches"][i]]
-    print(json.dumps({
-        "metric": "lambda_x_fold_path_fits_per_s", "value": w.B / (tot.sum() / 1e3), "unit": "fits/s", "n_gpus": 1,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": float(tot.sum()), "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "%s: Nystrom smoothed-hinge SVM with the shape of the paper's Table-4 data set (synthetic "
-                               "rows), n=%d, p=%d, m=%d landmarks (r=%d), %d folds, %d lambdas 1e2..1e-5; secondary "
-                               "workload, not BASELINE.json's metric configuration" % (args.workload, w.n, w.p,
-                                                                                        w.m_landmarks, r, w.V, w.L),
-                   "columns_per_step": w.B, "stop_tol": args.tol, "warm_start_rounds_tol": WARM_TOL, "tf32_delta": 2,
-                   "l2": "inputs larger than L2 (U alone is %.1f GB)" % (w.n * r * 8 / 1e9)},
-        "stages_ms_per_step": {"nystrom_setup_streamed": float(tot[0]), "sweep": float(tot[1]), "exact_cv": float(tot[2])},
-        "col_iters_per_step": col_iters / args.steps,
-        "sweep_useful_tflops": 4.0 * w.n * r * col_iters / args.steps / (tot[1] / 1e3) / 1e12,
-        "roofline": fam, "clocks": clocks}))
 
 
 def main():
@@ -439,18 +690,28 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
-    ap.add_argument("--workload", default="config1", choices=["config1", "nystrom_covtype", "nystrom_mnist8m46"],
-                    help="config1 = BASELINE.json's metric configuration (the bench line); the nystrom_* workloads are "
-                         "secondary single-GPU measurements (use --steps 1 --warmup 1: a step takes 20-100 s)")
-    ap.add_argument("--tol", type=float, default=1e-10, help="stop tolerance of the nystrom_* workloads")
+    ap.add_argument("--dtype", default="f64", choices=["f64"])
+    ap.add_argument("--workload", default="config1",
+                    choices=["config1", "config2", "config3", "config4", "nystrom_covtype", "nystrom_mnist8m46",
+                             "loo_config1", "narrow_config2", "narrow_config3"],
+                    help="config1 = BASELINE.json's metric configuration (the bench line, which also carries configs[3] "
+                         "as `large_config`); the others are single-GPU measurements of one problem "
+                         "(use --steps 1 --warmup 0 or 1: a pass takes seconds to a minute)")
+    ap.add_argument("--tol", type=float, default=1e-10, help="stop tolerance of the --workload runs other than config1")
+    ap.add_argument("--tf32-delta", type=int, default=-1, help="override the delta-form mode of a --workload run")
+    ap.add_argument("--gap-tol", type=float, default=0.0,
+                    help="outer control of PAPER.md:220-222 (reading G23) for a --workload run; 0 = fixed schedule")
+    ap.add_argument("--narrow-L", type=int, default=1, choices=[1, 2, 4])
+    ap.add_argument("--loo-lambdas", type=int, default=0, help="loo_config1: use this many lambdas of the grid (0 = all 50)")
+    ap.add_argument("--profile-all", action="store_true", help="time every contraction launch (profile = 2)")
+    ap.add_argument("--no-large", action="store_true", help="default line: skip the configs[3] pass (`large_config`)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if args.workload != "config1":
         if args.impl != "ours" or world != 1 or args.gpus != 1:
             raise SystemExit("--workload %s: one GPU, --impl ours only" % args.workload)
-        return run_nystrom_scale(args)
+        return run_single(args)
     from paper_2606_06742_b200.ranks import replica_seed
     w = wl.config1(seed=replica_seed(1001, rank if args.impl == "ours" else 0))
     if args.impl == "reference":

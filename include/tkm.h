@@ -68,7 +68,10 @@ typedef struct {
   int32_t check_every;/* iterations between host convergence polls; <= 0 => library default   */
   double warm_tol;    /* tolerance of rounds 0..R-2 (warm starts only); <= 0 => same as tol   */
   int32_t profile;    /* 1: time the two contractions of the first iteration after every poll */
-                      /* with CUDA events (read with tkm_path_profile); 0: no events          */
+                      /* with CUDA events (read with tkm_path_profile); 0: no events;         */
+                      /* 2: time EVERY contraction launch and count the column-iterations of  */
+                      /* each kernel family on the device (a measurement mode: ~4 events and  */
+                      /* two atomics per iteration; not for timed runs)                       */
   int32_t tf32_delta; /* 2: both contractions in delta form (also F = U Lam a: F+ = Fbar - U Lam da, two  */
                       /* FP64 GEMM-A per exact iteration).  1: delta-form GEMM-B only.  zeta = U^T z is kept in FP64 and advanced by        */
                       /* zeta += U^T (z - z_old) with the increment contracted in 3xTF32 on the     */
@@ -76,6 +79,13 @@ typedef struct {
                       /* vanishes at convergence); zeta is recomputed in FP64 after every           */
                       /* compaction (every check_every iterations).  Same fixed point and           */
                       /* tolerances as 0 (all FP64 DMMA); DESIGN.md section 12.                     */
+  double gap_tol;     /* outer control of PAPER.md:220-222 ("shrink delta ... until the KKT conditions of  */
+                      /* all SVM models are satisfied"; reading G23).  <= 0: the fixed schedule of `rounds`  */
+                      /* levels for every column.  > 0: after round k < rounds-1 a column whose solution     */
+                      /* certifies a duality gap of the NON-smoothed problem <= gap_tol (the certificate of   */
+                      /* tkm_path_duality_gap) keeps that level's minimiser and leaves the schedule; a warm_tol */
+                      /* iterate only screens: the column is first finished to `tol` at that level and tested  */
+                      /* again.  `rounds` is the cap: a column that reaches it with a larger gap gets flag 2.  */
 } tkm_loss_opts;
 
 /* Nystrom inputs for tkm_spectral_setup (reading G11). */
@@ -166,16 +176,23 @@ int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, const void* 
                        const tkm_path* const* warm, tkm_path** out, void* stream);
 void tkm_path_free(tkm_path* p);
 /* Shape and per-column diagnostics, all [host], any pointer may be NULL:
- * B, r; iters[B] (total over rounds), kkt[B] (last residual), flags[B] (1 = hit maxit),
+ * B, r; iters[B] (total over rounds), kkt[B] (last residual), flags[B] (bit 0 = hit maxit, bit 1 = reached the
+ * cap of the smoothing schedule with a duality gap > gap_tol; only with gap_tol > 0),
  * beta0[B]; total_col_iters = sum of iters (the unit of the roofline). */
 int tkm_path_info(const tkm_path* p, int32_t* B, int64_t* r, int32_t* iters, double* kkt,
                   int32_t* flags, double* beta0, int64_t* total_col_iters);
+/* Smoothing level every column ended on (reading G23): level[B] in [0, rounds), rounds - 1 under the fixed schedule,
+ * and smooth[B] = smooth0 eta^level (0 for the smooth losses); both [host], either may be NULL. */
+int tkm_path_levels(const tkm_path* p, int32_t* level, double* smooth);
 /* Sampled kernel timings of the sweep (only when tkm_loss_opts.profile was 1), all [host] arrays of 4, one
  * entry per kernel family and contraction: [0] FP64 DMMA GEMM-A, [1] FP64 DMMA GEMM-B, [2] tcgen05 3xTF32
  * delta GEMM-A, [3] tcgen05 3xTF32 delta GEMM-B.  ms = summed CUDA-event durations of the sampled launches (the
  * first iteration after every compaction -- every slot live -- and, in the delta forms, the exact last
  * iteration of the batch), flops = summed algorithmic flops 2 n r (live columns) of those launches
- * (4 n r per column-iteration over the two contractions), launches = their number. */
+ * (4 n r per column-iteration over the two contractions), launches = their number.
+ * With profile == 2 the three arrays are totals over ALL launches of the sweep and flops counts, per family,
+ * 2 n r for every column-iteration that was still unconverged when the launch ran (frozen slots that wait for
+ * the next compaction are multiplied but not counted): flops / ms is the time-weighted useful rate. */
 int tkm_path_profile(const tkm_path* p, double* ms, double* flops, int64_t* launches);
 /* Spectral coordinates of all columns: [dev] a_out, B x r FP64 row-major (ld = r). */
 int tkm_path_get_a(const tkm_path* p, double* a_out, void* stream);

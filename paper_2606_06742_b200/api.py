@@ -13,7 +13,7 @@ TKM_OK, TKM_ENOTCONV = 0, 5
 
 EXPORTED_SYMBOLS = [
     "tkm_gram", "tkm_gram_multi", "tkm_spectral_setup", "tkm_spectral_setup_multi", "tkm_spectral_setup_nystrom_x", "tkm_spectral_free", "tkm_spectral_info", "tkm_spectral_get_u",
-    "tkm_fit_path", "tkm_fit_path_multi", "tkm_path_free", "tkm_path_info", "tkm_path_profile", "tkm_path_get_a", "tkm_exact_cv", "tkm_cv_select", "tkm_path_duality_gap", "tkm_path_coef",
+    "tkm_fit_path", "tkm_fit_path_multi", "tkm_path_free", "tkm_path_info", "tkm_path_levels", "tkm_path_profile", "tkm_path_get_a", "tkm_exact_cv", "tkm_cv_select", "tkm_path_duality_gap", "tkm_path_coef",
     "tkm_predict", "tkm_cv_decision_values", "tkm_platt_fit", "tkm_platt_proba", "tkm_train_tune_host", "tkm_make_folds", "tkm_launch_count", "tkm_launch_count_reset",
     "tkm_dgemm_nt", "tkm_gemm_probe", "tkm_tf32x3_gemm_nt", "tkm_version", "tkm_last_error",
 ]
@@ -28,7 +28,8 @@ class TkmError(RuntimeError):
 class _LossOpts(C.Structure):
     _fields_ = [("smooth0", C.c_double), ("eta", C.c_double), ("rounds", C.c_int32), ("T", C.c_int32),
                 ("taus", C.POINTER(C.c_double)), ("restart", C.c_int32), ("check_every", C.c_int32),
-                ("warm_tol", C.c_double), ("profile", C.c_int32), ("tf32_delta", C.c_int32)]
+                ("warm_tol", C.c_double), ("profile", C.c_int32), ("tf32_delta", C.c_int32),
+                ("gap_tol", C.c_double)]
 
 
 class _Nystrom(C.Structure):
@@ -70,6 +71,7 @@ def lib():
     L.tkm_path_free.argtypes = [vp]
     L.tkm_path_free.restype = None
     L.tkm_path_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i64), vp, vp, vp, vp, C.POINTER(i64)]
+    L.tkm_path_levels.argtypes = [vp, vp, vp]
     L.tkm_path_profile.argtypes = [vp, vp, vp, vp]
     L.tkm_path_get_a.argtypes = [vp, vp, vp]
     L.tkm_exact_cv.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp]
@@ -273,6 +275,12 @@ class Path:
         _check(lib().tkm_path_info(self._h, None, None, _ptr(iters), _ptr(kkt), _ptr(flags), _ptr(beta0), None))
         return dict(iters=iters, kkt=kkt, flags=flags, beta0=beta0)
 
+    def levels(self):
+        """(level index, smoothing parameter) every column ended on (reading G23)."""
+        lev, sm = np.empty(self.B, dtype=np.int32), np.empty(self.B)
+        _check(lib().tkm_path_levels(self._h, _ptr(lev), _ptr(sm)))
+        return lev, sm
+
     def profile(self):
         """Sampled launches by family: index 0/1 = FP64 DMMA GEMM-A/B, 2/3 = tcgen05 3xTF32 delta GEMM-A/B."""
         ms, fl = np.zeros(4), np.zeros(4)
@@ -298,21 +306,21 @@ class Path:
             pass
 
 
-def _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, profile=False, tf32_delta=0):
+def _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, profile=False, tf32_delta=0, gap_tol=0.0):
     taus_arr = _host(taus if taus is not None else [], np.float64)
     o = _LossOpts(float(smooth0), float(eta), int(rounds), int(len(taus_arr)),
                   taus_arr.ctypes.data_as(C.POINTER(C.c_double)) if len(taus_arr) else None,
-                  int(bool(restart)), int(check_every), float(warm_tol), int(bool(profile)), int(tf32_delta))
+                  int(bool(restart)), int(check_every), float(warm_tol), int(profile), int(tf32_delta), float(gap_tol))
     return o, taus_arr
 
 
 def tkm_fit_path(spec: Spectral, y, loss: int, lambdas, foldid, V: int, tol: float, maxit: int,
                  smooth0=1.0, eta=0.125, rounds=4, taus=None, restart=True, check_every=0, warm_tol=0.0,
-                 warm: Path | None = None, profile=False, tf32_delta=0, stream=None) -> Path:
+                 warm: Path | None = None, profile=False, tf32_delta=0, gap_tol=0.0, stream=None) -> Path:
     y = _dev_f64(y, "y")
     lam = _host(lambdas, np.float64)
     fid = _host(foldid, np.int32)
-    o, keep = _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, profile, tf32_delta)
+    o, keep = _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, profile, tf32_delta, gap_tol)
     h = C.c_void_p()
     rc = lib().tkm_fit_path(spec._h, y.data_ptr(), loss, C.byref(o), _ptr(lam), len(lam), _ptr(fid), V,
                             float(tol), int(maxit), warm._h if warm is not None else None, C.byref(h),
@@ -323,12 +331,12 @@ def tkm_fit_path(spec: Spectral, y, loss: int, lambdas, foldid, V: int, tol: flo
 
 def tkm_fit_path_multi(specs, y, loss: int, lambdas, foldid, V: int, tol: float, maxit: int,
                        smooth0=1.0, eta=0.125, rounds=4, taus=None, restart=True, check_every=0, warm_tol=0.0,
-                       warm=None, profile=False, tf32_delta=0, stream=None):
+                       warm=None, profile=False, tf32_delta=0, gap_tol=0.0, stream=None):
     """One sweep over G spectral handles that share y, folds and the lambda grid -> list of G Paths."""
     y = _dev_f64(y, "y")
     lam = _host(lambdas, np.float64)
     fid = _host(foldid, np.int32)
-    o, keep = _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, profile, tf32_delta)
+    o, keep = _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, profile, tf32_delta, gap_tol)
     G = len(specs)
     hs = (C.c_void_p * G)(*[s._h for s in specs])
     hw = (C.c_void_p * G)(*[w._h for w in warm]) if warm is not None else None

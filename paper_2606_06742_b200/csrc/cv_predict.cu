@@ -72,7 +72,8 @@ struct GapEpi {
   const double* col_tau;
   const int32_t* col_v;
   int loss;
-  double smooth;
+  double smooth;             // smoothing level of every column, unless
+  const double* col_smooth;  // [B] per-column levels (reading G23: columns may end on different levels), or NULL
   double* lpart;   // [m blocks][ldpart] sum of the nominal loss over training rows
   double* dpart;   // [m blocks][ldpart] sum of d_j over training rows
   int64_t ldpart;
@@ -88,6 +89,7 @@ struct GapEpi {
       if (col >= N) continue;
       const int v = col_v[col];
       const double b0 = beta0[col], tau = col_tau[col];
+      const double sm = col_smooth ? col_smooth[col] : smooth;
 #pragma unroll
       for (int j = 0; j < TM; ++j)
 #pragma unroll
@@ -96,7 +98,7 @@ struct GapEpi {
           if (m < M && foldid[m] != v) {
             const double f = acc[i][j][e] + b0, yy = y[m];
             ls[i] += nominal_loss_dev(loss, yy, f, tau);
-            ds[i] -= yy * psi_dev(loss, yy, f, smooth, tau);
+            ds[i] -= yy * psi_dev(loss, yy, f, sm, tau);
           }
         }
     }
@@ -269,6 +271,29 @@ static int coef_device(const tkm_path* p, int col, double* out, cudaStream_t st)
   return TKM_OK;
 }
 
+// Gap certificate of every column of `p` at the coefficients (p->a, beta0) -- beta0 [dev] B, d_fold [dev] n --
+// for the level `smooth` (col_smooth == NULL) or per-column levels: primal and gap [dev] B.  Asynchronous;
+// the partial-sum scratch is stream-ordered.  Used by tkm_path_duality_gap and by the sweep's outer control.
+int path_gap_device(const tkm_path* p, const double* y, const int32_t* d_fold, const double* beta0, double smooth,
+                    const double* col_smooth, double* d_P, double* d_gap, cudaStream_t st) {
+  const tkm_spectral* s = p->spec;
+  const int64_t n = s->n, r = s->r;
+  const int B = p->B;
+  const int nblk = (int)ceil_div(n, gemm_f64_choose(&B, 1, (int)n, (int)r).BM);
+  const int64_t ldpart = round_up(B, 16);
+  DevBuf lpart, dpart;
+  TKM_TRY(lpart.alloc((size_t)nblk * ldpart * sizeof(double), true, st, true));
+  TKM_TRY(dpart.alloc((size_t)nblk * ldpart * sizeof(double), true, st, true));
+  GapEpi epi{y, d_fold, beta0, p->col_tau.as<double>(), p->col_v.as<int32_t>(), (int)p->loss, smooth, col_smooth,
+             lpart.as<double>(), dpart.as<double>(), ldpart};
+  TKM_TRY(gemm_f64_once(p->a.as<double>(), s->ldr, s->UL.as<double>(), s->ldr, B, (int)n, (int)r, epi, st));
+  gap_finalize_kernel<<<(unsigned)B, 256, 0, st>>>(lpart.as<double>(), dpart.as<double>(), ldpart, nblk, p->a.as<double>(),
+                                                   s->ldr, s->lam.as<double>(), (int)r, p->col_lam.as<double>(),
+                                                   p->col_nc.as<double>(), d_P, d_gap);
+  TKM_LAUNCH_CHECK();
+  return TKM_OK;
+}
+
 }  // namespace tkm
 
 using namespace tkm;
@@ -329,26 +354,18 @@ extern "C" int tkm_path_duality_gap(const tkm_path* p, const void* y, const int3
   TKM_TRY(device_check());
   cudaStream_t st = (cudaStream_t)stream;
   const tkm_spectral* s = p->spec;
-  const int64_t n = s->n, r = s->r;
+  const int64_t n = s->n;
   const int B = p->B;
   for (int64_t j = 0; j < n; ++j)
     if (foldid[j] < 0 || foldid[j] >= p->V) return set_error(TKM_EINVAL, "tkm_path_duality_gap: foldid out of range");
-  const int nblk = (int)ceil_div(n, gemm_f64_choose(&B, 1, (int)n, (int)r).BM);
-  const int64_t ldpart = round_up(B, 16);
-  DevBuf lpart, dpart, d_fold, d_P, d_gap;
-  TKM_TRY(lpart.alloc((size_t)nblk * ldpart * sizeof(double), true, st));
-  TKM_TRY(dpart.alloc((size_t)nblk * ldpart * sizeof(double), true, st));
+  DevBuf d_fold, d_P, d_gap;
   TKM_TRY(d_fold.alloc((size_t)n * sizeof(int32_t), false, st));
   TKM_TRY(d_P.alloc((size_t)B * sizeof(double), false, st));
   TKM_TRY(d_gap.alloc((size_t)B * sizeof(double), false, st));
   TKM_CUDA(cudaMemcpyAsync(d_fold.p, foldid, n * sizeof(int32_t), cudaMemcpyHostToDevice, st));
-  GapEpi epi{(const double*)y, d_fold.as<int32_t>(), p->beta0.as<double>(), p->col_tau.as<double>(),
-             p->col_v.as<int32_t>(), (int)p->loss, p->smooth_final, lpart.as<double>(), dpart.as<double>(), ldpart};
-  TKM_TRY(gemm_f64_once(p->a.as<double>(), s->ldr, s->UL.as<double>(), s->ldr, B, (int)n, (int)r, epi, st));
-  gap_finalize_kernel<<<(unsigned)B, 256, 0, st>>>(lpart.as<double>(), dpart.as<double>(), ldpart, nblk, p->a.as<double>(),
-                                                   s->ldr, s->lam.as<double>(), (int)r, p->col_lam.as<double>(),
-                                                   p->col_nc.as<double>(), d_P.as<double>(), d_gap.as<double>());
-  TKM_LAUNCH_CHECK();
+  // every column at the level it ended on (all the same under the fixed schedule)
+  TKM_TRY(path_gap_device(p, (const double*)y, d_fold.as<int32_t>(), p->beta0.as<double>(), p->smooth_final,
+                          p->col_smooth.p ? p->col_smooth.as<double>() : nullptr, d_P.as<double>(), d_gap.as<double>(), st));
   TKM_CUDA(cudaMemcpyAsync(primal, d_P.p, (size_t)B * sizeof(double), cudaMemcpyDeviceToHost, st));
   TKM_CUDA(cudaMemcpyAsync(gap, d_gap.p, (size_t)B * sizeof(double), cudaMemcpyDeviceToHost, st));
   TKM_CUDA(cudaStreamSynchronize(st));

@@ -37,8 +37,9 @@ struct tkm_path {
   tkm::DevBuf beta0;    // [B]
   tkm::DevBuf col_lam, col_tau, col_nc;   // [B] per-column lambda, tau, n_c
   tkm::DevBuf col_v;    // [B] int32 held-out fold (V = none)
-  std::vector<double> h_beta0, h_kkt;
-  std::vector<int32_t> h_iters, h_flags;
+  tkm::DevBuf col_smooth;   // [B] smoothing level each column ended on (reading G23), unset for the smooth losses
+  std::vector<double> h_beta0, h_kkt, h_smooth;
+  std::vector<int32_t> h_iters, h_flags, h_level;
   int64_t total_col_iters = 0;
   // sampled CUDA-event timings of the two contractions (tkm_loss_opts.profile)
   // by kernel family and contraction: [0] DMMA GEMM-A, [1] DMMA GEMM-B, [2] tcgen05 A, [3] tcgen05 B
@@ -48,6 +49,9 @@ struct tkm_path {
 };
 
 namespace tkm {
+// cv_predict.cu: duality-gap certificate of every column (reading G22) on device arrays, asynchronous
+int path_gap_device(const tkm_path* p, const double* y, const int32_t* d_fold, const double* beta0, double smooth,
+                    const double* col_smooth, double* d_P, double* d_gap, cudaStream_t st);
 // transpose.cu-style helpers living in spectral.cu
 int transpose_scale_f64(const double* src, int64_t lds, int64_t rows, int64_t cols, const double* row_scale,
                         double* dst, int64_t ldd, cudaStream_t st);   // dst[c][r] = src[r][c] * row_scale[r]

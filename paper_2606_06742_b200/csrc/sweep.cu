@@ -378,6 +378,8 @@ struct RoundArgs {
   double *beta, *beta_prev, *bbar, *rk;   // [G*B]
   int32_t *done, *iters_round, *col_of_slot;   // [G*B]
   int32_t* nslots;         // [G]
+  const int32_t* active;   // [G*B] by gc or NULL: columns that take part in this round (reading G23); the others
+                           //   start as finished and leave the batch in the compaction that follows
 };
 
 __global__ void __launch_bounds__(256) init_round_kernel(RoundArgs p) {
@@ -405,7 +407,7 @@ __global__ void __launch_bounds__(256) init_round_kernel(RoundArgs p) {
     p.beta_prev[gc] = p.beta[gc];
     p.bbar[gc] = p.beta[gc];
     p.rk[gc] = 1.0;
-    p.done[gc] = 0;
+    p.done[gc] = (p.active && !p.active[gc]) ? 1 : 0;
     p.iters_round[gc] = 0;
     p.col_of_slot[gc] = col;
     if (col == 0) p.nslots[grp] = p.B;
@@ -432,6 +434,8 @@ struct UpdateArgs {
   float* da_lo;
   int64_t ldda;
   double* mu;      // [G*B] by gc or NULL: momentum used for the new abar
+  unsigned long long* fam_cnt;   // [4] or NULL (profile == 2): column-iterations by kernel family of this iteration's
+  int famA, famB;                //   two contractions (0 DMMA A, 1 DMMA B, 2 tcgen05 A, 3 tcgen05 B)
 };
 
 // One CTA per live slot.  The vectors are walked in chunks of 256 x UPD_EPT pairs with all loads of a chunk
@@ -597,6 +601,10 @@ __global__ void __launch_bounds__(256, 2) update_kernel(UpdateArgs p) {
     if (p.mu) p.mu[gc] = mu;
     p.kkt[gc] = kkt;
     p.iters[gc] += 1;
+    if (p.fam_cnt) {
+      atomicAdd(p.fam_cnt + p.famA, 1ull);
+      atomicAdd(p.fam_cnt + p.famB, 1ull);
+    }
     const int itr = p.iters_round[gc] + 1;
     p.iters_round[gc] = itr;
     if (kkt <= p.tol && p.exact) {
@@ -736,6 +744,28 @@ __global__ void __launch_bounds__(256) compact_apply_kernel(CompactArgs p) {
     }
   }
   if (threadIdx.x == 0) p.col_of_slot[g0 + sl] = p.col_of_slot[g0 + src];
+}
+
+// ---- outer control of the smoothing schedule (reading G23) -------------------------------------
+// mode 0 (screen):  pass[gc] = onsched[gc] && gap[gc] <= gap_tol
+// mode 1 (certify): columns with pass[gc] && gap[gc] <= gap_tol leave the schedule: onsched = 0, level = rnd
+// mode 2 (cap):     columns still on the schedule after the last round whose gap exceeds gap_tol get flag bit 2
+__global__ void outer_control_kernel(int mode, int GB, double gap_tol, int rnd, const double* __restrict__ gap,
+                                     int32_t* __restrict__ onsched, int32_t* __restrict__ pass, int32_t* __restrict__ level,
+                                     int32_t* __restrict__ flags) {
+  const int gc = blockIdx.x * blockDim.x + threadIdx.x;
+  if (gc >= GB) return;
+  const bool ok = gap[gc] <= gap_tol;
+  if (mode == 0) {
+    pass[gc] = (onsched[gc] && ok) ? 1 : 0;
+  } else if (mode == 1) {
+    if (pass[gc] && ok) {
+      onsched[gc] = 0;
+      level[gc] = rnd;
+    }
+  } else if (onsched[gc] && !ok) {
+    flags[gc] |= 2;
+  }
 }
 
 static double curvature_of(tkm_loss loss, double smooth) {
@@ -962,14 +992,18 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
   TKM_TRY(h_ns.alloc((size_t)POLL_RING * GEMM_MAX_GROUPS * sizeof(int32_t)));
 
   // events: one "poll landed" event per ring entry; optional GEMM sampling events per ring entry
+  const int check_every = opts->check_every > 0 ? opts->check_every : 16;
+  // profile == 1: two sampled iterations per batch; profile == 2: every iteration (all launches timed; the
+  // useful flops come from device-side column-iteration counters) -- a measurement mode, not for timed runs
+  const int nsamp = opts->profile == 2 ? check_every : 2;
   struct Events {
-    cudaEvent_t poll[POLL_RING] = {}, pev[POLL_RING][8] = {};   // pev: 2 sampled iterations x (A0, A1, B0, B1)
+    cudaEvent_t poll[POLL_RING] = {};
+    std::vector<cudaEvent_t> pev;   // [POLL_RING][nsamp][4]: (A0, A1, B0, B1) per sampled iteration
     ~Events() {
       for (auto& e : poll)
         if (e) cudaEventDestroy(e);
-      for (auto& row : pev)
-        for (auto& e : row)
-          if (e) cudaEventDestroy(e);
+      for (auto& e : pev)
+        if (e) cudaEventDestroy(e);
     }
   } ev;
   // TKM_SWEEP_TRACE=<file>: one line per batch (round, batch, live columns, widest group, tiles, ms) -- a
@@ -983,9 +1017,13 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
     }
   } trace_guard{trace};
   for (auto& e : ev.poll) TKM_CUDA(cudaEventCreateWithFlags(&e, trace ? cudaEventDefault : cudaEventDisableTiming));
-  if (opts->profile)
-    for (auto& row : ev.pev)
-      for (auto& e : row) TKM_CUDA(cudaEventCreate(&e));
+  if (opts->profile) {
+    ev.pev.assign((size_t)POLL_RING * nsamp * 4, nullptr);
+    for (auto& e : ev.pev) TKM_CUDA(cudaEventCreate(&e));
+  }
+  auto pev = [&](int ring, int sidx, int q) -> cudaEvent_t { return ev.pev[((size_t)ring * nsamp + sidx) * 4 + q]; };
+  DevBuf fam_cnt;
+  if (opts->profile == 2) TKM_TRY(fam_cnt.alloc(4 * sizeof(unsigned long long), true, st, true));
 
   // GEMM problems: A = abar x (U Lam)^T, B = Zt x (U^T)^T
   GemmProblem prA, prB;
@@ -1022,27 +1060,41 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
   GemmArgs argsA, argsB;
   GemmTile tileA{-1, 0, 0}, tileB{-1, 0, 0};
 
-  const int check_every = opts->check_every > 0 ? opts->check_every : 16;
   const int restart = opts->restart ? 1 : 0;
   // sampled launches, by kernel family and contraction: [0] DMMA GEMM-A, [1] DMMA GEMM-B, [2] tcgen05 A, [3] tcgen05 B
   double prof_ms[4] = {0.0, 0.0, 0.0, 0.0}, prof_flops[4] = {0.0, 0.0, 0.0, 0.0};
   int64_t prof_launches[4] = {0, 0, 0, 0};
-  int samp_kind[POLL_RING][4];   // per ring slot: family index of (iteration 0: A, B; last iteration: A, B), -1 = not sampled
-  double smooth = opts->smooth0;
-  for (int rnd = 0; rnd < rounds; ++rnd) {
-    if (smoothed && rnd > 0) smooth *= opts->eta;   // PAPER.md:220 (Alg.1 l.22)
+  std::vector<int> samp_kind((size_t)POLL_RING * nsamp * 2, -1);   // [ring][sampled iteration][A, B]: family or -1
+  // One smoothing round (S3-S7 until every participating column has met `rtol`) at level `smooth`; `active`
+  // ([G*B] device, or NULL = all columns) selects the participating columns (outer control, reading G23).
+  auto run_round = [&](int rnd, double smooth, double rtol, const int32_t* active) -> int {
     const double curv = curvature_of(loss, smooth);
-    const double rtol = (rnd + 1 < rounds && opts->warm_tol > 0.0) ? opts->warm_tol : tol;
     RoundArgs ra{(int)r, B, ldr, gp, curv, p0->col_lam.as<double>(), p0->col_nc.as<double>(), col_c.as<double>(),
                  col_s.as<double>(), A.as<double>(), Aprev.as<double>(), Abar.as<double>(), beta.as<double>(),
                  beta_prev.as<double>(), bbar.as<double>(), rk.as<double>(), done.as<int32_t>(),
-                 iters_round.as<int32_t>(), col_of_slot.as<int32_t>(), nslots.as<int32_t>()};
+                 iters_round.as<int32_t>(), col_of_slot.as<int32_t>(), nslots.as<int32_t>(), active};
     init_round_kernel<<<dim3(B, G), 256, 0, st>>>(ra);
     TKM_LAUNCH_CHECK();
 
     // Host view of the live-slot counts: an upper bound that lags the device by at most two batches.
     int bound[GEMM_MAX_GROUPS];
     for (int g = 0; g < G; ++g) bound[g] = B;
+    if (active) {
+      // columns outside the round leave the batch before its first iteration; the counts are read back once
+      CompactArgs c0{B, (int)r, ldr, gp, nslots.as<int32_t>(), col_of_slot.as<int32_t>(), done.as<int32_t>(),
+                     fin_list.as<int32_t>(), tail_list.as<int32_t>(), counts.as<int32_t>(), A.as<double>(),
+                     Aprev.as<double>(), Abar.as<double>(), nullptr, nullptr, ldn, (int)n, nullptr, nullptr, nullptr,
+                     nullptr, ldr32};
+      compact_plan_kernel<<<G, 1024, 0, st>>>(c0);
+      TKM_LAUNCH_CHECK();
+      compact_apply_kernel<<<dim3(B, G), 256, 0, st>>>(c0);
+      TKM_LAUNCH_CHECK();
+      TKM_CUDA(cudaMemcpyAsync(h_ns.as<int32_t>(), nslots.p, GEMM_MAX_GROUPS * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+      TKM_CUDA(cudaStreamSynchronize(st));
+      int tot = 0;
+      for (int g = 0; g < G; ++g) tot += (bound[g] = h_ns.as<int32_t>()[g]);
+      if (tot == 0) return TKM_OK;
+    }
     int64_t batch = 0, done_polls = 0;
     bool finished = false;
     while (!finished) {
@@ -1152,9 +1204,11 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
         // sampled launches: right after a compaction every slot is live, so the counted flops are all useful; the
         // delta form has its FP64 GEMM-B on the last iteration of the batch instead
         // first iteration after a compaction (every slot live) and, in the delta forms, the exact last iteration
-        const int sidx = !opts->profile ? -1 : (k == 0 ? 0 : ((dz_on && k == check_every - 1) ? 1 : -1));
-        if (k == 0) samp_kind[ring][0] = samp_kind[ring][1] = samp_kind[ring][2] = samp_kind[ring][3] = -1;
-        if (sidx >= 0) TKM_CUDA(cudaEventRecord(ev.pev[ring][4 * sidx + 0], st));
+        const int sidx = !opts->profile ? -1 : (opts->profile == 2 ? k : (k == 0 ? 0 : ((dz_on && k == check_every - 1) ? 1 : -1)));
+        if (k == 0) std::fill(samp_kind.begin() + (size_t)ring * nsamp * 2, samp_kind.begin() + (size_t)(ring + 1) * nsamp * 2, -1);
+        int* sk = samp_kind.data() + ((size_t)ring * nsamp + std::max(sidx, 0)) * 2;
+        int famA = 0, famB = 0;
+        if (sidx >= 0) TKM_CUDA(cudaEventRecord(pev(ring, sidx, 0), st));
         int nblkA = (int)ceil_div(n, tileA.BM);
         if (df_on && !exact_it) {
           // F half: F+ = Fbar - U Lam da on the tcgen05 tensor cores, loss derivative in its epilogue
@@ -1165,26 +1219,23 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
                       dz_lo.as<float>(), ldn32, gpart.as<double>(), ldpart, dz_blk_rows};
           TKM_TRY(gemm_tf32_launch(targsF, tcfg, G, fe, st));
           nblkA = (int)ceil_div(n, TF32_BM);
-          if (sidx >= 0) {
-            TKM_CUDA(cudaEventRecord(ev.pev[ring][4 * sidx + 1], st));
-            samp_kind[ring][2 * sidx] = 2;
-          }
+          famA = 2;
         } else {
           LossEpi le{(const double*)y, d_fold.as<int32_t>(), col_of_slot.as<int32_t>(), bbar.as<double>(),
                      p0->col_nc.as<double>(), p0->col_tau.as<double>(), p0->col_v.as<int32_t>(), B, (int)loss, smooth,
                      Zt.as<double>(), ldn, gpart.as<double>(), ldpart, dz_on ? dz_hi.as<float>() : nullptr,
                      dz_on ? dz_lo.as<float>() : nullptr, ldn32, df_on ? Fb.as<double>() : nullptr, dz_blk_rows};
           TKM_TRY(gemm_f64_launch(argsA, tileA, G, le, st));
-          if (sidx >= 0) {
-            TKM_CUDA(cudaEventRecord(ev.pev[ring][4 * sidx + 1], st));
-            samp_kind[ring][2 * sidx] = 0;
-          }
           if (df_on) {   // exact iteration of the F half: also F = U Lam a, so that both recurrence states are exact
-            StoreEpi fs{Fp.as<double>(), ldn, (int64_t)B * ldn, 1.0};
+            StoreEpi fs{Fp.as<double>(), ldn, (int64_t)B * ldn, 1.0};   // (its time counts for family 0, its flops do not)
             TKM_TRY(gemm_f64_launch(argsA2, tileA, G, fs, st));
           }
         }
-        if (sidx >= 0) TKM_CUDA(cudaEventRecord(ev.pev[ring][4 * sidx + 2], st));
+        if (sidx >= 0) {
+          TKM_CUDA(cudaEventRecord(pev(ring, sidx, 1), st));
+          sk[0] = famA + ((df_on && exact_it) ? 8 : 0);   // + 8: the timed span holds two FP64 GEMM-A launches
+          TKM_CUDA(cudaEventRecord(pev(ring, sidx, 2), st));
+        }
         if (exact_it) {
           // FP64 contraction; in delta form it also re-establishes zeta = U^T z exactly
           SpecEpi se{col_of_slot.as<int32_t>(), p0->col_lam.as<double>(), B, Abar.as<double>(), ldr, Rho.as<double>(),
@@ -1212,9 +1263,10 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
                      Rho.as<double>()};
           TKM_TRY(gemm_tf32_launch(targs, tcfg, G, ze, st));
         }
+        famB = exact_it ? 1 : 3;
         if (sidx >= 0) {
-          TKM_CUDA(cudaEventRecord(ev.pev[ring][4 * sidx + 3], st));
-          samp_kind[ring][2 * sidx + 1] = exact_it ? 1 : 3;
+          TKM_CUDA(cudaEventRecord(pev(ring, sidx, 3), st));
+          sk[1] = famB;
         }
         UpdateArgs ua{(int)r, (int)n, B, nblkA, restart, maxit, exact_it ? 1 : 0, ldr,
                       ldpart, rtol, gp, nslots.as<int32_t>(), col_of_slot.as<int32_t>(), p0->col_lam.as<double>(),
@@ -1223,7 +1275,8 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
                       Abar.as<double>(), beta.as<double>(), beta_prev.as<double>(), bbar.as<double>(), rk.as<double>(),
                       kkt.as<double>(), done.as<int32_t>(), iters.as<int32_t>(), iters_round.as<int32_t>(),
                       flags.as<int32_t>(), df_on ? da_hi.as<float>() : nullptr, df_on ? da_lo.as<float>() : nullptr,
-                      ldr32, df_on ? mu.as<double>() : nullptr};
+                      ldr32, df_on ? mu.as<double>() : nullptr,
+                      opts->profile == 2 ? fam_cnt.as<unsigned long long>() : nullptr, famA, famB};
         update_kernel<<<dim3(std::max(nmax, 1), G), 256, 0, st>>>(ua);
         TKM_LAUNCH_CHECK();
       }
@@ -1267,14 +1320,16 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
         }
         if (opts->profile && live_then > 0) {
           // the sampled launches of batch b precede its poll event; flops = 2 n r (live columns) per launch
-          for (int q = 0; q < 4; ++q) {
-            const int kind = samp_kind[cur][q];
+          for (int q = 0; q < 2 * nsamp; ++q) {
+            int kind = samp_kind[(size_t)cur * nsamp * 2 + q];
             if (kind < 0) continue;
+            const int twice = kind >= 8 ? 2 : 1;   // kernel roofline: both launches of the span did 2 n r live flops
+            kind &= 7;
             float ms = 0.f;
-            TKM_CUDA(cudaEventElapsedTime(&ms, ev.pev[cur][4 * (q >> 1) + 2 * (q & 1)], ev.pev[cur][4 * (q >> 1) + 2 * (q & 1) + 1]));
+            TKM_CUDA(cudaEventElapsedTime(&ms, pev(cur, q >> 1, 2 * (q & 1)), pev(cur, q >> 1, 2 * (q & 1) + 1)));
             prof_ms[kind] += ms;
-            prof_flops[kind] += 2.0 * (double)live_then * (double)n * (double)r;
-            prof_launches[kind] += 1;
+            prof_flops[kind] += twice * 2.0 * (double)live_then * (double)n * (double)r;   // profile == 2: replaced below
+            prof_launches[kind] += twice;
           }
         }
         if (trace && b >= 1) {
@@ -1287,10 +1342,64 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
       }
       ++batch;
     }
+    return TKM_OK;
+  };
+
+  // Smoothing schedule (S8).  gap_tol <= 0: the fixed schedule of reading G7.  gap_tol > 0: the
+  // outer control of reading G23 -- after round k < R-1 a column whose iterate certifies a duality gap of the
+  // non-smoothed problem <= gap_tol is finished at THIS level to `tol` (when the round stopped at warm_tol), tested
+  // again on the converged point and, if certified, leaves the schedule with that level's minimiser.
+  const bool outer = smoothed && rounds > 1 && opts->gap_tol > 0.0;
+  DevBuf onsched, passed, level, d_gapP, d_gapV;
+  if (smoothed) {
+    TKM_TRY(level.alloc((size_t)GB * sizeof(int32_t), false, st, true));
+    std::vector<int32_t> h_lv(GB, rounds - 1);
+    TKM_CUDA(cudaMemcpyAsync(level.p, h_lv.data(), GB * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    TKM_CUDA(cudaStreamSynchronize(st));   // h_lv is a local
+  }
+  if (outer) {
+    TKM_TRY(onsched.alloc((size_t)GB * sizeof(int32_t), false, st, true));
+    TKM_TRY(passed.alloc((size_t)GB * sizeof(int32_t), true, st, true));
+    TKM_TRY(d_gapP.alloc((size_t)GB * sizeof(double), false, st, true));
+    TKM_TRY(d_gapV.alloc((size_t)GB * sizeof(double), false, st, true));
+    TKM_CUDA(cudaMemsetAsync(onsched.p, 0x01, (size_t)GB * sizeof(int32_t), st));   // any non-zero value = on the schedule
+  }
+  auto gap_pass = [&](double smooth) -> int {   // d_gapV[gc] = gap of column gc at (a_out, beta) for level `smooth`
+    for (int g = 0; g < G; ++g)
+      TKM_TRY(path_gap_device(out[g], (const double*)y, d_fold.as<int32_t>(), beta.as<double>() + (size_t)g * B, smooth,
+                              nullptr, d_gapP.as<double>() + (size_t)g * B, d_gapV.as<double>() + (size_t)g * B, st));
+    return TKM_OK;
+  };
+  auto control = [&](int mode, int rnd) -> int {
+    outer_control_kernel<<<(unsigned)ceil_div(GB, 256), 256, 0, st>>>(mode, GB, opts->gap_tol, rnd, d_gapV.as<double>(),
+                                                                     onsched.as<int32_t>(), passed.as<int32_t>(),
+                                                                     level.as<int32_t>(), flags.as<int32_t>());
+    TKM_LAUNCH_CHECK();
+    return TKM_OK;
+  };
+  double smooth = opts->smooth0;
+  for (int rnd = 0; rnd < rounds; ++rnd) {
+    if (smoothed && rnd > 0) smooth *= opts->eta;   // PAPER.md:220 (Alg.1 l.22)
+    const bool last = rnd + 1 == rounds;
+    const double rtol = (!last && opts->warm_tol > 0.0) ? opts->warm_tol : tol;
+    TKM_TRY(run_round(rnd, smooth, rtol, outer ? onsched.as<int32_t>() : nullptr));
+    if (!outer) continue;
+    TKM_TRY(gap_pass(smooth));
+    if (last) {
+      TKM_TRY(control(2, rnd));
+      break;
+    }
+    TKM_TRY(control(0, rnd));
+    if (rtol > tol) {   // the warm iterate only screens
+      TKM_TRY(run_round(rnd, smooth, tol, passed.as<int32_t>()));
+      TKM_TRY(gap_pass(smooth));
+    }
+    TKM_TRY(control(1, rnd));
   }
   // results: beta0 per group, diagnostics to the host
   std::vector<double> hb(GB), hk(GB);
-  std::vector<int32_t> hi(GB), hf(GB);
+  std::vector<int32_t> hi(GB), hf(GB), hl(GB, 0);
+  if (smoothed) TKM_CUDA(cudaMemcpyAsync(hl.data(), level.p, GB * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
   for (int g = 0; g < G; ++g)
     TKM_CUDA(cudaMemcpyAsync(out[g]->beta0.p, beta.as<double>() + (size_t)g * B, (size_t)B * sizeof(double),
                              cudaMemcpyDeviceToDevice, st));
@@ -1298,7 +1407,11 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
   TKM_CUDA(cudaMemcpyAsync(hk.data(), kkt.p, GB * sizeof(double), cudaMemcpyDeviceToHost, st));
   TKM_CUDA(cudaMemcpyAsync(hi.data(), iters.p, GB * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
   TKM_CUDA(cudaMemcpyAsync(hf.data(), flags.p, GB * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  unsigned long long h_fam[4] = {0, 0, 0, 0};
+  if (opts->profile == 2) TKM_CUDA(cudaMemcpyAsync(h_fam, fam_cnt.p, sizeof(h_fam), cudaMemcpyDeviceToHost, st));
   TKM_CUDA(cudaStreamSynchronize(st));
+  if (opts->profile == 2)   // every launch was timed: the useful work is what the device counted, column by column
+    for (int q = 0; q < 4; ++q) prof_flops[q] = 2.0 * (double)n * (double)r * (double)h_fam[q];
   bool notconv = false;
   for (int g = 0; g < G; ++g) {
     tkm_path* p = out[g];
@@ -1307,10 +1420,17 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
     p->h_kkt.assign(hk.begin() + (size_t)g * B, hk.begin() + (size_t)(g + 1) * B);
     p->h_iters.assign(hi.begin() + (size_t)g * B, hi.begin() + (size_t)(g + 1) * B);
     p->h_flags.assign(hf.begin() + (size_t)g * B, hf.begin() + (size_t)(g + 1) * B);
+    p->h_level.assign(hl.begin() + (size_t)g * B, hl.begin() + (size_t)(g + 1) * B);
+    p->h_smooth.assign(B, 0.0);
+    if (smoothed) {
+      for (int c = 0; c < B; ++c) p->h_smooth[c] = opts->smooth0 * std::pow(opts->eta, (double)p->h_level[c]);
+      TKM_TRY(p->col_smooth.alloc((size_t)B * sizeof(double), false, st));
+      TKM_CUDA(cudaMemcpy(p->col_smooth.p, p->h_smooth.data(), (size_t)B * sizeof(double), cudaMemcpyHostToDevice));
+    }
     p->total_col_iters = 0;
     for (int c = 0; c < B; ++c) {
       p->total_col_iters += p->h_iters[c];
-      notconv |= p->h_flags[c] != 0;
+      notconv |= (p->h_flags[c] & 1) != 0;
     }
   }
   // sampled timings cover all groups of the shared launches: reported on the first path
@@ -1345,6 +1465,13 @@ extern "C" int tkm_path_info(const tkm_path* p, int32_t* B, int64_t* r, int32_t*
   if (flags) memcpy(flags, p->h_flags.data(), p->B * sizeof(int32_t));
   if (beta0) memcpy(beta0, p->h_beta0.data(), p->B * sizeof(double));
   if (total_col_iters) *total_col_iters = p->total_col_iters;
+  return TKM_OK;
+}
+
+extern "C" int tkm_path_levels(const tkm_path* p, int32_t* level, double* smooth) {
+  if (!p) return set_error(TKM_EINVAL, "tkm_path_levels: NULL handle");
+  if (level) memcpy(level, p->h_level.data(), p->B * sizeof(int32_t));
+  if (smooth) memcpy(smooth, p->h_smooth.data(), p->B * sizeof(double));
   return TKM_OK;
 }
 
