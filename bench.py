@@ -712,6 +712,9 @@ def main():
         if args.impl != "ours" or world != 1 or args.gpus != 1:
             raise SystemExit("--workload %s: one GPU, --impl ours only" % args.workload)
         return run_single(args)
+    if args.tf32_delta >= 0:
+        global TF32_DELTA
+        TF32_DELTA = args.tf32_delta
     from paper_2606_06742_b200.ranks import replica_seed
     w = wl.config1(seed=replica_seed(1001, rank if args.impl == "ours" else 0))
     if args.impl == "reference":

@@ -157,7 +157,9 @@ int tkm_spectral_get_u(const tkm_spectral* s, double* U_out, void* stream);
  *   y       [dev]  n FP64 (+-1 for HINGE / LOGISTIC / DWD, checked; real for QUANTILE)
  *   lambdas [host] L values > 0          foldid [host] n values in [0, V), every fold non-empty
  *   tol     stop when max(|1^T z|, n_c ||rho||_2 / sqrt(n)) <= tol per column (reading G6)
- *   maxit   per column per round; columns that hit it are flagged and TKM_ENOTCONV is returned
+ *   maxit   per column per round; columns that hit it are flagged and TKM_ENOTCONV is returned (in the delta
+ *           forms both decisions -- converged, or out of iterations -- are taken on the exact iterations only,
+ *           so a column may run up to 2 check_every - 1 iterations past maxit before it is flagged)
  *   warm    optional path of the same shape on the same spectral handle to start from, or NULL
  * The path keeps a pointer to `s`, which must outlive it.  Synchronises `stream`. */
 int tkm_fit_path(const tkm_spectral* s, const void* y, tkm_loss loss, const tkm_loss_opts* opts,

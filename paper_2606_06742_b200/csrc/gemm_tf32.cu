@@ -37,8 +37,6 @@ __global__ void split_tf32_kblocked_kernel(const double* __restrict__ src, int64
   }
 }
 
-int tf32_bn_of(int cfg) { return cfg == 0 ? 64 : (cfg == 1 ? 128 : 256); }
-
 int split_tf32(const double* src, int64_t lds, int64_t rows, int64_t cols, float* hi, float* lo, int64_t ldo,
                cudaStream_t st) {
   dim3 grid((unsigned)rows, (unsigned)std::min<int64_t>(ceil_div(cols, 256), 64));
@@ -59,8 +57,9 @@ int split_tf32_kblocked(const double* src, int64_t lds, int64_t rows, int64_t co
 using namespace tkm;
 
 // Dt[N][M] (FP64) = P[N][K] Q[M][K]^T with both FP64 inputs split into TF32 (hi, lo) pairs on the fly and the
-// product formed by the 3xTF32 tcgen05 kernel (FP32 accumulation).  cfg: 0/1/2 = 64/128/256 slots per tile,
-// -1 = by N.  Test / calibration entry; ms [host] may be NULL, else the kernel time of `iters` launches.
+// product formed by the 3xTF32 tcgen05 kernel (FP32 accumulation).  cfg is ignored (kept for ABI stability: the
+// pair kernel has one tile shape).  Test / calibration entry; ms [host] may be NULL, else the kernel time of
+// `iters` launches.
 extern "C" int tkm_tf32x3_gemm_nt(const double* P, int64_t ldp, const double* Q, int64_t ldq, double* Dt, int64_t ldd,
                                   int64_t N, int64_t M, int64_t K, int32_t cfg, int32_t iters, float* ms, void* stream) {
   if (!P || !Q || !Dt || N < 1 || M < 1 || K < 1 || ldp < K || ldq < K || ldd < M || N > (1 << 24) || M > (1 << 24) ||
@@ -76,14 +75,14 @@ extern "C" int tkm_tf32x3_gemm_nt(const double* P, int64_t ldp, const double* Q,
   TKM_TRY(ql.alloc((size_t)M * ldk * sizeof(float), true, st));
   TKM_TRY(split_tf32(P, ldp, N, K, ph.as<float>(), pl.as<float>(), ldk, st));
   TKM_TRY(split_tf32(Q, ldq, M, K, qh.as<float>(), ql.as<float>(), ldk, st));
-  if (cfg < 0) cfg = N <= 64 ? 0 : (N <= 128 ? 1 : 2);
-  const int bn = tf32_bn_of(cfg);
   Tf32Args a;
   memset(&a, 0, sizeof(a));
-  TKM_TRY(make_tmap_f32(&a.p_hi, ph.as<float>(), N, K, ldk, bn));
-  TKM_TRY(make_tmap_f32(&a.p_lo, pl.as<float>(), N, K, ldk, bn));
+  TKM_TRY(make_tmap_f32(&a.p_hi, ph.as<float>(), N, K, ldk, TF32_PBOX));
+  TKM_TRY(make_tmap_f32(&a.p_lo, pl.as<float>(), N, K, ldk, TF32_PBOX));
   TKM_TRY(make_tmap_f32(&a.q_hi[0], qh.as<float>(), M, K, ldk, TF32_BM));
   TKM_TRY(make_tmap_f32(&a.q_lo[0], ql.as<float>(), M, K, ldk, TF32_BM));
+  Tf32Scratch sc;
+  TKM_TRY(sc.alloc(st));
   a.nslots = nullptr;
   a.p_group_rows = (int)N;
   a.N = (int)N;
@@ -95,13 +94,22 @@ extern "C" int tkm_tf32x3_gemm_nt(const double* P, int64_t ldp, const double* Q,
     TKM_CUDA(cudaEventCreate(&e0));
     TKM_CUDA(cudaEventCreate(&e1));
   }
-  int rc = gemm_tf32_launch(a, cfg, 1, epi, st);
+  int rc = gemm_tf32_launch(a, 1, sc, epi, st);
   if (ms && rc == TKM_OK) {
     cudaEventRecord(e0, st);
-    for (int i = 0; i < std::max(iters, 1) && rc == TKM_OK; ++i) rc = gemm_tf32_launch(a, cfg, 1, epi, st);
+    for (int i = 0; i < std::max(iters, 1) && rc == TKM_OK; ++i) rc = gemm_tf32_launch(a, 1, sc, epi, st);
     cudaEventRecord(e1, st);
   }
   cudaError_t e = cudaStreamSynchronize(st);   // the split buffers are freed on return
+  if (sc.dbg.p) {   // TKM_SK_DEBUG: intervals of pair 0's last launch
+    std::vector<unsigned long long> h(8192);
+    cudaMemcpy(h.data(), sc.dbg.p, 8192 * sizeof(unsigned long long), cudaMemcpyDeviceToHost);
+    fprintf(stderr, "mma full-wait stamps (delta clk): ");
+    for (int i = 1; i < 64 && h[i]; ++i) fprintf(stderr, "%llu ", h[i] - h[i - 1]);
+    fprintf(stderr, "\nproducer issue stamps (delta clk): ");
+    for (int i = 1; i < 64 && h[4096 + i]; ++i) fprintf(stderr, "%llu ", h[4096 + i] - h[4096 + i - 1]);
+    fprintf(stderr, "\nproducer[0] -> mma[0]: %lld clk\n", (long long)(h[0] - h[4096]));
+  }
   if (e != cudaSuccess) rc = set_error(TKM_ECUDA, "tkm_tf32x3_gemm_nt: %s", cudaGetErrorString(e));
   if (ms) {
     if (rc == TKM_OK) {

@@ -83,6 +83,7 @@ struct LossEpi {
   int64_t lddz;
   double* Fb;                // [G*B][ldz] by gs or NULL: keeps Fbar = U Lam abar for the delta-form GEMM-A
   int dz_blk_rows;           // 0: dz row-major; G*B: dz K-blocked (dz_index)
+
   template <class Cfg>
   __device__ __forceinline__ void run(double (&acc)[Cfg::TN][Cfg::TM][2], int n_blk0, int m_blk0, int warp_n,
                                       int warp_m, int lane, int N, int M, int grp, double* scratch) const {
@@ -179,47 +180,33 @@ struct SpecEpi {
   }
 };
 
-// ---- delta-form GEMM-B epilogue (tcgen05 kernel): zeta += U^T dz, rho = zeta + 2 lam abar --------------------
-// Thread = one spectral index i (a TMEM lane), 16 consecutive slots per call; for a fixed slot the 32 lanes
-// of a warp touch 32 consecutive doubles.
-struct ZetaEpi {
+// ---- epilogue of the tcgen05 delta-form contractions: the raw FP32 product, one slot per row ----------------------
+// Thread = one output index m (a TMEM lane), 16 consecutive slots per call; for a fixed slot the 32 lanes of a
+// warp store 128 contiguous bytes.  The FP64 state updates that consume the product (F+ = Fbar - U Lam da with the
+// loss derivative; zeta += U^T dz) are NOT fused here: a tensor-memory epilogue has 8 warps per SM to hide the
+// latency of ~8 FP64 loads and stores per element and ran at < 1 TB/s (ncu, profiles/r02_pair_kernel.md: 354 us
+// per launch at full width, tensor pipe 17 %), while the same arithmetic as a plain elementwise kernel over all
+// (slot, m) streams at HBM speed and the product costs 4 bytes per element to pass through L2.
+struct ProdEpi {
   static constexpr bool kReduce = false;
-  const int32_t* col_of_slot;   // [G*B]
-  const double* col_lam;        // [B]
+  float* out;        // [G*B][ldo] by gs
+  int64_t ldo;
   int B;
-  const double* Abar;           // [G*B][lda]
-  int64_t lda;
-  double* Zeta;                 // [G*B][lda]
-  double* Rho;                  // [G*B][lda]
-  __device__ __forceinline__ void chunk(const float (&v)[16], int i, int n0, int N, int M, int grp, double*, int) const {
-    if (i >= M) return;
-    const int g0 = grp * B;
+  __device__ __forceinline__ void chunk(const float (&v)[16], int m, int n0, int N, int M, int grp, double*, int) const {
+    if (m >= M) return;
+    float* base = out + (int64_t)(grp * B + n0) * ldo + m;
     const int cnt = min(16, N - n0);
-    // all loads of the chunk first (16 independent round trips in flight), then the arithmetic and the stores
-    double zo[16], ab[16], tl[16];
 #pragma unroll
     for (int k = 0; k < 16; ++k)
-      if (k < cnt) {
-        const int64_t o = (int64_t)(g0 + n0 + k) * lda + i;
-        zo[k] = Zeta[o];
-        ab[k] = Abar[o];
-        tl[k] = 2.0 * col_lam[col_of_slot[g0 + n0 + k]];
-      }
-#pragma unroll
-    for (int k = 0; k < 16; ++k)
-      if (k < cnt) {
-        const int64_t o = (int64_t)(g0 + n0 + k) * lda + i;
-        const double z = zo[k] + (double)v[k];
-        Zeta[o] = z;
-        Rho[o] = z + tl[k] * ab[k];
-      }
+      if (k < cnt) base[(int64_t)k * ldo] = v[k];
   }
 };
 
 // ---- K-split GEMM-B (thin U: r x B outputs, n ~ 10^5..10^6 deep) ------------------------------------------------
 // With few output tiles and a very long contraction the launch cannot fill the SMs, so K is cut into S ranges
-// (GemmArgs / Tf32Args::ksplit): every CTA stores its partial U^T z (or U^T dz) into part[split], and
-// spec_finalize_kernel sums the S partials in a fixed order and applies the SpecEpi / ZetaEpi arithmetic.
+// (GemmArgs::ksplit): every CTA stores its partial U^T z into part[split], and spec_finalize_kernel sums the S
+// partials in a fixed order and applies the SpecEpi arithmetic.  (The tcgen05 kernel needs none of this: its
+// stream-K partition cuts along K by itself.)
 struct PartEpi {   // FP64 DMMA kernel
   int B, ksplit;
   int64_t lda, split_stride;
@@ -246,21 +233,6 @@ struct PartEpi {   // FP64 DMMA kernel
   }
 };
 
-struct ZetaPartEpi {   // tcgen05 kernel
-  static constexpr bool kReduce = false;
-  int B, ksplit;
-  int64_t lda, split_stride;
-  double* part;
-  __device__ __forceinline__ void chunk(const float (&v)[16], int i, int n0, int N, int M, int grp, double*, int) const {
-    if (i >= M) return;
-    double* base = part + (int64_t)gemm_split_index(ksplit) * split_stride + (int64_t)(grp * B + n0) * lda + i;
-    const int cnt = min(16, N - n0);
-#pragma unroll
-    for (int k = 0; k < 16; ++k)
-      if (k < cnt) base[(int64_t)k * lda] = (double)v[k];
-  }
-};
-
 // zeta = (accumulate ? Zeta : 0) + sum_s part[s];  Zeta <- zeta (if kept);  rho = zeta + 2 lam abar
 __global__ void __launch_bounds__(256) spec_finalize_kernel(const double* __restrict__ part, int S, int64_t split_stride,
                                                             const int32_t* __restrict__ nslots,
@@ -281,22 +253,24 @@ __global__ void __launch_bounds__(256) spec_finalize_kernel(const double* __rest
   Rho[o] = z + 2.0 * col_lam[col_of_slot[grp * B + slot]] * Abar[o];
 }
 
-// ---- delta-form GEMM-A epilogue (tcgen05 kernel): F+ = Fbar - U Lam da, next extrapolation, loss derivative ----
-// Thread = one sample row m (a TMEM lane), 16 consecutive slots per call.  State per slot: Fb = Fbar_k (what the
-// loss saw), Fp = F_k.  With G = U Lam da_k from the accumulator:  F_{k+1} = Fbar_k - G,
-// Fbar_{k+1} = F_{k+1} + mu_{k+1} (F_{k+1} - F_k), then z, dz and the column sum of z exactly as in LossEpi.
-struct FLossEpi {
-  static constexpr bool kReduce = true;
+// ---- delta form of S5 (after the tcgen05 GEMM-A): F+ = Fbar - U Lam da, next extrapolation, loss derivative ------
+// One thread per (slot, sample m).  State per slot: Fb = Fbar_k (what the loss saw), Fp = F_k.  With G = U Lam da_k
+// from the tcgen05 product:  F_{k+1} = Fbar_k - G,  Fbar_{k+1} = F_{k+1} + mu_{k+1} (F_{k+1} - F_k), then z, dz and
+// the per-block column sums of z exactly as in LossEpi (summed in a fixed order by update_kernel).
+struct FLossArgs {
   const double* y;
   const int32_t* foldid;
+  const int32_t* nslots;        // [G]
   const int32_t* col_of_slot;   // [G*B]
   const double* bbar;           // [G*B] by gc
   const double* mu;             // [G*B] by gc: momentum that formed the current abar
   const double* col_nc;
   const double* col_tau;
   const int32_t* col_v;
-  int B, loss;
+  int B, loss, n;
   double smooth, inv_2s;
+  const float* prod;            // [G*B][ldprod] by gs: U Lam da
+  int64_t ldprod;
   double* Fb;                   // [G*B][ldz]
   double* Fp;                   // [G*B][ldz]
   double* Zt;                   // [G*B][ldz]
@@ -304,65 +278,42 @@ struct FLossEpi {
   float* dz_hi;
   float* dz_lo;
   int64_t lddz;
-  double* gpart;
+  double* gpart;                // [blocks along m][ldpart] by gs
   int64_t ldpart;
   int dz_blk_rows;
-  __device__ __forceinline__ void chunk(const float (&v)[16], int m, int n0, int N, int M, int grp, double* red,
-                                        int lane) const {
-    const bool live = m < M;
-    const double yv = live ? y[m] : 0.0;
-    const int fv = live ? foldid[m] : -1;
-    const int g0 = grp * B;
-    const int cnt = min(16, N - n0);
-    // per half chunk: all loads first (independent round trips in flight), then the arithmetic and the stores
+};
+constexpr int FLOSS_THREADS = 256, FLOSS_EPT = 2;   // samples per block: 512
+__global__ void __launch_bounds__(FLOSS_THREADS) floss_kernel(FLossArgs p) {
+  __shared__ double red[32];
+  const int slot = blockIdx.y, grp = blockIdx.z;
+  if (slot >= p.nslots[grp]) return;
+  const int gs = grp * p.B + slot, col = p.col_of_slot[gs], gc = grp * p.B + col;
+  const double mu = p.mu[gc], bb = p.bbar[gc], inv_nc = 1.0 / p.col_nc[col], tau = p.col_tau[col];
+  const int hv = p.col_v[col];
+  double zsum = 0.0;
 #pragma unroll
-    for (int h0 = 0; h0 < 16; h0 += 8) {
-      double fbv[8], fpv[8], zov[8], muv[8], bbv[8], ncv[8], tav[8];
-      int hv[8];
-#pragma unroll
-      for (int k = 0; k < 8; ++k)
-        if (h0 + k < cnt) {
-          const int gs = g0 + n0 + h0 + k, col = col_of_slot[gs], gc = g0 + col;
-          muv[k] = mu[gc];
-          bbv[k] = bbar[gc];
-          ncv[k] = 1.0 / col_nc[col];
-          tav[k] = col_tau[col];
-          hv[k] = col_v[col];
-          if (live) {
-            const int64_t o = (int64_t)gs * ldz + m;
-            fbv[k] = Fb[o];
-            fpv[k] = Fp[o];
-            zov[k] = Zt[o];
-          }
-        }
-#pragma unroll
-      for (int k = 0; k < 8; ++k)
-        if (h0 + k < cnt) {
-          double z = 0.0;
-          if (live) {
-            const int gs = g0 + n0 + h0 + k;
-            const int64_t o = (int64_t)gs * ldz + m;
-            const double fn = fbv[k] - (double)v[h0 + k];
-            const double fb = fn + muv[k] * (fn - fpv[k]);
-            Fp[o] = fn;
-            Fb[o] = fb;
-            if (fv != hv[k]) z = psi_fast(loss, yv, fb + bbv[k], smooth, inv_2s, tav[k]) * ncv[k];
-            const double d = z - zov[k];
-            Zt[o] = z;
-            const float h = to_tf32((float)d);
-            const int64_t od = dz_index(gs, m, lddz, dz_blk_rows);
-            dz_hi[od] = h;
-            dz_lo[od] = to_tf32((float)(d - (double)h));
-          }
-          const double t = warp_sum(z);
-          if (lane == 0) red[h0 + k] = t;
-        }
+  for (int e = 0; e < FLOSS_EPT; ++e) {
+    const int m = (blockIdx.x * FLOSS_EPT + e) * FLOSS_THREADS + threadIdx.x;
+    if (m < p.n) {
+      const int64_t o = (int64_t)gs * p.ldz + m;
+      const double fn = p.Fb[o] - (double)p.prod[(int64_t)gs * p.ldprod + m];
+      const double fb = fn + mu * (fn - p.Fp[o]);
+      p.Fp[o] = fn;
+      p.Fb[o] = fb;
+      double z = 0.0;
+      if (p.foldid[m] != hv) z = psi_fast(p.loss, p.y[m], fb + bb, p.smooth, p.inv_2s, tau) * inv_nc;
+      const double d = z - p.Zt[o];
+      p.Zt[o] = z;
+      const float h = to_tf32((float)d);
+      const int64_t od = dz_index(gs, m, p.lddz, p.dz_blk_rows);
+      p.dz_hi[od] = h;
+      p.dz_lo[od] = to_tf32((float)(d - (double)h));
+      zsum += z;
     }
   }
-  __device__ __forceinline__ void finish(int slot, double total, int mtile, int grp) const {
-    gpart[(int64_t)mtile * ldpart + grp * B + slot] = total;
-  }
-};
+  zsum = block_sum(zsum, red);   // fixed order: deterministic
+  if (threadIdx.x == 0) p.gpart[(int64_t)blockIdx.x * p.ldpart + gs] = zsum;
+}
 
 // ---- per-round initialisation (S3, G4): constants c, s; a' = a; abar = a; r = 1 ------------------
 struct RoundArgs {
@@ -434,6 +385,10 @@ struct UpdateArgs {
   float* da_lo;
   int64_t ldda;
   double* mu;      // [G*B] by gc or NULL: momentum used for the new abar
+  const float* zinc;   // [G*B][ldzinc] by gs or NULL: the tcgen05 product U^T dz of a delta-form iteration; then
+  int64_t ldzinc;      //   zeta <- zeta + zinc (FP64 state `Zeta`), rho = zeta + 2 lam abar is formed here
+  double* Zeta;        // [G*B][lda] by gs (with zinc)
+  double* RhoW;        // [G*B][lda]: rho is kept for the second pass when the vector does not fit one chunk
   unsigned long long* fam_cnt;   // [4] or NULL (profile == 2): column-iterations by kernel family of this iteration's
   int famA, famB;                //   two contractions (0 DMMA A, 1 DMMA B, 2 tcgen05 A, 3 tcgen05 B)
 };
@@ -457,7 +412,7 @@ __global__ void __launch_bounds__(256, 2) update_kernel(UpdateArgs p) {
   const double lamc = p.col_lam[col], c = p.col_c[col], s = p.col_s[gc], nc = p.col_nc[col];
   const double two_lam = 2.0 * lamc;
   const int64_t off2 = ((int64_t)gs * p.lda) >> 1;   // lda is a multiple of 16
-  const double2* __restrict__ Rho2 = reinterpret_cast<const double2*>(p.Rho) + off2;
+  const double2* Rho2 = reinterpret_cast<const double2*>(p.Rho) + off2;   // (may alias RhoW in the delta form)
   double2* __restrict__ A2 = reinterpret_cast<double2*>(p.A) + off2;
   double2* __restrict__ Ap2 = reinterpret_cast<double2*>(p.Aprev) + off2;
   double2* __restrict__ Ab2 = reinterpret_cast<double2*>(p.Abar) + off2;
@@ -469,17 +424,28 @@ __global__ void __launch_bounds__(256, 2) update_kernel(UpdateArgs p) {
   double2 rho[UPD_EPT], ab[UPD_EPT], lm[UPD_EPT], uu[UPD_EPT], a_old[UPD_EPT], a_new[UPD_EPT];
   double g0 = 0.0, qd = 0.0, r2 = 0.0;
   for (int b = tid; b < p.nblkA; b += 256) g0 += p.gpart[(int64_t)b * p.ldpart + gs];
+  double2* __restrict__ Zeta2 = p.zinc ? reinterpret_cast<double2*>(p.Zeta) + off2 : nullptr;
+  double2* RhoW2 = p.zinc ? reinterpret_cast<double2*>(p.RhoW) + off2 : nullptr;
+  const float2* __restrict__ zinc2 = p.zinc ? reinterpret_cast<const float2*>(p.zinc + (int64_t)gs * p.ldzinc) : nullptr;
   for (int base = 0; base < npair; base += 256 * UPD_EPT) {
 #pragma unroll
     for (int e = 0; e < UPD_EPT; ++e) {
       const int i = base + e * 256 + tid;
       if (i < npair) {
-        rho[e] = Rho2[i];
         lm[e] = lam2[i];
         uu[e] = u12[i];
-        if (single) {
-          ab[e] = Ab2[i];
-          a_old[e] = A2[i];
+        if (single || zinc2) ab[e] = Ab2[i];
+        if (single) a_old[e] = A2[i];
+        if (zinc2) {
+          // delta form of S6: zeta += U^T dz (the tcgen05 product), rho = zeta + 2 lam abar
+          const double2 ze = Zeta2[i];
+          const float2 zi = zinc2[i];   // columns beyond r are never written and stay zero
+          const double2 zn = make_double2(ze.x + (double)zi.x, ze.y + (double)zi.y);
+          Zeta2[i] = zn;
+          rho[e] = make_double2(zn.x + two_lam * ab[e].x, zn.y + two_lam * ab[e].y);
+          if (!single) RhoW2[i] = rho[e];
+        } else {
+          rho[e] = Rho2[i];
         }
       }
     }
@@ -520,7 +486,7 @@ __global__ void __launch_bounds__(256, 2) update_kernel(UpdateArgs p) {
       for (int e = 0; e < UPD_EPT; ++e) {
         const int i = base + e * 256 + tid;
         if (i < npair) {
-          rho[e] = Rho2[i];
+          rho[e] = zinc2 ? RhoW2[i] : Rho2[i];
           ab[e] = Ab2[i];
           a_old[e] = A2[i];
           lm[e] = lam2[i];
@@ -607,11 +573,15 @@ __global__ void __launch_bounds__(256, 2) update_kernel(UpdateArgs p) {
     }
     const int itr = p.iters_round[gc] + 1;
     p.iters_round[gc] = itr;
-    if (kkt <= p.tol && p.exact) {
-      p.done[gc] = 1;
-    } else if (itr >= p.maxit) {
-      p.done[gc] = 1;
-      p.flags[gc] = 1;
+    // a column leaves the batch only on an exact iteration (in the delta forms rho carries the drift of the
+    // recurrence): converged if its residual meets tol, else flagged once it has used up maxit
+    if (p.exact) {
+      if (kkt <= p.tol) {
+        p.done[gc] = 1;
+      } else if (itr >= p.maxit) {
+        p.done[gc] = 1;
+        p.flags[gc] |= 1;
+      }
     }
   }
 }
@@ -779,8 +749,19 @@ constexpr int KSPLIT_MAX = 16;
 constexpr int KBLOCK_F64_MIN_K = 16384;   // thin U: from this n on, the FP64 GEMM-B reads a K-blocked copy of U^T
 constexpr int KBLOCK_MIN_K = 8192;   // contraction depth from which the tcgen05 GEMM-B operands are kept K-blocked (no effect
                                     // at n = 2000, where U^T stays in L2; 2.4x at n = 581012)
-constexpr int DELTA_MIN_LIVE = 48;   // live columns (all groups) below which the delta forms are switched off
-constexpr int POLL_RING = 5;   // ring of poll results: up to POLL_RING - 2 batches may be in flight
+constexpr int DELTA_MIN_LIVE = 48;   // live columns (all groups) below which the delta forms are always switched off
+constexpr int POLL_RING = 8;   // ring of poll results: up to POLL_RING - 2 batches may be in flight
+
+// Live columns (all groups) from which a tcgen05 delta-form launch beats the FP64 DMMA launch it replaces.  The pair
+// kernel's time has a floor that does not depend on the width -- a chain of 12 dependent MMAs per 32-deep K tile at
+// about 55 ns each (measured, profiles/r02_pair_kernel.md) plus ~12 us of prologue and epilogue -- while the DMMA
+// launch costs 2 n r N / (18 TFLOP/s).  n = r = 2000: 121 columns; n = r >= 10^4: the floor DELTA_MIN_LIVE.
+static int delta_min_live(int64_t n, int64_t r) {
+  const double kt = 0.5 * ((double)ceil_div(n, 32) + (double)ceil_div(r, 32));   // mean K depth of the two contractions
+  const double t_tc = kt * 0.66e-6 + 12e-6;
+  const double cols = t_tc * 18e12 / (2.0 * (double)n * (double)r);
+  return std::max(DELTA_MIN_LIVE, (int)cols);
+}
 
 }  // namespace tkm
 
@@ -982,12 +963,17 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
         TKM_TRY(split_tf32(specs[g]->UL.as<double>(), ldr, n, r, ul_hi[g].as<float>(), ul_lo[g].as<float>(), ldr32, st));
     }
   }
+  GemmProblem prA2 = {};   // F = U Lam a on the exact iterations of the F half (same tiles as GEMM-A, P = a)
+  GemmArgs argsA2;
   Tf32Args targs, targsF;
+  DevBuf prodA, prodB;   // FP32 products of the tcgen05 contractions: U Lam da [G*B][ldn32], U^T dz [G*B][ldr32]
+  if (delta) TKM_TRY(prodB.alloc((size_t)GB * ldr32 * sizeof(float), true, st, true));
+  if (delta_f) TKM_TRY(prodA.alloc((size_t)GB * ldn32 * sizeof(float), true, st, true));
+  Tf32Scratch tsc;   // stream-K exchange buffers of the tcgen05 launches of this sweep
+  if (opts->tf32_delta != 0) TKM_TRY(tsc.alloc(st));
   memset(&targs, 0, sizeof(targs));
   memset(&targsF, 0, sizeof(targsF));
   int tcfg = -1;
-  GemmProblem prA2 = {};   // F = U Lam a on the exact iterations of the F half (same tiles as GEMM-A, P = a)
-  GemmArgs argsA2;
   PinBuf h_ns;   // [POLL_RING][GEMM_MAX_GROUPS] live-slot counts read back after every compaction
   TKM_TRY(h_ns.alloc((size_t)POLL_RING * GEMM_MAX_GROUPS * sizeof(int32_t)));
 
@@ -995,7 +981,13 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
   const int check_every = opts->check_every > 0 ? opts->check_every : 16;
   // profile == 1: two sampled iterations per batch; profile == 2: every iteration (all launches timed; the
   // useful flops come from device-side column-iteration counters) -- a measurement mode, not for timed runs
-  const int nsamp = opts->profile == 2 ? check_every : 2;
+  // With the delta forms on and a wide batch the exact FP64 iteration (two DMMA contractions against 2 x (ce - 1)
+  // tcgen05 ones) is the larger part of a batch: such batches run 2 x check_every iterations between exact ones.
+  const char* ce_env = getenv("TKM_CE_MULT");   // tuning aid: multiplier of the batch length of wide delta-form batches
+  const int ce_mult = ce_env && *ce_env ? std::max(1, std::min(8, atoi(ce_env))) : 2;
+  const int ce_max = opts->tf32_delta != 0 ? ce_mult * check_every : check_every;
+  const int nsamp = opts->profile == 2 ? ce_max : 2;
+  const int dmin = delta_min_live(s0->n, s0->r);
   struct Events {
     cudaEvent_t poll[POLL_RING] = {};
     std::vector<cudaEvent_t> pev;   // [POLL_RING][nsamp][4]: (A0, A1, B0, B1) per sampled iteration
@@ -1065,6 +1057,7 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
   double prof_ms[4] = {0.0, 0.0, 0.0, 0.0}, prof_flops[4] = {0.0, 0.0, 0.0, 0.0};
   int64_t prof_launches[4] = {0, 0, 0, 0};
   std::vector<int> samp_kind((size_t)POLL_RING * nsamp * 2, -1);   // [ring][sampled iteration][A, B]: family or -1
+  int ce_of[POLL_RING] = {};   // iterations of the batch in each ring slot (trace)
   // One smoothing round (S3-S7 until every participating column has met `rtol`) at level `smooth`; `active`
   // ([G*B] device, or NULL = all columns) selects the participating columns (outer control, reading G23).
   auto run_round = [&](int rnd, double smooth, double rtol, const int32_t* active) -> int {
@@ -1123,11 +1116,11 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
         argsB.nslots = nslots.as<int32_t>();
         tileB = tB;
       }
-      argsA.N = argsB.N = std::max(nmax, 1);
+      argsA.N = argsB.N = argsA2.N = std::max(nmax, 1);
       if (delta) {
-        const int want = nmax <= 64 ? 0 : (nmax <= 128 ? 1 : 2);
+        const int want = 0;   // one tile shape: the maps are built once
         if (want != tcfg) {
-          const int bn = tf32_bn_of(want);
+          const int bn = TF32_PBOX;
           if (kblk) {
             const int64_t kb = ldn32 / 32;
             TKM_TRY(make_tmap_f32(&targs.p_hi, dz_hi.as<float>(), kb * GB, 32, 32, bn));
@@ -1174,51 +1167,51 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
         }
         targs.N = targsF.N = std::max(nmax, 1);
       }
-      argsA2.N = argsA.N;
       // K-split of GEMM-B: only when its output tiles cannot fill the SMs and the contraction is long
-      int ksB = 1, ksT = 1;
+      int ksB = 1;
       if (ksplit_ok) {
-        const int64_t mt = ceil_div((int64_t)r, (int64_t)tileB.BM), mtT = ceil_div((int64_t)r, (int64_t)TF32_BM);
-        int64_t ctas = 0, ctasT = 0;
-        for (int g = 0; g < G; ++g) {
-          ctas += mt * ceil_div((int64_t)bound[g], (int64_t)tileB.BN);
-          if (delta) ctasT += mtT * ceil_div((int64_t)bound[g], (int64_t)tf32_bn_of(tcfg));
-        }
+        const int64_t mt = ceil_div((int64_t)r, (int64_t)tileB.BM);
+        int64_t ctas = 0;
+        for (int g = 0; g < G; ++g) ctas += mt * ceil_div((int64_t)bound[g], (int64_t)tileB.BN);
         const int64_t sm = 148;   // B200
-        // FP64 kernel: two resident CTAs per SM at least; tcgen05 kernel: one CTA per SM, so whole waves only
+        // FP64 kernel: two resident CTAs per SM at least
         if (ctas > 0 && 4 * ctas < 3 * sm) ksB = (int)std::min<int64_t>({(int64_t)KSPLIT_MAX, 2 * sm / ctas, (int64_t)n / 2048});
-        if (ctasT > 0 && 4 * ctasT < 3 * sm) ksT = (int)std::min<int64_t>({(int64_t)KSPLIT_MAX, sm / ctasT, (int64_t)n / 4096});
         ksB = std::max(ksB, 1);
-        ksT = std::max(ksT, 1);
       }
       argsB.ksplit = ksB;
-      targs.ksplit = ksT;
       // The delta forms pay while the batch is wide; the narrow tail is latency-bound either way and its slow
       // columns converge in fewer iterations on exact contractions, so it runs all-FP64 (the live set only
       // shrinks within a round, and every round starts with an exact iteration).
-      const bool dz_on = delta && ntot > DELTA_MIN_LIVE, df_on = delta_f && ntot > DELTA_MIN_LIVE;
-      for (int k = 0; k < check_every; ++k) {
+      const bool dz_on = delta && ntot > dmin, df_on = delta_f && ntot > dmin;
+      const int ce = (dz_on && ntot >= 4 * (int64_t)dmin) ? ce_max : check_every;   // iterations of this batch
+      ce_of[ring] = ce;
+      for (int k = 0; k < ce; ++k) {
         // FP64 GEMM-B: always without the delta form; with it, on the first iteration of a round (no zeta yet)
         // and on the last iteration of every batch, whose exact rho carries the stop test before the compaction
-        const bool exact_it = !dz_on || (batch == 0 && k == 0) || k == check_every - 1;
+        const bool exact_it = !dz_on || (batch == 0 && k == 0) || k == ce - 1;
         // sampled launches: right after a compaction every slot is live, so the counted flops are all useful; the
         // delta form has its FP64 GEMM-B on the last iteration of the batch instead
         // first iteration after a compaction (every slot live) and, in the delta forms, the exact last iteration
-        const int sidx = !opts->profile ? -1 : (opts->profile == 2 ? k : (k == 0 ? 0 : ((dz_on && k == check_every - 1) ? 1 : -1)));
+        const int sidx = !opts->profile ? -1 : (opts->profile == 2 ? k : (k == 0 ? 0 : ((dz_on && k == ce - 1) ? 1 : -1)));
         if (k == 0) std::fill(samp_kind.begin() + (size_t)ring * nsamp * 2, samp_kind.begin() + (size_t)(ring + 1) * nsamp * 2, -1);
         int* sk = samp_kind.data() + ((size_t)ring * nsamp + std::max(sidx, 0)) * 2;
         int famA = 0, famB = 0;
         if (sidx >= 0) TKM_CUDA(cudaEventRecord(pev(ring, sidx, 0), st));
         int nblkA = (int)ceil_div(n, tileA.BM);
         if (df_on && !exact_it) {
-          // F half: F+ = Fbar - U Lam da on the tcgen05 tensor cores, loss derivative in its epilogue
-          FLossEpi fe{(const double*)y, d_fold.as<int32_t>(), col_of_slot.as<int32_t>(), bbar.as<double>(),
-                      mu.as<double>(), p0->col_nc.as<double>(), p0->col_tau.as<double>(), p0->col_v.as<int32_t>(), B,
-                      (int)loss, smooth, smooth > 0.0 ? 1.0 / (2.0 * smooth) : 0.0, Fb.as<double>(), Fp.as<double>(),
-                      Zt.as<double>(), ldn, dz_hi.as<float>(),
-                      dz_lo.as<float>(), ldn32, gpart.as<double>(), ldpart, dz_blk_rows};
-          TKM_TRY(gemm_tf32_launch(targsF, tcfg, G, fe, st));
-          nblkA = (int)ceil_div(n, TF32_BM);
+          // F half: the product U Lam da on the tcgen05 tensor cores, then F+ = Fbar - U Lam da with the loss
+          // derivative as an elementwise pass over all (slot, sample)
+          ProdEpi pa{prodA.as<float>(), ldn32, B};
+          TKM_TRY(gemm_tf32_launch(targsF, G, tsc, pa, st));
+          if (sidx >= 0) TKM_CUDA(cudaEventRecord(pev(ring, sidx, 1), st));   // the contraction alone is the sampled span
+          FLossArgs fa{(const double*)y, d_fold.as<int32_t>(), nslots.as<int32_t>(), col_of_slot.as<int32_t>(),
+                       bbar.as<double>(), mu.as<double>(), p0->col_nc.as<double>(), p0->col_tau.as<double>(),
+                       p0->col_v.as<int32_t>(), B, (int)loss, (int)n, smooth, smooth > 0.0 ? 1.0 / (2.0 * smooth) : 0.0,
+                       prodA.as<float>(), ldn32, Fb.as<double>(), Fp.as<double>(), Zt.as<double>(), ldn,
+                       dz_hi.as<float>(), dz_lo.as<float>(), ldn32, gpart.as<double>(), ldpart, dz_blk_rows};
+          nblkA = (int)ceil_div(n, FLOSS_THREADS * FLOSS_EPT);
+          floss_kernel<<<dim3((unsigned)nblkA, (unsigned)std::max(nmax, 1), (unsigned)G), FLOSS_THREADS, 0, st>>>(fa);
+          TKM_LAUNCH_CHECK();
           famA = 2;
         } else {
           LossEpi le{(const double*)y, d_fold.as<int32_t>(), col_of_slot.as<int32_t>(), bbar.as<double>(),
@@ -1227,12 +1220,14 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
                      dz_on ? dz_lo.as<float>() : nullptr, ldn32, df_on ? Fb.as<double>() : nullptr, dz_blk_rows};
           TKM_TRY(gemm_f64_launch(argsA, tileA, G, le, st));
           if (df_on) {   // exact iteration of the F half: also F = U Lam a, so that both recurrence states are exact
-            StoreEpi fs{Fp.as<double>(), ldn, (int64_t)B * ldn, 1.0};   // (its time counts for family 0, its flops do not)
+            // (shifting the old F by the correction of Fbar instead was tried: the drift it leaves in F - F_prev is
+            // amplified by the momentum and tripled the iteration counts)
+            StoreEpi fs{Fp.as<double>(), ldn, (int64_t)B * ldn, 1.0};   // its time counts for family 0
             TKM_TRY(gemm_f64_launch(argsA2, tileA, G, fs, st));
           }
         }
         if (sidx >= 0) {
-          TKM_CUDA(cudaEventRecord(pev(ring, sidx, 1), st));
+          if (famA == 0) TKM_CUDA(cudaEventRecord(pev(ring, sidx, 1), st));
           sk[0] = famA + ((df_on && exact_it) ? 8 : 0);   // + 8: the timed span holds two FP64 GEMM-A launches
           TKM_CUDA(cudaEventRecord(pev(ring, sidx, 2), st));
         }
@@ -1251,17 +1246,10 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
           } else {
             TKM_TRY(gemm_f64_launch(argsB, tileB, G, se, st));
           }
-        } else if (ksT > 1) {
-          ZetaPartEpi pe{B, ksT, ldr, split_stride, zpart.as<double>()};
-          TKM_TRY(gemm_tf32_launch(targs, tcfg, G, pe, st));
-          spec_finalize_kernel<<<dim3((unsigned)ceil_div(r, 256), (unsigned)std::max(nmax, 1), (unsigned)G), 256, 0, st>>>(
-              zpart.as<double>(), ksT, split_stride, nslots.as<int32_t>(), col_of_slot.as<int32_t>(),
-              p0->col_lam.as<double>(), B, (int)r, ldr, Abar.as<double>(), Zeta.as<double>(), 1, Rho.as<double>());
-          TKM_LAUNCH_CHECK();
         } else {
-          ZetaEpi ze{col_of_slot.as<int32_t>(), p0->col_lam.as<double>(), B, Abar.as<double>(), ldr, Zeta.as<double>(),
-                     Rho.as<double>()};
-          TKM_TRY(gemm_tf32_launch(targs, tcfg, G, ze, st));
+          // delta form: the product U^T dz on the tcgen05 tensor cores; zeta += product and rho in update_kernel
+          ProdEpi pb{prodB.as<float>(), ldr32, B};
+          TKM_TRY(gemm_tf32_launch(targs, G, tsc, pb, st));
         }
         famB = exact_it ? 1 : 3;
         if (sidx >= 0) {
@@ -1276,6 +1264,7 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
                       kkt.as<double>(), done.as<int32_t>(), iters.as<int32_t>(), iters_round.as<int32_t>(),
                       flags.as<int32_t>(), df_on ? da_hi.as<float>() : nullptr, df_on ? da_lo.as<float>() : nullptr,
                       ldr32, df_on ? mu.as<double>() : nullptr,
+                      exact_it ? nullptr : prodB.as<float>(), ldr32, Zeta.as<double>(), Rho.as<double>(),
                       opts->profile == 2 ? fam_cnt.as<unsigned long long>() : nullptr, famA, famB};
         update_kernel<<<dim3(std::max(nmax, 1), G), 256, 0, st>>>(ua);
         TKM_LAUNCH_CHECK();
@@ -1297,7 +1286,7 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
       // Read back the polls of EARLIER batches while the GPU works on the ones just enqueued.  The host runs
       // one batch ahead while the live set is wide (fresh counts matter for the tile choice) and up to three
       // once it is narrow (batches of ~1 ms: slack against a descheduled host thread matters more).
-      const int lag = ntot > 256 ? 1 : POLL_RING - 2;
+      const int lag = ntot > 256 ? 2 : POLL_RING - 2;
       while (!finished && done_polls + lag <= batch) {
         const int64_t b = done_polls;
         const int cur = (int)(b % POLL_RING);
@@ -1335,7 +1324,8 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
         if (trace && b >= 1) {
           float bms = 0.f;
           cudaEventElapsedTime(&bms, ev.poll[(b - 1) % POLL_RING], ev.poll[cur]);
-          fprintf(trace, "%d %lld %d %d %d %d %.4f\n", rnd, (long long)b, live_then, max_then, tileA.cfg, tileB.cfg, bms);
+          fprintf(trace, "%d %lld %d %d %d %d %.4f %d\n", rnd, (long long)b, live_then, max_then, tileA.cfg, tileB.cfg, bms,
+                  ce_of[cur]);
         }
         ++done_polls;
         if (live == 0) finished = true;   // batches already enqueued beyond b find no live slot and do nothing

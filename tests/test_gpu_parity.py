@@ -300,8 +300,13 @@ def test_configs_2_3_reduced_n_against_an_oracle_fit(tkm, cfg, delta):
     L, V, T = w.L, w.V, w.T
     cols = None if cfg == 2 else [(t * (V + 1) + v) * L + l for t in range(T) for v in range(V + 1)
                                   for l in range(0, L, 5)]
-    X, y, spec, path, cv = _run_gpu(tkm, w, sigma, foldid, STOP_TOL, 400000, warm_tol=1e-3, tf32_delta=delta)
-    res, spec_o, worst, degenerate = _compare_path(tkm, w, sigma, foldid, spec, path, cv, columns=cols, warm_tol=1e-3)
+    # The stop tolerance is an input of both sides (reading G6).  On the check-loss columns the oracle's own tol = 1e-12
+    # iterate is 5e-11 .. 8e-11 (relative l2) away from its tol = 1e-14 iterate (condition ~ 70), so two sides that
+    # both stop at 1e-12 can be 1.5e-10 apart; at 3e-13 each is within 2e-11 of the minimiser.
+    stop = 3e-13 if cfg == 3 else STOP_TOL
+    X, y, spec, path, cv = _run_gpu(tkm, w, sigma, foldid, stop, 400000, warm_tol=1e-3, tf32_delta=delta)
+    res, spec_o, worst, degenerate = _compare_path(tkm, w, sigma, foldid, spec, path, cv, columns=cols, warm_tol=1e-3,
+                                                   stop_tol=stop)
     print("cfg %d at n = 1500, tf32_delta %d: worst relative l2 coefficient error %.3g" % (cfg, delta, worst))
     cv_loss, cv_err, cv_mean, best = cv
     if cols is None:
@@ -562,7 +567,7 @@ def test_train_tune_host_matches_oracle(tkm):
 
 # ------------------------------------------------------------------------------- tcgen05 3xTF32 contraction
 @pytest.mark.parametrize("N,M,K,cfg", [(64, 128, 32, 0), (37, 130, 70, 0), (128, 256, 512, 1), (300, 2000, 2000, -1),
-                                       (100, 333, 1001, 2)])
+                                       (100, 333, 1001, 2), (700, 520, 256, -1), (513, 128, 64, -1), (5, 1000, 96, -1)])
 def test_tf32x3_gemm_nt(tkm, N, M, K, cfg):
     """The tcgen05 (TMEM accumulator) 3xTF32 product against FP64: the error is that of FP32 accumulation in the
     tensor core, which truncates -- it grows like K 2^-24 relative to the size of the partial sums."""
