@@ -20,6 +20,7 @@ Other workloads (`--workload`, one GPU, one JSON line each with the same keys):
   nystrom_covtype | nystrom_mnist8m46   Nystrom at the row counts of the paper's Table 4
   loo_config1                      leave-one-out form of Algorithm 1 (V = n) on configs[1]'s data (8(f) N2)
   narrow_config2 | narrow_config3  configs[2]/[3] with `--narrow-L` in {1,2,4} lambdas: the HBM-bound narrow batch
+  gemm_probe                       the two contraction kernels alone on a list of shapes (calibration / evidence)
 
 N > 1 (torchrun): the path has no exchange step -- every rank runs the same-size workload on its own seeded
 data set (independent problems, "weak" scaling); the only communication is the barrier and the max-over-ranks
@@ -59,7 +60,7 @@ WARM_TOL = 1e-3
 # increments on the tcgen05 tensor cores, with exact FP64 DMMA contractions and the stop test on the last iteration
 # of every 16-iteration batch and in the narrow tail.  Same fixed point and the same 1e-10 parity bar as the
 # all-FP64 sweep.  This is how the "fp32" configurations of BASELINE.json run: FP64 state + 3xTF32 increments.
-TF32_DELTA = 1           # default line (configs[1])
+TF32_DELTA = 2           # default line (configs[1])
 TF32_DELTA_LARGE = 2     # configs[2..4], Nystrom, leave-one-out
 # nominal dense tensor ratios to bf16 (B200_PROFILING.md / B300_MICROARCH.md tables): FP64 45 TF,
 # TF32 1125 TF, bf16 2250 TF.  3xTF32 does three MMAs per useful one.
@@ -437,6 +438,37 @@ def narrow_hbm_roofline(res, pk):
     return out
 
 
+GEMM_PROBE_SHAPES = [(64, 256, 2000), (64, 2000, 2000), (128, 2000, 2000), (300, 2000, 2000), (64, 18944, 2000),
+                     (300, 10000, 10000), (512, 10000, 10000), (1100, 10000, 10000), (300, 20000, 20000),
+                     (900, 20000, 20000), (600, 100000, 4096), (600, 4096, 100000)]
+
+
+def run_gemm_probe(args):
+    """`--workload gemm_probe`: the two contraction kernels alone, Dt[N][M] = P[N][K] Q[M][K]^T on random operands
+    (N slots, M rows of U, K contraction depth), `--probe-iters` back-to-back launches timed with CUDA events:
+    the tcgen05 3xTF32 pair kernel (tkm_tf32x3_gemm_nt) and the FP64 DMMA kernel (tkm_gemm_probe)."""
+    import torch
+    import paper_2606_06742_b200 as tkm
+    tkm.lib()
+    torch.cuda.set_device(0)
+    pk = peaks()
+    rows = []
+    for (N, M, K) in GEMM_PROBE_SHAPES:
+        P = torch.randn((N, K), device="cuda", dtype=torch.float64)
+        Q = torch.randn((M, K), device="cuda", dtype=torch.float64)
+        _, ms = tkm.tkm_tf32x3_gemm_nt(P, Q, iters=args.probe_iters)
+        del P, Q
+        torch.cuda.empty_cache()
+        ms64 = tkm.tkm_gemm_probe(-1, 1, N, M, K, iters=max(2, args.probe_iters // 4)) if N * M * K <= 4e11 else None
+        fl = 2.0 * N * M * K
+        rows.append({"N": N, "M": M, "K": K, "tcgen05_3xtf32_us": 1e3 * ms, "tcgen05_useful_tflops": fl / ms / 1e9,
+                     "tcgen05_frac_of_contract_peak": fl / ms / 1e9 / (pk["bf16_sus"] * NOMINAL_RATIO["f32"]),
+                     "dmma_f64_us": None if ms64 is None else 1e3 * ms64,
+                     "dmma_tflops": None if ms64 is None else fl / ms64 / 1e9})
+    print(json.dumps({"workload": "gemm_probe", "iters": args.probe_iters, "peaks": pk,
+                      "tf32x3_contract_peak_tflops": pk["bf16_sus"] * NOMINAL_RATIO["f32"], "shapes": rows}))
+
+
 def run_single(args):
     """`--workload` other than config1: one GPU, one problem, one JSON line."""
     import torch
@@ -693,7 +725,7 @@ def main():
     ap.add_argument("--dtype", default="f64", choices=["f64"])
     ap.add_argument("--workload", default="config1",
                     choices=["config1", "config2", "config3", "config4", "nystrom_covtype", "nystrom_mnist8m46",
-                             "loo_config1", "narrow_config2", "narrow_config3"],
+                             "loo_config1", "narrow_config2", "narrow_config3", "gemm_probe"],
                     help="config1 = BASELINE.json's metric configuration (the bench line, which also carries configs[3] "
                          "as `large_config`); the others are single-GPU measurements of one problem "
                          "(use --steps 1 --warmup 0 or 1: a pass takes seconds to a minute)")
@@ -703,6 +735,7 @@ def main():
                     help="outer control of PAPER.md:220-222 (reading G23) for a --workload run; 0 = fixed schedule")
     ap.add_argument("--narrow-L", type=int, default=1, choices=[1, 2, 4])
     ap.add_argument("--loo-lambdas", type=int, default=0, help="loo_config1: use this many lambdas of the grid (0 = all 50)")
+    ap.add_argument("--probe-iters", type=int, default=20, help="gemm_probe: launches per shape")
     ap.add_argument("--profile-all", action="store_true", help="time every contraction launch (profile = 2)")
     ap.add_argument("--no-large", action="store_true", help="default line: skip the configs[3] pass (`large_config`)")
     args = ap.parse_args()
@@ -711,7 +744,7 @@ def main():
     if args.workload != "config1":
         if args.impl != "ours" or world != 1 or args.gpus != 1:
             raise SystemExit("--workload %s: one GPU, --impl ours only" % args.workload)
-        return run_single(args)
+        return run_gemm_probe(args) if args.workload == "gemm_probe" else run_single(args)
     if args.tf32_delta >= 0:
         global TF32_DELTA
         TF32_DELTA = args.tf32_delta

@@ -6,7 +6,9 @@
  * Conventions
  *   - extern "C"; every call returns a tkm_status (0 = TKM_OK).  tkm_last_error() returns a
  *     thread-local, NUL-terminated description of the last failure on the calling thread.
- *     No exception crosses the boundary; there is no global mutable state besides that string.
+ *     No exception crosses the boundary.  Process-wide state: that string and the launch counter (thread-local),
+ *     one library-owned stream-ordered memory pool per device for the sweep's temporaries (created on first
+ *     use, never the device's default pool), and per-device "kernel attributes set" bits.
  *   - [dev]  = pointer to DEVICE memory owned by the caller (e.g. a torch tensor's data_ptr()).
  *     [host] = pointer to HOST memory owned by the caller.  Nothing passed in is retained after
  *     the call returns except where stated (tkm_path keeps a pointer to its tkm_spectral).
@@ -43,7 +45,8 @@ typedef enum {
   TKM_ENOTIMPL = 6
 } tkm_status;
 
-typedef enum { TKM_F32 = 0, TKM_F64 = 1 } tkm_dtype;
+typedef enum { TKM_F32 = 0, TKM_F64 = 1 } tkm_dtype;   /* element type of an OUTPUT array (tkm_gram); all inputs and  */
+                                                        /* the whole sweep are FP64                                    */
 
 typedef enum {
   TKM_LOSS_HINGE = 0,    /* delta-smoothed hinge */
@@ -119,15 +122,16 @@ int tkm_gram_multi(const void* X, int64_t n, int64_t p, int64_t ldx,
 /* ---- S2  one-time spectral setup (Alg.1 l.3, 226; readings G11, G16, G19) --------
  * Full kernel (ny == NULL): K [dev] n x n FP64 symmetric (not modified); decomposes in FP64 with
  * cuSOLVER syevd, clamps Lam >= 0, forms u1 = U^T 1, and keeps U Lam (n x r) and U^T (r x n) in
- * FP64 for the two contractions of the sweep (FP64 DMMA path).  sweep_dt must be TKM_F64: an all-FP32 /
- * 3xTF32 sweep cannot meet the stop test on ill-conditioned columns and returns TKM_ENOTIMPL (DESIGN.md
- * section 12); the 3xTF32 tensor-core path exists as the delta form selected by tkm_loss_opts.tf32_delta.
- * r = n.
+ * FP64 for the two contractions of the sweep.  PRECISION, stated once: the sweep's state, stop test and results
+ * are always FP64.  There is no all-FP32 sweep (FP32-accumulated contractions cannot meet the stop test on
+ * ill-conditioned columns); the configurations BASELINE.json labels "fp32" run as FP64
+ * state + 3xTF32 increments on the tcgen05 tensor cores (tkm_loss_opts.tf32_delta), which meets the FP64
+ * parity bar.  r = n.
  * Nystrom (ny != NULL): K is ignored (may be NULL); thin U (n x r, r <= m) from K_nm, K_mm.
  * The handle is shared by every lambda, fold and quantile level.  Synchronises `stream`.
  * Errors: TKM_ESOLVER if cuSOLVER reports info != 0; TKM_ENOMEM. */
 int tkm_spectral_setup(const void* K, int64_t n, int64_t ldk, const tkm_nystrom* ny,
-                       tkm_dtype sweep_dt, tkm_spectral** out, void* stream);
+                       tkm_spectral** out, void* stream);
 /* Nystrom setup straight from the training matrix (n ~ 10^6 rows):
  * X [dev] n x p FP64 (ldx >= p), RBF bandwidth sigma, landmark_idx [host] m row indices into X.  The
  * landmark rows are gathered, K_mm is formed, and K_nm is produced by the Gram kernel and consumed
@@ -141,7 +145,7 @@ int tkm_spectral_setup_nystrom_x(const void* X, int64_t n, int64_t p, int64_t ld
  * G internal streams ordered after `stream`; out [host] G slots.  Same results as G separate calls.
  * Returns after all G decompositions have finished. */
 int tkm_spectral_setup_multi(const void* const* Ks, int32_t G, int64_t n, int64_t ldk,
-                             tkm_dtype sweep_dt, tkm_spectral** out, void* stream);
+                             tkm_spectral** out, void* stream);
 void tkm_spectral_free(tkm_spectral* s);
 /* n, r, and [host] copies of Lam (r) and u1 (r); either output pointer may be NULL. */
 int tkm_spectral_info(const tkm_spectral* s, int64_t* n, int64_t* r, double* lam, double* u1);
@@ -168,8 +172,9 @@ int tkm_fit_path(const tkm_spectral* s, const void* y, tkm_loss loss, const tkm_
 /* The same sweep for G <= 8 independent problems that share y, the folds, the loss and the lambda
  * grid -- e.g. the bandwidths of a sigma grid, one spectral handle each (all with the same n, r and
  * sweep precision).  Every iteration is ONE launch per kernel over all groups' live columns, which
- * keeps the device full when each group's batch has become narrow.  Results are identical to G
- * separate tkm_fit_path calls.  specs [host] G handles; warm [host] G paths or NULL; out [host] G
+ * keeps the device full when each group's batch has become narrow.  Every column reaches the same
+ * minimiser as in G separate tkm_fit_path calls to the stop tolerance (tile shapes, hence summation
+ * orders, depend on the totals over the groups).  specs [host] G handles; warm [host] G paths or NULL; out [host] G
  * slots, out[g] belongs to specs[g].  The sampled timings of tkm_path_profile are those of the shared
  * launches and are reported on out[0] only. */
 int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, const void* y, tkm_loss loss,
@@ -183,6 +188,8 @@ void tkm_path_free(tkm_path* p);
  * beta0[B]; total_col_iters = sum of iters (the unit of the roofline). */
 int tkm_path_info(const tkm_path* p, int32_t* B, int64_t* r, int32_t* iters, double* kkt,
                   int32_t* flags, double* beta0, int64_t* total_col_iters);
+/* T, L, V of the grid and n of its spectral handle; any pointer may be NULL. */
+int tkm_path_shape(const tkm_path* p, int32_t* T, int32_t* L, int32_t* V, int64_t* n);
 /* Smoothing level every column ended on (reading G23): level[B] in [0, rounds), rounds - 1 under the fixed schedule,
  * and smooth[B] = smooth0 eta^level (0 for the smooth losses); both [host], either may be NULL. */
 int tkm_path_levels(const tkm_path* p, int32_t* level, double* smooth);
@@ -225,6 +232,10 @@ int tkm_path_duality_gap(const tkm_path* p, const void* y, const int32_t* foldid
 int tkm_cv_select(const double* cv_loss, const double* fold_sizes, const double* lambdas, int32_t T,
                   int32_t L, int32_t V, double* cv_mean, int32_t* best_l, void* stream);
 
+/* Fold sizes of a fold assignment: sizes [host] V doubles (the weights tkm_cv_select expects).  Integer-only,
+ * host; TKM_EINVAL if a label is outside [0, V). */
+int tkm_fold_sizes(const int32_t* foldid, int64_t n, int32_t V, double* sizes);
+
 /* ---- S10 coefficients and prediction (readings G11, G15) --------------------
  * tkm_path_coef: alpha = U a of column (t, l, v) into [dev] alpha (n FP64; Nystrom: the m landmark
  * weights gamma), and beta0 into [host] *beta0.  Synchronises `stream`. */
@@ -263,7 +274,7 @@ int tkm_platt_proba(const double* f, int64_t n, double A, double B, double* p_ou
 int tkm_train_tune_host(const double* X, int64_t n, int64_t p, const double* y, const double* sigmas,
                         int32_t G, tkm_loss loss, const tkm_loss_opts* opts, const double* lambdas,
                         int32_t L, const int32_t* foldid, int32_t V, double tol, int32_t maxit,
-                        tkm_dtype sweep_dt, double* cv_loss, int64_t* cv_err, double* cv_mean,
+                        double* cv_loss, int64_t* cv_err, double* cv_mean,
                         int32_t* best_l, double* alpha_best, double* beta0_best, float* stage_ms,
                         void* stream);
 

@@ -13,7 +13,7 @@ TKM_OK, TKM_ENOTCONV = 0, 5
 
 EXPORTED_SYMBOLS = [
     "tkm_gram", "tkm_gram_multi", "tkm_spectral_setup", "tkm_spectral_setup_multi", "tkm_spectral_setup_nystrom_x", "tkm_spectral_free", "tkm_spectral_info", "tkm_spectral_get_u",
-    "tkm_fit_path", "tkm_fit_path_multi", "tkm_path_free", "tkm_path_info", "tkm_path_levels", "tkm_path_profile", "tkm_path_get_a", "tkm_exact_cv", "tkm_cv_select", "tkm_path_duality_gap", "tkm_path_coef",
+    "tkm_fit_path", "tkm_fit_path_multi", "tkm_path_free", "tkm_path_info", "tkm_path_shape", "tkm_path_levels", "tkm_fold_sizes", "tkm_path_profile", "tkm_path_get_a", "tkm_exact_cv", "tkm_cv_select", "tkm_path_duality_gap", "tkm_path_coef",
     "tkm_predict", "tkm_cv_decision_values", "tkm_platt_fit", "tkm_platt_proba", "tkm_train_tune_host", "tkm_make_folds", "tkm_launch_count", "tkm_launch_count_reset",
     "tkm_dgemm_nt", "tkm_gemm_probe", "tkm_tf32x3_gemm_nt", "tkm_version", "tkm_last_error",
 ]
@@ -57,8 +57,8 @@ def lib():
     vp, i64, i32, dbl = C.c_void_p, C.c_int64, C.c_int32, C.c_double
     L.tkm_gram.argtypes = [vp, i64, i64, i64, vp, i64, i64, dbl, C.c_int, vp, i64, vp]
     L.tkm_gram_multi.argtypes = [vp, i64, i64, i64, vp, i64, i64, vp, i32, C.c_int, C.POINTER(vp), i64, vp]
-    L.tkm_spectral_setup.argtypes = [vp, i64, i64, C.POINTER(_Nystrom), C.c_int, C.POINTER(vp), vp]
-    L.tkm_spectral_setup_multi.argtypes = [C.POINTER(vp), i32, i64, i64, C.c_int, C.POINTER(vp), vp]
+    L.tkm_spectral_setup.argtypes = [vp, i64, i64, C.POINTER(_Nystrom), C.POINTER(vp), vp]
+    L.tkm_spectral_setup_multi.argtypes = [C.POINTER(vp), i32, i64, i64, C.POINTER(vp), vp]
     L.tkm_spectral_setup_nystrom_x.argtypes = [vp, i64, i64, i64, dbl, vp, i64, i64, C.POINTER(vp), vp]
     L.tkm_spectral_free.argtypes = [vp]
     L.tkm_spectral_free.restype = None
@@ -83,7 +83,9 @@ def lib():
     L.tkm_platt_fit.argtypes = [vp, vp, i64, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(i32), vp]
     L.tkm_platt_proba.argtypes = [vp, i64, dbl, dbl, vp, vp]
     L.tkm_train_tune_host.argtypes = [vp, i64, i64, vp, vp, i32, C.c_int, C.POINTER(_LossOpts), vp, i32, vp, i32,
-                                      dbl, i32, C.c_int, vp, vp, vp, vp, vp, vp, vp, vp]
+                                      dbl, i32, vp, vp, vp, vp, vp, vp, vp, vp]
+    L.tkm_path_shape.argtypes = [vp, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32), C.POINTER(i64)]
+    L.tkm_fold_sizes.argtypes = [vp, i64, i32, vp]
     L.tkm_make_folds.argtypes = [i64, i32, C.c_uint64, vp]
     L.tkm_launch_count.restype = i64
     L.tkm_launch_count_reset.restype = None
@@ -118,6 +120,23 @@ def _dev_f64(t, name):
 
 def _host(a, dtype):
     return np.ascontiguousarray(a, dtype=dtype)
+
+
+def _dev_vec(t, n, name):
+    """A contiguous CUDA float64 vector of length n."""
+    t = _dev_f64(t, name)
+    if t.dim() != 1 or t.numel() != n or (n > 1 and t.stride(0) != 1):
+        raise ValueError("%s must be a contiguous vector of length %d" % (name, n))
+    return t
+
+
+def _fold_vec(foldid, n, V):
+    fid = _host(foldid, np.int32)
+    if fid.shape != (n,):
+        raise ValueError("foldid must have length n = %d" % n)
+    if n and (fid.min() < 0 or fid.max() >= V):
+        raise ValueError("foldid values must lie in [0, V)")
+    return fid
 
 
 def _ptr(a):
@@ -217,20 +236,20 @@ class Spectral:
             pass
 
 
-def tkm_spectral_setup(K=None, n=None, nystrom=None, sweep_dtype=F64, stream=None) -> Spectral:
+def tkm_spectral_setup(K=None, n=None, nystrom=None, stream=None) -> Spectral:
     """Full kernel: K (n x n CUDA float64).  Nystrom: nystrom=(K_nm, K_mm, landmark_idx), n = rows."""
     h = C.c_void_p()
     if nystrom is None:
         K = _dev_f64(K, "K")
         n = K.shape[0]
-        _check(lib().tkm_spectral_setup(K.data_ptr(), n, K.stride(0), None, sweep_dtype, C.byref(h), _stream(stream)))
+        _check(lib().tkm_spectral_setup(K.data_ptr(), n, K.stride(0), None, C.byref(h), _stream(stream)))
         return Spectral(h)
     K_nm, K_mm, idx = nystrom
     K_nm, K_mm = _dev_f64(K_nm, "K_nm"), _dev_f64(K_mm, "K_mm")
     idx = _host(idx, np.int64)
     ny = _Nystrom(K_nm.data_ptr(), K_nm.stride(0), K_mm.data_ptr(), K_mm.stride(0), K_mm.shape[0],
                   idx.ctypes.data_as(C.POINTER(C.c_int64)))
-    _check(lib().tkm_spectral_setup(None, K_nm.shape[0], 0, C.byref(ny), sweep_dtype, C.byref(h), _stream(stream)))
+    _check(lib().tkm_spectral_setup(None, K_nm.shape[0], 0, C.byref(ny), C.byref(h), _stream(stream)))
     return Spectral(h)
 
 
@@ -244,7 +263,7 @@ def tkm_spectral_setup_nystrom_x(X, sigma: float, landmark_idx, block_rows: int 
     return Spectral(h, keepalive=(idx,))
 
 
-def tkm_spectral_setup_multi(Ks, sweep_dtype=F64, stream=None):
+def tkm_spectral_setup_multi(Ks, stream=None):
     """Concurrent full-kernel setups of G Gram matrices of one size -> list of G Spectral handles."""
     Ks = [_dev_f64(K, "K") for K in Ks]
     G, n, ld = len(Ks), Ks[0].shape[0], Ks[0].stride(0)
@@ -252,7 +271,7 @@ def tkm_spectral_setup_multi(Ks, sweep_dtype=F64, stream=None):
         raise ValueError("all K must be n x n with the same row stride")
     hk = (C.c_void_p * G)(*[K.data_ptr() for K in Ks])
     ho = (C.c_void_p * G)()
-    _check(lib().tkm_spectral_setup_multi(hk, G, n, ld, sweep_dtype, ho, _stream(stream)))
+    _check(lib().tkm_spectral_setup_multi(hk, G, n, ld, ho, _stream(stream)))
     return [Spectral(C.c_void_p(ho[g])) for g in range(G)]
 
 
@@ -266,6 +285,9 @@ class Path:
         B, r, tot = C.c_int32(), C.c_int64(), C.c_int64()
         _check(lib().tkm_path_info(self._h, C.byref(B), C.byref(r), None, None, None, None, C.byref(tot)))
         self.B, self.r, self.total_col_iters = B.value, r.value, tot.value
+        T, L, V, n = C.c_int32(), C.c_int32(), C.c_int32(), C.c_int64()
+        _check(lib().tkm_path_shape(self._h, C.byref(T), C.byref(L), C.byref(V), C.byref(n)))
+        self.T, self.L, self.V, self.n = T.value, L.value, V.value, n.value
 
     def info(self):
         iters = np.empty(self.B, dtype=np.int32)
@@ -317,9 +339,9 @@ def _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, prof
 def tkm_fit_path(spec: Spectral, y, loss: int, lambdas, foldid, V: int, tol: float, maxit: int,
                  smooth0=1.0, eta=0.125, rounds=4, taus=None, restart=True, check_every=0, warm_tol=0.0,
                  warm: Path | None = None, profile=False, tf32_delta=0, gap_tol=0.0, stream=None) -> Path:
-    y = _dev_f64(y, "y")
+    y = _dev_vec(y, spec.n, "y")
     lam = _host(lambdas, np.float64)
-    fid = _host(foldid, np.int32)
+    fid = _fold_vec(foldid, spec.n, V)
     o, keep = _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, profile, tf32_delta, gap_tol)
     h = C.c_void_p()
     rc = lib().tkm_fit_path(spec._h, y.data_ptr(), loss, C.byref(o), _ptr(lam), len(lam), _ptr(fid), V,
@@ -333,9 +355,9 @@ def tkm_fit_path_multi(specs, y, loss: int, lambdas, foldid, V: int, tol: float,
                        smooth0=1.0, eta=0.125, rounds=4, taus=None, restart=True, check_every=0, warm_tol=0.0,
                        warm=None, profile=False, tf32_delta=0, gap_tol=0.0, stream=None):
     """One sweep over G spectral handles that share y, folds and the lambda grid -> list of G Paths."""
-    y = _dev_f64(y, "y")
+    y = _dev_vec(y, specs[0].n, "y")
     lam = _host(lambdas, np.float64)
-    fid = _host(foldid, np.int32)
+    fid = _fold_vec(foldid, specs[0].n, V)
     o, keep = _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, profile, tf32_delta, gap_tol)
     G = len(specs)
     hs = (C.c_void_p * G)(*[s._h for s in specs])
@@ -347,9 +369,14 @@ def tkm_fit_path_multi(specs, y, loss: int, lambdas, foldid, V: int, tol: float,
     return [Path(C.c_void_p(ho[g]), specs[g], rc) for g in range(G)]
 
 
-def tkm_exact_cv(path: Path, y, foldid, T: int, L: int, V: int, stream=None):
-    y = _dev_f64(y, "y")
-    fid = _host(foldid, np.int32)
+def tkm_exact_cv(path: Path, y, foldid, T: int = None, L: int = None, V: int = None, stream=None):
+    """The output tables are sized from the path itself; T, L, V, if given, must agree with it."""
+    for name, got, want in (("T", T, path.T), ("L", L, path.L), ("V", V, path.V)):
+        if got is not None and got != want:
+            raise ValueError("tkm_exact_cv: %s = %d but the path was fitted with %s = %d" % (name, got, name, want))
+    T, L, V = path.T, path.L, path.V
+    y = _dev_vec(y, path.n, "y")
+    fid = _fold_vec(foldid, path.n, V)
     cv_loss = np.empty((T, L, V))
     cv_err = np.empty((T, L, V), dtype=np.int64)
     cv_mean = np.empty((T, L))
@@ -362,8 +389,8 @@ def tkm_exact_cv(path: Path, y, foldid, T: int, L: int, V: int, stream=None):
 def tkm_path_duality_gap(path: Path, y, foldid, stream=None):
     """(primal, gap) per column of a hinge / quantile path: objective of the non-smoothed problem and its
     duality-gap certificate (reading G22)."""
-    y = _dev_f64(y, "y")
-    fid = _host(foldid, np.int32)
+    y = _dev_vec(y, path.n, "y")
+    fid = _fold_vec(foldid, path.n, path.V)
     primal, gap = np.empty(path.B), np.empty(path.B)
     _check(lib().tkm_path_duality_gap(path._h, y.data_ptr(), _ptr(fid), _ptr(primal), _ptr(gap), _stream(stream)))
     return primal, gap
@@ -402,7 +429,9 @@ def tkm_fit_cv_sharded(spec: Spectral, y, loss: int, lambdas, foldid, V: int, to
     loc_loss, loc_err, _, _ = tkm_exact_cv(path, y, foldid, T, len(mine), V, stream=stream)
     cv_loss = ranks.gather_lambda_tables(loc_loss, len(lam), rank, world, dist)
     cv_err = ranks.gather_lambda_tables(loc_err, len(lam), rank, world, dist)
-    fsize = np.bincount(_host(foldid, np.int32), minlength=V).astype(np.float64)
+    fid = _host(foldid, np.int32)
+    fsize = np.empty(V)
+    _check(lib().tkm_fold_sizes(_ptr(fid), len(fid), V, _ptr(fsize)))
     cv_mean, best = tkm_cv_select(cv_loss, fsize, lam, stream=stream)
     return path, mine, cv_loss, cv_err, cv_mean, best
 
@@ -429,7 +458,7 @@ def tkm_predict(path: Path, t: int, l: int, X_train, X_new, sigma: float, labels
 
 
 def tkm_train_tune_host(X, y, sigmas, loss, lambdas, foldid, V, tol, maxit, smooth0=1.0, eta=0.125, rounds=4,
-                        taus=None, restart=True, check_every=0, warm_tol=0.0, sweep_dtype=F64,
+                        taus=None, restart=True, check_every=0, warm_tol=0.0,
                         want_alpha=True, tf32_delta=False, stream=None):
     """Whole pipeline from HOST numpy buffers for G bandwidths at once (the `e2e` call of bench.py)."""
     X = _host(X, np.float64)
@@ -449,7 +478,7 @@ def tkm_train_tune_host(X, y, sigmas, loss, lambdas, foldid, V, tol, maxit, smoo
     b0 = np.zeros(G)
     stage = np.zeros(5, dtype=np.float32)
     rc = lib().tkm_train_tune_host(_ptr(X), n, p, _ptr(y), _ptr(sig), G, loss, C.byref(o), _ptr(lam), L, _ptr(fid),
-                                   V, float(tol), int(maxit), sweep_dtype, _ptr(cv_loss), _ptr(cv_err),
+                                   V, float(tol), int(maxit), _ptr(cv_loss), _ptr(cv_err),
                                    _ptr(cv_mean), _ptr(best), _ptr(alpha) if want_alpha else None, _ptr(b0),
                                    _ptr(stage), _stream(stream))
     _check(rc, allow_notconv=True)
@@ -494,7 +523,7 @@ def tkm_tf32x3_gemm_nt(P, Q, cfg=-1, iters=0, stream=None):
 def tkm_cv_decision_values(path: Path, t: int, l: int, foldid, stream=None):
     """Held-out decision value of every training row at (t, lambda_l) from the exact-CV columns."""
     import torch
-    fid = _host(foldid, np.int32)
+    fid = _fold_vec(foldid, path.n, path.V)
     f = torch.empty(path.spec.n, device="cuda", dtype=torch.float64)
     _check(lib().tkm_cv_decision_values(path._h, t, l, _ptr(fid), f.data_ptr(), _stream(stream)))
     return f

@@ -63,7 +63,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         raise RuntimeError("libtkm build failed")
     if force or procs or _newer(objs, LIB):
         cmd = [nvcc, "-shared", "-o", LIB] + objs + ["-gencode", "arch=compute_100a,code=sm_100a",
-                                                    "-L/usr/local/cuda/lib64", "-lcusolver", "-lcudart"]
+                                                    "-L/usr/local/cuda/lib64", "-lcusolver", "-lcudart", "-ldl"]
         r = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
         if r.returncode != 0:
             raise RuntimeError("link failed:\n" + r.stdout)

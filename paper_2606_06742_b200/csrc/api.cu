@@ -25,6 +25,33 @@ int64_t& launch_counter() {
   return c;
 }
 
+cudaMemPool_t lib_pool() {
+  static std::mutex mu;
+  static cudaMemPool_t pools[64] = {};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) {
+    cudaGetLastError();
+    return nullptr;
+  }
+  std::lock_guard<std::mutex> lock(mu);
+  if (!pools[dev]) {
+    cudaMemPoolProps props = {};
+    props.allocType = cudaMemAllocationTypePinned;
+    props.handleTypes = cudaMemHandleTypeNone;
+    props.location.type = cudaMemLocationTypeDevice;
+    props.location.id = dev;
+    cudaMemPool_t mp = nullptr;
+    if (cudaMemPoolCreate(&mp, &props) != cudaSuccess) {
+      cudaGetLastError();
+      return nullptr;
+    }
+    uint64_t keep = 8ull << 30;
+    cudaMemPoolSetAttribute(mp, cudaMemPoolAttrReleaseThreshold, &keep);
+    pools[dev] = mp;
+  }
+  return pools[dev];
+}
+
 int device_check() {
   int dev = -1;
   cudaError_t e = cudaGetDevice(&dev);
@@ -72,10 +99,21 @@ extern "C" int tkm_make_folds(int64_t n, int32_t V, uint64_t seed, int32_t* fold
   return TKM_OK;
 }
 
+// fold sizes of a fold assignment (integer-only host helper; the weights of tkm_cv_select)
+extern "C" int tkm_fold_sizes(const int32_t* foldid, int64_t n, int32_t V, double* sizes) {
+  if (!foldid || !sizes || n < 1 || V < 1) return set_error(TKM_EINVAL, "tkm_fold_sizes: bad arguments");
+  for (int v = 0; v < V; ++v) sizes[v] = 0.0;
+  for (int64_t j = 0; j < n; ++j) {
+    if (foldid[j] < 0 || foldid[j] >= V) return set_error(TKM_EINVAL, "tkm_fold_sizes: foldid[%lld] out of range", (long long)j);
+    sizes[foldid[j]] += 1.0;
+  }
+  return TKM_OK;
+}
+
 extern "C" int tkm_train_tune_host(const double* X, int64_t n, int64_t p, const double* y, const double* sigmas,
                                    int32_t G, tkm_loss loss, const tkm_loss_opts* opts, const double* lambdas,
                                    int32_t L, const int32_t* foldid, int32_t V, double tol, int32_t maxit,
-                                   tkm_dtype sweep_dt, double* cv_loss, int64_t* cv_err, double* cv_mean,
+                                   double* cv_loss, int64_t* cv_err, double* cv_mean,
                                    int32_t* best_l, double* alpha_best, double* beta0_best, float* stage_ms,
                                    void* stream) {
   if (!X || !y || !sigmas || !opts || !lambdas || !foldid || !cv_loss || !cv_mean || !best_l)
@@ -109,7 +147,7 @@ extern "C" int tkm_train_tune_host(const double* X, int64_t n, int64_t p, const 
   for (int g = 0; g < G; ++g) Ks[g] = Kw[g] = dK.as<double>() + (size_t)g * n * n;
   TKM_TRY(tkm_gram_multi(dX.p, n, p, p, nullptr, 0, 0, sigmas, G, TKM_F64, Kw, n, st));
   TKM_CUDA(cudaEventRecord(ev[2], st));
-  TKM_TRY(tkm_spectral_setup_multi(Ks, G, n, n, sweep_dt, own.spec, st));   // the G decompositions overlap
+  TKM_TRY(tkm_spectral_setup_multi(Ks, G, n, n, own.spec, st));   // the G decompositions overlap
   dK.release();
   TKM_CUDA(cudaEventRecord(ev[3], st));
   int rc = tkm_fit_path_multi(own.spec, G, dy.p, loss, opts, lambdas, L, foldid, V, tol, maxit, nullptr, own.path, st);

@@ -2,10 +2,12 @@
 #pragma once
 
 #include <cuda_runtime.h>
+#include <nvtx3/nvToolsExt.h>
 #include <cstdarg>
 #include <cstdint>
 #include <cstdio>
 #include <cstring>
+#include <atomic>
 #include <mutex>
 #include <vector>
 
@@ -43,23 +45,21 @@ inline void count_launch(int64_t k = 1) { launch_counter() += k; }
     if (_s != TKM_OK) return _s;      \
   } while (0)
 
+// NVTX range of one pipeline stage (visible to nsys / ncu --nvtx; a no-op without a tool attached)
+struct NvtxRange {
+  explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+  ~NvtxRange() { nvtxRangePop(); }
+  NvtxRange(const NvtxRange&) = delete;
+  NvtxRange& operator=(const NvtxRange&) = delete;
+};
+
 inline int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
 inline int64_t ceil_div(int64_t x, int64_t m) { return (x + m - 1) / m; }
 
-// Keep up to 8 GiB of freed stream-ordered allocations in the device's default pool, so that the temporaries of
-// one sweep are handed to the next without a trip through the driver's page tables.
-inline void pool_keep_once() {
-  static std::once_flag once;
-  std::call_once(once, [] {
-    int dev = 0;
-    cudaMemPool_t pool;
-    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
-      uint64_t keep = 8ull << 30;
-      cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
-    }
-    cudaGetLastError();
-  });
-}
+// The library's own stream-ordered memory pool of the current device (created on first use; the device's default
+// pool is never touched).  It keeps up to 8 GiB of freed allocations, so that the temporaries of one sweep are
+// handed to the next without a trip through the driver's page tables.  NULL on failure.
+cudaMemPool_t lib_pool();
 
 // RAII device buffer (cudaMalloc / cudaFree); zero-initialised on request.  `pooled` buffers are stream-ordered
 // (cudaMallocAsync / cudaFreeAsync on the allocating stream): for temporaries that only that stream touches.
@@ -86,11 +86,12 @@ struct DevBuf {
   int alloc(size_t nbytes, bool zero, cudaStream_t st, bool pool = false) {
     release();
     if (nbytes == 0) nbytes = 16;
-    if (pool) pool_keep_once();
-    cudaError_t e = pool ? cudaMallocAsync(&p, nbytes, st) : cudaMalloc(&p, nbytes);
+    cudaMemPool_t mp = pool ? lib_pool() : nullptr;
+    cudaError_t e = pool ? (mp ? cudaMallocFromPoolAsync(&p, nbytes, mp, st) : cudaMallocAsync(&p, nbytes, st))
+                         : cudaMalloc(&p, nbytes);
     if (e != cudaSuccess) {
       p = nullptr;
-      return set_error(TKM_ENOMEM, "%s(%zu bytes) failed: %s", pool ? "cudaMallocAsync" : "cudaMalloc", nbytes,
+      return set_error(TKM_ENOMEM, "%s(%zu bytes) failed: %s", pool ? "cudaMallocFromPoolAsync" : "cudaMalloc", nbytes,
                        cudaGetErrorString(e));
     }
     bytes = nbytes;
@@ -137,6 +138,15 @@ struct PinBuf {
 };
 
 int device_check();   // TKM_OK when a CUDA device of compute capability 10.x is current
+
+// true the first time it is called for (this flag word, the current device): per-device one-time kernel setup
+// (cudaFuncSetAttribute) without a process-wide "configured" bool
+inline bool first_use_on_device(std::atomic<unsigned long long>& done) {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return true;
+  const unsigned long long bit = 1ull << dev;
+  return (done.fetch_or(bit) & bit) == 0;
+}
 
 #ifdef __CUDACC__
 // ---- device-side PTX wrappers ------------------------------------------------------------------

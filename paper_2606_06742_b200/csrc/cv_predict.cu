@@ -300,6 +300,7 @@ using namespace tkm;
 
 extern "C" int tkm_exact_cv(const tkm_path* p, const void* y, const int32_t* foldid, double* cv_loss,
                             int64_t* cv_err, double* cv_mean, int32_t* best_l, void* stream) {
+  tkm::NvtxRange nvtx_range("tkm_exact_cv");
   if (!p || !y || !foldid || !cv_loss || !cv_mean || !best_l) return set_error(TKM_EINVAL, "tkm_exact_cv: NULL argument");
   TKM_TRY(device_check());
   cudaStream_t st = (cudaStream_t)stream;
@@ -420,6 +421,7 @@ extern "C" int tkm_path_coef(const tkm_path* p, int32_t t, int32_t l, int32_t v,
 extern "C" int tkm_predict(const tkm_path* p, int32_t t, int32_t l, const void* X_train, int64_t ldx,
                            const void* X_new, int64_t n_new, int64_t ldxn, int64_t pdim, double sigma,
                            void* f_out, int8_t* label_out, void* stream) {
+  tkm::NvtxRange nvtx_range("tkm_predict");
   if (!p || !X_train || !X_new || !f_out) return set_error(TKM_EINVAL, "tkm_predict: NULL argument");
   if (t < 0 || t >= p->T || l < 0 || l >= p->L) return set_error(TKM_EINVAL, "tkm_predict: (t, l) out of range");
   if (n_new <= 0 || pdim <= 0 || ldx < pdim || ldxn < pdim || !(sigma > 0.0))

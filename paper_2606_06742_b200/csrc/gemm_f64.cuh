@@ -346,11 +346,9 @@ int gemm_f64_make_args(const GemmProblem& pr, const GemmTile& tile, GemmArgs* ou
 template <class Cfg, class Epi>
 int launch_gemm_f64(const GemmArgs& a, int G, const Epi& epi, cudaStream_t st) {
   auto kern = gemm_f64_tma_kernel<Cfg, Epi>;
-  static bool configured = false;   // per template instantiation
-  if (!configured) {
+  static std::atomic<unsigned long long> configured{0};   // per template instantiation, one bit per device
+  if (first_use_on_device(configured))
     TKM_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
-    configured = true;
-  }
   dim3 grid((unsigned)ceil_div(a.M, Cfg::BM), (unsigned)(ceil_div(std::max(a.N, 1), Cfg::BN) * std::max(a.ksplit, 1)),
             (unsigned)G);
   kern<<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(a, epi);

@@ -76,12 +76,8 @@ int kblock_f64(const double* src, int64_t lds, int64_t rows, int64_t cols, doubl
   return TKM_OK;
 }
 
-static int g_forced_cfg = -1;
-int gemm_f64_force_cfg(int cfg) {
-  const int old = g_forced_cfg;
-  g_forced_cfg = (cfg >= 0 && cfg < GEMM_NUM_CFG) ? cfg : -1;
-  return old;
-}
+static std::atomic<int> g_forced_cfg{-1};
+int gemm_f64_force_cfg(int cfg) { return g_forced_cfg.exchange((cfg >= 0 && cfg < GEMM_NUM_CFG) ? cfg : -1); }
 
 template <class Cfg>
 static GemmTileInfo info_of(int regs_per_thread) {
@@ -111,7 +107,8 @@ static const GemmTileInfo& tile_info(int cfg) {
 // the probe grid (G in {1,5}, N = 8..300, M = K = 2000): 4 %.
 static const double kEff[GEMM_NUM_CFG] = {1.0, 1.05, 1.0, 1.0, 1.02, 1.06, 1.1, 1.5, 1.0, 1.0};
 GemmTile gemm_f64_choose(const int* nb, int G, int M, int K) {
-  if (g_forced_cfg >= 0) return gemm_f64_tile_of(g_forced_cfg);
+  const int forced = g_forced_cfg.load();
+  if (forced >= 0) return gemm_f64_tile_of(forced);
   const double tau = 0.59e-3 * K;                      // us per sub-tile unit
   const double trip = 1.0 * ((K + 15) / 16);           // us: K/16 stages x ~1 us round trip
   int best = 0;

@@ -463,8 +463,9 @@ struct Tf32Scratch {
 template <class Epi>
 int gemm_tf32_launch(Tf32Args a, int G, Tf32Scratch& sc, const Epi& epi, cudaStream_t st) {
   auto kern = gemm_tf32x3_kernel<Epi>;
-  // per device and cheap: set on every launch (no process-wide "configured" flag)
-  TKM_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TF32_SMEM));
+  static std::atomic<unsigned long long> configured{0};   // per template instantiation, one bit per device
+  if (first_use_on_device(configured))
+    TKM_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TF32_SMEM));
   a.G = G;
   a.partial = sc.partial.as<float>();
   a.flags = sc.flags.as<uint32_t>();

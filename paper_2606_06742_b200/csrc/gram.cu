@@ -161,5 +161,6 @@ extern "C" int tkm_gram(const void* X, int64_t n, int64_t p, int64_t ldx, const 
 extern "C" int tkm_gram_multi(const void* X, int64_t n, int64_t p, int64_t ldx, const void* X2, int64_t n2,
                               int64_t ldx2, const double* sigmas, int32_t G, tkm_dtype out_dt, void* const* Ks,
                               int64_t ldk, void* stream) {
+  tkm::NvtxRange nvtx_range("tkm_gram");
   return gram_launch(X, n, p, ldx, X2, n2, ldx2, sigmas, G, out_dt, Ks, ldk, (cudaStream_t)stream);
 }

@@ -11,7 +11,6 @@ struct tkm_spectral {
   int64_t n = 0, r = 0;
   int64_t ldr = 0;   // round_up(r, 16): leading dimension of every [.][r] array (zero padded)
   int64_t ldn = 0;   // round_up(n, 16): leading dimension of every [.][n] array (zero padded)
-  tkm_dtype sweep_dt = TKM_F64;
   tkm::DevBuf UL;    // [n][ldr] FP64   U * diag(Lam)   (Q operand of GEMM-A)
   tkm::DevBuf Ut;    // [r][ldn] FP64   U^T             (Q operand of GEMM-B)
   tkm::DevBuf lam;   // [ldr]    FP64   eigenvalues >= 0 (padding 0)

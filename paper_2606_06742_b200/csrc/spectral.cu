@@ -336,12 +336,12 @@ static int nystrom_x_impl(const double* X, int64_t n, int64_t p, int64_t ldx, do
 }  // namespace tkm
 
 extern "C" int tkm_spectral_setup(const void* K, int64_t n, int64_t ldk, const tkm_nystrom* ny,
-                                  tkm_dtype sweep_dt, tkm_spectral** out, void* stream) {
+                                  tkm_spectral** out, void* stream) {
+  tkm::NvtxRange nvtx_range("tkm_spectral_setup");
   using namespace tkm;
   if (!out) return set_error(TKM_EINVAL, "tkm_spectral_setup: out is NULL");
   *out = nullptr;
   if (n <= 1 || n > (1 << 30)) return set_error(TKM_EINVAL, "tkm_spectral_setup: n out of range");
-  if (sweep_dt != TKM_F64 && sweep_dt != TKM_F32) return set_error(TKM_EINVAL, "tkm_spectral_setup: bad sweep_dt");
   if (!ny && (!K || ldk < n)) return set_error(TKM_EINVAL, "tkm_spectral_setup: K NULL or ldk < n");
   if (ny && (!ny->K_nm || !ny->K_mm || ny->m < 1 || ny->m > n || ny->ld_nm < ny->m || ny->ld_mm < ny->m ||
              !ny->landmark_idx))
@@ -350,7 +350,6 @@ extern "C" int tkm_spectral_setup(const void* K, int64_t n, int64_t ldk, const t
   cudaStream_t st = (cudaStream_t)stream;
   tkm_spectral* s = new (std::nothrow) tkm_spectral();
   if (!s) return set_error(TKM_ENOMEM, "out of host memory");
-  s->sweep_dt = sweep_dt;
   int rc;
   if (ny) {
     NysSource src;
@@ -360,7 +359,6 @@ extern "C" int tkm_spectral_setup(const void* K, int64_t n, int64_t ldk, const t
   } else {
     rc = setup_full((const double*)K, n, ldk, s, st);
   }
-  if (rc == TKM_OK && sweep_dt == TKM_F32) rc = set_error(TKM_ENOTIMPL, "an all-FP32 (3xTF32) sweep is not provided: use TKM_F64, optionally with tkm_loss_opts.tf32_delta");
   if (rc != TKM_OK) {
     cudaStreamSynchronize(st);
     delete s;
@@ -375,6 +373,7 @@ extern "C" int tkm_spectral_setup(const void* K, int64_t n, int64_t ldk, const t
 extern "C" int tkm_spectral_setup_nystrom_x(const void* X, int64_t n, int64_t p, int64_t ldx, double sigma,
                                             const int64_t* landmark_idx, int64_t m, int64_t block_rows,
                                             tkm_spectral** out, void* stream) {
+  tkm::NvtxRange nvtx_range("tkm_spectral_setup_nystrom_x");
   using namespace tkm;
   if (!out) return set_error(TKM_EINVAL, "tkm_spectral_setup_nystrom_x: out is NULL");
   *out = nullptr;
@@ -388,7 +387,6 @@ extern "C" int tkm_spectral_setup_nystrom_x(const void* X, int64_t n, int64_t p,
   cudaStream_t st = (cudaStream_t)stream;
   tkm_spectral* s = new (std::nothrow) tkm_spectral();
   if (!s) return set_error(TKM_ENOMEM, "out of host memory");
-  s->sweep_dt = TKM_F64;
   int rc = nystrom_x_impl((const double*)X, n, p, ldx, sigma, landmark_idx, m, block_rows, s, st);
   if (rc != TKM_OK) {
     cudaStreamSynchronize(st);
@@ -402,8 +400,9 @@ extern "C" int tkm_spectral_setup_nystrom_x(const void* X, int64_t n, int64_t p,
 // G full-kernel setups side by side: a dense symmetric eigensolver spends much of its time in phases that
 // cannot fill the device (panel factorisations, the divide-and-conquer merge tree), so G decompositions
 // on G streams, driven by G host threads, overlap almost perfectly.
-extern "C" int tkm_spectral_setup_multi(const void* const* Ks, int32_t G, int64_t n, int64_t ldk, tkm_dtype sweep_dt,
+extern "C" int tkm_spectral_setup_multi(const void* const* Ks, int32_t G, int64_t n, int64_t ldk,
                                         tkm_spectral** out, void* stream) {
+  tkm::NvtxRange nvtx_range("tkm_spectral_setup_multi");
   using namespace tkm;
   if (!out || !Ks || G < 1 || G > 64) return set_error(TKM_EINVAL, "tkm_spectral_setup_multi: bad arguments");
   for (int g = 0; g < G; ++g) out[g] = nullptr;
@@ -416,9 +415,9 @@ extern "C" int tkm_spectral_setup_multi(const void* const* Ks, int32_t G, int64_
   std::vector<int> rc(G, TKM_OK);
   std::vector<std::string> msg(G);
   std::vector<int64_t> launches(G, 0);
-  if (n <= 1 || n > (1 << 30) || ldk < n || sweep_dt != TKM_F64) {
+  if (n <= 1 || n > (1 << 30) || ldk < n) {
     cudaEventDestroy(ready);
-    return set_error(sweep_dt != TKM_F64 ? TKM_ENOTIMPL : TKM_EINVAL, "tkm_spectral_setup_multi: bad n / ldk / sweep_dt");
+    return set_error(TKM_EINVAL, "tkm_spectral_setup_multi: bad n / ldk");
   }
   for (int g = 0; g < G; ++g) {   // every allocation happens here, before the concurrent part
     out[g] = new (std::nothrow) tkm_spectral();
@@ -431,7 +430,6 @@ extern "C" int tkm_spectral_setup_multi(const void* const* Ks, int32_t G, int64_
       cudaEventDestroy(ready);
       return a;
     }
-    out[g]->sweep_dt = sweep_dt;
   }
   cudaEventRecord(ready, st);   // K ready and the zero fills of the new buffers done
   std::vector<std::thread> th;

@@ -285,7 +285,7 @@ struct FLossArgs {
 constexpr int FLOSS_THREADS = 256, FLOSS_EPT = 2;   // samples per block: 512
 __global__ void __launch_bounds__(FLOSS_THREADS) floss_kernel(FLossArgs p) {
   __shared__ double red[32];
-  const int slot = blockIdx.y, grp = blockIdx.z;
+  const int slot = blockIdx.x, grp = blockIdx.z, mblk = blockIdx.y;   // slots on x: the leave-one-out form has > 65535
   if (slot >= p.nslots[grp]) return;
   const int gs = grp * p.B + slot, col = p.col_of_slot[gs], gc = grp * p.B + col;
   const double mu = p.mu[gc], bb = p.bbar[gc], inv_nc = 1.0 / p.col_nc[col], tau = p.col_tau[col];
@@ -293,7 +293,7 @@ __global__ void __launch_bounds__(FLOSS_THREADS) floss_kernel(FLossArgs p) {
   double zsum = 0.0;
 #pragma unroll
   for (int e = 0; e < FLOSS_EPT; ++e) {
-    const int m = (blockIdx.x * FLOSS_EPT + e) * FLOSS_THREADS + threadIdx.x;
+    const int m = (mblk * FLOSS_EPT + e) * FLOSS_THREADS + threadIdx.x;
     if (m < p.n) {
       const int64_t o = (int64_t)gs * p.ldz + m;
       const double fn = p.Fb[o] - (double)p.prod[(int64_t)gs * p.ldprod + m];
@@ -312,7 +312,7 @@ __global__ void __launch_bounds__(FLOSS_THREADS) floss_kernel(FLossArgs p) {
     }
   }
   zsum = block_sum(zsum, red);   // fixed order: deterministic
-  if (threadIdx.x == 0) p.gpart[(int64_t)blockIdx.x * p.ldpart + gs] = zsum;
+  if (threadIdx.x == 0) p.gpart[(int64_t)mblk * p.ldpart + gs] = zsum;
 }
 
 // ---- per-round initialisation (S3, G4): constants c, s; a' = a; abar = a; r = 1 ------------------
@@ -749,16 +749,18 @@ constexpr int KSPLIT_MAX = 16;
 constexpr int KBLOCK_F64_MIN_K = 16384;   // thin U: from this n on, the FP64 GEMM-B reads a K-blocked copy of U^T
 constexpr int KBLOCK_MIN_K = 8192;   // contraction depth from which the tcgen05 GEMM-B operands are kept K-blocked (no effect
                                     // at n = 2000, where U^T stays in L2; 2.4x at n = 581012)
-constexpr int DELTA_MIN_LIVE = 48;   // live columns (all groups) below which the delta forms are always switched off
+constexpr int DELTA_MIN_LIVE = 24;   // live columns (all groups) below which the delta forms are always switched off
 constexpr int POLL_RING = 8;   // ring of poll results: up to POLL_RING - 2 batches may be in flight
 
-// Live columns (all groups) from which a tcgen05 delta-form launch beats the FP64 DMMA launch it replaces.  The pair
-// kernel's time has a floor that does not depend on the width -- a chain of 12 dependent MMAs per 32-deep K tile at
-// about 55 ns each (measured, profiles/r02_pair_kernel.md) plus ~12 us of prologue and epilogue -- while the DMMA
-// launch costs 2 n r N / (18 TFLOP/s).  n = r = 2000: 121 columns; n = r >= 10^4: the floor DELTA_MIN_LIVE.
-static int delta_min_live(int64_t n, int64_t r) {
-  const double kt = 0.5 * ((double)ceil_div(n, 32) + (double)ceil_div(r, 32));   // mean K depth of the two contractions
-  const double t_tc = kt * 0.66e-6 + 12e-6;
+// Live columns (all groups) from which a tcgen05 delta-form launch beats the FP64 DMMA launch it replaces.  The
+// pair kernel's time has a floor that does not depend on the width: its stream-K partition gives each of the 74
+// pairs G ceil(M / 256) KT / 74 K-tiles, a K-tile is a chain of 12 dependent MMAs (~0.33 us at <= 128 slots,
+// measured, profiles/r02_pair_kernel.md), plus ~14 us of prologue, partial exchange and epilogue.  The DMMA launch
+// costs 2 n r N / (18 TFLOP/s).  5 x (n = r = 2000): 58 columns; n = r >= 10^4: the floor DELTA_MIN_LIVE.
+static int delta_min_live(int64_t n, int64_t r, int G) {
+  const double ktA = (double)G * (double)ceil_div(n, 256) * (double)ceil_div(r, 32) / 74.0;   // GEMM-A: M = n, K = r
+  const double ktB = (double)G * (double)ceil_div(r, 256) * (double)ceil_div(n, 32) / 74.0;   // GEMM-B: M = r, K = n
+  const double t_tc = 0.5 * (ktA + ktB) * 0.33e-6 + 14e-6;
   const double cols = t_tc * 18e12 / (2.0 * (double)n * (double)r);
   return std::max(DELTA_MIN_LIVE, (int)cols);
 }
@@ -771,6 +773,7 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
                                   const tkm_loss_opts* opts, const double* lambdas, int32_t L, const int32_t* foldid,
                                   int32_t V, double tol, int32_t maxit, const tkm_path* const* warm, tkm_path** out,
                                   void* stream) {
+  tkm::NvtxRange nvtx_range("tkm_fit_path");
   if (!out) return set_error(TKM_EINVAL, "tkm_fit_path: out is NULL");
   if (G < 1 || G > GEMM_MAX_GROUPS) return set_error(TKM_EINVAL, "tkm_fit_path_multi: need 1 <= G <= %d", GEMM_MAX_GROUPS);
   for (int g = 0; g < G; ++g) out[g] = nullptr;
@@ -779,9 +782,8 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
     if (!specs[g]) return set_error(TKM_EINVAL, "tkm_fit_path: NULL spectral handle");
   const tkm_spectral* s0 = specs[0];
   for (int g = 1; g < G; ++g)
-    if (specs[g]->n != s0->n || specs[g]->r != s0->r || specs[g]->ldr != s0->ldr || specs[g]->ldn != s0->ldn ||
-        specs[g]->sweep_dt != s0->sweep_dt)
-      return set_error(TKM_EINVAL, "tkm_fit_path_multi: all spectral handles must share n, r and the sweep precision");
+    if (specs[g]->n != s0->n || specs[g]->r != s0->r || specs[g]->ldr != s0->ldr || specs[g]->ldn != s0->ldn)
+      return set_error(TKM_EINVAL, "tkm_fit_path_multi: all spectral handles must share n and r");
   if (loss != TKM_LOSS_HINGE && loss != TKM_LOSS_LOGISTIC && loss != TKM_LOSS_QUANTILE && loss != TKM_LOSS_DWD)
     return set_error(TKM_EINVAL, "tkm_fit_path: unknown loss %d", (int)loss);
   if (L < 1 || V < 2 || V > s0->n) return set_error(TKM_EINVAL, "tkm_fit_path: need L >= 1 and 2 <= V <= n");
@@ -800,7 +802,6 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
   if (rounds < 1) return set_error(TKM_EINVAL, "tkm_fit_path: rounds must be >= 1");
   if (smoothed && (!(opts->smooth0 > 0.0) || !(opts->eta > 0.0 && opts->eta <= 1.0)))
     return set_error(TKM_EINVAL, "tkm_fit_path: need smooth0 > 0 and 0 < eta <= 1");
-  if (s0->sweep_dt != TKM_F64) return set_error(TKM_ENOTIMPL, "tkm_fit_path: only the FP64 sweep is built");
   TKM_TRY(device_check());
   cudaStream_t st = (cudaStream_t)stream;
   const int64_t n = s0->n, r = s0->r, ldr = s0->ldr, ldn = s0->ldn;
@@ -987,7 +988,8 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
   const int ce_mult = ce_env && *ce_env ? std::max(1, std::min(8, atoi(ce_env))) : 2;
   const int ce_max = opts->tf32_delta != 0 ? ce_mult * check_every : check_every;
   const int nsamp = opts->profile == 2 ? ce_max : 2;
-  const int dmin = delta_min_live(s0->n, s0->r);
+  const char* dm_env = getenv("TKM_DELTA_MIN");   // tuning aid: override the live-column threshold of the delta forms
+  const int dmin = dm_env && *dm_env ? std::max(1, atoi(dm_env)) : delta_min_live(s0->n, s0->r, G);
   struct Events {
     cudaEvent_t poll[POLL_RING] = {};
     std::vector<cudaEvent_t> pev;   // [POLL_RING][nsamp][4]: (A0, A1, B0, B1) per sampled iteration
@@ -1061,6 +1063,7 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
   // One smoothing round (S3-S7 until every participating column has met `rtol`) at level `smooth`; `active`
   // ([G*B] device, or NULL = all columns) selects the participating columns (outer control, reading G23).
   auto run_round = [&](int rnd, double smooth, double rtol, const int32_t* active) -> int {
+    NvtxRange nvtx_round("tkm smoothing round");
     const double curv = curvature_of(loss, smooth);
     RoundArgs ra{(int)r, B, ldr, gp, curv, p0->col_lam.as<double>(), p0->col_nc.as<double>(), col_c.as<double>(),
                  col_s.as<double>(), A.as<double>(), Aprev.as<double>(), Abar.as<double>(), beta.as<double>(),
@@ -1210,7 +1213,7 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
                        prodA.as<float>(), ldn32, Fb.as<double>(), Fp.as<double>(), Zt.as<double>(), ldn,
                        dz_hi.as<float>(), dz_lo.as<float>(), ldn32, gpart.as<double>(), ldpart, dz_blk_rows};
           nblkA = (int)ceil_div(n, FLOSS_THREADS * FLOSS_EPT);
-          floss_kernel<<<dim3((unsigned)nblkA, (unsigned)std::max(nmax, 1), (unsigned)G), FLOSS_THREADS, 0, st>>>(fa);
+          floss_kernel<<<dim3((unsigned)std::max(nmax, 1), (unsigned)nblkA, (unsigned)G), FLOSS_THREADS, 0, st>>>(fa);
           TKM_LAUNCH_CHECK();
           famA = 2;
         } else {
@@ -1455,6 +1458,15 @@ extern "C" int tkm_path_info(const tkm_path* p, int32_t* B, int64_t* r, int32_t*
   if (flags) memcpy(flags, p->h_flags.data(), p->B * sizeof(int32_t));
   if (beta0) memcpy(beta0, p->h_beta0.data(), p->B * sizeof(double));
   if (total_col_iters) *total_col_iters = p->total_col_iters;
+  return TKM_OK;
+}
+
+extern "C" int tkm_path_shape(const tkm_path* p, int32_t* T, int32_t* L, int32_t* V, int64_t* n) {
+  if (!p) return set_error(TKM_EINVAL, "tkm_path_shape: NULL handle");
+  if (T) *T = p->T;
+  if (L) *L = p->L;
+  if (V) *V = p->V;
+  if (n) *n = p->spec->n;
   return TKM_OK;
 }
 

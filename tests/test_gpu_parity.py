@@ -300,13 +300,15 @@ def test_configs_2_3_reduced_n_against_an_oracle_fit(tkm, cfg, delta):
     L, V, T = w.L, w.V, w.T
     cols = None if cfg == 2 else [(t * (V + 1) + v) * L + l for t in range(T) for v in range(V + 1)
                                   for l in range(0, L, 5)]
-    # The stop tolerance is an input of both sides (reading G6).  On the check-loss columns the oracle's own tol = 1e-12
-    # iterate is 5e-11 .. 8e-11 (relative l2) away from its tol = 1e-14 iterate (condition ~ 70), so two sides that
-    # both stop at 1e-12 can be 1.5e-10 apart; at 3e-13 each is within 2e-11 of the minimiser.
-    stop = 3e-13 if cfg == 3 else STOP_TOL
-    X, y, spec, path, cv = _run_gpu(tkm, w, sigma, foldid, stop, 400000, warm_tol=1e-3, tf32_delta=delta)
+    # The stop tolerance is an input (reading G6); the comparison target is the minimiser.  On the check-loss columns
+    # the oracle's own tol = 1e-12 iterate is 5e-11 .. 8e-11 (relative l2) away from its tol = 1e-14 iterate (condition
+    # ~ 70), so two sides that BOTH stop at 1e-12 can be 1.5e-10 apart although each is inside the 1e-10 budget.  The
+    # reference therefore stops at 3e-13 here (within 2e-11 of the minimiser; at 1e-13 some of its columns sit on the
+    # rounding floor of the residual and never stop); the GPU keeps the 1e-12 of every other test (3e-13 is below
+    # the rounding floor of ITS residual on some of these columns).  DESIGN.md section 7.
+    X, y, spec, path, cv = _run_gpu(tkm, w, sigma, foldid, STOP_TOL, 400000, warm_tol=1e-3, tf32_delta=delta)
     res, spec_o, worst, degenerate = _compare_path(tkm, w, sigma, foldid, spec, path, cv, columns=cols, warm_tol=1e-3,
-                                                   stop_tol=stop)
+                                                   stop_tol=3e-13 if cfg == 3 else STOP_TOL)
     print("cfg %d at n = 1500, tf32_delta %d: worst relative l2 coefficient error %.3g" % (cfg, delta, worst))
     cv_loss, cv_err, cv_mean, best = cv
     if cols is None:
@@ -319,6 +321,8 @@ def test_configs_2_3_reduced_n_against_an_oracle_fit(tkm, cfg, delta):
         fsize = np.bincount(foldid, minlength=V).astype(np.float64)
         for t in range(T):
             for l in range(0, L, 5):
+                if any((t * (V + 1) + v) * L + l in degenerate for v in range(V)):
+                    continue                      # beta0 of a hold-out column is not unique there (G18)
                 pooled = 0.0
                 for v in range(V):
                     c = (t * (V + 1) + v) * L + l
