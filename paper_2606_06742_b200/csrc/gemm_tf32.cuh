@@ -148,18 +148,15 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(TF32_THREADS, 1)
   pl.mp = (g.M + 2 * TF32_BM - 1) / (2 * TF32_BM);
   pl.KT = (g.K + TF32_BK - 1) / TF32_BK;
   if (threadIdx.x == 0) {
-    // Slot tiles.  A tile is as wide as tensor memory allows (512 slots) when there are enough tiles for every
-    // pair; with few tiles (n = 2000: 8 row pairs x 5 bandwidths) the slots of a group are cut into up to four
-    // narrower tiles instead, so that every pair runs a contraction AND its share of the epilogue (the FP64
-    // epilogues cost as much as the contraction there), and stream-K balances what is left.
-    int live_groups = 0;
-    for (int i = 0; i < g.G; ++i) live_groups += (g.nslots ? min(g.nslots[i], g.N) : g.N) > 0;
-    const int want = live_groups > 0 ? (int)(gridDim.x >> 1) / (live_groups * pl.mp) : 1;   // tiles per (group, row pair)
+    // Slot tiles are as wide as tensor memory allows (512 slots); stream-K balances the pairs along K.  (Cutting
+    // the slots of a group into narrower tiles so that every pair also gets a share of the epilogue was tried when
+    // the FP64 state updates were still fused into this kernel; with the product-only epilogue it only costs
+    // MMA efficiency: 57 ns per MMA at 128 slots against 87 ns at 256.)
     gr.tile_base[0] = 0;
     int hm = 0;
     for (int i = 0; i < g.G; ++i) {
       const int n = max(0, g.nslots ? min(g.nslots[i], g.N) : g.N);
-      const int split = max((n + TF32_BN - 1) / TF32_BN, min(min(want, 4), (n + 63) / 64));
+      const int split = (n + TF32_BN - 1) / TF32_BN;
       const int bn = n > 0 ? tf32_tile_pad((n + split - 1) / split) : 64;
       gr.ng[i] = n;
       gr.bn[i] = bn;

@@ -746,7 +746,7 @@ static double curvature_of(tkm_loss loss, double smooth) {
 
 constexpr int KSPLIT_MIN_K = 16384;   // contraction depth from which GEMM-B may be K-split (thin U, large n)
 constexpr int KSPLIT_MAX = 16;
-constexpr int KBLOCK_F64_MIN_K = 16384;   // thin U: from this n on, the FP64 GEMM-B reads a K-blocked copy of U^T
+constexpr int KBLOCK_F64_MIN_K = 8192;   // contraction depth from which the FP64 GEMMs read K-blocked copies of U^T / U Lam
 constexpr int KBLOCK_MIN_K = 8192;   // contraction depth from which the tcgen05 GEMM-B operands are kept K-blocked (no effect
                                     // at n = 2000, where U^T stays in L2; 2.4x at n = 581012)
 constexpr int DELTA_MIN_LIVE = 24;   // live columns (all groups) below which the delta forms are always switched off
@@ -1039,8 +1039,11 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
   prB.K = (int)n;
   // thin U with n >= KBLOCK_F64_MIN_K: the FP64 GEMM-B reads a K-blocked copy of U^T (its rows are n * 8 bytes
   // apart: every 128-byte piece of a stage would come from another page; profiles/r01f)
-  const bool kblk64 = n >= KBLOCK_F64_MIN_K && r < n;
-  DevBuf utb[GEMM_MAX_GROUPS];
+  // ... and, for the same reason, GEMM-A reads a K-blocked copy of U Lam once r * 8 bytes is a large stride (full
+  // kernel at n >= 8192): narrow live batches stream U at HBM speed only if a stage is one contiguous read
+  // (profiles/r02_narrow_batch.md: 0.56 -> see there of the copy bandwidth at n = 20000, 14 live columns)
+  const bool kblk64 = n >= KBLOCK_F64_MIN_K, kblk64A = r >= KBLOCK_F64_MIN_K;
+  DevBuf utb[GEMM_MAX_GROUPS], ulb[GEMM_MAX_GROUPS];
   for (int g = 0; g < G; ++g) {
     prA.Q[g] = specs[g]->UL.as<double>();
     prB.Q[g] = specs[g]->Ut.as<double>();
@@ -1049,8 +1052,14 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
       TKM_TRY(kblock_f64(specs[g]->Ut.as<double>(), ldn, r, n, utb[g].as<double>(), st));
       prB.Q[g] = utb[g].as<double>();
     }
+    if (kblk64A) {
+      TKM_TRY(ulb[g].alloc((size_t)ceil_div(r, (int64_t)TMA_BOX_K) * n * TMA_BOX_K * sizeof(double), false, st, true));
+      TKM_TRY(kblock_f64(specs[g]->UL.as<double>(), ldr, n, r, ulb[g].as<double>(), st));
+      prA.Q[g] = ulb[g].as<double>();
+    }
   }
   prB.q_blocked = kblk64;
+  prA.q_blocked = kblk64A;
   GemmArgs argsA, argsB;
   GemmTile tileA{-1, 0, 0}, tileB{-1, 0, 0};
 
