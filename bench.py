@@ -424,12 +424,12 @@ def narrow_hbm_roofline(res, pk):
     pr = res["prof"]
     out = []
     n, r = res["n"], res["r"]
-    for i in (0, 1):
+    for i in (0, 1, 2, 3):     # 2, 3: the tcgen05 delta-form contractions (hi + lo FP32 operands: the same bytes)
         nl = int(pr["launches"][i])
         if not nl:
             continue
         live = pr["flops"][i] / nl / (2.0 * n * r)          # average live columns of the sampled launches
-        by = n * r * 8.0 + live * (r + n) * 8.0
+        by = n * r * 8.0 + live * (r + n) * 8.0 + (live * (n if i == 2 else r) * 4.0 if i >= 2 else 0.0)
         ms = pr["ms"][i] / nl
         out.append({"bound": "hbm", "kernel": FAMILY[i], "achieved": by / (ms / 1e3) / 1e9, "peak": pk["hbm"],
                     "unit": "GB/s", "frac": by / (ms / 1e3) / 1e9 / pk["hbm"], "traffic": None,
@@ -498,7 +498,7 @@ def run_single(args):
         w = wl.CONFIGS[cfg]()
         frac = {1: [0.5], 2: [0.4, 0.7], 4: [0.3, 0.5, 0.7, 0.9]}[args.narrow_L]
         kw["lam_idx"] = [int(round(f * (w.L - 1))) for f in frac]
-        kw["tf32_delta"] = 0 if args.tf32_delta < 0 else args.tf32_delta
+        kw["tf32_delta"] = TF32_DELTA_LARGE if args.tf32_delta < 0 else args.tf32_delta   # 0: the all-FP64 DMMA stream
         what = ("%s: BASELINE.json configs[%d] at full n = %d with %d lambda(s) (grid indices %s): B = %d columns, the "
                 "HBM-bound narrow batch of SURVEY.md 8(d)" % (name, cfg, w.n, args.narrow_L, kw["lam_idx"],
                                                                w.T * args.narrow_L * (w.V + 1)))

@@ -746,10 +746,11 @@ static double curvature_of(tkm_loss loss, double smooth) {
 
 constexpr int KSPLIT_MIN_K = 16384;   // contraction depth from which GEMM-B may be K-split (thin U, large n)
 constexpr int KSPLIT_MAX = 16;
-constexpr int KBLOCK_F64_MIN_K = 8192;   // contraction depth from which the FP64 GEMMs read K-blocked copies of U^T / U Lam
+constexpr int KBLOCK_F64_MIN_K = 16384;   // thin U: from this n on, the FP64 GEMM-B reads a K-blocked copy of U^T
 constexpr int KBLOCK_MIN_K = 8192;   // contraction depth from which the tcgen05 GEMM-B operands are kept K-blocked (no effect
                                     // at n = 2000, where U^T stays in L2; 2.4x at n = 581012)
-constexpr int DELTA_MIN_LIVE = 24;   // live columns (all groups) below which the delta forms are always switched off
+constexpr int DELTA_MIN_LIVE = 24;   // live columns (all groups) below which the delta forms are switched off when U is L2-sized
+constexpr int DELTA_MIN_FLOOR = 8;   // ... and when U streams from HBM
 constexpr int POLL_RING = 8;   // ring of poll results: up to POLL_RING - 2 batches may be in flight
 
 // Live columns (all groups) from which a tcgen05 delta-form launch beats the FP64 DMMA launch it replaces.  The
@@ -762,6 +763,11 @@ static int delta_min_live(int64_t n, int64_t r, int G) {
   const double ktB = (double)G * (double)ceil_div(r, 256) * (double)ceil_div(n, 32) / 74.0;   // GEMM-B: M = r, K = n
   const double t_tc = 0.5 * (ktA + ktB) * 0.33e-6 + 14e-6;
   const double cols = t_tc * 18e12 / (2.0 * (double)n * (double)r);
+  // Once one operand copy is far beyond L2 (n >= 10^4) even the narrowest batch is a stream of U from HBM, and the
+  // pair kernel streams at 5.3-6.4 TB/s where the DMMA kernel reaches 3.0-3.7 (profiles/r02_narrow_batch.md): the
+  // delta forms then stay on down to a handful of columns.  At 5 x n = 2000 (160 MB, half of it L2 hits in the
+  // tail) the measured optimum is the model's 58 (1 / 16 / 32 / 58: 1265 / 736 / 710 / 680 ms sweeps).
+  if ((double)G * (double)n * (double)r * 8.0 > 2.0 * 126e6) return DELTA_MIN_FLOOR;
   return std::max(DELTA_MIN_LIVE, (int)cols);
 }
 
@@ -1039,10 +1045,10 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
   prB.K = (int)n;
   // thin U with n >= KBLOCK_F64_MIN_K: the FP64 GEMM-B reads a K-blocked copy of U^T (its rows are n * 8 bytes
   // apart: every 128-byte piece of a stage would come from another page; profiles/r01f)
-  // ... and, for the same reason, GEMM-A reads a K-blocked copy of U Lam once r * 8 bytes is a large stride (full
-  // kernel at n >= 8192): narrow live batches stream U at HBM speed only if a stage is one contiguous read
-  // (profiles/r02_narrow_batch.md: 0.56 -> see there of the copy bandwidth at n = 20000, 14 live columns)
-  const bool kblk64 = n >= KBLOCK_F64_MIN_K, kblk64A = r >= KBLOCK_F64_MIN_K;
+  // (K-blocked FP64 copies of BOTH operands for the full kernel at n >= 8192 were measured in round 2 and bought
+  // nothing: 3452 against 3664 GB/s at n = 20000 with 14 live columns, profiles/r02_narrow_batch.md -- with rows
+  // "only" 160 KB apart the 128-byte pieces of a stage are not what limits the stream; kblk64A stays off.)
+  const bool kblk64 = n >= KBLOCK_F64_MIN_K && r < n, kblk64A = false;
   DevBuf utb[GEMM_MAX_GROUPS], ulb[GEMM_MAX_GROUPS];
   for (int g = 0; g < G; ++g) {
     prA.Q[g] = specs[g]->UL.as<double>();
