@@ -53,11 +53,11 @@ struct CvEpi {
     double tot;
     if (cta_row_reduce<Cfg>(ls, warp_n, warp_m, lane, scratch, tot)) {
       const int col = n_blk0 + (int)threadIdx.x;
-      if (col < N) lpart[(int64_t)blockIdx.x * ldpart + col] = tot;
+      if (col < N) lpart[(int64_t)gemm_m_block() * ldpart + col] = tot;
     }
     if (cta_row_reduce<Cfg>(es, warp_n, warp_m, lane, scratch, tot)) {
       const int col = n_blk0 + (int)threadIdx.x;
-      if (col < N) epart[(int64_t)blockIdx.x * ldpart + col] = tot;
+      if (col < N) epart[(int64_t)gemm_m_block() * ldpart + col] = tot;
     }
   }
 };
@@ -105,11 +105,11 @@ struct GapEpi {
     double tot;
     if (cta_row_reduce<Cfg>(ls, warp_n, warp_m, lane, scratch, tot)) {
       const int col = n_blk0 + (int)threadIdx.x;
-      if (col < N) lpart[(int64_t)blockIdx.x * ldpart + col] = tot;
+      if (col < N) lpart[(int64_t)gemm_m_block() * ldpart + col] = tot;
     }
     if (cta_row_reduce<Cfg>(ds, warp_n, warp_m, lane, scratch, tot)) {
       const int col = n_blk0 + (int)threadIdx.x;
-      if (col < N) dpart[(int64_t)blockIdx.x * ldpart + col] = tot;
+      if (col < N) dpart[(int64_t)gemm_m_block() * ldpart + col] = tot;
     }
   }
 };

@@ -36,14 +36,19 @@ struct GemmArgs {
   const int32_t* nslots;                // [G] device, live rows of each group; NULL => N for all
   int p_group_rows;                     // row offset between consecutive groups in P
   int N, M, K;                          // N: upper bound of the live rows (the grid covers it)
-  int ksplit;                           // <= 1: one CTA contracts all of K; S > 1: blockIdx.y = split * n_tiles + n_tile,
+  int ksplit;                           // <= 1: one CTA contracts all of K; S > 1: blockIdx.x = split * n_tiles + n_tile,
                                         // split s contracts K-tiles [s KT/S, (s+1) KT/S) and the epilogue sees a partial sum
   int q_blk_rows;                       // 0: Q_g row-major [M][K]; > 0: Q_g K-blocked [K/16][q_blk_rows][16] (map over
                                         // [(K/16) q_blk_rows][16]): a stage's Q tile is one contiguous read (thin U, K = n large)
 };
 
 // K-split index of this CTA, for epilogues that store partial sums (ksplit as in GemmArgs / Tf32Args)
-__device__ __forceinline__ int gemm_split_index(int ksplit) { return ksplit > 1 ? (int)(blockIdx.y / (gridDim.y / ksplit)) : 0; }
+__device__ __forceinline__ int gemm_split_index(int ksplit) { return ksplit > 1 ? (int)(blockIdx.x / (gridDim.x / ksplit)) : 0; }
+// Grid: x = (K-split, slot tile) -- fastest, so that the CTAs that share a Q tile (the same rows of U) are
+// scheduled together and the tile is read from HBM once (ncu at n = 20000, 900 slots, with x = row tile: 48 GB of
+// DRAM reads per launch against 3.3 GB algorithmic); y = row tile of the output (index of the per-tile partial sums
+// the epilogues write); z = group.
+__device__ __forceinline__ int gemm_m_block() { return (int)blockIdx.y; }
 
 template <int TN_, int WN_, int TM_, int WM_, int STAGES_>
 struct GemmCfg {
@@ -157,8 +162,8 @@ __global__ void __launch_bounds__(Cfg::THREADS)
 
   const int grp = blockIdx.z;
   const int N = g.nslots ? min(g.nslots[grp], g.N) : g.N;
-  const int S = max(g.ksplit, 1), ny = (int)gridDim.y / S, split = (int)blockIdx.y / ny;
-  const int m_blk0 = blockIdx.x * BM, n_blk0 = ((int)blockIdx.y - split * ny) * BN;
+  const int S = max(g.ksplit, 1), ny = (int)gridDim.x / S, split = (int)blockIdx.x / ny;
+  const int m_blk0 = blockIdx.y * BM, n_blk0 = ((int)blockIdx.x - split * ny) * BN;
   if (n_blk0 >= N) return;   // the grid is sized for an upper bound of the live slots
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int KT_all = (g.K + TMA_BOX_K - 1) / TMA_BOX_K;
@@ -349,7 +354,8 @@ int launch_gemm_f64(const GemmArgs& a, int G, const Epi& epi, cudaStream_t st) {
   static std::atomic<unsigned long long> configured{0};   // per template instantiation, one bit per device
   if (first_use_on_device(configured))
     TKM_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
-  dim3 grid((unsigned)ceil_div(a.M, Cfg::BM), (unsigned)(ceil_div(std::max(a.N, 1), Cfg::BN) * std::max(a.ksplit, 1)),
+  if (ceil_div(a.M, Cfg::BM) > 65535) return set_error(TKM_EINVAL, "GEMM: more than 65535 row tiles");
+  dim3 grid((unsigned)(ceil_div(std::max(a.N, 1), Cfg::BN) * std::max(a.ksplit, 1)), (unsigned)ceil_div(a.M, Cfg::BM),
             (unsigned)G);
   kern<<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(a, epi);
   TKM_LAUNCH_CHECK();

@@ -138,7 +138,7 @@ struct LossEpi {
     double tot;
     if (cta_row_reduce<Cfg>(colsum, warp_n, warp_m, lane, scratch, tot)) {
       const int slot = n_blk0 + (int)threadIdx.x;
-      if (slot < N) gpart[(int64_t)blockIdx.x * ldpart + g0 + slot] = tot;
+      if (slot < N) gpart[(int64_t)gemm_m_block() * ldpart + g0 + slot] = tot;
     }
   }
 };
@@ -282,7 +282,7 @@ struct FLossArgs {
   int64_t ldpart;
   int dz_blk_rows;
 };
-constexpr int FLOSS_THREADS = 256, FLOSS_EPT = 2;   // samples per block: 512
+constexpr int FLOSS_THREADS = 256, FLOSS_EPT = 4;   // samples per block: 1024
 __global__ void __launch_bounds__(FLOSS_THREADS) floss_kernel(FLossArgs p) {
   __shared__ double red[32];
   const int slot = blockIdx.x, grp = blockIdx.z, mblk = blockIdx.y;   // slots on x: the leave-one-out form has > 65535
@@ -290,20 +290,42 @@ __global__ void __launch_bounds__(FLOSS_THREADS) floss_kernel(FLossArgs p) {
   const int gs = grp * p.B + slot, col = p.col_of_slot[gs], gc = grp * p.B + col;
   const double mu = p.mu[gc], bb = p.bbar[gc], inv_nc = 1.0 / p.col_nc[col], tau = p.col_tau[col];
   const int hv = p.col_v[col];
+  const int64_t row = (int64_t)gs * p.ldz;
+  const double* __restrict__ y = p.y;
+  const int32_t* __restrict__ fold = p.foldid;
+  const float* __restrict__ prod = p.prod + (int64_t)gs * p.ldprod;
+  double* __restrict__ Fb = p.Fb + row;
+  double* __restrict__ Fp = p.Fp + row;
+  double* __restrict__ Zt = p.Zt + row;
+  // all loads of the thread's samples first (independent round trips in flight), then the arithmetic and the stores
+  double fbv[FLOSS_EPT], fpv[FLOSS_EPT], zov[FLOSS_EPT], yv[FLOSS_EPT];
+  float pv[FLOSS_EPT];
+  int fv[FLOSS_EPT];
+#pragma unroll
+  for (int e = 0; e < FLOSS_EPT; ++e) {
+    const int m = (mblk * FLOSS_EPT + e) * FLOSS_THREADS + threadIdx.x;
+    if (m < p.n) {
+      fbv[e] = Fb[m];
+      fpv[e] = Fp[m];
+      zov[e] = Zt[m];
+      pv[e] = prod[m];
+      yv[e] = y[m];
+      fv[e] = fold[m];
+    }
+  }
   double zsum = 0.0;
 #pragma unroll
   for (int e = 0; e < FLOSS_EPT; ++e) {
     const int m = (mblk * FLOSS_EPT + e) * FLOSS_THREADS + threadIdx.x;
     if (m < p.n) {
-      const int64_t o = (int64_t)gs * p.ldz + m;
-      const double fn = p.Fb[o] - (double)p.prod[(int64_t)gs * p.ldprod + m];
-      const double fb = fn + mu * (fn - p.Fp[o]);
-      p.Fp[o] = fn;
-      p.Fb[o] = fb;
+      const double fn = fbv[e] - (double)pv[e];
+      const double fb = fn + mu * (fn - fpv[e]);
+      Fp[m] = fn;
+      Fb[m] = fb;
       double z = 0.0;
-      if (p.foldid[m] != hv) z = psi_fast(p.loss, p.y[m], fb + bb, p.smooth, p.inv_2s, tau) * inv_nc;
-      const double d = z - p.Zt[o];
-      p.Zt[o] = z;
+      if (fv[e] != hv) z = psi_fast(p.loss, yv[e], fb + bb, p.smooth, p.inv_2s, tau) * inv_nc;
+      const double d = z - zov[e];
+      Zt[m] = z;
       const float h = to_tf32((float)d);
       const int64_t od = dz_index(gs, m, p.lddz, p.dz_blk_rows);
       p.dz_hi[od] = h;
