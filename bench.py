@@ -340,7 +340,7 @@ def time_weighted(prof2, tp):
 
 # ----------------------------------------------------------------------------------------- single-problem runner
 def run_problem(tkm, w, *, tf32_delta, tol, warm_tol, profile=1, nystrom_streamed=False, loo=False, lam_idx=None,
-                clocks_index=0, gap_tol=0.0):
+                clocks_index=0, gap_tol=0.0, delta_min_live=0):
     """One pass of S1..S9 over ONE (X, sigma) problem on the current device; X, y resident.  Returns a dict of stage
     times (ms), column-iterations, sampled kernel families and clocks."""
     import torch
@@ -381,7 +381,7 @@ def run_problem(tkm, w, *, tf32_delta, tol, warm_tol, profile=1, nystrom_streame
     e2 = ev()
     path = tkm.tkm_fit_path(spec, y, w.loss, lambdas, foldid, V, tol, MAXIT, smooth0=w.smooth0, eta=w.eta,
                             rounds=w.rounds, taus=taus, warm_tol=warm_tol, tf32_delta=tf32_delta, profile=profile,
-                            gap_tol=gap_tol)
+                            gap_tol=gap_tol, delta_min_live=delta_min_live)
     e3 = ev()
     cv = tkm.tkm_exact_cv(path, y, foldid, w.T, len(lambdas), V)
     e4 = ev()
@@ -480,7 +480,7 @@ def run_single(args):
     name = args.workload
     pk, traffic = peaks(), traffic_table()
     kw = dict(tf32_delta=TF32_DELTA_LARGE if args.tf32_delta < 0 else args.tf32_delta, tol=args.tol, warm_tol=WARM_TOL,
-              profile=2 if args.profile_all else 1, gap_tol=args.gap_tol)
+              profile=2 if args.profile_all else 1, gap_tol=args.gap_tol, delta_min_live=args.delta_min_live)
     if name.startswith("nystrom_"):
         w = wl.nystrom_paper_shape(name[len("nystrom_"):])
         kw["nystrom_streamed"] = True
@@ -512,7 +512,7 @@ def run_single(args):
     for it in range(args.warmup + args.steps):
         res = run_problem(tkm, w, **kw)          # the last pass is reported (a pass takes seconds to a minute)
     knobs = {"tf32_delta": kw["tf32_delta"], "stop_tol": args.tol, "warm_start_rounds_tol": WARM_TOL,
-             "gap_tol": args.gap_tol, "profile": kw["profile"],
+             "gap_tol": args.gap_tol, "profile": kw["profile"], "delta_min_live": args.delta_min_live,
              "l2": "inputs larger than L2" if w.n * res["r"] * 8 > 126e6 else "not flushed"}
     d = problem_summary(res, pk, traffic, what, knobs)
     total_ms = sum(d["stages_ms"].values())
@@ -574,7 +574,7 @@ def run_ours(args, w, rank, world):
         e2 = ev()
         paths = tkm.tkm_fit_path_multi(specs, y, w.loss, w.lambdas, foldid, w.V, tol, MAXIT, smooth0=w.smooth0,
                                        eta=w.eta, rounds=w.rounds, warm_tol=WARM_TOL, tf32_delta=TF32_DELTA,
-                                       profile=profile)
+                                       profile=profile, delta_min_live=args.delta_min_live)
         e3 = ev()
         best = [int(tkm.tkm_exact_cv(path, y, foldid, w.T, w.L, w.V)[3][0]) for path in paths]
         e4 = ev()
@@ -733,6 +733,8 @@ def main():
     ap.add_argument("--tf32-delta", type=int, default=-1, help="override the delta-form mode of a --workload run")
     ap.add_argument("--gap-tol", type=float, default=0.0,
                     help="outer control of PAPER.md:220-222 (reading G23) for a --workload run; 0 = fixed schedule")
+    ap.add_argument("--delta-min-live", type=int, default=0,
+                    help="live columns at or below which a delta-form sweep runs all-FP64 (0 = the library's cost model)")
     ap.add_argument("--narrow-L", type=int, default=1, choices=[1, 2, 4])
     ap.add_argument("--loo-lambdas", type=int, default=0, help="loo_config1: use this many lambdas of the grid (0 = all 50)")
     ap.add_argument("--probe-iters", type=int, default=20, help="gemm_probe: launches per shape")

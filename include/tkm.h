@@ -89,6 +89,10 @@ typedef struct {
                       /* tkm_path_duality_gap) keeps that level's minimiser and leaves the schedule; a warm_tol */
                       /* iterate only screens: the column is first finished to `tol` at that level and tested  */
                       /* again.  `rounds` is the cap: a column that reaches it with a larger gap gets flag 2.  */
+  int32_t delta_min_live; /* live columns (all groups) at or below which a delta-form sweep runs all-FP64; <= 0:   */
+                      /* the library's cost model of the two contraction kernels (58 at 5 x n = 2000, 8 once U     */
+                      /* streams from HBM; never engaged for tiny problems).  Tests set it to exercise the delta   */
+                      /* forms on small inputs.                                                                    */
 } tkm_loss_opts;
 
 /* Nystrom inputs for tkm_spectral_setup (reading G11). */

@@ -29,7 +29,7 @@ class _LossOpts(C.Structure):
     _fields_ = [("smooth0", C.c_double), ("eta", C.c_double), ("rounds", C.c_int32), ("T", C.c_int32),
                 ("taus", C.POINTER(C.c_double)), ("restart", C.c_int32), ("check_every", C.c_int32),
                 ("warm_tol", C.c_double), ("profile", C.c_int32), ("tf32_delta", C.c_int32),
-                ("gap_tol", C.c_double)]
+                ("gap_tol", C.c_double), ("delta_min_live", C.c_int32)]
 
 
 class _Nystrom(C.Structure):
@@ -328,21 +328,24 @@ class Path:
             pass
 
 
-def _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, profile=False, tf32_delta=0, gap_tol=0.0):
+def _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, profile=False, tf32_delta=0, gap_tol=0.0,
+          delta_min_live=0):
     taus_arr = _host(taus if taus is not None else [], np.float64)
     o = _LossOpts(float(smooth0), float(eta), int(rounds), int(len(taus_arr)),
                   taus_arr.ctypes.data_as(C.POINTER(C.c_double)) if len(taus_arr) else None,
-                  int(bool(restart)), int(check_every), float(warm_tol), int(profile), int(tf32_delta), float(gap_tol))
+                  int(bool(restart)), int(check_every), float(warm_tol), int(profile), int(tf32_delta), float(gap_tol),
+                  int(delta_min_live))
     return o, taus_arr
 
 
 def tkm_fit_path(spec: Spectral, y, loss: int, lambdas, foldid, V: int, tol: float, maxit: int,
                  smooth0=1.0, eta=0.125, rounds=4, taus=None, restart=True, check_every=0, warm_tol=0.0,
-                 warm: Path | None = None, profile=False, tf32_delta=0, gap_tol=0.0, stream=None) -> Path:
+                 warm: Path | None = None, profile=False, tf32_delta=0, gap_tol=0.0, delta_min_live=0, stream=None) -> Path:
     y = _dev_vec(y, spec.n, "y")
     lam = _host(lambdas, np.float64)
     fid = _fold_vec(foldid, spec.n, V)
-    o, keep = _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, profile, tf32_delta, gap_tol)
+    o, keep = _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, profile, tf32_delta, gap_tol,
+                    delta_min_live)
     h = C.c_void_p()
     rc = lib().tkm_fit_path(spec._h, y.data_ptr(), loss, C.byref(o), _ptr(lam), len(lam), _ptr(fid), V,
                             float(tol), int(maxit), warm._h if warm is not None else None, C.byref(h),
@@ -353,12 +356,13 @@ def tkm_fit_path(spec: Spectral, y, loss: int, lambdas, foldid, V: int, tol: flo
 
 def tkm_fit_path_multi(specs, y, loss: int, lambdas, foldid, V: int, tol: float, maxit: int,
                        smooth0=1.0, eta=0.125, rounds=4, taus=None, restart=True, check_every=0, warm_tol=0.0,
-                       warm=None, profile=False, tf32_delta=0, gap_tol=0.0, stream=None):
+                       warm=None, profile=False, tf32_delta=0, gap_tol=0.0, delta_min_live=0, stream=None):
     """One sweep over G spectral handles that share y, folds and the lambda grid -> list of G Paths."""
     y = _dev_vec(y, specs[0].n, "y")
     lam = _host(lambdas, np.float64)
     fid = _fold_vec(foldid, specs[0].n, V)
-    o, keep = _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, profile, tf32_delta, gap_tol)
+    o, keep = _opts(loss, smooth0, eta, rounds, taus, restart, check_every, warm_tol, profile, tf32_delta, gap_tol,
+                    delta_min_live)
     G = len(specs)
     hs = (C.c_void_p * G)(*[s._h for s in specs])
     hw = (C.c_void_p * G)(*[w._h for w in warm]) if warm is not None else None

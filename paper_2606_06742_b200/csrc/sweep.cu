@@ -1016,8 +1016,7 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
   const int ce_mult = ce_env && *ce_env ? std::max(1, std::min(8, atoi(ce_env))) : 2;
   const int ce_max = opts->tf32_delta != 0 ? ce_mult * check_every : check_every;
   const int nsamp = opts->profile == 2 ? ce_max : 2;
-  const char* dm_env = getenv("TKM_DELTA_MIN");   // tuning aid: override the live-column threshold of the delta forms
-  const int dmin = dm_env && *dm_env ? std::max(1, atoi(dm_env)) : delta_min_live(s0->n, s0->r, G);
+  const int dmin = opts->delta_min_live > 0 ? opts->delta_min_live : delta_min_live(s0->n, s0->r, G);
   struct Events {
     cudaEvent_t poll[POLL_RING] = {};
     std::vector<cudaEvent_t> pev;   // [POLL_RING][nsamp][4]: (A0, A1, B0, B1) per sampled iteration

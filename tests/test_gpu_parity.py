@@ -461,7 +461,7 @@ def test_outer_control_matches_the_oracle(tkm, loss_name, warm_tol, delta):
     sigma = float(w.sigmas[0])
     foldid = tkm.tkm_make_folds(w.n, w.V, w.fold_seed)
     X, y, spec, path, cv = _run_gpu(tkm, w, sigma, foldid, STOP_TOL, 400000, warm_tol=warm_tol, tf32_delta=delta,
-                                    gap_tol=gap_tol)
+                                    gap_tol=gap_tol, delta_min_live=16)
     lev_g, sm_g = path.levels()
     info = path.info()
     assert (info["flags"] & 1).sum() == 0
@@ -660,7 +660,11 @@ def test_delta_form_sweep_keeps_fp64_parity(tkm, name, mode):
          "logit_ragged": lambda: wl.config2(n=333, p=9, L=7, V=3)}[name]()
     sigma = float(w.sigmas[0])
     foldid = tkm.tkm_make_folds(w.n, w.V, w.fold_seed)
-    X, y, spec, path, cv = _run_gpu(tkm, w, sigma, foldid, STOP_TOL, 400000, tf32_delta=mode)
+    X, y, spec, path, cv = _run_gpu(tkm, w, sigma, foldid, STOP_TOL, 400000, tf32_delta=mode,
+                                    delta_min_live=16, profile=1)   # small n: the cost model alone would stay all-FP64
+    if name != "logit_ragged":      # (a handful of batches there: the sampled first iterations may all be exact ones)
+        assert path.profile()["launches"][3] > 0 and (mode == 1 or path.profile()["launches"][2] > 0), \
+            "the delta form never engaged"
     res, spec_o, worst, degenerate = _compare_path(tkm, w, sigma, foldid, spec, path, cv)
     print("%s (delta form %d): worst relative l2 coefficient error %.3g" % (name, mode, worst))
     cv_o = o.exact_cv(spec_o, res, w.y, foldid, w.loss, w.taus)
@@ -732,7 +736,10 @@ def test_thin_u_long_contraction_ksplit_parity(tkm, mode):
     spec_o = o.nystrom_setup(w.X, sigma, idx)
     assert spec.r == spec_o.r
     tol = 1e-11
-    path = tkm.tkm_fit_path(spec, y, w.loss, w.lambdas, foldid, w.V, tol, 200000, rounds=w.rounds, tf32_delta=mode)
+    path = tkm.tkm_fit_path(spec, y, w.loss, w.lambdas, foldid, w.V, tol, 200000, rounds=w.rounds, tf32_delta=mode,
+                            delta_min_live=16, profile=1)
+    if mode:
+        assert path.profile()["launches"][3] > 0, "the delta form never engaged"
     info = path.info()
     assert info["flags"].sum() == 0 and np.all(info["kkt"] <= tol)
     if "res" not in _KSPLIT_ORACLE:      # the oracle's fit takes most of a minute: once for both modes
