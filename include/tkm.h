@@ -75,13 +75,13 @@ typedef struct {
                       /* 2: time EVERY contraction launch and count the column-iterations of  */
                       /* each kernel family on the device (a measurement mode: ~4 events and  */
                       /* two atomics per iteration; not for timed runs)                       */
-  int32_t tf32_delta; /* 2: both contractions in delta form (also F = U Lam a: F+ = Fbar - U Lam da, two  */
-                      /* FP64 GEMM-A per exact iteration).  1: delta-form GEMM-B only.  zeta = U^T z is kept in FP64 and advanced by        */
-                      /* zeta += U^T (z - z_old) with the increment contracted in 3xTF32 on the     */
-                      /* tcgen05 tensor cores (its error is relative to the increment, which        */
-                      /* vanishes at convergence); zeta is recomputed in FP64 after every           */
-                      /* compaction (every check_every iterations).  Same fixed point and           */
-                      /* tolerances as 0 (all FP64 DMMA); DESIGN.md section 12.                     */
+  int32_t tf32_delta; /* 0: every contraction in FP64 (DMMA).  1: delta form of GEMM-B: zeta = U^T z is kept in FP64  */
+                      /* and advanced by zeta += U^T (z - z_old), the increment contracted in 3xTF32 on the tcgen05  */
+                      /* tensor cores (its error is relative to the increment, which vanishes at convergence).      */
+                      /* 2: also GEMM-A: F+ = Fbar - U Lam da.  The recurrences restart from exact FP64 products on  */
+                      /* the first iteration of a round and the last iteration of every batch (check_every, twice  */
+                      /* that in wide batches), and only those exact iterations decide convergence.  Same fixed    */
+                      /* point and tolerances as 0; DESIGN.md section 12.                                           */
   double gap_tol;     /* outer control of PAPER.md:220-222 ("shrink delta ... until the KKT conditions of  */
                       /* all SVM models are satisfied"; reading G23).  <= 0: the fixed schedule of `rounds`  */
                       /* levels for every column.  > 0: after round k < rounds-1 a column whose solution     */
@@ -98,11 +98,11 @@ typedef struct {
 /* Nystrom inputs for tkm_spectral_setup (reading G11). */
 typedef struct {
   const double* K_nm;        /* [dev] n x m cross kernel k(x_i, x_landmark_j), FP64            */
-  int64_t ld_nm;
+  int64_t ld_nm;             /* leading dimensions must be EVEN (16-byte aligned rows), else TKM_EINVAL */
   const double* K_mm;        /* [dev] m x m landmark kernel, FP64                              */
   int64_t ld_mm;
   int64_t m;                 /* number of landmarks                                            */
-  const int64_t* landmark_idx; /* [host] m row indices into X (kept for tkm_predict)           */
+  const int64_t* landmark_idx; /* [host] m row indices into X, each in [0, n) (kept for tkm_predict) */
 } tkm_nystrom;
 
 /* ---- S1  RBF Gram matrix (PAPER.md:69 kernel="rbf"; reading G12) -----------------------------
@@ -199,7 +199,8 @@ int tkm_path_shape(const tkm_path* p, int32_t* T, int32_t* L, int32_t* V, int64_
 int tkm_path_levels(const tkm_path* p, int32_t* level, double* smooth);
 /* Sampled kernel timings of the sweep (only when tkm_loss_opts.profile was 1), all [host] arrays of 4, one
  * entry per kernel family and contraction: [0] FP64 DMMA GEMM-A, [1] FP64 DMMA GEMM-B, [2] tcgen05 3xTF32
- * delta GEMM-A, [3] tcgen05 3xTF32 delta GEMM-B.  ms = summed CUDA-event durations of the sampled launches (the
+ * delta GEMM-A, [3] tcgen05 3xTF32 delta GEMM-B (the contraction launches alone, not the elementwise passes that
+ * consume their products).  ms = summed CUDA-event durations of the sampled launches (the
  * first iteration after every compaction -- every slot live -- and, in the delta forms, the exact last
  * iteration of the batch), flops = summed algorithmic flops 2 n r (live columns) of those launches
  * (4 n r per column-iteration over the two contractions), launches = their number.
@@ -304,8 +305,9 @@ int tkm_gemm_probe(int32_t cfg, int32_t G, int32_t N, int32_t M, int32_t K, int3
                    void* stream);
 /* 3xTF32 contraction on the tcgen05 tensor cores (the FP32 variant of the sweep's products), test and
  * calibration entry: Dt[N][M] (FP64, [dev]) = P[N][K] Q[M][K]^T with the FP64 inputs split on the fly into
- * TF32 (hi, lo) pairs and accumulated in FP32 as lo*hi + hi*lo + hi*hi.  cfg: 0/1/2 = 64/128/256 slots per
- * tile, -1 = chosen from N.  ms [host] NULL or the milliseconds per launch over `iters` timed launches.
+ * TF32 (hi, lo) pairs and accumulated in FP32 as lo*hi + hi*lo + hi*hi.  cfg is ignored (the CTA-pair kernel has
+ * one tile shape: 256 rows x up to 512 slots, stream-K over K).  ms [host] NULL or the milliseconds per launch over
+ * `iters` timed launches.
  * Synchronises `stream`. */
 int tkm_tf32x3_gemm_nt(const double* P, int64_t ldp, const double* Q, int64_t ldq, double* Dt, int64_t ldd,
                        int64_t N, int64_t M, int64_t K, int32_t cfg, int32_t iters, float* ms, void* stream);

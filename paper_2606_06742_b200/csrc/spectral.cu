@@ -346,6 +346,15 @@ extern "C" int tkm_spectral_setup(const void* K, int64_t n, int64_t ldk, const t
   if (ny && (!ny->K_nm || !ny->K_mm || ny->m < 1 || ny->m > n || ny->ld_nm < ny->m || ny->ld_mm < ny->m ||
              !ny->landmark_idx))
     return set_error(TKM_EINVAL, "tkm_spectral_setup: bad tkm_nystrom fields");
+  if (ny) {
+    if ((ny->ld_nm & 1) || (ny->ld_mm & 1))
+      return set_error(TKM_EINVAL, "tkm_spectral_setup: ld_nm and ld_mm must be even (the TMA operands need 16-byte aligned rows); "
+                                   "pad K_nm / K_mm to an even leading dimension");
+    for (int64_t j = 0; j < ny->m; ++j)
+      if (ny->landmark_idx[j] < 0 || ny->landmark_idx[j] >= n)
+        return set_error(TKM_EINVAL, "tkm_spectral_setup: landmark_idx[%lld] = %lld is outside [0, n)", (long long)j,
+                         (long long)ny->landmark_idx[j]);
+  }
   TKM_TRY(device_check());
   cudaStream_t st = (cudaStream_t)stream;
   tkm_spectral* s = new (std::nothrow) tkm_spectral();
