@@ -269,8 +269,16 @@ def library_probes(tkm):
     return out
 
 
-def family_rooflines(prof, tp, traffic, probes=None):
-    """One roofline object per kernel family with sampled launches.  prof: dict(ms, flops, launches) arrays of 4."""
+L2_BYTES = 126e6     # B200 L2 (B200_PROFILING.md): a U operand set larger than this streams from HBM every launch
+
+
+def family_rooflines(prof, tp, traffic, probes=None, geom=None, hbm_peak=None, tkeys=None):
+    """One roofline object per kernel family with sampled launches.  prof: dict(ms, flops, launches) arrays of 4.
+    geom = (n, r, G): with it every object also carries the HBM side of the same launches (`hbm`: algorithmic bytes
+    = G n r 8 for the U operand of the G groups + live (n + r) 8 for the moving operand and the result, over the
+    measured copy bandwidth) and `binding` = the side the roofline model says binds at the launches' arithmetic
+    intensity (flops per algorithmic byte against the ridge point peak flops / peak bandwidth; "tensor" whenever
+    the U operands of one launch fit in L2)."""
     out = []
     for i in range(4):
         nl = int(prof["launches"][i])
@@ -280,7 +288,7 @@ def family_rooflines(prof, tp, traffic, probes=None):
         ach = (fl / 1e12) / (ms / 1e3) if ms > 0 else 0.0
         f64 = i < 2
         peak = tp["f64_contract"] if f64 else tp["tf32x3_contract"]
-        tr = traffic.get("fam%d" % i)
+        tr = traffic.get((tkeys or {}).get(i, "fam%d" % i))
         d = {"bound": "tensor", "kernel": FAMILY[i], "achieved": ach, "peak": peak, "unit": "TFLOP/s",
              "frac": ach / peak, "traffic": tr[0] if tr else None, "traffic_source": tr[1] if tr else None,
              "peak_source": tp["src"] + (" x nominal f64/bf16 ratio %.4f" % NOMINAL_RATIO["f64"] if f64 else
@@ -289,6 +297,17 @@ def family_rooflines(prof, tp, traffic, probes=None):
         if f64:
             d["peak_dmma_issue"] = tp["f64_issue"]
             d["frac_of_issue"] = ach / tp["f64_issue"]
+        if geom and hbm_peak and fl > 0:
+            n, r, G = geom
+            live = fl / nl / (2.0 * n * r)
+            u_bytes = G * n * r * 8.0
+            by = u_bytes + live * (n + r) * 8.0
+            gbs = by / (ms / nl / 1e3) / 1e9
+            ai, ridge = fl / nl / by, peak * 1e12 / (hbm_peak * 1e9)
+            d["hbm"] = {"achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
+                        "algorithmic_bytes_per_launch": by, "avg_live_columns": live,
+                        "flops_per_byte": ai, "ridge_flops_per_byte": ridge}
+            d["binding"] = "hbm" if (ai < ridge and u_bytes > L2_BYTES) else "tensor"
         if probes:
             pm = probes["cublas_dgemm_tflops"] if f64 else probes["cublas_tf32_tflops"] / 3.0
             d["peak_measured"] = pm
@@ -315,7 +334,35 @@ def merge_families(fams, idx):
         d["frac_of_issue"] = ach / d["peak_dmma_issue"]
     if "peak_measured" in d:
         d["frac_of_measured"] = ach / d["peak_measured"]
+    if all("hbm" in f for f in sel):
+        by = sum(f["hbm"]["algorithmic_bytes_per_launch"] * f["sampled_launches"] for f in sel)
+        h = dict(d["hbm"])
+        gbs = by / (ms / 1e3) / 1e9
+        h.update(achieved=gbs, frac=gbs / h["peak"], algorithmic_bytes_per_launch=by / nl, flops_per_byte=fl / by,
+                 avg_live_columns=sum(f["hbm"]["avg_live_columns"] * f["sampled_launches"] for f in sel) / nl)
+        d["hbm"] = h
+        d["binding"] = max(sel, key=lambda f: f["sampled_ms"])["binding"]
     return d
+
+
+def binding_side(d):
+    """The roofline object the bench line carries: `bound` is the side that binds the sampled launches (see
+    family_rooflines); the other side's figures stay in the object under `tensor_side` / `hbm_side`."""
+    if d is None or d.get("binding") != "hbm":
+        if d is not None and "hbm" in d:
+            d = dict(d)
+            d["hbm_side"] = d.pop("hbm")
+        return d
+    h = d["hbm"]
+    t = {k: d[k] for k in ("achieved", "peak", "unit", "frac", "peak_source", "frac_of_issue", "peak_dmma_issue",
+                           "peak_measured", "frac_of_measured", "peak_measured_source") if k in d}
+    o = {k: v for k, v in d.items() if k not in t and k != "hbm"}
+    o.update(bound="hbm", achieved=h["achieved"], peak=h["peak"], unit="GB/s", frac=h["frac"],
+             peak_source="MEASURED_PEAKS.json copy bandwidth",
+             algorithmic_bytes_per_launch=h["algorithmic_bytes_per_launch"],
+             avg_live_columns=h["avg_live_columns"], flops_per_byte=h["flops_per_byte"],
+             ridge_flops_per_byte=h["ridge_flops_per_byte"], tensor_side=t)
+    return o
 
 
 def time_weighted(prof2, tp):
@@ -399,10 +446,10 @@ def run_problem(tkm, w, *, tf32_delta, tol, warm_tol, profile=1, nystrom_streame
     return out
 
 
-def problem_summary(res, pk, traffic, what, knobs, probes=None):
+def problem_summary(res, pk, traffic, what, knobs, probes=None, tkeys=None):
     tp = tensor_peaks(pk, res["clocks"].get("sm_mhz"))
-    fams = family_rooflines(res["prof"], tp, traffic, probes)
     n, r = res["n"], res["r"]
+    fams = family_rooflines(res["prof"], tp, traffic, probes, geom=(n, r, 1), hbm_peak=pk["hbm"], tkeys=tkeys)
     sweep_s = res["sweep_ms"] / 1e3
     total_ms = res["gram_ms"] + res["setup_ms"] + res["sweep_ms"] + res["cv_ms"]
     d = {"workload": what, "columns": res["B"], "launch_config": knobs,
@@ -413,7 +460,8 @@ def problem_summary(res, pk, traffic, what, knobs, probes=None):
          "sweep_useful_tflops": 4.0 * n * r * res["col_iters"] / sweep_s / 1e12,
          "gram_gbs": res["gram_bytes"] / (res["gram_ms"] / 1e3) / 1e9 if res["gram_ms"] > 0 else None,
          "gram_frac_of_hbm": res["gram_bytes"] / (res["gram_ms"] / 1e3) / 1e9 / pk["hbm"] if res["gram_ms"] > 0 else None,
-         "roofline": max(fams, key=lambda f: f["sampled_ms"]) if fams else None, "roofline_families": fams,
+         "roofline": binding_side(max(fams, key=lambda f: f["sampled_ms"])) if fams else None,
+         "roofline_families": [binding_side(f) for f in fams],
          "peak_device_memory_gb": res["peak_mem_gb"], "clocks": res["clocks"], "selected_lambda_index": res["best_l"]}
     return d
 
@@ -514,7 +562,8 @@ def run_single(args):
     knobs = {"tf32_delta": kw["tf32_delta"], "stop_tol": args.tol, "warm_start_rounds_tol": WARM_TOL,
              "gap_tol": args.gap_tol, "profile": kw["profile"], "delta_min_live": args.delta_min_live,
              "l2": "inputs larger than L2" if w.n * res["r"] * 8 > 126e6 else "not flushed"}
-    d = problem_summary(res, pk, traffic, what, knobs)
+    tkeys = {2: "config3_tcgen05_full_width", 3: "config3_tcgen05_full_width"} if name == "config3" else None
+    d = problem_summary(res, pk, traffic, what, knobs, tkeys=tkeys)
     total_ms = sum(d["stages_ms"].values())
     line = {"metric": METRIC, "value": d["fits_per_s"], "unit": UNIT, "n_gpus": 1, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": total_ms, "higher_is_better": True, "scaling": "weak",
@@ -654,7 +703,7 @@ def run_ours(args, w, rank, world):
     pk, traffic = peaks(), traffic_table()
     tp = tensor_peaks(pk, clocks.get("sm_mhz") if clocks else None)
     probes = library_probes(tkm) if world == 1 else None
-    fams = family_rooflines(prof, tp, traffic, probes)
+    fams = family_rooflines(prof, tp, traffic, probes, geom=(w.n, w.n, len(w.sigmas)), hbm_peak=pk["hbm"])
     # the FP64 DMMA kernel (both epilogues) and the tcgen05 kernel (both delta forms): the dominant one -- the larger
     # share of the sampled kernel time -- is `roofline`
     roof_f64, roof_tf32 = merge_families(fams, (0, 1)), merge_families(fams, (2, 3))
@@ -683,7 +732,7 @@ def run_ours(args, w, rank, world):
             "col_iters_per_step": prof["col_iters"] / args.steps,
             "sweep_useful_tflops": 4.0 * w.n * w.n * prof["col_iters"] / sweep_s / 1e12,
             "gram_gbs": gram_gbs, "gram_frac_of_hbm": gram_gbs / pk["hbm"],
-            "roofline": roofline, "roofline_other_kernel": roofline_other, "clocks": clocks, "gpu_launches": int(launches),
+            "roofline": binding_side(roofline), "roofline_other_kernel": binding_side(roofline_other), "clocks": clocks, "gpu_launches": int(launches),
             "e2e": {"value": world * fits_per_step / (ms_e2e / args.steps / 1e3), "unit": UNIT,
                     "h2d_bytes_per_step": int(nb_in), "d2h_bytes_per_step": int(nb_out),
                     "ms_per_step": ms_e2e / args.steps,
@@ -707,7 +756,8 @@ def run_ours(args, w, rank, world):
                 "n=20000, p=28, 5 folds, 50 lambdas 1e1..1e-6, gamma 1 -> 1/512 in 4 rounds; ONE pass (no warm-up "
                 "pass, outside the timed region of `value`)",
                 {"tf32_delta": TF32_DELTA_LARGE, "stop_tol": 1e-10, "warm_start_rounds_tol": WARM_TOL,
-                 "l2": "inputs larger than L2 (U Lam and U^T: 3.2 GB each)"}, probes)
+                 "l2": "inputs larger than L2 (U Lam and U^T: 3.2 GB each)"}, probes,
+                tkeys={2: "config3_tcgen05_full_width", 3: "config3_tcgen05_full_width"})
         ncol, secs, its = oracle_sample_step(w)
         line["cpu_baseline"] = {"value": ncol / secs, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
                                 "sample": sample_text(w, ncol, secs, its)}
