@@ -255,6 +255,22 @@ int tkm_predict(const tkm_path* p, int32_t t, int32_t l,
                 const void* X_train, int64_t ldx, const void* X_new, int64_t n_new, int64_t ldxn,
                 int64_t pdim, double sigma, void* f_out, int8_t* label_out, void* stream);
 
+/* tkm_predict_noalloc: tkm_predict for callers that may not allocate (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc).  Same arguments, same two kernels, same result; it calls no
+ * cudaMalloc / cudaFree / stream-ordered allocation and no allocating library routine, and it does not synchronise
+ * (fully asynchronous on `stream`).  The coefficient vector between the two kernels -- tkm_predict's only device
+ * temporary -- lives in a static device array of TKM_PREDICT_NOALLOC_MAX_COEF FP64 (512 KB, held by every GPU
+ * that loads the library until the process exits).
+ *   Limit: the number of coefficients (training rows n; Nystrom: landmarks m) must not exceed
+ *   TKM_PREDICT_NOALLOC_MAX_COEF, else TKM_EINVAL with a message naming the limit (use tkm_predict).
+ *   Sharing: every call on one device uses the same array, and it keeps the last call's contents (each call
+ *   overwrites all entries it reads, so nothing needs clearing).  Calls that can overlap on the GPU -- different
+ *   streams, or graph branches without a dependency -- RACE on it: serialise them. */
+#define TKM_PREDICT_NOALLOC_MAX_COEF 65536
+int tkm_predict_noalloc(const tkm_path* p, int32_t t, int32_t l,
+                        const void* X_train, int64_t ldx, const void* X_new, int64_t n_new, int64_t ldxn,
+                        int64_t pdim, double sigma, void* f_out, int8_t* label_out, void* stream);
+
 /* ---- probability calibration on the exact-CV path (G21) ----
  * tkm_cv_decision_values: f_out [dev] n FP64, f_out[j] = held-out decision value of training row j at
  * (t, lambda_l), i.e. from the column that held out fold foldid[j] (no refitting).  foldid [host] n.

@@ -9,7 +9,7 @@ missing `libtkm.so` or a missing GPU raises.
 from .api import (  # noqa: F401
     TkmError, LOSS_HINGE, LOSS_LOGISTIC, LOSS_QUANTILE, LOSS_DWD, F32, F64,
     lib, lib_path, tkm_version, tkm_last_error, tkm_make_folds,
-    tkm_gram, tkm_gram_multi, tkm_spectral_setup, tkm_spectral_setup_multi, tkm_spectral_setup_nystrom_x, tkm_fit_path, tkm_fit_path_multi, tkm_exact_cv, tkm_cv_select, tkm_path_duality_gap, tkm_fit_cv_sharded, tkm_predict, tkm_path_coef,
+    tkm_gram, tkm_gram_multi, tkm_spectral_setup, tkm_spectral_setup_multi, tkm_spectral_setup_nystrom_x, tkm_fit_path, tkm_fit_path_multi, tkm_exact_cv, tkm_cv_select, tkm_path_duality_gap, tkm_fit_cv_sharded, tkm_predict, tkm_predict_noalloc, tkm_path_coef,
     tkm_train_tune_host, tkm_cv_decision_values, tkm_platt_fit, tkm_platt_proba, tkm_dgemm_nt, tkm_gemm_probe, tkm_tf32x3_gemm_nt, tkm_launch_count, tkm_launch_count_reset,
     Spectral, Path, EXPORTED_SYMBOLS,
 )

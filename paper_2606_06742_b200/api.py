@@ -14,7 +14,7 @@ TKM_OK, TKM_ENOTCONV = 0, 5
 EXPORTED_SYMBOLS = [
     "tkm_gram", "tkm_gram_multi", "tkm_spectral_setup", "tkm_spectral_setup_multi", "tkm_spectral_setup_nystrom_x", "tkm_spectral_free", "tkm_spectral_info", "tkm_spectral_get_u",
     "tkm_fit_path", "tkm_fit_path_multi", "tkm_path_free", "tkm_path_info", "tkm_path_shape", "tkm_path_levels", "tkm_fold_sizes", "tkm_path_profile", "tkm_path_get_a", "tkm_exact_cv", "tkm_cv_select", "tkm_path_duality_gap", "tkm_path_coef",
-    "tkm_predict", "tkm_cv_decision_values", "tkm_platt_fit", "tkm_platt_proba", "tkm_train_tune_host", "tkm_make_folds", "tkm_launch_count", "tkm_launch_count_reset",
+    "tkm_predict", "tkm_predict_noalloc", "tkm_cv_decision_values", "tkm_platt_fit", "tkm_platt_proba", "tkm_train_tune_host", "tkm_make_folds", "tkm_launch_count", "tkm_launch_count_reset",
     "tkm_dgemm_nt", "tkm_gemm_probe", "tkm_tf32x3_gemm_nt", "tkm_version", "tkm_last_error",
 ]
 
@@ -79,6 +79,7 @@ def lib():
     L.tkm_cv_select.argtypes = [vp, vp, vp, i32, i32, i32, vp, vp, vp]
     L.tkm_path_coef.argtypes = [vp, i32, i32, i32, vp, C.POINTER(dbl), vp]
     L.tkm_predict.argtypes = [vp, i32, i32, vp, i64, vp, i64, i64, i64, dbl, vp, vp, vp]
+    L.tkm_predict_noalloc.argtypes = [vp, i32, i32, vp, i64, vp, i64, i64, i64, dbl, vp, vp, vp]
     L.tkm_cv_decision_values.argtypes = [vp, i32, i32, vp, vp, vp]
     L.tkm_platt_fit.argtypes = [vp, vp, i64, C.POINTER(dbl), C.POINTER(dbl), C.POINTER(i32), vp]
     L.tkm_platt_proba.argtypes = [vp, i64, dbl, dbl, vp, vp]
@@ -459,6 +460,26 @@ def tkm_predict(path: Path, t: int, l: int, X_train, X_new, sigma: float, labels
                              X_new.stride(0), p, float(sigma), f.data_ptr(),
                              lab.data_ptr() if lab is not None else None, _stream(stream)))
     return f, lab
+
+
+PREDICT_NOALLOC_MAX_COEF = 65536
+
+
+def tkm_predict_noalloc(path: Path, t: int, l: int, X_train, X_new, sigma: float, f_out, label_out=None, stream=None):
+    """tkm_predict without any allocation (include/tkm.h): the caller passes the outputs (f_out: n_new FP64 on the
+    device, label_out: n_new int8 or None); asynchronous on `stream`."""
+    import torch
+    X_train, X_new = _dev_f64(X_train, "X_train"), _dev_f64(X_new, "X_new")
+    n_new, p = X_new.shape
+    if not (f_out.is_cuda and f_out.dtype == torch.float64 and f_out.is_contiguous() and f_out.numel() >= n_new):
+        raise ValueError("f_out: contiguous float64 CUDA tensor of n_new elements")
+    if label_out is not None and not (label_out.is_cuda and label_out.dtype == torch.int8 and
+                                      label_out.is_contiguous() and label_out.numel() >= n_new):
+        raise ValueError("label_out: contiguous int8 CUDA tensor of n_new elements")
+    _check(lib().tkm_predict_noalloc(path._h, t, l, X_train.data_ptr(), X_train.stride(0), X_new.data_ptr(), n_new,
+                                     X_new.stride(0), p, float(sigma), f_out.data_ptr(),
+                                     label_out.data_ptr() if label_out is not None else None, _stream(stream)))
+    return f_out, label_out
 
 
 def tkm_train_tune_host(X, y, sigmas, loss, lambdas, foldid, V, tol, maxit, smooth0=1.0, eta=0.125, rounds=4,

@@ -442,3 +442,65 @@ extern "C" int tkm_predict(const tkm_path* p, int32_t t, int32_t l, const void* 
   TKM_CUDA(cudaStreamSynchronize(st));   // `coef` is freed on return
   return TKM_OK;
 }
+
+// ---- tkm_predict_noalloc: the serving call for callers that may not allocate -------------------------------
+// Same two kernels as tkm_predict (tmatvec_kernel: alpha = U a of the selected column; predict_kernel: the fused
+// cross-kernel contraction); the coefficient vector `alpha` between them -- tkm_predict's only device temporary --
+// lives in a file-scope device array instead of a cudaMalloc'ed buffer.  Every device that loads the library
+// holds these 512 KB until the process exits.
+namespace tkm {
+static __device__ __align__(256) double g_predict_coef[TKM_PREDICT_NOALLOC_MAX_COEF];
+
+// In host code `g_predict_coef` is the host-side shadow of the symbol, not a device address: the kernels get the
+// address cudaGetSymbolAddress returns for the CURRENT device, looked up once per device (no allocation: the array
+// is part of the loaded module) and cached.
+static int predict_coef_scratch(double** out) {
+  static double* addr[64] = {};
+  static std::atomic<unsigned long long> have{0};
+  int dev = -1;
+  TKM_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) return set_error(TKM_EINVAL, "tkm_predict_noalloc: device ordinal %d outside 0..63", dev);
+  const unsigned long long bit = 1ull << dev;
+  if (!(have.load(std::memory_order_acquire) & bit)) {
+    double* ptr = nullptr;
+    cudaError_t e = cudaGetSymbolAddress((void**)&ptr, g_predict_coef);
+    if (e != cudaSuccess || !ptr)
+      return set_error(TKM_ECUDA, "tkm_predict_noalloc: cudaGetSymbolAddress failed on device %d: %s", dev,
+                       cudaGetErrorString(e));
+    addr[dev] = ptr;   // racing first calls on one device store the same address
+    have.fetch_or(bit, std::memory_order_release);
+  }
+  *out = addr[dev];
+  return TKM_OK;
+}
+}  // namespace tkm
+
+extern "C" int tkm_predict_noalloc(const tkm_path* p, int32_t t, int32_t l, const void* X_train, int64_t ldx,
+                                   const void* X_new, int64_t n_new, int64_t ldxn, int64_t pdim, double sigma,
+                                   void* f_out, int8_t* label_out, void* stream) {
+  if (!p || !X_train || !X_new || !f_out) return set_error(TKM_EINVAL, "tkm_predict_noalloc: NULL argument");
+  if (t < 0 || t >= p->T || l < 0 || l >= p->L) return set_error(TKM_EINVAL, "tkm_predict_noalloc: (t, l) out of range");
+  if (n_new <= 0 || pdim <= 0 || ldx < pdim || ldxn < pdim || !(sigma > 0.0))
+    return set_error(TKM_EINVAL, "tkm_predict_noalloc: bad shape or sigma");
+  const tkm_spectral* s = p->spec;
+  const int64_t ncoef = s->m > 0 ? s->m : s->n;
+  if (ncoef > TKM_PREDICT_NOALLOC_MAX_COEF)
+    return set_error(TKM_EINVAL,
+                     "tkm_predict_noalloc: %lld coefficients (training rows, or Nystrom landmarks) exceed the static "
+                     "scratch of TKM_PREDICT_NOALLOC_MAX_COEF = %d; use tkm_predict",
+                     (long long)ncoef, (int)TKM_PREDICT_NOALLOC_MAX_COEF);
+  if (n_new > (int64_t)PQ * 2147483647LL) return set_error(TKM_EINVAL, "tkm_predict_noalloc: n_new too large");
+  TKM_TRY(device_check());
+  cudaStream_t st = (cudaStream_t)stream;
+  double* coef = nullptr;
+  TKM_TRY(predict_coef_scratch(&coef));
+  const int col = (t * (p->V + 1) + p->V) * p->L + l;
+  // tmatvec_kernel writes all `ncoef` entries predict_kernel reads: nothing of the previous call's contents is used
+  TKM_TRY(coef_device(p, col, coef, st));
+  predict_kernel<<<(unsigned)ceil_div(n_new, PQ), 128, 0, st>>>(
+      (const double*)X_train, ldx, s->m > 0 ? s->d_landmark_idx.as<int64_t>() : nullptr, (int)ncoef,
+      (const double*)X_new, ldxn, (int)n_new, (int)pdim, -1.0 / (2.0 * sigma * sigma), coef,
+      p->beta0.as<double>() + col, (double*)f_out, label_out);
+  TKM_LAUNCH_CHECK();
+  return TKM_OK;   // asynchronous: nothing to free, so no synchronisation
+}

@@ -38,6 +38,13 @@ def test_library_exports_every_declared_symbol(tkm):
     assert tkm.tkm_version() == 1
 
 
+def test_no_alloc_limit_of_the_binding_is_the_header_constant(tkm):
+    from paper_2606_06742_b200.api import PREDICT_NOALLOC_MAX_COEF
+    txt = open(os.path.join(ROOT, "include", "tkm.h")).read()
+    m = re.search(r"#define\s+TKM_PREDICT_NOALLOC_MAX_COEF\s+(\d+)", txt)
+    assert m and int(m.group(1)) == PREDICT_NOALLOC_MAX_COEF == 65536
+
+
 def test_sass_has_fp64_tensor_core_and_tma_instructions(tkm):
     import subprocess
     out = subprocess.run(["cuobjdump", "-sass", tkm.lib_path()], capture_output=True, text=True).stdout
