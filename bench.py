@@ -102,6 +102,8 @@ class ClockSampler:
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
+    PERIOD_MS = 200    # --clock-period-ms; 0 = no sampler (experiments only: the line then has no clocks evidence)
+
     def __init__(self, index):
         self.index, self.proc, self.lines, self.t0 = index, None, [], 0.0
 
@@ -113,9 +115,11 @@ class ClockSampler:
         self.t0 = time.monotonic()
 
     def start(self):
+        if self.PERIOD_MS <= 0:
+            return
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                          "--format=csv,noheader,nounits", "-lms", str(int(self.PERIOD_MS))],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
@@ -541,6 +545,42 @@ def run_gemm_probe(args):
                       "tf32x3_contract_peak_tflops": pk["bf16_sus"] * NOMINAL_RATIO["f32"], "shapes": rows}))
 
 
+def run_setup_probe(args):
+    """`--workload setup_probe`: wall time of the spectral set-up alone on configs[1]'s five Gram matrices, call by
+    call (`--probe-iters` calls each): all five at once (tkm_spectral_setup_multi), one after the other
+    (tkm_spectral_setup x 5), a single one through the multi entry, and -- as a library yardstick, never on the
+    product path -- torch.linalg.eigh x 5.  The spread of the per-call times is the point (profiles/r02_host_stalls.md)."""
+    import torch
+    import paper_2606_06742_b200 as tkm
+    tkm.lib()
+    torch.cuda.set_device(0)
+    w = wl.config1(seed=1001)
+    X = torch.from_numpy(w.X).cuda()
+
+    def timed(fn, G):
+        Ks = tkm.tkm_gram_multi(X, w.sigmas[:G])
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        out = fn(Ks)
+        torch.cuda.synchronize()
+        dt = (time.perf_counter() - t0) * 1e3
+        for o in out:
+            if hasattr(o, "close"):
+                o.close()
+        return dt
+
+    cases = [("setup_multi_5", lambda Ks: tkm.tkm_spectral_setup_multi(Ks), 5),
+             ("setup_single_x5", lambda Ks: [tkm.tkm_spectral_setup(K) for K in Ks], 5),
+             ("setup_multi_1", lambda Ks: tkm.tkm_spectral_setup_multi(Ks), 1),
+             ("torch_linalg_eigh_x5", lambda Ks: [torch.linalg.eigh(K) for K in Ks], 5)]
+    out = {"workload": "setup_probe", "n": w.n, "calls": args.probe_iters, "unit": "ms of wall time per call"}
+    for name, fn, G in cases:
+        timed(fn, G)
+        ts = [timed(fn, G) for _ in range(args.probe_iters)]
+        out[name] = {"median": float(np.median(ts)), "min": min(ts), "max": max(ts), "each": [round(t, 1) for t in ts]}
+    print(json.dumps(out))
+
+
 def run_single(args):
     """`--workload` other than config1: one GPU, one problem, one JSON line."""
     import torch
@@ -697,8 +737,10 @@ def run_ours(args, w, rank, world):
     sampler.mark()
     tkm.tkm_launch_count_reset()
     s_ev = ev()
+    step_marks = [s_ev]
     for _ in range(args.steps):
         _, pr = step_device(True)
+        step_marks.append(ev())
         for k in ("ms", "flops", "launches"):
             prof[k] += pr[k]
         prof["col_iters"] += pr["col_iters"]
@@ -754,6 +796,7 @@ def run_ours(args, w, rank, world):
             "stages_ms_per_step": {"gram": stage[0] / args.steps, "eig_setup": stage[1] / args.steps,
                                    "sweep": stage[2] / args.steps, "exact_cv": stage[3] / args.steps},
             "ms_per_step_outside_stages": ms_per_step - stage_sum,
+            "ms_of_each_step": [round(a.elapsed_time(b), 2) for a, b in zip(step_marks[:-1], step_marks[1:])],
             "exact_cv_ms_per_grid": stage[3] / args.steps / len(w.sigmas),
             "fits_per_s_sweep_only": args.steps * fits_per_step / sweep_s,
             "col_iters_per_step": prof["col_iters"] / args.steps,
@@ -802,7 +845,7 @@ def main():
     ap.add_argument("--dtype", default="f64", choices=["f64"])
     ap.add_argument("--workload", default="config1",
                     choices=["config1", "config2", "config3", "config4", "nystrom_covtype", "nystrom_mnist8m46",
-                             "loo_config1", "narrow_config2", "narrow_config3", "gemm_probe"],
+                             "loo_config1", "narrow_config2", "narrow_config3", "gemm_probe", "setup_probe"],
                     help="config1 = BASELINE.json's metric configuration (the bench line, which also carries configs[3] "
                          "as `large_config`); the others are single-GPU measurements of one problem "
                          "(use --steps 1 --warmup 0 or 1: a pass takes seconds to a minute)")
@@ -816,13 +859,18 @@ def main():
     ap.add_argument("--loo-lambdas", type=int, default=0, help="loo_config1: use this many lambdas of the grid (0 = all 50)")
     ap.add_argument("--probe-iters", type=int, default=20, help="gemm_probe: launches per shape")
     ap.add_argument("--profile-all", action="store_true", help="time every contraction launch (profile = 2)")
+    ap.add_argument("--clock-period-ms", type=int, default=200,
+                    help="nvidia-smi sampling period of the clocks evidence; 0 = no sampler (experiments only)")
     ap.add_argument("--no-large", action="store_true", help="default line: skip the configs[3] pass (`large_config`)")
     args = ap.parse_args()
+    ClockSampler.PERIOD_MS = args.clock_period_ms
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if args.workload != "config1":
         if args.impl != "ours" or world != 1 or args.gpus != 1:
             raise SystemExit("--workload %s: one GPU, --impl ours only" % args.workload)
+        if args.workload == "setup_probe":
+            return run_setup_probe(args)
         return run_gemm_probe(args) if args.workload == "gemm_probe" else run_single(args)
     if args.tf32_delta >= 0:
         global TF32_DELTA

@@ -52,6 +52,22 @@ cudaMemPool_t lib_pool() {
   return pools[dev];
 }
 
+cudaStream_t lib_worker_stream(int i) {
+  static std::mutex mu;
+  static cudaStream_t streams[64][64] = {};
+  int dev = 0;
+  if (i < 0 || i >= 64 || cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) {
+    cudaGetLastError();
+    return nullptr;
+  }
+  std::lock_guard<std::mutex> lock(mu);
+  if (!streams[dev][i] && cudaStreamCreateWithFlags(&streams[dev][i], cudaStreamNonBlocking) != cudaSuccess) {
+    cudaGetLastError();
+    streams[dev][i] = nullptr;
+  }
+  return streams[dev][i];
+}
+
 int device_check() {
   int dev = -1;
   cudaError_t e = cudaGetDevice(&dev);

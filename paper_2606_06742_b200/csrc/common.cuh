@@ -5,6 +5,7 @@
 #include <nvtx3/nvToolsExt.h>
 #include <cstdarg>
 #include <cstdint>
+#include <cstdlib>
 #include <cstdio>
 #include <cstring>
 #include <atomic>
@@ -61,12 +62,26 @@ inline int64_t ceil_div(int64_t x, int64_t m) { return (x + m - 1) / m; }
 // handed to the next without a trip through the driver's page tables.  NULL on failure.
 cudaMemPool_t lib_pool();
 
-// RAII device buffer (cudaMalloc / cudaFree); zero-initialised on request.  `pooled` buffers are stream-ordered
-// (cudaMallocAsync / cudaFreeAsync on the allocating stream): for temporaries that only that stream touches.
+// Worker stream `i` (0..63) of the current device: non-blocking streams the library creates once per device and keeps
+// (tkm_spectral_setup_multi runs its G decompositions on them).  NULL on failure.
+cudaStream_t lib_worker_stream(int i);
+
+// RAII device buffer, zero-initialised on request.  All memory comes from the library's pool (lib_pool), so that
+// after the first step no allocation or free goes through the kernel-mode driver (on shared boxes those calls stall
+// for 0.3-0.8 s at random: profiles/r02_host_stalls.md).  Two lifetimes:
+//   pool = true  : a temporary of ONE stream -- stream-ordered cudaFreeAsync on the allocating stream;
+//   pool = false : memory of a handle (tkm_spectral, tkm_path) or of a call that synchronises before it returns --
+//                  released at an arbitrary later time from an arbitrary thread, so release() first waits for the
+//                  device (what cudaFree does implicitly) and then returns the block to the pool.  The memory is
+//                  valid in stream order of the allocating stream `st`: other streams must depend on `st` (they do:
+//                  every producer of a handle runs on the call's stream or waits for an event recorded on it).
+// Without a pool (cudaMemPoolCreate failed) it falls back to cudaMalloc / cudaFree.
 struct DevBuf {
   void* p = nullptr;
   size_t bytes = 0;
-  bool pooled = false;
+  bool pooled = false;       // stream-ordered temporary
+  bool from_pool = false;    // handle lifetime, but allocated from the pool
+  int dev = -1;
   cudaStream_t pool_st = nullptr;
   DevBuf() = default;
   DevBuf(const DevBuf&) = delete;
@@ -74,29 +89,41 @@ struct DevBuf {
   ~DevBuf() { release(); }
   void release() {
     if (p) {
-      if (pooled)
+      if (pooled) {
         cudaFreeAsync(p, pool_st);
-      else
+      } else if (from_pool) {
+        int cur = -1;
+        cudaGetDevice(&cur);
+        if (cur != dev && dev >= 0) cudaSetDevice(dev);
+        cudaDeviceSynchronize();
+        if (cudaFreeAsync(p, (cudaStream_t)0) != cudaSuccess) cudaGetLastError();
+        if (cur != dev && cur >= 0) cudaSetDevice(cur);
+      } else {
         cudaFree(p);
+      }
     }
     p = nullptr;
     bytes = 0;
-    pooled = false;
+    pooled = from_pool = false;
   }
   int alloc(size_t nbytes, bool zero, cudaStream_t st, bool pool = false) {
     release();
     if (nbytes == 0) nbytes = 16;
-    cudaMemPool_t mp = pool ? lib_pool() : nullptr;
-    cudaError_t e = pool ? (mp ? cudaMallocFromPoolAsync(&p, nbytes, mp, st) : cudaMallocAsync(&p, nbytes, st))
-                         : cudaMalloc(&p, nbytes);
+    cudaMemPool_t mp = lib_pool();
+    cudaError_t e;
+    if (pool)
+      e = mp ? cudaMallocFromPoolAsync(&p, nbytes, mp, st) : cudaMallocAsync(&p, nbytes, st);
+    else
+      e = mp ? cudaMallocFromPoolAsync(&p, nbytes, mp, st) : cudaMalloc(&p, nbytes);
     if (e != cudaSuccess) {
       p = nullptr;
-      return set_error(TKM_ENOMEM, "%s(%zu bytes) failed: %s", pool ? "cudaMallocFromPoolAsync" : "cudaMalloc", nbytes,
-                       cudaGetErrorString(e));
+      return set_error(TKM_ENOMEM, "device allocation of %zu bytes failed: %s", nbytes, cudaGetErrorString(e));
     }
     bytes = nbytes;
     pooled = pool;
+    from_pool = !pool && mp != nullptr;
     pool_st = st;
+    cudaGetDevice(&dev);
     if (zero) {
       e = cudaMemsetAsync(p, 0, nbytes, st);
       if (e != cudaSuccess) return set_error(TKM_ECUDA, "cudaMemsetAsync failed: %s", cudaGetErrorString(e));
@@ -108,10 +135,12 @@ struct DevBuf {
     p = o.p;
     bytes = o.bytes;
     pooled = o.pooled;
+    from_pool = o.from_pool;
+    dev = o.dev;
     pool_st = o.pool_st;
     o.p = nullptr;
     o.bytes = 0;
-    o.pooled = false;
+    o.pooled = o.from_pool = false;
   }
   template <class T>
   T* as() const { return reinterpret_cast<T*>(p); }

@@ -68,10 +68,24 @@ __device__ __forceinline__ void consumer_sync() {
   asm volatile("bar.sync 1, %0;\n" ::"n"(COUNT) : "memory");
 }
 
+// Fragment load from a pipeline stage: an explicit shared-space load.  The stage base is an integer-aligned
+// address, so a plain C++ dereference compiled to GENERIC loads (LD.E), whose reads of shared memory are not
+// ordered with the mbarrier.arrive that hands the stage back to the TMA producer: with a starved ring (first wave of
+// a launch on freshly mapped operands, two CTAs per SM) the refill of K-tile kt + STAGES landed before the last
+// loads of K-tile kt had read the stage -- four elements of one fragment row wrong in a few hundred outputs per launch
+// (found at n = 581 012 in the streamed Nystrom set-up; profiles/r02_host_stalls.md, second part).  LDS goes
+// through the same in-order shared-memory pipe as the arrive; `volatile` keeps the loads between the wait and the
+// arrive in program order.
+__device__ __forceinline__ double lds_f64(uint32_t saddr) {
+  double v;
+  asm volatile("ld.shared.f64 %0, [%1];\n" : "=d"(v) : "r"(saddr));
+  return v;
+}
+
 // K loop of one consumer warp with exactly NV live 8-row sub-tiles (compile time).
 template <class Cfg, int NV>
-__device__ __forceinline__ void gemm_k_body(double (&acc)[Cfg::TN][Cfg::TM][2], const uint8_t* p_base,
-                                            const uint8_t* q_base, const uint32_t (&off)[4], uint64_t* full_bar,
+__device__ __forceinline__ void gemm_k_body(double (&acc)[Cfg::TN][Cfg::TM][2], uint32_t p_base,
+                                            uint32_t q_base, const uint32_t (&off)[4], uint64_t* full_bar,
                                             uint64_t* empty_bar, int KT, int lane) {
   constexpr int TM = Cfg::TM, STAGES = Cfg::STAGES;
   // with one or two accumulator tiles per warp the four MMAs of a stage would form one dependent chain:
@@ -82,19 +96,27 @@ __device__ __forceinline__ void gemm_k_body(double (&acc)[Cfg::TN][Cfg::TM][2], 
   for (int i = 0; i < (SPLIT ? NV : 1); ++i)
 #pragma unroll
     for (int j = 0; j < TM; ++j) acc2[i][j][0] = acc2[i][j][1] = 0.0;
-  int s = 0;
+  // A stage is handed back to the producer ONE K-tile late, after the wait for the next tile: every MMA of the
+  // finished tile has then issued, so its fragment loads have returned.  Arriving right after the loads were ISSUED
+  // is not enough -- nothing orders an in-flight LDS before a later mbarrier.arrive of the same warp, and with a
+  // starved ring the TMA refill of K-tile kt + STAGES overtook the last loads of K-tile kt (see lds_f64).
+  int s = 0, s_prev = 0;
   uint32_t phase = 0;
   for (int kt = 0; kt < KT; ++kt) {
     mbar_wait(&full_bar[s], phase);
-    const uint8_t* ps = p_base + (size_t)s * Cfg::STAGE_BYTES;
-    const uint8_t* qs = q_base + (size_t)s * Cfg::STAGE_BYTES;
+    if (kt > 0) {
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&empty_bar[s_prev]);
+    }
+    const uint32_t ps = p_base + (uint32_t)s * Cfg::STAGE_BYTES;   // shared-space byte addresses
+    const uint32_t qs = q_base + (uint32_t)s * Cfg::STAGE_BYTES;
 #pragma unroll
     for (int ks = 0; ks < 4; ++ks) {
       double a[NV], b[TM];
 #pragma unroll
-      for (int j = 0; j < TM; ++j) b[j] = *reinterpret_cast<const double*>(qs + j * 8 * GEMM_ROW_BYTES + off[ks]);
+      for (int j = 0; j < TM; ++j) b[j] = lds_f64(qs + j * 8 * GEMM_ROW_BYTES + off[ks]);
 #pragma unroll
-      for (int i = 0; i < NV; ++i) a[i] = *reinterpret_cast<const double*>(ps + i * 8 * GEMM_ROW_BYTES + off[ks]);
+      for (int i = 0; i < NV; ++i) a[i] = lds_f64(ps + i * 8 * GEMM_ROW_BYTES + off[ks]);
 #pragma unroll
       for (int i = 0; i < NV; ++i)
 #pragma unroll
@@ -105,13 +127,12 @@ __device__ __forceinline__ void gemm_k_body(double (&acc)[Cfg::TN][Cfg::TM][2], 
             dmma_884(acc[i][j][0], acc[i][j][1], a[i], b[j]);
         }
     }
-    __syncwarp();
-    if (lane == 0) mbar_arrive(&empty_bar[s]);
+    s_prev = s;
     if (++s == STAGES) {
       s = 0;
       phase ^= 1;
     }
-  }
+  }   // the last tile's stage is never refilled: no release needed
   if (SPLIT) {
 #pragma unroll
     for (int i = 0; i < NV; ++i)
@@ -137,8 +158,8 @@ __device__ __forceinline__ void gemm_k_idle(uint64_t* full_bar, uint64_t* empty_
   }
 }
 template <class Cfg, int NV>
-__device__ __forceinline__ void gemm_k_loop(int nv, double (&acc)[Cfg::TN][Cfg::TM][2], const uint8_t* p_base,
-                                            const uint8_t* q_base, const uint32_t (&off)[4], uint64_t* full_bar,
+__device__ __forceinline__ void gemm_k_loop(int nv, double (&acc)[Cfg::TN][Cfg::TM][2], uint32_t p_base,
+                                            uint32_t q_base, const uint32_t (&off)[4], uint64_t* full_bar,
                                             uint64_t* empty_bar, int KT, int lane) {
   if constexpr (NV == 0) {
     gemm_k_idle<Cfg>(full_bar, empty_bar, KT, lane);
@@ -225,8 +246,8 @@ __global__ void __launch_bounds__(Cfg::THREADS)
 
   // The K loop is instantiated once per possible number of live sub-tiles so that every MMA and every
   // fragment load is unconditional (a ragged last N tile costs only the sub-tiles it has).
-  const uint8_t* p_base = tiles + p_row;
-  const uint8_t* q_base = tiles + q_row;
+  const uint32_t p_base = smem_u32(tiles) + p_row;
+  const uint32_t q_base = smem_u32(tiles) + q_row;
   gemm_k_loop<Cfg, TN>(nv, acc, p_base, q_base, off, full_bar, empty_bar, KT, lane);
 
   epi.template run<Cfg>(acc, n_blk0, m_blk0, warp_n, warp_m, lane, N, g.M, grp, scratch);

@@ -79,6 +79,7 @@ struct Tf32Args {
   uint32_t* flags;
   uint32_t epoch;
   int min_range;   // smallest range of a pair in K-tiles (tf32_min_range, or the TKM_SK_MINRANGE tuning override)
+  int terms;       // 3: lo*hi + hi*lo + hi*hi (the product); 1: hi*hi only (TKM_TF32_TERMS=1, precision experiments)
   unsigned long long* dbg;   // tuning aid (TKM_SK_DEBUG): clock64 stamps of pair 0 [0..] MMA full-wait done, [4096..] producer issue
 };
 
@@ -276,7 +277,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(TF32_THREADS, 1)
           const uint32_t acc0 = kt == sg.k0 ? 0u : 1u;
           if (elect_one()) {
             if (g.dbg && pair == 0 && kt - sg.k0 < 2048) g.dbg[kt - sg.k0] = clock64();
-            if (!two) {
+            if (g.terms == 1) {
+#pragma unroll
+              for (int k = 0; k < 4; ++k) {
+                const uint64_t o = (uint64_t)(k * 2);
+                umma_tf32_pair(tmem_base, a_hi + o, b_hi + o, idesc0, k == 0 ? acc0 : 1u);
+                if (two) umma_tf32_pair(tmem_base + 256, a_hi + o, b_hi + b1_off + o, idesc1, k == 0 ? acc0 : 1u);
+              }
+            } else if (!two) {
 #pragma unroll
               for (int k = 0; k < 4; ++k) {
                 const uint64_t o = (uint64_t)(k * 2);   // 8 floats = 32 B, in units of 16 B
@@ -469,6 +477,8 @@ int gemm_tf32_launch(Tf32Args a, int G, Tf32Scratch& sc, const Epi& epi, cudaStr
   a.epoch = ++sc.epoch;
   const int64_t units = (int64_t)G * ceil_div(a.M, 2 * TF32_BM) * ceil_div(std::max(a.N, 1), TF32_BN) * ceil_div(a.K, TF32_BK);
   a.dbg = sc.dbg.p ? sc.dbg.as<unsigned long long>() : nullptr;
+  const char* tm = getenv("TKM_TF32_TERMS");
+  a.terms = tm && *tm == '1' ? 1 : 3;
   const char* mr = getenv("TKM_SK_MINRANGE");
   a.min_range = mr && *mr ? std::max(1, atoi(mr)) : tf32_min_range((int)ceil_div(a.K, TF32_BK));
   const int pairs = (int)std::max<int64_t>(1, std::min<int64_t>(TF32_MAX_PAIRS, units / a.min_range));

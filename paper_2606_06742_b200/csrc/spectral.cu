@@ -8,6 +8,8 @@
 
 #include <algorithm>
 #include <cmath>
+#include <condition_variable>
+#include <functional>
 #include <mutex>
 #include <new>
 #include <string>
@@ -83,7 +85,21 @@ struct Solver {
     static std::vector<cusolverDnHandle_t> p;
     return p;
   }
+  // a persistent set-up worker (below) keeps one handle of its own: the handle then always sees the same thread
+  // and the same stream
+  static cusolverDnHandle_t& thread_handle() {
+    static thread_local cusolverDnHandle_t h = nullptr;
+    return h;
+  }
+  static bool& thread_keeps_handle() {
+    static thread_local bool k = false;
+    return k;
+  }
   int acquire() {
+    if (thread_keeps_handle() && thread_handle()) {
+      h = thread_handle();
+      return TKM_OK;
+    }
     {
       std::lock_guard<std::mutex> lk(mu());
       if (!pool().empty()) {
@@ -100,6 +116,10 @@ struct Solver {
   }
   ~Solver() {
     if (!h) return;
+    if (thread_keeps_handle()) {
+      thread_handle() = h;
+      return;
+    }
     std::lock_guard<std::mutex> lk(mu());
     if (pool().size() < 16)
       pool().push_back(h);
@@ -118,17 +138,13 @@ static int syevd_inplace(double* A, int64_t lda, int64_t n, double* W, cudaStrea
   cusolverStatus_t cs = cusolverDnDsyevd_bufferSize(sv.h, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER,
                                                     (int)n, A, (int)lda, W, &lwork);
   if (cs != CUSOLVER_STATUS_SUCCESS) return set_error(TKM_ESOLVER, "Dsyevd_bufferSize failed (%d)", (int)cs);
-  // stream-ordered temporaries: cudaFree would synchronise the whole device and stall the other setups of a
-  // tkm_spectral_setup_multi call that run concurrently on their own streams
-  struct AsyncBuf {
-    void* p = nullptr;
-    cudaStream_t st;
-    ~AsyncBuf() {
-      if (p) cudaFreeAsync(p, st);
-    }
-  } work{nullptr, st}, info{nullptr, st};
-  TKM_CUDA(cudaMallocAsync(&work.p, (size_t)std::max(lwork, 1) * sizeof(double), st));
-  TKM_CUDA(cudaMallocAsync(&info.p, sizeof(int), st));
+  // stream-ordered temporaries from the library's pool (64 MB of workspace at n = 2000): cudaFree would synchronise
+  // the whole device and stall the other setups of a tkm_spectral_setup_multi call, and the device's DEFAULT pool
+  // (release threshold 0) hands its memory back to the driver at every synchronisation -- a kernel-mode allocation
+  // per decomposition per step, which on shared boxes stalled for 0.1-1.6 s at random (profiles/r02_host_stalls.md)
+  DevBuf work, info;
+  TKM_TRY(work.alloc((size_t)std::max(lwork, 1) * sizeof(double), false, st, true));
+  TKM_TRY(info.alloc(sizeof(int), false, st, true));
   TKM_CUDA(cudaMemsetAsync(info.p, 0, sizeof(int), st));
   cs = cusolverDnDsyevd(sv.h, CUSOLVER_EIG_MODE_VECTOR, CUBLAS_FILL_MODE_LOWER, (int)n, A, (int)lda, W,
                         (double*)work.p, lwork, (int*)info.p);
@@ -406,6 +422,66 @@ extern "C" int tkm_spectral_setup_nystrom_x(const void* X, int64_t n, int64_t p,
   return TKM_OK;
 }
 
+namespace tkm {
+// Persistent set-up workers: one host thread per (device, index), created on first use and kept for the life of the
+// process, each with its own non-blocking stream and its own cuSOLVER handle.  Starting a thread per decomposition
+// and binding it to the device cost nothing on average but stalled for 0.1-1 s in one call out of five on shared
+// boxes (profiles/r02_host_stalls.md); a parked thread that is woken by a condition variable does not.
+class SetupWorker {
+ public:
+  SetupWorker(int dev, int idx) : dev_(dev), idx_(idx) {
+    std::thread([this] { run(); }).detach();
+  }
+  void submit(std::function<void(cudaStream_t)> f) {
+    std::lock_guard<std::mutex> lk(mu_);
+    job_ = std::move(f);
+    state_ = 1;
+    cv_.notify_all();
+  }
+  void wait() {
+    std::unique_lock<std::mutex> lk(mu_);
+    cv_.wait(lk, [&] { return state_ == 0; });
+  }
+
+ private:
+  void run() {
+    Solver::thread_keeps_handle() = true;
+    bool ok = cudaSetDevice(dev_) == cudaSuccess;
+    cudaStream_t st = ok ? lib_worker_stream(idx_) : nullptr;
+    for (;;) {
+      std::unique_lock<std::mutex> lk(mu_);
+      cv_.wait(lk, [&] { return state_ == 1; });
+      std::function<void(cudaStream_t)> f = std::move(job_);
+      lk.unlock();
+      f(st);   // st == NULL: the job reports the failure
+      lk.lock();
+      state_ = 0;
+      cv_.notify_all();
+    }
+  }
+  int dev_, idx_;
+  std::mutex mu_;
+  std::condition_variable cv_;
+  std::function<void(cudaStream_t)> job_;
+  int state_ = 0;   // 0 idle, 1 job pending or running
+};
+
+// the workers of the current device (never destroyed: their threads are parked in run()); `call_mu` serialises
+// concurrent tkm_spectral_setup_multi calls on one device
+struct SetupWorkers {
+  std::mutex call_mu;
+  SetupWorker* w[64] = {};
+};
+static SetupWorkers* setup_workers(int dev) {
+  static std::mutex mu;
+  static SetupWorkers* per_dev[64] = {};
+  if (dev < 0 || dev >= 64) return nullptr;
+  std::lock_guard<std::mutex> lk(mu);
+  if (!per_dev[dev]) per_dev[dev] = new (std::nothrow) SetupWorkers();
+  return per_dev[dev];
+}
+}  // namespace tkm
+
 // G full-kernel setups side by side: a dense symmetric eigensolver spends much of its time in phases that
 // cannot fill the device (panel factorisations, the divide-and-conquer merge tree), so G decompositions
 // on G streams, driven by G host threads, overlap almost perfectly.
@@ -441,22 +517,34 @@ extern "C" int tkm_spectral_setup_multi(const void* const* Ks, int32_t G, int64_
     }
   }
   cudaEventRecord(ready, st);   // K ready and the zero fills of the new buffers done
-  std::vector<std::thread> th;
-  for (int g = 0; g < G; ++g)
-    th.emplace_back([&, g] {
-      cudaStream_t s2 = nullptr;
-      if (cudaSetDevice(dev) != cudaSuccess || cudaStreamCreateWithFlags(&s2, cudaStreamNonBlocking) != cudaSuccess) {
-        rc[g] = TKM_ECUDA;
-        msg[g] = "tkm_spectral_setup_multi: could not create a stream";
-        return;
-      }
-      cudaStreamWaitEvent(s2, ready, 0);
-      rc[g] = compute_full((const double*)Ks[g], n, ldk, out[g], s2);   // synchronises s2
-      if (rc[g] != TKM_OK) msg[g] = err_buf();
-      launches[g] = launch_counter();
-      cudaStreamDestroy(s2);
-    });
-  for (auto& t : th) t.join();
+  SetupWorkers* sw = setup_workers(dev);
+  if (!sw) {
+    cudaEventDestroy(ready);
+    for (int g = 0; g < G; ++g) {
+      delete out[g];
+      out[g] = nullptr;
+    }
+    return set_error(TKM_ECUDA, "tkm_spectral_setup_multi: device ordinal %d outside 0..63", dev);
+  }
+  {
+    std::lock_guard<std::mutex> call_lock(sw->call_mu);
+    for (int g = 0; g < G; ++g) {
+      if (!sw->w[g]) sw->w[g] = new SetupWorker(dev, g);
+      sw->w[g]->submit([&, g](cudaStream_t s2) {
+        if (!s2) {
+          rc[g] = TKM_ECUDA;
+          msg[g] = "tkm_spectral_setup_multi: could not create a stream";
+          return;
+        }
+        const int64_t before = launch_counter();
+        cudaStreamWaitEvent(s2, ready, 0);
+        rc[g] = compute_full((const double*)Ks[g], n, ldk, out[g], s2);   // synchronises s2
+        if (rc[g] != TKM_OK) msg[g] = err_buf();
+        launches[g] = launch_counter() - before;
+      });
+    }
+    for (int g = 0; g < G; ++g) sw->w[g]->wait();
+  }
   cudaEventDestroy(ready);
   int bad = TKM_OK;
   for (int g = 0; g < G; ++g) {

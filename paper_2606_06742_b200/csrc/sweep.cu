@@ -1003,8 +1003,10 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
   memset(&targs, 0, sizeof(targs));
   memset(&targsF, 0, sizeof(targsF));
   int tcfg = -1;
-  PinBuf h_ns;   // [POLL_RING][GEMM_MAX_GROUPS] live-slot counts read back after every compaction
-  TKM_TRY(h_ns.alloc((size_t)POLL_RING * GEMM_MAX_GROUPS * sizeof(int32_t)));
+  // [POLL_RING][GEMM_MAX_GROUPS] live-slot counts read back after every compaction; pinned once per host thread and
+  // kept (cudaMallocHost is a kernel-mode call: none of those in a warm step, see DevBuf)
+  static thread_local PinBuf h_ns;
+  if (!h_ns.p) TKM_TRY(h_ns.alloc((size_t)POLL_RING * GEMM_MAX_GROUPS * sizeof(int32_t)));
 
   // events: one "poll landed" event per ring entry; optional GEMM sampling events per ring entry
   const int check_every = opts->check_every > 0 ? opts->check_every : 16;

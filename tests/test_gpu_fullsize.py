@@ -150,6 +150,14 @@ def _nystrom_first_order(tkm, w, streamed):
     else:
         spec = tkm.tkm_spectral_setup(nystrom=(K_nm, K_mm, idx))
     assert spec.n == w.n and 0 < spec.r <= w.m_landmarks
+    # U has orthonormal columns (a pipeline race in the FP64 GEMM once left a few hundred wrong entries in the
+    # first row block of Phi at this size: 2e-5 here; fixed)
+    U = spec.U()
+    orth = float((U.T @ U - torch.eye(spec.r, device="cuda", dtype=torch.float64)).abs().max())
+    del U
+    torch.cuda.empty_cache()
+    print("nystrom n=%d: max |U^T U - I| = %.2e" % (w.n, orth))
+    assert orth < 1e-8
     path = tkm.tkm_fit_path(spec, y, w.loss, w.lambdas, foldid, w.V, TOL, MAXIT, smooth0=w.smooth0, eta=w.eta,
                             rounds=w.rounds, warm_tol=WARM_TOL, tf32_delta=2)    # both contractions in delta form
     info = path.info()

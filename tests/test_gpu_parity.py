@@ -759,3 +759,31 @@ def test_thin_u_long_contraction_ksplit_parity(tkm, mode):
     cv = tkm.tkm_exact_cv(path, y, foldid, 1, w.L, w.V)
     cv_o = o.exact_cv(spec_o, res, w.y, foldid, w.loss)
     assert np.max(np.abs(cv[0] - cv_o[0])) <= CV_TOL and np.array_equal(cv[1], cv_o[1]) and np.array_equal(cv[3], cv_o[3])
+
+
+def test_dmma_gemm_is_exact_on_freshly_mapped_operands(tkm):
+    """Regression for a pipeline race of gemm_f64_tma_kernel: the consumer warps handed a stage back to the TMA
+    producer right after ISSUING their fragment loads, and with a starved ring (first wave of a launch whose Q operand
+    is freshly mapped memory, two CTAs per SM) the refill overtook the last loads -- four elements of one fragment
+    row came from K-tile kt + STAGES.  Integer-valued operands make every product and sum exact in FP64, so the
+    result must EQUAL the reference; P[n][l] = (l // 16)^2 + 1000 n tells a stale K-tile or row apart."""
+    import torch
+    from paper_2606_06742_b200.api import lib, _check
+    N, M, K, ldd = 2048, 32768, 2048, 32768 + 64
+    l = torch.arange(K, device="cuda", dtype=torch.float64)
+    P = ((l // 16) ** 2).repeat(N, 1).contiguous() + torch.arange(N, device="cuda", dtype=torch.float64)[:, None] * 1000.0
+    Q0 = torch.ones((M, K), device="cuda", dtype=torch.float64)
+    Q0[:, ::7] = 2.0
+    ref = P @ Q0.T
+    for rep in range(6):
+        # a new allocation for Q and the output on every repetition (the caching allocator is emptied first)
+        torch.cuda.empty_cache()
+        D = torch.empty((N, ldd), device="cuda", dtype=torch.float64)
+        Q = torch.empty((M + 64 * (rep + 1), K), device="cuda", dtype=torch.float64)[:M]
+        Q.copy_(Q0)
+        torch.cuda.synchronize()
+        _check(lib().tkm_dgemm_nt(P.data_ptr(), K, Q.data_ptr(), Q.stride(0), D.data_ptr(), ldd, N, M, K, None))
+        torch.cuda.synchronize()
+        wrong = int((D[:, :M] != ref).sum())
+        assert wrong == 0, "repetition %d: %d wrong elements" % (rep, wrong)
+        del D, Q
