@@ -13,7 +13,8 @@ and S10 coefficients in the e2e leg.  `value` = columns fitted per second by the
 and y resident in HBM before the timed region; `fits_per_s_sweep_only` = SURVEY.md 8(d)'s B / t_sweep; `e2e` =
 the same through tkm_train_tune_host from pinned HOST buffers.  The same JSON line carries `large_config`: one
 pass of BASELINE.json configs[3] (the largest full-kernel single-GPU configuration, n = 20000, 900 columns) with
-its own stage times, roofline and clocks (outside the timed region of `value`; `--no-large` skips it).
+its own stage times, roofline and clocks (outside the timed region of `value`; `--no-large` skips it), and
+`single_tf32_increments` (tf32_delta = 3: one step of the same workload with single-TF32 increment products).
 
 Other workloads (`--workload`, one GPU, one JSON line each with the same keys):
   config2 | config3 | config4      BASELINE.json configs[2..4] at full size
@@ -291,7 +292,7 @@ def library_probes(tkm):
 L2_BYTES = 126e6     # B200 L2 (B200_PROFILING.md): a U operand set larger than this streams from HBM every launch
 
 
-def family_rooflines(prof, tp, traffic, probes=None, geom=None, hbm_peak=None, tkeys=None):
+def family_rooflines(prof, tp, traffic, probes=None, geom=None, hbm_peak=None, tkeys=None, single_tf32=False):
     """One roofline object per kernel family with sampled launches.  prof: dict(ms, flops, launches) arrays of 4.
     geom = (n, r, G): with it every object also carries the HBM side of the same launches (`hbm`: algorithmic bytes
     = G n r 8 for the U operand of the G groups + live (n + r) 8 for the moving operand and the result, over the
@@ -306,20 +307,24 @@ def family_rooflines(prof, tp, traffic, probes=None, geom=None, hbm_peak=None, t
         ms, fl = float(prof["ms"][i]), float(prof["flops"][i])
         ach = (fl / 1e12) / (ms / 1e3) if ms > 0 else 0.0
         f64 = i < 2
-        peak = tp["f64_contract"] if f64 else tp["tf32x3_contract"]
+        # tf32_delta = 3: one TF32 MMA per useful product and 4-byte operands (hi parts only)
+        peak = tp["f64_contract"] if f64 else tp["tf32x3_contract"] * (3.0 if single_tf32 else 1.0)
         tr = traffic.get((tkeys or {}).get(i, "fam%d" % i))
-        d = {"bound": "tensor", "kernel": FAMILY[i], "achieved": ach, "peak": peak, "unit": "TFLOP/s",
+        d = {"bound": "tensor", "kernel": FAMILY[i].replace("3xTF32", "1xTF32") if single_tf32 else FAMILY[i],
+             "achieved": ach, "peak": peak, "unit": "TFLOP/s",
              "frac": ach / peak, "traffic": tr[0] if tr else None, "traffic_source": tr[1] if tr else None,
              "peak_source": tp["src"] + (" x nominal f64/bf16 ratio %.4f" % NOMINAL_RATIO["f64"] if f64 else
-                                         " x nominal tf32/bf16 ratio 0.5 / 3 MMAs per useful product"),
-             "sampled_launches": nl, "avg_launch_ms": ms / nl, "avg_flops_per_launch": fl / nl, "sampled_ms": ms}
+                                         (" x nominal tf32/bf16 ratio 0.5 (one MMA per useful product)" if single_tf32 else
+                                          " x nominal tf32/bf16 ratio 0.5 / 3 MMAs per useful product")),
+             "sampled_launches": nl, "avg_launch_ms": ms / nl, "avg_flops_per_launch": fl / nl, "sampled_ms": ms,
+             "family": i}
         if f64:
             d["peak_dmma_issue"] = tp["f64_issue"]
             d["frac_of_issue"] = ach / tp["f64_issue"]
         if geom and hbm_peak and fl > 0:
             n, r, G = geom
             live = fl / nl / (2.0 * n * r)
-            u_bytes = G * n * r * 8.0
+            u_bytes = G * n * r * (4.0 if (single_tf32 and not f64) else 8.0)
             by = u_bytes + live * (n + r) * 8.0
             gbs = by / (ms / nl / 1e3) / 1e9
             ai, ridge = fl / nl / by, peak * 1e12 / (hbm_peak * 1e9)
@@ -328,7 +333,7 @@ def family_rooflines(prof, tp, traffic, probes=None, geom=None, hbm_peak=None, t
                         "flops_per_byte": ai, "ridge_flops_per_byte": ridge}
             d["binding"] = "hbm" if (ai < ridge and u_bytes > L2_BYTES) else "tensor"
         if probes:
-            pm = probes["cublas_dgemm_tflops"] if f64 else probes["cublas_tf32_tflops"] / 3.0
+            pm = probes["cublas_dgemm_tflops"] if f64 else probes["cublas_tf32_tflops"] / (1.0 if single_tf32 else 3.0)
             d["peak_measured"] = pm
             d["frac_of_measured"] = ach / pm
             d["peak_measured_source"] = ("cuBLAS DGEMM 8192^3 on this box" if f64 else
@@ -339,7 +344,7 @@ def family_rooflines(prof, tp, traffic, probes=None, geom=None, hbm_peak=None, t
 
 def merge_families(fams, idx):
     """Sum families (e.g. DMMA GEMM-A + GEMM-B = the FP64 kernel) into one roofline object."""
-    sel = [f for f in fams if FAMILY.index(f["kernel"]) in idx]
+    sel = [f for f in fams if f["family"] in idx]
     if not sel:
         return None
     ms = sum(f["sampled_ms"] for f in sel)
@@ -384,11 +389,12 @@ def binding_side(d):
     return o
 
 
-def time_weighted(prof2, tp):
+def time_weighted(prof2, tp, single_tf32=False):
     """All launches of one sweep (profile = 2): useful flops the device counted / total kernel time, per family."""
     out = {}
     for name, idx, peak, issue in (("fp64_dmma", (0, 1), tp["f64_contract"], tp["f64_issue"]),
-                                   ("tcgen05_3xtf32", (2, 3), tp["tf32x3_contract"], None)):
+                                   ("tcgen05_1xtf32" if single_tf32 else "tcgen05_3xtf32", (2, 3),
+                                    tp["tf32x3_contract"] * (3.0 if single_tf32 else 1.0), None)):
         ms = float(sum(prof2["ms"][i] for i in idx))
         fl = float(sum(prof2["flops"][i] for i in idx))
         nl = int(sum(prof2["launches"][i] for i in idx))
@@ -459,7 +465,7 @@ def run_problem(tkm, w, *, tf32_delta, tol, warm_tol, profile=1, nystrom_streame
         raise RuntimeError("columns hit maxit: the timed work is not the stated work")
     out = dict(gram_ms=e0.elapsed_time(e1), setup_ms=e1.elapsed_time(e2), sweep_ms=e2.elapsed_time(e3),
                cv_ms=e3.elapsed_time(e4), col_iters=int(path.total_col_iters), B=path.B, r=spec.r, n=w.n,
-               prof=path.profile(), profile_mode=profile, clocks=clocks, gram_bytes=gram_bytes, best_l=[int(b) for b in cv[3]],
+               prof=path.profile(), profile_mode=profile, tf32_delta=tf32_delta, clocks=clocks, gram_bytes=gram_bytes, best_l=[int(b) for b in cv[3]],
                peak_mem_gb=torch.cuda.max_memory_allocated() / 1e9, iters_max=int(path.info()["iters"].max()))
     path.close()
     spec.close()
@@ -470,14 +476,15 @@ def run_problem(tkm, w, *, tf32_delta, tol, warm_tol, profile=1, nystrom_streame
 def problem_summary(res, pk, traffic, what, knobs, probes=None, tkeys=None):
     tp = tensor_peaks(pk, res["clocks"].get("sm_mhz"))
     n, r = res["n"], res["r"]
-    fams = family_rooflines(res["prof"], tp, traffic, probes, geom=(n, r, 1), hbm_peak=pk["hbm"], tkeys=tkeys)
+    fams = family_rooflines(res["prof"], tp, traffic, probes, geom=(n, r, 1), hbm_peak=pk["hbm"], tkeys=tkeys,
+                            single_tf32=knobs.get("tf32_delta") == 3)
     sweep_s = res["sweep_ms"] / 1e3
     total_ms = res["gram_ms"] + res["setup_ms"] + res["sweep_ms"] + res["cv_ms"]
 
     def dominance(f):
         # profile = 1 samples ONE exact and ONE delta iteration per batch, but a batch of 16 (or 32) iterations holds
         # one exact iteration and 15 (31) delta iterations: the tcgen05 families stand for 15 x their sampled time
-        return f["sampled_ms"] * (15.0 if FAMILY.index(f["kernel"]) >= 2 and res.get("profile_mode") != 2
+        return f["sampled_ms"] * (15.0 if f["family"] >= 2 and res.get("profile_mode") != 2
                                   else 1.0)
 
     d = {"workload": what, "columns": res["B"], "launch_config": knobs,
@@ -505,7 +512,8 @@ def narrow_hbm_roofline(res, pk):
         if not nl:
             continue
         live = pr["flops"][i] / nl / (2.0 * n * r)          # average live columns of the sampled launches
-        by = n * r * 8.0 + live * (r + n) * 8.0 + (live * (n if i == 2 else r) * 4.0 if i >= 2 else 0.0)
+        ub = 4.0 if (i >= 2 and res.get("tf32_delta") == 3) else 8.0   # single-TF32 mode reads the hi parts only
+        by = n * r * ub + live * (r + n) * ub + (live * (n if i == 2 else r) * 4.0 if i >= 2 else 0.0)
         ms = pr["ms"][i] / nl
         out.append({"bound": "hbm", "kernel": FAMILY[i], "achieved": by / (ms / 1e3) / 1e9, "peak": pk["hbm"],
                     "unit": "GB/s", "frac": by / (ms / 1e3) / 1e9 / pk["hbm"], "traffic": None,
@@ -640,7 +648,8 @@ def run_single(args):
         if line["roofline_hbm"]:
             line["roofline"] = max(line["roofline_hbm"], key=lambda f: f["avg_launch_ms"])
     if args.profile_all:
-        line["time_weighted"] = time_weighted(res["prof"], tensor_peaks(pk, res["clocks"].get("sm_mhz")))
+        line["time_weighted"] = time_weighted(res["prof"], tensor_peaks(pk, res["clocks"].get("sm_mhz")),
+                                              single_tf32=kw["tf32_delta"] == 3)
     line["gpu_launches"] = int(tkm.tkm_launch_count())
     print(json.dumps(line))
 
@@ -675,7 +684,7 @@ def run_ours(args, w, rank, world):
         e.record()
         return e
 
-    def step_device(collect, profile=1):
+    def step_device(collect, profile=1, mode=None):
         """One pass of the hot path: S1 + S2 per bandwidth, S3-S8 for all bandwidths as groups of one
         sweep (tkm_fit_path_multi), S9 per bandwidth."""
         flush.zero_()
@@ -686,7 +695,8 @@ def run_ours(args, w, rank, world):
         del Ks
         e2 = ev()
         paths = tkm.tkm_fit_path_multi(specs, y, w.loss, w.lambdas, foldid, w.V, tol, MAXIT, smooth0=w.smooth0,
-                                       eta=w.eta, rounds=w.rounds, warm_tol=WARM_TOL, tf32_delta=TF32_DELTA,
+                                       eta=w.eta, rounds=w.rounds, warm_tol=WARM_TOL,
+                                       tf32_delta=TF32_DELTA if mode is None else mode,
                                        profile=profile, delta_min_live=args.delta_min_live)
         e3 = ev()
         best = [int(tkm.tkm_exact_cv(path, y, foldid, w.T, w.L, w.V)[3][0]) for path in paths]
@@ -772,7 +782,8 @@ def run_ours(args, w, rank, world):
     pk, traffic = peaks(), traffic_table()
     tp = tensor_peaks(pk, clocks.get("sm_mhz") if clocks else None)
     probes = library_probes(tkm) if world == 1 else None
-    fams = family_rooflines(prof, tp, traffic, probes, geom=(w.n, w.n, len(w.sigmas)), hbm_peak=pk["hbm"])
+    fams = family_rooflines(prof, tp, traffic, probes, geom=(w.n, w.n, len(w.sigmas)), hbm_peak=pk["hbm"],
+                            single_tf32=TF32_DELTA == 3)
     # the FP64 DMMA kernel (both epilogues) and the tcgen05 kernel (both delta forms): the dominant one -- the larger
     # share of the sampled kernel time -- is `roofline`
     roof_f64, roof_tf32 = merge_families(fams, (0, 1)), merge_families(fams, (2, 3))
@@ -782,7 +793,7 @@ def run_ours(args, w, rank, world):
     if roof_tf32 is not None:
         tr = traffic.get("config1_tcgen05_full_width")
         roof_tf32["traffic"], roof_tf32["traffic_source"] = (tr[0], tr[1]) if tr else (None, None)
-    if TF32_DELTA == 2 and roof_tf32 is not None:
+    if TF32_DELTA >= 2 and roof_tf32 is not None:
         roofline, roofline_other = roof_tf32, roof_f64
     else:
         roofline, roofline_other = roof_f64, roof_tf32
@@ -813,7 +824,19 @@ def run_ours(args, w, rank, world):
         line["peaks_measured_here"] = probes
         # every launch of one more step, outside the timed region: the time-weighted fractions
         _, pr2 = step_device(True, profile=2)
-        line["roofline_time_weighted"] = time_weighted(pr2, tp)
+        line["roofline_time_weighted"] = time_weighted(pr2, tp, single_tf32=TF32_DELTA == 3)
+        if TF32_DELTA == 2:
+            # beyond BASELINE.json's "3xTF32 split": the same step with single-TF32 increment products (tf32_delta = 3,
+            # include/tkm.h) -- one warm-up and one measured step outside the timed region; NOT part of `value`
+            step_device(False, mode=3)
+            b3, pr3 = step_device(True, mode=3)
+            line["single_tf32_increments"] = {
+                "what": "tf32_delta = 3: increments contracted in one TF32 product (hi parts only: half the operand bytes, "
+                        "a third of the MMAs); FP64 state, exact restarts and stop tests unchanged, same 1e-10 parity "
+                        "tests (tests/test_gpu_parity.py); an option, not the configuration of `value`",
+                "sweep_ms": float(pr3["stage"][2]), "fits_per_s_sweep_only": fits_per_step / (float(pr3["stage"][2]) / 1e3),
+                "step_ms": float(pr3["stage"].sum()), "fits_per_s": fits_per_step / (float(pr3["stage"].sum()) / 1e3),
+                "col_iters": int(pr3["col_iters"]), "selected_lambda_index": b3}
         if not args.no_large:
             # the largest full-kernel single-GPU configuration of BASELINE.json: one pass, its own roofline and clocks
             del X, y, flush

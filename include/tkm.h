@@ -82,6 +82,11 @@ typedef struct {
                       /* the first iteration of a round and the last iteration of every batch (check_every, twice  */
                       /* that in wide batches), and only those exact iterations decide convergence.  Same fixed    */
                       /* point and tolerances as 0; DESIGN.md section 12.                                           */
+                      /* 3: as 2 with SINGLE-TF32 increment products (operands rounded to TF32, hi parts only: half  */
+                      /* the operand bytes, a third of the MMAs).  The increments then carry a relative error of     */
+                      /* 2^-11 instead of 2^-21; state, exact restarts and every convergence decision stay FP64, so   */
+                      /* the result meets the same tolerances (the trajectory, not the fixed point, is perturbed);    */
+                      /* an option beyond the "3xTF32 split" BASELINE.json names -- not the default of bench.py.     */
   double gap_tol;     /* outer control of PAPER.md:220-222 ("shrink delta ... until the KKT conditions of  */
                       /* all SVM models are satisfied"; reading G23).  <= 0: the fixed schedule of `rounds`  */
                       /* levels for every column.  > 0: after round k < rounds-1 a column whose solution     */

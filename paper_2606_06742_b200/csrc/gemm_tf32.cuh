@@ -23,7 +23,9 @@
 //
 // The number of live slots N_g of every group is read from device memory; slot tiles are padded to a multiple of
 // 64 (each CTA's half to a multiple of 32 = one TMA box); the depth of the TMA -> MMA ring follows from the widest
-// tile of the launch (2 stages at 512 slots, 5 at <= 64).
+// tile of the launch (2 stages at 512 slots, 5 at <= 64).  With Tf32Args.terms == 1 (single-TF32 products:
+// tkm_loss_opts.tf32_delta = 3) a stage holds the hi tiles only: the ring is twice as deep (4 .. 8 stages), a launch
+// streams half the bytes and the issuer sends one MMA per K-step instead of three.
 //
 // Warp roles (320 threads per CTA): warp 0 = TMA producer (its loads complete on the LEADER's full barrier),
 // warp 1 = MMA issuer (leader CTA only), warps 2..9 = epilogue (warp w owns TMEM lanes 32 (w % 4) .. +31, i.e. 32
@@ -47,7 +49,7 @@ constexpr int TF32_A_BYTES = TF32_BM * 128;
 constexpr int TF32_RED_BYTES = 4 * TF32_BN * 8;        // per-warp slot sums of a reducing epilogue
 constexpr int TF32_TILE_SMEM = 208 * 1024;             // shared memory of the TMA -> MMA ring
 constexpr size_t TF32_SMEM = TF32_TILE_SMEM + TF32_RED_BYTES + 1024;    // + alignment slack
-constexpr int TF32_MAX_STAGES = 6;
+constexpr int TF32_MAX_STAGES = 8;
 constexpr int TF32_THREADS = 320;
 constexpr int TF32_MIN_UNITS = 8;      // K-tiles below which a pair is not worth starting
 // Smallest range of a pair, in K-tiles: at least half a tile's depth (a tile then has at most two helpers, whose
@@ -79,14 +81,16 @@ struct Tf32Args {
   uint32_t* flags;
   uint32_t epoch;
   int min_range;   // smallest range of a pair in K-tiles (tf32_min_range, or the TKM_SK_MINRANGE tuning override)
-  int terms;       // 3: lo*hi + hi*lo + hi*hi (the product); 1: hi*hi only (TKM_TF32_TERMS=1, precision experiments)
+  int terms;       // 3 (or 0): lo*hi + hi*lo + hi*hi, the 3xTF32 product; 1: hi*hi only -- a single TF32 product (11-bit
+                   // operands): the lo tiles are neither loaded nor multiplied (half the bytes, a third of the MMAs)
   unsigned long long* dbg;   // tuning aid (TKM_SK_DEBUG): clock64 stamps of pair 0 [0..] MMA full-wait done, [4096..] producer issue
 };
 
 // slots of a pair tile after padding
 __host__ __device__ inline int tf32_tile_pad(int nt) { return ((nt + 63) >> 6) << 6; }
-__host__ __device__ inline int tf32_stages_of(int half_rows) {
-  const int s = TF32_TILE_SMEM / (2 * TF32_A_BYTES + half_rows * 256);
+// copies = 2: every operand as (hi, lo); 1: hi only (Tf32Args.terms == 1)
+__host__ __device__ inline int tf32_stages_of(int half_rows, int copies) {
+  const int s = TF32_TILE_SMEM / (copies * (TF32_A_BYTES + half_rows * 128));
   return s < TF32_MAX_STAGES ? s : TF32_MAX_STAGES;
 }
 
@@ -184,8 +188,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(TF32_THREADS, 1)
 
   const uint32_t rank = cluster_ctarank();            // 0 = leader
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int stage_bytes = 2 * TF32_A_BYTES + half_max * 256;   // one layout for the launch: Q hi | Q lo | P hi | P lo
-  const int STAGES = tf32_stages_of(half_max);
+  const int nt = g.terms == 1 ? 1 : 2;                                // operand copies per stage
+  const int stage_bytes = nt * (TF32_A_BYTES + half_max * 128);      // one layout for the launch: Q hi | (Q lo) | P hi | (P lo)
+  const int STAGES = tf32_stages_of(half_max, nt);
   uint8_t* tiles = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   double* epi_red = reinterpret_cast<double*>(tiles + TF32_TILE_SMEM);   // [4][TF32_BN]
 
@@ -220,7 +225,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(TF32_THREADS, 1)
       const int p0 = prow + (int)rank * (sg.n0 >> 1);              // first slot row of this CTA's half of range 0
       const int p1 = prow + sg.n0 + (int)rank * (sg.n1 >> 1);      // ... of range 1
       const int half = (sg.n0 + sg.n1) >> 1;
-      const uint32_t seg_bytes = 2u * (uint32_t)(2 * TF32_A_BYTES + half * 256);   // both CTAs
+      const uint32_t seg_bytes = 2u * (uint32_t)(nt * (TF32_A_BYTES + half * 128));   // both CTAs
       const CUtensorMap* qh = &g.q_hi[sg.grp];
       const CUtensorMap* ql = &g.q_lo[sg.grp];
       for (int kt = sg.k0; kt < sg.k1; ++kt) {
@@ -235,13 +240,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(TF32_THREADS, 1)
           if (g.dbg && pair == 0 && rank == 0 && kt - sg.k0 < 2048) g.dbg[4096 + kt - sg.k0] = clock64();
           if (rank == 0) mbar_arrive_expect_tx(&full_bar[s], seg_bytes);
           tma_load_2d_pair(st, qh, xq, yq, lead_bar);
-          tma_load_2d_pair(st + TF32_A_BYTES, ql, xq, yq, lead_bar);
-          uint8_t* ph = st + 2 * TF32_A_BYTES;
+          if (nt == 2) tma_load_2d_pair(st + TF32_A_BYTES, ql, xq, yq, lead_bar);
+          uint8_t* ph = st + nt * TF32_A_BYTES;
           uint8_t* plo = ph + half_max * 128;
           for (int b = 0; b < half; b += TF32_PBOX) {
             const int row = (b < (sg.n0 >> 1) ? p0 + b : p1 + (b - (sg.n0 >> 1))) + yoff;
             tma_load_2d_pair(ph + b * 128, &g.p_hi, xp, row, lead_bar);
-            tma_load_2d_pair(plo + b * 128, &g.p_lo, xp, row, lead_bar);
+            if (nt == 2) tma_load_2d_pair(plo + b * 128, &g.p_lo, xp, row, lead_bar);
           }
         }
         __syncwarp();
@@ -272,8 +277,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(TF32_THREADS, 1)
           tc_fence_after();
           const uint8_t* st = tiles + (size_t)s * stage_bytes;
           const uint64_t a_hi = umma_smem_desc_sw128(st), a_lo = umma_smem_desc_sw128(st + TF32_A_BYTES);
-          const uint64_t b_hi = umma_smem_desc_sw128(st + 2 * TF32_A_BYTES);
-          const uint64_t b_lo = umma_smem_desc_sw128(st + 2 * TF32_A_BYTES + half_max * 128);
+          const uint64_t b_hi = umma_smem_desc_sw128(st + nt * TF32_A_BYTES);
+          const uint64_t b_lo = umma_smem_desc_sw128(st + nt * TF32_A_BYTES + half_max * 128);   // nt == 2 only
           const uint32_t acc0 = kt == sg.k0 ? 0u : 1u;
           if (elect_one()) {
             if (g.dbg && pair == 0 && kt - sg.k0 < 2048) g.dbg[kt - sg.k0] = clock64();
@@ -477,8 +482,7 @@ int gemm_tf32_launch(Tf32Args a, int G, Tf32Scratch& sc, const Epi& epi, cudaStr
   a.epoch = ++sc.epoch;
   const int64_t units = (int64_t)G * ceil_div(a.M, 2 * TF32_BM) * ceil_div(std::max(a.N, 1), TF32_BN) * ceil_div(a.K, TF32_BK);
   a.dbg = sc.dbg.p ? sc.dbg.as<unsigned long long>() : nullptr;
-  const char* tm = getenv("TKM_TF32_TERMS");
-  a.terms = tm && *tm == '1' ? 1 : 3;
+  if (a.terms != 1) a.terms = 3;
   const char* mr = getenv("TKM_SK_MINRANGE");
   a.min_range = mr && *mr ? std::max(1, atoi(mr)) : tf32_min_range((int)ceil_div(a.K, TF32_BK));
   const int pairs = (int)std::max<int64_t>(1, std::min<int64_t>(TF32_MAX_PAIRS, units / a.min_range));

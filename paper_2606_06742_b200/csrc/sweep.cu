@@ -828,6 +828,7 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
   const bool smoothed = loss == TKM_LOSS_HINGE || loss == TKM_LOSS_QUANTILE;   // logistic and DWD are smooth
   const int rounds = smoothed ? opts->rounds : 1;
   if (rounds < 1) return set_error(TKM_EINVAL, "tkm_fit_path: rounds must be >= 1");
+  if (opts->tf32_delta < 0 || opts->tf32_delta > 3) return set_error(TKM_EINVAL, "tkm_fit_path: tf32_delta must be 0..3");
   if (smoothed && (!(opts->smooth0 > 0.0) || !(opts->eta > 0.0 && opts->eta <= 1.0)))
     return set_error(TKM_EINVAL, "tkm_fit_path: need smooth0 > 0 and 0 < eta <= 1");
   TKM_TRY(device_check());
@@ -973,7 +974,7 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
   DevBuf zpart;
   if (ksplit_ok) TKM_TRY(zpart.alloc((size_t)KSPLIT_MAX * split_stride * sizeof(double), false, st, true));
   // F half (tf32_delta == 2): Fbar / F state, the (hi, lo) step operand, U Lam as (hi, lo), momentum per column
-  const bool delta_f = opts->tf32_delta == 2;
+  const bool delta_f = opts->tf32_delta >= 2;
   const int64_t ldr32 = round_up(r, 32);
   const bool kblk_f = delta_f && n >= KBLOCK_MIN_K;   // U Lam (hi, lo) K-blocked: [r/32][n][32]
   DevBuf Fb, Fp, da_hi, da_lo, mu, ul_hi[GEMM_MAX_GROUPS], ul_lo[GEMM_MAX_GROUPS];
@@ -1002,6 +1003,7 @@ extern "C" int tkm_fit_path_multi(const tkm_spectral* const* specs, int32_t G, c
   if (opts->tf32_delta != 0) TKM_TRY(tsc.alloc(st));
   memset(&targs, 0, sizeof(targs));
   memset(&targsF, 0, sizeof(targsF));
+  targs.terms = targsF.terms = opts->tf32_delta == 3 ? 1 : 3;   // mode 3: single-TF32 products (hi tiles only)
   int tcfg = -1;
   // [POLL_RING][GEMM_MAX_GROUPS] live-slot counts read back after every compaction; pinned once per host thread and
   // kept (cudaMallocHost is a kernel-mode call: none of those in a warm step, see DevBuf)

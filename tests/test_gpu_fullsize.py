@@ -64,7 +64,7 @@ def _first_order(w, tkm, path, K, y_np, foldid, cols, smooth_final):
     return worst, fs
 
 
-@pytest.mark.parametrize("cfg,delta", [(2, 0), (3, 0), (3, 2)])
+@pytest.mark.parametrize("cfg,delta", [(2, 0), (3, 0), (3, 2), (3, 3)])
 def test_full_kernel_configs_first_order_optimality(tkm, cfg, delta):
     import torch
     w = wl.CONFIGS[cfg]()

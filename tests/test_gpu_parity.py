@@ -287,7 +287,7 @@ def test_config1_full_size_bench_configuration(tkm):
                 assert np.abs(alpha[foldid == v]).max() < 1e-8 * sc
 
 
-@pytest.mark.parametrize("cfg,delta", [(2, 0), (2, 2), (3, 0), (3, 2)])
+@pytest.mark.parametrize("cfg,delta", [(2, 0), (2, 2), (3, 0), (3, 2), (3, 3)])
 def test_configs_2_3_reduced_n_against_an_oracle_fit(tkm, cfg, delta):
     """BASELINE.json configs[2] (logistic, 100 lambdas, 10 folds) and configs[3] (check loss, tau in {.1,.5,.9}
     stacked on one U, 50 lambdas, 5 folds): their generators, full lambda grids, folds and quantile levels at
@@ -332,7 +332,7 @@ def test_configs_2_3_reduced_n_against_an_oracle_fit(tkm, cfg, delta):
                 assert abs(cv_mean[t, l] - pooled / w.n) <= CV_TOL
 
 
-@pytest.mark.parametrize("delta", [0, 2])
+@pytest.mark.parametrize("delta", [0, 2, 3])
 def test_config4_parity_set_5000_row_subsample(tkm, delta):
     """BASELINE.json configs[4]: "fp64 oracle on a 5000-row subsample" -- a seeded 5000-row subsample of the
     n = 100000 data set with its own bandwidth (median heuristic on the subsample) and its own m = 1024 landmarks
@@ -650,12 +650,12 @@ def test_platt_on_held_out_decision_values(tkm):
 
 
 # ------------------------------------------------------------------------------- delta-form GEMM-B (tcgen05)
-@pytest.mark.parametrize("mode", [1, 2])
+@pytest.mark.parametrize("mode", [1, 2, 3])
 @pytest.mark.parametrize("name", ["cfg0", "kqr_ragged", "logit_ragged"])
 def test_delta_form_sweep_keeps_fp64_parity(tkm, name, mode):
     """tkm_loss_opts.tf32_delta: zeta = U^T z (mode 1) and also F = U Lam a (mode 2) advanced by 3xTF32 increments
     on the tcgen05 tensor cores, exact FP64 contractions and stop test on the last iteration of every batch
-    (DESIGN.md 12).  Same 1e-10 coefficient bar."""
+    (DESIGN.md 12); mode 3: the same with single-TF32 increment products.  Same 1e-10 coefficient bar."""
     w = {"cfg0": lambda: wl.config0(), "kqr_ragged": lambda: wl.config3(n=261, p=5, L=5, V=4, taus=(0.1, 0.5, 0.9)),
          "logit_ragged": lambda: wl.config2(n=333, p=9, L=7, V=3)}[name]()
     sigma = float(w.sigmas[0])
