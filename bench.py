@@ -515,7 +515,8 @@ def narrow_hbm_roofline(res, pk):
         ub = 4.0 if (i >= 2 and res.get("tf32_delta") == 3) else 8.0   # single-TF32 mode reads the hi parts only
         by = n * r * ub + live * (r + n) * ub + (live * (n if i == 2 else r) * 4.0 if i >= 2 else 0.0)
         ms = pr["ms"][i] / nl
-        out.append({"bound": "hbm", "kernel": FAMILY[i], "achieved": by / (ms / 1e3) / 1e9, "peak": pk["hbm"],
+        name = FAMILY[i].replace("3xTF32", "1xTF32") if res.get("tf32_delta") == 3 else FAMILY[i]
+        out.append({"bound": "hbm", "kernel": name, "achieved": by / (ms / 1e3) / 1e9, "peak": pk["hbm"],
                     "unit": "GB/s", "frac": by / (ms / 1e3) / 1e9 / pk["hbm"], "traffic": None,
                     "avg_live_columns": live, "avg_launch_ms": ms, "algorithmic_bytes_per_launch": by,
                     "sampled_launches": nl})
