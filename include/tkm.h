@@ -6,9 +6,12 @@
  * Conventions
  *   - extern "C"; every call returns a tkm_status (0 = TKM_OK).  tkm_last_error() returns a
  *     thread-local, NUL-terminated description of the last failure on the calling thread.
- *     No exception crosses the boundary.  Process-wide state: that string and the launch counter (thread-local),
- *     one library-owned stream-ordered memory pool per device for the sweep's temporaries (created on first
- *     use, never the device's default pool), and per-device "kernel attributes set" bits.
+ *     No exception crosses the boundary.  Process-wide state: that string, the launch counter and a small pinned
+ *     read-back buffer (all thread-local); per device, created on first use and kept until the process exits: one
+ *     library-owned stream-ordered memory pool that serves EVERY device allocation of the library (temporaries and
+ *     handle memory; up to 8 GiB of freed memory is retained; never the device's default pool), the worker threads,
+ *     streams and cuSOLVER handles of tkm_spectral_setup_multi, "kernel attributes set" bits, and the 512 KB static
+ *     device array of tkm_predict_noalloc.
  *   - [dev]  = pointer to DEVICE memory owned by the caller (e.g. a torch tensor's data_ptr()).
  *     [host] = pointer to HOST memory owned by the caller.  Nothing passed in is retained after
  *     the call returns except where stated (tkm_path keeps a pointer to its tkm_spectral).

@@ -550,6 +550,33 @@ def test_fit_path_multi_matches_oracle_per_group(tkm):
         tkm.tkm_fit_path_multi([specs[0], other], y, w.loss, w.lambdas, foldid, w.V, STOP_TOL, 100)
 
 
+@pytest.mark.parametrize("mode", [1, 2, 3])
+def test_fit_path_multi_agrees_with_single_calls_in_the_delta_forms(tkm, mode):
+    """Groups of one launch against separate tkm_fit_path calls with the delta forms on: tile choice and the
+    all-FP64 switch depend on totals over the groups, so the iterates differ -- the minimisers must not
+    (include/tkm.h: "same minimiser within tol")."""
+    w = wl.config0(n=260, p=5, L=8, V=3, seed=13)
+    sig = [0.6 * float(w.sigmas[0]), 1.5 * float(w.sigmas[0])]
+    foldid = tkm.tkm_make_folds(w.n, w.V, w.fold_seed)
+    X, y = dev(w.X), dev(w.y)
+    specs = [tkm.tkm_spectral_setup(tkm.tkm_gram(X, s)) for s in sig]
+    kw = dict(rounds=w.rounds, tf32_delta=mode, delta_min_live=16, profile=1)
+    multi = tkm.tkm_fit_path_multi(specs, y, w.loss, w.lambdas, foldid, w.V, STOP_TOL, 400000, **kw)
+    assert multi[0].profile()["launches"][3] > 0, "the delta form never engaged"
+    for spec, pm in zip(specs, multi):
+        ps = tkm.tkm_fit_path(spec, y, w.loss, w.lambdas, foldid, w.V, STOP_TOL, 400000, **kw)
+        assert pm.status == 0 and ps.status == 0
+        am, as_ = pm.a().cpu().numpy(), ps.a().cpu().numpy()
+        U = spec.U().cpu().numpy()
+        worst = 0.0
+        for c in range(pm.B):
+            fm, fs = U @ am[c], U @ as_[c]
+            worst = max(worst, np.linalg.norm(fm - fs) / max(np.linalg.norm(fs), 1e-300))
+        print("mode %d: multi vs single, worst relative l2 difference of alpha %.3g" % (mode, worst))
+        assert worst <= 2 * COEF_TOL_F64      # each side is within COEF_TOL_F64 of the minimiser
+        ps.close()
+
+
 def test_train_tune_host_matches_oracle(tkm):
     """The end-to-end call bench.py times as `e2e`: host buffers in, CV tables and coefficients out."""
     w = wl.config0(n=120, p=4, L=5, V=3, seed=5)
