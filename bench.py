@@ -852,6 +852,12 @@ def run_ours(args, w, rank, world):
                 {"tf32_delta": TF32_DELTA_LARGE, "stop_tol": 1e-10, "warm_start_rounds_tol": WARM_TOL,
                  "l2": "inputs larger than L2 (U Lam and U^T: 3.2 GB each)"}, probes,
                 tkeys={2: "config3_tcgen05_full_width", 3: "config3_tcgen05_full_width"})
+            if TF32_DELTA_LARGE == 2:
+                # the same pass with single-TF32 increment products (tf32_delta = 3): an option, reported beside
+                r3s = run_problem(tkm, w3, tf32_delta=3, tol=1e-10, warm_tol=WARM_TOL, profile=1, clocks_index=local)
+                line["large_config"]["single_tf32_increments"] = {
+                    "sweep_ms": r3s["sweep_ms"], "fits_per_s_sweep_only": r3s["B"] / (r3s["sweep_ms"] / 1e3),
+                    "col_iters": r3s["col_iters"], "selected_lambda_index": r3s["best_l"], "clocks": r3s["clocks"]}
         ncol, secs, its = oracle_sample_step(w)
         line["cpu_baseline"] = {"value": ncol / secs, "unit": UNIT, "cores": blas_threads(), "kind": "oracle",
                                 "sample": sample_text(w, ncol, secs, its)}
