@@ -814,3 +814,38 @@ def test_dmma_gemm_is_exact_on_freshly_mapped_operands(tkm):
         wrong = int((D[:, :M] != ref).sum())
         assert wrong == 0, "repetition %d: %d wrong elements" % (rep, wrong)
         del D, Q
+
+
+@pytest.mark.parametrize("mode", [0, 2, 3])
+def test_whole_step_is_bitwise_reproducible(tkm, mode):
+    """Two passes of the whole hot path on the same inputs -- Gram, concurrent decompositions, grouped sweep with
+    its device-side compaction and stream-K partial exchange, exact CV -- must give the SAME BITS: every reduction
+    has a fixed order and the schedule depends on device-side counts with a fixed lag, never on host timing."""
+    import torch
+    w = wl.config1(seed=1001)
+    w.sigmas = w.sigmas[1:4]
+    foldid = tkm.tkm_make_folds(w.n, w.V, w.fold_seed)
+    X, y = dev(w.X), dev(w.y)
+
+    def one_pass():
+        Ks = tkm.tkm_gram_multi(X, w.sigmas)
+        specs = tkm.tkm_spectral_setup_multi(Ks)
+        Us = [sp.U() for sp in specs]
+        paths = tkm.tkm_fit_path_multi(specs, y, w.loss, w.lambdas, foldid, w.V, 1e-11, 200000, smooth0=w.smooth0,
+                                       eta=w.eta, rounds=w.rounds, warm_tol=1e-3, tf32_delta=mode)
+        out = []
+        for K, U, path in zip(Ks, Us, paths):
+            info = path.info()
+            out.append((K, U, path.a(), info["beta0"], info["iters"], tkm.tkm_exact_cv(path, y, foldid, w.T, w.L, w.V)))
+            path.close()
+        for sp in specs:
+            sp.close()
+        return out
+
+    first, second = one_pass(), one_pass()
+    for g, (a, b) in enumerate(zip(first, second)):
+        assert torch.equal(a[0], b[0]), "Gram matrix of bandwidth %d differs between two passes" % g
+        assert torch.equal(a[1], b[1]), "eigenvectors of bandwidth %d differ" % g
+        assert torch.equal(a[2], b[2]), "coefficients of bandwidth %d differ" % g
+        assert np.array_equal(a[3], b[3]) and np.array_equal(a[4], b[4])
+        assert all(np.array_equal(p, q) for p, q in zip(a[5], b[5]))
