@@ -105,7 +105,12 @@ static const GemmTileInfo& tile_info(int cfg) {
 //   - narrow warp tiles need more fragment loads per MMA: per-configuration factor kEff.
 // The SM with the most tiles sets the time.  Mean regret against the best measured configuration over
 // the probe grid (G in {1,5}, N = 8..300, M = K = 2000): 4 %.
-static const double kEff[GEMM_NUM_CFG] = {1.0, 1.05, 1.0, 1.0, 1.02, 1.06, 1.1, 1.5, 1.0, 1.0};
+// (the factor of the 8-slot tile was re-fitted at the end of round 2 -- 1.5 -> 1.1 -- on a probe grid of G in {1,5},
+// N = 4..300 and six (M, K) shapes from 2000^2 to 4096 x 100000, every configuration timed per shape: with the slot
+// tiles fastest in the grid, LDS fragment loads and the late stage release, the 8 x 64 tile is the fastest stream up
+// to ~48 slots (its CTAs share a U tile through L2).  Mean regret of the choice over the grid 7.3 % -> 2.5 %;
+// worst at N = 12..40: 27-50 % -> <= 6 %.)
+static const double kEff[GEMM_NUM_CFG] = {1.0, 1.05, 1.0, 1.0, 1.02, 1.06, 1.1, 1.1, 1.0, 1.0};
 GemmTile gemm_f64_choose(const int* nb, int G, int M, int K) {
   const int forced = g_forced_cfg.load();
   if (forced >= 0) return gemm_f64_tile_of(forced);
