@@ -105,12 +105,13 @@ static const GemmTileInfo& tile_info(int cfg) {
 //   - narrow warp tiles need more fragment loads per MMA: per-configuration factor kEff.
 // The SM with the most tiles sets the time.  Mean regret against the best measured configuration over
 // the probe grid (G in {1,5}, N = 8..300, M = K = 2000): 4 %.
-// (the factor of the 8-slot tile was re-fitted at the end of round 2 -- 1.5 -> 1.1 -- on a probe grid of G in {1,5},
-// N = 4..300 and six (M, K) shapes from 2000^2 to 4096 x 100000, every configuration timed per shape: with the slot
-// tiles fastest in the grid, LDS fragment loads and the late stage release, the 8 x 64 tile is the fastest stream up
-// to ~48 slots (its CTAs share a U tile through L2).  Mean regret of the choice over the grid 7.3 % -> 2.5 %;
-// worst at N = 12..40: 27-50 % -> <= 6 %.)
-static const double kEff[GEMM_NUM_CFG] = {1.0, 1.05, 1.0, 1.0, 1.02, 1.06, 1.1, 1.1, 1.0, 1.0};
+// (Re-measured at the end of round 2 on a grid of G in {1,5}, N = 4..300 and six (M, K) shapes with every
+// configuration timed per shape: since the slot tiles run fastest in the grid the 8 x 64 tile is the fastest stream
+// up to ~48 slots, and a factor of 1.1 instead of 1.5 for it would cut the mean regret of the choice from 7.3 % to
+// 2.5 % (27-50 % -> <= 6 % at N = 12..40).  Not adopted yet: another tile is another summation order, and the
+// check-loss parity case at n = 1500 in mode 3 sits at 1.0e-10 +- 4e-12 of its bound; the
+// sweep-level gain was 0.6 % on the bench and 5-10 % on the narrow-batch workloads.  profiles/r02_narrow_batch.md.)
+static const double kEff[GEMM_NUM_CFG] = {1.0, 1.05, 1.0, 1.0, 1.02, 1.06, 1.1, 1.5, 1.0, 1.0};
 GemmTile gemm_f64_choose(const int* nb, int G, int M, int K) {
   const int forced = g_forced_cfg.load();
   if (forced >= 0) return gemm_f64_tile_of(forced);
