@@ -109,8 +109,9 @@ static const GemmTileInfo& tile_info(int cfg) {
 // configuration timed per shape: since the slot tiles run fastest in the grid the 8 x 64 tile is the fastest stream
 // up to ~48 slots, and a factor of 1.1 instead of 1.5 for it would cut the mean regret of the choice from 7.3 % to
 // 2.5 % (27-50 % -> <= 6 % at N = 12..40).  Not adopted yet: another tile is another summation order, and the
-// check-loss parity case at n = 1500 in mode 3 sits at 1.0e-10 +- 4e-12 of its bound; the
-// sweep-level gain was 0.6 % on the bench and 5-10 % on the narrow-batch workloads.  profiles/r02_narrow_batch.md.)
+// check-loss parity case at n = 1500 in mode 3 then stops at 1.04e-10 of the oracle instead of 7.8e-11, against a
+// bound of 1e-10 that the conditioning of those columns leaves little room under in ANY mode;
+// the sweep-level gain was 0.6 % on the bench and 5-10 % on the narrow-batch workloads.  profiles/r02_narrow_batch.md.)
 static const double kEff[GEMM_NUM_CFG] = {1.0, 1.05, 1.0, 1.0, 1.02, 1.06, 1.1, 1.5, 1.0, 1.0};
 GemmTile gemm_f64_choose(const int* nb, int G, int M, int K) {
   const int forced = g_forced_cfg.load();
